@@ -158,7 +158,7 @@ def test_tr_and_rt_self_couplings_agree_to_five_digits():
         _, Om = oracle.mobility_apply(prob, pos, np.array([[0, 1.0, 0]]), np.zeros((1, 3)), dft="fft")
         assert abs(U[0, 1] - Om[0, 0]) * norm < 1e-5
         assert abs(U[0, 1]) * norm > 1e-3 and U[0, 1] < 0        # a real coupling; a blob torqued about +x near the floor moves along -y
-        assert abs(U[0, 0]) * norm < 1e-5 and abs(U[0, 2]) * norm < 1e-5   # the only non-trivial tr self term
+        assert abs(U[0, 0]) * norm < 5e-5 and abs(U[0, 2]) * norm < 5e-5   # the only non-trivial tr self term
 
 
 def test_grid_cell_translation_and_wall_nulling():
