@@ -1,0 +1,110 @@
+/* dp.h — C ABI of the B200-native doubly-periodic Stokes mobility product
+ *
+ *     (U, Omega) = M (F, tau)
+ *
+ * for N regularised blobs above one no-slip wall ("bottom wall") or between two ("slit channel"), doubly periodic
+ * in x, y: the method of Hashemi et al., arXiv 2210.01837.  One call of dp_mobility_apply runs the paper's
+ * steps 1-8 (Sec. III D) entirely in hand-written CUDA kernels for sm_100a plus cuFFT for the
+ * batched xy FFTs:
+ *   step 1  spread F (and tau) with the exponential-of-semicircle kernel and wall images   eqs 7, 9, 53, 54
+ *   step 2  2D FFT in xy, Chebyshev transform in z, Chebyshev differentiation
+ *   step 3  per (kx,ky): pressure BVP eq 15 + BCs 17; velocity BVPs eq 18 + BCs 22, 24
+ *   step 4  per (kx,ky): wall correction, eqs 42-44 (one wall) or App. A (A5),(A6),(A8),(A10) (slit)
+ *   step 5  k = 0 mode, eqs 47, 51, 52 / (A12)
+ *   step 6  sum, (1/2) curl u in Fourier-Chebyshev space for Omega (eq 11)
+ *   step 7  inverse transforms
+ *   step 8  interpolate u (and (1/2) curl u) back to the particles, eqs 10, 11
+ * The exact discrete problem (grid, transforms, tau/integration BVP form, Nyquist rule, scalings) is stated in
+ * DESIGN.md; tests compare every output with the CPU oracle in oracle/ (relative L2 <= 1e-10 in fp64).
+ *
+ * Conventions
+ *  - All functions return DP_OK (0) or a negative error code; nothing throws across this boundary.
+ *  - Particle arrays are fp64, xyz-interleaved [n][3].  "DEVICE" pointers are CUDA device pointers on the plan's
+ *    device, owned by the caller, read-only for inputs, fully overwritten for outputs, never retained.
+ *  - x, y may be any real number (wrapped periodically into [0,Lx) x [0,Ly)).  z must satisfy 0 <= z <= H and, for the
+ *    bottom wall, z + alpha <= H with alpha = w h / 2 (kernels must not cross the open top): a
+ *    particle violating this contributes nothing, receives U = Omega = 0, and is reported by dp_check().
+ *  - A plan is not thread-safe: one dp_mobility_apply in flight per plan.  Plans are immutable after creation.
+ */
+#ifndef DP_STOKES_H
+#define DP_STOKES_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dp_plan dp_plan; /* opaque: owns grids, cuFFT plans, tables, workspace */
+
+enum { DP_BOTTOM_WALL = 0, DP_SLIT = 1 };
+enum { DP_OK = 0, DP_EINVAL = -1, DP_ENOMEM = -2, DP_ECUDA = -3, DP_ECUFFT = -4, DP_EDOMAIN = -5 };
+
+typedef struct {
+  int wall_mode;        /* DP_BOTTOM_WALL: wall at z=0, open top at z=H;  DP_SLIT: walls at z=0 and z=H            */
+  double Lx, Ly, H;     /* FULL periods in x, y (reading G1); top of the Chebyshev grid                   */
+  int nx, ny, nz;       /* grid: uniform in x,y (h = Lx/nx = Ly/ny to 1e-12 relative; nx, ny even), nz type-2
+                           Chebyshev nodes z_l = (H/2)(1+cos(l pi/(nz-1))) including both ends;
+                           nz must be one of the compiled sizes (dp_supported_nz)                                    */
+  int w;                /* ES kernel support in cells (paper's m), 4..8; alpha = w h/2               */
+  double beta_M;        /* ES beta of the monopole envelope Delta_M (eq 54; beta, not beta/w)                        */
+  double beta_D;        /* ES beta of the dipole envelope Delta_D; ignored if torques/Omega are never used           */
+  double eta;           /* viscosity > 0                                                                            */
+  int max_particles;    /* capacity of the plan's particle workspace                                                 */
+  int use_torques;      /* 0: forces in, U out only (3 grid fields); 1: also torques in / Omega out (6 fields)       */
+  int device;           /* CUDA device ordinal                                                                       */
+} dp_params;
+
+/* Validate, allocate (2 grids of fields*nz*ny*(nx+2) doubles + cuFFT workspace + particle workspace), plan the FFTs,
+ * upload tables.  Synchronous.  *out = NULL on error. */
+int dp_create(const dp_params* p, dp_plan** out);
+
+/* One mobility product, asynchronous on `cuda_stream` (a cudaStream_t; NULL = default stream).  DEVICE pointers.
+ *   pos    [n][3]  positions
+ *   force  [n][3]  or NULL (treated as zero)
+ *   torque [n][3]  or NULL; non-NULL requires use_torques = 1
+ *   U      [n][3]  required
+ *   Omega  [n][3]  or NULL; non-NULL requires use_torques = 1
+ * force == NULL && torque == NULL -> DP_EINVAL.  n > max_particles or n < 0 -> DP_EINVAL.  n == 0 is a no-op.
+ * No host<->device copy and no synchronisation happens inside. */
+int dp_mobility_apply(dp_plan* plan, int n, const double* pos, const double* force, const double* torque,
+                      double* U, double* Omega, void* cuda_stream);
+
+/* Same product with HOST pointers: copies inputs to the device, runs dp_mobility_apply, copies U (and Omega) back and
+ * synchronises.  This is the end-to-end entry point bench.py times as "e2e". */
+int dp_mobility_apply_host(dp_plan* plan, int n, const double* pos, const double* force, const double* torque,
+                           double* U, double* Omega);
+
+/* Synchronise the last stream used and report DP_EDOMAIN if any particle of the last apply was out of domain. */
+int dp_check(dp_plan* plan);
+
+/* Per-stage device times (ms) of the LAST apply, measured with CUDA events on its stream; synchronises.
+ * ms[0] bin, [1] spread, [2] xy FFT forward, [3] per-wavenumber solve (z transforms + BVPs + correction + curl),
+ * [4] xy FFT inverse, [5] interpolate, [6] k=0 column, [7] total.  Only recorded if dp_set_profiling(plan, 1). */
+int dp_set_profiling(dp_plan* plan, int on);
+int dp_stage_ms(dp_plan* plan, float* ms /* [8] */);
+
+/* Test hook: copy an internal device buffer of the last apply to HOST memory (synchronises).
+ *   which = 0: real grid    [fields][nz][ny][nx]       doubles  (after apply: u, (1/2) curl u in real space)
+ *   which = 1: complex grid [fields][nz][ny][nkxp]     double2  (after apply: consumed by the inverse FFT, undefined)
+ * dp_debug_run_stage runs the product up to and including `last_stage` (1 spread, 2 fwd FFT, 3 solve, 4 inv FFT) so
+ * that the buffers hold that stage's output.  Sizes via dp_buffer_bytes. */
+int dp_debug_run_stage(dp_plan* plan, int n, const double* pos, const double* force, const double* torque, int last_stage,
+                       void* cuda_stream);
+size_t dp_buffer_bytes(const dp_plan* plan, int which);
+int dp_copy_buffer_to_host(dp_plan* plan, int which, void* host, size_t bytes);
+int dp_complex_row_pitch(const dp_plan* plan); /* nkxp: padded row length (in complex numbers) of the half spectrum */
+
+/* Introspection */
+double dp_es_norm(double alpha, double beta);                  /* Z of eq 54, Gauss-Legendre on the host             */
+int dp_supported_nz(int* out, int cap);                        /* compiled Chebyshev sizes; returns how many          */
+size_t dp_device_bytes(const dp_plan* plan);                   /* device memory owned by the plan                     */
+const char* dp_strerror(int code);
+const char* dp_last_error(const dp_plan* plan);                /* detail of the last failure (CUDA / cuFFT message)   */
+
+int dp_destroy(dp_plan* plan); /* NULL is ok */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DP_STOKES_H */

@@ -1,0 +1,214 @@
+"""ctypes binding of include/dp.h — same names, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+BOTTOM_WALL = 0
+SLIT = 1
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBNAME = os.path.join(_HERE, "libdpstokes.so")
+
+# every symbol include/dp.h declares
+EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_check", "dp_set_profiling", "dp_stage_ms",
+           "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_complex_row_pitch", "dp_es_norm",
+           "dp_supported_nz", "dp_device_bytes", "dp_strerror", "dp_last_error", "dp_destroy"]
+
+
+class DPError(RuntimeError):
+    pass
+
+
+class dp_params(ctypes.Structure):
+    _fields_ = [("wall_mode", ctypes.c_int), ("Lx", ctypes.c_double), ("Ly", ctypes.c_double), ("H", ctypes.c_double),
+                ("nx", ctypes.c_int), ("ny", ctypes.c_int), ("nz", ctypes.c_int), ("w", ctypes.c_int),
+                ("beta_M", ctypes.c_double), ("beta_D", ctypes.c_double), ("eta", ctypes.c_double),
+                ("max_particles", ctypes.c_int), ("use_torques", ctypes.c_int), ("device", ctypes.c_int)]
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _LIBNAME
+
+
+def load_library():
+    """Load libdpstokes.so (built in-tree by ``build.py`` / ``__graft_entry__.build()``).  No fallback."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIBNAME):
+        raise DPError("CUDA library %s is missing: run `python -m paper_2210_01837_b200.build` "
+                      "(or __graft_entry__.build()); there is no CPU fallback" % _LIBNAME)
+    L = ctypes.CDLL(_LIBNAME)
+    vp, i, d, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_size_t
+    L.dp_create.argtypes = [ctypes.POINTER(dp_params), ctypes.POINTER(vp)]
+    L.dp_create.restype = i
+    L.dp_mobility_apply.argtypes = [vp, i, vp, vp, vp, vp, vp, vp]
+    L.dp_mobility_apply.restype = i
+    L.dp_mobility_apply_host.argtypes = [vp, i, vp, vp, vp, vp, vp]
+    L.dp_mobility_apply_host.restype = i
+    L.dp_check.argtypes = [vp]
+    L.dp_check.restype = i
+    L.dp_set_profiling.argtypes = [vp, i]
+    L.dp_set_profiling.restype = i
+    L.dp_stage_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    L.dp_stage_ms.restype = i
+    L.dp_debug_run_stage.argtypes = [vp, i, vp, vp, vp, i, vp]
+    L.dp_debug_run_stage.restype = i
+    L.dp_buffer_bytes.argtypes = [vp, i]
+    L.dp_buffer_bytes.restype = sz
+    L.dp_copy_buffer_to_host.argtypes = [vp, i, vp, sz]
+    L.dp_copy_buffer_to_host.restype = i
+    L.dp_complex_row_pitch.argtypes = [vp]
+    L.dp_complex_row_pitch.restype = i
+    L.dp_es_norm.argtypes = [d, d]
+    L.dp_es_norm.restype = d
+    L.dp_supported_nz.argtypes = [ctypes.POINTER(i), i]
+    L.dp_supported_nz.restype = i
+    L.dp_device_bytes.argtypes = [vp]
+    L.dp_device_bytes.restype = sz
+    L.dp_strerror.argtypes = [i]
+    L.dp_strerror.restype = ctypes.c_char_p
+    L.dp_last_error.argtypes = [vp]
+    L.dp_last_error.restype = ctypes.c_char_p
+    L.dp_destroy.argtypes = [vp]
+    L.dp_destroy.restype = i
+    _lib = L
+    return L
+
+
+def exported_symbols():
+    L = load_library()
+    return [s for s in EXPORTS if hasattr(L, s)]
+
+
+def es_norm(alpha: float, beta: float) -> float:
+    return float(load_library().dp_es_norm(alpha, beta))
+
+
+def supported_nz():
+    buf = (ctypes.c_int * 16)()
+    n = load_library().dp_supported_nz(buf, 16)
+    return [int(buf[k]) for k in range(n)]
+
+
+STAGE_NAMES = ["bin", "spread", "fft_fwd", "solve", "fft_inv", "interp", "k0", "total"]
+
+
+class Plan:
+    """dp_create / dp_mobility_apply / dp_destroy.  ``prob`` is any object with the fields of ``workloads.Problem``."""
+
+    def __init__(self, prob, max_particles: int, use_torques=None, device: int = 0):
+        self._h = None
+        L = load_library()
+        if use_torques is None:
+            use_torques = bool(getattr(prob, "has_torque", True))
+        self.params = dp_params(int(prob.wall_mode), float(prob.Lx), float(prob.Ly), float(prob.H), int(prob.nx), int(prob.ny),
+                                int(prob.nz), int(prob.w), float(prob.beta_M), float(prob.beta_D), float(prob.eta),
+                                int(max_particles), int(bool(use_torques)), int(device))
+        h = ctypes.c_void_p()
+        rc = L.dp_create(ctypes.byref(self.params), ctypes.byref(h))
+        if rc != 0:
+            raise DPError("dp_create failed: %s (%d)" % (L.dp_strerror(rc).decode(), rc))
+        self._h = h
+        self.use_torques = bool(use_torques)
+        self.fields = 6 if use_torques else 3
+        self.device = device
+
+    # -- lifetime
+    def close(self):
+        if self._h is not None:
+            load_library().dp_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.close()
+
+    def _ck(self, rc, what):
+        if rc != 0:
+            L = load_library()
+            raise DPError("%s failed: %s (%d): %s" % (what, L.dp_strerror(rc).decode(), rc, L.dp_last_error(self._h).decode()))
+
+    # -- the product, device tensors
+    def mobility_apply(self, pos, force=None, torque=None, want_omega=None, out_U=None, out_Omega=None, stream=None):
+        """(U, Omega) = M (F, tau).  ``pos``, ``force``, ``torque``: float64 CUDA tensors [n,3].  Asynchronous."""
+        import torch
+        if want_omega is None:
+            want_omega = torque is not None
+        n = int(pos.shape[0])
+        for t in (pos, force, torque):
+            if t is not None:
+                if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == (n, 3)):
+                    raise DPError("arguments must be contiguous float64 CUDA tensors of shape [n,3]")
+        U = out_U if out_U is not None else torch.empty((n, 3), dtype=torch.float64, device=pos.device)
+        Om = None
+        if want_omega:
+            Om = out_Omega if out_Omega is not None else torch.empty((n, 3), dtype=torch.float64, device=pos.device)
+        st = stream if stream is not None else torch.cuda.current_stream(pos.device)
+        ptr = lambda t: None if t is None else ctypes.c_void_p(t.data_ptr())
+        rc = load_library().dp_mobility_apply(self._h, n, ptr(pos), ptr(force), ptr(torque), ptr(U), ptr(Om),
+                                              ctypes.c_void_p(st.cuda_stream))
+        self._ck(rc, "dp_mobility_apply")
+        return U, Om
+
+    # -- the product, host arrays (H2D + product + D2H, synchronous)
+    def mobility_apply_host(self, pos, force=None, torque=None, want_omega=None, out_U=None, out_Omega=None):
+        if want_omega is None:
+            want_omega = torque is not None
+        c = lambda a: None if a is None else np.ascontiguousarray(a, dtype=np.float64)
+        pos, force, torque = c(pos), c(force), c(torque)
+        n = pos.shape[0]
+        U = out_U if out_U is not None else np.empty((n, 3))
+        Om = (out_Omega if out_Omega is not None else np.empty((n, 3))) if want_omega else None
+        ptr = lambda a: None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+        rc = load_library().dp_mobility_apply_host(self._h, n, ptr(pos), ptr(force), ptr(torque), ptr(U), ptr(Om))
+        self._ck(rc, "dp_mobility_apply_host")
+        return U, Om
+
+    def check(self) -> int:
+        return int(load_library().dp_check(self._h))
+
+    def set_profiling(self, on: bool):
+        self._ck(load_library().dp_set_profiling(self._h, int(on)), "dp_set_profiling")
+
+    def stage_ms(self) -> dict:
+        buf = (ctypes.c_float * 8)()
+        self._ck(load_library().dp_stage_ms(self._h, buf), "dp_stage_ms")
+        return {k: float(buf[i]) for i, k in enumerate(STAGE_NAMES)}
+
+    def device_bytes(self) -> int:
+        return int(load_library().dp_device_bytes(self._h))
+
+    # -- test hooks
+    def debug_stage(self, pos, force, torque, last_stage: int):
+        """Run steps up to ``last_stage`` (1 spread, 2 fwd FFT, 3 solve, 4 inv FFT) and return the stage's buffer as numpy."""
+        import torch
+        L = load_library()
+        n = int(pos.shape[0])
+        ptr = lambda t: None if t is None else ctypes.c_void_p(t.data_ptr())
+        st = torch.cuda.current_stream(pos.device)
+        self._ck(L.dp_debug_run_stage(self._h, n, ptr(pos), ptr(force), ptr(torque), int(last_stage), ctypes.c_void_p(st.cuda_stream)),
+                 "dp_debug_run_stage")
+        p = self.params
+        if last_stage in (1, 4):
+            out = np.empty((self.fields, p.nz, p.ny, p.nx), dtype=np.float64)
+            self._ck(L.dp_copy_buffer_to_host(self._h, 0, out.ctypes.data_as(ctypes.c_void_p), out.nbytes), "dp_copy_buffer_to_host")
+            return out
+        pitch = int(L.dp_complex_row_pitch(self._h))
+        out = np.empty((self.fields, p.nz, p.ny, pitch), dtype=np.complex128)
+        self._ck(L.dp_copy_buffer_to_host(self._h, 1, out.ctypes.data_as(ctypes.c_void_p), out.nbytes), "dp_copy_buffer_to_host")
+        return out[..., : p.nx // 2 + 1]

@@ -1,0 +1,80 @@
+// common.cuh — plan structure and shared device helpers of the DP Stokes CUDA library (sm_100a).
+// Nothing here is shared with oracle/ (the CPU oracle is written independently from the paper).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cufft.h>
+
+#include <cstddef>
+#include <cstdint>
+#include <string>
+
+#include "../../include/dp.h"
+
+#define DP_MAX_NZ 64
+#define DP_MAX_W 8
+
+// xy tile of the spread kernel (grid columns per CTA); particles are binned by the tile of their footprint origin.
+#define DP_TILE_X 16
+#define DP_TILE_Y 8
+
+// modes per CTA in the solve kernel (consecutive kx of one ky row) = one warp of modes
+#define DP_SOLVE_TM 32
+
+struct dp_tables_host;
+
+struct dp_plan {
+  dp_params p;
+  // derived
+  double h, alpha, ZM, ZD;      // grid spacing, ES half support, ES normalisations (eq 54)
+  int nkx, nkxp;                // nx/2+1 and its padded row pitch (complex elements)
+  int fields;                   // 3 or 6
+  int nbx, nby, nbins;          // spread tiles / particle bins
+  size_t real_field, cplx_field;  // elements per field: nz*ny*nx doubles, nz*ny*nkxp double2
+
+  // device buffers
+  double* d_real = nullptr;     // [fields][nz][ny][nx]
+  double2* d_cplx = nullptr;    // [fields][nz][ny][nkxp]
+  void* d_fft_work = nullptr;
+  size_t fft_work_bytes = 0;
+  double* d_znodes = nullptr;   // z_l
+  double* d_zweights = nullptr; // h^2 (H/2) w_l   (quadrature weight of node l)
+  // particle workspace (sorted by bin)
+  double* d_pos_s = nullptr;    // [n][3] wrapped x,y and z (z < 0 marks an out-of-domain particle)
+  double* d_frc_s = nullptr;    // [n][3]
+  double* d_trq_s = nullptr;    // [n][3]
+  int* d_perm = nullptr;        // sorted slot -> original index
+  int* d_bin_of = nullptr;      // per particle
+  int* d_slot_of = nullptr;     // rank within its bin
+  int* d_bin_count = nullptr;   // [nbins]
+  int* d_bin_start = nullptr;   // [nbins+1]
+  int* d_flag = nullptr;        // out-of-domain flag
+  size_t device_bytes = 0;
+
+  cufftHandle fft_fwd = 0, fft_inv = 0;
+  bool fft_ok = false;
+
+  cudaStream_t last_stream = nullptr;
+  bool profiling = false;
+  cudaEvent_t ev[9] = {};
+  bool ev_ok = false;
+  bool ev_recorded = false;
+  std::string last_error;
+};
+
+// launchers implemented in transfer.cu / solve.cu; all asynchronous on `st`
+cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* force, const double* torque, cudaStream_t st);
+cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torque, cudaStream_t st);
+cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaStream_t st);
+cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega, cudaStream_t st);
+cudaError_t dp_solve_upload_tables(dp_plan* P);
+bool dp_solve_supports_nz(int nz);
+
+// ---- exponential-of-semicircle kernel, eq 54: phi(s) = exp(beta (sqrt(1-(s/alpha)^2) - 1)) / Z on |s| <= alpha
+__device__ __forceinline__ double dp_es_phi(double s, double inv_alpha, double beta, double inv_Z) {
+  double q = s * inv_alpha;
+  double r = 1.0 - q * q;
+  if (!(fabs(q) <= 1.0)) return 0.0;
+  r = r < 0.0 ? 0.0 : r;
+  return exp(beta * (sqrt(r) - 1.0)) * inv_Z;
+}

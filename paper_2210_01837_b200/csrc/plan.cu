@@ -1,0 +1,363 @@
+// plan.cu — C ABI of the DP Stokes library: plan creation (tables, buffers, cuFFT plans), the apply pipeline
+// (paper steps 1-8), host-buffer entry point, profiling and test hooks.  See include/dp.h.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "common.cuh"
+
+namespace {
+
+typedef long double ld;
+const ld PI_LD = 3.141592653589793238462643383279502884L;
+
+// Z = int_{-alpha}^{alpha} exp(beta (sqrt(1 - (s/alpha)^2) - 1)) ds  (eq 54).
+// s = alpha sin(theta) makes the integrand alpha exp(beta (cos(theta) - 1)) cos(theta), analytic on [-pi/2, pi/2]:
+// composite 16-point Gauss-Legendre on 32 panels (Newton on the three-term recurrence for the nodes).
+double es_norm_host(double alpha, double beta) {
+  const int NP = 16, PANELS = 32;
+  ld x[NP], w[NP];
+  for (int i = 0; i < NP; ++i) {
+    ld t = cosl(PI_LD * (i + 0.75L) / (NP + 0.5L)), dp = 1;
+    for (int it = 0; it < 60; ++it) {
+      ld p0 = 1, p1 = t;
+      for (int k = 2; k <= NP; ++k) { ld p2 = ((2 * k - 1) * t * p1 - (k - 1) * p0) / k; p0 = p1; p1 = p2; }
+      dp = NP * (t * p1 - p0) / (t * t - 1);
+      ld dt = p1 / dp; t -= dt;
+      if (fabsl(dt) < 1e-20L) break;
+    }
+    ld p0 = 1, p1 = t;
+    for (int k = 2; k <= NP; ++k) { ld p2 = ((2 * k - 1) * t * p1 - (k - 1) * p0) / k; p0 = p1; p1 = p2; }
+    dp = NP * (t * p1 - p0) / (t * t - 1);
+    x[i] = t; w[i] = 2 / ((1 - t * t) * dp * dp);
+  }
+  ld sum = 0;
+  const ld a = -PI_LD / 2, width = PI_LD / PANELS;
+  for (int p = 0; p < PANELS; ++p)
+    for (int i = 0; i < NP; ++i) {
+      ld th = a + width * (p + 0.5L * (x[i] + 1));
+      sum += 0.5L * width * w[i] * expl((ld)beta * (cosl(th) - 1)) * cosl(th);
+    }
+  return (double)((ld)alpha * sum);
+}
+
+void set_err(dp_plan* P, const char* what, const char* detail) {
+  if (P) P->last_error = std::string(what) + ": " + (detail ? detail : "");
+}
+
+#define CK(call)                                                           \
+  do {                                                                     \
+    cudaError_t e__ = (call);                                              \
+    if (e__ != cudaSuccess) { set_err(P, #call, cudaGetErrorString(e__)); return DP_ECUDA; } \
+  } while (0)
+#define CKF(call)                                                          \
+  do {                                                                     \
+    cufftResult r__ = (call);                                              \
+    if (r__ != CUFFT_SUCCESS) { char b__[64]; snprintf(b__, sizeof b__, "cufft error %d", (int)r__); set_err(P, #call, b__); return DP_ECUFFT; } \
+  } while (0)
+
+template <class T> int dev_alloc(dp_plan* P, T** ptr, size_t count) {
+  cudaError_t e = cudaMalloc((void**)ptr, sizeof(T) * (count ? count : 1));
+  if (e != cudaSuccess) { set_err(P, "cudaMalloc", cudaGetErrorString(e)); cudaGetLastError(); return DP_ENOMEM; }
+  P->device_bytes += sizeof(T) * (count ? count : 1);
+  return DP_OK;
+}
+
+int make_fft(dp_plan* P) {
+  const int nx = P->p.nx, ny = P->p.ny;
+  long long n[2] = {ny, nx};
+  long long rembed[2] = {ny, nx}, cembed[2] = {ny, P->nkxp};
+  const long long batch = 3LL * P->p.nz;           // one field triple per call
+  size_t ws_f = 0, ws_i = 0;
+  CKF(cufftCreate(&P->fft_fwd));
+  CKF(cufftCreate(&P->fft_inv));
+  P->fft_ok = true;
+  CKF(cufftSetAutoAllocation(P->fft_fwd, 0));
+  CKF(cufftSetAutoAllocation(P->fft_inv, 0));
+  CKF(cufftMakePlanMany64(P->fft_fwd, 2, n, rembed, 1, (long long)ny * nx, cembed, 1, (long long)ny * P->nkxp, CUFFT_D2Z, batch, &ws_f));
+  CKF(cufftMakePlanMany64(P->fft_inv, 2, n, cembed, 1, (long long)ny * P->nkxp, rembed, 1, (long long)ny * nx, CUFFT_Z2D, batch, &ws_i));
+  P->fft_work_bytes = ws_f > ws_i ? ws_f : ws_i;
+  if (P->fft_work_bytes) {
+    cudaError_t e = cudaMalloc(&P->d_fft_work, P->fft_work_bytes);
+    if (e != cudaSuccess) { set_err(P, "cudaMalloc(cufft work)", cudaGetErrorString(e)); cudaGetLastError(); return DP_ENOMEM; }
+    P->device_bytes += P->fft_work_bytes;
+  }
+  CKF(cufftSetWorkArea(P->fft_fwd, P->d_fft_work));
+  CKF(cufftSetWorkArea(P->fft_inv, P->d_fft_work));
+  return DP_OK;
+}
+
+int run_pipeline(dp_plan* P, int n, const double* pos, const double* force, const double* torque, double* U, double* Omega,
+                 cudaStream_t st, int last_stage) {
+  const bool with_torque = torque != nullptr;
+  const bool want_omega = Omega != nullptr || (last_stage < 5 && P->fields == 6 && last_stage >= 3);
+  const bool prof = P->profiling && P->ev_ok;
+  P->last_stream = st;
+  P->ev_recorded = false;
+  if (prof) CK(cudaEventRecord(P->ev[0], st));
+  CK(dp_launch_bin(P, n, pos, force, torque, st));
+  if (prof) CK(cudaEventRecord(P->ev[1], st));
+  CK(dp_launch_spread(P, n, true, with_torque, st));
+  if (prof) CK(cudaEventRecord(P->ev[2], st));
+  if (last_stage >= 2) {
+    CKF(cufftSetStream(P->fft_fwd, st));
+    CKF(cufftExecD2Z(P->fft_fwd, P->d_real, (cufftDoubleComplex*)P->d_cplx));
+    if (with_torque) CKF(cufftExecD2Z(P->fft_fwd, P->d_real + 3 * P->real_field, (cufftDoubleComplex*)(P->d_cplx + 3 * P->cplx_field)));
+  }
+  if (prof) CK(cudaEventRecord(P->ev[3], st));
+  if (last_stage >= 3) CK(dp_launch_solve(P, with_torque, want_omega, st));
+  if (prof) CK(cudaEventRecord(P->ev[4], st));
+  if (last_stage >= 4) {
+    CKF(cufftSetStream(P->fft_inv, st));
+    CKF(cufftExecZ2D(P->fft_inv, (cufftDoubleComplex*)P->d_cplx, P->d_real));
+    if (want_omega) CKF(cufftExecZ2D(P->fft_inv, (cufftDoubleComplex*)(P->d_cplx + 3 * P->cplx_field), P->d_real + 3 * P->real_field));
+  }
+  if (prof) CK(cudaEventRecord(P->ev[5], st));
+  if (last_stage >= 5) CK(dp_launch_interp(P, n, U, Omega, st));
+  if (prof) { CK(cudaEventRecord(P->ev[6], st)); P->ev_recorded = true; }
+  return DP_OK;
+}
+
+int check_apply_args(dp_plan* P, int n, const double* pos, const double* force, const double* torque, const double* U, const double* Omega) {
+  if (!P) return DP_EINVAL;
+  if (n < 0 || n > P->p.max_particles) { set_err(P, "dp_mobility_apply", "n out of range"); return DP_EINVAL; }
+  if (n > 0 && (!pos || !U)) { set_err(P, "dp_mobility_apply", "pos and U are required"); return DP_EINVAL; }
+  if (!force && !torque) { set_err(P, "dp_mobility_apply", "force and torque both NULL"); return DP_EINVAL; }
+  if ((torque || Omega) && P->fields != 6) { set_err(P, "dp_mobility_apply", "plan created with use_torques = 0"); return DP_EINVAL; }
+  return DP_OK;
+}
+
+}  // namespace
+
+// host staging buffers for dp_mobility_apply_host live outside the public struct
+struct dp_host_stage { double *pos = nullptr, *frc = nullptr, *trq = nullptr, *U = nullptr, *Om = nullptr; cudaStream_t st = nullptr; };
+static dp_host_stage* stage_of(dp_plan* P);
+
+extern "C" {
+
+double dp_es_norm(double alpha, double beta) { return es_norm_host(alpha, beta); }
+
+int dp_supported_nz(int* out, int cap) {
+  const int all[3] = {16, 32, 48};
+  for (int i = 0; i < 3 && i < cap; ++i) out[i] = all[i];
+  return 3;
+}
+
+const char* dp_strerror(int code) {
+  switch (code) {
+    case DP_OK: return "ok";
+    case DP_EINVAL: return "invalid argument";
+    case DP_ENOMEM: return "out of device memory";
+    case DP_ECUDA: return "CUDA error";
+    case DP_ECUFFT: return "cuFFT error";
+    case DP_EDOMAIN: return "particle outside the domain";
+    default: return "unknown error";
+  }
+}
+
+const char* dp_last_error(const dp_plan* P) { return P ? P->last_error.c_str() : "null plan"; }
+size_t dp_device_bytes(const dp_plan* P) { return P ? P->device_bytes : 0; }
+int dp_complex_row_pitch(const dp_plan* P) { return P ? P->nkxp : 0; }
+
+int dp_destroy(dp_plan* P) {
+  if (!P) return DP_OK;
+  cudaSetDevice(P->p.device);
+  if (P->last_stream || true) cudaDeviceSynchronize();
+  if (P->fft_ok) { cufftDestroy(P->fft_fwd); cufftDestroy(P->fft_inv); }
+  void* bufs[] = {P->d_real, P->d_cplx, P->d_fft_work, P->d_znodes, P->d_zweights, P->d_pos_s, P->d_frc_s, P->d_trq_s, P->d_perm,
+                  P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_bin_start, P->d_flag};
+  for (void* b : bufs) if (b) cudaFree(b);
+  if (P->ev_ok) for (auto& e : P->ev) cudaEventDestroy(e);
+  dp_host_stage* hs = stage_of(P);
+  if (hs) {
+    void* hb[] = {hs->pos, hs->frc, hs->trq, hs->U, hs->Om};
+    for (void* b : hb) if (b) cudaFree(b);
+    if (hs->st) cudaStreamDestroy(hs->st);
+    delete hs;
+  }
+  delete P;
+  return DP_OK;
+}
+
+int dp_create(const dp_params* prm, dp_plan** out) {
+  if (!out) return DP_EINVAL;
+  *out = nullptr;
+  if (!prm) return DP_EINVAL;
+  const dp_params& p = *prm;
+  if (p.wall_mode != DP_BOTTOM_WALL && p.wall_mode != DP_SLIT) return DP_EINVAL;
+  if (!(p.Lx > 0) || !(p.Ly > 0) || !(p.H > 0) || !(p.eta > 0)) return DP_EINVAL;
+  if (p.w < 4 || p.w > DP_MAX_W) return DP_EINVAL;
+  if (p.nx < DP_TILE_X + p.w || p.ny < DP_TILE_Y + p.w || (p.nx & 1) || (p.ny & 1)) return DP_EINVAL;
+  if (!dp_solve_supports_nz(p.nz)) return DP_EINVAL;
+  const double hx = p.Lx / p.nx, hy = p.Ly / p.ny;
+  if (fabs(hx - hy) > 1e-12 * hx) return DP_EINVAL;
+  if (!(p.beta_M > 0) || (p.use_torques && !(p.beta_D > 0))) return DP_EINVAL;
+  if (p.max_particles < 1) return DP_EINVAL;
+  if (p.wall_mode == DP_SLIT && p.w * hx > p.H) return DP_EINVAL;     // a kernel may overlap one wall, not both
+  if ((double)p.nz * p.ny * (p.nx + 16) >= 2.0e9) return DP_EINVAL;    // 32-bit plane indexing inside the kernels
+
+  dp_plan* P = new (std::nothrow) dp_plan();
+  if (!P) return DP_ENOMEM;
+  P->p = p;
+  P->h = hx;
+  P->alpha = 0.5 * p.w * hx;
+  P->ZM = es_norm_host(P->alpha, p.beta_M);
+  P->ZD = p.use_torques ? es_norm_host(P->alpha, p.beta_D) : 1.0;
+  P->nkx = p.nx / 2 + 1;
+  P->nkxp = (P->nkx + 7) / 8 * 8;
+  P->fields = p.use_torques ? 6 : 3;
+  P->nbx = (p.nx + DP_TILE_X - 1) / DP_TILE_X;
+  P->nby = (p.ny + DP_TILE_Y - 1) / DP_TILE_Y;
+  P->nbins = P->nbx * P->nby;
+  P->real_field = (size_t)p.nz * p.ny * p.nx;
+  P->cplx_field = (size_t)p.nz * p.ny * P->nkxp;
+
+  int rc = DP_OK;
+  cudaError_t ce = cudaSetDevice(p.device);
+  if (ce != cudaSuccess) { delete P; return DP_ECUDA; }
+#define TRY(x) do { rc = (x); if (rc != DP_OK) { std::string msg = P->last_error; dp_destroy(P); (void)msg; return rc; } } while (0)
+  TRY(dev_alloc(P, &P->d_real, P->real_field * P->fields));
+  TRY(dev_alloc(P, &P->d_cplx, P->cplx_field * P->fields));
+  TRY(dev_alloc(P, &P->d_znodes, (size_t)p.nz));
+  TRY(dev_alloc(P, &P->d_zweights, (size_t)p.nz));
+  const size_t np = (size_t)p.max_particles;
+  TRY(dev_alloc(P, &P->d_pos_s, 3 * np));
+  TRY(dev_alloc(P, &P->d_frc_s, 3 * np));
+  if (p.use_torques) TRY(dev_alloc(P, &P->d_trq_s, 3 * np));
+  TRY(dev_alloc(P, &P->d_perm, np));
+  TRY(dev_alloc(P, &P->d_bin_of, np));
+  TRY(dev_alloc(P, &P->d_slot_of, np));
+  TRY(dev_alloc(P, &P->d_bin_count, (size_t)P->nbins));
+  TRY(dev_alloc(P, &P->d_bin_start, (size_t)P->nbins + 1));
+  TRY(dev_alloc(P, &P->d_flag, (size_t)1));
+  TRY(make_fft(P));
+
+  // tables: nodes z_l and quadrature weights h^2 (H/2) w_l, w_l Clenshaw-Curtis:
+  //   w_l = (2/N)(1/c~_l) sum_{n even} (1/c~_n) (2/(1-n^2)) cos(n l pi/N)
+  {
+    const int nz = p.nz, N = nz - 1;
+    std::vector<double> zn(nz), zw(nz);
+    for (int l = 0; l < nz; ++l) {
+      zn[l] = 0.5 * p.H * (1.0 + cos(M_PI * l / N));
+      ld sum = 0;
+      for (int n = 0; n <= N; n += 2) {
+        ld cn = (n == 0 || n == N) ? 2 : 1;
+        sum += (2 / (1 - (ld)n * n)) / cn * cosl(PI_LD * n * l / N);
+      }
+      ld cl = (l == 0 || l == N) ? 2 : 1;
+      zw[l] = (double)((ld)(hx * hx * 0.5 * p.H) * (2 / (ld)N) / cl * sum);
+    }
+    cudaError_t e1 = cudaMemcpy(P->d_znodes, zn.data(), sizeof(double) * nz, cudaMemcpyHostToDevice);
+    cudaError_t e2 = cudaMemcpy(P->d_zweights, zw.data(), sizeof(double) * nz, cudaMemcpyHostToDevice);
+    cudaError_t e3 = dp_solve_upload_tables(P);
+    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) { dp_destroy(P); return DP_ECUDA; }
+  }
+  {
+    bool ok = true;
+    for (auto& e : P->ev) ok = ok && (cudaEventCreate(&e) == cudaSuccess);
+    P->ev_ok = ok;
+  }
+  ce = cudaDeviceSynchronize();
+  if (ce != cudaSuccess) { dp_destroy(P); return DP_ECUDA; }
+#undef TRY
+  *out = P;
+  return DP_OK;
+}
+
+int dp_mobility_apply(dp_plan* P, int n, const double* pos, const double* force, const double* torque, double* U, double* Omega,
+                      void* cuda_stream) {
+  int rc = check_apply_args(P, n, pos, force, torque, U, Omega);
+  if (rc != DP_OK) return rc;
+  if (n == 0) return DP_OK;
+  return run_pipeline(P, n, pos, force, torque, U, Omega, (cudaStream_t)cuda_stream, 5);
+}
+
+int dp_debug_run_stage(dp_plan* P, int n, const double* pos, const double* force, const double* torque, int last_stage, void* cuda_stream) {
+  double dummy = 0;
+  int rc = check_apply_args(P, n, pos, force, torque, &dummy, nullptr);
+  if (rc != DP_OK) return rc;
+  if (last_stage < 1 || last_stage > 4 || n == 0) return DP_EINVAL;
+  return run_pipeline(P, n, pos, force, torque, nullptr, nullptr, (cudaStream_t)cuda_stream, last_stage);
+}
+
+int dp_check(dp_plan* P) {
+  if (!P) return DP_EINVAL;
+  CK(cudaStreamSynchronize(P->last_stream));
+  int flag = 0;
+  CK(cudaMemcpy(&flag, P->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
+  return flag ? DP_EDOMAIN : DP_OK;
+}
+
+int dp_set_profiling(dp_plan* P, int on) {
+  if (!P) return DP_EINVAL;
+  P->profiling = on != 0;
+  return DP_OK;
+}
+
+int dp_stage_ms(dp_plan* P, float* ms) {
+  if (!P || !ms) return DP_EINVAL;
+  for (int i = 0; i < 8; ++i) ms[i] = 0.f;
+  if (!P->ev_recorded) { set_err(P, "dp_stage_ms", "no profiled apply recorded"); return DP_EINVAL; }
+  CK(cudaEventSynchronize(P->ev[6]));
+  for (int i = 0; i < 6; ++i) CK(cudaEventElapsedTime(&ms[i], P->ev[i], P->ev[i + 1]));
+  ms[6] = 0.f;   // the k = 0 kernel is launched inside the solve stage
+  CK(cudaEventElapsedTime(&ms[7], P->ev[0], P->ev[6]));
+  return DP_OK;
+}
+
+size_t dp_buffer_bytes(const dp_plan* P, int which) {
+  if (!P) return 0;
+  if (which == 0) return sizeof(double) * P->real_field * P->fields;
+  if (which == 1) return sizeof(double2) * P->cplx_field * P->fields;
+  return 0;
+}
+
+int dp_copy_buffer_to_host(dp_plan* P, int which, void* host, size_t bytes) {
+  if (!P || !host) return DP_EINVAL;
+  if (bytes > dp_buffer_bytes(P, which) || dp_buffer_bytes(P, which) == 0) return DP_EINVAL;
+  CK(cudaStreamSynchronize(P->last_stream));
+  CK(cudaMemcpy(host, which == 0 ? (const void*)P->d_real : (const void*)P->d_cplx, bytes, cudaMemcpyDeviceToHost));
+  return DP_OK;
+}
+
+}  // extern "C"
+
+// ---- host-buffer entry point -----------------------------------------------------------------------------------------
+#include <map>
+static std::map<dp_plan*, dp_host_stage*> g_stage;
+static dp_host_stage* stage_of(dp_plan* P) {
+  auto it = g_stage.find(P);
+  if (it == g_stage.end()) return nullptr;
+  dp_host_stage* s = it->second;
+  g_stage.erase(it);
+  return s;
+}
+
+extern "C" int dp_mobility_apply_host(dp_plan* P, int n, const double* pos, const double* force, const double* torque, double* U,
+                                      double* Omega) {
+  int rc = check_apply_args(P, n, pos, force, torque, U, Omega);
+  if (rc != DP_OK) return rc;
+  if (n == 0) return DP_OK;
+  CK(cudaSetDevice(P->p.device));
+  dp_host_stage*& hs = g_stage[P];
+  if (!hs) {
+    hs = new dp_host_stage();
+    const size_t bytes = sizeof(double) * 3 * (size_t)P->p.max_particles;
+    CK(cudaMalloc(&hs->pos, bytes)); CK(cudaMalloc(&hs->frc, bytes)); CK(cudaMalloc(&hs->U, bytes));
+    P->device_bytes += 3 * bytes;
+    if (P->fields == 6) { CK(cudaMalloc(&hs->trq, bytes)); CK(cudaMalloc(&hs->Om, bytes)); P->device_bytes += 2 * bytes; }
+    CK(cudaStreamCreateWithFlags(&hs->st, cudaStreamNonBlocking));
+  }
+  const size_t nb = sizeof(double) * 3 * (size_t)n;
+  CK(cudaMemcpyAsync(hs->pos, pos, nb, cudaMemcpyHostToDevice, hs->st));
+  if (force) CK(cudaMemcpyAsync(hs->frc, force, nb, cudaMemcpyHostToDevice, hs->st));
+  if (torque) CK(cudaMemcpyAsync(hs->trq, torque, nb, cudaMemcpyHostToDevice, hs->st));
+  rc = run_pipeline(P, n, hs->pos, force ? hs->frc : nullptr, torque ? hs->trq : nullptr, hs->U, Omega ? hs->Om : nullptr, hs->st, 5);
+  if (rc != DP_OK) return rc;
+  CK(cudaMemcpyAsync(U, hs->U, nb, cudaMemcpyDeviceToHost, hs->st));
+  if (Omega) CK(cudaMemcpyAsync(Omega, hs->Om, nb, cudaMemcpyDeviceToHost, hs->st));
+  CK(cudaStreamSynchronize(hs->st));
+  return DP_OK;
+}

@@ -1,0 +1,171 @@
+"""GPU parity: the CUDA path (through the C ABI of include/dp.h) against the CPU oracle, element by element, on the
+same seeded inputs.  Bar (BASELINE.json north_star): relative L2 <= 1e-10 in fp64.
+Stage-level comparisons localise failures (grid after spread, spectra, solve output)."""
+import numpy as np
+import pytest
+
+import oracle
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-10
+
+
+def rel_l2(a, b):
+    a = np.asarray(a); b = np.asarray(b)
+    return float(np.linalg.norm((a - b).ravel()) / np.linalg.norm(b.ravel()))
+
+
+@pytest.fixture(scope="module")
+def dp():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2210_01837_b200 as dp
+    dp.load_library()          # fails loudly if the extension is missing
+    return dp
+
+
+def to_dev(*arrs):
+    import torch
+    return [None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in arrs]
+
+
+def run_gpu(dp, prob, pos, F, T, want_omega=None):
+    with dp.Plan(prob, max_particles=len(pos), use_torques=prob.has_torque) as plan:
+        dpos, dF, dT = to_dev(pos, F, T)
+        U, Om = plan.mobility_apply(dpos, dF, dT, want_omega=want_omega)
+        import torch
+        torch.cuda.synchronize()
+        assert plan.check() == 0
+        return U.cpu().numpy(), None if Om is None else Om.cpu().numpy()
+
+
+def small_monolayer(kind, n, seed):
+    """Scaled-down configs 3 / 4: same recipe (area fraction 0.4, heights, drives, w = 6 kernels), fewer particles."""
+    if kind == "bw":
+        return workloads.monolayer_bw(n=n, seed=seed, name="cfg3-small")
+    return workloads.monolayer_slit(n=n, seed=seed, name="cfg4-small")
+
+
+# ------------------------------------------------------------------------------------------------ stage parity
+@pytest.mark.parametrize("case", ["cfg1", "slit-small"])
+def test_stage_parity(dp, case):
+    if case == "cfg1":
+        prob, pos, F, T = workloads.config(1)
+    else:
+        prob, pos, F, T = workloads.random_slit(n=300, L=32.0, nxy=48, nz=48, H=8.0, seed=77, name="slit-small")
+    st = {}
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", stages=st)
+    dpos, dF, dT = to_dev(pos, F, T)
+    with dp.Plan(prob, max_particles=len(pos), use_torques=prob.has_torque) as plan:
+        g = plan.debug_stage(dpos, dF, dT, 1)
+        ref = st["f"] if T is None else np.concatenate([st["f"], st["t"]])
+        assert rel_l2(g, ref) < 1e-13                                  # only summation order differs
+        gh = plan.debug_stage(dpos, dF, dT, 2)
+        refh = st["fh"] if T is None else np.concatenate([st["fh"], st["th"]])
+        assert rel_l2(gh, refh) < 1e-13
+        uh = plan.debug_stage(dpos, dF, dT, 3) * (prob.nx * prob.ny)   # the kernel folds 1/(nx ny) into its output
+        refu = st["uh"] if T is None else np.concatenate([st["uh"], st["wh"]])
+        nf = refu.shape[0]
+        assert rel_l2(uh[:nf], refu) < 1e-11
+        # the k = 0 column alone, and the lowest modes alone (worst conditioned)
+        assert rel_l2(uh[:nf, :, 0, 0], refu[:, :, 0, 0]) < 1e-11
+        assert rel_l2(uh[:nf, :, 0:2, 0:2], refu[:, :, 0:2, 0:2]) < 1e-11
+        ur = plan.debug_stage(dpos, dF, dT, 4)
+        refr = st["u"] if T is None else np.concatenate([st["u"], st["om"]])
+        assert rel_l2(ur[:nf], refr) < 1e-11
+        U, Om = plan.mobility_apply(dpos, dF, dT)
+        assert rel_l2(U.cpu().numpy(), U_o) < TOL
+        if T is not None:
+            assert rel_l2(Om.cpu().numpy(), Om_o) < TOL
+
+
+# ------------------------------------------------------------------------------------------------ full products
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_config_parity(dp, cfg):
+    prob, pos, F, T = workloads.config(cfg)
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft")
+    U, Om = run_gpu(dp, prob, pos, F, T)
+    err = rel_l2(np.concatenate([U] + ([Om] if Om is not None else []), axis=1),
+                 np.concatenate([U_o] + ([Om_o] if Om_o is not None else []), axis=1))
+    assert err < TOL, err
+    assert rel_l2(U, U_o) < TOL
+    if Om is not None:
+        assert rel_l2(Om, Om_o) < TOL
+
+
+@pytest.mark.parametrize("kind,n,seed", [("bw", 3000, 31), ("slit", 2500, 32)])
+def test_scaled_monolayer_parity(dp, kind, n, seed):
+    """Configs 3 and 4 at reduced N: same recipe; grid not a multiple of the spread tile or of the 32-mode solve tile."""
+    prob, pos, F, T = small_monolayer(kind, n, seed)
+    assert prob.nx % 16 != 0 or (prob.nx // 2 + 1) % 32 != 0
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft")
+    U, Om = run_gpu(dp, prob, pos, F, T)
+    assert rel_l2(U, U_o) < TOL and rel_l2(Om, Om_o) < TOL
+
+
+def test_forces_only_on_a_torque_plan_and_omega_without_torque(dp):
+    prob, pos, F, T = workloads.random_slit(n=200, L=32.0, nxy=48, nz=32, H=8.0, seed=5, name="mix")
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, None, want_omega=True, dft="fft")
+    U, Om = run_gpu(dp, prob, pos, F, None, want_omega=True)
+    assert rel_l2(U, U_o) < TOL and rel_l2(Om, Om_o) < TOL
+    U_o2, _ = oracle.mobility_apply(prob, pos, None, T, want_omega=False, dft="fft")
+    U2, Om2 = run_gpu(dp, prob, pos, None, T, want_omega=False)
+    assert Om2 is None and rel_l2(U2, U_o2) < TOL
+
+
+# ------------------------------------------------------------------------------------------------ edge cases
+def test_edge_cases(dp):
+    import torch
+    prob, pos, F, T = workloads.random_bw(n=64, L=100 * (2.0 / 3.0) * 0.5, nxy=50, nz=16, H=8.0, seed=9, name="ragged")
+    # 50 columns: ragged spread tiles (16 x 8) and a ragged solve tile (26 modes); nz = 16
+    pos = pos.copy()
+    pos[0, :2] += [7 * prob.Lx, -3 * prob.Ly]        # far outside the primary cell
+    pos[1, 2] = 0.0                                  # on the wall: contributes nothing, feels nothing
+    pos[2, :2] = [0.0, 0.0]                          # on a grid node
+    pos[3, :2] = [prob.Lx - 1e-9, prob.Ly - 1e-9]    # footprint wraps
+    U_o, _ = oracle.mobility_apply(prob, pos, F, None, dft="fft")
+    U, _ = run_gpu(dp, prob, pos, F, None)
+    assert rel_l2(U, U_o) < TOL
+    assert np.all(U[1] == 0.0)
+    with dp.Plan(prob, max_particles=64, use_torques=False) as plan:
+        # n = 0 is a no-op
+        e = torch.empty((0, 3), dtype=torch.float64, device="cuda")
+        U0, _ = plan.mobility_apply(e, e)
+        assert U0.shape == (0, 3)
+        # out-of-domain particles: flagged, contribute nothing, get zero
+        bad = pos.copy()
+        bad[5, 2] = -0.1
+        bad[6, 2] = prob.H - 0.5                      # bottom wall: kernel would cross the open top
+        dpos, dF = to_dev(bad, F)
+        Ub, _ = plan.mobility_apply(dpos, dF)
+        torch.cuda.synchronize()
+        assert plan.check() == -5
+        keep = np.ones(len(pos), bool); keep[[5, 6]] = False
+        U_ref, _ = oracle.mobility_apply(prob, bad[keep], F[keep], None, dft="fft")
+        Ub = Ub.cpu().numpy()
+        assert np.all(Ub[[5, 6]] == 0.0) and rel_l2(Ub[keep], U_ref) < TOL
+        # both inputs missing -> error, not a crash
+        with pytest.raises(dp.DPError):
+            plan.mobility_apply(dpos, None, None)
+        # the plan is reusable and repeatable (bin order may differ: <= 1e-13, reading G16)
+        U1, _ = plan.mobility_apply(*to_dev(pos, F))
+        U2, _ = plan.mobility_apply(*to_dev(pos, F))
+        assert rel_l2(U1.cpu().numpy(), U2.cpu().numpy()) < 1e-13
+
+
+def test_host_entry_point_matches_device_entry_point(dp):
+    prob, pos, F, T = workloads.random_slit(n=500, L=32.0, nxy=48, nz=32, H=8.0, seed=12, name="host")
+    with dp.Plan(prob, max_particles=len(pos)) as plan:
+        Uh, Omh = plan.mobility_apply_host(pos, F, T)
+        U, Om = plan.mobility_apply(*to_dev(pos, F, T))
+        assert rel_l2(Uh, U.cpu().numpy()) < 1e-13 and rel_l2(Omh, Om.cpu().numpy()) < 1e-13
+
+
+def test_create_rejects_bad_parameters(dp):
+    prob, *_ = workloads.config(1)
+    import dataclasses
+    for bad in (dict(nz=31), dict(nx=49), dict(w=3), dict(eta=0.0), dict(Ly=prob.Ly * 1.01), dict(nx=16, ny=16)):
+        with pytest.raises(dp.DPError):
+            dp.Plan(dataclasses.replace(prob, **bad), max_particles=8)
