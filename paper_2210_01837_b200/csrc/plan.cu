@@ -123,6 +123,7 @@ int run_pipeline(dp_plan* P, int n, const double* pos, const double* force, cons
 int check_apply_args(dp_plan* P, int n, const double* pos, const double* force, const double* torque, const double* U, const double* Omega) {
   if (!P) return DP_EINVAL;
   if (n < 0 || n > P->p.max_particles) { set_err(P, "dp_mobility_apply", "n out of range"); return DP_EINVAL; }
+  if (n == 0) return DP_OK;                      // nothing to do; pointers of empty arrays may legitimately be NULL
   if (n > 0 && (!pos || !U)) { set_err(P, "dp_mobility_apply", "pos and U are required"); return DP_EINVAL; }
   if (!force && !torque) { set_err(P, "dp_mobility_apply", "force and torque both NULL"); return DP_EINVAL; }
   if ((torque || Omega) && P->fields != 6) { set_err(P, "dp_mobility_apply", "plan created with use_torques = 0"); return DP_EINVAL; }
