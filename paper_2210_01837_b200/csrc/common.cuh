@@ -16,7 +16,7 @@
 
 // xy tile of the spread kernel (grid columns per CTA); particles are binned by the tile of their footprint origin.
 #define DP_TILE_X 16
-#define DP_TILE_Y 8
+#define DP_TILE_Y 4
 
 // modes per CTA in the solve kernel (consecutive kx of one ky row) = one warp of modes
 #define DP_SOLVE_TM 32
@@ -44,6 +44,7 @@ struct dp_plan {
   double* d_frc_s = nullptr;    // [n][3]
   double* d_trq_s = nullptr;    // [n][3]
   int* d_perm = nullptr;        // sorted slot -> original index
+  int4* d_meta = nullptr;       // sorted footprint records: wrapped origin node (i0, j0), plane range [lmin, lmax]
   int* d_bin_of = nullptr;      // per particle
   int* d_slot_of = nullptr;     // rank within its bin
   int* d_bin_count = nullptr;   // [nbins]

@@ -4,19 +4,21 @@
 //   Delta^W = phi(x)phi(y)[phi(z - z_j) - phi(z + z_j) - (slit) phi(z - (2H - z_j))]
 // Step 8 (eqs 10, 11): U_j = sum_g u(x_g) Delta_M^W(x_g - r_j) h^2 (H/2) w_l, Omega_j likewise with Delta_D^W.
 //
-// B200 design: particles are counting-sorted by the xy tile (16 x 8 grid columns) that contains the origin of
-// their w x w footprint.  One CTA owns one tile of one field triple: it accumulates every footprint that touches
-// the tile into a shared-memory tile [3][nz][8][16] (each thread owns one column and a fixed residue class of the plane index, so no
-// atomics and no conflicts), then streams the whole tile to HBM once with 16-byte coalesced stores — every grid
-// value is written exactly once, zeros included, so there is no memset pass and no global atomic.
+// B200 design: particles are counting-sorted by the xy tile (16 x 4 grid columns) that contains the origin of
+// their w x w footprint.  One CTA owns one tile of one field triple and gathers every footprint that touches it into
+// per-thread register accumulators (each thread owns one column and a fixed residue class of the plane index, so no
+// atomics and no conflicts), then stores the tile to HBM once in 128-byte row segments — every grid value is written
+// exactly once, zeros included, so there is no memset pass and no global atomic.
 #include "common.cuh"
 
 namespace {
 
 constexpr int TX = DP_TILE_X, TY = DP_TILE_Y;
-constexpr int ZSPLIT = 2;                       // z residue classes per column
+constexpr int ZSPLIT = 4;                       // z residue classes per column
 constexpr int SPREAD_THREADS = TX * TY * ZSPLIT;
-constexpr int PCH = 16;                         // particles staged per chunk
+constexpr int PCH = 32;                         // particles staged per chunk
+constexpr int MAXB = 6;                         // origin bins per direction that can reach a tile (w <= 8, TY = 4)
+constexpr int MAXR = 2 * MAXB;                  // candidate ranges per tile: one per bin row, two when the x range wraps
 
 struct GridGeom {
   int nx, ny, nz, w, wall_mode, nbx, nby;
@@ -35,13 +37,36 @@ __device__ __forceinline__ int origin_cell(double xw, double alpha, double h, in
 __device__ __forceinline__ int origin_bins(int X0, int Teff, int T, int w, int n, int* out) {
   int o = X0 - (w - 1); o %= n; if (o < 0) o += n;
   int left = Teff + w - 1, cnt = 0;
-  while (left > 0 && cnt < 4) {
+  while (left > 0 && cnt < MAXB) {
     int b = o / T, bend = min((b + 1) * T, n);
     out[cnt++] = b;
     left -= bend - o;
     o = bend == n ? 0 : bend;
   }
   return cnt;
+}
+
+// ---------------------------------------------------------------------------------------------- z weights
+// zeta(l; z_p) = phi(z_l - z_p) - phi(z_l + z_p) - [slit] phi(z_l - (2H - z_p))   (eq 9, PAPER.md:95, 620)
+// phi(s) of eq 54 with 1/alpha and 1/Z precomputed (support test |s| <= alpha inclusive, reading G6)
+__device__ __forceinline__ double es_phi(double s, double inv_alpha, double beta, double inv_Z) {
+  const double q = s * inv_alpha;
+  if (!(fabs(q) <= 1.0)) return 0.0;
+  double r = 1.0 - q * q; r = r < 0.0 ? 0.0 : r;
+  return exp(beta * (sqrt(r) - 1.0)) * inv_Z;
+}
+__device__ __forceinline__ double zeta_weight(double zl, double zp, double H, int wall_mode, double inv_alpha, double beta, double inv_Z) {
+  double v = es_phi(zl - zp, inv_alpha, beta, inv_Z) - es_phi(zl + zp, inv_alpha, beta, inv_Z);
+  if (wall_mode == DP_SLIT) v -= es_phi(zl - (2.0 * H - zp), inv_alpha, beta, inv_Z);
+  return v;
+}
+// node range with z_l in [max(0, zp - alpha), min(H, zp + alpha)] (nodes decrease with l); covers every image term
+__device__ __forceinline__ void z_range(const double* zn, int nz, double zp, double alpha, double H, int& lmin, int& lmax) {
+  double hi = zp + alpha, lo = zp - alpha;
+  int a = 0, b = nz - 1;
+  while (a < nz && zn[a] > hi) ++a;
+  while (b >= 0 && zn[b] < lo) --b;
+  lmin = a; lmax = b;
 }
 
 // ---------------------------------------------------------------------------------------------- binning
@@ -94,8 +119,9 @@ __global__ void k_scan(int nbins, const int* __restrict__ cnt, int* __restrict__
 
 __global__ void k_bin_scatter(int n, const double* __restrict__ pos, const double* __restrict__ force,
                               const double* __restrict__ torque, GridGeom g, const int* __restrict__ bin_of,
-                              const int* __restrict__ slot_of, const int* __restrict__ bin_start, int* __restrict__ perm,
-                              double* __restrict__ pos_s, double* __restrict__ frc_s, double* __restrict__ trq_s) {
+                              const int* __restrict__ slot_of, const int* __restrict__ bin_start, const double* __restrict__ znodes,
+                              int* __restrict__ perm, int4* __restrict__ meta, double* __restrict__ pos_s, double* __restrict__ frc_s,
+                              double* __restrict__ trq_s) {
   int p = blockIdx.x * blockDim.x + threadIdx.x;
   if (p >= n) return;
   int d = bin_start[bin_of[p]] + slot_of[p];
@@ -105,34 +131,17 @@ __global__ void k_bin_scatter(int n, const double* __restrict__ pos, const doubl
   double xw = 0.0, yw = 0.0;
   if (ok) { xw = x - floor(x / g.Lx) * g.Lx; yw = y - floor(y / g.Ly) * g.Ly; }
   pos_s[3 * (size_t)d] = xw; pos_s[3 * (size_t)d + 1] = yw; pos_s[3 * (size_t)d + 2] = ok ? z : -1.0;   // z < 0: skipped
+  // footprint record: wrapped origin node (i0, j0) and plane range [lmin, lmax]; lmin > lmax marks a skipped particle
+  int4 m = make_int4(0, 0, 1, 0);
+  if (ok) {
+    m.x = origin_cell(xw, g.alpha, g.h, g.nx); m.y = origin_cell(yw, g.alpha, g.h, g.ny);
+    z_range(znodes, g.nz, z, g.alpha, g.H, m.z, m.w);
+  }
+  meta[d] = m;
   for (int c = 0; c < 3; ++c) {
     if (frc_s) frc_s[3 * (size_t)d + c] = force ? force[3 * (size_t)p + c] : 0.0;
     if (trq_s) trq_s[3 * (size_t)d + c] = torque ? torque[3 * (size_t)p + c] : 0.0;
   }
-}
-
-// ---------------------------------------------------------------------------------------------- z weights
-// zeta(l; z_p) = phi(z_l - z_p) - phi(z_l + z_p) - [slit] phi(z_l - (2H - z_p))   (eq 9, PAPER.md:95, 620)
-__device__ __forceinline__ double zeta_weight(double zl, double zp, double H, int wall_mode, double alpha, double beta, double Z) {
-  double q, r, v = 0.0;
-  q = (zl - zp) / alpha; if (fabs(q) <= 1.0) { r = 1.0 - q * q; r = r < 0.0 ? 0.0 : r; v += exp(beta * (sqrt(r) - 1.0)) / Z; }
-  q = (zl + zp) / alpha; if (fabs(q) <= 1.0) { r = 1.0 - q * q; r = r < 0.0 ? 0.0 : r; v -= exp(beta * (sqrt(r) - 1.0)) / Z; }
-  if (wall_mode == DP_SLIT) { q = (zl - (2.0 * H - zp)) / alpha; if (fabs(q) <= 1.0) { r = 1.0 - q * q; r = r < 0.0 ? 0.0 : r; v -= exp(beta * (sqrt(r) - 1.0)) / Z; } }
-  return v;
-}
-__device__ __forceinline__ double xy_weight(double s, double alpha, double beta, double Z) {
-  double q = s / alpha;
-  if (!(fabs(q) <= 1.0)) return 0.0;
-  double r = 1.0 - q * q; r = r < 0.0 ? 0.0 : r;
-  return exp(beta * (sqrt(r) - 1.0)) / Z;
-}
-// node range with z_l in [max(0, zp - alpha), min(H, zp + alpha)] (nodes decrease with l); covers every image term
-__device__ __forceinline__ void z_range(const double* zn, int nz, double zp, double alpha, double H, int& lmin, int& lmax) {
-  double hi = zp + alpha, lo = zp - alpha;
-  int a = 0, b = nz - 1;
-  while (a < nz && zn[a] > hi) ++a;
-  while (b >= 0 && zn[b] < lo) --b;
-  lmin = a; lmax = b;
 }
 
 // ---------------------------------------------------------------------------------------------- spread
@@ -144,112 +153,166 @@ struct SpreadArgs {
   int field0[2];             // first output field of each group
   int ngroups;
   const int* bin_start;
+  const int4* meta;          // sorted footprint records (i0, j0, lmin, lmax)
   const double* znodes;
   double* grid;
   size_t real_field;
 };
 
-__global__ void __launch_bounds__(SPREAD_THREADS) k_spread(SpreadArgs A) {
-  extern __shared__ double smem[];
-  const GridGeom& g = A.g;
-  const int nz = g.nz, w = g.w;
-  double* acc = smem;                                   // [3][nz][TY][TX]
-  double* s_zn = acc + 3 * nz * TY * TX;                // [nz]
-  double* s_wx = s_zn + nz;                             // [PCH][DP_MAX_W]
-  double* s_wy = s_wx + PCH * DP_MAX_W;                 // [PCH][DP_MAX_W]
-  double* s_zt = s_wy + PCH * DP_MAX_W;                 // [PCH][nz]
-  double* s_val = s_zt + PCH * nz;                      // [PCH][3]
-  int* s_meta = (int*)(s_val + PCH * 3);                // [PCH][4]: i0, j0, lmin, lmax
+// One CTA = one tile of TX x TY grid columns of one field triple.  Thread (ti, tj, tz) owns column (ti, tj) and the
+// planes l = ZSPLIT*li + tz; its 3*NZ/ZSPLIT partial sums live in registers for the whole kernel, so there is no
+// shared-memory tile, no atomic and no memset.  Global-memory round trips per CTA: bin_start -> candidate records
+// (footprint, position, value: one batch of independent loads per warp) -> stores.  The candidates (the bins whose
+// footprints can reach the tile, merged into contiguous ranges of the sorted arrays) are culled by warp ballot, the 1-D
+// ES weights of the survivors are evaluated once per CTA into shared memory, every thread adds the particles covering
+// its column, and each value is stored to HBM exactly once (128-byte row segments per warp).
+template <int NZ>
+__global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(SpreadArgs A) {
+  constexpr int NL = NZ / ZSPLIT;
+  constexpr int NW = SPREAD_THREADS / 32;
+  __shared__ double s_zn[NZ];
+  __shared__ double s_wx[PCH][DP_MAX_W], s_wy[PCH][DP_MAX_W], s_zt[PCH][NZ], s_val[PCH][3], s_pos[PCH][3];
+  __shared__ int4 s_meta[PCH];                // i0, j0 (wrapped origin node), lmin, lmax
+  __shared__ int s_rbeg[MAXR], s_rend[MAXR], s_rcnt[MAXR];  // candidate ranges in the sorted arrays, hits per range
 
+  const GridGeom& g = A.g;
+  const int w = g.w;
   const int grp = blockIdx.y;
   const int bx = blockIdx.x % g.nbx, by = blockIdx.x / g.nbx;
   const int X0 = bx * TX, Y0 = by * TY;
-  const int t = threadIdx.x;
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
   const int ti = t % TX, tj = (t / TX) % TY, tz = t / (TX * TY);
   const int gi = X0 + ti, gj = Y0 + tj;
-  const double beta = A.beta[grp], Z = A.Z[grp];
+  const bool in_grid = gi < g.nx && gj < g.ny;
+  const double beta = A.beta[grp], inv_Z = 1.0 / A.Z[grp], inv_alpha = 1.0 / g.alpha;
   const double* __restrict__ val = A.val_s[grp];
 
-  for (int i = t; i < 3 * nz * TY * TX; i += SPREAD_THREADS) acc[i] = 0.0;
-  for (int i = t; i < nz; i += SPREAD_THREADS) s_zn[i] = A.znodes[i];
+  double acc[NL][3];
+#pragma unroll
+  for (int li = 0; li < NL; ++li) { acc[li][0] = 0.0; acc[li][1] = 0.0; acc[li][2] = 0.0; }
 
-  // origin bins whose footprints can reach this tile: origin columns in the cyclic range [X0-w+1, X0+TXeff-1]
-  int bxs[4], bys[4];
-  const int ncx = origin_bins(X0, min(TX, g.nx - X0), TX, w, g.nx, bxs);
-  const int ncy = origin_bins(Y0, min(TY, g.ny - Y0), TY, w, g.ny, bys);
+  for (int i = t; i < NZ; i += SPREAD_THREADS) s_zn[i] = A.znodes[i];
+  // bins whose footprints can reach this tile: origin columns in the cyclic range [X0-w+1, X0+TXeff-1] (same in y);
+  // the x-bins of one bin row are consecutive in memory, so each row gives one range (two when the range wraps in x)
+  int nr;
+  {
+    int o = X0 - (w - 1); o %= g.nx; if (o < 0) o += g.nx;
+    const int len = min(TX, g.nx - X0) + w - 1;                 // <= nx (checked at create)
+    const int b0 = o / TX, b1 = (o + len - 1 < g.nx) ? (o + len - 1) / TX : g.nbx - 1;
+    const int wrap_b1 = (o + len - 1 < g.nx) ? -1 : (o + len - 1 - g.nx) / TX;     // second piece: bins 0 .. wrap_b1
+    int bys[MAXB];
+    const int ncy = origin_bins(Y0, min(TY, g.ny - Y0), TY, w, g.ny, bys);
+    const int per_row = wrap_b1 >= 0 ? 2 : 1;
+    nr = ncy * per_row;
+    if (t < nr) {
+      const int row = bys[t / per_row], piece = t % per_row;
+      const int ba = piece == 0 ? b0 : 0, bb = piece == 0 ? b1 : min(wrap_b1, b0 - 1);
+      s_rbeg[t] = A.bin_start[row * g.nbx + ba];
+      s_rend[t] = bb >= ba ? A.bin_start[row * g.nbx + bb + 1] : s_rbeg[t];
+    }
+  }
+  __syncthreads();
 
-  for (int cy = 0; cy < ncy; ++cy) {
-    for (int cx = 0; cx < ncx; ++cx) {
-      const int b = bys[cy] * g.nbx + bxs[cx];
-      const int pbeg = A.bin_start[b], pend = A.bin_start[b + 1];
-      for (int c0 = pbeg; c0 < pend; c0 += PCH) {
-        const int np = min(PCH, pend - c0);
-        __syncthreads();
-        // ---- phase A: footprint weights of the chunk
-        if (t < np) {
-          const double* r = A.pos_s + 3 * (size_t)(c0 + t);
-          double zp = r[2];
-          int lmin = 1, lmax = 0;
-          int i0 = 0, j0 = 0;
-          if (zp >= 0.0) {
-            i0 = origin_cell(r[0], g.alpha, g.h, g.nx);
-            j0 = origin_cell(r[1], g.alpha, g.h, g.ny);
-            z_range(s_zn, nz, zp, g.alpha, g.H, lmin, lmax);
-          }
-          s_meta[4 * t] = i0; s_meta[4 * t + 1] = j0; s_meta[4 * t + 2] = lmin; s_meta[4 * t + 3] = lmax;
-          for (int c = 0; c < 3; ++c) s_val[3 * t + c] = val[3 * (size_t)(c0 + t) + c];
+  // ---- cull pass 1: hits per range (one warp per range; records stay in registers for pass 2 when the range is short)
+  for (int r = wid; r < nr; r += NW) {
+    int cnt = 0;
+    for (int p0 = s_rbeg[r]; p0 < s_rend[r]; p0 += 32) {
+      const int p = p0 + lane;
+      bool hit = false;
+      if (p < s_rend[r]) {
+        const int4 m = A.meta[p];
+        int dx = X0 - m.x; if (dx < 0) dx += g.nx;            // tile columns X0 .. X0+TX-1 vs footprint i0 .. i0+w-1 (cyclic)
+        int dy = Y0 - m.y; if (dy < 0) dy += g.ny;
+        hit = m.z <= m.w && (dx < w || dx > g.nx - TX) && (dy < w || dy > g.ny - TY);
+      }
+      cnt += __popc(__ballot_sync(0xffffffffu, hit));
+    }
+    if (lane == 0) s_rcnt[r] = cnt;
+  }
+  __syncthreads();
+  int total = 0;
+  for (int r = 0; r < nr; ++r) total += s_rcnt[r];
+
+  for (int c0 = 0; c0 < total; c0 += PCH) {
+    const int nl = min(PCH, total - c0);
+    // ---- cull pass 2: list positions [c0, c0+PCH) in range order; the hit lanes fetch position and value
+    for (int r = wid; r < nr; r += NW) {
+      int pos0 = 0;
+      for (int q = 0; q < r; ++q) pos0 += s_rcnt[q];
+      if (pos0 >= c0 + PCH || pos0 + s_rcnt[r] <= c0) continue;
+      for (int p0 = s_rbeg[r]; p0 < s_rend[r]; p0 += 32) {
+        const int p = p0 + lane;
+        bool hit = false;
+        int4 m = make_int4(0, 0, 1, 0);
+        double px = 0, py = 0, pz = 0, v0 = 0, v1 = 0, v2 = 0;
+        if (p < s_rend[r]) {
+          m = A.meta[p];
+          px = A.pos_s[3 * (size_t)p]; py = A.pos_s[3 * (size_t)p + 1]; pz = A.pos_s[3 * (size_t)p + 2];
+          v0 = val[3 * (size_t)p]; v1 = val[3 * (size_t)p + 1]; v2 = val[3 * (size_t)p + 2];
+          int dx = X0 - m.x; if (dx < 0) dx += g.nx;
+          int dy = Y0 - m.y; if (dy < 0) dy += g.ny;
+          hit = m.z <= m.w && (dx < w || dx > g.nx - TX) && (dy < w || dy > g.ny - TY);
         }
-        for (int i = t; i < np * 2 * w; i += SPREAD_THREADS) {
-          int q = i / (2 * w), rr = i % (2 * w);
-          const double* r = A.pos_s + 3 * (size_t)(c0 + q);
-          if (rr < w) {
-            double xw = r[0];
-            double i0 = ceil((xw - g.alpha) / g.h);         // unwrapped origin: distances use the unwrapped node
-            s_wx[q * DP_MAX_W + rr] = xy_weight((i0 + rr) * g.h - xw, g.alpha, beta, Z);
-          } else {
-            double yw = r[1];
-            double j0 = ceil((yw - g.alpha) / g.h);
-            s_wy[q * DP_MAX_W + rr - w] = xy_weight((j0 + (rr - w)) * g.h - yw, g.alpha, beta, Z);
-          }
+        const unsigned msk = __ballot_sync(0xffffffffu, hit);
+        const int q = pos0 + __popc(msk & ((1u << lane) - 1u)) - c0;
+        if (hit && q >= 0 && q < PCH) {
+          s_meta[q] = m;
+          s_pos[q][0] = px; s_pos[q][1] = py; s_pos[q][2] = pz;
+          s_val[q][0] = v0; s_val[q][1] = v1; s_val[q][2] = v2;
         }
-        for (int i = t; i < np * nz; i += SPREAD_THREADS) {
-          int q = i / nz, l = i % nz;
-          double zp = A.pos_s[3 * (size_t)(c0 + q) + 2];
-          s_zt[q * nz + l] = zp >= 0.0 ? zeta_weight(s_zn[l], zp, g.H, g.wall_mode, g.alpha, beta, Z) : 0.0;
-        }
-        __syncthreads();
-        // ---- phase B: each thread adds to its own column (ti, tj), z residue class tz
-        for (int q = 0; q < np; ++q) {
-          int a = gi - s_meta[4 * q]; if (a < 0) a += g.nx;
-          int bb = gj - s_meta[4 * q + 1]; if (bb < 0) bb += g.ny;
-          if (a < w && bb < w && gi < g.nx && gj < g.ny) {
-            const double wxy = s_wx[q * DP_MAX_W + a] * s_wy[q * DP_MAX_W + bb];
-            const double v0 = s_val[3 * q], v1 = s_val[3 * q + 1], v2 = s_val[3 * q + 2];
-            const int lmin = s_meta[4 * q + 2], lmax = s_meta[4 * q + 3];
-            // a thread owns the planes l = tz (mod ZSPLIT) of its column for EVERY particle: no two threads ever touch the same cell
-            for (int l = lmin + ((tz - lmin) & (ZSPLIT - 1)); l <= lmax; l += ZSPLIT) {
-              const double wgt = wxy * s_zt[q * nz + l];
-              double* o = acc + (l * TY + tj) * TX + ti;
-              o[0] += v0 * wgt;
-              o[nz * TY * TX] += v1 * wgt;
-              o[2 * nz * TY * TX] += v2 * wgt;
+        pos0 += __popc(msk);
+      }
+    }
+    __syncthreads();
+    // ---- weights of the listed particles: phi(x_i - x), phi(y_j - y), zeta(l; z) (eqs 9, 54)
+    constexpr int ITEMS = 2 * DP_MAX_W + NZ;
+    for (int i = t; i < nl * ITEMS; i += SPREAD_THREADS) {
+      const int q = i / ITEMS, rr = i % ITEMS;
+      if (rr < DP_MAX_W) {
+        const double xw = s_pos[q][0], i0 = ceil((xw - g.alpha) / g.h);   // unwrapped origin: distances use the unwrapped node
+        s_wx[q][rr] = rr < w ? es_phi((i0 + rr) * g.h - xw, inv_alpha, beta, inv_Z) : 0.0;
+      } else if (rr < 2 * DP_MAX_W) {
+        const int b = rr - DP_MAX_W;
+        const double yw = s_pos[q][1], j0 = ceil((yw - g.alpha) / g.h);
+        s_wy[q][b] = b < w ? es_phi((j0 + b) * g.h - yw, inv_alpha, beta, inv_Z) : 0.0;
+      } else {
+        const int l = rr - 2 * DP_MAX_W;
+        s_zt[q][l] = (l >= s_meta[q].z && l <= s_meta[q].w) ? zeta_weight(s_zn[l], s_pos[q][2], g.H, g.wall_mode, inv_alpha, beta, inv_Z) : 0.0;
+      }
+    }
+    __syncthreads();
+    // ---- accumulate: each thread adds the particles covering its column to its own planes
+    if (in_grid) {
+      for (int q = 0; q < nl; ++q) {
+        const int4 m = s_meta[q];
+        int a = gi - m.x; if (a < 0) a += g.nx;
+        int bb = gj - m.y; if (bb < 0) bb += g.ny;
+        if (a < w && bb < w) {
+          const double wxy = s_wx[q][a] * s_wy[q][bb];
+          const double v0 = s_val[q][0] * wxy, v1 = s_val[q][1] * wxy, v2 = s_val[q][2] * wxy;
+#pragma unroll
+          for (int li = 0; li < NL; ++li) {
+            const int l = ZSPLIT * li + tz;
+            if (l >= m.z && l <= m.w) {            // zeta vanishes outside [lmin, lmax]: skipping is exact
+              const double zt = s_zt[q][l];
+              acc[li][0] = fma(v0, zt, acc[li][0]);
+              acc[li][1] = fma(v1, zt, acc[li][1]);
+              acc[li][2] = fma(v2, zt, acc[li][2]);
             }
           }
         }
       }
     }
+    if (c0 + PCH < total) __syncthreads();
   }
-  __syncthreads();
-  // ---- flush the tile: every value written once, 16-byte stores
-  const int rows = 3 * nz * TY;
-  for (int i = t; i < rows * (TX / 2); i += SPREAD_THREADS) {
-    int row = i / (TX / 2), i2 = (i % (TX / 2)) * 2;
-    int j = row % TY, l = (row / TY) % nz, c = row / (TY * nz);
-    int col = X0 + i2, rowg = Y0 + j;
-    if (col < g.nx && rowg < g.ny) {
-      double2 v = *reinterpret_cast<const double2*>(acc + ((c * nz + l) * TY + j) * TX + i2);
-      double* dst = A.grid + (size_t)(A.field0[grp] + c) * A.real_field + ((size_t)l * g.ny + rowg) * g.nx + col;
-      *reinterpret_cast<double2*>(dst) = v;       // nx even, col even: 16-byte aligned
+  // ---- store: every grid value written exactly once
+  if (in_grid) {
+#pragma unroll
+    for (int li = 0; li < NL; ++li) {
+      const int l = ZSPLIT * li + tz;
+      double* dst = A.grid + (size_t)A.field0[grp] * A.real_field + ((size_t)l * g.ny + gj) * g.nx + gi;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) dst[c * A.real_field] = acc[li][c];
     }
   }
 }
@@ -292,10 +355,10 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs 
       __syncwarp();
       for (int k = 0; k < nk; ++k) {
         double* sw = s_w[wid][k];
-        if (lane < w) sw[lane] = xy_weight((fi0 + lane) * g.h - xw, g.alpha, A.beta[k], A.Z[k]);
-        else if (lane >= 8 && lane < 8 + w) sw[DP_MAX_W + lane - 8] = xy_weight((fj0 + (lane - 8)) * g.h - yw, g.alpha, A.beta[k], A.Z[k]);
+        if (lane < w) sw[lane] = es_phi((fi0 + lane) * g.h - xw, 1.0 / g.alpha, A.beta[k], 1.0 / A.Z[k]);
+        else if (lane >= 8 && lane < 8 + w) sw[DP_MAX_W + lane - 8] = es_phi((fj0 + (lane - 8)) * g.h - yw, 1.0 / g.alpha, A.beta[k], 1.0 / A.Z[k]);
         for (int l = lmin + lane; l <= lmax; l += 32)
-          sw[2 * DP_MAX_W + l] = zeta_weight(s_zn[l], zp, g.H, g.wall_mode, g.alpha, A.beta[k], A.Z[k]);
+          sw[2 * DP_MAX_W + l] = zeta_weight(s_zn[l], zp, g.H, g.wall_mode, 1.0 / g.alpha, A.beta[k], 1.0 / A.Z[k]);
       }
       __syncwarp();
       const int ww = w * w, nent = (lmax - lmin + 1) * ww;
@@ -331,10 +394,6 @@ GridGeom make_geom(const dp_plan* P) {
   return g;
 }
 
-size_t spread_smem_bytes(int nz) {
-  return sizeof(double) * ((size_t)3 * nz * TY * TX + nz + 2 * PCH * DP_MAX_W + (size_t)PCH * nz + PCH * 3) + sizeof(int) * PCH * 4;
-}
-
 }  // namespace
 
 cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* force, const double* torque, cudaStream_t st) {
@@ -346,8 +405,8 @@ cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* fo
   const int T = 256, B = (n + T - 1) / T;
   k_bin_count<<<B, T, 0, st>>>(n, pos, g, P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_flag);
   k_scan<<<1, 1024, 0, st>>>(P->nbins, P->d_bin_count, P->d_bin_start);
-  k_bin_scatter<<<B, T, 0, st>>>(n, pos, force, torque, g, P->d_bin_of, P->d_slot_of, P->d_bin_start, P->d_perm, P->d_pos_s,
-                                P->d_frc_s, P->fields == 6 ? P->d_trq_s : nullptr);
+  k_bin_scatter<<<B, T, 0, st>>>(n, pos, force, torque, g, P->d_bin_of, P->d_slot_of, P->d_bin_start, P->d_znodes, P->d_perm, P->d_meta,
+                                P->d_pos_s, P->d_frc_s, P->fields == 6 ? P->d_trq_s : nullptr);
   return cudaGetLastError();
 }
 
@@ -362,18 +421,17 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
   A.field0[0] = 0; A.field0[1] = 3;
   A.ngroups = with_torque ? 2 : 1;
   A.bin_start = P->d_bin_start;
+  A.meta = P->d_meta;
   A.znodes = P->d_znodes;
   A.grid = P->d_real;
   A.real_field = P->real_field;
-  size_t smem = spread_smem_bytes(P->p.nz);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(k_spread, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
   dim3 grid(P->nbins, A.ngroups);
-  k_spread<<<grid, SPREAD_THREADS, smem, st>>>(A);
+  switch (P->p.nz) {
+    case 16: k_spread<16><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
+    case 32: k_spread<32><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
+    case 48: k_spread<48><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
+    default: return cudaErrorInvalidValue;
+  }
   return cudaGetLastError();
 }
 
