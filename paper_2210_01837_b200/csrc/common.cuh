@@ -45,6 +45,7 @@ struct dp_plan {
   double* d_trq_s = nullptr;    // [n][3]
   int* d_perm = nullptr;        // sorted slot -> original index
   int4* d_meta = nullptr;       // sorted footprint records: wrapped origin node (i0, j0), plane range [lmin, lmax]
+  double* d_wrec = nullptr;     // sorted 1-D ES weight records [2][max_particles][16 + nz] (transfer.cu)
   int* d_bin_of = nullptr;      // per particle
   int* d_slot_of = nullptr;     // rank within its bin
   int* d_bin_count = nullptr;   // [nbins]

@@ -167,7 +167,7 @@ int dp_destroy(dp_plan* P) {
   cudaSetDevice(P->p.device);
   if (P->last_stream || true) cudaDeviceSynchronize();
   if (P->fft_ok) { cufftDestroy(P->fft_fwd); cufftDestroy(P->fft_inv); }
-  void* bufs[] = {P->d_real, P->d_cplx, P->d_fft_work, P->d_znodes, P->d_zweights, P->d_pos_s, P->d_frc_s, P->d_trq_s, P->d_perm, P->d_meta,
+  void* bufs[] = {P->d_real, P->d_cplx, P->d_fft_work, P->d_znodes, P->d_zweights, P->d_pos_s, P->d_frc_s, P->d_trq_s, P->d_perm, P->d_meta, P->d_wrec,
                   P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_bin_start, P->d_flag};
   for (void* b : bufs) if (b) cudaFree(b);
   if (P->ev_ok) for (auto& e : P->ev) cudaEventDestroy(e);
@@ -229,6 +229,7 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   if (p.use_torques) TRY(dev_alloc(P, &P->d_trq_s, 3 * np));
   TRY(dev_alloc(P, &P->d_perm, np));
   TRY(dev_alloc(P, &P->d_meta, np));
+  TRY(dev_alloc(P, &P->d_wrec, np * (p.use_torques ? 2 : 1) * (2 * DP_MAX_W + p.nz)));
   TRY(dev_alloc(P, &P->d_bin_of, np));
   TRY(dev_alloc(P, &P->d_slot_of, np));
   TRY(dev_alloc(P, &P->d_bin_count, (size_t)P->nbins));

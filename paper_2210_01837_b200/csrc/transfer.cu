@@ -16,7 +16,7 @@ namespace {
 constexpr int TX = DP_TILE_X, TY = DP_TILE_Y;
 constexpr int ZSPLIT = 4;                       // z residue classes per column
 constexpr int SPREAD_THREADS = TX * TY * ZSPLIT;
-constexpr int PCH = 32;                         // particles staged per chunk
+constexpr int PCH = 40;                         // candidate particles staged per chunk
 constexpr int MAXB = 6;                         // origin bins per direction that can reach a tile (w <= 8, TY = 4)
 constexpr int MAXR = 2 * MAXB;                  // candidate ranges per tile: one per bin row, two when the x range wraps
 
@@ -144,58 +144,89 @@ __global__ void k_bin_scatter(int n, const double* __restrict__ pos, const doubl
   }
 }
 
+// ---------------------------------------------------------------------------------------------- 1-D ES weights
+// One record per particle and envelope (0: Delta_M, 1: Delta_D), in sorted order, evaluated once per product and used by
+// both spreading and interpolation:  rec[0..7] = phi(x_{i0+a} - x), rec[8..15] = phi(y_{j0+b} - y), rec[16+l] = zeta(l; z)
+// (eqs 9, 54).  One thread per record entry.
+struct WeightArgs {
+  GridGeom g;
+  const double* pos_s;
+  const int4* meta;
+  const double* znodes;
+  double beta[2], Z[2];
+  double* wrec;              // [2][cap][16 + nz]
+  size_t cap;
+};
+
+__global__ void k_weights(int n, WeightArgs A) {
+  const GridGeom& g = A.g;
+  const int wrec = 2 * DP_MAX_W + g.nz;
+  const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+  if (i >= (size_t)n * wrec) return;
+  const int p = (int)(i / wrec), rr = (int)(i % wrec), k = blockIdx.y;
+  const double beta = A.beta[k], inv_Z = 1.0 / A.Z[k], inv_alpha = 1.0 / g.alpha;
+  const int4 m = A.meta[p];
+  double v = 0.0;
+  if (m.z <= m.w) {
+    if (rr < 2 * DP_MAX_W) {
+      const int a = rr & (DP_MAX_W - 1);
+      const double xw = A.pos_s[3 * (size_t)p + (rr >= DP_MAX_W ? 1 : 0)];
+      const double i0 = ceil((xw - g.alpha) / g.h);            // unwrapped origin: distances use the unwrapped node
+      if (a < g.w) v = es_phi((i0 + a) * g.h - xw, inv_alpha, beta, inv_Z);
+    } else {
+      const int l = rr - 2 * DP_MAX_W;
+      if (l >= m.z && l <= m.w) v = zeta_weight(A.znodes[l], A.pos_s[3 * (size_t)p + 2], g.H, g.wall_mode, inv_alpha, beta, inv_Z);
+    }
+  }
+  A.wrec[((size_t)k * A.cap + p) * wrec + rr] = v;
+}
+
 // ---------------------------------------------------------------------------------------------- spread
 struct SpreadArgs {
   GridGeom g;
-  const double* pos_s;
   const double* val_s[2];    // forces, torques (sorted)
-  double beta[2], Z[2];
   int field0[2];             // first output field of each group
-  int ngroups;
   const int* bin_start;
   const int4* meta;          // sorted footprint records (i0, j0, lmin, lmax)
-  const double* znodes;
+  const double* wrec;        // sorted weight records
+  size_t cap;
   double* grid;
   size_t real_field;
 };
 
 // One CTA = one tile of TX x TY grid columns of one field triple.  Thread (ti, tj, tz) owns column (ti, tj) and the
 // planes l = ZSPLIT*li + tz; its 3*NZ/ZSPLIT partial sums live in registers for the whole kernel, so there is no
-// shared-memory tile, no atomic and no memset.  Global-memory round trips per CTA: bin_start -> candidate records
-// (footprint, position, value: one batch of independent loads per warp) -> stores.  The candidates (the bins whose
-// footprints can reach the tile, merged into contiguous ranges of the sorted arrays) are culled by warp ballot, the 1-D
-// ES weights of the survivors are evaluated once per CTA into shared memory, every thread adds the particles covering
-// its column, and each value is stored to HBM exactly once (128-byte row segments per warp).
+// shared-memory tile, no atomic and no memset.  The candidates (the bins whose footprints can reach the tile, merged
+// into contiguous ranges of the sorted arrays) are staged in shared memory with their footprint and weight records;
+// every thread adds the particles covering its column; each grid value is stored to HBM exactly once (128-byte row
+// segments per warp).  Dependent global round trips per CTA: bin_start -> candidate records -> stores.
 template <int NZ>
 __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(SpreadArgs A) {
   constexpr int NL = NZ / ZSPLIT;
-  constexpr int NW = SPREAD_THREADS / 32;
-  __shared__ double s_zn[NZ];
-  __shared__ double s_wx[PCH][DP_MAX_W], s_wy[PCH][DP_MAX_W], s_zt[PCH][NZ], s_val[PCH][3], s_pos[PCH][3];
+  constexpr int WREC = 2 * DP_MAX_W + NZ;
+  __shared__ double s_w[PCH][WREC];
+  __shared__ double s_val[PCH][3];
   __shared__ int4 s_meta[PCH];                // i0, j0 (wrapped origin node), lmin, lmax
-  __shared__ int s_rbeg[MAXR], s_rend[MAXR], s_rcnt[MAXR];  // candidate ranges in the sorted arrays, hits per range
+  __shared__ int s_rbeg[MAXR], s_roff[MAXR + 1];   // candidate ranges in the sorted arrays; prefix sums of their lengths
 
   const GridGeom& g = A.g;
   const int w = g.w;
-  const int grp = blockIdx.y;
-  const int bx = blockIdx.x % g.nbx, by = blockIdx.x / g.nbx;
-  const int X0 = bx * TX, Y0 = by * TY;
+  const int grp = blockIdx.z;
+  const int X0 = blockIdx.x * TX, Y0 = blockIdx.y * TY;
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
   const int ti = t % TX, tj = (t / TX) % TY, tz = t / (TX * TY);
   const int gi = X0 + ti, gj = Y0 + tj;
   const bool in_grid = gi < g.nx && gj < g.ny;
-  const double beta = A.beta[grp], inv_Z = 1.0 / A.Z[grp], inv_alpha = 1.0 / g.alpha;
   const double* __restrict__ val = A.val_s[grp];
+  const double* __restrict__ wrec = A.wrec + (size_t)grp * A.cap * WREC;
 
   double acc[NL][3];
 #pragma unroll
   for (int li = 0; li < NL; ++li) { acc[li][0] = 0.0; acc[li][1] = 0.0; acc[li][2] = 0.0; }
 
-  for (int i = t; i < NZ; i += SPREAD_THREADS) s_zn[i] = A.znodes[i];
   // bins whose footprints can reach this tile: origin columns in the cyclic range [X0-w+1, X0+TXeff-1] (same in y);
   // the x-bins of one bin row are consecutive in memory, so each row gives one range (two when the range wraps in x)
-  int nr;
-  {
+  if (wid == 0) {
     int o = X0 - (w - 1); o %= g.nx; if (o < 0) o += g.nx;
     const int len = min(TX, g.nx - X0) + w - 1;                 // <= nx (checked at create)
     const int b0 = o / TX, b1 = (o + len - 1 < g.nx) ? (o + len - 1) / TX : g.nbx - 1;
@@ -203,82 +234,44 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
     int bys[MAXB];
     const int ncy = origin_bins(Y0, min(TY, g.ny - Y0), TY, w, g.ny, bys);
     const int per_row = wrap_b1 >= 0 ? 2 : 1;
-    nr = ncy * per_row;
-    if (t < nr) {
-      const int row = bys[t / per_row], piece = t % per_row;
+    const int nr = ncy * per_row;
+    int beg = 0, cnt = 0;
+    if (lane < nr) {
+      const int row = bys[lane / per_row], piece = lane % per_row;
       const int ba = piece == 0 ? b0 : 0, bb = piece == 0 ? b1 : min(wrap_b1, b0 - 1);
-      s_rbeg[t] = A.bin_start[row * g.nbx + ba];
-      s_rend[t] = bb >= ba ? A.bin_start[row * g.nbx + bb + 1] : s_rbeg[t];
+      beg = A.bin_start[row * g.nbx + ba];
+      cnt = bb >= ba ? A.bin_start[row * g.nbx + bb + 1] - beg : 0;
     }
+    int incl = cnt;                                           // inclusive scan over the (<= MAXR) ranges
+#pragma unroll
+    for (int o2 = 1; o2 < 16; o2 <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o2); if (lane >= o2) incl += v; }
+    if (lane < MAXR) { s_rbeg[lane] = beg; s_roff[lane + 1] = incl; }
+    if (lane == 0) s_roff[0] = 0;
   }
   __syncthreads();
+  const int total = s_roff[MAXR];
 
-  // ---- cull pass 1: hits per range (one warp per range; records stay in registers for pass 2 when the range is short)
-  for (int r = wid; r < nr; r += NW) {
-    int cnt = 0;
-    for (int p0 = s_rbeg[r]; p0 < s_rend[r]; p0 += 32) {
-      const int p = p0 + lane;
-      bool hit = false;
-      if (p < s_rend[r]) {
-        const int4 m = A.meta[p];
-        int dx = X0 - m.x; if (dx < 0) dx += g.nx;            // tile columns X0 .. X0+TX-1 vs footprint i0 .. i0+w-1 (cyclic)
-        int dy = Y0 - m.y; if (dy < 0) dy += g.ny;
-        hit = m.z <= m.w && (dx < w || dx > g.nx - TX) && (dy < w || dy > g.ny - TY);
-      }
-      cnt += __popc(__ballot_sync(0xffffffffu, hit));
-    }
-    if (lane == 0) s_rcnt[r] = cnt;
-  }
-  __syncthreads();
-  int total = 0;
-  for (int r = 0; r < nr; ++r) total += s_rcnt[r];
-
+  // Every candidate is staged (no cull pass: the candidates of a range are contiguous, so their records arrive in one
+  // batch of independent coalesced loads); the exact footprint test happens per thread in the accumulation loop.
   for (int c0 = 0; c0 < total; c0 += PCH) {
     const int nl = min(PCH, total - c0);
-    // ---- cull pass 2: list positions [c0, c0+PCH) in range order; the hit lanes fetch position and value
-    for (int r = wid; r < nr; r += NW) {
-      int pos0 = 0;
-      for (int q = 0; q < r; ++q) pos0 += s_rcnt[q];
-      if (pos0 >= c0 + PCH || pos0 + s_rcnt[r] <= c0) continue;
-      for (int p0 = s_rbeg[r]; p0 < s_rend[r]; p0 += 32) {
-        const int p = p0 + lane;
-        bool hit = false;
-        int4 m = make_int4(0, 0, 1, 0);
-        double px = 0, py = 0, pz = 0, v0 = 0, v1 = 0, v2 = 0;
-        if (p < s_rend[r]) {
-          m = A.meta[p];
-          px = A.pos_s[3 * (size_t)p]; py = A.pos_s[3 * (size_t)p + 1]; pz = A.pos_s[3 * (size_t)p + 2];
-          v0 = val[3 * (size_t)p]; v1 = val[3 * (size_t)p + 1]; v2 = val[3 * (size_t)p + 2];
-          int dx = X0 - m.x; if (dx < 0) dx += g.nx;
-          int dy = Y0 - m.y; if (dy < 0) dy += g.ny;
-          hit = m.z <= m.w && (dx < w || dx > g.nx - TX) && (dy < w || dy > g.ny - TY);
-        }
-        const unsigned msk = __ballot_sync(0xffffffffu, hit);
-        const int q = pos0 + __popc(msk & ((1u << lane) - 1u)) - c0;
-        if (hit && q >= 0 && q < PCH) {
-          s_meta[q] = m;
-          s_pos[q][0] = px; s_pos[q][1] = py; s_pos[q][2] = pz;
-          s_val[q][0] = v0; s_val[q][1] = v1; s_val[q][2] = v2;
-        }
-        pos0 += __popc(msk);
-      }
+    if (t < nl) {
+      const int c = c0 + t;
+      int r = 0;
+#pragma unroll
+      for (int q = 1; q < MAXR; ++q) r += (c >= s_roff[q]) ? 1 : 0;
+      const int p = s_rbeg[r] + (c - s_roff[r]);
+      s_meta[t] = A.meta[p];
+      s_val[t][0] = val[3 * (size_t)p]; s_val[t][1] = val[3 * (size_t)p + 1]; s_val[t][2] = val[3 * (size_t)p + 2];
     }
-    __syncthreads();
-    // ---- weights of the listed particles: phi(x_i - x), phi(y_j - y), zeta(l; z) (eqs 9, 54)
-    constexpr int ITEMS = 2 * DP_MAX_W + NZ;
-    for (int i = t; i < nl * ITEMS; i += SPREAD_THREADS) {
-      const int q = i / ITEMS, rr = i % ITEMS;
-      if (rr < DP_MAX_W) {
-        const double xw = s_pos[q][0], i0 = ceil((xw - g.alpha) / g.h);   // unwrapped origin: distances use the unwrapped node
-        s_wx[q][rr] = rr < w ? es_phi((i0 + rr) * g.h - xw, inv_alpha, beta, inv_Z) : 0.0;
-      } else if (rr < 2 * DP_MAX_W) {
-        const int b = rr - DP_MAX_W;
-        const double yw = s_pos[q][1], j0 = ceil((yw - g.alpha) / g.h);
-        s_wy[q][b] = b < w ? es_phi((j0 + b) * g.h - yw, inv_alpha, beta, inv_Z) : 0.0;
-      } else {
-        const int l = rr - 2 * DP_MAX_W;
-        s_zt[q][l] = (l >= s_meta[q].z && l <= s_meta[q].w) ? zeta_weight(s_zn[l], s_pos[q][2], g.H, g.wall_mode, inv_alpha, beta, inv_Z) : 0.0;
-      }
+#pragma unroll 2
+    for (int i = t; i < nl * WREC; i += SPREAD_THREADS) {
+      const int q = i / WREC, e = i - q * WREC, c = c0 + q;
+      int r = 0;
+#pragma unroll
+      for (int k = 1; k < MAXR; ++k) r += (c >= s_roff[k]) ? 1 : 0;
+      const int p = s_rbeg[r] + (c - s_roff[r]);
+      s_w[q][e] = wrec[(size_t)p * WREC + e];
     }
     __syncthreads();
     // ---- accumulate: each thread adds the particles covering its column to its own planes
@@ -287,17 +280,23 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
         const int4 m = s_meta[q];
         int a = gi - m.x; if (a < 0) a += g.nx;
         int bb = gj - m.y; if (bb < 0) bb += g.ny;
-        if (a < w && bb < w) {
-          const double wxy = s_wx[q][a] * s_wy[q][bb];
+        if (a < w && bb < w && m.z <= m.w) {
+          const double wxy = s_w[q][a] * s_w[q][DP_MAX_W + bb];
           const double v0 = s_val[q][0] * wxy, v1 = s_val[q][1] * wxy, v2 = s_val[q][2] * wxy;
+          const double* zt = &s_w[q][2 * DP_MAX_W + tz];
+          // zeta vanishes outside [lmin, lmax]: skipping a half of the planes that lies outside is exact
+          if (m.z < ZSPLIT * (NL / 2)) {
 #pragma unroll
-          for (int li = 0; li < NL; ++li) {
-            const int l = ZSPLIT * li + tz;
-            if (l >= m.z && l <= m.w) {            // zeta vanishes outside [lmin, lmax]: skipping is exact
-              const double zt = s_zt[q][l];
-              acc[li][0] = fma(v0, zt, acc[li][0]);
-              acc[li][1] = fma(v1, zt, acc[li][1]);
-              acc[li][2] = fma(v2, zt, acc[li][2]);
+            for (int li = 0; li < NL / 2; ++li) {
+              const double z = zt[ZSPLIT * li];
+              acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+            }
+          }
+          if (m.w >= ZSPLIT * (NL / 2)) {
+#pragma unroll
+            for (int li = NL / 2; li < NL; ++li) {
+              const double z = zt[ZSPLIT * li];
+              acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
             }
           }
         }
@@ -320,10 +319,10 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
 // ---------------------------------------------------------------------------------------------- interpolate
 struct InterpArgs {
   GridGeom g;
-  const double* pos_s;
   const int* perm;
-  double beta[2], Z[2];
-  const double* znodes;
+  const int4* meta;
+  const double* wrec;
+  size_t cap;
   const double* zweights;    // h^2 (H/2) w_l
   const double* grid;
   size_t real_field;
@@ -333,39 +332,33 @@ struct InterpArgs {
 
 constexpr int INTERP_WARPS = 8;
 
+// One warp per particle (sorted order, so neighbouring warps gather from neighbouring columns): the lanes sweep the
+// w x w x (lmax-lmin+1) footprint, weights come from the particle's records, the six sums are reduced by shuffles.
 __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs A) {
-  __shared__ double s_w[INTERP_WARPS][2][2 * DP_MAX_W + DP_MAX_NZ];   // per warp, per kernel: wx[8], wy[8], zeta[nz]
-  __shared__ double s_zn[DP_MAX_NZ], s_zw[DP_MAX_NZ];
+  __shared__ double s_w[INTERP_WARPS][2][2 * DP_MAX_W + DP_MAX_NZ];   // per warp, per envelope: wx[8], wy[8], zeta[nz]
+  __shared__ double s_zw[DP_MAX_NZ];
   const GridGeom& g = A.g;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const int nz = g.nz, w = g.w;
-  for (int i = threadIdx.x; i < nz; i += blockDim.x) { s_zn[i] = A.znodes[i]; s_zw[i] = A.zweights[i]; }
+  const int nz = g.nz, w = g.w, wrec = 2 * DP_MAX_W + nz;
+  for (int i = threadIdx.x; i < nz; i += blockDim.x) s_zw[i] = A.zweights[i];
   __syncthreads();
   const int nk = A.Omega ? 2 : 1;
   for (int p = blockIdx.x * INTERP_WARPS + wid; p < n; p += gridDim.x * INTERP_WARPS) {
-    const double xw = A.pos_s[3 * (size_t)p], yw = A.pos_s[3 * (size_t)p + 1], zp = A.pos_s[3 * (size_t)p + 2];
+    const int4 m = A.meta[p];
     const int dst = A.perm[p];
     double s[6] = {0, 0, 0, 0, 0, 0};
-    if (zp >= 0.0) {
-      const double fi0 = ceil((xw - g.alpha) / g.h), fj0 = ceil((yw - g.alpha) / g.h);
-      int i0 = (int)fi0 % g.nx; if (i0 < 0) i0 += g.nx;
-      int j0 = (int)fj0 % g.ny; if (j0 < 0) j0 += g.ny;
-      int lmin, lmax;
-      z_range(s_zn, nz, zp, g.alpha, g.H, lmin, lmax);
+    if (m.z <= m.w) {
       __syncwarp();
       for (int k = 0; k < nk; ++k) {
-        double* sw = s_w[wid][k];
-        if (lane < w) sw[lane] = es_phi((fi0 + lane) * g.h - xw, 1.0 / g.alpha, A.beta[k], 1.0 / A.Z[k]);
-        else if (lane >= 8 && lane < 8 + w) sw[DP_MAX_W + lane - 8] = es_phi((fj0 + (lane - 8)) * g.h - yw, 1.0 / g.alpha, A.beta[k], 1.0 / A.Z[k]);
-        for (int l = lmin + lane; l <= lmax; l += 32)
-          sw[2 * DP_MAX_W + l] = zeta_weight(s_zn[l], zp, g.H, g.wall_mode, 1.0 / g.alpha, A.beta[k], 1.0 / A.Z[k]);
+        const double* rec = A.wrec + ((size_t)k * A.cap + p) * wrec;
+        for (int e = lane; e < wrec; e += 32) s_w[wid][k][e] = rec[e];
       }
       __syncwarp();
-      const int ww = w * w, nent = (lmax - lmin + 1) * ww;
+      const int ww = w * w, nent = (m.w - m.z + 1) * ww;
       for (int e = lane; e < nent; e += 32) {
-        int l = lmin + e / ww, rem = e % ww, b = rem / w, a = rem % w;
-        int i = i0 + a; if (i >= g.nx) i -= g.nx;
-        int j = j0 + b; if (j >= g.ny) j -= g.ny;
+        int l = m.z + e / ww, rem = e % ww, b = rem / w, a = rem % w;
+        int i = m.x + a; if (i >= g.nx) i -= g.nx;
+        int j = m.y + b; if (j >= g.ny) j -= g.ny;
         const size_t off = ((size_t)l * g.ny + j) * g.nx + i;
         const double wl = s_zw[l];
         for (int k = 0; k < nk; ++k) {
@@ -411,21 +404,31 @@ cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* fo
 }
 
 cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torque, cudaStream_t st) {
-  (void)n; (void)with_force;
+  (void)with_force;
+  const int ngroups = with_torque ? 2 : 1;
+  {
+    // weight records of both envelopes (the dipole records are also needed when only Omega is wanted: always built on 6-field plans)
+    WeightArgs W;
+    W.g = make_geom(P);
+    W.pos_s = P->d_pos_s; W.meta = P->d_meta; W.znodes = P->d_znodes;
+    W.beta[0] = P->p.beta_M; W.beta[1] = P->p.beta_D;
+    W.Z[0] = P->ZM; W.Z[1] = P->ZD;
+    W.wrec = P->d_wrec; W.cap = (size_t)P->p.max_particles;
+    const int wrec = 2 * DP_MAX_W + P->p.nz;
+    const size_t items = (size_t)n * wrec;
+    dim3 wg((unsigned)((items + 255) / 256), P->fields == 6 ? 2 : 1);
+    k_weights<<<wg, 256, 0, st>>>(n, W);
+  }
   SpreadArgs A;
   A.g = make_geom(P);
-  A.pos_s = P->d_pos_s;
   A.val_s[0] = P->d_frc_s; A.val_s[1] = P->d_trq_s;
-  A.beta[0] = P->p.beta_M; A.beta[1] = P->p.beta_D;
-  A.Z[0] = P->ZM; A.Z[1] = P->ZD;
   A.field0[0] = 0; A.field0[1] = 3;
-  A.ngroups = with_torque ? 2 : 1;
   A.bin_start = P->d_bin_start;
   A.meta = P->d_meta;
-  A.znodes = P->d_znodes;
+  A.wrec = P->d_wrec; A.cap = (size_t)P->p.max_particles;
   A.grid = P->d_real;
   A.real_field = P->real_field;
-  dim3 grid(P->nbins, A.ngroups);
+  dim3 grid(P->nbx, P->nby, ngroups);
   switch (P->p.nz) {
     case 16: k_spread<16><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
     case 32: k_spread<32><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
@@ -438,10 +441,9 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
 cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaStream_t st) {
   InterpArgs A;
   A.g = make_geom(P);
-  A.pos_s = P->d_pos_s; A.perm = P->d_perm;
-  A.beta[0] = P->p.beta_M; A.beta[1] = P->p.beta_D;
-  A.Z[0] = P->ZM; A.Z[1] = P->ZD;
-  A.znodes = P->d_znodes; A.zweights = P->d_zweights;
+  A.perm = P->d_perm; A.meta = P->d_meta;
+  A.wrec = P->d_wrec; A.cap = (size_t)P->p.max_particles;
+  A.zweights = P->d_zweights;
   A.grid = P->d_real; A.real_field = P->real_field;
   A.U = U; A.Omega = Omega;
   int blocks = (n + INTERP_WARPS - 1) / INTERP_WARPS;
