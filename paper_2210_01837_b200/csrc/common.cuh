@@ -18,8 +18,8 @@
 #define DP_TILE_X 16
 #define DP_TILE_Y 4
 
-// modes per CTA in the solve kernel (consecutive kx of one ky row) = one warp of modes
-#define DP_SOLVE_TM 32
+// modes per CTA in the solve kernel (consecutive modes of one row of the half spectrum); a lane is (mode, re/im)
+#define DP_SOLVE_TM 16
 
 struct dp_tables_host;
 

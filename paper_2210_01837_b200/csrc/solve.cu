@@ -12,11 +12,15 @@
 // chains (n even / n odd), each with one border unknown (c_0 resp. b_0) fixed by one combination of the two
 // boundary rows.  The chains are factored once per mode and reused for p, u, v, w.
 //
-// B200 mapping: one CTA = 32 consecutive kx of one ky row (a warp of modes).  All per-mode vectors live in shared
-// memory as [vector][n][mode] (mode fastest: conflict-free, and the HBM rows are 512-byte coalesced).  Work is split
-// into phases of independent items (vector x parity for the cosine transforms, part x chain for the sweeps);
-// each warp takes an item, its 32 lanes are the 32 modes, so the transform matrices are warp-uniform and come
-// straight from the constant bank as immediate operands of the DFMAs (fully unrolled, nz is a template parameter).
+// B200 mapping: one CTA = 16 consecutive modes of one row of the half spectrum, 6 warps.  A lane is (mode, part):
+// lane = 2*mode + part, part 0 = real, 1 = imaginary, so a warp row of a complex column is 256 contiguous bytes in HBM
+// and in shared memory ([column][n][lane], conflict free).  Every real operator of the method (cosine transforms,
+// z-derivative, tridiagonal sweeps) acts on a lane's own 32 numbers only, so a warp that owns a column needs no
+// synchronisation at all; the imaginary unit couples a lane to its neighbour (lane^1).  Work is split into phases of
+// independent column items, one warp per item, sized so that 5-6 of the 6 warps are busy in every long phase; the
+// sweeps run out of registers (all loads hoisted), divisions by constants are compile-time reciprocals, and the
+// transform matrices are warp-uniform constant-bank operands of fully unrolled DFMAs (nz is a template parameter).
+// Shared memory: 6 columns + 3 factor vectors = 61 KB at nz = 32 -> 3 CTAs (18 warps) per SM.
 #include <cmath>
 #include <vector>
 
@@ -24,15 +28,19 @@
 
 namespace {
 
-constexpr int TM = DP_SOLVE_TM;
-constexpr int SOLVE_THREADS = 256;
-constexpr int NWARPS = SOLVE_THREADS / 32;
-constexpr int NVEC = 13;      // real shared-memory vectors per mode (see kernel)
+constexpr int TM = DP_SOLVE_TM;        // modes per CTA
+constexpr int LN = 2 * TM;             // lanes of a complex column row (= 32)
+constexpr int SOLVE_WARPS = 6;
+constexpr int SOLVE_THREADS = SOLVE_WARPS * 32;
+static_assert(LN == 32, "a warp row is one complex column row");
 
-// ---- constant tables per compiled nz: CT[n][l] = cos(n l pi/N) (n = 0..N, l < nz/2), P[n], Q[n] (boundary-row
-//      functionals of a unit a_n, see kernel), XI[l] = cos(l pi/N)
+// ---- constant tables per compiled nz (N = nz-1, LH = nz/2):
+//   CA[n][l] = cos(n l pi/N), l < LH                       analysis rows (contiguous in l)
+//   SE[l][j] = cos(2j l pi/N), SO[l][j] = cos((2j+1) l pi/N), l, j < LH     synthesis rows (contiguous in j)
+//   P[n], Q[n]: boundary-row functionals of a unit a_n (see chain()), XI[l] = cos(l pi/N)
 template <int NZ> struct Tab {
-  static constexpr int CT = 0, P = NZ * (NZ / 2), Q = P + NZ, XI = Q + NZ, SIZE = XI + NZ;
+  static constexpr int LH = NZ / 2;
+  static constexpr int CA = 0, SE = CA + NZ * LH, SO = SE + LH * LH, P = SO + LH * LH, Q = P + NZ, XI = Q + NZ, SIZE = XI + NZ;
 };
 __constant__ double c_tab16[Tab<16>::SIZE];
 __constant__ double c_tab32[Tab<32>::SIZE];
@@ -45,472 +53,523 @@ template <> __device__ __forceinline__ const double* tab<48>() { return c_tab48;
 struct SolveArgs {
   double2* cplx;
   size_t cplx_field;
-  int nx, ny, nkx, nkxp;
+  int nx, ny, nkx;
+  int n_fast, n_slow, pitch;     // half spectrum stored as [field][l][slow][fast (pitch)]
+  int fast_is_x;                 // 1: fast index = kx index (cuFFT layout); 0: fast index = ky index (transposed layout)
   double Lx, Ly, H, eta;
   int wall_mode, torque, omega;
 };
 
-// ---- tridiagonal rows of a chain (n >= 1): d_n a_n + l_n a_{n-2} + u_n a_{n+2}
-template <int NZ> __device__ __forceinline__ double row_d(int n, double k2) { return n == 1 ? 1.0 + k2 * 0.125 : 1.0 + k2 / (2.0 * (n * n - 1)); }
-template <int NZ> __device__ __forceinline__ double row_l(int n, double k2) { return -k2 * (n == 2 ? 2.0 : 1.0) / (4.0 * n * (n - 1)); }
-template <int NZ> __device__ __forceinline__ double row_u(int n, double k2) { return (n + 2 <= NZ - 3) ? -k2 / (4.0 * n * (n + 1)) : 0.0; }
+// ---- tridiagonal rows of a chain (n >= 1): d_n a_n + l_n a_{n-2} + u_n a_{n+2}; all divisions are compile-time constants
+template <int NZ> __device__ __forceinline__ double row_d(int n, double k2) { return n == 1 ? fma(k2, 0.125, 1.0) : fma(k2, 1.0 / (2.0 * (n * n - 1)), 1.0); }
+template <int NZ> __device__ __forceinline__ double row_l(int n, double k2) { return k2 * (-(n == 2 ? 2.0 : 1.0) / (4.0 * n * (n - 1))); }
+template <int NZ> __device__ __forceinline__ double row_u(int n, double k2) { return (n + 2 <= NZ - 3) ? k2 * (-1.0 / (4.0 * n * (n + 1))) : 0.0; }
 
-// ---- DCT-I analysis of one real vector, one output parity (items of phases 1 and 6b)
+// ---- DCT-I analysis of a lane's column, in place:
 //   g^_n = (2/N)(1/c~_n) sum_l (1/c~_l) g_l cos(n l pi/N), folded with cos(n (N-l) pi/N) = (-1)^n cos(n l pi/N)
-template <int NZ> __device__ __forceinline__ void analysis_load(const double* v, int par, double* e) {
+template <int NZ> __device__ __forceinline__ void analysis_column(double* __restrict__ v) {
   constexpr int N = NZ - 1, LH = NZ / 2;
+  const double* __restrict__ T = tab<NZ>() + Tab<NZ>::CA;
+  double e[LH], o[LH];
 #pragma unroll
   for (int l = 0; l < LH; ++l) {
-    double a = v[l * TM], b = v[(N - l) * TM];
-    e[l] = par ? a - b : a + b;
+    const double a = v[l * LN], b = v[(N - l) * LN];
+    e[l] = a + b; o[l] = a - b;
   }
-  e[0] *= 0.5;
-}
-template <int NZ, int PAR> __device__ __forceinline__ void analysis_compute(double* v, const double* e) {
-  constexpr int N = NZ - 1, LH = NZ / 2;
-  const double* T = tab<NZ>();
+  e[0] *= 0.5; o[0] *= 0.5;
 #pragma unroll
   for (int j = 0; j < LH; ++j) {
-    const int n = 2 * j + PAR;
-    double acc = 0.0;
+    double ae = 0.0, ao = 0.0;
 #pragma unroll
-    for (int l = 0; l < LH; ++l) acc = fma(T[Tab<NZ>::CT + n * LH + l], e[l], acc);
-    v[n * TM] = acc * ((n == 0 || n == N) ? 1.0 / N : 2.0 / N);
+    for (int l = 0; l < LH; ++l) {
+      ae = fma(T[(2 * j) * LH + l], e[l], ae);
+      ao = fma(T[(2 * j + 1) * LH + l], o[l], ao);
+    }
+    v[(2 * j) * LN] = ae * (j == 0 ? 1.0 / N : 2.0 / N);
+    v[(2 * j + 1) * LN] = ao * ((2 * j + 1 == N) ? 1.0 / N : 2.0 / N);
   }
 }
 
-// ---- DCT-I synthesis of one real vector: g_l = sum_n g^_n cos(n l pi/N)
-template <int NZ> __device__ __forceinline__ void synthesis_inplace(double* v) {
+// ---- DCT-I synthesis of a lane's column, in place: g_l = sum_n g^_n cos(n l pi/N)
+template <int NZ> __device__ __forceinline__ void synthesis_column(double* __restrict__ v) {
   constexpr int N = NZ - 1, LH = NZ / 2;
-  const double* T = tab<NZ>();
-  double c[NZ];
+  const double* __restrict__ TE = tab<NZ>() + Tab<NZ>::SE;
+  const double* __restrict__ TO = tab<NZ>() + Tab<NZ>::SO;
+  double ce[LH], co[LH];
 #pragma unroll
-  for (int n = 0; n < NZ; ++n) c[n] = v[n * TM];
+  for (int j = 0; j < LH; ++j) { ce[j] = v[(2 * j) * LN]; co[j] = v[(2 * j + 1) * LN]; }
 #pragma unroll
   for (int l = 0; l < LH; ++l) {
     double E = 0.0, O = 0.0;
 #pragma unroll
     for (int j = 0; j < LH; ++j) {
-      E = fma(T[Tab<NZ>::CT + (2 * j) * LH + l], c[2 * j], E);
-      O = fma(T[Tab<NZ>::CT + (2 * j + 1) * LH + l], c[2 * j + 1], O);
+      E = fma(TE[l * LH + j], ce[j], E);
+      O = fma(TO[l * LH + j], co[j], O);
     }
-    v[l * TM] = E + O;
-    v[(N - l) * TM] = E - O;
+    v[l * LN] = E + O;
+    v[(N - l) * LN] = E - O;
   }
 }
 
-// ---- coefficient-space z-derivative, one output parity, top-down recurrence
-//   d_N = 0, d_n = d_{n+2} + 2(n+1) g_{n+1},  (D g)_n = (2/H) d_n (d_0 halved)
-//   dst[n] = scale * (D src)_n (+ dst[n] if ACC)
-template <int NZ, bool ACC> __device__ __forceinline__ void deriv_sweep(const double* src, double* dst, int par, double inv_s, double scale) {
+// ---- coefficient-space z-derivative of a lane's column (both parities), top-down recurrence
+//   d_N = 0, d_n = d_{n+2} + 2(n+1) g_{n+1},  (D g)_n = (2/H) d_n (d_0 halved);  dst[n] (+)= scale * (D src)_n
+template <int NZ, bool ACC> __device__ __forceinline__ void deriv_column(const double* __restrict__ src, double* __restrict__ dst, double inv_s, double scale) {
   constexpr int N = NZ - 1;
-  double d = 0.0;
-  const int ntop = ((N - par) & 1) ? N - 1 : N;       // largest n <= N with parity par
+  double g[NZ];
 #pragma unroll
-  for (int i = 0; i < NZ / 2; ++i) {
-    const int n = ntop - 2 * i;
-    if (n < 0) break;
-    if (n + 1 <= N) d = fma(2.0 * (n + 1), src[(n + 1) * TM], d);
-    const double val = d * inv_s * (n == 0 ? 0.5 : 1.0) * scale;
-    if (ACC) dst[n * TM] += val; else dst[n * TM] = val;
+  for (int n = 1; n <= N; ++n) g[n] = src[n * LN];
+  double d0 = 0.0, d1 = 0.0;          // running sums of the two parities
+  const double f = inv_s * scale;
+#pragma unroll
+  for (int n = N; n >= 0; --n) {
+    double& d = (n & 1) ? d1 : d0;
+    if (n + 1 <= N) d = fma(2.0 * (n + 1), g[n + 1], d);
+    const double val = d * (n == 0 ? 0.5 * f : f);
+    if (ACC) dst[n * LN] += val; else dst[n * LN] = val;
   }
 }
 
-// ---- one chain of one BVP: forward elimination, back substitution with the boundary functional, border unknown,
-//      double integration.  rho lives in col[n*TM] (own-parity slots, n <= N-2) and is overwritten by y's coefficients c_n.
-//      If dcol != nullptr the first-integral coefficients b_n / s (= d y/dz) of the OTHER parity are stored there.
-//      Returns S_c = sum of c_n over the chain (incl. c_0 for the even chain).
-template <int NZ>
-__device__ __forceinline__ double chain_solve(double* col, double* dcol, const double* mult, const double* invd, const double* ag,
-                                              int par, double k, double k2, double inv_s, double beta_bc, double Bg) {
-  constexpr int N = NZ - 1;
-  const double* T = tab<NZ>();
-  const int n0 = par ? 1 : 2;                    // first tridiagonal row
-  const int nrows = par ? (N - 1) / 2 : (N - 2) / 2;   // rows n0, n0+2, ... <= N-2
-  // forward elimination (rho'_j = rho_j - m_j rho'_{j-1}); even chain: row 2 carries (kappa^2/4) rho_0
-  double prev = 0.0;
+// ---- chain geometry: rows n0, n0+2, ... <= N-2 of parity PAR
+template <int NZ, int PAR> struct Ch {
+  static constexpr int N = NZ - 1, n0 = PAR ? 1 : 2, NR = PAR ? (N - 1) / 2 : (N - 2) / 2;
+};
+
+// ---- factorisation of one chain and its homogeneous ("border") solution, per mode (depends on |k| only):
+//   Fm[n] = Thomas multiplier, Fi[n] = inverse pivot, Fa[n] = a_n of the solution with unit border unknown,
+//   returns 1/B_g, B_g = boundary functional of that solution.
+template <int NZ, int PAR>
+__device__ __forceinline__ double factor_chain(double* __restrict__ Fm, double* __restrict__ Fi, double* __restrict__ Fa, double k, double k2,
+                                               double inv_s, bool store) {
+  constexpr int n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR;
+  const double* __restrict__ T = tab<NZ>();
+  double invd[NR], ag[NR];
+  double g = PAR ? k2 : 0.25 * k2 * k2;
 #pragma unroll
-  for (int j = 0; j < NZ / 2; ++j) {
+  for (int j = 0; j < NR; ++j) {
     const int n = n0 + 2 * j;
-    if (j >= nrows) break;
-    double r = col[n * TM];
-    if (j == 0) { if (!par) r = fma(0.25 * k2, col[0], r); }
-    else r = fma(-mult[n * TM], prev, r);
-    col[n * TM] = r;
-    prev = r;
+    double d = row_d<NZ>(n, k2);
+    if (j > 0) {
+      const double mu = row_l<NZ>(n, k2) * invd[j - 1];
+      d = fma(-mu, row_u<NZ>(n - 2, k2), d);
+      if (store) Fm[n * TM] = mu;
+      g = -mu * g;
+    }
+    invd[j] = 1.0 / d;
+    ag[j] = g;
   }
-  // back substitution a_j = (rho'_j - u_j a_{j+1}) / d'_j, accumulating B = (1/s) sum P_n a_n + k sum Q_n a_n
   double SP = 0.0, SQ = 0.0, next = 0.0;
 #pragma unroll
-  for (int j = NZ / 2 - 1; j >= 0; --j) {
+  for (int j = NR - 1; j >= 0; --j) {
     const int n = n0 + 2 * j;
-    if (j >= nrows) continue;
-    double a = (col[n * TM] - row_u<NZ>(n, k2) * next) * invd[n * TM];
-    col[n * TM] = a;
+    const double a = (ag[j] - row_u<NZ>(n, k2) * next) * invd[j];
     next = a;
-    SP = fma(T[Tab<NZ>::P + n], a, SP);
-    SQ = fma(T[Tab<NZ>::Q + n], a, SQ);
+    if (store) { Fa[n * TM] = a; Fi[n * TM] = invd[j]; }
+    SP = fma(T[Tab<NZ>::P + n], a, SP); SQ = fma(T[Tab<NZ>::Q + n], a, SQ);
   }
-  if (!par) { const double a0 = col[0]; SP = fma(T[Tab<NZ>::P + 0], a0, SP); SQ = fma(T[Tab<NZ>::Q + 0], a0, SQ); }
-  const double border = (beta_bc - (inv_s * SP + k * SQ)) / Bg;      // c_0 (even chain) or b_0 (odd chain)
-  // integrate a = a^rho + border a^g twice:  b_{n+1} = (cbar_n a_n - a_{n+2}) / (2(n+1)),  c_n = (cbar_{n-1} b_{n-1} - b_{n+1}) / (2n)
-  double Sc = 0.0, bprev;
-  double an = fma(border, ag[par * TM], col[par * TM]);   // a_0 (even) or a_1 (odd)
-  if (!par) { col[0] = border; Sc = border; bprev = 0.0; }
-  else { if (dcol) dcol[0] = border * inv_s; bprev = border; }
+  double Bg;
+  if (!PAR) {                                                // a_0 = rho_0 + kappa^2 c_0 ; c_0 = 1 also enters sum c_n directly
+    SP = fma(T[Tab<NZ>::P + 0], k2, SP); SQ = fma(T[Tab<NZ>::Q + 0], k2, SQ);
+    Bg = inv_s * SP + k * (1.0 + SQ);
+  } else {                                                   // b_0 = 1 enters sum b_n and c_1
+    Bg = inv_s * (1.0 + SP) + k * (1.0 + SQ);
+  }
+  return 1.0 / Bg;
+}
+
+// ---- one chain of one BVP for a lane: forward elimination, back substitution with the boundary functional, border
+//      unknown, double integration.  a[j] = (H/2)^2 r_n of row n = n0+2j on entry, rho0 = (H/2)^2 r_0 (even chain).
+//      Writes y's coefficients c_n of parity PAR to col and, if WITH_D, the coefficients of dy/dz of the OTHER parity to
+//      dcol.  Returns S_c = sum of the c_n written (incl. c_0 for the even chain).
+template <int NZ, int PAR, bool WITH_D>
+__device__ __forceinline__ double chain(double (&a)[Ch<NZ, PAR>::NR], double rho0, const double* __restrict__ Fm, const double* __restrict__ Fi,
+                                        const double* __restrict__ Fa, double* __restrict__ col, double* __restrict__ dcol, double k,
+                                        double k2, double inv_s, double beta_bc, double invBg) {
+  constexpr int N = NZ - 1, n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR;
+  const double* __restrict__ T = tab<NZ>();
+  double mult[NR], invd[NR], ag[NR];
 #pragma unroll
-  for (int i = 0; i < NZ / 2 + 1; ++i) {
-    const int n = par + 2 * i;
-    if (n > N) break;
-    double ap = 0.0;
-    if (n + 2 <= N - 2) ap = fma(border, ag[(n + 2) * TM], col[(n + 2) * TM]);
-    const double bn1 = ((n == 0 ? 2.0 : 1.0) * an - ap) / (2.0 * (n + 1));
+  for (int j = 0; j < NR; ++j) {
+    const int n = n0 + 2 * j;
+    mult[j] = j > 0 ? Fm[n * TM] : 0.0; invd[j] = Fi[n * TM]; ag[j] = Fa[n * TM];
+  }
+  if (!PAR) a[0] = fma(0.25 * k2, rho0, a[0]);               // even chain: row 2 carries (kappa^2/4) rho_0
+#pragma unroll
+  for (int j = 1; j < NR; ++j) a[j] = fma(-mult[j], a[j - 1], a[j]);
+  double SP = 0.0, SQ = 0.0, next = 0.0;
+#pragma unroll
+  for (int j = NR - 1; j >= 0; --j) {
+    const int n = n0 + 2 * j;
+    const double v = (a[j] - row_u<NZ>(n, k2) * next) * invd[j];
+    a[j] = v; next = v;
+    SP = fma(T[Tab<NZ>::P + n], v, SP); SQ = fma(T[Tab<NZ>::Q + n], v, SQ);
+  }
+  if (!PAR) { SP = fma(T[Tab<NZ>::P + 0], rho0, SP); SQ = fma(T[Tab<NZ>::Q + 0], rho0, SQ); }
+  const double border = (beta_bc - (inv_s * SP + k * SQ)) * invBg;       // c_0 (even chain) or b_0 (odd chain)
+#pragma unroll
+  for (int j = 0; j < NR; ++j) a[j] = fma(border, ag[j], a[j]);
+  // integrate twice:  b_{n+1} = (cbar_n a_n - a_{n+2}) / (2(n+1)),  c_n = (cbar_{n-1} b_{n-1} - b_{n+1}) / (2n)
+  double Sc = 0.0, bprev;
+  if (!PAR) { col[0] = border; Sc = border; bprev = 0.0; }
+  else { bprev = border; if (WITH_D) dcol[0] = border * inv_s; }
+#pragma unroll
+  for (int i = 0; i <= (N - PAR) / 2; ++i) {
+    const int n = PAR + 2 * i;
+    // a_n of parity PAR: n = 0 -> rho0 + border kappa^2 (even); n = n0 + 2j -> a[j]; n > N-2 -> 0
+    double an = 0.0, ap = 0.0;
+    if (n <= N - 2) an = (!PAR && n == 0) ? fma(border, k2, rho0) : a[n >= n0 ? (n - n0) / 2 : 0];
+    if (n + 2 <= N - 2) ap = a[(n + 2 - n0) / 2];
+    const double bn1 = ((n == 0 ? 2.0 : 1.0) * an - ap) * (1.0 / (2.0 * (n + 1)));
     if (n >= 1) {
-      const double c = ((n == 1 ? 2.0 : 1.0) * bprev - bn1) / (2.0 * n);
-      col[n * TM] = c;
+      const double c = ((n == 1 ? 2.0 : 1.0) * bprev - bn1) * (1.0 / (2.0 * n));
+      col[n * LN] = c;
       Sc += c;
     }
-    if (dcol && n + 1 <= N - 1) dcol[(n + 1) * TM] = bn1 * inv_s;
+    if (WITH_D && n + 1 <= N - 1) dcol[(n + 1) * LN] = bn1 * inv_s;
     bprev = bn1;
-    an = ap;
   }
-  if (dcol) { if (((N - par) & 1) == 1) dcol[N * TM] = 0.0; }   // (D y)_N = 0: slot N belongs to the chain whose b's have N's parity
+  if (WITH_D && ((N - PAR) & 1) == 1) dcol[N * LN] = 0.0;    // (D y)_N = 0: slot N belongs to the chain whose b's have N's parity
   return Sc;
 }
 
-// ---- 4x4 real system with two right-hand sides (real and imaginary part), partial pivoting after row equilibration
-__device__ void solve4(double M[4][4], double br[4], double bi[4]) {
+// ---- 4x4 real system, one right-hand side per lane, partial pivoting after row equilibration
+__device__ __forceinline__ void solve4(double M[4][4], double b[4]) {
+#pragma unroll
   for (int r = 0; r < 4; ++r) {
-    double mx = fmax(fmax(fabs(M[r][0]), fabs(M[r][1])), fmax(fabs(M[r][2]), fabs(M[r][3])));
-    double s = mx > 0.0 ? 1.0 / mx : 1.0;
+    const double mx = fmax(fmax(fabs(M[r][0]), fabs(M[r][1])), fmax(fabs(M[r][2]), fabs(M[r][3])));
+    const double s = mx > 0.0 ? 1.0 / mx : 1.0;
+#pragma unroll
     for (int c = 0; c < 4; ++c) M[r][c] *= s;
-    br[r] *= s; bi[r] *= s;
+    b[r] *= s;
   }
+#pragma unroll
   for (int c = 0; c < 4; ++c) {
-    int p = c; double best = fabs(M[c][c]);
-    for (int r = c + 1; r < 4; ++r) if (fabs(M[r][c]) > best) { best = fabs(M[r][c]); p = r; }
-    if (p != c) {
-      for (int q = 0; q < 4; ++q) { double t = M[c][q]; M[c][q] = M[p][q]; M[p][q] = t; }
-      double t = br[c]; br[c] = br[p]; br[p] = t; t = bi[c]; bi[c] = bi[p]; bi[p] = t;
+#pragma unroll
+    for (int r = c + 1; r < 4; ++r) {                       // bubble the largest pivot candidate into row c
+      if (fabs(M[r][c]) > fabs(M[c][c])) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) { const double t = M[c][q]; M[c][q] = M[r][q]; M[r][q] = t; }
+        const double t = b[c]; b[c] = b[r]; b[r] = t;
+      }
     }
+    const double ip = 1.0 / M[c][c];
+#pragma unroll
     for (int r = c + 1; r < 4; ++r) {
-      double f = M[r][c] / M[c][c];
-      for (int q = c; q < 4; ++q) M[r][q] -= f * M[c][q];
-      br[r] -= f * br[c]; bi[r] -= f * bi[c];
+      const double f = M[r][c] * ip;
+#pragma unroll
+      for (int q = c; q < 4; ++q) M[r][q] = fma(-f, M[c][q], M[r][q]);
+      b[r] = fma(-f, b[c], b[r]);
     }
+    M[c][c] = ip;                                            // keep the inverse pivot
   }
+#pragma unroll
   for (int r = 3; r >= 0; --r) {
-    double sr = br[r], si = bi[r];
-    for (int q = r + 1; q < 4; ++q) { sr -= M[r][q] * br[q]; si -= M[r][q] * bi[q]; }
-    br[r] = sr / M[r][r]; bi[r] = si / M[r][r];
+    double s = b[r];
+#pragma unroll
+    for (int q = r + 1; q < 4; ++q) s = fma(-M[r][q], b[q], s);
+    b[r] = s * M[r][r];
   }
 }
 
+// per-lane constants of a mode
+struct ModeK {
+  double k, k2, kxt, kyt, sgI;       // |k|, (k H/2)^2, derivative multipliers (0 on the unpaired Nyquist index), sign of Re/Im(i z)
+};
+
+// ---- pressure item (eqs 15, 17): right-hand side i k.f + dz f_z, chain PAR; p -> C3, dp/dz -> C4
+template <int NZ, int PAR>
+__device__ __forceinline__ double pressure_item(double* __restrict__ C, const double* __restrict__ F, int lane, int mode, const ModeK& K, double s,
+                                                double inv_s, double invBg) {
+  constexpr int N = NZ - 1, n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR, VS = NZ * LN;
+  const double* fxo = C + 0 * VS + (lane ^ 1);          // the OTHER part of f_x, f_y: i k f mixes re and im
+  const double* fyo = C + 1 * VS + (lane ^ 1);
+  const double* fz = C + 2 * VS + lane;
+  double a[NR], rho0 = 0.0;
+  double d = 0.0;
+  constexpr int ntop = ((N - PAR) & 1) ? N - 1 : N;     // largest n <= N with parity PAR
+  const double s2 = s * s;
+#pragma unroll
+  for (int i = 0; i <= ntop / 2; ++i) {
+    const int n = ntop - 2 * i;
+    if (n < 0) break;
+    if (n + 1 <= N) d = fma(2.0 * (n + 1), fz[(n + 1) * LN], d);
+    if (n <= N - 2) {
+      const double r = fma(K.sgI, fma(K.kxt, fxo[n * LN], K.kyt * fyo[n * LN]), d * (n == 0 ? 0.5 * inv_s : inv_s)) * s2;
+      if (n >= n0) a[(n - n0) / 2] = r; else rho0 = r;
+    }
+  }
+  return chain<NZ, PAR, true>(a, rho0, F + 0 * NZ * TM + mode, F + 1 * NZ * TM + mode, F + 2 * NZ * TM + mode, C + 3 * VS + lane, C + 4 * VS + lane,
+                              K.k, K.k2, inv_s, 0.0, invBg);
+}
+
+// ---- velocity item (eq 18 with BCs 22, 24): component COMP, chain PAR; f_c (column COMP) is overwritten by u_c
+template <int NZ, int PAR>
+__device__ __forceinline__ double velocity_item(int comp, double* __restrict__ C, const double* __restrict__ F, int lane, int mode, const ModeK& K,
+                                                double s, double inv_s, double eta, double invBg, double pH_own, double p0_own, double pH_oth,
+                                                double p0_oth) {
+  constexpr int N = NZ - 1, n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR, VS = NZ * LN;
+  double* col = C + comp * VS + lane;
+  double a[NR], rho0 = 0.0, gH, g0;
+  const double sc = s * s / eta;
+  if (comp < 2) {
+    const double kc = comp == 0 ? K.kxt : K.kyt;
+    const double* po = C + 3 * VS + (lane ^ 1);          // other part of p
+    const double f = K.sgI * kc;
+#pragma unroll
+    for (int i = 0; i <= (N - 2 - PAR) / 2; ++i) {
+      const int n = PAR + 2 * i;
+      const double r = (f * po[n * LN] - col[n * LN]) * sc;       // r = (i k_c p - f_c)/eta
+      if (n >= n0) a[(n - n0) / 2] = r; else rho0 = r;
+    }
+    // (dz + k) u(H) = -(i k_c/(2 k eta)) p(H) ; (dz - k) u(0) = +(i k_c/(2 k eta)) p(0)      (eq 22)
+    const double c = kc / (2.0 * K.k * eta);
+    gH = -K.sgI * c * pH_oth;
+    g0 = K.sgI * c * p0_oth;
+  } else {
+    const double* dp = C + 4 * VS + lane;
+#pragma unroll
+    for (int i = 0; i <= (N - 2 - PAR) / 2; ++i) {
+      const int n = PAR + 2 * i;
+      const double r = (dp[n * LN] - col[n * LN]) * sc;            // r = (dz p - f_z)/eta
+      if (n >= n0) a[(n - n0) / 2] = r; else rho0 = r;
+    }
+    // (dz + k) w(H) = p(H)/(2 eta) ; (dz - k) w(0) = p(0)/(2 eta)                              (eq 24)
+    gH = pH_own / (2.0 * eta);
+    g0 = p0_own / (2.0 * eta);
+  }
+  const double beta_bc = PAR ? 0.5 * (gH + g0) : 0.5 * (gH - g0);
+  return chain<NZ, PAR, false>(a, rho0, F + 0 * NZ * TM + mode, F + 1 * NZ * TM + mode, F + 2 * NZ * TM + mode, col, nullptr, K.k, K.k2, inv_s,
+                               beta_bc, invBg);
+}
+
+// ---- wall correction coefficients of a lane (own part), basis: 0 = z e^{-kz}, 1 = e^{-kz}, 2 = z e^{-k(H-z)}, 3 = e^{-k(H-z)}
+//   wall data (eq 27 / (A3) with no slip, u_wall = 0): u_0 = -u_DP(z=0) = -(S_even - S_odd), u_H = -u_DP(z=H) = -(S_even + S_odd)
+__device__ __forceinline__ void correction_coefficients(const double* __restrict__ s_sum, int lane, const ModeK& K, double H, int wall_mode,
+                                                        double cf[3][4]) {
+  double u0[3], uH[3], u0o[3], uHo[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const double se = s_sum[((1 + c) * 2 + 0) * LN + lane], so = s_sum[((1 + c) * 2 + 1) * LN + lane];
+    u0[c] = -(se - so); uH[c] = -(se + so);
+    u0o[c] = __shfl_xor_sync(0xffffffffu, u0[c], 1); uHo[c] = __shfl_xor_sync(0xffffffffu, uH[c], 1);
+  }
+  const double k = K.k, kxt = K.kxt, kyt = K.kyt, sgI = K.sgI;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { cf[c][0] = cf[c][1] = cf[c][2] = cf[c][3] = 0.0; }
+  if (wall_mode == DP_BOTTOM_WALL) {
+    // eqs 42-44: Q = i k w0 + kx u0 + ky v0 ; Wc = k w0 - i kx u0 - i ky v0
+    const double Q = fma(sgI * k, u0o[2], fma(kxt, u0[0], kyt * u0[1]));
+    const double Wc = fma(k, u0[2], -sgI * fma(kxt, u0o[0], kyt * u0o[1]));
+    const double ik = 1.0 / k;
+    cf[0][0] = -(kxt * ik) * Q; cf[1][0] = -(kyt * ik) * Q; cf[2][0] = Wc;
+    cf[0][1] = u0[0]; cf[1][1] = u0[1]; cf[2][1] = u0[2];
+  } else {
+    // App. A, no slip.  Unknowns [C0', D0', Cz, Dz] with C0' = C0/(2 eta), D0' = D0 e^{kH}/(2 eta) (basis e^{-k(H-z)}):
+    // (A8b), (A8d), (A10a), (A10b) after eliminating Cx+e Dx, e Cx+Dx (and y) with (A8a), (A8c); e = e^{-kH}.
+    const double e = exp(-k * H), ik = 1.0 / k;
+    const double g = (kxt * kxt + kyt * kyt) * H * ik;
+    double M[4][4] = {{0.0, 0.0, 1.0, e}, {H * e, H, e, 1.0}, {1.0, e, -k, k * e}, {e * (1.0 - g), 1.0 + g, -k * e, k}};
+    // right-hand sides: [w0, wH, -i(kx u0 + ky v0), -i(kx uH + ky vH)]  ->  own part of -i z = -sgI * other part of z
+    double b[4] = {u0[2], uH[2], -sgI * fma(kxt, u0o[0], kyt * u0o[1]), -sgI * fma(kxt, uHo[0], kyt * uHo[1])};
+    solve4(M, b);
+    const double C0 = b[0], D0 = b[1];
+    const double C0o = __shfl_xor_sync(0xffffffffu, C0, 1), D0o = __shfl_xor_sync(0xffffffffu, D0, 1);
+    const double iom = 1.0 / (-expm1(-k * H) * (1.0 + e));       // 1/(1 - e^2)
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const double kc = c == 0 ? kxt : kyt, q = kc * H * ik;
+      // C_c + e D_c = u0 ; e C_c + D_c = uH + i q (e C0' - D0')
+      const double r2 = fma(sgI * q, e * C0o - D0o, uH[c]);
+      cf[c][1] = (u0[c] - e * r2) * iom;
+      cf[c][3] = (r2 - e * u0[c]) * iom;
+      // (A5): -i (k_c/k) C0' z e^{-kz} + i (k_c/k) D0' z e^{-k(H-z)}
+      cf[c][0] = -sgI * (kc * ik) * C0o;
+      cf[c][2] = sgI * (kc * ik) * D0o;
+    }
+    // (A6): C0' z e^{-kz} + D0' z e^{-k(H-z)} + Cz e^{-kz} + Dz e^{-k(H-z)}
+    cf[2][0] = C0; cf[2][2] = D0; cf[2][1] = b[2]; cf[2][3] = b[3];
+  }
+}
+
+template <int NZ> struct SolveSmem {
+  static constexpr int VS = NZ * LN;                                   // one complex column [n][lane]
+  static constexpr int COLS = 6 * VS;                                  // C0..C5
+  static constexpr int FACT = COLS;                                    // [3][NZ][TM]: multipliers, inverse pivots, border solution
+  static constexpr int IBG = FACT + 3 * NZ * TM;                       // [2][TM] 1/B_g of the even / odd chain
+  static constexpr int SUM = IBG + 2 * TM;                             // [4][2][LN] S_c of (p,u,v,w) x (even, odd chain)
+  static constexpr int CORR = SUM + 8 * LN;                            // [12][LN] correction coefficients (slit)
+  static constexpr int DOUBLES = CORR + 12 * LN;
+};
+
 template <int NZ>
-__global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 2 : 1)) k_solve(SolveArgs A) {
+__global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(SolveArgs A) {
   extern __shared__ double smem[];
-  constexpr int N = NZ - 1, LH = NZ / 2, VS = NZ * TM;
-#define VEC(i) (smem + (size_t)(i) * VS)
-  // vectors: 0..9 = five complex columns C0..C4 (re, im); 10 = Thomas multipliers, 11 = inverse pivots, 12 = a^g
-  double* s_Bg = smem + (size_t)NVEC * VS;     // [2][TM]
-  double* s_sum = s_Bg + 2 * TM;               // [4][2][2][TM]  S_c of (p,u,v,w) x (re,im) x (even,odd chain)
-  double* s_corr = VEC(10);                    // [3][4][2][TM] correction coefficients (phases 6-7; factors are dead by then)
+  constexpr int N = NZ - 1, VS = NZ * LN;
+  typedef SolveSmem<NZ> S;
+  double* C = smem;                      // columns: 0 f_x->u, 1 f_y->v, 2 f_z->w, 3 t_x->p->dz u, 4 t_y->dz p->dz v, 5 (E, zE)
+  double* F = smem + S::FACT;
+  double* s_ibg = smem + S::IBG;
+  double* s_sum = smem + S::SUM;
+  double* s_corr = smem + S::CORR;
   const double* T = tab<NZ>();
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const int iy = blockIdx.y, ix = blockIdx.x * TM + lane;
-  const bool valid = ix < A.nkx;
+  const int mode = lane >> 1, part = lane & 1;
+  const int ifast = blockIdx.x * TM + mode, islow = blockIdx.y;
+  const int ix = A.fast_is_x ? ifast : islow, iy = A.fast_is_x ? islow : ifast;
+  const bool valid = ifast < A.n_fast;
   const bool zero_mode = (ix == 0 && iy == 0);
   const double s = 0.5 * A.H, inv_s = 1.0 / s, eta = A.eta;
-  double kx = 0.0, ky = 0.0, k = 1.0, kxt = 0.0, kyt = 0.0;
+  ModeK K;
+  K.k = 1.0; K.kxt = 0.0; K.kyt = 0.0; K.sgI = part ? 1.0 : -1.0;
   if (valid && !zero_mode) {
     const int nyq = (iy <= A.ny / 2) ? iy : iy - A.ny;
-    kx = 2.0 * M_PI * ix / A.Lx; ky = 2.0 * M_PI * nyq / A.Ly;
-    k = sqrt(kx * kx + ky * ky);                           // magnitude: always the full values (reading G5)
-    kxt = (ix == A.nx / 2) ? 0.0 : kx;                     // component multipliers vanish on the unpaired Nyquist index
-    kyt = (iy == A.ny / 2) ? 0.0 : ky;
+    const double kx = 2.0 * M_PI * ix / A.Lx, ky = 2.0 * M_PI * nyq / A.Ly;
+    K.k = sqrt(kx * kx + ky * ky);                         // magnitude: always the full values (reading G5)
+    K.kxt = (ix == A.nx / 2) ? 0.0 : kx;                   // component multipliers vanish on the unpaired Nyquist index
+    K.kyt = (iy == A.ny / 2) ? 0.0 : ky;
   }
-  const double k2 = (k * s) * (k * s);
-  const int m = lane;
+  K.k2 = (K.k * s) * (K.k * s);
+  const size_t plane = (size_t)A.n_slow * A.pitch;
+  const size_t off0 = (size_t)islow * A.pitch + ifast;
+  const double* gin = reinterpret_cast<const double*>(A.cplx);
 
   // ---------------- phase 0: load the nodal columns, fold the algebraic part of (1/2) curl t into f (eq 7)
-  for (int l = wid; l < NZ; l += NWARPS) {
-    double2 f[3] = {{0, 0}, {0, 0}, {0, 0}}, t[3] = {{0, 0}, {0, 0}, {0, 0}};
+  for (int l = wid; l < NZ; l += SOLVE_WARPS) {
+    double f[3] = {0, 0, 0}, t[3] = {0, 0, 0};
     if (valid) {
-      const size_t off = ((size_t)l * A.ny + iy) * A.nkxp + ix;
+      const size_t o = 2 * (l * plane + off0) + part;
 #pragma unroll
-      for (int c = 0; c < 3; ++c) f[c] = A.cplx[c * A.cplx_field + off];
+      for (int c = 0; c < 3; ++c) f[c] = gin[2 * (c * A.cplx_field) + o];
       if (A.torque) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) t[c] = A.cplx[(3 + c) * A.cplx_field + off];
+        for (int c = 0; c < 3; ++c) t[c] = gin[2 * ((3 + c) * A.cplx_field) + o];
       }
     }
-    const int o = l * TM + m;
-    VEC(0)[o] = f[0].x - 0.5 * kyt * t[2].y;  VEC(1)[o] = f[0].y + 0.5 * kyt * t[2].x;
-    VEC(2)[o] = f[1].x + 0.5 * kxt * t[2].y;  VEC(3)[o] = f[1].y - 0.5 * kxt * t[2].x;
-    VEC(4)[o] = f[2].x - 0.5 * (kxt * t[1].y - kyt * t[0].y);
-    VEC(5)[o] = f[2].y + 0.5 * (kxt * t[1].x - kyt * t[0].x);
-    VEC(6)[o] = t[0].x; VEC(7)[o] = t[0].y; VEC(8)[o] = t[1].x; VEC(9)[o] = t[1].y;
+    const int o = l * LN + lane;
+    if (A.torque) {
+      const double t0o = __shfl_xor_sync(0xffffffffu, t[0], 1), t1o = __shfl_xor_sync(0xffffffffu, t[1], 1), t2o = __shfl_xor_sync(0xffffffffu, t[2], 1);
+      f[0] = fma(0.5 * K.sgI * K.kyt, t2o, f[0]);                       // f_x += (1/2) i k_y t_z
+      f[1] = fma(-0.5 * K.sgI * K.kxt, t2o, f[1]);                      // f_y -= (1/2) i k_x t_z
+      f[2] = fma(0.5 * K.sgI, K.kxt * t1o - K.kyt * t0o, f[2]);         // f_z += (1/2) i (k_x t_y - k_y t_x)
+      C[3 * VS + o] = t[0]; C[4 * VS + o] = t[1];
+    }
+    C[0 * VS + o] = f[0]; C[1 * VS + o] = f[1]; C[2 * VS + o] = f[2];
   }
   __syncthreads();
 
-  // ---------------- phase 1: Chebyshev analysis of the 3 (or 5) complex columns; item = (real vector, output parity)
+  // ---------------- phase 1: Chebyshev analysis of the 3 (or 5) columns, one warp per column; warp 5: chain factorisation
+  if (wid < (A.torque ? 5 : 3)) {
+    analysis_column<NZ>(C + wid * VS + lane);
+  } else if (wid == 5) {
+    const bool store = part == 0;
+    const double i0 = factor_chain<NZ, 0>(F + mode, F + NZ * TM + mode, F + 2 * NZ * TM + mode, K.k, K.k2, inv_s, store);
+    const double i1 = factor_chain<NZ, 1>(F + mode, F + NZ * TM + mode, F + 2 * NZ * TM + mode, K.k, K.k2, inv_s, store);
+    if (store) { s_ibg[mode] = i0; s_ibg[TM + mode] = i1; }
+  }
+  __syncthreads();
+
+  // ---------------- phase 2: f_x -= (1/2) D t_y, f_y += (1/2) D t_x (eq 7); warps 2-5: e^{-k z_l} and z_l e^{-k z_l} at the nodes -> C5
+  if (wid < 2) {
+    if (A.torque) deriv_column<NZ, true>(C + (wid == 0 ? 4 : 3) * VS + lane, C + wid * VS + lane, inv_s, wid == 0 ? -0.5 : 0.5);
+  } else {
+    for (int l = wid - 2; l < NZ; l += SOLVE_WARPS - 2) {
+      const double zl = s * (1.0 + T[Tab<NZ>::XI + l]);
+      const double E = exp(-K.k * zl);
+      C[5 * VS + l * LN + lane] = part ? zl * E : E;
+    }
+  }
+  __syncthreads();
+
+  // ---------------- phase 3: pressure BVP (eqs 15, 17), one warp per chain; warp 2: Chebyshev coefficients of (E, zE) (step 6)
+  if (wid == 0) s_sum[(0 * 2 + 0) * LN + lane] = pressure_item<NZ, 0>(C, F, lane, mode, K, s, inv_s, s_ibg[mode]);
+  else if (wid == 1) s_sum[(0 * 2 + 1) * LN + lane] = pressure_item<NZ, 1>(C, F, lane, mode, K, s, inv_s, s_ibg[TM + mode]);
+  else if (wid == 2) analysis_column<NZ>(C + 5 * VS + lane);
+  __syncthreads();
+
+  // ---------------- phase 4: velocity BVPs (eq 18) with BCs (22), (24); one warp per (component, chain)
   {
-    const int items = (A.torque ? 10 : 6) * 2;
-    for (int base = 0; base < items; base += NWARPS) {
-      const int item = base + wid;
-      const bool act = item < items;
-      double e[LH];
-      double* v = VEC(act ? item >> 1 : 0) + m;
-      if (act) analysis_load<NZ>(v, item & 1, e);
-      __syncthreads();
-      if (act) { if (item & 1) analysis_compute<NZ, 1>(v, e); else analysis_compute<NZ, 0>(v, e); }
-    }
+    const int comp = wid >> 1;
+    const double se = s_sum[0 * LN + lane], so = s_sum[1 * LN + lane];
+    const double pH = se + so, p0 = se - so;              // p(H) = sum p_n, p(0) = sum (-1)^n p_n  ("direct summation")
+    const double pHo = __shfl_xor_sync(0xffffffffu, pH, 1), p0o = __shfl_xor_sync(0xffffffffu, p0, 1);
+    double Sc;
+    if (wid & 1) Sc = velocity_item<NZ, 1>(comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[TM + mode], pH, p0, pHo, p0o);
+    else Sc = velocity_item<NZ, 0>(comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], pH, p0, pHo, p0o);
+    s_sum[((1 + comp) * 2 + (wid & 1)) * LN + lane] = Sc;
   }
   __syncthreads();
 
-  // ---------------- phase 2: chain factorisation + homogeneous solutions (2 items); D t_y, D t_x into f_x, f_y (8 items)
-  {
-    const int items = A.torque ? 10 : 2;
-    for (int item = wid; item < items; item += NWARPS) {
-      if (item < 2) {
-        const int par = item;
-        double* mult = VEC(10) + m; double* invd = VEC(11) + m; double* ag = VEC(12) + m;
-        const int n0 = par ? 1 : 2, nrows = par ? (N - 1) / 2 : (N - 2) / 2;
-        double dprev = 1.0, g = par ? k2 : 0.25 * k2 * k2;
+  // ---------------- phase 5: correction coefficients (bottom wall: every warp for itself; slit: warp 0, shared)
+  double cf[3][4];
+  if (A.wall_mode == DP_BOTTOM_WALL) {
+    correction_coefficients(s_sum, lane, K, A.H, DP_BOTTOM_WALL, cf);
+  } else {
+    if (wid == 0) {
+      correction_coefficients(s_sum, lane, K, A.H, DP_SLIT, cf);
 #pragma unroll
-        for (int j = 0; j < NZ / 2; ++j) {
-          const int n = n0 + 2 * j;
-          if (j >= nrows) break;
-          double d = row_d<NZ>(n, k2);
-          if (j > 0) {
-            const double mu = row_l<NZ>(n, k2) / dprev;
-            d = fma(-mu, row_u<NZ>(n - 2, k2), d);
-            mult[n * TM] = mu;
-            g = -mu * g;
-          }
-          invd[n * TM] = 1.0 / d;
-          ag[n * TM] = g;
-          dprev = d;
-        }
-        double SP = 0.0, SQ = 0.0, next = 0.0;
+      for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int j = NZ / 2 - 1; j >= 0; --j) {
-          const int n = n0 + 2 * j;
-          if (j >= nrows) continue;
-          const double a = (ag[n * TM] - row_u<NZ>(n, k2) * next) * invd[n * TM];
-          ag[n * TM] = a; next = a;
-          SP = fma(T[Tab<NZ>::P + n], a, SP); SQ = fma(T[Tab<NZ>::Q + n], a, SQ);
-        }
-        if (!par) {
-          ag[0] = k2;                                      // a_0 = rho_0 + kappa^2 c_0
-          SP = fma(T[Tab<NZ>::P + 0], k2, SP); SQ = fma(T[Tab<NZ>::Q + 0], k2, SQ);
-          s_Bg[m] = inv_s * SP + k * (1.0 + SQ);           // c_0 = 1 also enters sum c_n directly
-        } else {
-          s_Bg[TM + m] = inv_s * (1.0 + SP) + k * (1.0 + SQ);   // b_0 = 1 enters sum b_n and c_1
-        }
-      } else {
-        // f_x -= (1/2) D t_y ; f_y += (1/2) D t_x   (eq 7; the ik x t_z parts were folded in phase 0)
-        const int q = item - 2, col = 3 + (q >> 2), part = (q >> 1) & 1, par = q & 1;
-        const double* src = VEC(2 * col + part) + m;
-        double* dst = (col == 4 ? VEC(0 + part) : VEC(2 + part)) + m;
-        deriv_sweep<NZ, true>(src, dst, par, inv_s, col == 4 ? -0.5 : 0.5);
-      }
+        for (int b = 0; b < 4; ++b) s_corr[(c * 4 + b) * LN + lane] = cf[c][b];
     }
-  }
-  __syncthreads();
-
-  // ---------------- phases 3+4: pressure right-hand side (eq 15) and pressure BVP with BCs (17); item = (part, chain)
-  if (wid < 4) {
-    const int part = wid >> 1, par = wid & 1;
-    double* col = VEC(6 + part) + m;                      // C3 := p
-    double* dcol = VEC(8 + part) + m;                     // C4 := dp/dz
-    const double* fz = VEC(4 + part) + m;
-    const double* fxo = VEC(0 + (1 - part)) + m;          // the OTHER part of f_x, f_y: i k f mixes re and im
-    const double* fyo = VEC(2 + (1 - part)) + m;
-    const double sg = part ? 1.0 : -1.0;                  // Re(i k f) = -k Im f ; Im(i k f) = +k Re f
-    double d = 0.0;
-    const int ntop = ((N - par) & 1) ? N - 1 : N;
-#pragma unroll
-    for (int i = 0; i < NZ / 2; ++i) {
-      const int n = ntop - 2 * i;
-      if (n < 0) break;
-      if (n + 1 <= N) d = fma(2.0 * (n + 1), fz[(n + 1) * TM], d);
-      double r = 0.0;
-      if (n <= N - 2) r = sg * (kxt * fxo[n * TM] + kyt * fyo[n * TM]) + d * inv_s * (n == 0 ? 0.5 : 1.0);
-      col[n * TM] = r * s * s;
-    }
-    const double Sc = chain_solve<NZ>(col, dcol, VEC(10) + m, VEC(11) + m, VEC(12) + m, par, k, k2, inv_s, 0.0, s_Bg[par * TM + m]);
-    s_sum[((0 * 2 + part) * 2 + par) * TM + m] = Sc;
-  }
-  __syncthreads();
-
-  // ---------------- phase 5: velocity BVPs (eq 18) with BCs (22), (24); item = (component, part, chain)
-  for (int item = wid; item < 12; item += NWARPS) {
-    const int comp = item >> 2, part = (item >> 1) & 1, par = item & 1;
-    double* col = VEC(2 * comp + part) + m;               // f_c, overwritten by u_c
-    const double pH_re = s_sum[(0 * 2 + 0) * 2 * TM + m] + s_sum[((0 * 2 + 0) * 2 + 1) * TM + m];
-    const double p0_re = s_sum[(0 * 2 + 0) * 2 * TM + m] - s_sum[((0 * 2 + 0) * 2 + 1) * TM + m];
-    const double pH_im = s_sum[(0 * 2 + 1) * 2 * TM + m] + s_sum[((0 * 2 + 1) * 2 + 1) * TM + m];
-    const double p0_im = s_sum[(0 * 2 + 1) * 2 * TM + m] - s_sum[((0 * 2 + 1) * 2 + 1) * TM + m];
-    double gH, g0;
-    const int nlo = par ? 1 : 0;
-    if (comp < 2) {
-      const double kc = comp == 0 ? kxt : kyt;
-      const double* po = VEC(6 + (1 - part)) + m;         // other part of p
-      const double sg = part ? 1.0 : -1.0;
-#pragma unroll
-      for (int i = 0; i < NZ / 2; ++i) {
-        const int n = nlo + 2 * i;
-        if (n > N - 2) break;
-        col[n * TM] = (sg * kc * po[n * TM] - col[n * TM]) * (s * s / eta);     // r = (i k_c p - f_c)/eta
-      }
-      const double c = kc / (2.0 * k * eta);
-      // (dz + k) u(H) = -(i k_c/(2 k eta)) p(H) ; (dz - k) u(0) = +(i k_c/(2 k eta)) p(0)      (eq 22)
-      gH = part ? -c * pH_re : c * pH_im;
-      g0 = part ? c * p0_re : -c * p0_im;
-    } else {
-      const double* dp = VEC(8 + part) + m;
-#pragma unroll
-      for (int i = 0; i < NZ / 2; ++i) {
-        const int n = nlo + 2 * i;
-        if (n > N - 2) break;
-        col[n * TM] = (dp[n * TM] - col[n * TM]) * (s * s / eta);              // r = (dz p - f_z)/eta
-      }
-      // (dz + k) w(H) = p(H)/(2 eta) ; (dz - k) w(0) = p(0)/(2 eta)                              (eq 24)
-      gH = (part ? pH_im : pH_re) / (2.0 * eta);
-      g0 = (part ? p0_im : p0_re) / (2.0 * eta);
-    }
-    const double beta_bc = par ? 0.5 * (gH + g0) : 0.5 * (gH - g0);
-    const double Sc = chain_solve<NZ>(col, nullptr, VEC(10) + m, VEC(11) + m, VEC(12) + m, par, k, k2, inv_s, beta_bc, s_Bg[par * TM + m]);
-    s_sum[(((1 + comp) * 2 + part) * 2 + par) * TM + m] = Sc;
-  }
-  __syncthreads();
-
-  // ---------------- phase 6a: E_l = exp(-k z_l), z_l E_l at the nodes (C3); warp 0: correction coefficients
-  for (int l = wid; l < NZ; l += NWARPS) {
-    const double zl = s * (1.0 + T[Tab<NZ>::XI + l]);
-    const double E = exp(-k * zl);
-    VEC(6)[l * TM + m] = E;
-    VEC(7)[l * TM + m] = zl * E;
-  }
-  if (wid == 0) {
-    // wall data (eq 27 / (A3) with no slip, u_wall = 0): u_0 = -u_DP(z=0) = -(S_even - S_odd), u_H = -u_DP(z=H) = -(S_even + S_odd)
-    double u0r[3], u0i[3], uHr[3], uHi[3];
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-      const double er = s_sum[(((1 + c) * 2 + 0) * 2 + 0) * TM + m], orr = s_sum[(((1 + c) * 2 + 0) * 2 + 1) * TM + m];
-      const double ei = s_sum[(((1 + c) * 2 + 1) * 2 + 0) * TM + m], oi = s_sum[(((1 + c) * 2 + 1) * 2 + 1) * TM + m];
-      u0r[c] = -(er - orr); u0i[c] = -(ei - oi); uHr[c] = -(er + orr); uHi[c] = -(ei + oi);
-    }
-    // coefficient layout: s_corr[((c*4 + basis)*2 + part)*TM + m], basis: 0 = z e^{-kz}, 1 = e^{-kz}, 2 = z e^{-k(H-z)}, 3 = e^{-k(H-z)}
-    double cf[3][4][2];
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-      for (int b = 0; b < 4; ++b) { cf[c][b][0] = 0.0; cf[c][b][1] = 0.0; }
-    if (A.wall_mode == DP_BOTTOM_WALL) {
-      // eqs 42-44: Q = i k w0 + kx u0 + ky v0 ; Wc = k w0 - i kx u0 - i ky v0
-      const double Qr = -k * u0i[2] + kxt * u0r[0] + kyt * u0r[1], Qi = k * u0r[2] + kxt * u0i[0] + kyt * u0i[1];
-      const double Wr = k * u0r[2] + kxt * u0i[0] + kyt * u0i[1], Wi = k * u0i[2] - kxt * u0r[0] - kyt * u0r[1];
-      cf[0][0][0] = -(kxt / k) * Qr; cf[0][0][1] = -(kxt / k) * Qi;
-      cf[1][0][0] = -(kyt / k) * Qr; cf[1][0][1] = -(kyt / k) * Qi;
-      cf[2][0][0] = Wr; cf[2][0][1] = Wi;
-#pragma unroll
-      for (int c = 0; c < 3; ++c) { cf[c][1][0] = u0r[c]; cf[c][1][1] = u0i[c]; }
-    } else {
-      // App. A, no slip.  Unknowns [C0', D0', Cz, Dz] with C0' = C0/(2 eta), D0' = D0 e^{kH}/(2 eta) (basis e^{-k(H-z)}):
-      // (A8b), (A8d), (A10a), (A10b) after eliminating Cx+e Dx, e Cx+Dx (and y) with (A8a), (A8c); e = e^{-kH}.
-      const double e = exp(-k * A.H), H = A.H;
-      const double g = (kxt * kxt + kyt * kyt) * H / k;
-      double M[4][4] = {{0.0, 0.0, 1.0, e}, {H * e, H, e, 1.0}, {1.0, e, -k, k * e}, {e * (1.0 - g), 1.0 + g, -k * e, k}};
-      double br[4] = {u0r[2], uHr[2], kxt * u0i[0] + kyt * u0i[1], kxt * uHi[0] + kyt * uHi[1]};
-      double bi[4] = {u0i[2], uHi[2], -(kxt * u0r[0] + kyt * u0r[1]), -(kxt * uHr[0] + kyt * uHr[1])};
-      solve4(M, br, bi);
-      const double C0r = br[0], C0i = bi[0], D0r = br[1], D0i = bi[1];
-      const double om = -expm1(-k * H) * (1.0 + e);       // 1 - e^2
-#pragma unroll
-      for (int c = 0; c < 2; ++c) {
-        const double kc = c == 0 ? kxt : kyt, q = kc * H / k;
-        // C_c + e D_c = u0 ; e C_c + D_c = uH + i q (e C0' - D0')
-        const double r2r = uHr[c] - q * (e * C0i - D0i), r2i = uHi[c] + q * (e * C0r - D0r);
-        cf[c][1][0] = (u0r[c] - e * r2r) / om; cf[c][1][1] = (u0i[c] - e * r2i) / om;
-        cf[c][3][0] = (r2r - e * u0r[c]) / om; cf[c][3][1] = (r2i - e * u0i[c]) / om;
-        // (A5): -i (k_c/k) C0' z e^{-kz} + i (k_c/k) D0' z e^{-k(H-z)}
-        cf[c][0][0] = (kc / k) * C0i; cf[c][0][1] = -(kc / k) * C0r;
-        cf[c][2][0] = -(kc / k) * D0i; cf[c][2][1] = (kc / k) * D0r;
-      }
-      // (A6): C0' z e^{-kz} + D0' z e^{-k(H-z)} + Cz e^{-kz} + Dz e^{-k(H-z)}
-      cf[2][0][0] = C0r; cf[2][0][1] = C0i; cf[2][2][0] = D0r; cf[2][2][1] = D0i;
-      cf[2][1][0] = br[2]; cf[2][1][1] = bi[2]; cf[2][3][0] = br[3]; cf[2][3][1] = bi[3];
-    }
-#pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-      for (int b = 0; b < 4; ++b) { s_corr[((c * 4 + b) * 2 + 0) * TM + m] = cf[c][b][0]; s_corr[((c * 4 + b) * 2 + 1) * TM + m] = cf[c][b][1]; }
-  }
-  __syncthreads();
-
-  // ---------------- phase 6b: Chebyshev coefficients of E and zE (step 6)
-  {
-    double e[LH];
-    const bool act = wid < 4;
-    double* v = VEC(6 + (act ? wid >> 1 : 0)) + m;
-    if (act) analysis_load<NZ>(v, wid & 1, e);
     __syncthreads();
-    if (act) { if (wid & 1) analysis_compute<NZ, 1>(v, e); else analysis_compute<NZ, 0>(v, e); }
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int b = 0; b < 4; ++b) cf[c][b] = s_corr[(c * 4 + b) * LN + lane];
   }
-  __syncthreads();
 
-  // ---------------- phase 7: total coefficients = DP + correction;  T[z e^{-k(H-z)}]_n = (-1)^n (H e_n - ze_n), T[e^{-k(H-z)}]_n = (-1)^n e_n
-  for (int n = wid; n < NZ; n += NWARPS) {
-    const double en = VEC(6)[n * TM + m], zen = VEC(7)[n * TM + m];
+  // ---------------- phase 6: total coefficients = DP + correction;  T[z e^{-k(H-z)}]_n = (-1)^n (H e_n - ze_n), T[e^{-k(H-z)}]_n = (-1)^n e_n
+  for (int n = wid; n < NZ; n += SOLVE_WARPS) {
+    const double mine = C[5 * VS + n * LN + lane], other = C[5 * VS + n * LN + (lane ^ 1)];
+    const double en = part ? other : mine, zen = part ? mine : other;
     const double sgn = (n & 1) ? -1.0 : 1.0;
     const double b2 = sgn * (A.H * en - zen), b3 = sgn * en;
 #pragma unroll
-    for (int c = 0; c < 3; ++c)
-#pragma unroll
-      for (int part = 0; part < 2; ++part) {
-        double add = s_corr[((c * 4 + 0) * 2 + part) * TM + m] * zen + s_corr[((c * 4 + 1) * 2 + part) * TM + m] * en;
-        if (A.wall_mode == DP_SLIT) add += s_corr[((c * 4 + 2) * 2 + part) * TM + m] * b2 + s_corr[((c * 4 + 3) * 2 + part) * TM + m] * b3;
-        VEC(2 * c + part)[n * TM + m] += add;
-      }
+    for (int c = 0; c < 3; ++c) {
+      double add = fma(cf[c][0], zen, cf[c][1] * en);
+      if (A.wall_mode == DP_SLIT) add = fma(cf[c][2], b2, fma(cf[c][3], b3, add));
+      C[c * VS + n * LN + lane] += add;
+    }
   }
   __syncthreads();
 
-  // ---------------- phase 8: dz u, dz v of the TOTAL in coefficient space (reading G12) -> C3, C4
+  // ---------------- phase 7: dz u, dz v of the TOTAL in coefficient space (reading G12) -> C3, C4; synthesis back to the nodes
   if (A.omega) {
-    const int comp = wid >> 2, part = (wid >> 1) & 1, par = wid & 1;     // 8 items = 8 warps
-    deriv_sweep<NZ, false>(VEC(2 * comp + part) + m, VEC(6 + 2 * comp + part) + m, par, inv_s, 1.0);
+    if (wid < 2) deriv_column<NZ, false>(C + wid * VS + lane, C + (3 + wid) * VS + lane, inv_s, 1.0);
+    else if (wid == 2) synthesis_column<NZ>(C + 2 * VS + lane);
+    __syncthreads();
+    if (wid < 2) synthesis_column<NZ>(C + wid * VS + lane);
+    else if (wid == 3 || wid == 4) synthesis_column<NZ>(C + wid * VS + lane);
+  } else {
+    if (wid < 3) synthesis_column<NZ>(C + wid * VS + lane);
   }
   __syncthreads();
 
-  // ---------------- phase 9: synthesis back to the nodes
-  {
-    const int items = A.omega ? 10 : 6;
-    for (int item = wid; item < items; item += NWARPS) synthesis_inplace<NZ>(VEC(item) + m);
-  }
-  __syncthreads();
-
-  // ---------------- phase 10: (1/2) curl u (eq 11), scale by 1/(nx ny) for the unnormalised inverse FFT, store
+  // ---------------- phase 8: (1/2) curl u (eq 11), scale by 1/(nx ny) for the unnormalised inverse FFT, store
   const double scl = 1.0 / ((double)A.nx * (double)A.ny);
-  if (valid && !zero_mode) {
-    for (int l = wid; l < NZ; l += NWARPS) {
-      const int o = l * TM + m;
-      const size_t off = ((size_t)l * A.ny + iy) * A.nkxp + ix;
-      const double ur = VEC(0)[o], ui = VEC(1)[o], vr = VEC(2)[o], vi = VEC(3)[o], wr = VEC(4)[o], wi = VEC(5)[o];
-      A.cplx[0 * A.cplx_field + off] = make_double2(ur * scl, ui * scl);
-      A.cplx[1 * A.cplx_field + off] = make_double2(vr * scl, vi * scl);
-      A.cplx[2 * A.cplx_field + off] = make_double2(wr * scl, wi * scl);
+  double* gout = reinterpret_cast<double*>(A.cplx);
+  for (int l = wid; l < NZ; l += SOLVE_WARPS) {
+    const int o = l * LN + lane;
+    const double u = C[0 * VS + o], v = C[1 * VS + o], w = C[2 * VS + o];
+    double om[3] = {0, 0, 0};
+    if (A.omega) {
+      const double du = C[3 * VS + o], dv = C[4 * VS + o];
+      const double uo = __shfl_xor_sync(0xffffffffu, u, 1), vo = __shfl_xor_sync(0xffffffffu, v, 1), wo = __shfl_xor_sync(0xffffffffu, w, 1);
+      om[0] = 0.5 * (K.sgI * K.kyt * wo - dv);                          // (1/2)(i k_y w - dz v)
+      om[1] = 0.5 * (du - K.sgI * K.kxt * wo);                          // (1/2)(dz u - i k_x w)
+      om[2] = 0.5 * K.sgI * (K.kxt * vo - K.kyt * uo);                  // (1/2)(i k_x v - i k_y u)
+    }
+    if (valid && !zero_mode) {
+      const size_t og = 2 * (l * plane + off0) + part;
+      gout[2 * (0 * A.cplx_field) + og] = u * scl;
+      gout[2 * (1 * A.cplx_field) + og] = v * scl;
+      gout[2 * (2 * A.cplx_field) + og] = w * scl;
       if (A.omega) {
-        const double dur = VEC(6)[o], dui = VEC(7)[o], dvr = VEC(8)[o], dvi = VEC(9)[o];
-        A.cplx[3 * A.cplx_field + off] = make_double2(0.5 * (-kyt * wi - dvr) * scl, 0.5 * (kyt * wr - dvi) * scl);
-        A.cplx[4 * A.cplx_field + off] = make_double2(0.5 * (dur + kxt * wi) * scl, 0.5 * (dui - kxt * wr) * scl);
-        A.cplx[5 * A.cplx_field + off] = make_double2(-0.5 * (kxt * vi - kyt * ui) * scl, 0.5 * (kxt * vr - kyt * ur) * scl);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) gout[2 * ((3 + c) * A.cplx_field) + og] = om[c] * scl;
       }
     }
   }
-#undef VEC
 }
 
 // ---- k = 0 column (paper step 5; eqs 47, 51, 52; (A12) with no slip): one CTA of 64 threads
@@ -529,7 +588,7 @@ __global__ void k_zero_mode(SolveArgs A, int nz, const double* __restrict__ ct_f
     double ar = 0.0, ai = 0.0;
     if (q < 2 || A.torque) {
       for (int l = 0; l < nz; ++l) {
-        double2 v = A.cplx[field * A.cplx_field + (size_t)l * A.ny * A.nkxp];
+        double2 v = A.cplx[field * A.cplx_field + (size_t)l * A.n_slow * A.pitch];
         double wgt = ct_full[n * nz + l] * ((l == 0 || l == N) ? 0.5 : 1.0);
         ar += wgt * v.x; ai += wgt * v.y;
       }
@@ -585,7 +644,7 @@ __global__ void k_zero_mode(SolveArgs A, int nz, const double* __restrict__ ct_f
       for (int comp = 0; comp < 2; ++comp)
         for (int part = 0; part < 2; ++part) { u[comp][part] += cs * uc[comp][part][n]; du[comp][part] += cs * ub[comp][part][n]; }
     }
-    const size_t off = (size_t)l * A.ny * A.nkxp;
+    const size_t off = (size_t)l * A.n_slow * A.pitch;
     A.cplx[0 * A.cplx_field + off] = make_double2(u[0][0] * scl, u[0][1] * scl);
     A.cplx[1 * A.cplx_field + off] = make_double2(u[1][0] * scl, u[1][1] * scl);
     A.cplx[2 * A.cplx_field + off] = make_double2(0.0, 0.0);
@@ -597,7 +656,7 @@ __global__ void k_zero_mode(SolveArgs A, int nz, const double* __restrict__ ct_f
   }
 }
 
-template <int NZ> size_t solve_smem_bytes() { return sizeof(double) * ((size_t)NVEC * NZ * TM + 2 * TM + 16 * TM); }
+template <int NZ> size_t solve_smem_bytes() { return sizeof(double) * (size_t)SolveSmem<NZ>::DOUBLES; }
 
 template <int NZ> void host_tables(std::vector<double>& out) {
   typedef long double ld;
@@ -605,7 +664,12 @@ template <int NZ> void host_tables(std::vector<double>& out) {
   constexpr int N = NZ - 1, LH = NZ / 2;
   out.assign(Tab<NZ>::SIZE, 0.0);
   for (int n = 0; n <= N; ++n)
-    for (int l = 0; l < LH; ++l) out[Tab<NZ>::CT + n * LH + l] = (double)cosl(PI * n * l / N);
+    for (int l = 0; l < LH; ++l) out[Tab<NZ>::CA + n * LH + l] = (double)cosl(PI * n * l / N);
+  for (int l = 0; l < LH; ++l)
+    for (int j = 0; j < LH; ++j) {
+      out[Tab<NZ>::SE + l * LH + j] = (double)cosl(PI * (2 * j) * l / N);
+      out[Tab<NZ>::SO + l * LH + j] = (double)cosl(PI * (2 * j + 1) * l / N);
+    }
   for (int l = 0; l <= N; ++l) out[Tab<NZ>::XI + l] = (double)cosl(PI * l / N);
   // P_n, Q_n: with a = unit vector e_n (n <= N-2), b_m = (cbar_{m-1} a_{m-1} - a_{m+1})/(2m) (1 <= m <= N-1),
   // c_m = (cbar_{m-1} b_{m-1} - b_{m+1})/(2m) (1 <= m <= N), b_0 = 0:  P_n = sum of b_m over m of the other parity,
@@ -629,7 +693,7 @@ template <int NZ> cudaError_t launch_nz(const SolveArgs& A, cudaStream_t st) {
     if (e != cudaSuccess) return e;
     attr = true;
   }
-  dim3 grid((A.nkx + TM - 1) / TM, A.ny);
+  dim3 grid((A.n_fast + TM - 1) / TM, A.n_slow);
   k_solve<NZ><<<grid, SOLVE_THREADS, smem, st>>>(A);
   return cudaGetLastError();
 }
@@ -666,7 +730,8 @@ cudaError_t dp_solve_upload_tables(dp_plan* P) {
 cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega, cudaStream_t st) {
   SolveArgs A;
   A.cplx = P->d_cplx; A.cplx_field = P->cplx_field;
-  A.nx = P->p.nx; A.ny = P->p.ny; A.nkx = P->nkx; A.nkxp = P->nkxp;
+  A.nx = P->p.nx; A.ny = P->p.ny; A.nkx = P->nkx;
+  A.n_fast = P->nkx; A.n_slow = P->p.ny; A.pitch = P->nkxp; A.fast_is_x = 1;
   A.Lx = P->p.Lx; A.Ly = P->p.Ly; A.H = P->p.H; A.eta = P->p.eta;
   A.wall_mode = P->p.wall_mode; A.torque = with_torque_field ? 1 : 0; A.omega = want_omega ? 1 : 0;
   cudaError_t e;
