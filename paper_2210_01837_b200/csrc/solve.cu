@@ -60,6 +60,13 @@ struct SolveArgs {
   int wall_mode, torque, omega;
 };
 
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 // ---- tridiagonal rows of a chain (n >= 1): d_n a_n + l_n a_{n-2} + u_n a_{n+2}; all divisions are compile-time constants
 template <int NZ> __device__ __forceinline__ double row_d(int n, double k2) { return n == 1 ? fma(k2, 0.125, 1.0) : fma(k2, 1.0 / (2.0 * (n * n - 1)), 1.0); }
 template <int NZ> __device__ __forceinline__ double row_l(int n, double k2) { return k2 * (-(n == 2 ? 2.0 : 1.0) / (4.0 * n * (n - 1))); }
@@ -180,8 +187,8 @@ __device__ __forceinline__ double factor_chain(double* __restrict__ Fm, double* 
 //      unknown, double integration.  a[j] = (H/2)^2 r_n of row n = n0+2j on entry, rho0 = (H/2)^2 r_0 (even chain).
 //      Writes y's coefficients c_n of parity PAR to col and, if WITH_D, the coefficients of dy/dz of the OTHER parity to
 //      dcol.  Returns S_c = sum of the c_n written (incl. c_0 for the even chain).
-template <int NZ, int PAR, bool WITH_D>
-__device__ __forceinline__ double chain(double (&a)[Ch<NZ, PAR>::NR], double rho0, const double* __restrict__ Fm, const double* __restrict__ Fi,
+template <int NZ, int PAR>
+__device__ __forceinline__ double chain(bool WITH_D, double (&a)[Ch<NZ, PAR>::NR], double rho0, const double* __restrict__ Fm, const double* __restrict__ Fi,
                                         const double* __restrict__ Fa, double* __restrict__ col, double* __restrict__ dcol, double k,
                                         double k2, double inv_s, double beta_bc, double invBg) {
   constexpr int N = NZ - 1, n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR;
@@ -275,70 +282,59 @@ struct ModeK {
   double k, k2, kxt, kyt, sgI;       // |k|, (k H/2)^2, derivative multipliers (0 on the unpaired Nyquist index), sign of Re/Im(i z)
 };
 
-// ---- pressure item (eqs 15, 17): right-hand side i k.f + dz f_z, chain PAR; p -> C3, dp/dz -> C4
+// ---- one BVP item of a lane: kind 0 = pressure (eqs 15, 17): right-hand side i k.f + dz f_z, p -> C3, dp/dz -> C4;
+//      kind 1 = u or v (comp 0, 1), kind 2 = w (eq 18 with BCs 22, 24): f_c (column comp) is overwritten by u_c.
+//      One code path per parity so that the chain sweeps exist once in the instruction stream.
 template <int NZ, int PAR>
-__device__ __forceinline__ double pressure_item(double* __restrict__ C, const double* __restrict__ F, int lane, int mode, const ModeK& K, double s,
-                                                double inv_s, double invBg) {
+__device__ __noinline__ double bvp_item(int kind, int comp, double* __restrict__ C, const double* __restrict__ F, int lane, int mode, ModeK K,
+                                        double s, double inv_s, double eta, double invBg, double pH_own, double p0_own, double pH_oth, double p0_oth) {
   constexpr int N = NZ - 1, n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR, VS = NZ * LN;
-  const double* fxo = C + 0 * VS + (lane ^ 1);          // the OTHER part of f_x, f_y: i k f mixes re and im
-  const double* fyo = C + 1 * VS + (lane ^ 1);
-  const double* fz = C + 2 * VS + lane;
-  double a[NR], rho0 = 0.0;
-  double d = 0.0;
-  constexpr int ntop = ((N - PAR) & 1) ? N - 1 : N;     // largest n <= N with parity PAR
-  const double s2 = s * s;
+  double a[NR], rho0 = 0.0, beta_bc = 0.0;
+  double* col;
+  if (kind == 0) {
+    const double* fxo = C + 0 * VS + (lane ^ 1);          // the OTHER part of f_x, f_y: i k f mixes re and im
+    const double* fyo = C + 1 * VS + (lane ^ 1);
+    const double* fz = C + 2 * VS + lane;
+    double d = 0.0;
+    constexpr int ntop = ((N - PAR) & 1) ? N - 1 : N;     // largest n <= N with parity PAR
+    const double s2 = s * s;
 #pragma unroll
-  for (int i = 0; i <= ntop / 2; ++i) {
-    const int n = ntop - 2 * i;
-    if (n < 0) break;
-    if (n + 1 <= N) d = fma(2.0 * (n + 1), fz[(n + 1) * LN], d);
-    if (n <= N - 2) {
-      const double r = fma(K.sgI, fma(K.kxt, fxo[n * LN], K.kyt * fyo[n * LN]), d * (n == 0 ? 0.5 * inv_s : inv_s)) * s2;
-      if (n >= n0) a[(n - n0) / 2] = r; else rho0 = r;
+    for (int i = 0; i <= ntop / 2; ++i) {
+      const int n = ntop - 2 * i;
+      if (n < 0) break;
+      if (n + 1 <= N) d = fma(2.0 * (n + 1), fz[(n + 1) * LN], d);
+      if (n <= N - 2) {
+        const double r = fma(K.sgI, fma(K.kxt, fxo[n * LN], K.kyt * fyo[n * LN]), d * (n == 0 ? 0.5 * inv_s : inv_s)) * s2;
+        if (n >= n0) a[n >= n0 ? (n - n0) / 2 : 0] = r; else rho0 = r;
+      }
     }
-  }
-  return chain<NZ, PAR, true>(a, rho0, F + 0 * NZ * TM + mode, F + 1 * NZ * TM + mode, F + 2 * NZ * TM + mode, C + 3 * VS + lane, C + 4 * VS + lane,
-                              K.k, K.k2, inv_s, 0.0, invBg);
-}
-
-// ---- velocity item (eq 18 with BCs 22, 24): component COMP, chain PAR; f_c (column COMP) is overwritten by u_c
-template <int NZ, int PAR>
-__device__ __forceinline__ double velocity_item(int comp, double* __restrict__ C, const double* __restrict__ F, int lane, int mode, const ModeK& K,
-                                                double s, double inv_s, double eta, double invBg, double pH_own, double p0_own, double pH_oth,
-                                                double p0_oth) {
-  constexpr int N = NZ - 1, n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR, VS = NZ * LN;
-  double* col = C + comp * VS + lane;
-  double a[NR], rho0 = 0.0, gH, g0;
-  const double sc = s * s / eta;
-  if (comp < 2) {
-    const double kc = comp == 0 ? K.kxt : K.kyt;
-    const double* po = C + 3 * VS + (lane ^ 1);          // other part of p
-    const double f = K.sgI * kc;
-#pragma unroll
-    for (int i = 0; i <= (N - 2 - PAR) / 2; ++i) {
-      const int n = PAR + 2 * i;
-      const double r = (f * po[n * LN] - col[n * LN]) * sc;       // r = (i k_c p - f_c)/eta
-      if (n >= n0) a[(n - n0) / 2] = r; else rho0 = r;
-    }
-    // (dz + k) u(H) = -(i k_c/(2 k eta)) p(H) ; (dz - k) u(0) = +(i k_c/(2 k eta)) p(0)      (eq 22)
-    const double c = kc / (2.0 * K.k * eta);
-    gH = -K.sgI * c * pH_oth;
-    g0 = K.sgI * c * p0_oth;
+    col = C + 3 * VS + lane;
   } else {
-    const double* dp = C + 4 * VS + lane;
+    col = C + comp * VS + lane;
+    const double sc = s * s / eta;
+    double gH, g0;
+    // kind 1: r = (i k_c p - f_c)/eta ; kind 2: r = (dz p - f_z)/eta
+    const double* src = kind == 1 ? C + 3 * VS + (lane ^ 1) : C + 4 * VS + lane;
+    const double kc = comp == 0 ? K.kxt : K.kyt;
+    const double f = kind == 1 ? K.sgI * kc : 1.0;
 #pragma unroll
     for (int i = 0; i <= (N - 2 - PAR) / 2; ++i) {
       const int n = PAR + 2 * i;
-      const double r = (dp[n * LN] - col[n * LN]) * sc;            // r = (dz p - f_z)/eta
-      if (n >= n0) a[(n - n0) / 2] = r; else rho0 = r;
+      const double r = (f * src[n * LN] - col[n * LN]) * sc;
+      if (n >= n0) a[n >= n0 ? (n - n0) / 2 : 0] = r; else rho0 = r;
     }
-    // (dz + k) w(H) = p(H)/(2 eta) ; (dz - k) w(0) = p(0)/(2 eta)                              (eq 24)
-    gH = pH_own / (2.0 * eta);
-    g0 = p0_own / (2.0 * eta);
+    if (kind == 1) {
+      // (dz + k) u(H) = -(i k_c/(2 k eta)) p(H) ; (dz - k) u(0) = +(i k_c/(2 k eta)) p(0)      (eq 22)
+      const double c = kc / (2.0 * K.k * eta);
+      gH = -K.sgI * c * pH_oth; g0 = K.sgI * c * p0_oth;
+    } else {
+      // (dz + k) w(H) = p(H)/(2 eta) ; (dz - k) w(0) = p(0)/(2 eta)                              (eq 24)
+      gH = pH_own / (2.0 * eta); g0 = p0_own / (2.0 * eta);
+    }
+    beta_bc = PAR ? 0.5 * (gH + g0) : 0.5 * (gH - g0);
   }
-  const double beta_bc = PAR ? 0.5 * (gH + g0) : 0.5 * (gH - g0);
-  return chain<NZ, PAR, false>(a, rho0, F + 0 * NZ * TM + mode, F + 1 * NZ * TM + mode, F + 2 * NZ * TM + mode, col, nullptr, K.k, K.k2, inv_s,
-                               beta_bc, invBg);
+  return chain<NZ, PAR>(kind == 0, a, rho0, F + 0 * NZ * TM + mode, F + 1 * NZ * TM + mode, F + 2 * NZ * TM + mode, col, C + 4 * VS + lane,
+                        K.k, K.k2, inv_s, beta_bc, invBg);
 }
 
 // ---- wall correction coefficients of a lane (own part), basis: 0 = z e^{-kz}, 1 = e^{-kz}, 2 = z e^{-k(H-z)}, 3 = e^{-k(H-z)}
@@ -433,44 +429,40 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
   const size_t off0 = (size_t)islow * A.pitch + ifast;
   const double* gin = reinterpret_cast<const double*>(A.cplx);
 
-  // ---------------- phase 0: load the nodal columns, fold the algebraic part of (1/2) curl t into f (eq 7)
-  for (int l = wid; l < NZ; l += SOLVE_WARPS) {
-    double f[3] = {0, 0, 0}, t[3] = {0, 0, 0};
-    if (valid) {
-      const size_t o = 2 * (l * plane + off0) + part;
+  // ---------------- phase 0: all nodal columns go HBM -> shared memory as 8-byte cp.async (no registers, everything in
+  // flight at once); t_z is only needed for the fold and travels through registers.  While the loads fly: warps 0, 1 factor
+  // the two chains, warps 2-5 evaluate e^{-k z_l} and z_l e^{-k z_l} at the nodes (-> C5).  Then every warp folds the
+  // algebraic part of (1/2) curl t into f for the rows it loaded itself (eq 7).
+  constexpr int ROWS = (NZ + SOLVE_WARPS - 1) / SOLVE_WARPS;
+  double tz[ROWS];
 #pragma unroll
-      for (int c = 0; c < 3; ++c) f[c] = gin[2 * (c * A.cplx_field) + o];
-      if (A.torque) {
+  for (int r = 0; r < ROWS; ++r) {
+    const int l = wid + r * SOLVE_WARPS;
+    tz[r] = 0.0;
+    if (l < NZ) {
+      const int o = l * LN + lane;
+      if (valid) {
+        const size_t og = 2 * (l * plane + off0) + part;
 #pragma unroll
-        for (int c = 0; c < 3; ++c) t[c] = gin[2 * ((3 + c) * A.cplx_field) + o];
+        for (int c = 0; c < 3; ++c) cp_async8(&C[c * VS + o], &gin[2 * (c * A.cplx_field) + og]);
+        if (A.torque) {
+          cp_async8(&C[3 * VS + o], &gin[2 * (3 * A.cplx_field) + og]);
+          cp_async8(&C[4 * VS + o], &gin[2 * (4 * A.cplx_field) + og]);
+          tz[r] = __ldg(&gin[2 * (5 * A.cplx_field) + og]);
+        }
+      } else {
+#pragma unroll
+        for (int c = 0; c < 5; ++c) C[c * VS + o] = 0.0;
       }
     }
-    const int o = l * LN + lane;
-    if (A.torque) {
-      const double t0o = __shfl_xor_sync(0xffffffffu, t[0], 1), t1o = __shfl_xor_sync(0xffffffffu, t[1], 1), t2o = __shfl_xor_sync(0xffffffffu, t[2], 1);
-      f[0] = fma(0.5 * K.sgI * K.kyt, t2o, f[0]);                       // f_x += (1/2) i k_y t_z
-      f[1] = fma(-0.5 * K.sgI * K.kxt, t2o, f[1]);                      // f_y -= (1/2) i k_x t_z
-      f[2] = fma(0.5 * K.sgI, K.kxt * t1o - K.kyt * t0o, f[2]);         // f_z += (1/2) i (k_x t_y - k_y t_x)
-      C[3 * VS + o] = t[0]; C[4 * VS + o] = t[1];
-    }
-    C[0 * VS + o] = f[0]; C[1 * VS + o] = f[1]; C[2 * VS + o] = f[2];
   }
-  __syncthreads();
-
-  // ---------------- phase 1: Chebyshev analysis of the 3 (or 5) columns, one warp per column; warp 5: chain factorisation
-  if (wid < (A.torque ? 5 : 3)) {
-    analysis_column<NZ>(C + wid * VS + lane);
-  } else if (wid == 5) {
-    const bool store = part == 0;
-    const double i0 = factor_chain<NZ, 0>(F + mode, F + NZ * TM + mode, F + 2 * NZ * TM + mode, K.k, K.k2, inv_s, store);
-    const double i1 = factor_chain<NZ, 1>(F + mode, F + NZ * TM + mode, F + 2 * NZ * TM + mode, K.k, K.k2, inv_s, store);
-    if (store) { s_ibg[mode] = i0; s_ibg[TM + mode] = i1; }
-  }
-  __syncthreads();
-
-  // ---------------- phase 2: f_x -= (1/2) D t_y, f_y += (1/2) D t_x (eq 7); warps 2-5: e^{-k z_l} and z_l e^{-k z_l} at the nodes -> C5
-  if (wid < 2) {
-    if (A.torque) deriv_column<NZ, true>(C + (wid == 0 ? 4 : 3) * VS + lane, C + wid * VS + lane, inv_s, wid == 0 ? -0.5 : 0.5);
+  cp_async_commit();
+  if (wid == 0) {
+    const double ib = factor_chain<NZ, 0>(F + mode, F + NZ * TM + mode, F + 2 * NZ * TM + mode, K.k, K.k2, inv_s, part == 0);
+    if (part == 0) s_ibg[mode] = ib;
+  } else if (wid == 1) {
+    const double ib = factor_chain<NZ, 1>(F + mode, F + NZ * TM + mode, F + 2 * NZ * TM + mode, K.k, K.k2, inv_s, part == 0);
+    if (part == 0) s_ibg[TM + mode] = ib;
   } else {
     for (int l = wid - 2; l < NZ; l += SOLVE_WARPS - 2) {
       const double zl = s * (1.0 + T[Tab<NZ>::XI + l]);
@@ -478,26 +470,57 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
       C[5 * VS + l * LN + lane] = part ? zl * E : E;
     }
   }
-  __syncthreads();
-
-  // ---------------- phase 3: pressure BVP (eqs 15, 17), one warp per chain; warp 2: Chebyshev coefficients of (E, zE) (step 6)
-  if (wid == 0) s_sum[(0 * 2 + 0) * LN + lane] = pressure_item<NZ, 0>(C, F, lane, mode, K, s, inv_s, s_ibg[mode]);
-  else if (wid == 1) s_sum[(0 * 2 + 1) * LN + lane] = pressure_item<NZ, 1>(C, F, lane, mode, K, s, inv_s, s_ibg[TM + mode]);
-  else if (wid == 2) analysis_column<NZ>(C + 5 * VS + lane);
-  __syncthreads();
-
-  // ---------------- phase 4: velocity BVPs (eq 18) with BCs (22), (24); one warp per (component, chain)
-  {
-    const int comp = wid >> 1;
-    const double se = s_sum[0 * LN + lane], so = s_sum[1 * LN + lane];
-    const double pH = se + so, p0 = se - so;              // p(H) = sum p_n, p(0) = sum (-1)^n p_n  ("direct summation")
-    const double pHo = __shfl_xor_sync(0xffffffffu, pH, 1), p0o = __shfl_xor_sync(0xffffffffu, p0, 1);
-    double Sc;
-    if (wid & 1) Sc = velocity_item<NZ, 1>(comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[TM + mode], pH, p0, pHo, p0o);
-    else Sc = velocity_item<NZ, 0>(comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], pH, p0, pHo, p0o);
-    s_sum[((1 + comp) * 2 + (wid & 1)) * LN + lane] = Sc;
+  cp_async_wait_all();
+  __syncwarp();
+  if (A.torque) {
+#pragma unroll
+    for (int r = 0; r < ROWS; ++r) {
+      const int l = wid + r * SOLVE_WARPS;
+      if (l < NZ) {
+        const int o = l * LN + lane, oo = l * LN + (lane ^ 1);
+        const double t2o = __shfl_xor_sync(0xffffffffu, tz[r], 1);
+        const double t0o = C[3 * VS + oo], t1o = C[4 * VS + oo];
+        C[0 * VS + o] = fma(0.5 * K.sgI * K.kyt, t2o, C[0 * VS + o]);                       // f_x += (1/2) i k_y t_z
+        C[1 * VS + o] = fma(-0.5 * K.sgI * K.kxt, t2o, C[1 * VS + o]);                      // f_y -= (1/2) i k_x t_z
+        C[2 * VS + o] = fma(0.5 * K.sgI, K.kxt * t1o - K.kyt * t0o, C[2 * VS + o]);         // f_z += (1/2) i (k_x t_y - k_y t_x)
+      }
+    }
   }
   __syncthreads();
+
+  // ---------------- phase 1: Chebyshev analysis, one warp per column: f_x, f_y, f_z, (E, zE) [, t_x, t_y]   (step 2; step 6)
+  {
+    const int col = wid < 3 ? wid : (wid == 3 ? 5 : wid - 1);          // warps 0-2: C0-C2, warp 3: C5, warps 4, 5: C3, C4
+    if (wid < 4 || A.torque) analysis_column<NZ>(C + col * VS + lane);
+  }
+  __syncthreads();
+
+  // ---------------- phase 2: f_x -= (1/2) D t_y, f_y += (1/2) D t_x (eq 7)
+  if (A.torque) {
+    if (wid < 2) deriv_column<NZ, true>(C + (wid == 0 ? 4 : 3) * VS + lane, C + wid * VS + lane, inv_s, wid == 0 ? -0.5 : 0.5);
+    __syncthreads();
+  }
+
+  // ---------------- phases 3, 4: pressure BVP (eqs 15, 17), one warp per chain; then the velocity BVPs (eq 18) with BCs
+  // (22), (24), one warp per (component, chain)
+#pragma unroll 1
+  for (int ph = 0; ph < 2; ++ph) {
+    if (ph == 1 || wid < 2) {
+      const int comp = wid >> 1, par = wid & 1;
+      const int kind = ph == 0 ? 0 : (comp == 2 ? 2 : 1);
+      double pH = 0.0, p0 = 0.0;
+      if (ph == 1) {
+        const double se = s_sum[0 * LN + lane], so = s_sum[1 * LN + lane];
+        pH = se + so; p0 = se - so;                       // p(H) = sum p_n, p(0) = sum (-1)^n p_n  ("direct summation")
+      }
+      const double pHo = __shfl_xor_sync(0xffffffffu, pH, 1), p0o = __shfl_xor_sync(0xffffffffu, p0, 1);
+      double Sc;
+      if (par) Sc = bvp_item<NZ, 1>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[TM + mode], pH, p0, pHo, p0o);
+      else Sc = bvp_item<NZ, 0>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], pH, p0, pHo, p0o);
+      s_sum[((ph == 0 ? 0 : 1 + comp) * 2 + par) * LN + lane] = Sc;
+    }
+    __syncthreads();
+  }
 
   // ---------------- phase 5: correction coefficients (bottom wall: every warp for itself; slit: warp 0, shared)
   double cf[3][4];
@@ -536,13 +559,9 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
   // ---------------- phase 7: dz u, dz v of the TOTAL in coefficient space (reading G12) -> C3, C4; synthesis back to the nodes
   if (A.omega) {
     if (wid < 2) deriv_column<NZ, false>(C + wid * VS + lane, C + (3 + wid) * VS + lane, inv_s, 1.0);
-    else if (wid == 2) synthesis_column<NZ>(C + 2 * VS + lane);
     __syncthreads();
-    if (wid < 2) synthesis_column<NZ>(C + wid * VS + lane);
-    else if (wid == 3 || wid == 4) synthesis_column<NZ>(C + wid * VS + lane);
-  } else {
-    if (wid < 3) synthesis_column<NZ>(C + wid * VS + lane);
   }
+  if (wid < (A.omega ? 5 : 3)) synthesis_column<NZ>(C + wid * VS + lane);
   __syncthreads();
 
   // ---------------- phase 8: (1/2) curl u (eq 11), scale by 1/(nx ny) for the unnormalised inverse FFT, store
