@@ -53,6 +53,8 @@ typedef struct {
   int max_particles;    /* capacity of the plan's particle workspace                                                 */
   int use_torques;      /* 0: forces in, U out only (3 grid fields); 1: also torques in / Omega out (6 fields)       */
   int device;           /* CUDA device ordinal                                                                       */
+  int fft_backend;      /* 0: the library's own shared-memory FFT passes when nx, ny allow them (nx/2 and ny products
+                           of 2, 3, 5; nx <= 4320, ny <= 4320), else cuFFT;  1: always cuFFT (kept for comparison)    */
 } dp_params;
 
 /* Validate, allocate (2 grids of fields*nz*ny*(nx+2) doubles + cuFFT workspace + particle workspace), plan the FFTs,
@@ -86,7 +88,8 @@ int dp_stage_ms(dp_plan* plan, float* ms /* [8] */);
 
 /* Test hook: copy an internal device buffer of the last apply to HOST memory (synchronises).
  *   which = 0: real grid    [fields][nz][ny][nx]       doubles  (after apply: u, (1/2) curl u in real space)
- *   which = 1: complex grid [fields][nz][ny][nkxp]     double2  (after apply: consumed by the inverse FFT, undefined)
+ *   which = 1: complex grid [fields][nz][ny][nkxp]     double2  (after apply: consumed by the inverse FFT, undefined;
+ *              with the own FFT passes the internal layout is transposed and digit-reversed in ky — the copy undoes it)
  * dp_debug_run_stage runs the product up to and including `last_stage` (1 spread, 2 fwd FFT, 3 solve, 4 inv FFT) so
  * that the buffers hold that stage's output.  Sizes via dp_buffer_bytes. */
 int dp_debug_run_stage(dp_plan* plan, int n, const double* pos, const double* force, const double* torque, int last_stage,
@@ -94,6 +97,7 @@ int dp_debug_run_stage(dp_plan* plan, int n, const double* pos, const double* fo
 size_t dp_buffer_bytes(const dp_plan* plan, int which);
 int dp_copy_buffer_to_host(dp_plan* plan, int which, void* host, size_t bytes);
 int dp_complex_row_pitch(const dp_plan* plan); /* nkxp: padded row length (in complex numbers) of the half spectrum */
+int dp_fft_backend(const dp_plan* plan);       /* 0: own shared-memory FFT passes in use, 1: cuFFT                    */
 
 /* Introspection */
 double dp_es_norm(double alpha, double beta);                  /* Z of eq 54, Gauss-Legendre on the host             */

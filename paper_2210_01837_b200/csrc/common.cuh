@@ -34,7 +34,7 @@ struct dp_plan {
 
   // device buffers
   double* d_real = nullptr;     // [fields][nz][ny][nx]
-  double2* d_cplx = nullptr;    // [fields][nz][ny][nkxp]
+  double2* d_cplx = nullptr;    // [fields][nz][ny][nkxp] (cuFFT path) or [fields][nz][nkx][ny] (own FFT passes)
   void* d_fft_work = nullptr;
   size_t fft_work_bytes = 0;
   double* d_znodes = nullptr;   // z_l
@@ -55,6 +55,9 @@ struct dp_plan {
 
   cufftHandle fft_fwd = 0, fft_inv = 0;
   bool fft_ok = false;
+  // own shared-memory FFT passes (fft.cu): half spectrum stored transposed, [field][nz][nkx][ny], ky digit-reversed
+  bool own_fft = false;
+  void* fft_own = nullptr;
 
   cudaStream_t last_stream = nullptr;
   bool profiling = false;
@@ -71,6 +74,15 @@ cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaSt
 cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega, cudaStream_t st);
 cudaError_t dp_solve_upload_tables(dp_plan* P);
 bool dp_solve_supports_nz(int nz);
+// fft.cu: the xy FFTs as two shared-memory passes per direction
+bool dp_fft_own_supported(int nx, int ny);
+cudaError_t dp_fft_own_create(dp_plan* P);
+void dp_fft_own_destroy(dp_plan* P);
+size_t dp_fft_own_cplx_field(const dp_plan* P);
+const int* dp_fft_own_ky_table(const dp_plan* P);
+cudaError_t dp_fft_own_forward(dp_plan* P, int nfields, cudaStream_t st);
+cudaError_t dp_fft_own_inverse(dp_plan* P, int nfields, cudaStream_t st);
+cudaError_t dp_fft_own_untranspose(dp_plan* P, double2* dst, cudaStream_t st);
 
 // ---- exponential-of-semicircle kernel, eq 54: phi(s) = exp(beta (sqrt(1-(s/alpha)^2) - 1)) / Z on |s| <= alpha
 __device__ __forceinline__ double dp_es_phi(double s, double inv_alpha, double beta, double inv_Z) {

@@ -1,0 +1,370 @@
+// fft.cu — the batched 2D xy FFTs of the DP Stokes solver (paper step 2 and step 7) as two
+// shared-memory passes per direction instead of a library plan:
+//
+//   forward   pass X: every real grid row (f, l, y, :) -> real-to-complex FFT along x -> written TRANSPOSED into the half
+//                     spectrum T[f][l][kx][y]  (y contiguous)
+//             pass Y: every row T[f][l][kx][:] -> complex FFT along y, in place; ky stays at its digit-reversed position
+//   (per-wavenumber solve on T: it is pointwise in (kx, ky), so it only needs ky as a function of the position)
+//   inverse   pass Y: inverse FFT along y in place (digit-reversed in, natural out)
+//             pass X: gather T[f][l][:][y] -> complex-to-real FFT along x -> real grid row
+//
+// Each pass reads every grid value once and writes it once (4 passes per product and field instead of the ten of the
+// library's multi-kernel plans at 4320 x 4320).  A row lives in shared memory for its whole transform (fft_engine.cuh);
+// contiguous rows move with bulk asynchronous copies (cp.async.bulk + mbarrier), so no thread spends registers or issue
+// slots on them; one persistent CTA per SM holds the twiddle table and two independent row slots (320 threads each,
+// named barriers), so that one slot's copies overlap the other slot's butterflies.
+// The real transform of length nx is a complex transform of length M = nx/2 on z[m] = x[2m] + i x[2m+1] with the usual
+// split  X[k] = E[k] + W_nx^k O[k],  E = (Z[k] + conj Z[M-k])/2,  O = -i (Z[k] - conj Z[M-k])/2.
+#include <cstdint>
+#include <cstdio>
+#include <vector>
+
+#include "common.cuh"
+#include "fft_engine.cuh"
+
+namespace {
+
+using namespace dpfft;
+
+constexpr int NSLOT = 2;
+constexpr int TPS = 320;                       // threads per slot (10 warps; 20 warps per SM leave 96 registers per thread): 270 / 240 / 288 lines per stage at n = 4320
+constexpr int FFT_THREADS = NSLOT * TPS;
+constexpr int SLOT_ELEMS = 4320;               // complex elements a slot can hold (69 120 bytes)
+
+struct dp_fft_own {
+  Factors Fx, Fy;            // M = nx/2 and ny
+  int rbx = 1, rby = 1;      // rows per slot batch in the x and y passes
+  double2* d_tw_x = nullptr;   // exp(-2 pi i j / M), j < M
+  double2* d_post_x = nullptr; // exp(-2 pi i k / nx), k <= M/2
+  double2* d_tw_y = nullptr;   // exp(-2 pi i j / ny), j < ny
+  unsigned short* d_pos_x = nullptr;   // position of Z[k] after the forward x transform
+  int* d_ky_of_pos = nullptr;          // FFT-order ky index held at position p of a transformed y row
+  size_t smem_x = 0, smem_y = 0;
+  int grid = 148;
+};
+
+// ---- PTX wrappers: mbarrier, bulk asynchronous copies, named barriers
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gmem_src, unsigned bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
+               "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void bulk_store(void* gmem_dst, const void* smem_src, unsigned bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gmem_dst), "r"(smem_u32(smem_src)), "r"(bytes) : "memory");
+  asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+}
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_proxy() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void slot_barrier(int slot) { asm volatile("bar.sync %0, %1;" ::"r"(slot + 1), "r"(TPS) : "memory"); }
+
+struct FftYArgs {
+  double2* data;          // rows of n complex numbers, contiguous
+  long long rows;
+  const double2* tw;
+  Factors F;
+  int rb;                 // rows per slot batch
+};
+
+struct FftXArgs {
+  double* real;           // [planes][ny][nx]
+  double2* cplx;          // [planes][nkx][ny]
+  long long planes;       // fields * nz
+  int nx, ny, M;
+  const double2* tw;      // length M
+  const double2* post;    // length M/2 + 1
+  const unsigned short* pos;
+  Factors F;
+  int rb;                 // rows (consecutive y) per slot batch; divides ny
+};
+
+__host__ __device__ inline size_t align16(size_t b) { return (b + 15) / 16 * 16; }
+
+// ---------------------------------------------------------------------------------------------- pass Y (in place)
+template <bool INV>
+__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_y(FftYArgs A) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int n = A.F.n;
+  double2* tw = reinterpret_cast<double2*>(smem_raw);
+  const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
+  double2* buf = tw + n + (size_t)slot * A.rb * n;
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(tw + n + (size_t)NSLOT * A.rb * n) + slot;
+  for (int i = threadIdx.x; i < n; i += FFT_THREADS) tw[i] = A.tw[i];
+  if (st == 0) mbar_init(mbar, 1);
+  fence_async_proxy();
+  __syncthreads();
+  unsigned phase = 0;
+  const long long nbatch = (A.rows + A.rb - 1) / A.rb;
+  for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
+    const long long row0 = b * A.rb;
+    const int nr = (int)((A.rows - row0) < A.rb ? (A.rows - row0) : A.rb);
+    double2* g = A.data + row0 * n;
+    const unsigned bytes = (unsigned)nr * n * 16u;
+    if (st == 0) { mbar_expect_tx(mbar, bytes); bulk_load(buf, g, bytes, mbar); }
+    mbar_wait(mbar, phase);
+    phase ^= 1;
+    if (!INV) {
+      int S = n;
+      for (int j = 0; j < A.F.ns; ++j) {
+        S /= A.F.r[j];
+        stage_dispatch<false>(A.F.r[j], buf, tw, n, S, nr, n, st, TPS);
+        if (j + 1 < A.F.ns) slot_barrier(slot);
+      }
+    } else {
+      int S = 1;
+      for (int j = A.F.ns - 1; j >= 0; --j) {
+        stage_dispatch<true>(A.F.r[j], buf, tw, n, S, nr, n, st, TPS);
+        S *= A.F.r[j];
+        if (j > 0) slot_barrier(slot);
+      }
+    }
+    fence_async_proxy();
+    slot_barrier(slot);
+    if (st == 0) { bulk_store(g, buf, bytes); bulk_wait_read(); }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- pass X forward
+__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int M = A.M, npost = M / 2 + 1;
+  double2* tw = reinterpret_cast<double2*>(smem_raw);
+  double2* post = tw + M;
+  const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
+  double2* buf = post + npost + (size_t)slot * A.rb * M;
+  unsigned short* pos = reinterpret_cast<unsigned short*>(post + npost + (size_t)NSLOT * A.rb * M);
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(reinterpret_cast<unsigned char*>(pos) + align16(sizeof(unsigned short) * M)) + slot;
+  for (int i = threadIdx.x; i < M; i += FFT_THREADS) { tw[i] = A.tw[i]; pos[i] = A.pos[i]; }
+  for (int i = threadIdx.x; i < npost; i += FFT_THREADS) post[i] = A.post[i];
+  if (st == 0) mbar_init(mbar, 1);
+  fence_async_proxy();
+  __syncthreads();
+  unsigned phase = 0;
+  const int rb = A.rb, ny = A.ny, nkx = M + 1;
+  const long long nbatch = A.planes * (ny / rb);
+  const unsigned bytes = (unsigned)rb * A.nx * 8u;
+  for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
+    const long long row0 = b * rb;                       // flat row index over (plane, y)
+    const long long pl = row0 / ny;
+    const int y0 = (int)(row0 - pl * ny);
+    if (st == 0) { mbar_expect_tx(mbar, bytes); bulk_load(buf, A.real + row0 * A.nx, bytes, mbar); }
+    mbar_wait(mbar, phase);
+    phase ^= 1;
+    int S = M;
+    for (int j = 0; j < A.F.ns; ++j) {
+      S /= A.F.r[j];
+      stage_dispatch<false>(A.F.r[j], buf, tw, M, S, rb, M, st, TPS);
+      slot_barrier(slot);
+    }
+    // split into the spectra of the real rows and write them transposed: T[pl][kx][y0 + r]
+    double2* out = A.cplx + (size_t)pl * nkx * ny + y0;
+    for (int idx = st; idx < npost * rb; idx += TPS) {
+      const int k = idx / rb, r = idx - k * rb;
+      const int km = (k == 0) ? 0 : M - k;
+      const double2 z1 = buf[r * M + pos[k]], z2 = buf[r * M + pos[km]];
+      const double2 E = make_double2(0.5 * (z1.x + z2.x), 0.5 * (z1.y - z2.y));
+      const double2 O = make_double2(0.5 * (z1.y + z2.y), -0.5 * (z1.x - z2.x));
+      const double2 B = cmul(O, post[k]);
+      out[(size_t)k * ny + r] = cadd(E, B);
+      if (2 * k != M) out[(size_t)(M - k) * ny + r] = make_double2(E.x - B.x, -(E.y - B.y));
+    }
+    slot_barrier(slot);                                  // every read of buf is done before the next bulk load lands
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- pass X inverse
+__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_inv(FftXArgs A) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int M = A.M, npost = M / 2 + 1;
+  double2* tw = reinterpret_cast<double2*>(smem_raw);
+  double2* post = tw + M;
+  const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
+  double2* buf = post + npost + (size_t)slot * A.rb * M;
+  unsigned short* pos = reinterpret_cast<unsigned short*>(post + npost + (size_t)NSLOT * A.rb * M);
+  for (int i = threadIdx.x; i < M; i += FFT_THREADS) { tw[i] = A.tw[i]; pos[i] = A.pos[i]; }
+  for (int i = threadIdx.x; i < npost; i += FFT_THREADS) post[i] = A.post[i];
+  __syncthreads();
+  const int rb = A.rb, ny = A.ny, nkx = M + 1;
+  const long long nbatch = A.planes * (ny / rb);
+  const unsigned bytes = (unsigned)rb * A.nx * 8u;
+  for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
+    const long long row0 = b * rb;
+    const long long pl = row0 / ny;
+    const int y0 = (int)(row0 - pl * ny);
+    const double2* in = A.cplx + (size_t)pl * nkx * ny + y0;
+    // Z'[k] = (X[k] + conj X[M-k]) + i conj(W^k) (X[k] - conj X[M-k]) at its digit-reversed position (unnormalised C2R)
+#pragma unroll 4
+    for (int idx = st; idx < npost * rb; idx += TPS) {
+      const int k = idx / rb, r = idx - k * rb;
+      const double2 X1 = __ldg(in + (size_t)k * ny + r), X2 = __ldg(in + (size_t)(M - k) * ny + r);
+      if (k == 0) {
+        buf[r * M + pos[0]] = make_double2(X1.x + X2.x, X1.x - X2.x);      // imaginary parts of X[0], X[M] are ignored
+      } else {
+        const double2 Aa = make_double2(X1.x + X2.x, X1.y - X2.y), D = make_double2(X1.x - X2.x, X1.y + X2.y);
+        const double2 Bq = cmulc(D, post[k]);
+        buf[r * M + pos[k]] = make_double2(Aa.x - Bq.y, Aa.y + Bq.x);
+        if (2 * k != M) buf[r * M + pos[M - k]] = make_double2(Aa.x + Bq.y, Bq.x - Aa.y);
+      }
+    }
+    slot_barrier(slot);
+    int S = 1;
+    for (int j = A.F.ns - 1; j >= 0; --j) {
+      stage_dispatch<true>(A.F.r[j], buf, tw, M, S, rb, M, st, TPS);
+      S *= A.F.r[j];
+      if (j > 0) slot_barrier(slot);
+    }
+    fence_async_proxy();
+    slot_barrier(slot);
+    if (st == 0) { bulk_store(A.real + row0 * A.nx, buf, bytes); bulk_wait_read(); }
+    slot_barrier(slot);                                  // the store has read buf before anyone refills it
+  }
+}
+
+// test hook: transposed, digit-reversed half spectrum -> natural layout [planes][ny][nkxp]
+__global__ void k_fft_untranspose(const double2* __restrict__ T, double2* __restrict__ out, const int* __restrict__ ky_of_pos, int ny, int nkx,
+                                  int nkxp, long long planes) {
+  const long long total = planes * nkx * ny;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
+    const int p = (int)(i % ny);
+    const long long q = i / ny;
+    const int kx = (int)(q % nkx);
+    const long long pl = q / nkx;
+    out[(pl * ny + ky_of_pos[p]) * nkxp + kx] = T[i];
+  }
+}
+
+template <class T> cudaError_t upload(T** dst, const std::vector<T>& v, dp_plan* P) {
+  cudaError_t e = cudaMalloc((void**)dst, sizeof(T) * v.size());
+  if (e != cudaSuccess) return e;
+  P->device_bytes += sizeof(T) * v.size();
+  return cudaMemcpy(*dst, v.data(), sizeof(T) * v.size(), cudaMemcpyHostToDevice);
+}
+
+size_t smem_bytes_y(int n, int rb) { return sizeof(double2) * ((size_t)n + (size_t)NSLOT * rb * n) + 8 * NSLOT; }
+size_t smem_bytes_x(int M, int rb) {
+  return sizeof(double2) * ((size_t)M + (M / 2 + 1) + (size_t)NSLOT * rb * M) + align16(sizeof(unsigned short) * M) + 8 * NSLOT;
+}
+
+}  // namespace
+
+bool dp_fft_own_supported(int nx, int ny) {
+  Factors F;
+  if (nx % 2 || nx / 2 > SLOT_ELEMS / 2 || ny > SLOT_ELEMS || ny % 2) return false;
+  return factorize(nx / 2, &F) && factorize(ny, &F);
+}
+
+size_t dp_fft_own_cplx_field(const dp_plan* P) { return (size_t)P->p.nz * (P->p.nx / 2 + 1) * P->p.ny; }
+const int* dp_fft_own_ky_table(const dp_plan* P) { return P->fft_own ? static_cast<const dp_fft_own*>(P->fft_own)->d_ky_of_pos : nullptr; }
+
+void dp_fft_own_destroy(dp_plan* P) {
+  dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
+  if (!O) return;
+  void* bufs[] = {O->d_tw_x, O->d_post_x, O->d_tw_y, O->d_pos_x, O->d_ky_of_pos};
+  for (void* b : bufs) if (b) cudaFree(b);
+  delete O;
+  P->fft_own = nullptr;
+}
+
+cudaError_t dp_fft_own_create(dp_plan* P) {
+  typedef long double ld;
+  const ld PI = 3.141592653589793238462643383279502884L;
+  const int nx = P->p.nx, ny = P->p.ny, M = nx / 2;
+  dp_fft_own* O = new dp_fft_own();
+  P->fft_own = O;
+  if (!factorize(M, &O->Fx) || !factorize(ny, &O->Fy)) return cudaErrorInvalidValue;
+  // rows per slot batch: as many as fit the slot; in the x passes the batch must tile a plane's ny rows
+  O->rby = SLOT_ELEMS / ny < 1 ? 1 : SLOT_ELEMS / ny;
+  int rbmax = SLOT_ELEMS / M;                // <= 2 rows at nx = 4320: a batch is rb * nx doubles = rb * M complex
+  if (rbmax < 1) rbmax = 1;
+  if (rbmax > 64) rbmax = 64;
+  O->rbx = 1;
+  for (int r = rbmax; r >= 1; --r) if (ny % r == 0) { O->rbx = r; break; }
+  std::vector<double2> twx(M), post(M / 2 + 1), twy(ny);
+  for (int j = 0; j < M; ++j) twx[j] = make_double2((double)cosl(2 * PI * j / M), (double)-sinl(2 * PI * j / M));
+  for (int k = 0; k <= M / 2; ++k) post[k] = make_double2((double)cosl(2 * PI * k / nx), (double)-sinl(2 * PI * k / nx));
+  for (int j = 0; j < ny; ++j) twy[j] = make_double2((double)cosl(2 * PI * j / ny), (double)-sinl(2 * PI * j / ny));
+  std::vector<unsigned short> posx(M);
+  for (int k = 0; k < M; ++k) posx[k] = (unsigned short)position_of(O->Fx, k);
+  std::vector<int> kyp(ny);
+  for (int k = 0; k < ny; ++k) kyp[position_of(O->Fy, k)] = k;
+  cudaError_t e;
+  if ((e = upload(&O->d_tw_x, twx, P)) != cudaSuccess) return e;
+  if ((e = upload(&O->d_post_x, post, P)) != cudaSuccess) return e;
+  if ((e = upload(&O->d_tw_y, twy, P)) != cudaSuccess) return e;
+  if ((e = upload(&O->d_pos_x, posx, P)) != cudaSuccess) return e;
+  if ((e = upload(&O->d_ky_of_pos, kyp, P)) != cudaSuccess) return e;
+  O->smem_x = smem_bytes_x(M, O->rbx);
+  O->smem_y = smem_bytes_y(ny, O->rby);
+  if ((e = cudaFuncSetAttribute(k_fft_y<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(k_fft_y<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(k_fft_x_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(k_fft_x_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;
+  int sms = 0;
+  if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->p.device)) != cudaSuccess) return e;
+  O->grid = sms > 0 ? sms : 148;
+  return cudaSuccess;
+}
+
+static FftXArgs x_args(dp_plan* P, int nfields) {
+  dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
+  FftXArgs A;
+  A.real = P->d_real; A.cplx = P->d_cplx; A.planes = (long long)nfields * P->p.nz;
+  A.nx = P->p.nx; A.ny = P->p.ny; A.M = P->p.nx / 2;
+  A.tw = O->d_tw_x; A.post = O->d_post_x; A.pos = O->d_pos_x; A.F = O->Fx; A.rb = O->rbx;
+  return A;
+}
+static FftYArgs y_args(dp_plan* P, int nfields) {
+  dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
+  FftYArgs A;
+  A.data = P->d_cplx; A.rows = (long long)nfields * P->p.nz * (P->p.nx / 2 + 1);
+  A.tw = O->d_tw_y; A.F = O->Fy; A.rb = O->rby;
+  return A;
+}
+static int grid_for(const dp_fft_own* O, long long nbatch) {
+  const long long need = (nbatch + NSLOT - 1) / NSLOT;
+  return (int)(need < O->grid ? (need < 1 ? 1 : need) : O->grid);
+}
+
+cudaError_t dp_fft_own_forward(dp_plan* P, int nfields, cudaStream_t st) {
+  dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
+  const FftXArgs X = x_args(P, nfields);
+  k_fft_x_fwd<<<grid_for(O, X.planes * (X.ny / X.rb)), FFT_THREADS, O->smem_x, st>>>(X);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const FftYArgs Y = y_args(P, nfields);
+  k_fft_y<false><<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb), FFT_THREADS, O->smem_y, st>>>(Y);
+  return cudaGetLastError();
+}
+
+cudaError_t dp_fft_own_inverse(dp_plan* P, int nfields, cudaStream_t st) {
+  dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
+  const FftYArgs Y = y_args(P, nfields);
+  k_fft_y<true><<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb), FFT_THREADS, O->smem_y, st>>>(Y);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return e;
+  const FftXArgs X = x_args(P, nfields);
+  k_fft_x_inv<<<grid_for(O, X.planes * (X.ny / X.rb)), FFT_THREADS, O->smem_x, st>>>(X);
+  return cudaGetLastError();
+}
+
+cudaError_t dp_fft_own_untranspose(dp_plan* P, double2* dst, cudaStream_t st) {
+  dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
+  k_fft_untranspose<<<1024, 256, 0, st>>>(P->d_cplx, dst, O->d_ky_of_pos, P->p.ny, P->p.nx / 2 + 1, P->nkxp, (long long)P->fields * P->p.nz);
+  return cudaGetLastError();
+}

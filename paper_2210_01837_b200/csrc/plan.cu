@@ -102,17 +102,25 @@ int run_pipeline(dp_plan* P, int n, const double* pos, const double* force, cons
   CK(dp_launch_spread(P, n, true, with_torque, st));
   if (prof) CK(cudaEventRecord(P->ev[2], st));
   if (last_stage >= 2) {
-    CKF(cufftSetStream(P->fft_fwd, st));
-    CKF(cufftExecD2Z(P->fft_fwd, P->d_real, (cufftDoubleComplex*)P->d_cplx));
-    if (with_torque) CKF(cufftExecD2Z(P->fft_fwd, P->d_real + 3 * P->real_field, (cufftDoubleComplex*)(P->d_cplx + 3 * P->cplx_field)));
+    if (P->own_fft) {
+      CK(dp_fft_own_forward(P, with_torque ? 6 : 3, st));
+    } else {
+      CKF(cufftSetStream(P->fft_fwd, st));
+      CKF(cufftExecD2Z(P->fft_fwd, P->d_real, (cufftDoubleComplex*)P->d_cplx));
+      if (with_torque) CKF(cufftExecD2Z(P->fft_fwd, P->d_real + 3 * P->real_field, (cufftDoubleComplex*)(P->d_cplx + 3 * P->cplx_field)));
+    }
   }
   if (prof) CK(cudaEventRecord(P->ev[3], st));
   if (last_stage >= 3) CK(dp_launch_solve(P, with_torque, want_omega, st));
   if (prof) CK(cudaEventRecord(P->ev[4], st));
   if (last_stage >= 4) {
-    CKF(cufftSetStream(P->fft_inv, st));
-    CKF(cufftExecZ2D(P->fft_inv, (cufftDoubleComplex*)P->d_cplx, P->d_real));
-    if (want_omega) CKF(cufftExecZ2D(P->fft_inv, (cufftDoubleComplex*)(P->d_cplx + 3 * P->cplx_field), P->d_real + 3 * P->real_field));
+    if (P->own_fft) {
+      CK(dp_fft_own_inverse(P, want_omega ? 6 : 3, st));
+    } else {
+      CKF(cufftSetStream(P->fft_inv, st));
+      CKF(cufftExecZ2D(P->fft_inv, (cufftDoubleComplex*)P->d_cplx, P->d_real));
+      if (want_omega) CKF(cufftExecZ2D(P->fft_inv, (cufftDoubleComplex*)(P->d_cplx + 3 * P->cplx_field), P->d_real + 3 * P->real_field));
+    }
   }
   if (prof) CK(cudaEventRecord(P->ev[5], st));
   if (last_stage >= 5) CK(dp_launch_interp(P, n, U, Omega, st));
@@ -167,6 +175,7 @@ int dp_destroy(dp_plan* P) {
   cudaSetDevice(P->p.device);
   if (P->last_stream || true) cudaDeviceSynchronize();
   if (P->fft_ok) { cufftDestroy(P->fft_fwd); cufftDestroy(P->fft_inv); }
+  dp_fft_own_destroy(P);
   void* bufs[] = {P->d_real, P->d_cplx, P->d_fft_work, P->d_znodes, P->d_zweights, P->d_pos_s, P->d_frc_s, P->d_trq_s, P->d_perm, P->d_meta, P->d_wrec,
                   P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_bin_start, P->d_flag};
   for (void* b : bufs) if (b) cudaFree(b);
@@ -196,6 +205,7 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   if (fabs(hx - hy) > 1e-12 * hx) return DP_EINVAL;
   if (!(p.beta_M > 0) || (p.use_torques && !(p.beta_D > 0))) return DP_EINVAL;
   if (p.max_particles < 1) return DP_EINVAL;
+  if (p.fft_backend != 0 && p.fft_backend != 1) return DP_EINVAL;
   if (p.wall_mode == DP_SLIT && p.w * hx > p.H) return DP_EINVAL;     // a kernel may overlap one wall, not both
   if ((double)p.nz * p.ny * (p.nx + 16) >= 2.0e9) return DP_EINVAL;    // 32-bit plane indexing inside the kernels
 
@@ -213,7 +223,8 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   P->nby = (p.ny + DP_TILE_Y - 1) / DP_TILE_Y;
   P->nbins = P->nbx * P->nby;
   P->real_field = (size_t)p.nz * p.ny * p.nx;
-  P->cplx_field = (size_t)p.nz * p.ny * P->nkxp;
+  P->own_fft = p.fft_backend == 0 && dp_fft_own_supported(p.nx, p.ny);
+  P->cplx_field = P->own_fft ? dp_fft_own_cplx_field(P) : (size_t)p.nz * p.ny * P->nkxp;
 
   int rc = DP_OK;
   cudaError_t ce = cudaSetDevice(p.device);
@@ -235,7 +246,12 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   TRY(dev_alloc(P, &P->d_bin_count, (size_t)P->nbins));
   TRY(dev_alloc(P, &P->d_bin_start, (size_t)P->nbins + 1));
   TRY(dev_alloc(P, &P->d_flag, (size_t)1));
-  TRY(make_fft(P));
+  if (P->own_fft) {
+    cudaError_t fe = dp_fft_own_create(P);
+    if (fe != cudaSuccess) { set_err(P, "dp_fft_own_create", cudaGetErrorString(fe)); dp_destroy(P); return DP_ECUDA; }
+  } else {
+    TRY(make_fft(P));
+  }
 
   // tables: nodes z_l and quadrature weights h^2 (H/2) w_l, w_l Clenshaw-Curtis:
   //   w_l = (2/N)(1/c~_l) sum_{n even} (1/c~_n) (2/(1-n^2)) cos(n l pi/N)
@@ -313,14 +329,29 @@ int dp_stage_ms(dp_plan* P, float* ms) {
 size_t dp_buffer_bytes(const dp_plan* P, int which) {
   if (!P) return 0;
   if (which == 0) return sizeof(double) * P->real_field * P->fields;
-  if (which == 1) return sizeof(double2) * P->cplx_field * P->fields;
+  if (which == 1) return sizeof(double2) * (size_t)P->p.nz * P->p.ny * P->nkxp * P->fields;     // natural layout, see dp.h
   return 0;
 }
+
+int dp_fft_backend(const dp_plan* P) { return P ? (P->own_fft ? 0 : 1) : -1; }
 
 int dp_copy_buffer_to_host(dp_plan* P, int which, void* host, size_t bytes) {
   if (!P || !host) return DP_EINVAL;
   if (bytes > dp_buffer_bytes(P, which) || dp_buffer_bytes(P, which) == 0) return DP_EINVAL;
   CK(cudaStreamSynchronize(P->last_stream));
+  if (which == 1 && P->own_fft) {
+    // the own FFT passes keep the half spectrum transposed with ky digit-reversed: hand out the natural layout
+    double2* tmp = nullptr;
+    const size_t full = dp_buffer_bytes(P, 1);
+    CK(cudaMalloc(&tmp, full));
+    cudaError_t e = cudaMemsetAsync(tmp, 0, full, P->last_stream);
+    if (e == cudaSuccess) e = dp_fft_own_untranspose(P, tmp, P->last_stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(P->last_stream);
+    if (e == cudaSuccess) e = cudaMemcpy(host, tmp, bytes, cudaMemcpyDeviceToHost);
+    cudaFree(tmp);
+    CK(e);
+    return DP_OK;
+  }
   CK(cudaMemcpy(host, which == 0 ? (const void*)P->d_real : (const void*)P->d_cplx, bytes, cudaMemcpyDeviceToHost));
   return DP_OK;
 }

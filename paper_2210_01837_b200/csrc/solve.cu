@@ -55,7 +55,8 @@ struct SolveArgs {
   size_t cplx_field;
   int nx, ny, nkx;
   int n_fast, n_slow, pitch;     // half spectrum stored as [field][l][slow][fast (pitch)]
-  int fast_is_x;                 // 1: fast index = kx index (cuFFT layout); 0: fast index = ky index (transposed layout)
+  int fast_is_x;                 // 1: fast index = kx index (cuFFT layout); 0: fast index = position along ky (transposed layout)
+  const int* ky_of_pos;          // transposed layout: FFT-order ky index stored at each position (digit reversal of the y pass), or null
   double Lx, Ly, H, eta;
   int wall_mode, torque, omega;
 };
@@ -411,8 +412,9 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int mode = lane >> 1, part = lane & 1;
   const int ifast = blockIdx.x * TM + mode, islow = blockIdx.y;
-  const int ix = A.fast_is_x ? ifast : islow, iy = A.fast_is_x ? islow : ifast;
   const bool valid = ifast < A.n_fast;
+  const int ix = A.fast_is_x ? ifast : islow;
+  const int iy = A.fast_is_x ? islow : ((A.ky_of_pos && valid) ? __ldg(A.ky_of_pos + ifast) : ifast);
   const bool zero_mode = (ix == 0 && iy == 0);
   const double s = 0.5 * A.H, inv_s = 1.0 / s, eta = A.eta;
   ModeK K;
@@ -750,7 +752,8 @@ cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega,
   SolveArgs A;
   A.cplx = P->d_cplx; A.cplx_field = P->cplx_field;
   A.nx = P->p.nx; A.ny = P->p.ny; A.nkx = P->nkx;
-  A.n_fast = P->nkx; A.n_slow = P->p.ny; A.pitch = P->nkxp; A.fast_is_x = 1;
+  A.n_fast = P->nkx; A.n_slow = P->p.ny; A.pitch = P->nkxp; A.fast_is_x = 1; A.ky_of_pos = nullptr;
+  if (P->own_fft) { A.n_fast = P->p.ny; A.n_slow = P->nkx; A.pitch = P->p.ny; A.fast_is_x = 0; A.ky_of_pos = dp_fft_own_ky_table(P); }
   A.Lx = P->p.Lx; A.Ly = P->p.Ly; A.H = P->p.H; A.eta = P->p.eta;
   A.wall_mode = P->p.wall_mode; A.torque = with_torque_field ? 1 : 0; A.omega = want_omega ? 1 : 0;
   cudaError_t e;
