@@ -17,6 +17,7 @@
 // split  X[k] = E[k] + W_nx^k O[k],  E = (Z[k] + conj Z[M-k])/2,  O = -i (Z[k] - conj Z[M-k])/2.
 #include <cstdint>
 #include <cstdio>
+#include <cstdlib>
 #include <vector>
 
 #include "common.cuh"
@@ -27,20 +28,28 @@ namespace {
 using namespace dpfft;
 
 constexpr int NSLOT = 2;
-constexpr int TPS = 320;                       // threads per slot (10 warps; 20 warps per SM leave 96 registers per thread): 270 / 240 / 288 lines per stage at n = 4320
+#ifndef DP_FFT_TPS
+#define DP_FFT_TPS 256
+#endif
+constexpr int TPS = DP_FFT_TPS;               // threads per slot
 constexpr int FFT_THREADS = NSLOT * TPS;
 constexpr int SLOT_ELEMS = 4320;               // complex elements a slot can hold (69 120 bytes)
 
 struct dp_fft_own {
   Factors Fx, Fy;            // M = nx/2 and ny
   int rbx = 1, rby = 1;      // rows per slot batch in the x and y passes
-  double2* d_tw_x = nullptr;   // exp(-2 pi i j / M), j < M
+  int off_x[MAX_STAGES] = {}, off_y[MAX_STAGES] = {}, ntw_x = 0, ntw_y = 0;   // per-stage twiddle tables (fft_engine.cuh)
+  double2* d_tw_x = nullptr;   // stage tables of the length-M transform
   double2* d_post_x = nullptr; // exp(-2 pi i k / nx), k <= M/2
-  double2* d_tw_y = nullptr;   // exp(-2 pi i j / ny), j < ny
+  double2* d_tw_y = nullptr;   // stage tables of the length-ny transform
   unsigned short* d_pos_x = nullptr;   // position of Z[k] after the forward x transform
   int* d_ky_of_pos = nullptr;          // FFT-order ky index held at position p of a transformed y row
   size_t smem_x = 0, smem_y = 0;
   int grid = 148;
+  void (*ky_fwd)(struct FftYArgs) = nullptr;
+  void (*ky_inv)(struct FftYArgs) = nullptr;
+  void (*kx_fwd)(struct FftXArgs) = nullptr;
+  void (*kx_inv)(struct FftXArgs) = nullptr;
 };
 
 // ---- PTX wrappers: mbarrier, bulk asynchronous copies, named barriers
@@ -71,13 +80,15 @@ __device__ __forceinline__ void bulk_store(void* gmem_dst, const void* smem_src,
   asm volatile("cp.async.bulk.commit_group;" ::: "memory");
 }
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_proxy() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void slot_barrier(int slot) { asm volatile("bar.sync %0, %1;" ::"r"(slot + 1), "r"(TPS) : "memory"); }
 
 struct FftYArgs {
   double2* data;          // rows of n complex numbers, contiguous
   long long rows;
-  const double2* tw;
+  const double2* tw;      // stage tables, ntw entries
+  int ntw, off[MAX_STAGES];
   Factors F;
   int rb;                 // rows per slot batch
 };
@@ -87,7 +98,8 @@ struct FftXArgs {
   double2* cplx;          // [planes][nkx][ny]
   long long planes;       // fields * nz
   int nx, ny, M;
-  const double2* tw;      // length M
+  const double2* tw;      // stage tables, ntw entries
+  int ntw, off[MAX_STAGES];
   const double2* post;    // length M/2 + 1
   const unsigned short* pos;
   Factors F;
@@ -96,82 +108,164 @@ struct FftXArgs {
 
 __host__ __device__ inline size_t align16(size_t b) { return (b + 15) / 16 * 16; }
 
+// hooks of edge_lines (called between the loads of a round and its arithmetic), plain values only
+struct MidNone { __device__ __forceinline__ void operator()(int, int) const {} };
+struct MidStoreDrained {      // forward y pass, round 0: the slot's previous bulk store has read the buffer
+  int slot, st;
+  __device__ __forceinline__ void operator()(int rd, int) const {
+    if (rd == 0) { if (st == 0) bulk_wait_read(); slot_barrier(slot); }
+  }
+};
+struct MidPrefetch {          // inverse y pass, last round: all inputs are in registers, refill the buffer with the next rows
+  int slot, st;
+  uint64_t* mbar;
+  void* buf;
+  const void* next;           // null: nothing left
+  unsigned bytes;
+  __device__ __forceinline__ void operator()(int rd, int nrounds) const {
+    if (rd == nrounds - 1) {
+      slot_barrier(slot);
+      if (st == 0 && next) { mbar_expect_tx(mbar, bytes); bulk_load(buf, next, bytes, mbar); }
+    }
+  }
+};
+
+// The kernels are templates on the factorisation <R0, R1, R2> of the hot sizes (no runtime dispatch, every index into the
+// argument arrays static, only three butterflies in the instruction stream); <0, 0, 0> is the general version that
+// reads the radices from its arguments.
+template <int R0, bool INV, class Mid>
+__device__ __forceinline__ void run_edge(int r0, const double2* src, double2* dst, const double2* tw1, int n, int rows, int tid, const Mid& mid) {
+  if constexpr (R0 > 0) edge_lines<R0, INV>(src, dst, tw1, n, rows, (size_t)n, (size_t)n, tid, TPS, mid);
+  else edge_dispatch<INV>(r0, src, dst, tw1, n, rows, (size_t)n, (size_t)n, tid, TPS, mid);
+}
+// the shared-memory stages after (forward) or before (inverse) the edge stage, with the slot's barrier between stages;
+// LAST_BARRIER: also after the final one
+template <int R0, int R1, int R2, bool INV, bool LAST_BARRIER, class FA>
+__device__ __forceinline__ void run_inner(const FA& A, double2* buf, const double2* tw, int n, int rows, int tid, int slot) {
+  if constexpr (R0 > 0) {
+    constexpr int S1 = R2;                       // stride of stage 1 (n = R0 R1 R2)
+    if (!INV) {
+      stage_lines<R1, false>(buf, tw + A.off[1], n, S1, rows, n, tid, TPS);
+      slot_barrier(slot);
+      stage_lines<R2, false>(buf, tw + A.off[2], n, 1, rows, n, tid, TPS);
+      if (LAST_BARRIER) slot_barrier(slot);
+    } else {
+      stage_lines<R2, true>(buf, tw + A.off[2], n, 1, rows, n, tid, TPS);
+      slot_barrier(slot);
+      stage_lines<R1, true>(buf, tw + A.off[1], n, S1, rows, n, tid, TPS);
+      if (LAST_BARRIER) slot_barrier(slot);
+    }
+  } else if (!INV) {
+    int S = n / A.F.r[0];
+    for (int j = 1; j < A.F.ns; ++j) {
+      S /= A.F.r[j];
+      stage_dispatch<false>(A.F.r[j], buf, tw + A.off[j], n, S, rows, n, tid, TPS);
+      if (LAST_BARRIER || j + 1 < A.F.ns) slot_barrier(slot);
+    }
+  } else {
+    int S = 1;
+    for (int j = A.F.ns - 1; j >= 1; --j) {
+      stage_dispatch<true>(A.F.r[j], buf, tw + A.off[j], n, S, rows, n, tid, TPS);
+      S *= A.F.r[j];
+      if (LAST_BARRIER || j > 1) slot_barrier(slot);
+    }
+  }
+}
+
 // ---------------------------------------------------------------------------------------------- pass Y (in place)
-template <bool INV>
-__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_y(FftYArgs A) {
+// Forward: the first stage reads the row from global memory (edge_lines), the other stages run in shared memory, the
+// result leaves with one bulk store.  While a slot's bulk store drains, its next row's global loads are already in
+// flight; the stage-1 results are written to shared memory only after the store has finished reading it.
+template <int R0, int R1, int R2>
+__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_y_fwd(FftYArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int n = A.F.n;
   double2* tw = reinterpret_cast<double2*>(smem_raw);
   const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
-  double2* buf = tw + n + (size_t)slot * A.rb * n;
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(tw + n + (size_t)NSLOT * A.rb * n) + slot;
-  for (int i = threadIdx.x; i < n; i += FFT_THREADS) tw[i] = A.tw[i];
-  if (st == 0) mbar_init(mbar, 1);
-  fence_async_proxy();
+  double2* buf = tw + A.ntw + (size_t)slot * A.rb * n;
+  for (int i = threadIdx.x; i < A.ntw; i += FFT_THREADS) tw[i] = A.tw[i];
   __syncthreads();
-  unsigned phase = 0;
   const long long nbatch = (A.rows + A.rb - 1) / A.rb;
   for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
     const long long row0 = b * A.rb;
     const int nr = (int)((A.rows - row0) < A.rb ? (A.rows - row0) : A.rb);
     double2* g = A.data + row0 * n;
-    const unsigned bytes = (unsigned)nr * n * 16u;
-    if (st == 0) { mbar_expect_tx(mbar, bytes); bulk_load(buf, g, bytes, mbar); }
-    mbar_wait(mbar, phase);
-    phase ^= 1;
-    if (!INV) {
-      int S = n;
-      for (int j = 0; j < A.F.ns; ++j) {
-        S /= A.F.r[j];
-        stage_dispatch<false>(A.F.r[j], buf, tw, n, S, nr, n, st, TPS);
-        if (j + 1 < A.F.ns) slot_barrier(slot);
-      }
-    } else {
-      int S = 1;
-      for (int j = A.F.ns - 1; j >= 0; --j) {
-        stage_dispatch<true>(A.F.r[j], buf, tw, n, S, nr, n, st, TPS);
-        S *= A.F.r[j];
-        if (j > 0) slot_barrier(slot);
-      }
-    }
+    const MidStoreDrained mid{slot, st};
+    run_edge<R0, false>(A.F.r[0], g, buf, tw + A.off[0], n, nr, st, mid);
+    slot_barrier(slot);
+    run_inner<R0, R1, R2, false, false>(A, buf, tw, n, nr, st, slot);
     fence_async_proxy();
     slot_barrier(slot);
-    if (st == 0) { bulk_store(g, buf, bytes); bulk_wait_read(); }
+    if (st == 0) bulk_store(g, buf, (unsigned)nr * n * 16u);
   }
+  if (st == 0) bulk_wait_all();
 }
 
-// ---------------------------------------------------------------------------------------------- pass X forward
-__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
+// Inverse: the row arrives with one bulk load, all stages but the last run in shared memory, the last stage (largest
+// stride) stores its results straight to global memory.  As soon as that stage has read the row, the slot's next bulk
+// load is issued, so it flies during the last stage's arithmetic and stores.
+template <int R0, int R1, int R2>
+__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_y_inv(FftYArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
-  const int M = A.M, npost = M / 2 + 1;
+  const int n = A.F.n;
   double2* tw = reinterpret_cast<double2*>(smem_raw);
-  double2* post = tw + M;
   const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
-  double2* buf = post + npost + (size_t)slot * A.rb * M;
-  unsigned short* pos = reinterpret_cast<unsigned short*>(post + npost + (size_t)NSLOT * A.rb * M);
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(reinterpret_cast<unsigned char*>(pos) + align16(sizeof(unsigned short) * M)) + slot;
-  for (int i = threadIdx.x; i < M; i += FFT_THREADS) { tw[i] = A.tw[i]; pos[i] = A.pos[i]; }
-  for (int i = threadIdx.x; i < npost; i += FFT_THREADS) post[i] = A.post[i];
+  double2* buf = tw + A.ntw + (size_t)slot * A.rb * n;
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(tw + A.ntw + (size_t)NSLOT * A.rb * n) + slot;
+  for (int i = threadIdx.x; i < A.ntw; i += FFT_THREADS) tw[i] = A.tw[i];
   if (st == 0) mbar_init(mbar, 1);
   fence_async_proxy();
   __syncthreads();
   unsigned phase = 0;
+  const long long nbatch = (A.rows + A.rb - 1) / A.rb;
+  const long long stride = (long long)gridDim.x * NSLOT;
+  long long b = (long long)blockIdx.x * NSLOT + slot;
+  if (st == 0 && b < nbatch) {
+    const long long row0 = b * A.rb;
+    const int nr = (int)((A.rows - row0) < A.rb ? (A.rows - row0) : A.rb);
+    mbar_expect_tx(mbar, (unsigned)nr * n * 16u);
+    bulk_load(buf, A.data + row0 * n, (unsigned)nr * n * 16u, mbar);
+  }
+  for (; b < nbatch; b += stride) {
+    const long long row0 = b * A.rb;
+    const int nr = (int)((A.rows - row0) < A.rb ? (A.rows - row0) : A.rb);
+    double2* g = A.data + row0 * n;
+    mbar_wait(mbar, phase);
+    phase ^= 1;
+    run_inner<R0, R1, R2, true, true>(A, buf, tw, n, nr, st, slot);
+    const long long nrow0 = (b + stride) * A.rb;
+    const bool more = b + stride < nbatch;
+    const int nnr = more ? (int)((A.rows - nrow0) < A.rb ? (A.rows - nrow0) : A.rb) : 0;
+    const MidPrefetch mid{slot, st, mbar, buf, more ? (const void*)(A.data + nrow0 * n) : nullptr, (unsigned)nnr * n * 16u};
+    run_edge<R0, true>(A.F.r[0], buf, g, tw + A.off[0], n, nr, st, mid);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- pass X forward
+template <int R0, int R1, int R2>
+__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  const int M = A.M, npost = M / 2 + 1;
+  double2* tw = reinterpret_cast<double2*>(smem_raw);
+  double2* post = tw + A.ntw;
+  const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
+  double2* buf = post + npost + (size_t)slot * A.rb * M;
+  unsigned short* pos = reinterpret_cast<unsigned short*>(post + npost + (size_t)NSLOT * A.rb * M);
+  for (int i = threadIdx.x; i < A.ntw; i += FFT_THREADS) tw[i] = A.tw[i];
+  for (int i = threadIdx.x; i < M; i += FFT_THREADS) pos[i] = A.pos[i];
+  for (int i = threadIdx.x; i < npost; i += FFT_THREADS) post[i] = A.post[i];
+  __syncthreads();
   const int rb = A.rb, ny = A.ny, nkx = M + 1;
   const long long nbatch = A.planes * (ny / rb);
-  const unsigned bytes = (unsigned)rb * A.nx * 8u;
+  const MidNone nomid;
   for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
     const long long row0 = b * rb;                       // flat row index over (plane, y)
     const long long pl = row0 / ny;
     const int y0 = (int)(row0 - pl * ny);
-    if (st == 0) { mbar_expect_tx(mbar, bytes); bulk_load(buf, A.real + row0 * A.nx, bytes, mbar); }
-    mbar_wait(mbar, phase);
-    phase ^= 1;
-    int S = M;
-    for (int j = 0; j < A.F.ns; ++j) {
-      S /= A.F.r[j];
-      stage_dispatch<false>(A.F.r[j], buf, tw, M, S, rb, M, st, TPS);
-      slot_barrier(slot);
-    }
+    // a real row of nx doubles is read as M complex numbers z[m] = x[2m] + i x[2m+1]
+    run_edge<R0, false>(A.F.r[0], reinterpret_cast<const double2*>(A.real + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
+    slot_barrier(slot);
+    run_inner<R0, R1, R2, false, true>(A, buf, tw, M, rb, st, slot);
     // split into the spectra of the real rows and write them transposed: T[pl][kx][y0 + r]
     double2* out = A.cplx + (size_t)pl * nkx * ny + y0;
     for (int idx = st; idx < npost * rb; idx += TPS) {
@@ -184,25 +278,27 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
       out[(size_t)k * ny + r] = cadd(E, B);
       if (2 * k != M) out[(size_t)(M - k) * ny + r] = make_double2(E.x - B.x, -(E.y - B.y));
     }
-    slot_barrier(slot);                                  // every read of buf is done before the next bulk load lands
+    slot_barrier(slot);                                  // every read of buf is done before the next batch overwrites it
   }
 }
 
 // ---------------------------------------------------------------------------------------------- pass X inverse
+template <int R0, int R1, int R2>
 __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_inv(FftXArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int M = A.M, npost = M / 2 + 1;
   double2* tw = reinterpret_cast<double2*>(smem_raw);
-  double2* post = tw + M;
+  double2* post = tw + A.ntw;
   const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
   double2* buf = post + npost + (size_t)slot * A.rb * M;
   unsigned short* pos = reinterpret_cast<unsigned short*>(post + npost + (size_t)NSLOT * A.rb * M);
-  for (int i = threadIdx.x; i < M; i += FFT_THREADS) { tw[i] = A.tw[i]; pos[i] = A.pos[i]; }
+  for (int i = threadIdx.x; i < A.ntw; i += FFT_THREADS) tw[i] = A.tw[i];
+  for (int i = threadIdx.x; i < M; i += FFT_THREADS) pos[i] = A.pos[i];
   for (int i = threadIdx.x; i < npost; i += FFT_THREADS) post[i] = A.post[i];
   __syncthreads();
   const int rb = A.rb, ny = A.ny, nkx = M + 1;
   const long long nbatch = A.planes * (ny / rb);
-  const unsigned bytes = (unsigned)rb * A.nx * 8u;
+  const MidNone nomid;
   for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
     const long long row0 = b * rb;
     const long long pl = row0 / ny;
@@ -223,16 +319,10 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_inv(FftXArgs A) {
       }
     }
     slot_barrier(slot);
-    int S = 1;
-    for (int j = A.F.ns - 1; j >= 0; --j) {
-      stage_dispatch<true>(A.F.r[j], buf, tw, M, S, rb, M, st, TPS);
-      S *= A.F.r[j];
-      if (j > 0) slot_barrier(slot);
-    }
-    fence_async_proxy();
-    slot_barrier(slot);
-    if (st == 0) { bulk_store(A.real + row0 * A.nx, buf, bytes); bulk_wait_read(); }
-    slot_barrier(slot);                                  // the store has read buf before anyone refills it
+    run_inner<R0, R1, R2, true, true>(A, buf, tw, M, rb, st, slot);
+    // last stage: results go straight to the real grid rows (z[m] = x[2m] + i x[2m+1])
+    run_edge<R0, true>(A.F.r[0], buf, reinterpret_cast<double2*>(A.real + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
+    slot_barrier(slot);                                  // the stage has read buf before the next batch refills it
   }
 }
 
@@ -249,6 +339,26 @@ __global__ void k_fft_untranspose(const double2* __restrict__ T, double2* __rest
   }
 }
 
+
+// kernel selection: the static instantiations cover the three-stage factorisations of the benchmark sizes
+// (4320: 16.18.15, 2160: 16.9.15, 1080: 8.9.15, 540: 4.9.15); anything else runs the general kernel
+#define DP_FFT_STATIC_LIST(X) X(16, 18, 15) X(16, 9, 15) X(8, 9, 15) X(4, 9, 15)
+inline bool is3(const Factors& F, int a, int b, int c) { return F.ns == 3 && F.r[0] == a && F.r[1] == b && F.r[2] == c; }
+typedef void (*KernelY)(FftYArgs);
+typedef void (*KernelX)(FftXArgs);
+KernelY pick_y(const Factors& F, bool inv) {
+#define X(a, b, c) if (is3(F, a, b, c)) return inv ? k_fft_y_inv<a, b, c> : k_fft_y_fwd<a, b, c>;
+  DP_FFT_STATIC_LIST(X)
+#undef X
+  return inv ? k_fft_y_inv<0, 0, 0> : k_fft_y_fwd<0, 0, 0>;
+}
+KernelX pick_x(const Factors& F, bool inv) {
+#define X(a, b, c) if (is3(F, a, b, c)) return inv ? k_fft_x_inv<a, b, c> : k_fft_x_fwd<a, b, c>;
+  DP_FFT_STATIC_LIST(X)
+#undef X
+  return inv ? k_fft_x_inv<0, 0, 0> : k_fft_x_fwd<0, 0, 0>;
+}
+
 template <class T> cudaError_t upload(T** dst, const std::vector<T>& v, dp_plan* P) {
   cudaError_t e = cudaMalloc((void**)dst, sizeof(T) * v.size());
   if (e != cudaSuccess) return e;
@@ -256,9 +366,27 @@ template <class T> cudaError_t upload(T** dst, const std::vector<T>& v, dp_plan*
   return cudaMemcpy(*dst, v.data(), sizeof(T) * v.size(), cudaMemcpyHostToDevice);
 }
 
-size_t smem_bytes_y(int n, int rb) { return sizeof(double2) * ((size_t)n + (size_t)NSLOT * rb * n) + 8 * NSLOT; }
-size_t smem_bytes_x(int M, int rb) {
-  return sizeof(double2) * ((size_t)M + (M / 2 + 1) + (size_t)NSLOT * rb * M) + align16(sizeof(unsigned short) * M) + 8 * NSLOT;
+size_t smem_bytes_y(int n, int ntw, int rb) { return sizeof(double2) * ((size_t)ntw + (size_t)NSLOT * rb * n) + 8 * NSLOT; }
+size_t smem_bytes_x(int M, int ntw, int rb) {
+  return sizeof(double2) * ((size_t)ntw + (M / 2 + 1) + (size_t)NSLOT * rb * M) + align16(sizeof(unsigned short) * M) + 8 * NSLOT;
+}
+
+// tuning override: DP_FFT_FACTORS_X / DP_FFT_FACTORS_Y = comma-separated radices (product must equal the length)
+bool factors_from_env(const char* name, int n, Factors* F) {
+  const char* e = getenv(name);
+  if (!e || !*e) return false;
+  Factors G; G.n = n; G.ns = 0;
+  long prod = 1;
+  while (*e && G.ns < MAX_STAGES) {
+    char* end = nullptr;
+    const long r = strtol(e, &end, 10);
+    if (end == e || !radix_supported((int)r)) return false;
+    G.r[G.ns++] = (int)r; prod *= r;
+    e = (*end == ',') ? end + 1 : end;
+  }
+  if (prod != n || *e) return false;
+  *F = G;
+  return true;
 }
 
 }  // namespace
@@ -288,6 +416,8 @@ cudaError_t dp_fft_own_create(dp_plan* P) {
   dp_fft_own* O = new dp_fft_own();
   P->fft_own = O;
   if (!factorize(M, &O->Fx) || !factorize(ny, &O->Fy)) return cudaErrorInvalidValue;
+  factors_from_env("DP_FFT_FACTORS_X", M, &O->Fx);
+  factors_from_env("DP_FFT_FACTORS_Y", ny, &O->Fy);
   // rows per slot batch: as many as fit the slot; in the x passes the batch must tile a plane's ny rows
   O->rby = SLOT_ELEMS / ny < 1 ? 1 : SLOT_ELEMS / ny;
   int rbmax = SLOT_ELEMS / M;                // <= 2 rows at nx = 4320: a batch is rb * nx doubles = rb * M complex
@@ -295,10 +425,12 @@ cudaError_t dp_fft_own_create(dp_plan* P) {
   if (rbmax > 64) rbmax = 64;
   O->rbx = 1;
   for (int r = rbmax; r >= 1; --r) if (ny % r == 0) { O->rbx = r; break; }
-  std::vector<double2> twx(M), post(M / 2 + 1), twy(ny);
-  for (int j = 0; j < M; ++j) twx[j] = make_double2((double)cosl(2 * PI * j / M), (double)-sinl(2 * PI * j / M));
+  O->ntw_x = stage_tables(O->Fx, O->off_x, nullptr, true);
+  O->ntw_y = stage_tables(O->Fy, O->off_y, nullptr, true);
+  std::vector<double2> twx(O->ntw_x + 1), post(M / 2 + 1), twy(O->ntw_y + 1);
+  stage_tables(O->Fx, O->off_x, twx.data(), true);
+  stage_tables(O->Fy, O->off_y, twy.data(), true);
   for (int k = 0; k <= M / 2; ++k) post[k] = make_double2((double)cosl(2 * PI * k / nx), (double)-sinl(2 * PI * k / nx));
-  for (int j = 0; j < ny; ++j) twy[j] = make_double2((double)cosl(2 * PI * j / ny), (double)-sinl(2 * PI * j / ny));
   std::vector<unsigned short> posx(M);
   for (int k = 0; k < M; ++k) posx[k] = (unsigned short)position_of(O->Fx, k);
   std::vector<int> kyp(ny);
@@ -309,12 +441,15 @@ cudaError_t dp_fft_own_create(dp_plan* P) {
   if ((e = upload(&O->d_tw_y, twy, P)) != cudaSuccess) return e;
   if ((e = upload(&O->d_pos_x, posx, P)) != cudaSuccess) return e;
   if ((e = upload(&O->d_ky_of_pos, kyp, P)) != cudaSuccess) return e;
-  O->smem_x = smem_bytes_x(M, O->rbx);
-  O->smem_y = smem_bytes_y(ny, O->rby);
-  if ((e = cudaFuncSetAttribute(k_fft_y<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(k_fft_y<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(k_fft_x_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(k_fft_x_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;
+  O->smem_x = smem_bytes_x(M, O->ntw_x, O->rbx);
+  O->smem_y = smem_bytes_y(ny, O->ntw_y, O->rby);
+  if (O->smem_x > 227 * 1024 || O->smem_y > 227 * 1024) return cudaErrorInvalidValue;
+  O->ky_fwd = pick_y(O->Fy, false); O->ky_inv = pick_y(O->Fy, true);
+  O->kx_fwd = pick_x(O->Fx, false); O->kx_inv = pick_x(O->Fx, true);
+  if ((e = cudaFuncSetAttribute(O->ky_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(O->ky_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(O->kx_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(O->kx_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;
   int sms = 0;
   if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->p.device)) != cudaSuccess) return e;
   O->grid = sms > 0 ? sms : 148;
@@ -326,14 +461,16 @@ static FftXArgs x_args(dp_plan* P, int nfields) {
   FftXArgs A;
   A.real = P->d_real; A.cplx = P->d_cplx; A.planes = (long long)nfields * P->p.nz;
   A.nx = P->p.nx; A.ny = P->p.ny; A.M = P->p.nx / 2;
-  A.tw = O->d_tw_x; A.post = O->d_post_x; A.pos = O->d_pos_x; A.F = O->Fx; A.rb = O->rbx;
+  A.tw = O->d_tw_x; A.ntw = O->ntw_x; A.post = O->d_post_x; A.pos = O->d_pos_x; A.F = O->Fx; A.rb = O->rbx;
+  for (int j = 0; j < MAX_STAGES; ++j) A.off[j] = O->off_x[j];
   return A;
 }
 static FftYArgs y_args(dp_plan* P, int nfields) {
   dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
   FftYArgs A;
   A.data = P->d_cplx; A.rows = (long long)nfields * P->p.nz * (P->p.nx / 2 + 1);
-  A.tw = O->d_tw_y; A.F = O->Fy; A.rb = O->rby;
+  A.tw = O->d_tw_y; A.ntw = O->ntw_y; A.F = O->Fy; A.rb = O->rby;
+  for (int j = 0; j < MAX_STAGES; ++j) A.off[j] = O->off_y[j];
   return A;
 }
 static int grid_for(const dp_fft_own* O, long long nbatch) {
@@ -344,22 +481,22 @@ static int grid_for(const dp_fft_own* O, long long nbatch) {
 cudaError_t dp_fft_own_forward(dp_plan* P, int nfields, cudaStream_t st) {
   dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
   const FftXArgs X = x_args(P, nfields);
-  k_fft_x_fwd<<<grid_for(O, X.planes * (X.ny / X.rb)), FFT_THREADS, O->smem_x, st>>>(X);
+  O->kx_fwd<<<grid_for(O, X.planes * (X.ny / X.rb)), FFT_THREADS, O->smem_x, st>>>(X);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   const FftYArgs Y = y_args(P, nfields);
-  k_fft_y<false><<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb), FFT_THREADS, O->smem_y, st>>>(Y);
+  O->ky_fwd<<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb), FFT_THREADS, O->smem_y, st>>>(Y);
   return cudaGetLastError();
 }
 
 cudaError_t dp_fft_own_inverse(dp_plan* P, int nfields, cudaStream_t st) {
   dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
   const FftYArgs Y = y_args(P, nfields);
-  k_fft_y<true><<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb), FFT_THREADS, O->smem_y, st>>>(Y);
+  O->ky_inv<<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb), FFT_THREADS, O->smem_y, st>>>(Y);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   const FftXArgs X = x_args(P, nfields);
-  k_fft_x_inv<<<grid_for(O, X.planes * (X.ny / X.rb)), FFT_THREADS, O->smem_x, st>>>(X);
+  O->kx_inv<<<grid_for(O, X.planes * (X.ny / X.rb)), FFT_THREADS, O->smem_x, st>>>(X);
   return cudaGetLastError();
 }
 
