@@ -30,7 +30,12 @@ import numpy as np
 import workloads
 
 METRIC = "ms per DP-wall mobility product M·F at N=1M; particles/s; % of HBM roofline"
-MY_KERNELS_PER_STEP = 7      # k_bin_count, k_scan, k_bin_scatter, k_spread, k_solve<nz>, k_zero_mode, k_interp (+ cuFFT's own)
+# kernels of this library launched per product: k_bin_count, k_scan, k_bin_scatter, k_weights, k_spread, k_solve<nz>, k_zero_mode,
+# k_interp, plus k_fft_x_fwd, k_fft_y_fwd, k_fft_y_inv, k_fft_x_inv with the library's own FFT passes (else cuFFT's kernels)
+MY_KERNELS_PER_STEP = {"own": 12, "cufft": 8}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one launch, from the committed ncu --set full capture
+# (profiles/r1_c_full_summary.md); None where no capture exists for that workload
+NCU_TRAFFIC_GB = {("k_solve<32>", 5): 57.63}
 
 
 def hbm_peak():
@@ -145,6 +150,7 @@ def main():
     ap.add_argument("--impl", default="b200")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--fft", choices=["own", "cufft"], default="own", help="xy FFT backend (own shared-memory passes, or cuFFT for comparison)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
@@ -177,7 +183,8 @@ def main():
     n = len(pos)
     fin = 6 if T is not None else 3
     fout = fin
-    plan = dp.Plan(prob, max_particles=n, use_torques=T is not None, device=local_rank)
+    plan = dp.Plan(prob, max_particles=n, use_torques=T is not None, device=local_rank, fft_backend=0 if args.fft == "own" else 1)
+    fft_backend = plan.fft_backend()
     dpos = torch.from_numpy(pos).to(dev)
     dF = torch.from_numpy(F).to(dev)
     dT = torch.from_numpy(T).to(dev) if T is not None else None
@@ -262,8 +269,10 @@ def main():
     kernel_name = {"spread": "k_spread", "solve": "k_solve<%d>" % prob.nz, "interp": "k_interp"}[dom]
     mid = sum(by[k] for k in ("fft_fwd", "solve", "fft_inv")) / 1e9
     mid_ms = sum(stage_ms.get(k, 0.0) for k in ("fft_fwd", "solve", "fft_inv"))
+    traffic = NCU_TRAFFIC_GB.get((kernel_name, args.config))
     roofline = {"bound": "hbm", "kernel": kernel_name, "achieved": mine[dom]["GBps"], "peak": peak, "unit": "GB/s",
-                "frac": mine[dom]["frac"], "traffic": None, "peak_source": peak_src,
+                "frac": mine[dom]["frac"], "traffic": traffic * 1e9 if traffic else None, "peak_source": peak_src,
+                "note": "k_solve is co-bound by the fp64 pipe and shared memory (profiles/r1_c_full_summary.md); the fraction is of the HBM roofline",
                 "fft_chebyshev_solve_stages": {"algorithmic_GB": mid, "ms": mid_ms, "GBps": mid / (mid_ms * 1e-3) if mid_ms else None,
                                                "frac": (mid / (mid_ms * 1e-3) / peak) if mid_ms else None},
                 "whole_product": {"algorithmic_GB": sum(by.values()) / 1e9, "ms": ms_step,
@@ -279,8 +288,9 @@ def main():
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": dict(workloads_describe(args.config), n_particles=n, grid=[prob.nx, prob.ny, prob.nz], wall_mode=["bottom_wall", "slit"][prob.wall_mode],
                            fields_in=fin, fields_out=fout, w=prob.w, l2="inputs (%.1f GB of grids per product) far exceed the 126 MB L2" % (sum(by.values()) / 1e9 / 4),
-                           parallelism="replicas" if world > 1 else "single GPU", plan_device_GB=plan.device_bytes() / 1e9),
-            "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": MY_KERNELS_PER_STEP * args.steps,
+                           parallelism="replicas" if world > 1 else "single GPU", plan_device_GB=plan.device_bytes() / 1e9,
+                           fft_backend=fft_backend),
+            "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": MY_KERNELS_PER_STEP[fft_backend] * args.steps,
             "stages": stages, "roofline": roofline, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     plan.close()

@@ -9,10 +9,13 @@
 //             pass X: gather T[f][l][:][y] -> complex-to-real FFT along x -> real grid row
 //
 // Each pass reads every grid value once and writes it once (4 passes per product and field instead of the ten of the
-// library's multi-kernel plans at 4320 x 4320).  A row lives in shared memory for its whole transform (fft_engine.cuh);
-// contiguous rows move with bulk asynchronous copies (cp.async.bulk + mbarrier), so no thread spends registers or issue
-// slots on them; one persistent CTA per SM holds the twiddle table and two independent row slots (320 threads each,
-// named barriers), so that one slot's copies overlap the other slot's butterflies.
+// library's multi-kernel plans at 4320 x 4320).  A row (or a batch of short rows) lives in shared memory for its whole
+// transform (fft_engine.cuh).  One persistent CTA per SM holds the small twiddle tables and two independent row slots
+// (256 threads each, named barriers, 128 registers per thread), so that one slot's memory phases overlap the other slot's
+// butterflies.  The stage with the largest stride exchanges its data directly with global memory (coalesced: consecutive
+// threads take consecutive elements); the other side of the y passes is one bulk asynchronous copy per row
+// (cp.async.bulk + mbarrier), prefetched in the inverse pass; the other side of the x passes is the transposed
+// scatter / gather of 16-byte elements (rb consecutive y per kx).
 // The real transform of length nx is a complex transform of length M = nx/2 on z[m] = x[2m] + i x[2m+1] with the usual
 // split  X[k] = E[k] + W_nx^k O[k],  E = (Z[k] + conj Z[M-k])/2,  O = -i (Z[k] - conj Z[M-k])/2.
 #include <cstdint>
@@ -304,11 +307,9 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_inv(FftXArgs A) {
     const long long pl = row0 / ny;
     const int y0 = (int)(row0 - pl * ny);
     const double2* in = A.cplx + (size_t)pl * nkx * ny + y0;
-    // Z'[k] = (X[k] + conj X[M-k]) + i conj(W^k) (X[k] - conj X[M-k]) at its digit-reversed position (unnormalised C2R)
-#pragma unroll 4
-    for (int idx = st; idx < npost * rb; idx += TPS) {
-      const int k = idx / rb, r = idx - k * rb;
-      const double2 X1 = __ldg(in + (size_t)k * ny + r), X2 = __ldg(in + (size_t)(M - k) * ny + r);
+    // Z'[k] = (X[k] + conj X[M-k]) + i conj(W^k) (X[k] - conj X[M-k]) at its digit-reversed position (unnormalised C2R).
+    // All of a thread's gathered values are loaded before any is used: one round of global latency per batch.
+    auto put = [&](int k, int r, double2 X1, double2 X2) {
       if (k == 0) {
         buf[r * M + pos[0]] = make_double2(X1.x + X2.x, X1.x - X2.x);      // imaginary parts of X[0], X[M] are ignored
       } else {
@@ -316,6 +317,26 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_inv(FftXArgs A) {
         const double2 Bq = cmulc(D, post[k]);
         buf[r * M + pos[k]] = make_double2(Aa.x - Bq.y, Aa.y + Bq.x);
         if (2 * k != M) buf[r * M + pos[M - k]] = make_double2(Aa.x + Bq.y, Bq.x - Aa.y);
+      }
+    };
+    if constexpr (R0 > 0) {
+      constexpr int Ms = R0 * R1 * R2, RB = SLOT_ELEMS / Ms, ITEMS = (Ms / 2 + 1) * RB, NIT = (ITEMS + TPS - 1) / TPS;
+      double2 X1[NIT], X2[NIT];
+#pragma unroll
+      for (int i = 0; i < NIT; ++i) {
+        const int idx = st + i * TPS, k = idx / RB, r = idx - k * RB;
+        if (idx < ITEMS) { X1[i] = __ldg(in + (size_t)k * ny + r); X2[i] = __ldg(in + (size_t)(Ms - k) * ny + r); }
+      }
+#pragma unroll
+      for (int i = 0; i < NIT; ++i) {
+        const int idx = st + i * TPS, k = idx / RB, r = idx - k * RB;
+        if (idx < ITEMS) put(k, r, X1[i], X2[i]);
+      }
+    } else {
+#pragma unroll 4
+      for (int idx = st; idx < npost * rb; idx += TPS) {
+        const int k = idx / rb, r = idx - k * rb;
+        put(k, r, __ldg(in + (size_t)k * ny + r), __ldg(in + (size_t)(M - k) * ny + r));
       }
     }
     slot_barrier(slot);
@@ -342,7 +363,7 @@ __global__ void k_fft_untranspose(const double2* __restrict__ T, double2* __rest
 
 // kernel selection: the static instantiations cover the three-stage factorisations of the benchmark sizes
 // (4320: 16.18.15, 2160: 16.9.15, 1080: 8.9.15, 540: 4.9.15); anything else runs the general kernel
-#define DP_FFT_STATIC_LIST(X) X(16, 18, 15) X(16, 9, 15) X(8, 9, 15) X(4, 9, 15)
+#define DP_FFT_STATIC_LIST(X) X(16, 18, 15) X(16, 9, 15) X(8, 9, 15) X(4, 9, 15) X(18, 16, 15) X(18, 8, 15)
 inline bool is3(const Factors& F, int a, int b, int c) { return F.ns == 3 && F.r[0] == a && F.r[1] == b && F.r[2] == c; }
 typedef void (*KernelY)(FftYArgs);
 typedef void (*KernelX)(FftXArgs);
@@ -352,8 +373,8 @@ KernelY pick_y(const Factors& F, bool inv) {
 #undef X
   return inv ? k_fft_y_inv<0, 0, 0> : k_fft_y_fwd<0, 0, 0>;
 }
-KernelX pick_x(const Factors& F, bool inv) {
-#define X(a, b, c) if (is3(F, a, b, c)) return inv ? k_fft_x_inv<a, b, c> : k_fft_x_fwd<a, b, c>;
+KernelX pick_x(const Factors& F, bool inv, int rb) {     // the static kernels assume rb = SLOT_ELEMS / M rows per batch
+#define X(a, b, c) if (is3(F, a, b, c) && rb == SLOT_ELEMS / (a * b * c)) return inv ? k_fft_x_inv<a, b, c> : k_fft_x_fwd<a, b, c>;
   DP_FFT_STATIC_LIST(X)
 #undef X
   return inv ? k_fft_x_inv<0, 0, 0> : k_fft_x_fwd<0, 0, 0>;
@@ -445,7 +466,7 @@ cudaError_t dp_fft_own_create(dp_plan* P) {
   O->smem_y = smem_bytes_y(ny, O->ntw_y, O->rby);
   if (O->smem_x > 227 * 1024 || O->smem_y > 227 * 1024) return cudaErrorInvalidValue;
   O->ky_fwd = pick_y(O->Fy, false); O->ky_inv = pick_y(O->Fy, true);
-  O->kx_fwd = pick_x(O->Fx, false); O->kx_inv = pick_x(O->Fx, true);
+  O->kx_fwd = pick_x(O->Fx, false, O->rbx); O->kx_inv = pick_x(O->Fx, true, O->rbx);
   if ((e = cudaFuncSetAttribute(O->ky_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(O->ky_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(O->kx_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;

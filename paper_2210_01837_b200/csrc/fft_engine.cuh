@@ -8,17 +8,14 @@
 // Whoever consumes the spectrum pointwise (the per-wavenumber solve) reads k from the position; nothing is reordered.
 // A line is one thread's work item; consecutive threads take consecutive m, so shared-memory accesses of a warp are
 // contiguous 16-byte elements except in the stage with S = 1, whose stride is r_s elements (conflict free for odd r_s).
-// The twiddles of stage j come from that stage's own table  tw_j[(t-1) S + m] = W_L^{t m}  (t = 1..r_j-1, m < S), again
-// contiguous in m; all stage tables together hold fewer than N entries (stage_tables()).
+// The twiddles of an inner stage j come from that stage's own table  tw_j[(t-1) S + m] = W_L^{t m}  (t = 1..r_j-1, m < S),
+// again contiguous in m.  The stage with the largest stride (j = 1) moves its data straight between global and shared
+// memory (edge_lines) and generates its twiddles by recurrence from W_N^m, so all tables together are a few KB.
 #pragma once
 
 #include <cmath>
 
 #include "fft_radix.cuh"
-
-#ifndef DP_FFT_PAIRS
-#define DP_FFT_PAIRS 0
-#endif
 
 namespace dpfft {
 
@@ -62,98 +59,6 @@ DP_HD void stage_lines(double2* __restrict__ buf, const double2* __restrict__ tw
 }
 
 
-// ---- a line of radix 16 or 18 shared by two adjacent threads (h = 0, 1): 2 x R2 decomposition with the radix-2 step
-// first.  Each thread reads all R inputs (the partner reads the same addresses in the same instruction, so the shared-
-// memory wavefronts are not doubled), folds them into its own R2 values, runs the R2-point DFT and stores R2 outputs:
-//   16 = 2 x 8, Cooley-Tukey:  y[n2] = (x[n2] +- x[8+n2]) W_16^{h n2},  X[h + 2 k2] = DFT_8(y)[k2]
-//   18 = 2 x 9, Good-Thomas:   y[n2] = x[(2 n2) % 18] +- x[(9 + 2 n2) % 18],  X[(9 h + 10 k2) % 18] = DFT_9(y)[k2]
-// Half the registers of a whole line (no spills at 96 registers per thread) and twice the threads per stage.
-template <int R> struct PairMap;
-template <> struct PairMap<16> {
-  static constexpr int R2 = 8;
-  static constexpr bool CT = true;
-  DP_HD static constexpr int in(int n1, int n2) { return 8 * n1 + n2; }
-  DP_HD static int out(int h, int k2) { return h + 2 * k2; }
-};
-template <> struct PairMap<18> {
-  static constexpr int R2 = 9;
-  static constexpr bool CT = false;
-  DP_HD static constexpr int in(int n1, int n2) { return (9 * n1 + 2 * n2) % 18; }
-  DP_HD static int out(int h, int k2) { const int o = (10 * k2) % 18 + 9 * h; return o >= 18 ? o - 18 : o; }
-};
-
-template <int R, bool INV>
-DP_HD void pair_load(const double2* __restrict__ p, const double2* __restrict__ w, int S, int h, double2 (&y)[PairMap<R>::R2]) {
-  typedef PairMap<R> PM;
-  constexpr int R2 = PM::R2;
-  const double sg = h ? -1.0 : 1.0;
-#pragma unroll
-  for (int n2 = 0; n2 < R2; ++n2) {
-    const int i0 = PM::in(0, n2), i1 = PM::in(1, n2);
-    double2 a = p[i0 * S], c = p[i1 * S];
-    if (INV && S > 1) {
-      if (i0 > 0) a = cmulc(a, w[i0 * S]);
-      c = cmulc(c, w[i1 * S]);
-    }
-    y[n2] = make_double2(fma(sg, c.x, a.x), fma(sg, c.y, a.y));
-    if (PM::CT && n2 > 0) {
-      // W_16^{h n2} (conjugated for the inverse): identity for h = 0
-      const double cs = h ? tw_cos16(n2) : 1.0, sn = h ? tw_sin16(n2) : 0.0;
-      y[n2] = INV ? cmulc(y[n2], make_double2(cs, -sn)) : cmul(y[n2], make_double2(cs, -sn));
-    }
-  }
-  Dft<R2, INV>::run(y);
-}
-
-template <int R, bool INV>
-DP_HD void pair_store(double2* __restrict__ p, const double2* __restrict__ w, int S, int h, const double2 (&y)[PairMap<R>::R2]) {
-  typedef PairMap<R> PM;
-#pragma unroll
-  for (int k2 = 0; k2 < PM::R2; ++k2) {
-    const int o = PM::out(h, k2);
-    double2 v = y[k2];
-    if (!INV && S > 1) { if (k2 > 0 || h) v = cmul(v, w[(o > 0 ? o : 1) * S]); }
-    p[o * S] = v;
-  }
-}
-
-// The two threads of a pair are adjacent lanes of one warp; all loads of the warp complete (__syncwarp) before any
-// thread stores into the line it shares.  (On the host the pair is simply processed together.)
-template <int R, bool INV>
-DP_HD void stage_pairs(double2* __restrict__ buf, const double2* __restrict__ tw, int n, int S, int rows, int row_stride, int tid, int nth) {
-  constexpr int R2 = PairMap<R>::R2;
-  const int per_row = n / R;
-  const int L = R * S;
-  const int total = 2 * rows * per_row;
-#ifdef __CUDA_ARCH__
-  for (int base = 0; base < total; base += nth) {
-    const int wid = base + tid;
-    const bool active = wid < total;
-    const int h = wid & 1, id = active ? (wid >> 1) : 0;
-    const int row = id / per_row, q = id - row * per_row;
-    const int b = q / S, m = q - b * S;
-    double2* p = buf + (size_t)row * row_stride + b * L + m;
-    const double2* w = tw + m - S;           // w[t S] = W_L^{t m}
-    double2 y[R2];
-    if (active) pair_load<R, INV>(p, w, S, h, y);
-    __syncwarp();
-    if (active) pair_store<R, INV>(p, w, S, h, y);
-  }
-#else
-  for (int id = tid; id < total / 2; id += nth) {
-    const int row = id / per_row, q = id - row * per_row;
-    const int b = q / S, m = q - b * S;
-    double2* p = buf + (size_t)row * row_stride + b * L + m;
-    const double2* w = tw + m - S;
-    double2 y0[R2], y1[R2];
-    pair_load<R, INV>(p, w, S, 0, y0);
-    pair_load<R, INV>(p, w, S, 1, y1);
-    pair_store<R, INV>(p, w, S, 0, y0);
-    pair_store<R, INV>(p, w, S, 1, y1);
-  }
-#endif
-}
-
 template <bool INV>
 DP_HD void stage_dispatch(int R, double2* buf, const double2* tw, int n, int S, int rows, int row_stride, int tid, int nth) {
   switch (R) {
@@ -164,13 +69,8 @@ DP_HD void stage_dispatch(int R, double2* buf, const double2* tw, int n, int S, 
     case 8: stage_lines<8, INV>(buf, tw, n, S, rows, row_stride, tid, nth); break;
     case 9: stage_lines<9, INV>(buf, tw, n, S, rows, row_stride, tid, nth); break;
     case 15: stage_lines<15, INV>(buf, tw, n, S, rows, row_stride, tid, nth); break;
-#if DP_FFT_PAIRS
-    case 16: stage_pairs<16, INV>(buf, tw, n, S, rows, row_stride, tid, nth); break;
-    case 18: stage_pairs<18, INV>(buf, tw, n, S, rows, row_stride, tid, nth); break;
-#else
     case 16: stage_lines<16, INV>(buf, tw, n, S, rows, row_stride, tid, nth); break;
     case 18: stage_lines<18, INV>(buf, tw, n, S, rows, row_stride, tid, nth); break;
-#endif
     default: break;
   }
 }

@@ -169,3 +169,95 @@ def test_create_rejects_bad_parameters(dp):
     for bad in (dict(nz=31), dict(nx=49), dict(w=3), dict(eta=0.0), dict(Ly=prob.Ly * 1.01), dict(nx=16, ny=16)):
         with pytest.raises(dp.DPError):
             dp.Plan(dataclasses.replace(prob, **bad), max_particles=8)
+
+
+# ------------------------------------------------------------------------------------------------ xy FFT passes
+def _rfft2(a):
+    return np.fft.rfft2(a, axes=(-2, -1))
+
+
+@pytest.mark.parametrize("kind,nxy,nz,n", [("bw", 216, 32, 1500), ("slit", 240, 48, 1500), ("bw", 50, 16, 64), ("bw", 1080, 16, 3000)])
+def test_own_fft_passes_match_the_dft_and_cufft(dp, kind, nxy, nz, n):
+    """The library's own xy FFT passes (transposed, digit-reversed half spectrum) against the unnormalised DFT definition
+    (numpy.fft.rfft2, the primitive the oracle's DFT is pinned to) and against the cuFFT backend; nxy = 50 cannot be
+    factored into the compiled radices' batch shapes differently: it exercises the general kernels, 1080 the static ones."""
+    L = nxy * (2.0 / 3.0)
+    mk = workloads.random_bw if kind == "bw" else workloads.random_slit
+    prob, pos, F, T = mk(n=n, L=L, nxy=nxy, nz=nz, H=8.0, seed=41, name="fft")
+    if nxy >= 1000:
+        T = None                                                     # three fields are enough at this size
+    dpos, dF, dT = to_dev(pos, F, T)
+    res = {}
+    for backend in (0, 1):
+        with dp.Plan(prob, max_particles=n, use_torques=T is not None, fft_backend=backend) as plan:
+            assert plan.fft_backend() == ("own" if backend == 0 else "cufft")
+            g = plan.debug_stage(dpos, dF, dT, 1)
+            gh = plan.debug_stage(dpos, dF, dT, 2)
+            assert rel_l2(gh, _rfft2(g)) < 1e-14
+            uh = plan.debug_stage(dpos, dF, dT, 3)
+            ur = plan.debug_stage(dpos, dF, dT, 4)
+            nf = 6 if T is not None else 3
+            back = np.fft.irfft2(uh[:nf], s=(prob.ny, prob.nx), axes=(-2, -1)) * (prob.nx * prob.ny)
+            assert rel_l2(ur[:nf], back) < 1e-13
+            U, Om = plan.mobility_apply(dpos, dF, dT)
+            res[backend] = U.cpu().numpy()
+    assert rel_l2(res[0], res[1]) < 1e-13
+
+
+def test_unsupported_fft_size_falls_back_to_cufft(dp):
+    prob, pos, F, T = workloads.random_bw(n=64, L=28 * (2.0 / 3.0), nxy=28, nz=16, H=8.0, seed=3, name="seven")   # 28 = 4 * 7
+    with dp.Plan(prob, max_particles=64, use_torques=False) as plan:
+        assert plan.fft_backend() == "cufft"
+        U_o, _ = oracle.mobility_apply(prob, pos, F, None, dft="fft")
+        U, _ = plan.mobility_apply(*to_dev(pos, F))
+        assert rel_l2(U.cpu().numpy(), U_o) < TOL
+
+
+def test_full_size_fft_passes_on_sampled_planes_and_backends_agree(dp):
+    """BASELINE config 5 (4320 x 4320 x 32, N = 1,048,576, the configuration bench.py times, same launch configuration):
+    the oracle cannot finish this size, so (i) sampled planes of the forward spectrum are compared with numpy's rfft2 of
+    the spread grid, (ii) the whole product is compared between the own FFT passes and the cuFFT backend, and (iii) the
+    properties that hold at any size are checked: U = 0 for a particle on the wall, and the product is linear."""
+    import torch
+    prob, pos, F, T = workloads.config(5)
+    n = len(pos)
+    pos = pos.copy()
+    pos[7, 2] = 0.0
+    dpos, dF, dT = to_dev(pos, F, T)
+    with dp.Plan(prob, max_particles=n, use_torques=True, fft_backend=0) as plan:
+        assert plan.fft_backend() == "own"
+        U, Om = plan.mobility_apply(dpos, dF, dT)
+        U2, Om2 = plan.mobility_apply(dpos, 2.0 * dF, 2.0 * dT)
+        torch.cuda.synchronize()
+        assert plan.check() == 0
+        U, Om, U2, Om2 = (t.cpu().numpy() for t in (U, Om, U2, Om2))
+        assert np.all(U[7] == 0.0) and np.all(Om[7] == 0.0)
+        assert rel_l2(U2, 2.0 * U) < 1e-13 and rel_l2(Om2, 2.0 * Om) < 1e-13
+        # sampled planes of the forward transform of field 0 (f_x), near the wall (only field 0 is copied to the host: 4.8 GB)
+        import ctypes
+        L = dp.load_library()
+        st = torch.cuda.current_stream()
+        ptr = lambda t: ctypes.c_void_p(t.data_ptr())
+        for stage, which in ((1, 0), (2, 1)):
+            rc = L.dp_debug_run_stage(plan._h, n, ptr(dpos), ptr(dF), ptr(dT), stage, ctypes.c_void_p(st.cuda_stream))
+            assert rc == 0
+            torch.cuda.synchronize()
+            if stage == 1:
+                planes = {}
+                real = np.empty((1, prob.nz, prob.ny, prob.nx))
+                assert L.dp_copy_buffer_to_host(plan._h, 0, real.ctypes.data_as(ctypes.c_void_p), real.nbytes) == 0
+                for f, l in ((0, prob.nz - 3), (0, prob.nz - 6)):
+                    assert np.abs(real[f, l]).max() > 0
+                    planes[(f, l)] = _rfft2(real[f, l])
+                del real
+            else:
+                pitch = int(L.dp_complex_row_pitch(plan._h))
+                spec = np.empty((1, prob.nz, prob.ny, pitch), dtype=np.complex128)
+                assert L.dp_copy_buffer_to_host(plan._h, 1, spec.ctypes.data_as(ctypes.c_void_p), spec.nbytes) == 0
+                for (f, l), ref in planes.items():
+                    assert rel_l2(spec[f, l, :, : prob.nx // 2 + 1], ref) < 1e-14
+                del spec
+    with dp.Plan(prob, max_particles=n, use_torques=True, fft_backend=1) as plan:
+        Uc, Omc = plan.mobility_apply(dpos, dF, dT)
+        torch.cuda.synchronize()
+        assert rel_l2(Uc.cpu().numpy(), U) < 1e-12 and rel_l2(Omc.cpu().numpy(), Om) < 1e-12
