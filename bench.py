@@ -150,6 +150,8 @@ def main():
     ap.add_argument("--impl", default="b200")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--transfer-fp32", action="store_true", help="time the fp32 spread/interpolate variant as the main number")
+    ap.add_argument("--no-fp32-variant", action="store_true", help="skip the extra timing of the fp32 spread/interpolate variant")
     ap.add_argument("--fft", choices=["own", "cufft"], default="own", help="xy FFT backend (own shared-memory passes, or cuFFT for comparison)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
@@ -183,7 +185,8 @@ def main():
     n = len(pos)
     fin = 6 if T is not None else 3
     fout = fin
-    plan = dp.Plan(prob, max_particles=n, use_torques=T is not None, device=local_rank, fft_backend=0 if args.fft == "own" else 1)
+    plan = dp.Plan(prob, max_particles=n, use_torques=T is not None, device=local_rank, fft_backend=0 if args.fft == "own" else 1,
+                   transfer_fp32=args.transfer_fp32)
     fft_backend = plan.fft_backend()
     dpos = torch.from_numpy(pos).to(dev)
     dF = torch.from_numpy(F).to(dev)
@@ -251,6 +254,35 @@ def main():
         e2e = {"value": world * n / dt, "unit": "particles/s", "ms_per_step": dt * 1e3,
                "h2d_bytes_per_step": int(24 * n * (3 if T is not None else 2)), "d2h_bytes_per_step": int(24 * n * (2 if T is not None else 1))}
 
+    # ---- the optional fp32 spread/interpolate variant (north_star: "also timed"), same inputs, same timing rules
+    variant = None
+    plan_bytes = plan.device_bytes()
+    if not args.transfer_fp32 and not args.no_fp32_variant and args.fft == "own":
+        plan.close()
+        plan = dp.Plan(prob, max_particles=n, use_torques=T is not None, device=local_rank, transfer_fp32=True)
+        plan.set_profiling(True)
+        for _ in range(args.warmup):
+            plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
+        barrier()
+        v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        v0.record(stream)
+        for _ in range(args.steps):
+            plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
+        v1.record(stream)
+        barrier()
+        vms = v0.elapsed_time(v1) / args.steps
+        if dist is not None:
+            t = torch.tensor([vms], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            vms = float(t.item())
+        plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
+        vst = plan.stage_ms()
+        variant = {"ms_per_step": vms, "value": world * n / (vms * 1e-3), "unit": "particles/s",
+                   "what": "spreading and interpolation accumulate in fp32, real-space grids stored in fp32; FFTs and solves fp64; "
+                           "matches the oracle to <= 1e-5 (tests)",
+                   "stage_ms": {k: vst[k] for k in ("spread", "fft_fwd", "solve", "fft_inv", "interp")},
+                   "plan_device_GB": plan.device_bytes() / 1e9}
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -288,10 +320,10 @@ def main():
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": dict(workloads_describe(args.config), n_particles=n, grid=[prob.nx, prob.ny, prob.nz], wall_mode=["bottom_wall", "slit"][prob.wall_mode],
                            fields_in=fin, fields_out=fout, w=prob.w, l2="inputs (%.1f GB of grids per product) far exceed the 126 MB L2" % (sum(by.values()) / 1e9 / 4),
-                           parallelism="replicas" if world > 1 else "single GPU", plan_device_GB=plan.device_bytes() / 1e9,
-                           fft_backend=fft_backend),
+                           parallelism="replicas" if world > 1 else "single GPU", plan_device_GB=plan_bytes / 1e9,
+                           fft_backend=fft_backend, transfer_fp32=bool(args.transfer_fp32)),
             "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": MY_KERNELS_PER_STEP[fft_backend] * args.steps,
-            "stages": stages, "roofline": roofline, "cpu_baseline": cpu}
+            "stages": stages, "roofline": roofline, "cpu_baseline": cpu, "fp32_transfer_variant": variant}
     print(json.dumps(line), flush=True)
     plan.close()
     if dist is not None:

@@ -55,6 +55,10 @@ typedef struct {
   int device;           /* CUDA device ordinal                                                                       */
   int fft_backend;      /* 0: the library's own shared-memory FFT passes when nx, ny allow them (nx/2 and ny products
                            of 2, 3, 5; nx <= 4320, ny <= 4320), else cuFFT;  1: always cuFFT (kept for comparison)    */
+  int transfer_fp32;    /* 0: everything fp64;  1: optional variant — spreading and interpolation accumulate in fp32 and
+                           the real-space grids are stored in fp32 (half the bytes of steps 1, 8 and of the real side of the
+                           x FFT passes); transforms and solves stay fp64.  Needs the own FFT passes (fft_backend = 0 and a
+                           supported size).  Matches the fp64 product to ~1e-6 relative (tests: <= 1e-5 vs the oracle).   */
 } dp_params;
 
 /* Validate, allocate (2 grids of fields*nz*ny*(nx+2) doubles + cuFFT workspace + particle workspace), plan the FFTs,

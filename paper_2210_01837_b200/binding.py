@@ -27,7 +27,7 @@ class dp_params(ctypes.Structure):
                 ("nx", ctypes.c_int), ("ny", ctypes.c_int), ("nz", ctypes.c_int), ("w", ctypes.c_int),
                 ("beta_M", ctypes.c_double), ("beta_D", ctypes.c_double), ("eta", ctypes.c_double),
                 ("max_particles", ctypes.c_int), ("use_torques", ctypes.c_int), ("device", ctypes.c_int),
-                ("fft_backend", ctypes.c_int)]
+                ("fft_backend", ctypes.c_int), ("transfer_fp32", ctypes.c_int)]
 
 
 _lib = None
@@ -106,14 +106,14 @@ STAGE_NAMES = ["bin", "spread", "fft_fwd", "solve", "fft_inv", "interp", "k0", "
 class Plan:
     """dp_create / dp_mobility_apply / dp_destroy.  ``prob`` is any object with the fields of ``workloads.Problem``."""
 
-    def __init__(self, prob, max_particles: int, use_torques=None, device: int = 0, fft_backend: int = 0):
+    def __init__(self, prob, max_particles: int, use_torques=None, device: int = 0, fft_backend: int = 0, transfer_fp32: bool = False):
         self._h = None
         L = load_library()
         if use_torques is None:
             use_torques = bool(getattr(prob, "has_torque", True))
         self.params = dp_params(int(prob.wall_mode), float(prob.Lx), float(prob.Ly), float(prob.H), int(prob.nx), int(prob.ny),
                                 int(prob.nz), int(prob.w), float(prob.beta_M), float(prob.beta_D), float(prob.eta),
-                                int(max_particles), int(bool(use_torques)), int(device), int(fft_backend))
+                                int(max_particles), int(bool(use_torques)), int(device), int(fft_backend), int(bool(transfer_fp32)))
         h = ctypes.c_void_p()
         rc = L.dp_create(ctypes.byref(self.params), ctypes.byref(h))
         if rc != 0:

@@ -136,8 +136,8 @@ struct MidPrefetch {          // inverse y pass, last round: all inputs are in r
 // The kernels are templates on the factorisation <R0, R1, R2> of the hot sizes (no runtime dispatch, every index into the
 // argument arrays static, only three butterflies in the instruction stream); <0, 0, 0> is the general version that
 // reads the radices from its arguments.
-template <int R0, bool INV, class Mid>
-__device__ __forceinline__ void run_edge(int r0, const double2* src, double2* dst, const double2* tw1, int n, int rows, int tid, const Mid& mid) {
+template <int R0, bool INV, class Mid, class TS, class TD>
+__device__ __forceinline__ void run_edge(int r0, const TS* src, TD* dst, const double2* tw1, int n, int rows, int tid, const Mid& mid) {
   if constexpr (R0 > 0) edge_lines<R0, INV>(src, dst, tw1, n, rows, (size_t)n, (size_t)n, tid, TPS, mid);
   else edge_dispatch<INV>(r0, src, dst, tw1, n, rows, (size_t)n, (size_t)n, tid, TPS, mid);
 }
@@ -245,7 +245,7 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_y_inv(FftYArgs A) {
 }
 
 // ---------------------------------------------------------------------------------------------- pass X forward
-template <int R0, int R1, int R2>
+template <int R0, int R1, int R2, bool F32>
 __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int M = A.M, npost = M / 2 + 1;
@@ -266,7 +266,8 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
     const long long pl = row0 / ny;
     const int y0 = (int)(row0 - pl * ny);
     // a real row of nx doubles is read as M complex numbers z[m] = x[2m] + i x[2m+1]
-    run_edge<R0, false>(A.F.r[0], reinterpret_cast<const double2*>(A.real + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
+    if constexpr (F32) run_edge<R0, false>(A.F.r[0], reinterpret_cast<const float2*>(reinterpret_cast<const float*>(A.real) + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
+    else run_edge<R0, false>(A.F.r[0], reinterpret_cast<const double2*>(A.real + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
     slot_barrier(slot);
     run_inner<R0, R1, R2, false, true>(A, buf, tw, M, rb, st, slot);
     // split into the spectra of the real rows and write them transposed: T[pl][kx][y0 + r]
@@ -286,7 +287,7 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
 }
 
 // ---------------------------------------------------------------------------------------------- pass X inverse
-template <int R0, int R1, int R2>
+template <int R0, int R1, int R2, bool F32>
 __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_inv(FftXArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int M = A.M, npost = M / 2 + 1;
@@ -342,7 +343,8 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_inv(FftXArgs A) {
     slot_barrier(slot);
     run_inner<R0, R1, R2, true, true>(A, buf, tw, M, rb, st, slot);
     // last stage: results go straight to the real grid rows (z[m] = x[2m] + i x[2m+1])
-    run_edge<R0, true>(A.F.r[0], buf, reinterpret_cast<double2*>(A.real + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
+    if constexpr (F32) run_edge<R0, true>(A.F.r[0], (const double2*)buf, reinterpret_cast<float2*>(reinterpret_cast<float*>(A.real) + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
+    else run_edge<R0, true>(A.F.r[0], (const double2*)buf, reinterpret_cast<double2*>(A.real + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
     slot_barrier(slot);                                  // the stage has read buf before the next batch refills it
   }
 }
@@ -373,11 +375,13 @@ KernelY pick_y(const Factors& F, bool inv) {
 #undef X
   return inv ? k_fft_y_inv<0, 0, 0> : k_fft_y_fwd<0, 0, 0>;
 }
-KernelX pick_x(const Factors& F, bool inv, int rb) {     // the static kernels assume rb = SLOT_ELEMS / M rows per batch
-#define X(a, b, c) if (is3(F, a, b, c) && rb == SLOT_ELEMS / (a * b * c)) return inv ? k_fft_x_inv<a, b, c> : k_fft_x_fwd<a, b, c>;
+KernelX pick_x(const Factors& F, bool inv, int rb, bool f32) {     // the static kernels assume rb = SLOT_ELEMS / M rows per batch
+#define X(a, b, c)                                                                                             \
+  if (is3(F, a, b, c) && rb == SLOT_ELEMS / (a * b * c))                                                       \
+    return f32 ? (inv ? k_fft_x_inv<a, b, c, true> : k_fft_x_fwd<a, b, c, true>) : (inv ? k_fft_x_inv<a, b, c, false> : k_fft_x_fwd<a, b, c, false>);
   DP_FFT_STATIC_LIST(X)
 #undef X
-  return inv ? k_fft_x_inv<0, 0, 0> : k_fft_x_fwd<0, 0, 0>;
+  return f32 ? (inv ? k_fft_x_inv<0, 0, 0, true> : k_fft_x_fwd<0, 0, 0, true>) : (inv ? k_fft_x_inv<0, 0, 0, false> : k_fft_x_fwd<0, 0, 0, false>);
 }
 
 template <class T> cudaError_t upload(T** dst, const std::vector<T>& v, dp_plan* P) {
@@ -466,7 +470,7 @@ cudaError_t dp_fft_own_create(dp_plan* P) {
   O->smem_y = smem_bytes_y(ny, O->ntw_y, O->rby);
   if (O->smem_x > 227 * 1024 || O->smem_y > 227 * 1024) return cudaErrorInvalidValue;
   O->ky_fwd = pick_y(O->Fy, false); O->ky_inv = pick_y(O->Fy, true);
-  O->kx_fwd = pick_x(O->Fx, false, O->rbx); O->kx_inv = pick_x(O->Fx, true, O->rbx);
+  O->kx_fwd = pick_x(O->Fx, false, O->rbx, P->p.transfer_fp32 != 0); O->kx_inv = pick_x(O->Fx, true, O->rbx, P->p.transfer_fp32 != 0);
   if ((e = cudaFuncSetAttribute(O->ky_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(O->ky_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(O->kx_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;

@@ -81,8 +81,14 @@ DP_HD void stage_dispatch(int R, double2* buf, const double2* tw, int n, int S, 
 // Its twiddles W_n^{t m} come from a recurrence on W_n^m (table tw1[m], m < S): no shared-memory traffic beyond one
 // load per line.  mid(round, nrounds) is called by every thread of the group between the loads of a round and its
 // arithmetic: the place where the caller synchronises buffer reuse (all rounds have the same trip count).
-template <int R, bool INV, class Mid>
-DP_HD void edge_lines(const double2* __restrict__ src, double2* __restrict__ dst, const double2* __restrict__ tw1, int n, int rows,
+// src / dst may hold float2 elements (the optional fp32 real grid of the x passes): converted on load / store.
+DP_HD double2 ld2(const double2* p) { return *p; }
+DP_HD double2 ld2(const float2* p) { const float2 v = *p; return make_double2((double)v.x, (double)v.y); }
+DP_HD void st2(double2* p, double2 v) { *p = v; }
+DP_HD void st2(float2* p, double2 v) { *p = make_float2((float)v.x, (float)v.y); }
+
+template <int R, bool INV, class Mid, class TS, class TD>
+DP_HD void edge_lines(const TS* __restrict__ src, TD* __restrict__ dst, const double2* __restrict__ tw1, int n, int rows,
                       size_t src_row_stride, size_t dst_row_stride, int tid, int nth, Mid mid) {
   const int S = n / R;
   const int total = rows * S;
@@ -91,12 +97,12 @@ DP_HD void edge_lines(const double2* __restrict__ src, double2* __restrict__ dst
     const int id = rd * nth + tid;
     const bool active = id < total;
     const int row = active ? id / S : 0, m = active ? id - row * S : 0;
-    const double2* ps = src + row * src_row_stride + m;
-    double2* pd = dst + row * dst_row_stride + m;
+    const TS* ps = src + row * src_row_stride + m;
+    TD* pd = dst + row * dst_row_stride + m;
     double2 x[R];
     if (active) {
 #pragma unroll
-      for (int t = 0; t < R; ++t) x[t] = ps[t * S];
+      for (int t = 0; t < R; ++t) x[t] = ld2(ps + t * S);
     }
     mid(rd, nrounds);
     if (active) {
@@ -112,13 +118,13 @@ DP_HD void edge_lines(const double2* __restrict__ src, double2* __restrict__ dst
         for (int t = 1; t < R; ++t) { x[t] = cmul(x[t], cur); if (t + 1 < R) cur = cmul(cur, w); }
       }
 #pragma unroll
-      for (int t = 0; t < R; ++t) pd[t * S] = x[t];
+      for (int t = 0; t < R; ++t) st2(pd + t * S, x[t]);
     }
   }
 }
 
-template <bool INV, class Mid>
-DP_HD void edge_dispatch(int R, const double2* src, double2* dst, const double2* tw1, int n, int rows, size_t src_row_stride,
+template <bool INV, class Mid, class TS, class TD>
+DP_HD void edge_dispatch(int R, const TS* src, TD* dst, const double2* tw1, int n, int rows, size_t src_row_stride,
                          size_t dst_row_stride, int tid, int nth, Mid mid) {
   switch (R) {
     case 2: edge_lines<2, INV>(src, dst, tw1, n, rows, src_row_stride, dst_row_stride, tid, nth, mid); break;

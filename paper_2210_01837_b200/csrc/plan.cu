@@ -206,6 +206,8 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   if (!(p.beta_M > 0) || (p.use_torques && !(p.beta_D > 0))) return DP_EINVAL;
   if (p.max_particles < 1) return DP_EINVAL;
   if (p.fft_backend != 0 && p.fft_backend != 1) return DP_EINVAL;
+  if (p.transfer_fp32 != 0 && p.transfer_fp32 != 1) return DP_EINVAL;
+  if (p.transfer_fp32 && !(p.fft_backend == 0 && dp_fft_own_supported(p.nx, p.ny))) return DP_EINVAL;   // fp32 grids are read by the own x passes only
   if (p.wall_mode == DP_SLIT && p.w * hx > p.H) return DP_EINVAL;     // a kernel may overlap one wall, not both
   if ((double)p.nz * p.ny * (p.nx + 16) >= 2.0e9) return DP_EINVAL;    // 32-bit plane indexing inside the kernels
 
@@ -230,7 +232,7 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   cudaError_t ce = cudaSetDevice(p.device);
   if (ce != cudaSuccess) { delete P; return DP_ECUDA; }
 #define TRY(x) do { rc = (x); if (rc != DP_OK) { std::string msg = P->last_error; dp_destroy(P); (void)msg; return rc; } } while (0)
-  TRY(dev_alloc(P, &P->d_real, P->real_field * P->fields));
+  TRY(dev_alloc(P, &P->d_real, p.transfer_fp32 ? (P->real_field * P->fields + 1) / 2 : P->real_field * P->fields));   // fp32 grids: half the bytes
   TRY(dev_alloc(P, &P->d_cplx, P->cplx_field * P->fields));
   TRY(dev_alloc(P, &P->d_znodes, (size_t)p.nz));
   TRY(dev_alloc(P, &P->d_zweights, (size_t)p.nz));
@@ -350,6 +352,15 @@ int dp_copy_buffer_to_host(dp_plan* P, int which, void* host, size_t bytes) {
     if (e == cudaSuccess) e = cudaMemcpy(host, tmp, bytes, cudaMemcpyDeviceToHost);
     cudaFree(tmp);
     CK(e);
+    return DP_OK;
+  }
+  if (which == 0 && P->p.transfer_fp32) {
+    // the real grids are stored in fp32: widen on the host so that the hook always hands out doubles
+    const size_t cnt = bytes / sizeof(double);
+    std::vector<float> tmp(cnt);
+    CK(cudaMemcpy(tmp.data(), P->d_real, cnt * sizeof(float), cudaMemcpyDeviceToHost));
+    double* out = static_cast<double*>(host);
+    for (size_t i = 0; i < cnt; ++i) out[i] = (double)tmp[i];
     return DP_OK;
   }
   CK(cudaMemcpy(host, which == 0 ? (const void*)P->d_real : (const void*)P->d_cplx, bytes, cudaMemcpyDeviceToHost));

@@ -200,7 +200,9 @@ struct SpreadArgs {
 // into contiguous ranges of the sorted arrays) are staged in shared memory with their footprint and weight records;
 // every thread adds the particles covering its column; each grid value is stored to HBM exactly once (128-byte row
 // segments per warp).  Dependent global round trips per CTA: bin_start -> candidate records -> stores.
-template <int NZ>
+// GT = double, or float for the optional fp32 variant (accumulators and grid in fp32; the weight records stay fp64 and are
+// rounded when they are used).
+template <int NZ, class GT>
 __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(SpreadArgs A) {
   constexpr int NL = NZ / ZSPLIT;
   constexpr int WREC = 2 * DP_MAX_W + NZ;
@@ -220,9 +222,9 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
   const double* __restrict__ val = A.val_s[grp];
   const double* __restrict__ wrec = A.wrec + (size_t)grp * A.cap * WREC;
 
-  double acc[NL][3];
+  GT acc[NL][3];
 #pragma unroll
-  for (int li = 0; li < NL; ++li) { acc[li][0] = 0.0; acc[li][1] = 0.0; acc[li][2] = 0.0; }
+  for (int li = 0; li < NL; ++li) { acc[li][0] = 0; acc[li][1] = 0; acc[li][2] = 0; }
 
   // bins whose footprints can reach this tile: origin columns in the cyclic range [X0-w+1, X0+TXeff-1] (same in y);
   // the x-bins of one bin row are consecutive in memory, so each row gives one range (two when the range wraps in x)
@@ -281,21 +283,21 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
         int a = gi - m.x; if (a < 0) a += g.nx;
         int bb = gj - m.y; if (bb < 0) bb += g.ny;
         if (a < w && bb < w && m.z <= m.w) {
-          const double wxy = s_w[q][a] * s_w[q][DP_MAX_W + bb];
-          const double v0 = s_val[q][0] * wxy, v1 = s_val[q][1] * wxy, v2 = s_val[q][2] * wxy;
+          const GT wxy = (GT)s_w[q][a] * (GT)s_w[q][DP_MAX_W + bb];
+          const GT v0 = (GT)s_val[q][0] * wxy, v1 = (GT)s_val[q][1] * wxy, v2 = (GT)s_val[q][2] * wxy;
           const double* zt = &s_w[q][2 * DP_MAX_W + tz];
           // zeta vanishes outside [lmin, lmax]: skipping a half of the planes that lies outside is exact
           if (m.z < ZSPLIT * (NL / 2)) {
 #pragma unroll
             for (int li = 0; li < NL / 2; ++li) {
-              const double z = zt[ZSPLIT * li];
+              const GT z = (GT)zt[ZSPLIT * li];
               acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
             }
           }
           if (m.w >= ZSPLIT * (NL / 2)) {
 #pragma unroll
             for (int li = NL / 2; li < NL; ++li) {
-              const double z = zt[ZSPLIT * li];
+              const GT z = (GT)zt[ZSPLIT * li];
               acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
             }
           }
@@ -309,7 +311,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
 #pragma unroll
     for (int li = 0; li < NL; ++li) {
       const int l = ZSPLIT * li + tz;
-      double* dst = A.grid + (size_t)A.field0[grp] * A.real_field + ((size_t)l * g.ny + gj) * g.nx + gi;
+      GT* dst = reinterpret_cast<GT*>(A.grid) + (size_t)A.field0[grp] * A.real_field + ((size_t)l * g.ny + gj) * g.nx + gi;
 #pragma unroll
       for (int c = 0; c < 3; ++c) dst[c * A.real_field] = acc[li][c];
     }
@@ -334,6 +336,7 @@ constexpr int INTERP_WARPS = 8;
 
 // One warp per particle (sorted order, so neighbouring warps gather from neighbouring columns): the lanes sweep the
 // w x w x (lmax-lmin+1) footprint, weights come from the particle's records, the six sums are reduced by shuffles.
+template <class GT>
 __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs A) {
   __shared__ double s_w[INTERP_WARPS][2][2 * DP_MAX_W + DP_MAX_NZ];   // per warp, per envelope: wx[8], wy[8], zeta[nz]
   __shared__ double s_zw[DP_MAX_NZ];
@@ -346,7 +349,7 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs 
   for (int p = blockIdx.x * INTERP_WARPS + wid; p < n; p += gridDim.x * INTERP_WARPS) {
     const int4 m = A.meta[p];
     const int dst = A.perm[p];
-    double s[6] = {0, 0, 0, 0, 0, 0};
+    GT s[6] = {0, 0, 0, 0, 0, 0};
     if (m.z <= m.w) {
       __syncwarp();
       for (int k = 0; k < nk; ++k) {
@@ -360,11 +363,11 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs 
         int i = m.x + a; if (i >= g.nx) i -= g.nx;
         int j = m.y + b; if (j >= g.ny) j -= g.ny;
         const size_t off = ((size_t)l * g.ny + j) * g.nx + i;
-        const double wl = s_zw[l];
+        const GT wl = (GT)s_zw[l];
         for (int k = 0; k < nk; ++k) {
           const double* sw = s_w[wid][k];
-          const double wgt = sw[a] * sw[DP_MAX_W + b] * sw[2 * DP_MAX_W + l];
-          const double* gp = A.grid + (size_t)(3 * k) * A.real_field + off;
+          const GT wgt = (GT)sw[a] * (GT)sw[DP_MAX_W + b] * (GT)sw[2 * DP_MAX_W + l];
+          const GT* gp = reinterpret_cast<const GT*>(A.grid) + (size_t)(3 * k) * A.real_field + off;
           s[3 * k + 0] += __ldg(gp) * wgt * wl;
           s[3 * k + 1] += __ldg(gp + A.real_field) * wgt * wl;
           s[3 * k + 2] += __ldg(gp + 2 * A.real_field) * wgt * wl;
@@ -373,8 +376,8 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs 
     }
     for (int c = 0; c < 3 * nk; ++c)
       for (int o = 16; o > 0; o >>= 1) s[c] += __shfl_xor_sync(0xffffffffu, s[c], o);
-    if (lane < 3) A.U[3 * (size_t)dst + lane] = lane == 0 ? s[0] : (lane == 1 ? s[1] : s[2]);
-    if (A.Omega && lane >= 3 && lane < 6) A.Omega[3 * (size_t)dst + lane - 3] = lane == 3 ? s[3] : (lane == 4 ? s[4] : s[5]);
+    if (lane < 3) A.U[3 * (size_t)dst + lane] = (double)(lane == 0 ? s[0] : (lane == 1 ? s[1] : s[2]));
+    if (A.Omega && lane >= 3 && lane < 6) A.Omega[3 * (size_t)dst + lane - 3] = (double)(lane == 3 ? s[3] : (lane == 4 ? s[4] : s[5]));
     __syncwarp();
   }
 }
@@ -429,10 +432,11 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
   A.grid = P->d_real;
   A.real_field = P->real_field;
   dim3 grid(P->nbx, P->nby, ngroups);
+  const bool f32 = P->p.transfer_fp32 != 0;
   switch (P->p.nz) {
-    case 16: k_spread<16><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
-    case 32: k_spread<32><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
-    case 48: k_spread<48><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
+    case 16: if (f32) k_spread<16, float><<<grid, SPREAD_THREADS, 0, st>>>(A); else k_spread<16, double><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
+    case 32: if (f32) k_spread<32, float><<<grid, SPREAD_THREADS, 0, st>>>(A); else k_spread<32, double><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
+    case 48: if (f32) k_spread<48, float><<<grid, SPREAD_THREADS, 0, st>>>(A); else k_spread<48, double><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
     default: return cudaErrorInvalidValue;
   }
   return cudaGetLastError();
@@ -450,6 +454,7 @@ cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaSt
   const int maxb = 148 * 64;
   if (blocks > maxb) blocks = maxb;
   if (blocks < 1) blocks = 1;
-  k_interp<<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A);
+  if (P->p.transfer_fp32) k_interp<float><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A);
+  else k_interp<double><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A);
   return cudaGetLastError();
 }

@@ -261,3 +261,37 @@ def test_full_size_fft_passes_on_sampled_planes_and_backends_agree(dp):
         Uc, Omc = plan.mobility_apply(dpos, dF, dT)
         torch.cuda.synchronize()
         assert rel_l2(Uc.cpu().numpy(), U) < 1e-12 and rel_l2(Omc.cpu().numpy(), Om) < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------ fp32 transfer variant
+@pytest.mark.parametrize("case", ["cfg1", "cfg2", "bw-mono", "slit-mono"])
+def test_fp32_transfer_variant_matches_the_oracle_to_1e5(dp, case):
+    """north_star: the optional fp32 spread/interpolate variant (fp32 accumulation and fp32 real-space grids, fp64 transforms
+    and solves) must match the oracle to a relative L2 error <= 1e-5."""
+    if case == "cfg1":
+        prob, pos, F, T = workloads.config(1)
+    elif case == "cfg2":
+        prob, pos, F, T = workloads.config(2)
+    elif case == "bw-mono":
+        prob, pos, F, T = small_monolayer("bw", 3000, 31)
+    else:
+        prob, pos, F, T = small_monolayer("slit", 2500, 32)
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft")
+    with dp.Plan(prob, max_particles=len(pos), use_torques=prob.has_torque, transfer_fp32=True) as plan:
+        U, Om = plan.mobility_apply(*to_dev(pos, F, T))
+        import torch
+        torch.cuda.synchronize()
+        assert plan.check() == 0
+        e = rel_l2(U.cpu().numpy(), U_o)
+        assert 1e-9 < e < 1e-5, e                       # really fp32 (not silently fp64), and within the bar
+        if Om is not None:
+            assert rel_l2(Om.cpu().numpy(), Om_o) < 1e-5
+        # the spread grid handed out by the test hook is the fp32 grid widened to doubles
+        g = plan.debug_stage(*to_dev(pos, F, T), 1)
+        st = {}
+        oracle.mobility_apply(prob, pos, F, T, dft="fft", stages=st)
+        ref = st["f"] if T is None else np.concatenate([st["f"], st["t"]])
+        assert 1e-9 < rel_l2(g, ref) < 1e-6
+    # the variant needs the own FFT passes
+    with pytest.raises(dp.DPError):
+        dp.Plan(prob, max_particles=len(pos), use_torques=prob.has_torque, transfer_fp32=True, fft_backend=1)
