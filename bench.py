@@ -47,12 +47,15 @@ def hbm_peak():
         return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def stage_bytes(prob, n, fin, fout):
-    """Algorithmic (compulsory) bytes per product and stage, DESIGN.md §'Algorithmic bytes'."""
+def stage_bytes(prob, n, fin, fout, zero_planes=0):
+    """Algorithmic (compulsory) bytes per product and stage: every grid value read once and
+    written once per stage.  Planes above every footprint hold no force (exactly zero): with ``zero_planes`` of the nz input
+    planes skipped, the input side of spread / forward FFT / solve shrinks by that share — the bytes really needed."""
     G = prob.nx * prob.ny * prob.nz
     Kz = (prob.nx // 2 + 1) * prob.ny * prob.nz
     R, C = 8.0 * G, 16.0 * Kz
-    return {"spread": fin * R + 72.0 * n, "fft_fwd": fin * (R + C), "solve": (fin + fout) * C,
+    a = 1.0 - zero_planes / float(prob.nz)
+    return {"spread": a * fin * R + 72.0 * n, "fft_fwd": a * fin * (R + C), "solve": (a * fin + fout) * C,
             "fft_inv": fout * (C + R), "interp": fout * R + 72.0 * n}
 
 
@@ -152,6 +155,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--transfer-fp32", action="store_true", help="time the fp32 spread/interpolate variant as the main number")
     ap.add_argument("--no-fp32-variant", action="store_true", help="skip the extra timing of the fp32 spread/interpolate variant")
+    ap.add_argument("--dense-planes", action="store_true", help="transform every plane (do not skip the planes no footprint reaches)")
     ap.add_argument("--fft", choices=["own", "cufft"], default="own", help="xy FFT backend (own shared-memory passes, or cuFFT for comparison)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
@@ -186,7 +190,7 @@ def main():
     fin = 6 if T is not None else 3
     fout = fin
     plan = dp.Plan(prob, max_particles=n, use_torques=T is not None, device=local_rank, fft_backend=0 if args.fft == "own" else 1,
-                   transfer_fp32=args.transfer_fp32)
+                   transfer_fp32=args.transfer_fp32, dense_planes=args.dense_planes)
     fft_backend = plan.fft_backend()
     dpos = torch.from_numpy(pos).to(dev)
     dF = torch.from_numpy(F).to(dev)
@@ -225,6 +229,7 @@ def main():
             stage_acc.setdefault(k, []).append(v)
     stage_ms = {k: float(np.median(v)) for k, v in stage_acc.items()}
     assert plan.check() == 0
+    zero_planes = plan.zero_planes()
     ms_step = ms_total / args.steps
     if dist is not None:
         t = torch.tensor([ms_step], dtype=torch.float64, device=dev)
@@ -254,12 +259,15 @@ def main():
         e2e = {"value": world * n / dt, "unit": "particles/s", "ms_per_step": dt * 1e3,
                "h2d_bytes_per_step": int(24 * n * (3 if T is not None else 2)), "d2h_bytes_per_step": int(24 * n * (2 if T is not None else 1))}
 
-    # ---- the optional fp32 spread/interpolate variant (north_star: "also timed"), same inputs, same timing rules
-    variant = None
+    # ---- two more timings of the same product on the same inputs, same rules (3 warm-ups, CUDA events, max over ranks):
+    #      the optional fp32 spread/interpolate variant (north_star: "also timed"), and the product with the zero-plane
+    #      skipping switched off (every plane spread, transformed and loaded)
     plan_bytes = plan.device_bytes()
-    if not args.transfer_fp32 and not args.no_fp32_variant and args.fft == "own":
+
+    def time_variant(**kw):
+        nonlocal plan
         plan.close()
-        plan = dp.Plan(prob, max_particles=n, use_torques=T is not None, device=local_rank, transfer_fp32=True)
+        plan = dp.Plan(prob, max_particles=n, use_torques=T is not None, device=local_rank, **kw)
         plan.set_profiling(True)
         for _ in range(args.warmup):
             plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
@@ -277,11 +285,18 @@ def main():
             vms = float(t.item())
         plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
         vst = plan.stage_ms()
-        variant = {"ms_per_step": vms, "value": world * n / (vms * 1e-3), "unit": "particles/s",
-                   "what": "spreading and interpolation accumulate in fp32, real-space grids stored in fp32; FFTs and solves fp64; "
-                           "matches the oracle to <= 1e-5 (tests)",
-                   "stage_ms": {k: vst[k] for k in ("spread", "fft_fwd", "solve", "fft_inv", "interp")},
-                   "plan_device_GB": plan.device_bytes() / 1e9}
+        return {"ms_per_step": vms, "value": world * n / (vms * 1e-3), "unit": "particles/s",
+                "stage_ms": {k: vst[k] for k in ("spread", "fft_fwd", "solve", "fft_inv", "interp")},
+                "plan_device_GB": plan.device_bytes() / 1e9}
+
+    variant = dense = None
+    if not args.transfer_fp32 and not args.no_fp32_variant and args.fft == "own":
+        variant = time_variant(transfer_fp32=True, dense_planes=args.dense_planes)
+        variant["what"] = ("spreading and interpolation accumulate in fp32, real-space grids stored in fp32; FFTs and solves fp64; "
+                           "matches the oracle to <= 1e-5 (tests)")
+        if not args.dense_planes and zero_planes > 0:
+            dense = time_variant(transfer_fp32=False, dense_planes=True)
+            dense["what"] = "same fp64 product with dense_planes = 1: the %d planes no footprint reaches are spread, transformed and loaded too" % zero_planes
 
     if rank != 0:
         if dist is not None:
@@ -289,7 +304,8 @@ def main():
         return
 
     peak, peak_src = hbm_peak()
-    by = stage_bytes(prob, n, fin, fout)
+    by = stage_bytes(prob, n, fin, fout, zero_planes)
+    by_dense = stage_bytes(prob, n, fin, fout, 0)
     stages = {}
     for k, b in by.items():
         t_ms = stage_ms.get(k, 0.0)
@@ -308,7 +324,8 @@ def main():
                 "fft_chebyshev_solve_stages": {"algorithmic_GB": mid, "ms": mid_ms, "GBps": mid / (mid_ms * 1e-3) if mid_ms else None,
                                                "frac": (mid / (mid_ms * 1e-3) / peak) if mid_ms else None},
                 "whole_product": {"algorithmic_GB": sum(by.values()) / 1e9, "ms": ms_step,
-                                  "frac": sum(by.values()) / 1e9 / (ms_step * 1e-3) / peak}}
+                                  "frac": sum(by.values()) / 1e9 / (ms_step * 1e-3) / peak,
+                                  "algorithmic_GB_if_all_planes_dense": sum(by_dense.values()) / 1e9}}
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
@@ -321,9 +338,10 @@ def main():
             "config": dict(workloads_describe(args.config), n_particles=n, grid=[prob.nx, prob.ny, prob.nz], wall_mode=["bottom_wall", "slit"][prob.wall_mode],
                            fields_in=fin, fields_out=fout, w=prob.w, l2="inputs (%.1f GB of grids per product) far exceed the 126 MB L2" % (sum(by.values()) / 1e9 / 4),
                            parallelism="replicas" if world > 1 else "single GPU", plan_device_GB=plan_bytes / 1e9,
-                           fft_backend=fft_backend, transfer_fp32=bool(args.transfer_fp32)),
+                           fft_backend=fft_backend, transfer_fp32=bool(args.transfer_fp32),
+                           zero_planes_skipped=zero_planes, nz=prob.nz),
             "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": MY_KERNELS_PER_STEP[fft_backend] * args.steps,
-            "stages": stages, "roofline": roofline, "cpu_baseline": cpu, "fp32_transfer_variant": variant}
+            "stages": stages, "roofline": roofline, "cpu_baseline": cpu, "fp32_transfer_variant": variant, "all_planes_dense": dense}
     print(json.dumps(line), flush=True)
     plan.close()
     if dist is not None:

@@ -59,6 +59,10 @@ typedef struct {
                            the real-space grids are stored in fp32 (half the bytes of steps 1, 8 and of the real side of the
                            x FFT passes); transforms and solves stay fp64.  Needs the own FFT passes (fft_backend = 0 and a
                            supported size).  Matches the fp64 product to ~1e-6 relative (tests: <= 1e-5 vs the oracle).   */
+  int dense_planes;     /* 0 (default): planes of the Chebyshev grid above every particle's footprint hold no force, so their
+                           forward transforms are identically zero; the product finds the highest touched plane while
+                           binning and skips the spreading stores, forward FFT passes and solve loads of the planes above
+                           it (exact: the skipped values are zeros).  1: treat every plane as dense.                        */
 } dp_params;
 
 /* Validate, allocate (2 grids of fields*nz*ny*(nx+2) doubles + cuFFT workspace + particle workspace), plan the FFTs,
@@ -101,6 +105,7 @@ int dp_debug_run_stage(dp_plan* plan, int n, const double* pos, const double* fo
 size_t dp_buffer_bytes(const dp_plan* plan, int which);
 int dp_copy_buffer_to_host(dp_plan* plan, int which, void* host, size_t bytes);
 int dp_complex_row_pitch(const dp_plan* plan); /* nkxp: padded row length (in complex numbers) of the half spectrum */
+int dp_zero_planes(dp_plan* plan);             /* synchronises; number of leading planes (l = 0 is z = H) the last apply skipped */
 int dp_fft_backend(const dp_plan* plan);       /* 0: own shared-memory FFT passes in use, 1: cuFFT                    */
 
 /* Introspection */

@@ -14,7 +14,7 @@ _LIBNAME = os.path.join(_HERE, "libdpstokes.so")
 
 # every symbol include/dp.h declares
 EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_check", "dp_set_profiling", "dp_stage_ms",
-           "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_complex_row_pitch", "dp_fft_backend", "dp_es_norm",
+           "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_complex_row_pitch", "dp_zero_planes", "dp_fft_backend", "dp_es_norm",
            "dp_supported_nz", "dp_device_bytes", "dp_strerror", "dp_last_error", "dp_destroy"]
 
 
@@ -27,7 +27,8 @@ class dp_params(ctypes.Structure):
                 ("nx", ctypes.c_int), ("ny", ctypes.c_int), ("nz", ctypes.c_int), ("w", ctypes.c_int),
                 ("beta_M", ctypes.c_double), ("beta_D", ctypes.c_double), ("eta", ctypes.c_double),
                 ("max_particles", ctypes.c_int), ("use_torques", ctypes.c_int), ("device", ctypes.c_int),
-                ("fft_backend", ctypes.c_int), ("transfer_fp32", ctypes.c_int)]
+                ("fft_backend", ctypes.c_int), ("transfer_fp32", ctypes.c_int),
+                ("dense_planes", ctypes.c_int)]
 
 
 _lib = None
@@ -67,6 +68,8 @@ def load_library():
     L.dp_copy_buffer_to_host.restype = i
     L.dp_complex_row_pitch.argtypes = [vp]
     L.dp_complex_row_pitch.restype = i
+    L.dp_zero_planes.argtypes = [vp]
+    L.dp_zero_planes.restype = i
     L.dp_fft_backend.argtypes = [vp]
     L.dp_fft_backend.restype = i
     L.dp_es_norm.argtypes = [d, d]
@@ -106,14 +109,16 @@ STAGE_NAMES = ["bin", "spread", "fft_fwd", "solve", "fft_inv", "interp", "k0", "
 class Plan:
     """dp_create / dp_mobility_apply / dp_destroy.  ``prob`` is any object with the fields of ``workloads.Problem``."""
 
-    def __init__(self, prob, max_particles: int, use_torques=None, device: int = 0, fft_backend: int = 0, transfer_fp32: bool = False):
+    def __init__(self, prob, max_particles: int, use_torques=None, device: int = 0, fft_backend: int = 0, transfer_fp32: bool = False,
+                 dense_planes: bool = False):
         self._h = None
         L = load_library()
         if use_torques is None:
             use_torques = bool(getattr(prob, "has_torque", True))
         self.params = dp_params(int(prob.wall_mode), float(prob.Lx), float(prob.Ly), float(prob.H), int(prob.nx), int(prob.ny),
                                 int(prob.nz), int(prob.w), float(prob.beta_M), float(prob.beta_D), float(prob.eta),
-                                int(max_particles), int(bool(use_torques)), int(device), int(fft_backend), int(bool(transfer_fp32)))
+                                int(max_particles), int(bool(use_torques)), int(device), int(fft_backend), int(bool(transfer_fp32)),
+                                int(bool(dense_planes)))
         h = ctypes.c_void_p()
         rc = L.dp_create(ctypes.byref(self.params), ctypes.byref(h))
         if rc != 0:
@@ -192,6 +197,9 @@ class Plan:
         buf = (ctypes.c_float * 8)()
         self._ck(load_library().dp_stage_ms(self._h, buf), "dp_stage_ms")
         return {k: float(buf[i]) for i, k in enumerate(STAGE_NAMES)}
+
+    def zero_planes(self) -> int:
+        return int(load_library().dp_zero_planes(self._h))
 
     def fft_backend(self) -> str:
         return ["own", "cufft"][int(load_library().dp_fft_backend(self._h))]

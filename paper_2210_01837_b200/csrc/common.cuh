@@ -51,6 +51,7 @@ struct dp_plan {
   int* d_bin_count = nullptr;   // [nbins]
   int* d_bin_start = nullptr;   // [nbins+1]
   int* d_flag = nullptr;        // out-of-domain flag
+  int* d_lmin = nullptr;        // lowest plane index touched by any footprint of the current apply (planes below it are zero)
   size_t device_bytes = 0;
 
   cufftHandle fft_fwd = 0, fft_inv = 0;
@@ -68,7 +69,7 @@ struct dp_plan {
 };
 
 // launchers implemented in transfer.cu / solve.cu; all asynchronous on `st`
-cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* force, const double* torque, cudaStream_t st);
+cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* force, const double* torque, bool dense, cudaStream_t st);
 cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torque, cudaStream_t st);
 cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaStream_t st);
 cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega, cudaStream_t st);

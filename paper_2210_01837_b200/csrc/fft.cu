@@ -94,6 +94,8 @@ struct FftYArgs {
   int ntw, off[MAX_STAGES];
   Factors F;
   int rb;                 // rows per slot batch
+  const int* lmin;        // forward pass: planes l < *lmin of every field are zero and skipped (null: none)
+  int nz, nkx, fields;    // rows = fields * nz * nkx
 };
 
 struct FftXArgs {
@@ -107,6 +109,8 @@ struct FftXArgs {
   const unsigned short* pos;
   Factors F;
   int rb;                 // rows (consecutive y) per slot batch; divides ny
+  const int* lmin;        // forward pass: planes l < *lmin of every field are zero and skipped (null: none)
+  int nz;                 // planes = fields * nz
 };
 
 __host__ __device__ inline size_t align16(size_t b) { return (b + 15) / 16 * 16; }
@@ -188,10 +192,15 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_y_fwd(FftYArgs A) {
   double2* buf = tw + A.ntw + (size_t)slot * A.rb * n;
   for (int i = threadIdx.x; i < A.ntw; i += FFT_THREADS) tw[i] = A.tw[i];
   __syncthreads();
-  const long long nbatch = (A.rows + A.rb - 1) / A.rb;
+  // rows of the planes l >= lm of each field: per field one contiguous range of ra rows, cut into batches of rb
+  int lm = A.lmin ? __ldg(A.lmin) : 0;
+  lm = lm < 0 ? 0 : (lm > A.nz ? A.nz : lm);
+  const long long ra = (long long)(A.nz - lm) * A.nkx, per_field = (ra + A.rb - 1) / A.rb;
+  const long long nbatch = per_field * A.fields;
   for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
-    const long long row0 = b * A.rb;
-    const int nr = (int)((A.rows - row0) < A.rb ? (A.rows - row0) : A.rb);
+    const long long f = b / per_field, j = b - f * per_field;
+    const long long row0 = (f * A.nz + lm) * A.nkx + j * A.rb;
+    const int nr = (int)((ra - j * A.rb) < A.rb ? (ra - j * A.rb) : A.rb);
     double2* g = A.data + row0 * n;
     const MidStoreDrained mid{slot, st};
     run_edge<R0, false>(A.F.r[0], g, buf, tw + A.off[0], n, nr, st, mid);
@@ -259,12 +268,16 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
   for (int i = threadIdx.x; i < npost; i += FFT_THREADS) post[i] = A.post[i];
   __syncthreads();
   const int rb = A.rb, ny = A.ny, nkx = M + 1;
-  const long long nbatch = A.planes * (ny / rb);
+  int lm = A.lmin ? __ldg(A.lmin) : 0;
+  lm = lm < 0 ? 0 : (lm > A.nz ? A.nz : lm);
+  const int act = A.nz - lm, bpp = ny / rb;              // planes per field that can hold force; batches per plane
+  const long long nbatch = (A.planes / A.nz) * act * bpp;
   const MidNone nomid;
   for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
-    const long long row0 = b * rb;                       // flat row index over (plane, y)
-    const long long pl = row0 / ny;
-    const int y0 = (int)(row0 - pl * ny);
+    const long long pa = b / bpp;                        // index among the active planes
+    const int y0 = (int)(b - pa * bpp) * rb;
+    const long long pl = (pa / act) * A.nz + lm + pa % act;
+    const long long row0 = pl * ny + y0;                 // flat row index over (plane, y)
     // a real row of nx doubles is read as M complex numbers z[m] = x[2m] + i x[2m+1]
     if constexpr (F32) run_edge<R0, false>(A.F.r[0], reinterpret_cast<const float2*>(reinterpret_cast<const float*>(A.real) + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
     else run_edge<R0, false>(A.F.r[0], reinterpret_cast<const double2*>(A.real + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
@@ -487,6 +500,7 @@ static FftXArgs x_args(dp_plan* P, int nfields) {
   A.real = P->d_real; A.cplx = P->d_cplx; A.planes = (long long)nfields * P->p.nz;
   A.nx = P->p.nx; A.ny = P->p.ny; A.M = P->p.nx / 2;
   A.tw = O->d_tw_x; A.ntw = O->ntw_x; A.post = O->d_post_x; A.pos = O->d_pos_x; A.F = O->Fx; A.rb = O->rbx;
+  A.lmin = P->d_lmin; A.nz = P->p.nz;
   for (int j = 0; j < MAX_STAGES; ++j) A.off[j] = O->off_x[j];
   return A;
 }
@@ -495,6 +509,7 @@ static FftYArgs y_args(dp_plan* P, int nfields) {
   FftYArgs A;
   A.data = P->d_cplx; A.rows = (long long)nfields * P->p.nz * (P->p.nx / 2 + 1);
   A.tw = O->d_tw_y; A.ntw = O->ntw_y; A.F = O->Fy; A.rb = O->rby;
+  A.lmin = P->d_lmin; A.nz = P->p.nz; A.nkx = P->p.nx / 2 + 1; A.fields = nfields;
   for (int j = 0; j < MAX_STAGES; ++j) A.off[j] = O->off_y[j];
   return A;
 }

@@ -97,7 +97,10 @@ int run_pipeline(dp_plan* P, int n, const double* pos, const double* force, cons
   P->last_stream = st;
   P->ev_recorded = false;
   if (prof) CK(cudaEventRecord(P->ev[0], st));
-  CK(dp_launch_bin(P, n, pos, force, torque, st));
+  // the zero planes are skipped only with the own FFT passes (cuFFT transforms every plane) and only in full products
+  // (the test hooks hand out whole grids)
+  const bool dense = P->p.dense_planes || !P->own_fft || last_stage < 5;
+  CK(dp_launch_bin(P, n, pos, force, torque, dense, st));
   if (prof) CK(cudaEventRecord(P->ev[1], st));
   CK(dp_launch_spread(P, n, true, with_torque, st));
   if (prof) CK(cudaEventRecord(P->ev[2], st));
@@ -177,7 +180,7 @@ int dp_destroy(dp_plan* P) {
   if (P->fft_ok) { cufftDestroy(P->fft_fwd); cufftDestroy(P->fft_inv); }
   dp_fft_own_destroy(P);
   void* bufs[] = {P->d_real, P->d_cplx, P->d_fft_work, P->d_znodes, P->d_zweights, P->d_pos_s, P->d_frc_s, P->d_trq_s, P->d_perm, P->d_meta, P->d_wrec,
-                  P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_bin_start, P->d_flag};
+                  P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_bin_start, P->d_flag, P->d_lmin};
   for (void* b : bufs) if (b) cudaFree(b);
   if (P->ev_ok) for (auto& e : P->ev) cudaEventDestroy(e);
   dp_host_stage* hs = stage_of(P);
@@ -207,6 +210,7 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   if (p.max_particles < 1) return DP_EINVAL;
   if (p.fft_backend != 0 && p.fft_backend != 1) return DP_EINVAL;
   if (p.transfer_fp32 != 0 && p.transfer_fp32 != 1) return DP_EINVAL;
+  if (p.dense_planes != 0 && p.dense_planes != 1) return DP_EINVAL;
   if (p.transfer_fp32 && !(p.fft_backend == 0 && dp_fft_own_supported(p.nx, p.ny))) return DP_EINVAL;   // fp32 grids are read by the own x passes only
   if (p.wall_mode == DP_SLIT && p.w * hx > p.H) return DP_EINVAL;     // a kernel may overlap one wall, not both
   if ((double)p.nz * p.ny * (p.nx + 16) >= 2.0e9) return DP_EINVAL;    // 32-bit plane indexing inside the kernels
@@ -248,6 +252,7 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   TRY(dev_alloc(P, &P->d_bin_count, (size_t)P->nbins));
   TRY(dev_alloc(P, &P->d_bin_start, (size_t)P->nbins + 1));
   TRY(dev_alloc(P, &P->d_flag, (size_t)1));
+  TRY(dev_alloc(P, &P->d_lmin, (size_t)1));
   if (P->own_fft) {
     cudaError_t fe = dp_fft_own_create(P);
     if (fe != cudaSuccess) { set_err(P, "dp_fft_own_create", cudaGetErrorString(fe)); dp_destroy(P); return DP_ECUDA; }
@@ -336,6 +341,14 @@ size_t dp_buffer_bytes(const dp_plan* P, int which) {
 }
 
 int dp_fft_backend(const dp_plan* P) { return P ? (P->own_fft ? 0 : 1) : -1; }
+
+int dp_zero_planes(dp_plan* P) {
+  if (!P) return DP_EINVAL;
+  CK(cudaStreamSynchronize(P->last_stream));
+  int lm = 0;
+  CK(cudaMemcpy(&lm, P->d_lmin, sizeof(int), cudaMemcpyDeviceToHost));
+  return lm < 0 ? 0 : (lm > P->p.nz ? P->p.nz : lm);
+}
 
 int dp_copy_buffer_to_host(dp_plan* P, int which, void* host, size_t bytes) {
   if (!P || !host) return DP_EINVAL;

@@ -56,6 +56,7 @@ struct SolveArgs {
   int nx, ny, nkx;
   int n_fast, n_slow, pitch;     // half spectrum stored as [field][l][slow][fast (pitch)]
   int fast_is_x;                 // 1: fast index = kx index (cuFFT layout); 0: fast index = position along ky (transposed layout)
+  const int* lmin;               // planes l < *lmin of the input hold zeros that were never written: not read
   const int* ky_of_pos;          // transposed layout: FFT-order ky index stored at each position (digit reversal of the y pass), or null
   double Lx, Ly, H, eta;
   int wall_mode, torque, omega;
@@ -436,6 +437,7 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
   // the two chains, warps 2-5 evaluate e^{-k z_l} and z_l e^{-k z_l} at the nodes (-> C5).  Then every warp folds the
   // algebraic part of (1/2) curl t into f for the rows it loaded itself (eq 7).
   constexpr int ROWS = (NZ + SOLVE_WARPS - 1) / SOLVE_WARPS;
+  const int lm = __ldg(A.lmin);
   double tz[ROWS];
 #pragma unroll
   for (int r = 0; r < ROWS; ++r) {
@@ -443,7 +445,7 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
     tz[r] = 0.0;
     if (l < NZ) {
       const int o = l * LN + lane;
-      if (valid) {
+      if (valid && l >= lm) {
         const size_t og = 2 * (l * plane + off0) + part;
 #pragma unroll
         for (int c = 0; c < 3; ++c) cp_async8(&C[c * VS + o], &gin[2 * (c * A.cplx_field) + og]);
@@ -608,7 +610,7 @@ __global__ void k_zero_mode(SolveArgs A, int nz, const double* __restrict__ ct_f
     const int field = q < 2 ? q : (q == 2 ? 3 : 4);
     double ar = 0.0, ai = 0.0;
     if (q < 2 || A.torque) {
-      for (int l = 0; l < nz; ++l) {
+      for (int l = A.lmin[0] < 0 ? 0 : A.lmin[0]; l < nz; ++l) {
         double2 v = A.cplx[field * A.cplx_field + (size_t)l * A.n_slow * A.pitch];
         double wgt = ct_full[n * nz + l] * ((l == 0 || l == N) ? 0.5 : 1.0);
         ar += wgt * v.x; ai += wgt * v.y;
@@ -752,7 +754,7 @@ cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega,
   SolveArgs A;
   A.cplx = P->d_cplx; A.cplx_field = P->cplx_field;
   A.nx = P->p.nx; A.ny = P->p.ny; A.nkx = P->nkx;
-  A.n_fast = P->nkx; A.n_slow = P->p.ny; A.pitch = P->nkxp; A.fast_is_x = 1; A.ky_of_pos = nullptr;
+  A.n_fast = P->nkx; A.n_slow = P->p.ny; A.pitch = P->nkxp; A.fast_is_x = 1; A.ky_of_pos = nullptr; A.lmin = P->d_lmin;
   if (P->own_fft) { A.n_fast = P->p.ny; A.n_slow = P->nkx; A.pitch = P->p.ny; A.fast_is_x = 0; A.ky_of_pos = dp_fft_own_ky_table(P); }
   A.Lx = P->p.Lx; A.Ly = P->p.Ly; A.H = P->p.H; A.eta = P->p.eta;
   A.wall_mode = P->p.wall_mode; A.torque = with_torque_field ? 1 : 0; A.omega = want_omega ? 1 : 0;

@@ -121,9 +121,10 @@ __global__ void k_bin_scatter(int n, const double* __restrict__ pos, const doubl
                               const double* __restrict__ torque, GridGeom g, const int* __restrict__ bin_of,
                               const int* __restrict__ slot_of, const int* __restrict__ bin_start, const double* __restrict__ znodes,
                               int* __restrict__ perm, int4* __restrict__ meta, double* __restrict__ pos_s, double* __restrict__ frc_s,
-                              double* __restrict__ trq_s) {
+                              double* __restrict__ trq_s, int* __restrict__ lmin_all) {
   int p = blockIdx.x * blockDim.x + threadIdx.x;
-  if (p >= n) return;
+  int my_lmin = 0x7fffffff;
+  if (p < n) {
   int d = bin_start[bin_of[p]] + slot_of[p];
   perm[d] = p;
   double x = pos[3 * (size_t)p], y = pos[3 * (size_t)p + 1], z = pos[3 * (size_t)p + 2];
@@ -142,6 +143,11 @@ __global__ void k_bin_scatter(int n, const double* __restrict__ pos, const doubl
     if (frc_s) frc_s[3 * (size_t)d + c] = force ? force[3 * (size_t)p + c] : 0.0;
     if (trq_s) trq_s[3 * (size_t)d + c] = torque ? torque[3 * (size_t)p + c] : 0.0;
   }
+  if (ok && m.z <= m.w) my_lmin = m.z;
+  }
+  // highest plane (lowest index) any footprint touches: one atomic per warp
+  my_lmin = __reduce_min_sync(0xffffffffu, my_lmin);
+  if ((threadIdx.x & 31) == 0 && my_lmin != 0x7fffffff) atomicMin(lmin_all, my_lmin);
 }
 
 // ---------------------------------------------------------------------------------------------- 1-D ES weights
@@ -192,6 +198,7 @@ struct SpreadArgs {
   size_t cap;
   double* grid;
   size_t real_field;
+  const int* lmin;           // planes l < *lmin hold no force: not stored (the forward FFT passes skip them)
 };
 
 // One CTA = one tile of TX x TY grid columns of one field triple.  Thread (ti, tj, tz) owns column (ti, tj) and the
@@ -306,11 +313,13 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
     }
     if (c0 + PCH < total) __syncthreads();
   }
-  // ---- store: every grid value written exactly once
+  // ---- store: every grid value of the planes that can hold force written exactly once
   if (in_grid) {
+    const int lm = __ldg(A.lmin);
 #pragma unroll
     for (int li = 0; li < NL; ++li) {
       const int l = ZSPLIT * li + tz;
+      if (l < lm) continue;
       GT* dst = reinterpret_cast<GT*>(A.grid) + (size_t)A.field0[grp] * A.real_field + ((size_t)l * g.ny + gj) * g.nx + gi;
 #pragma unroll
       for (int c = 0; c < 3; ++c) dst[c * A.real_field] = acc[li][c];
@@ -392,9 +401,11 @@ GridGeom make_geom(const dp_plan* P) {
 
 }  // namespace
 
-cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* force, const double* torque, cudaStream_t st) {
+cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* force, const double* torque, bool dense, cudaStream_t st) {
   GridGeom g = make_geom(P);
   cudaError_t e = cudaMemsetAsync(P->d_bin_count, 0, sizeof(int) * P->nbins, st);
+  if (e != cudaSuccess) return e;
+  e = cudaMemsetAsync(P->d_lmin, 0x7f, sizeof(int), st);          // 0x7f7f7f7f: "no plane touched yet"
   if (e != cudaSuccess) return e;
   e = cudaMemsetAsync(P->d_flag, 0, sizeof(int), st);
   if (e != cudaSuccess) return e;
@@ -402,7 +413,8 @@ cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* fo
   k_bin_count<<<B, T, 0, st>>>(n, pos, g, P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_flag);
   k_scan<<<1, 1024, 0, st>>>(P->nbins, P->d_bin_count, P->d_bin_start);
   k_bin_scatter<<<B, T, 0, st>>>(n, pos, force, torque, g, P->d_bin_of, P->d_slot_of, P->d_bin_start, P->d_znodes, P->d_perm, P->d_meta,
-                                P->d_pos_s, P->d_frc_s, P->fields == 6 ? P->d_trq_s : nullptr);
+                                P->d_pos_s, P->d_frc_s, P->fields == 6 ? P->d_trq_s : nullptr, P->d_lmin);
+  if (dense) { e = cudaMemsetAsync(P->d_lmin, 0, sizeof(int), st); if (e != cudaSuccess) return e; }   // every plane is transformed
   return cudaGetLastError();
 }
 
@@ -431,6 +443,7 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
   A.wrec = P->d_wrec; A.cap = (size_t)P->p.max_particles;
   A.grid = P->d_real;
   A.real_field = P->real_field;
+  A.lmin = P->d_lmin;
   dim3 grid(P->nbx, P->nby, ngroups);
   const bool f32 = P->p.transfer_fp32 != 0;
   switch (P->p.nz) {

@@ -295,3 +295,32 @@ def test_fp32_transfer_variant_matches_the_oracle_to_1e5(dp, case):
     # the variant needs the own FFT passes
     with pytest.raises(dp.DPError):
         dp.Plan(prob, max_particles=len(pos), use_torques=prob.has_torque, transfer_fp32=True, fft_backend=1)
+
+
+# ------------------------------------------------------------------------------------------------ zero planes
+def test_skipping_the_zero_planes_is_exact(dp):
+    """Planes above every footprint hold no force; the product skips their spreading stores, forward FFT passes and solve
+    loads.  Skipping changes no arithmetic: the result equals the dense-plane product to the run-to-run noise of the spreading order
+    and the oracle to 1e-10."""
+    import torch
+    prob, pos, F, T = small_monolayer("bw", 3000, 31)          # heights 1 + Exp(0.5): the top of the z grid stays empty
+    dpos, dF, dT = to_dev(pos, F, T)
+    out = {}
+    for dense in (False, True):
+        with dp.Plan(prob, max_particles=len(pos), use_torques=True, dense_planes=dense) as plan:
+            # stale data in the buffers must not matter: run a different product first
+            plan.mobility_apply(dpos, 3.0 * dF, dT)
+            U, Om = plan.mobility_apply(dpos, dF, dT)
+            torch.cuda.synchronize()
+            zp = plan.zero_planes()
+            assert (zp == 0) if dense else (3 <= zp < prob.nz), zp
+            out[dense] = (U.cpu().numpy(), Om.cpu().numpy())
+    # same arithmetic on the same values; only the bin order of spreading differs from run to run (<= 1e-13, reading G16)
+    assert rel_l2(out[False][0], out[True][0]) < 1e-13 and rel_l2(out[False][1], out[True][1]) < 1e-13
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft")
+    assert rel_l2(out[False][0], U_o) < TOL and rel_l2(out[False][1], Om_o) < TOL
+    # a slit with particles up to the top wall has no empty plane
+    prob, pos, F, T = small_monolayer("slit", 2500, 32)
+    with dp.Plan(prob, max_particles=len(pos), use_torques=True) as plan:
+        plan.mobility_apply(*to_dev(pos, F, T))
+        assert plan.zero_planes() == 0
