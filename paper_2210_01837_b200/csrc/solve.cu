@@ -88,12 +88,13 @@ template <int NZ> __device__ __forceinline__ void analysis_column(double* __rest
   e[0] *= 0.5; o[0] *= 0.5;
 #pragma unroll
   for (int j = 0; j < LH; ++j) {
-    double ae = 0.0, ao = 0.0;
+    double ae0 = 0.0, ae1 = 0.0, ao0 = 0.0, ao1 = 0.0;      // two partial sums per output (see synthesis_column)
 #pragma unroll
-    for (int l = 0; l < LH; ++l) {
-      ae = fma(T[(2 * j) * LH + l], e[l], ae);
-      ao = fma(T[(2 * j + 1) * LH + l], o[l], ao);
+    for (int l = 0; l < LH; l += 2) {
+      ae0 = fma(T[(2 * j) * LH + l], e[l], ae0); ae1 = fma(T[(2 * j) * LH + l + 1], e[l + 1], ae1);
+      ao0 = fma(T[(2 * j + 1) * LH + l], o[l], ao0); ao1 = fma(T[(2 * j + 1) * LH + l + 1], o[l + 1], ao1);
     }
+    const double ae = ae0 + ae1, ao = ao0 + ao1;
     v[(2 * j) * LN] = ae * (j == 0 ? 1.0 / N : 2.0 / N);
     v[(2 * j + 1) * LN] = ao * ((2 * j + 1 == N) ? 1.0 / N : 2.0 / N);
   }
@@ -107,14 +108,17 @@ template <int NZ> __device__ __forceinline__ void synthesis_column(double* __res
   double ce[LH], co[LH];
 #pragma unroll
   for (int j = 0; j < LH; ++j) { ce[j] = v[(2 * j) * LN]; co[j] = v[(2 * j + 1) * LN]; }
+  // two partial sums per output: with a single dependent chain per output the compiler interleaves many outputs and then
+  // spends one uniform-register move per DFMA on juggling the table operands
 #pragma unroll
   for (int l = 0; l < LH; ++l) {
-    double E = 0.0, O = 0.0;
+    double E0 = 0.0, E1 = 0.0, O0 = 0.0, O1 = 0.0;
 #pragma unroll
-    for (int j = 0; j < LH; ++j) {
-      E = fma(TE[l * LH + j], ce[j], E);
-      O = fma(TO[l * LH + j], co[j], O);
+    for (int j = 0; j < LH; j += 2) {
+      E0 = fma(TE[l * LH + j], ce[j], E0); E1 = fma(TE[l * LH + j + 1], ce[j + 1], E1);
+      O0 = fma(TO[l * LH + j], co[j], O0); O1 = fma(TO[l * LH + j + 1], co[j + 1], O1);
     }
+    const double E = E0 + E1, O = O0 + O1;
     v[l * LN] = E + O;
     v[(N - l) * LN] = E - O;
   }
