@@ -34,8 +34,8 @@ METRIC = "ms per DP-wall mobility product M·F at N=1M; particles/s; % of HBM ro
 # k_interp, plus k_fft_x_fwd, k_fft_y_fwd, k_fft_y_inv, k_fft_x_inv with the library's own FFT passes (else cuFFT's kernels)
 MY_KERNELS_PER_STEP = {"own": 12, "cufft": 8}
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one launch, from the committed ncu --set full capture
-# (profiles/r1_c_README.md); None where no capture exists for that workload
-NCU_TRAFFIC_GB = {("k_solve<32>", 5): 57.63}
+# (profiles/r1_d_README.md: 18.83 GB read with 11 of 32 input planes skipped + 29.00 GB written); None where no capture exists
+NCU_TRAFFIC_GB = {("k_solve<32>", 5): 47.83}
 
 
 def hbm_peak():
@@ -320,7 +320,7 @@ def main():
     traffic = NCU_TRAFFIC_GB.get((kernel_name, args.config))
     roofline = {"bound": "hbm", "kernel": kernel_name, "achieved": mine[dom]["GBps"], "peak": peak, "unit": "GB/s",
                 "frac": mine[dom]["frac"], "traffic": traffic * 1e9 if traffic else None, "peak_source": peak_src,
-                "note": "k_solve is co-bound by the fp64 pipe and shared memory (profiles/r1_c_README.md); the fraction is of the HBM roofline",
+                "note": "k_solve is co-bound by the fp64 pipe and shared memory (profiles/r1_d_README.md); the fraction is of the HBM roofline",
                 "fft_chebyshev_solve_stages": {"algorithmic_GB": mid, "ms": mid_ms, "GBps": mid / (mid_ms * 1e-3) if mid_ms else None,
                                                "frac": (mid / (mid_ms * 1e-3) / peak) if mid_ms else None},
                 "whole_product": {"algorithmic_GB": sum(by.values()) / 1e9, "ms": ms_step,
