@@ -345,13 +345,15 @@ constexpr int INTERP_WARPS = 8;
 
 // One warp per particle (sorted order, so neighbouring warps gather from neighbouring columns): the lanes sweep the
 // w x w x (lmax-lmin+1) footprint, weights come from the particle's records, the six sums are reduced by shuffles.
-template <class GT>
+// W = kernel support (compile-time: the footprint index arithmetic of the inner loop then has no integer division)
+template <class GT, int W>
 __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs A) {
   __shared__ double s_w[INTERP_WARPS][2][2 * DP_MAX_W + DP_MAX_NZ];   // per warp, per envelope: wx[8], wy[8], zeta[nz]
   __shared__ double s_zw[DP_MAX_NZ];
   const GridGeom& g = A.g;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const int nz = g.nz, w = g.w, wrec = 2 * DP_MAX_W + nz;
+  constexpr int w = W;
+  const int nz = g.nz, wrec = 2 * DP_MAX_W + nz;
   for (int i = threadIdx.x; i < nz; i += blockDim.x) s_zw[i] = A.zweights[i];
   __syncthreads();
   const int nk = A.Omega ? 2 : 1;
@@ -366,7 +368,9 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs 
         for (int e = lane; e < wrec; e += 32) s_w[wid][k][e] = rec[e];
       }
       __syncwarp();
-      const int ww = w * w, nent = (m.w - m.z + 1) * ww;
+      constexpr int ww = w * w;
+      const int nent = (m.w - m.z + 1) * ww;
+#pragma unroll 2
       for (int e = lane; e < nent; e += 32) {
         int l = m.z + e / ww, rem = e % ww, b = rem / w, a = rem % w;
         int i = m.x + a; if (i >= g.nx) i -= g.nx;
@@ -467,7 +471,16 @@ cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaSt
   const int maxb = 148 * 64;
   if (blocks > maxb) blocks = maxb;
   if (blocks < 1) blocks = 1;
-  if (P->p.transfer_fp32) k_interp<float><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A);
-  else k_interp<double><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A);
+  const bool f32 = P->p.transfer_fp32 != 0;
+#define DP_INTERP_CASE(WW)                                                              \
+  case WW:                                                                              \
+    if (f32) k_interp<float, WW><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A);           \
+    else k_interp<double, WW><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A);              \
+    break;
+  switch (P->p.w) {
+    DP_INTERP_CASE(4) DP_INTERP_CASE(5) DP_INTERP_CASE(6) DP_INTERP_CASE(7) DP_INTERP_CASE(8)
+    default: return cudaErrorInvalidValue;
+  }
+#undef DP_INTERP_CASE
   return cudaGetLastError();
 }
