@@ -216,6 +216,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
   __shared__ double s_w[PCH][WREC];
   __shared__ double s_val[PCH][3];
   __shared__ int4 s_meta[PCH];                // i0, j0 (wrapped origin node), lmin, lmax
+  __shared__ int s_src[PCH];                  // index of each staged candidate in the sorted particle arrays
   __shared__ int s_rbeg[MAXR], s_roff[MAXR + 1];   // candidate ranges in the sorted arrays; prefix sums of their lengths
 
   const GridGeom& g = A.g;
@@ -264,23 +265,23 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
   // batch of independent coalesced loads); the exact footprint test happens per thread in the accumulation loop.
   for (int c0 = 0; c0 < total; c0 += PCH) {
     const int nl = min(PCH, total - c0);
-    if (t < nl) {
+    if (t < nl) {                                             // position of candidate c0 + t in the sorted arrays, once
       const int c = c0 + t;
       int r = 0;
 #pragma unroll
       for (int q = 1; q < MAXR; ++q) r += (c >= s_roff[q]) ? 1 : 0;
-      const int p = s_rbeg[r] + (c - s_roff[r]);
+      s_src[t] = s_rbeg[r] + (c - s_roff[r]);
+    }
+    __syncthreads();
+    if (t < nl) {
+      const int p = s_src[t];
       s_meta[t] = A.meta[p];
       s_val[t][0] = val[3 * (size_t)p]; s_val[t][1] = val[3 * (size_t)p + 1]; s_val[t][2] = val[3 * (size_t)p + 2];
     }
 #pragma unroll 2
     for (int i = t; i < nl * WREC; i += SPREAD_THREADS) {
-      const int q = i / WREC, e = i - q * WREC, c = c0 + q;
-      int r = 0;
-#pragma unroll
-      for (int k = 1; k < MAXR; ++k) r += (c >= s_roff[k]) ? 1 : 0;
-      const int p = s_rbeg[r] + (c - s_roff[r]);
-      s_w[q][e] = wrec[(size_t)p * WREC + e];
+      const int q = i / WREC, e = i - q * WREC;
+      s_w[q][e] = wrec[(size_t)s_src[q] * WREC + e];
     }
     __syncthreads();
     // ---- accumulate: each thread adds the particles covering its column to its own planes
