@@ -59,6 +59,27 @@ def stage_bytes(prob, n, fin, fout, zero_planes=0):
             "fft_inv": fout * (C + R), "interp": fout * R + 72.0 * n}
 
 
+def replica_seed(base_seed: int, rank: int) -> int:
+    """N > 1 = N independent replicas (the product does not shard): each rank draws its own particles from
+    the same recipe; rank 0 keeps the configuration's own seed."""
+    return base_seed + 17 * rank
+
+
+def max_over_ranks(dist, value: float, device) -> float:
+    """Device time of the slowest rank (the contract's timing rule); no other collective exists on this path."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(n_per_rank: int, world: int, ms_step: float) -> float:
+    """particles/s of all replicas together."""
+    return world * n_per_rank / (ms_step * 1e-3)
+
+
 class ClockSampler(threading.Thread):
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -184,7 +205,7 @@ def main():
 
     prob, pos, F, T = workloads.config(args.config)
     if world > 1:      # replicas: each rank draws its own particles from the same recipe
-        prob, pos, F, T = (workloads.monolayer_bw(n=prob.n, seed=prob.seed + 17 * rank, name=prob.name) if args.config in (3, 5)
+        prob, pos, F, T = (workloads.monolayer_bw(n=prob.n, seed=replica_seed(prob.seed, rank), name=prob.name) if args.config in (3, 5)
                            else workloads.config(args.config))
     n = len(pos)
     fin = 6 if T is not None else 3
@@ -230,12 +251,8 @@ def main():
     stage_ms = {k: float(np.median(v)) for k, v in stage_acc.items()}
     assert plan.check() == 0
     zero_planes = plan.zero_planes()
-    ms_step = ms_total / args.steps
-    if dist is not None:
-        t = torch.tensor([ms_step], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step = float(t.item())
-    value = world * n / (ms_step * 1e-3)
+    ms_step = max_over_ranks(dist, ms_total / args.steps, dev)
+    value = whole_job_value(n, world, ms_step)
 
     # ---- end to end: host buffers in (pinned), host buffers out, through dp_mobility_apply_host
     e2e = None
@@ -251,11 +268,7 @@ def main():
         t0 = time.perf_counter()
         for _ in range(args.steps):
             plan.mobility_apply_host(npv(hp), npv(hF), npv(hT), out_U=npv(hU), out_Omega=npv(hO))   # synchronous
-        dt = (time.perf_counter() - t0) / args.steps
-        if dist is not None:
-            t = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = max_over_ranks(dist, (time.perf_counter() - t0) / args.steps, dev)
         e2e = {"value": world * n / dt, "unit": "particles/s", "ms_per_step": dt * 1e3,
                "h2d_bytes_per_step": int(24 * n * (3 if T is not None else 2)), "d2h_bytes_per_step": int(24 * n * (2 if T is not None else 1))}
 
@@ -278,11 +291,7 @@ def main():
             plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
         v1.record(stream)
         barrier()
-        vms = v0.elapsed_time(v1) / args.steps
-        if dist is not None:
-            t = torch.tensor([vms], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            vms = float(t.item())
+        vms = max_over_ranks(dist, v0.elapsed_time(v1) / args.steps, dev)
         plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
         vst = plan.stage_ms()
         return {"ms_per_step": vms, "value": world * n / (vms * 1e-3), "unit": "particles/s",
