@@ -4,8 +4,9 @@
  *
  * for N regularised blobs above one no-slip wall ("bottom wall") or between two ("slit channel"), doubly periodic
  * in x, y: the method of Hashemi et al., arXiv 2210.01837.  One call of dp_mobility_apply runs the paper's
- * steps 1-8 (Sec. III D) entirely in hand-written CUDA kernels for sm_100a plus cuFFT for the
- * batched xy FFTs:
+ * steps 1-8 (Sec. III D) entirely in this library's hand-written CUDA kernels for sm_100a (the xy
+ * FFTs included: two shared-memory passes per direction; cuFFT only when fft_backend = 1 asks for it or the grid size
+ * has a prime factor > 5):
  *   step 1  spread F (and tau) with the exponential-of-semicircle kernel and wall images   eqs 7, 9, 53, 54
  *   step 2  2D FFT in xy, Chebyshev transform in z, Chebyshev differentiation
  *   step 3  per (kx,ky): pressure BVP eq 15 + BCs 17; velocity BVPs eq 18 + BCs 22, 24
@@ -15,7 +16,7 @@
  *   step 7  inverse transforms
  *   step 8  interpolate u (and (1/2) curl u) back to the particles, eqs 10, 11
  * The exact discrete problem (grid, transforms, tau/integration BVP form, Nyquist rule, scalings) is stated in
- * DESIGN.md; tests compare every output with the CPU oracle in oracle/ (relative L2 <= 1e-10 in fp64).
+ * DESIGN.md §2; tests compare every output with the CPU oracle in oracle/ (relative L2 <= 1e-10 in fp64).
  *
  * Conventions
  *  - All functions return DP_OK (0) or a negative error code; nothing throws across this boundary.
@@ -24,7 +25,10 @@
  *  - x, y may be any real number (wrapped periodically into [0,Lx) x [0,Ly)).  z must satisfy 0 <= z <= H and, for the
  *    bottom wall, z + alpha <= H with alpha = w h / 2 (kernels must not cross the open top): a
  *    particle violating this contributes nothing, receives U = Omega = 0, and is reported by dp_check().
- *  - A plan is not thread-safe: one dp_mobility_apply in flight per plan.  Plans are immutable after creation.
+ *  - A plan is not thread-safe: one call in flight per plan.  Plans are immutable after creation.  Every entry point
+ *    that touches the device makes the plan's device current for its own duration and restores the caller's device;
+ *    all device state (tables, workspaces, kernel attributes) is per plan, so plans on different devices coexist in
+ *    one process.
  */
 #ifndef DP_STOKES_H
 #define DP_STOKES_H
@@ -35,41 +39,49 @@
 extern "C" {
 #endif
 
-typedef struct dp_plan dp_plan; /* opaque: owns grids, cuFFT plans, tables, workspace */
+typedef struct dp_plan dp_plan; /* opaque: owns grids, FFT tables (or cuFFT plans), solver tables, workspace */
 
 enum { DP_BOTTOM_WALL = 0, DP_SLIT = 1 };
 enum { DP_OK = 0, DP_EINVAL = -1, DP_ENOMEM = -2, DP_ECUDA = -3, DP_ECUFFT = -4, DP_EDOMAIN = -5 };
 
+/* Problem statement of the paper: box doubly periodic in xy with wall(s), ES kernel (w, beta) per envelope
+ * (eqs 53-54), viscosity.  The first block of fields is SURVEY.md §8(b)'s struct; the second block
+ * ("extensions") was added by this build and is documented in DESIGN.md §1. */
 typedef struct {
-  int wall_mode;        /* DP_BOTTOM_WALL: wall at z=0, open top at z=H;  DP_SLIT: walls at z=0 and z=H            */
-  double Lx, Ly, H;     /* FULL periods in x, y (reading G1); top of the Chebyshev grid                   */
+  int wall_mode;        /* DP_BOTTOM_WALL: wall at z=0, open top at z=H;  DP_SLIT: walls at z=0 and z=H   */
+  double Lx, Ly, H;     /* FULL periods in x, y (reading G1); top of the Chebyshev grid                       */
   int nx, ny, nz;       /* grid: uniform in x,y (h = Lx/nx = Ly/ny to 1e-12 relative; nx, ny even), nz type-2
                            Chebyshev nodes z_l = (H/2)(1+cos(l pi/(nz-1))) including both ends;
-                           nz must be one of the compiled sizes (dp_supported_nz)                                    */
-  int w;                /* ES kernel support in cells (paper's m), 4..8; alpha = w h/2               */
-  double beta_M;        /* ES beta of the monopole envelope Delta_M (eq 54; beta, not beta/w)                        */
-  double beta_D;        /* ES beta of the dipole envelope Delta_D; ignored if torques/Omega are never used           */
-  double eta;           /* viscosity > 0                                                                            */
-  int max_particles;    /* capacity of the plan's particle workspace                                                 */
-  int use_torques;      /* 0: forces in, U out only (3 grid fields); 1: also torques in / Omega out (6 fields)       */
-  int device;           /* CUDA device ordinal                                                                       */
-  int fft_backend;      /* 0: the library's own shared-memory FFT passes when nx, ny allow them (nx/2 and ny products
-                           of 2, 3, 5; nx <= 4320, ny <= 4320), else cuFFT;  1: always cuFFT (kept for comparison)    */
+                           8 <= nz <= 64 (dp_supported_nz lists the sizes with a compiled fast path)                     */
+  int w;                /* ES kernel support in cells (paper's m), 4..8; alpha = w h/2                   */
+  double beta_M;        /* ES beta of the monopole envelope Delta_M (eq 54; beta, not beta/w)                            */
+  double beta_D;        /* ES beta of the dipole envelope Delta_D; ignored if torques/Omega are never used               */
+  double a;             /* nominal blob radius: informational only (nothing in the product depends on it, G9);
+                           compare with dp_effective_radius()                                                             */
+  double eta;           /* viscosity > 0                                                                                */
+  int max_particles;    /* capacity of the plan's particle workspace                                                     */
   int transfer_fp32;    /* 0: everything fp64;  1: optional variant — spreading and interpolation accumulate in fp32 and
                            the real-space grids are stored in fp32 (half the bytes of steps 1, 8 and of the real side of the
                            x FFT passes); transforms and solves stay fp64.  Needs the own FFT passes (fft_backend = 0 and a
                            supported size).  Matches the fp64 product to ~1e-6 relative (tests: <= 1e-5 vs the oracle).   */
+  int device;           /* CUDA device ordinal                                                                           */
+  /* ---- extensions beyond SURVEY.md §8(b) ---- */
+  int use_torques;      /* 0: forces in, U out only (3 grid fields); 1: also torques in / Omega out (6 fields) */
+  int fft_backend;      /* 0: the library's own shared-memory FFT passes when nx, ny allow them (nx/2 and ny products
+                           of 2, 3, 5; nx, ny <= 4320), else cuFFT;  1: always cuFFT (kept for comparison)                */
   int dense_planes;     /* 0 (default): planes of the Chebyshev grid above every particle's footprint hold no force, so their
                            forward transforms are identically zero; the product finds the highest touched plane while
                            binning and skips the spreading stores, forward FFT passes and solve loads of the planes above
                            it (exact: the skipped values are zeros).  1: treat every plane as dense.                        */
 } dp_params;
 
-/* Validate, allocate (2 grids of fields*nz*ny*(nx+2) doubles + cuFFT workspace + particle workspace), plan the FFTs,
- * upload tables.  Synchronous.  *out = NULL on error. */
+/* Plan creation for the problem of PAPER.md:74 (box, walls) with the grid of PAPER.md:319 and the ES kernel of eq 54.
+ * Validates, allocates (two grids of fields*nz*ny*nx doubles resp. fields*nz*(nx/2+1)*ny complex + particle workspace),
+ * builds the FFT twiddle tables (or cuFFT plans), uploads the solver tables.  Synchronous.  *out = NULL on error. */
 int dp_create(const dp_params* p, dp_plan** out);
 
-/* One mobility product, asynchronous on `cuda_stream` (a cudaStream_t; NULL = default stream).  DEVICE pointers.
+/* One mobility product (U, Omega) = M (F, tau): eqs 2, 7, 10, 11 by steps 1-8 of Sec. III D
+ * (PAPER.md:325-333).  Asynchronous on `cuda_stream` (a cudaStream_t; NULL = default stream).  DEVICE pointers.
  *   pos    [n][3]  positions
  *   force  [n][3]  or NULL (treated as zero)
  *   torque [n][3]  or NULL; non-NULL requires use_torques = 1
@@ -80,37 +92,51 @@ int dp_create(const dp_params* p, dp_plan** out);
 int dp_mobility_apply(dp_plan* plan, int n, const double* pos, const double* force, const double* torque,
                       double* U, double* Omega, void* cuda_stream);
 
-/* Same product with HOST pointers: copies inputs to the device, runs dp_mobility_apply, copies U (and Omega) back and
- * synchronises.  This is the end-to-end entry point bench.py times as "e2e". */
+/* The same product (same equations) with HOST pointers: copies inputs to the device, runs dp_mobility_apply, copies U
+ * (and Omega) back and synchronises.  This is the end-to-end entry point bench.py times as "e2e". */
 int dp_mobility_apply_host(dp_plan* plan, int n, const double* pos, const double* force, const double* torque,
                            double* U, double* Omega);
 
-/* Synchronise the last stream used and report DP_EDOMAIN if any particle of the last apply was out of domain. */
+/* Domain check of the last product: "kernels must never extend outside open boundaries" (footnote 44) and
+ * 0 <= z <= H.  Synchronises the last stream used; DP_EDOMAIN if any particle of the last apply was out of domain. */
 int dp_check(dp_plan* plan);
 
+/* Effective hydrodynamic radius R_h (a length, = c(beta) h) of a blob regularised by the plan's ES kernel in an unbounded
+ * fluid: dipole = 0: from the translational self mobility 1/(6 pi eta R_h) of Delta_M; dipole = 1: from the rotational self
+ * mobility 1/(8 pi eta R_h^3) of Delta_D (eq 8, for the Gaussian analogue; eq 56: R_h/h
+ * is intrinsic to the kernel; Tables I-II, print it).  Host-side 1-D quadrature (DESIGN.md pin P1), no
+ * device work.  Returns a negative number on a NULL plan or dipole = 1 on a plan without torques. */
+double dp_effective_radius(const dp_plan* plan, int dipole);
+
 /* Per-stage device times (ms) of the LAST apply, measured with CUDA events on its stream; synchronises.
- * ms[0] bin, [1] spread, [2] xy FFT forward, [3] per-wavenumber solve (z transforms + BVPs + correction + curl),
- * [4] xy FFT inverse, [5] interpolate, [6] k=0 column, [7] total.  Only recorded if dp_set_profiling(plan, 1). */
+ * ms[0] bin, [1] spread (step 1), [2] xy FFT forward (step 2), [3] per-wavenumber solve (z transforms + BVPs + correction +
+ * curl, steps 2-6), [4] xy FFT inverse (step 7), [5] interpolate (step 8), [6] k=0 column, [7] total.
+ * Only recorded if dp_set_profiling(plan, 1). */
 int dp_set_profiling(dp_plan* plan, int on);
 int dp_stage_ms(dp_plan* plan, float* ms /* [8] */);
 
-/* Test hook: copy an internal device buffer of the last apply to HOST memory (synchronises).
+/* Test hooks: copy an internal device buffer of the last apply to HOST memory (synchronises).
  *   which = 0: real grid    [fields][nz][ny][nx]       doubles  (after apply: u, (1/2) curl u in real space)
  *   which = 1: complex grid [fields][nz][ny][nkxp]     double2  (after apply: consumed by the inverse FFT, undefined;
  *              with the own FFT passes the internal layout is transposed and digit-reversed in ky — the copy undoes it)
- * dp_debug_run_stage runs the product up to and including `last_stage` (1 spread, 2 fwd FFT, 3 solve, 4 inv FFT) so
- * that the buffers hold that stage's output.  Sizes via dp_buffer_bytes. */
+ * dp_debug_run_stage runs the product up to and including `last_stage` (1 spread = step 1, 2 fwd FFT = step 2(xy), 3 solve =
+ * steps 2(z)-6, 4 inv FFT = step 7) so that the buffers hold that stage's output.  Sizes via dp_buffer_bytes.
+ * dp_copy_plane_to_host copies ONE xy plane (field, l) of buffer `which`: ny*nx doubles resp. ny*nkxp double2 in the
+ * natural layout — what the full-size parity tests use to compare sampled planes and columns with the oracle. */
 int dp_debug_run_stage(dp_plan* plan, int n, const double* pos, const double* force, const double* torque, int last_stage,
                        void* cuda_stream);
 size_t dp_buffer_bytes(const dp_plan* plan, int which);
 int dp_copy_buffer_to_host(dp_plan* plan, int which, void* host, size_t bytes);
+int dp_copy_plane_to_host(dp_plan* plan, int which, int field, int l, void* host, size_t bytes);
 int dp_complex_row_pitch(const dp_plan* plan); /* nkxp: padded row length (in complex numbers) of the half spectrum */
 int dp_zero_planes(dp_plan* plan);             /* synchronises; number of leading planes (l = 0 is z = H) the last apply skipped */
 int dp_fft_backend(const dp_plan* plan);       /* 0: own shared-memory FFT passes in use, 1: cuFFT                    */
 
 /* Introspection */
-double dp_es_norm(double alpha, double beta);                  /* Z of eq 54, Gauss-Legendre on the host             */
-int dp_supported_nz(int* out, int cap);                        /* compiled Chebyshev sizes; returns how many          */
+double dp_es_norm(double alpha, double beta);                  /* Z of eq 54, Gauss-Legendre on the host */
+double dp_es_radius_over_h(int w, double beta, int dipole);    /* c(beta) = R_h/h of eq 56 for support w and this
+                                                                  beta: what dp_effective_radius divides by h; needs no plan  */
+int dp_supported_nz(int* out, int cap);                        /* Chebyshev sizes with a compiled solve kernel; returns how many */
 size_t dp_device_bytes(const dp_plan* plan);                   /* device memory owned by the plan                     */
 const char* dp_strerror(int code);
 const char* dp_last_error(const dp_plan* plan);                /* detail of the last failure (CUDA / cuFFT message)   */

@@ -6,9 +6,11 @@ path and never imports ``paper_2210_01837_b200``.
 
 The arithmetic lives in ``dp_oracle.cpp`` (plain C++, fp64 with long-double dense solves, explicit O(n^2)
 DFT sums); this file only builds it, marshals numpy arrays, and strings the paper's eight steps
- together in the paper's order.  ``dft="fft"`` replaces the explicit xy DFT sums by the
-library primitive ``numpy.fft.rfft2 / irfft2`` (same definition, see ``tests/test_oracle_dft.py``) so that
-the large configurations finish; everything else is unchanged.
+ together in the paper's order.  The xy transforms (O2, O11) exist in three forms of the SAME sums:
+``dft="naive"`` — the explicit O(n^2) sums (the definition); ``dft="fft"`` — the oracle's own plain recursive
+mixed-radix FFT in ``dp_oracle.cpp`` (allowed beyond the sizes the naive sums finish, validated
+against them in ``tests/test_oracle_basics.py``); ``dft="numpy"`` — ``numpy.fft.rfft2 / irfft2``, kept only as an
+independent cross-check of the other two.  Everything else is unchanged by the choice.
 """
 from __future__ import annotations
 
@@ -62,6 +64,9 @@ def lib():
         L.or_interp.argtypes = [p, i, p, p, d, p]
         L.or_dft_xy_forward.argtypes = [i, i, ctypes.c_long, p, p]
         L.or_dft_xy_inverse.argtypes = [i, i, ctypes.c_long, p, p]
+        L.or_fft_xy_forward.argtypes = [i, i, ctypes.c_long, p, p]
+        L.or_fft_xy_inverse.argtypes = [i, i, ctypes.c_long, p, p]
+        L.or_solve_modes.argtypes = [p, ctypes.c_long, p, p, p, p, p, p]
         L.or_bvp_solve.argtypes = [i, d, d, p, p, p, p]
         L.or_solve.argtypes = [p, p, p, p, p, p]
         _lib = L
@@ -163,10 +168,11 @@ def dft_xy_forward(real: np.ndarray, dft: str = "naive") -> np.ndarray:
     """Step 2, xy part (O2): unnormalised forward DFT over the last two axes (j, i) -> half spectrum (ny, nx/2+1)."""
     real = _f64(real)
     ny, nx = real.shape[-2:]
-    if dft == "fft":
+    if dft == "numpy":
         return np.ascontiguousarray(np.fft.rfft2(real, axes=(-2, -1)))
     out = np.empty(real.shape[:-1] + (nx // 2 + 1,), dtype=np.complex128)
-    lib().or_dft_xy_forward(nx, ny, int(np.prod(real.shape[:-2], dtype=np.int64)), _ptr(real), _ptr(out))
+    fn = {"naive": lib().or_dft_xy_forward, "fft": lib().or_fft_xy_forward}[dft]
+    fn(nx, ny, int(np.prod(real.shape[:-2], dtype=np.int64)), _ptr(real), _ptr(out))
     return out
 
 
@@ -174,10 +180,11 @@ def dft_xy_inverse(spec: np.ndarray, nx: int, dft: str = "naive") -> np.ndarray:
     """Step 7, xy part (O11): inverse DFT with Hermitian completion and 1/(nx ny)."""
     spec = np.ascontiguousarray(spec, dtype=np.complex128)
     ny = spec.shape[-2]
-    if dft == "fft":
+    if dft == "numpy":
         return np.ascontiguousarray(np.fft.irfft2(spec, s=(ny, nx), axes=(-2, -1)))
     out = np.empty(spec.shape[:-1] + (nx,))
-    lib().or_dft_xy_inverse(nx, ny, int(np.prod(spec.shape[:-2], dtype=np.int64)), _ptr(spec), _ptr(out))
+    fn = {"naive": lib().or_dft_xy_inverse, "fft": lib().or_fft_xy_inverse}[dft]
+    fn(nx, ny, int(np.prod(spec.shape[:-2], dtype=np.int64)), _ptr(spec), _ptr(out))
     return out
 
 
@@ -193,11 +200,28 @@ def solve(prob, fh, th=None, want_omega=False, want_coef=False):
     return uh, wh, dump
 
 
+def solve_modes(prob, ix, iy, fh, th=None, want_omega=False):
+    """Steps 2(z)-6 (O3-O10) on a LIST of wavenumbers: column q of ``fh`` / ``th`` ([3, nz, nmodes]) is the nodal-in-z
+    spectrum at (kx index ix[q], ky index iy[q] in FFT order).  Same arithmetic as ``solve`` (one body in dp_oracle.cpp)."""
+    ix = np.ascontiguousarray(ix, dtype=np.int32)
+    iy = np.ascontiguousarray(iy, dtype=np.int32)
+    fh = np.ascontiguousarray(fh, dtype=np.complex128)
+    th = None if th is None else np.ascontiguousarray(th, dtype=np.complex128)
+    assert fh.shape == (3, prob.nz, len(ix)) and len(ix) == len(iy)
+    P = _params(prob)
+    uh = np.empty_like(fh)
+    wh = np.empty_like(fh) if want_omega else None
+    lib().or_solve_modes(ctypes.byref(P), len(ix), _ptr(ix), _ptr(iy), _ptr(fh), _ptr(th), _ptr(uh), _ptr(wh))
+    return uh, wh
+
+
 def mobility_apply(prob, pos, force=None, torque=None, want_omega=None, dft="naive", stages=None, timing=None):
     """(U, Omega) = M (F, tau): the paper's steps 1-8 in order.
 
     ``stages`` (dict) receives the intermediate arrays (grid after spread, spectra, ...) when given.
     ``timing`` (dict) receives per-step wall-clock seconds when given.
+    Intermediate arrays are released as soon as the next step has consumed them (unless ``stages`` keeps them), so that
+    the large configurations fit in host memory.
     """
     if force is None and torque is None:
         raise ValueError("need forces and/or torques")
@@ -205,21 +229,31 @@ def mobility_apply(prob, pos, force=None, torque=None, want_omega=None, dft="nai
         want_omega = torque is not None
     n = np.asarray(pos).shape[0]
     tm = {} if timing is None else timing
+    keep = stages is not None
     t0 = time.perf_counter()
     f = spread(prob, pos, force if force is not None else np.zeros((n, 3)), prob.beta_M)          # step 1
     t = spread(prob, pos, torque, prob.beta_D) if torque is not None else None
     tm["spread"] = time.perf_counter() - t0; t0 = time.perf_counter()
     fh = dft_xy_forward(f, dft)                                                                      # step 2 (xy)
     th = dft_xy_forward(t, dft) if t is not None else None
+    if keep:
+        stages.update(f=f, t=t)
+    del f, t
     tm["dft_fwd"] = time.perf_counter() - t0; t0 = time.perf_counter()
-    uh, wh, coef = solve(prob, fh, th, want_omega=want_omega, want_coef=stages is not None)       # steps 2(z)-6
+    uh, wh, coef = solve(prob, fh, th, want_omega=want_omega, want_coef=keep)                     # steps 2(z)-6
+    if keep:
+        stages.update(fh=fh, th=th, ucoef=coef)
+    del fh, th, coef
     tm["solve"] = time.perf_counter() - t0; t0 = time.perf_counter()
     u = dft_xy_inverse(uh, prob.nx, dft)                                                             # step 7
     om = dft_xy_inverse(wh, prob.nx, dft) if want_omega else None
+    if keep:
+        stages.update(uh=uh, wh=wh)
+    del uh, wh
     tm["dft_inv"] = time.perf_counter() - t0; t0 = time.perf_counter()
     U = interp(prob, pos, u, prob.beta_M)                                                            # step 8
     Om = interp(prob, pos, om, prob.beta_D) if want_omega else None
     tm["interp"] = time.perf_counter() - t0
-    if stages is not None:
-        stages.update(f=f, t=t, fh=fh, th=th, uh=uh, wh=wh, ucoef=coef, u=u, om=om)
+    if keep:
+        stages.update(u=u, om=om)
     return U, Om

@@ -321,6 +321,110 @@ void or_dft_xy_inverse(int nx, int ny, long nplanes, const double* in_ri, double
 }  // extern "C"
 
 // ------------------------------------------------------------------------------------------------
+// The oracle's own plain FFT (SURVEY.md §8(d) "CPU baseline": "its own plain recursive mixed-radix FFT, validated
+// against its naive DFT").  It computes exactly the sums of or_dft_xy_forward / or_dft_xy_inverse (O2, O11), by the
+// textbook Cooley-Tukey recursion on the smallest prime factor p of n (n = p m):
+//   X[k + q m] = sum_{r<p} W_n^{r (k + q m)} Y_r[k],   Y_r = DFT_m of x[r], x[r+p], ...,   k < m, q < p,
+// and the plain O(n^2) sum when n is prime.  No real-input trick, no blocking, out of place, twiddles from one table
+// exp(sign 2 pi i j / n) evaluated in long double.  Pinned against the naive sums in tests/test_oracle_basics.py.
+static int smallest_prime_factor(int n) {
+    for (int p = 2; (long)p * p <= n; ++p) if (n % p == 0) return p;
+    return n;
+}
+
+// DFT of the n numbers in[0], in[istride], ... -> out[0..n-1]; root[j * rstep] = exp(sign 2 pi i j / n), j < n
+static void fft_plain(int n, const cd* in, long istride, cd* out, const cd* root, long rstep) {
+    if (n == 1) { out[0] = in[0]; return; }
+    const int p = smallest_prime_factor(n), m = n / p;
+    if (p == n) {
+        for (int k = 0; k < n; ++k) {
+            cd s = 0;
+            for (int j = 0; j < n; ++j) s += in[j * istride] * root[(long)((long)j * k % n) * rstep];
+            out[k] = s;
+        }
+        return;
+    }
+    for (int r = 0; r < p; ++r) fft_plain(m, in + r * istride, istride * p, out + (long)r * m, root, rstep * p);
+    cd tsmall[8];
+    std::vector<cd> tlarge;
+    cd* t = tsmall;
+    if (p > 8) { tlarge.resize(p); t = tlarge.data(); }
+    for (int k = 0; k < m; ++k) {
+        for (int r = 0; r < p; ++r) t[r] = out[(long)r * m + k] * root[(long)r * k * rstep];              // W_n^{r k}, r k < n
+        for (int q = 0; q < p; ++q) {
+            cd s = 0;
+            for (int r = 0; r < p; ++r) s += t[r] * root[(long)((r * q) % p) * m * rstep];                  // W_n^{r q m} = W_p^{r q}
+            out[k + (long)q * m] = s;
+        }
+    }
+}
+
+static void root_table(int n, int sign, std::vector<cd>& root) {
+    root.resize(n);
+    for (int j = 0; j < n; ++j) root[j] = cd((double)cosl(2 * PI_L * j / n), (double)(sign * sinl(2 * PI_L * j / n)));
+}
+
+extern "C" {
+
+// O2 through fft_plain: same definition as or_dft_xy_forward (x then y, unnormalised, half spectrum kept)
+void or_fft_xy_forward(int nx, int ny, long nplanes, const double* in, double* out_ri) {
+    cd* out = reinterpret_cast<cd*>(out_ri);
+    const int nkx = nx / 2 + 1;
+    std::vector<cd> rx, ry;
+    root_table(nx, -1, rx); root_table(ny, -1, ry);
+#pragma omp parallel
+    {
+        std::vector<cd> row(nx), spec(nx), g((size_t)ny * nkx), col(ny), cs(ny);
+#pragma omp for schedule(dynamic, 1)
+        for (long pl = 0; pl < nplanes; ++pl) {
+            const double* f = in + (size_t)pl * nx * ny;
+            for (int j = 0; j < ny; ++j) {
+                for (int i = 0; i < nx; ++i) row[i] = cd(f[(size_t)j * nx + i], 0.0);
+                fft_plain(nx, row.data(), 1, spec.data(), rx.data(), 1);
+                for (int kx = 0; kx < nkx; ++kx) g[(size_t)j * nkx + kx] = spec[kx];
+            }
+            cd* o = out + (size_t)pl * ny * nkx;
+            for (int kx = 0; kx < nkx; ++kx) {
+                for (int j = 0; j < ny; ++j) col[j] = g[(size_t)j * nkx + kx];
+                fft_plain(ny, col.data(), 1, cs.data(), ry.data(), 1);
+                for (int ky = 0; ky < ny; ++ky) o[(size_t)ky * nkx + kx] = cs[ky];
+            }
+        }
+    }
+}
+
+// O11 through fft_plain: inverse in y on the half spectrum, Hermitian completion of every x row
+// (u^(nx - n_x) = conj u^(n_x) after the y sum), inverse in x, real part, 1/(nx ny)
+void or_fft_xy_inverse(int nx, int ny, long nplanes, const double* in_ri, double* out) {
+    const cd* in = reinterpret_cast<const cd*>(in_ri);
+    const int nkx = nx / 2 + 1;
+    std::vector<cd> rx, ry;
+    root_table(nx, +1, rx); root_table(ny, +1, ry);
+#pragma omp parallel
+    {
+        std::vector<cd> row(nx), res(nx), g((size_t)ny * nkx), col(ny), cs(ny);
+#pragma omp for schedule(dynamic, 1)
+        for (long pl = 0; pl < nplanes; ++pl) {
+            const cd* uh = in + (size_t)pl * ny * nkx;
+            for (int kx = 0; kx < nkx; ++kx) {
+                for (int ky = 0; ky < ny; ++ky) col[ky] = uh[(size_t)ky * nkx + kx];
+                fft_plain(ny, col.data(), 1, cs.data(), ry.data(), 1);
+                for (int j = 0; j < ny; ++j) g[(size_t)j * nkx + kx] = cs[j];
+            }
+            double* u = out + (size_t)pl * nx * ny;
+            for (int j = 0; j < ny; ++j) {
+                for (int kx = 0; kx < nkx; ++kx) row[kx] = g[(size_t)j * nkx + kx];
+                for (int kx = 1; kx < nkx; ++kx) if (nx - kx >= nkx) row[nx - kx] = std::conj(g[(size_t)j * nkx + kx]);
+                fft_plain(nx, row.data(), 1, res.data(), rx.data(), 1);
+                for (int i = 0; i < nx; ++i) u[(size_t)j * nx + i] = res[i].real() / ((double)nx * ny);
+            }
+        }
+    }
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------
 // Dense LU with partial pivoting, long double matrix (real), complex or real right-hand sides.
 struct LU {
     int n;
@@ -442,12 +546,18 @@ void or_bvp_solve(int nz, double H, double k, const double* r_ri, const double* 
     for (int n = 0; n < nz; ++n) { y_ri[2 * n] = (double)b[n].real(); y_ri[2 * n + 1] = (double)b[n].imag(); }
 }
 
-// O3-O10 for every retained wavenumber.  Inputs: nodal-in-z half spectra of the spread force field fh[3][nz][ny][nkx]
-// and (optional) torque field th; outputs: nodal-in-z half spectra of u (uh) and, if wanted, of (1/2) curl u (wh).
-// If dump_coef != NULL it receives the Chebyshev coefficients of the total velocity [3][nz][ny][nkx] (stage dump).
-void or_solve(const or_params* P, const double* fh_ri, const double* th_ri, double* uh_ri, double* wh_ri, double* dump_coef_ri) {
+}  // extern "C"
+
+// O3-O10 for a set of retained wavenumbers.  Inputs: nodal-in-z spectra of the spread force field fh[3][nz][K] and
+// (optional) torque field th, K columns, column q belonging to the wavenumber index pair (ix, iy); outputs: nodal-in-z
+// spectra of u (uh) and, if wanted, of (1/2) curl u (wh), same layout.  ixs == NULL: the columns are the whole half
+// spectrum in its natural order, K = ny * nkx, q = iy * nkx + ix (or_solve); else column q is mode (ixs[q], iys[q])
+// (or_solve_modes: the same body on a list of modes, for full-size parity checks on sampled columns).
+// If dump_coef != NULL it receives the Chebyshev coefficients of the total velocity [3][nz][K] (stage dump).
+static void solve_columns(const or_params* P, long ncols, const int* ixs, const int* iys, const double* fh_ri, const double* th_ri,
+                          double* uh_ri, double* wh_ri, double* dump_coef_ri) {
     const int nx = P->nx, ny = P->ny, nz = P->nz, nkx = nx / 2 + 1;
-    const size_t K = (size_t)ny * nkx, field = K * nz;
+    const size_t K = (size_t)ncols, field = K * nz;
     const cd* fh = reinterpret_cast<const cd*>(fh_ri);
     const cd* th = reinterpret_cast<const cd*>(th_ri);
     cd* uh = reinterpret_cast<cd*>(uh_ri);
@@ -464,7 +574,7 @@ void or_solve(const or_params* P, const double* fh_ri, const double* th_ri, doub
         LU lu;
 #pragma omp for schedule(dynamic, 64)
         for (long q = 0; q < (long)K; ++q) {
-            const int iy = (int)(q / nkx), ix = (int)(q % nkx);
+            const int iy = ixs ? iys[q] : (int)(q / nkx), ix = ixs ? ixs[q] : (int)(q % nkx);
             const int nyq = (iy <= ny / 2) ? iy : iy - ny;          // FFT order
             const ld kx = 2 * PI_L * ix / (ld)P->Lx, ky = 2 * PI_L * nyq / (ld)P->Ly;
             const ld k = sqrtl(kx * kx + ky * ky);                  // magnitude always uses the full values (G5)
@@ -608,6 +718,19 @@ void or_solve(const or_params* P, const double* fh_ri, const double* th_ri, doub
             }
         }
     }
+}
+
+extern "C" {
+
+// every retained wavenumber: fh, th, uh, wh, dump are half spectra [3][nz][ny][nkx]
+void or_solve(const or_params* P, const double* fh_ri, const double* th_ri, double* uh_ri, double* wh_ri, double* dump_coef_ri) {
+    solve_columns(P, (long)P->ny * (P->nx / 2 + 1), nullptr, nullptr, fh_ri, th_ri, uh_ri, wh_ri, dump_coef_ri);
+}
+
+// a list of wavenumbers (ix[q], iy[q]), q < nmodes: arrays [3][nz][nmodes]
+void or_solve_modes(const or_params* P, long nmodes, const int* ix, const int* iy, const double* fh_ri, const double* th_ri,
+                    double* uh_ri, double* wh_ri) {
+    solve_columns(P, nmodes, ix, iy, fh_ri, th_ri, uh_ri, wh_ri, nullptr);
 }
 
 }  // extern "C"

@@ -13,8 +13,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBNAME = os.path.join(_HERE, "libdpstokes.so")
 
 # every symbol include/dp.h declares
-EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_check", "dp_set_profiling", "dp_stage_ms",
-           "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_complex_row_pitch", "dp_zero_planes", "dp_fft_backend", "dp_es_norm",
+EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_check", "dp_effective_radius", "dp_set_profiling", "dp_stage_ms",
+           "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_copy_plane_to_host", "dp_complex_row_pitch", "dp_zero_planes", "dp_fft_backend", "dp_es_norm", "dp_es_radius_over_h",
            "dp_supported_nz", "dp_device_bytes", "dp_strerror", "dp_last_error", "dp_destroy"]
 
 
@@ -25,10 +25,10 @@ class DPError(RuntimeError):
 class dp_params(ctypes.Structure):
     _fields_ = [("wall_mode", ctypes.c_int), ("Lx", ctypes.c_double), ("Ly", ctypes.c_double), ("H", ctypes.c_double),
                 ("nx", ctypes.c_int), ("ny", ctypes.c_int), ("nz", ctypes.c_int), ("w", ctypes.c_int),
-                ("beta_M", ctypes.c_double), ("beta_D", ctypes.c_double), ("eta", ctypes.c_double),
-                ("max_particles", ctypes.c_int), ("use_torques", ctypes.c_int), ("device", ctypes.c_int),
-                ("fft_backend", ctypes.c_int), ("transfer_fp32", ctypes.c_int),
-                ("dense_planes", ctypes.c_int)]
+                ("beta_M", ctypes.c_double), ("beta_D", ctypes.c_double), ("a", ctypes.c_double), ("eta", ctypes.c_double),
+                ("max_particles", ctypes.c_int), ("transfer_fp32", ctypes.c_int), ("device", ctypes.c_int),
+                # extensions beyond SURVEY.md §8(b)
+                ("use_torques", ctypes.c_int), ("fft_backend", ctypes.c_int), ("dense_planes", ctypes.c_int)]
 
 
 _lib = None
@@ -66,6 +66,10 @@ def load_library():
     L.dp_buffer_bytes.restype = sz
     L.dp_copy_buffer_to_host.argtypes = [vp, i, vp, sz]
     L.dp_copy_buffer_to_host.restype = i
+    L.dp_copy_plane_to_host.argtypes = [vp, i, i, i, vp, sz]
+    L.dp_copy_plane_to_host.restype = i
+    L.dp_effective_radius.argtypes = [vp, i]
+    L.dp_effective_radius.restype = d
     L.dp_complex_row_pitch.argtypes = [vp]
     L.dp_complex_row_pitch.restype = i
     L.dp_zero_planes.argtypes = [vp]
@@ -74,6 +78,8 @@ def load_library():
     L.dp_fft_backend.restype = i
     L.dp_es_norm.argtypes = [d, d]
     L.dp_es_norm.restype = d
+    L.dp_es_radius_over_h.argtypes = [i, d, i]
+    L.dp_es_radius_over_h.restype = d
     L.dp_supported_nz.argtypes = [ctypes.POINTER(i), i]
     L.dp_supported_nz.restype = i
     L.dp_device_bytes.argtypes = [vp]
@@ -116,9 +122,9 @@ class Plan:
         if use_torques is None:
             use_torques = bool(getattr(prob, "has_torque", True))
         self.params = dp_params(int(prob.wall_mode), float(prob.Lx), float(prob.Ly), float(prob.H), int(prob.nx), int(prob.ny),
-                                int(prob.nz), int(prob.w), float(prob.beta_M), float(prob.beta_D), float(prob.eta),
-                                int(max_particles), int(bool(use_torques)), int(device), int(fft_backend), int(bool(transfer_fp32)),
-                                int(bool(dense_planes)))
+                                int(prob.nz), int(prob.w), float(prob.beta_M), float(prob.beta_D), float(getattr(prob, "a", 1.0)),
+                                float(prob.eta), int(max_particles), int(bool(transfer_fp32)), int(device),
+                                int(bool(use_torques)), int(fft_backend), int(bool(dense_planes)))
         h = ctypes.c_void_p()
         rc = L.dp_create(ctypes.byref(self.params), ctypes.byref(h))
         if rc != 0:
@@ -206,6 +212,32 @@ class Plan:
 
     def device_bytes(self) -> int:
         return int(load_library().dp_device_bytes(self._h))
+
+    def effective_radius(self, dipole: bool = False) -> float:
+        """R_h of the plan's ES kernel (dp_effective_radius): host-side quadrature, no device work."""
+        r = float(load_library().dp_effective_radius(self._h, int(bool(dipole))))
+        if r < 0:
+            raise DPError("dp_effective_radius: invalid request")
+        return r
+
+    def copy_plane(self, which: int, field: int, l: int) -> np.ndarray:
+        """One xy plane of an internal buffer (test hook): which = 0 real [ny, nx], 1 half spectrum [ny, nx/2+1] (natural layout)."""
+        L = load_library()
+        p = self.params
+        if which == 0:
+            out = np.empty((p.ny, p.nx), dtype=np.float64)
+        else:
+            out = np.empty((p.ny, int(L.dp_complex_row_pitch(self._h))), dtype=np.complex128)
+        self._ck(L.dp_copy_plane_to_host(self._h, which, field, l, out.ctypes.data_as(ctypes.c_void_p), out.nbytes), "dp_copy_plane_to_host")
+        return out if which == 0 else out[:, : p.nx // 2 + 1]
+
+    def run_stage(self, pos, force, torque, last_stage: int):
+        """dp_debug_run_stage without copying anything back (use copy_plane / debug buffers afterwards)."""
+        import torch
+        ptr = lambda t: None if t is None else ctypes.c_void_p(t.data_ptr())
+        st = torch.cuda.current_stream(pos.device)
+        self._ck(load_library().dp_debug_run_stage(self._h, int(pos.shape[0]), ptr(pos), ptr(force), ptr(torque), int(last_stage),
+                                                    ctypes.c_void_p(st.cuda_stream)), "dp_debug_run_stage")
 
     # -- test hooks
     def debug_stage(self, pos, force, torque, last_stage: int):

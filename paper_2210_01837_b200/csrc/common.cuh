@@ -60,6 +60,9 @@ struct dp_plan {
   bool own_fft = false;
   void* fft_own = nullptr;
 
+  void* host_stage = nullptr;   // device staging buffers of dp_mobility_apply_host (plan.cu), allocated on first use
+  double* d_ct_full = nullptr;  // cos(n l pi/(nz-1)) [nz][nz] for the k = 0 kernel (solve.cu), per plan
+
   cudaStream_t last_stream = nullptr;
   bool profiling = false;
   cudaEvent_t ev[9] = {};
@@ -73,7 +76,8 @@ cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* fo
 cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torque, cudaStream_t st);
 cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaStream_t st);
 cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega, cudaStream_t st);
-cudaError_t dp_solve_upload_tables(dp_plan* P);
+cudaError_t dp_solve_upload_tables(dp_plan* P);      // per plan: constant tables, k = 0 cosine table, kernel attributes on the plan's device
+void dp_solve_destroy_tables(dp_plan* P);
 bool dp_solve_supports_nz(int nz);
 // fft.cu: the xy FFTs as two shared-memory passes per direction
 bool dp_fft_own_supported(int nx, int ny);
@@ -84,6 +88,7 @@ const int* dp_fft_own_ky_table(const dp_plan* P);
 cudaError_t dp_fft_own_forward(dp_plan* P, int nfields, cudaStream_t st);
 cudaError_t dp_fft_own_inverse(dp_plan* P, int nfields, cudaStream_t st);
 cudaError_t dp_fft_own_untranspose(dp_plan* P, double2* dst, cudaStream_t st);
+cudaError_t dp_fft_own_untranspose_plane(dp_plan* P, size_t plane_index, double2* dst, cudaStream_t st);
 
 // ---- exponential-of-semicircle kernel, eq 54: phi(s) = exp(beta (sqrt(1-(s/alpha)^2) - 1)) / Z on |s| <= alpha
 __device__ __forceinline__ double dp_es_phi(double s, double inv_alpha, double beta, double inv_Z) {

@@ -131,6 +131,7 @@ struct MidPrefetch {          // inverse y pass, last round: all inputs are in r
   unsigned bytes;
   __device__ __forceinline__ void operator()(int rd, int nrounds) const {
     if (rd == nrounds - 1) {
+      fence_async_proxy();      // generic-proxy accesses of buf (this batch's stages) before the async-proxy refill
       slot_barrier(slot);
       if (st == 0 && next) { mbar_expect_tx(mbar, bytes); bulk_load(buf, next, bytes, mbar); }
     }
@@ -409,6 +410,7 @@ size_t smem_bytes_x(int M, int ntw, int rb) {
   return sizeof(double2) * ((size_t)ntw + (M / 2 + 1) + (size_t)NSLOT * rb * M) + align16(sizeof(unsigned short) * M) + 8 * NSLOT;
 }
 
+#ifdef DP_FFT_TUNING
 // tuning override: DP_FFT_FACTORS_X / DP_FFT_FACTORS_Y = comma-separated radices (product must equal the length)
 bool factors_from_env(const char* name, int n, Factors* F) {
   const char* e = getenv(name);
@@ -426,6 +428,7 @@ bool factors_from_env(const char* name, int n, Factors* F) {
   *F = G;
   return true;
 }
+#endif
 
 }  // namespace
 
@@ -454,8 +457,10 @@ cudaError_t dp_fft_own_create(dp_plan* P) {
   dp_fft_own* O = new dp_fft_own();
   P->fft_own = O;
   if (!factorize(M, &O->Fx) || !factorize(ny, &O->Fy)) return cudaErrorInvalidValue;
+#ifdef DP_FFT_TUNING              // tuning builds only: override the factorisation from the environment
   factors_from_env("DP_FFT_FACTORS_X", M, &O->Fx);
   factors_from_env("DP_FFT_FACTORS_Y", ny, &O->Fy);
+#endif
   // rows per slot batch: as many as fit the slot; in the x passes the batch must tile a plane's ny rows
   O->rby = SLOT_ELEMS / ny < 1 ? 1 : SLOT_ELEMS / ny;
   int rbmax = SLOT_ELEMS / M;                // <= 2 rows at nx = 4320: a batch is rb * nx doubles = rb * M complex
@@ -537,6 +542,13 @@ cudaError_t dp_fft_own_inverse(dp_plan* P, int nfields, cudaStream_t st) {
   if (e != cudaSuccess) return e;
   const FftXArgs X = x_args(P, nfields);
   O->kx_inv<<<grid_for(O, X.planes * (X.ny / X.rb)), FFT_THREADS, O->smem_x, st>>>(X);
+  return cudaGetLastError();
+}
+
+cudaError_t dp_fft_own_untranspose_plane(dp_plan* P, size_t plane_index, double2* dst, cudaStream_t st) {
+  dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
+  const size_t plane = (size_t)(P->p.nx / 2 + 1) * P->p.ny;
+  k_fft_untranspose<<<1024, 256, 0, st>>>(P->d_cplx + plane_index * plane, dst, O->d_ky_of_pos, P->p.ny, P->p.nx / 2 + 1, P->nkxp, 1);
   return cudaGetLastError();
 }
 

@@ -1,4 +1,4 @@
-// plan.cu — C ABI of the DP Stokes library: plan creation (tables, buffers, cuFFT plans), the apply pipeline
+// plan.cu — C ABI of the DP Stokes library: plan creation (tables, buffers, FFT tables or cuFFT plans), the apply pipeline
 // (paper steps 1-8), host-buffer entry point, profiling and test hooks.  See include/dp.h.
 #include <cmath>
 #include <cstdio>
@@ -43,6 +43,101 @@ double es_norm_host(double alpha, double beta) {
   return (double)((ld)alpha * sum);
 }
 
+// Gauss-Legendre nodes / weights on [-1, 1] by Newton on the three-term recurrence
+void gl_rule(int n, std::vector<ld>& x, std::vector<ld>& w) {
+  x.resize(n); w.resize(n);
+  for (int i = 0; i < n; ++i) {
+    ld t = cosl(PI_LD * (i + 0.75L) / (n + 0.5L)), dp = 1;
+    for (int it = 0; it < 80; ++it) {
+      ld p0 = 1, p1 = t;
+      for (int k = 2; k <= n; ++k) { ld p2 = ((2 * k - 1) * t * p1 - (k - 1) * p0) / k; p0 = p1; p1 = p2; }
+      dp = n * (t * p1 - p0) / (t * t - 1);
+      const ld dt = p1 / dp; t -= dt;
+      if (fabsl(dt) < 1e-19L) break;
+    }
+    ld p0 = 1, p1 = t;
+    for (int k = 2; k <= n; ++k) { ld p2 = ((2 * k - 1) * t * p1 - (k - 1) * p0) / k; p0 = p1; p1 = p2; }
+    dp = n * (t * p1 - p0) / (t * t - 1);
+    x[i] = t; w[i] = 2 / ((1 - t * t) * dp * dp);
+  }
+}
+
+// Effective hydrodynamic radius of a blob whose envelope is the tensor product phi(x) phi(y) phi(z) of the ES kernel
+// (eq 53-54) in an UNBOUNDED fluid, in units of the grid spacing h (alpha = w/2).  c(beta) = R_h/h is
+// intrinsic to the kernel (eq 56 and PAPER.md:362-364); the paper tabulates it in Tables I-II.
+//   monopole (translation-translation self mobility 1/(6 pi eta R_h), eq 1 in Fourier space, isotropic by cubic symmetry):
+//       1/(6 pi R_h) = (2/3) int_0^inf g(t)^3 dt,   g(t) = (1/pi) int_0^inf |phi^(q)|^2 exp(-q^2 t) dq,
+//       phi^(q) = int phi(s) cos(q s) ds;
+//   dipole (rotation-rotation self mobility 1/(8 pi eta R_h^3)):  R_h = (3/(4 pi))^{1/3} / int phi(s)^2 ds.
+// Both reduce to the Gaussian relations of eq 8.
+double es_radius_over_h(int w, double beta, bool dipole) {
+  const ld alpha = 0.5L * w;
+  const double Z = es_norm_host((double)alpha, beta);
+  // nodes s = alpha sin(theta): integrands analytic in theta
+  std::vector<ld> gx, gw;
+  gl_rule(24, gx, gw);
+  const int PANELS = 8;
+  std::vector<ld> s_nodes, s_wphi;          // s_k and w_k phi(s_k) ds
+  for (int p = 0; p < PANELS; ++p)
+    for (size_t i = 0; i < gx.size(); ++i) {
+      const ld width = PI_LD / PANELS, th = -PI_LD / 2 + width * (p + 0.5L * (gx[i] + 1));
+      const ld phi = expl((ld)beta * (cosl(th) - 1)) / (ld)Z;
+      s_nodes.push_back(alpha * sinl(th));
+      s_wphi.push_back(0.5L * width * gw[i] * phi * alpha * cosl(th));
+    }
+  if (dipole) {
+    ld i2 = 0;
+    for (size_t k = 0; k < s_nodes.size(); ++k) {
+      const ld c = sqrtl(1 - (s_nodes[k] / alpha) * (s_nodes[k] / alpha));
+      i2 += s_wphi[k] * expl((ld)beta * (c - 1)) / (ld)Z;          // phi^2 ds = (phi ds) phi
+    }
+    return (double)(cbrtl(3 / (4 * PI_LD)) / i2);
+  }
+  // int_0^inf g^3 dt = int_0^1 g(t)^3 dt + int_1^inf g(t)^3 dt.  In the second part t = 1/y^2 and q = r y give
+  //   g(t) = (y/pi) G(y),  G(y) = int_0^inf |phi^(r y)|^2 exp(-r^2) dr,   int_1^inf g^3 dt = (2/pi^3) int_0^1 G(y)^3 dy,
+  // so both parts are integrals of smooth functions over [0, 1] (the t^{-3/2} tail is integrated exactly by the map).
+  auto phihat2 = [&](ld qq) {
+    ld ph = 0;
+    for (size_t k = 0; k < s_nodes.size(); ++k) ph += s_wphi[k] * cosl(qq * s_nodes[k]);
+    return ph * ph;
+  };
+  // part 1: |phi^(q)|^2 on a composite rule in q over [0, QMAX]; beyond QMAX |phi^|^2 <= (2 phi(alpha)/q)^2 ~ e^{-2 beta}
+  const ld QMAX = 48.0L;
+  const int QPAN = 96;
+  std::vector<ld> q, p2w;                   // q_j and weight_j |phi^(q_j)|^2
+  for (int p = 0; p < QPAN; ++p)
+    for (size_t i = 0; i < gx.size(); ++i) {
+      const ld width = QMAX / QPAN, qq = width * (p + 0.5L * (gx[i] + 1));
+      q.push_back(qq); p2w.push_back(0.5L * width * gw[i] * phihat2(qq));
+    }
+  ld part1 = 0, part2 = 0;
+  const int TPAN = 4;
+  for (int p = 0; p < TPAN; ++p)
+    for (size_t i = 0; i < gx.size(); ++i) {
+      const ld width = 1.0L / TPAN, t = width * (p + 0.5L * (gx[i] + 1));
+      ld g = 0;
+      for (size_t j = 0; j < q.size(); ++j) g += p2w[j] * expl(-q[j] * q[j] * t);
+      g /= PI_LD;
+      part1 += 0.5L * width * gw[i] * g * g * g;
+    }
+  // part 2: G(y) with r in [0, RMAX] (exp(-RMAX^2) ~ 1e-22)
+  const ld RMAX = 7.0L;
+  const int RPAN = 7;
+  for (int p = 0; p < TPAN; ++p)
+    for (size_t i = 0; i < gx.size(); ++i) {
+      const ld width = 1.0L / TPAN, y = width * (p + 0.5L * (gx[i] + 1));
+      ld G = 0;
+      for (int pr = 0; pr < RPAN; ++pr)
+        for (size_t k = 0; k < gx.size(); ++k) {
+          const ld wr = RMAX / RPAN, r = wr * (pr + 0.5L * (gx[k] + 1));
+          G += 0.5L * wr * gw[k] * phihat2(r * y) * expl(-r * r);
+        }
+      part2 += 0.5L * width * gw[i] * G * G * G;
+    }
+  const ld integ = part1 + 2 * part2 / (PI_LD * PI_LD * PI_LD);
+  return (double)(1 / (6 * PI_LD * (2.0L / 3.0L) * integ));
+}
+
 void set_err(dp_plan* P, const char* what, const char* detail) {
   if (P) P->last_error = std::string(what) + ": " + (detail ? detail : "");
 }
@@ -57,6 +152,17 @@ void set_err(dp_plan* P, const char* what, const char* detail) {
     cufftResult r__ = (call);                                              \
     if (r__ != CUFFT_SUCCESS) { char b__[64]; snprintf(b__, sizeof b__, "cufft error %d", (int)r__); set_err(P, #call, b__); return DP_ECUFFT; } \
   } while (0)
+
+// makes the plan's device current for the lifetime of the guard and restores the caller's device afterwards
+struct DeviceGuard {
+  int prev = -1;
+  bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { prev = -1; cudaGetLastError(); }
+    if (prev != dev) ok = cudaSetDevice(dev) == cudaSuccess;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 template <class T> int dev_alloc(dp_plan* P, T** ptr, size_t count) {
   cudaError_t e = cudaMalloc((void**)ptr, sizeof(T) * (count ? count : 1));
@@ -143,13 +249,27 @@ int check_apply_args(dp_plan* P, int n, const double* pos, const double* force, 
 
 }  // namespace
 
-// host staging buffers for dp_mobility_apply_host live outside the public struct
-struct dp_host_stage { double *pos = nullptr, *frc = nullptr, *trq = nullptr, *U = nullptr, *Om = nullptr; cudaStream_t st = nullptr; };
-static dp_host_stage* stage_of(dp_plan* P);
+// device staging buffers of dp_mobility_apply_host: owned by the plan (dp_plan::host_stage), allocated on first use, all or nothing
+struct dp_host_stage {
+  double *pos = nullptr, *frc = nullptr, *trq = nullptr, *U = nullptr, *Om = nullptr;
+  cudaStream_t st = nullptr;
+  size_t bytes = 0;
+  void release() {
+    void* hb[] = {pos, frc, trq, U, Om};
+    for (void* b : hb) if (b) cudaFree(b);
+    if (st) cudaStreamDestroy(st);
+    pos = frc = trq = U = Om = nullptr; st = nullptr; bytes = 0;
+  }
+};
 
 extern "C" {
 
 double dp_es_norm(double alpha, double beta) { return es_norm_host(alpha, beta); }
+
+double dp_es_radius_over_h(int w, double beta, int dipole) {
+  if (w < 1 || !(beta > 0) || (dipole != 0 && dipole != 1)) return -1.0;
+  return es_radius_over_h(w, beta, dipole != 0);
+}
 
 int dp_supported_nz(int* out, int cap) {
   const int all[3] = {16, 32, 48};
@@ -175,21 +295,20 @@ int dp_complex_row_pitch(const dp_plan* P) { return P ? P->nkxp : 0; }
 
 int dp_destroy(dp_plan* P) {
   if (!P) return DP_OK;
-  cudaSetDevice(P->p.device);
-  if (P->last_stream || true) cudaDeviceSynchronize();
+  DeviceGuard guard(P->p.device);
+  cudaDeviceSynchronize();
   if (P->fft_ok) { cufftDestroy(P->fft_fwd); cufftDestroy(P->fft_inv); }
   dp_fft_own_destroy(P);
   void* bufs[] = {P->d_real, P->d_cplx, P->d_fft_work, P->d_znodes, P->d_zweights, P->d_pos_s, P->d_frc_s, P->d_trq_s, P->d_perm, P->d_meta, P->d_wrec,
                   P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_bin_start, P->d_flag, P->d_lmin};
   for (void* b : bufs) if (b) cudaFree(b);
   if (P->ev_ok) for (auto& e : P->ev) cudaEventDestroy(e);
-  dp_host_stage* hs = stage_of(P);
-  if (hs) {
-    void* hb[] = {hs->pos, hs->frc, hs->trq, hs->U, hs->Om};
-    for (void* b : hb) if (b) cudaFree(b);
-    if (hs->st) cudaStreamDestroy(hs->st);
+  if (P->host_stage) {
+    dp_host_stage* hs = static_cast<dp_host_stage*>(P->host_stage);
+    hs->release();
     delete hs;
   }
+  dp_solve_destroy_tables(P);
   delete P;
   return DP_OK;
 }
@@ -233,8 +352,9 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   P->cplx_field = P->own_fft ? dp_fft_own_cplx_field(P) : (size_t)p.nz * p.ny * P->nkxp;
 
   int rc = DP_OK;
-  cudaError_t ce = cudaSetDevice(p.device);
-  if (ce != cudaSuccess) { delete P; return DP_ECUDA; }
+  DeviceGuard guard(p.device);
+  if (!guard.ok) { cudaGetLastError(); delete P; return DP_ECUDA; }
+  cudaError_t ce = cudaSuccess;
 #define TRY(x) do { rc = (x); if (rc != DP_OK) { std::string msg = P->last_error; dp_destroy(P); (void)msg; return rc; } } while (0)
   TRY(dev_alloc(P, &P->d_real, p.transfer_fp32 ? (P->real_field * P->fields + 1) / 2 : P->real_field * P->fields));   // fp32 grids: half the bytes
   TRY(dev_alloc(P, &P->d_cplx, P->cplx_field * P->fields));
@@ -297,6 +417,8 @@ int dp_mobility_apply(dp_plan* P, int n, const double* pos, const double* force,
   int rc = check_apply_args(P, n, pos, force, torque, U, Omega);
   if (rc != DP_OK) return rc;
   if (n == 0) return DP_OK;
+  DeviceGuard guard(P->p.device);
+  if (!guard.ok) { set_err(P, "cudaSetDevice", "cannot select the plan's device"); cudaGetLastError(); return DP_ECUDA; }
   return run_pipeline(P, n, pos, force, torque, U, Omega, (cudaStream_t)cuda_stream, 5);
 }
 
@@ -305,11 +427,14 @@ int dp_debug_run_stage(dp_plan* P, int n, const double* pos, const double* force
   int rc = check_apply_args(P, n, pos, force, torque, &dummy, nullptr);
   if (rc != DP_OK) return rc;
   if (last_stage < 1 || last_stage > 4 || n == 0) return DP_EINVAL;
+  DeviceGuard guard(P->p.device);
+  if (!guard.ok) { cudaGetLastError(); return DP_ECUDA; }
   return run_pipeline(P, n, pos, force, torque, nullptr, nullptr, (cudaStream_t)cuda_stream, last_stage);
 }
 
 int dp_check(dp_plan* P) {
   if (!P) return DP_EINVAL;
+  DeviceGuard guard(P->p.device);
   CK(cudaStreamSynchronize(P->last_stream));
   int flag = 0;
   CK(cudaMemcpy(&flag, P->d_flag, sizeof(int), cudaMemcpyDeviceToHost));
@@ -326,6 +451,7 @@ int dp_stage_ms(dp_plan* P, float* ms) {
   if (!P || !ms) return DP_EINVAL;
   for (int i = 0; i < 8; ++i) ms[i] = 0.f;
   if (!P->ev_recorded) { set_err(P, "dp_stage_ms", "no profiled apply recorded"); return DP_EINVAL; }
+  DeviceGuard guard(P->p.device);
   CK(cudaEventSynchronize(P->ev[6]));
   for (int i = 0; i < 6; ++i) CK(cudaEventElapsedTime(&ms[i], P->ev[i], P->ev[i + 1]));
   ms[6] = 0.f;   // the k = 0 kernel is launched inside the solve stage
@@ -344,6 +470,7 @@ int dp_fft_backend(const dp_plan* P) { return P ? (P->own_fft ? 0 : 1) : -1; }
 
 int dp_zero_planes(dp_plan* P) {
   if (!P) return DP_EINVAL;
+  DeviceGuard guard(P->p.device);
   CK(cudaStreamSynchronize(P->last_stream));
   int lm = 0;
   CK(cudaMemcpy(&lm, P->d_lmin, sizeof(int), cudaMemcpyDeviceToHost));
@@ -353,6 +480,7 @@ int dp_zero_planes(dp_plan* P) {
 int dp_copy_buffer_to_host(dp_plan* P, int which, void* host, size_t bytes) {
   if (!P || !host) return DP_EINVAL;
   if (bytes > dp_buffer_bytes(P, which) || dp_buffer_bytes(P, which) == 0) return DP_EINVAL;
+  DeviceGuard guard(P->p.device);
   CK(cudaStreamSynchronize(P->last_stream));
   if (which == 1 && P->own_fft) {
     // the own FFT passes keep the half spectrum transposed with ky digit-reversed: hand out the natural layout
@@ -382,32 +510,80 @@ int dp_copy_buffer_to_host(dp_plan* P, int which, void* host, size_t bytes) {
 
 }  // extern "C"
 
-// ---- host-buffer entry point -----------------------------------------------------------------------------------------
-#include <map>
-static std::map<dp_plan*, dp_host_stage*> g_stage;
-static dp_host_stage* stage_of(dp_plan* P) {
-  auto it = g_stage.find(P);
-  if (it == g_stage.end()) return nullptr;
-  dp_host_stage* s = it->second;
-  g_stage.erase(it);
-  return s;
+// ---- one plane of an internal buffer (test hook of the full-size parity tests)
+extern "C" int dp_copy_plane_to_host(dp_plan* P, int which, int field, int l, void* host, size_t bytes) {
+  if (!P || !host || field < 0 || field >= P->fields || l < 0 || l >= P->p.nz) return DP_EINVAL;
+  DeviceGuard guard(P->p.device);
+  CK(cudaStreamSynchronize(P->last_stream));
+  const size_t plane_index = (size_t)field * P->p.nz + l;
+  if (which == 0) {
+    const size_t cnt = (size_t)P->p.ny * P->p.nx;
+    if (bytes != cnt * sizeof(double)) return DP_EINVAL;
+    if (P->p.transfer_fp32) {
+      std::vector<float> tmp(cnt);
+      CK(cudaMemcpy(tmp.data(), reinterpret_cast<const float*>(P->d_real) + plane_index * cnt, cnt * sizeof(float), cudaMemcpyDeviceToHost));
+      double* out = static_cast<double*>(host);
+      for (size_t i = 0; i < cnt; ++i) out[i] = (double)tmp[i];
+      return DP_OK;
+    }
+    CK(cudaMemcpy(host, P->d_real + plane_index * cnt, bytes, cudaMemcpyDeviceToHost));
+    return DP_OK;
+  }
+  if (which == 1) {
+    const size_t cnt = (size_t)P->p.ny * P->nkxp;
+    if (bytes != cnt * sizeof(double2)) return DP_EINVAL;
+    if (!P->own_fft) {
+      CK(cudaMemcpy(host, P->d_cplx + plane_index * cnt, bytes, cudaMemcpyDeviceToHost));
+      return DP_OK;
+    }
+    double2* tmp = nullptr;
+    CK(cudaMalloc(&tmp, bytes));
+    cudaError_t e = cudaMemsetAsync(tmp, 0, bytes, P->last_stream);
+    if (e == cudaSuccess) e = dp_fft_own_untranspose_plane(P, plane_index, tmp, P->last_stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(P->last_stream);
+    if (e == cudaSuccess) e = cudaMemcpy(host, tmp, bytes, cudaMemcpyDeviceToHost);
+    cudaFree(tmp);
+    CK(e);
+    return DP_OK;
+  }
+  return DP_EINVAL;
 }
 
+extern "C" double dp_effective_radius(const dp_plan* P, int dipole) {
+  if (!P || (dipole != 0 && dipole != 1)) return -1.0;
+  if (dipole && P->fields != 6) return -1.0;
+  return P->h * es_radius_over_h(P->p.w, dipole ? P->p.beta_D : P->p.beta_M, dipole != 0);
+}
+
+// ---- host-buffer entry point -----------------------------------------------------------------------------------------
 extern "C" int dp_mobility_apply_host(dp_plan* P, int n, const double* pos, const double* force, const double* torque, double* U,
                                       double* Omega) {
   int rc = check_apply_args(P, n, pos, force, torque, U, Omega);
   if (rc != DP_OK) return rc;
   if (n == 0) return DP_OK;
-  CK(cudaSetDevice(P->p.device));
-  dp_host_stage*& hs = g_stage[P];
-  if (!hs) {
-    hs = new dp_host_stage();
+  DeviceGuard guard(P->p.device);
+  if (!guard.ok) { set_err(P, "cudaSetDevice", "cannot select the plan's device"); cudaGetLastError(); return DP_ECUDA; }
+  if (!P->host_stage) {
+    dp_host_stage* fresh = new (std::nothrow) dp_host_stage();
+    if (!fresh) return DP_ENOMEM;
     const size_t bytes = sizeof(double) * 3 * (size_t)P->p.max_particles;
-    CK(cudaMalloc(&hs->pos, bytes)); CK(cudaMalloc(&hs->frc, bytes)); CK(cudaMalloc(&hs->U, bytes));
-    P->device_bytes += 3 * bytes;
-    if (P->fields == 6) { CK(cudaMalloc(&hs->trq, bytes)); CK(cudaMalloc(&hs->Om, bytes)); P->device_bytes += 2 * bytes; }
-    CK(cudaStreamCreateWithFlags(&hs->st, cudaStreamNonBlocking));
+    const int nbuf = P->fields == 6 ? 5 : 3;
+    double** slots[5] = {&fresh->pos, &fresh->frc, &fresh->U, &fresh->trq, &fresh->Om};
+    cudaError_t e = cudaSuccess;
+    for (int i = 0; i < nbuf && e == cudaSuccess; ++i) e = cudaMalloc((void**)slots[i], bytes);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&fresh->st, cudaStreamNonBlocking);
+    if (e != cudaSuccess) {                       // all or nothing: nothing half-initialised survives a failed attempt
+      set_err(P, "dp_mobility_apply_host staging", cudaGetErrorString(e));
+      cudaGetLastError();
+      fresh->release();
+      delete fresh;
+      return e == cudaErrorMemoryAllocation ? DP_ENOMEM : DP_ECUDA;
+    }
+    fresh->bytes = (size_t)nbuf * bytes;
+    P->device_bytes += fresh->bytes;
+    P->host_stage = fresh;
   }
+  dp_host_stage* hs = static_cast<dp_host_stage*>(P->host_stage);
   const size_t nb = sizeof(double) * 3 * (size_t)n;
   CK(cudaMemcpyAsync(hs->pos, pos, nb, cudaMemcpyHostToDevice, hs->st));
   if (force) CK(cudaMemcpyAsync(hs->frc, force, nb, cudaMemcpyHostToDevice, hs->st));

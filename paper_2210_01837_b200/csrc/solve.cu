@@ -712,20 +712,17 @@ template <int NZ> void host_tables(std::vector<double>& out) {
   }
 }
 
+template <int NZ> cudaError_t set_attr_nz() {      // per device: called by every plan at creation, on its own device
+  return cudaFuncSetAttribute(k_solve<NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)solve_smem_bytes<NZ>());
+}
+
 template <int NZ> cudaError_t launch_nz(const SolveArgs& A, cudaStream_t st) {
-  static bool attr = false;
   const size_t smem = solve_smem_bytes<NZ>();
-  if (!attr) {
-    cudaError_t e = cudaFuncSetAttribute(k_solve<NZ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attr = true;
-  }
   dim3 grid((A.n_fast + TM - 1) / TM, A.n_slow);
   k_solve<NZ><<<grid, SOLVE_THREADS, smem, st>>>(A);
   return cudaGetLastError();
 }
 
-double* g_ct_full[3] = {nullptr, nullptr, nullptr};   // device cos tables for the k = 0 kernel (per compiled nz)
 int nz_slot(int nz) { return nz == 16 ? 0 : nz == 32 ? 1 : nz == 48 ? 2 : -1; }
 
 }  // namespace
@@ -741,17 +738,23 @@ cudaError_t dp_solve_upload_tables(dp_plan* P) {
   else if (nz == 48) { host_tables<48>(t); e = cudaMemcpyToSymbol(c_tab48, t.data(), sizeof(double) * t.size()); }
   else return cudaErrorInvalidValue;
   if (e != cudaSuccess) return e;
-  const int slot = nz_slot(nz);
-  if (!g_ct_full[slot]) {
+  if (nz == 16) e = set_attr_nz<16>(); else if (nz == 32) e = set_attr_nz<32>(); else e = set_attr_nz<48>();
+  if (e != cudaSuccess) return e;
+  if (!P->d_ct_full) {
     typedef long double ld;
     const ld PI = 3.141592653589793238462643383279502884L;
     std::vector<double> ct((size_t)nz * nz);
     for (int n = 0; n < nz; ++n) for (int l = 0; l < nz; ++l) ct[(size_t)n * nz + l] = (double)cosl(PI * n * l / (nz - 1));
-    e = cudaMalloc(&g_ct_full[slot], sizeof(double) * ct.size());
+    e = cudaMalloc(&P->d_ct_full, sizeof(double) * ct.size());
     if (e != cudaSuccess) return e;
-    e = cudaMemcpy(g_ct_full[slot], ct.data(), sizeof(double) * ct.size(), cudaMemcpyHostToDevice);
+    P->device_bytes += sizeof(double) * ct.size();
+    e = cudaMemcpy(P->d_ct_full, ct.data(), sizeof(double) * ct.size(), cudaMemcpyHostToDevice);
   }
   return e;
+}
+
+void dp_solve_destroy_tables(dp_plan* P) {
+  if (P->d_ct_full) { cudaFree(P->d_ct_full); P->d_ct_full = nullptr; }
 }
 
 cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega, cudaStream_t st) {
@@ -770,6 +773,6 @@ cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega,
     default: return cudaErrorInvalidValue;
   }
   if (e != cudaSuccess) return e;
-  k_zero_mode<<<1, 64, 0, st>>>(A, P->p.nz, g_ct_full[nz_slot(P->p.nz)]);
+  k_zero_mode<<<1, 64, 0, st>>>(A, P->p.nz, P->d_ct_full);
   return cudaGetLastError();
 }

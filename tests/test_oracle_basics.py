@@ -152,6 +152,7 @@ def test_dft_forward_is_rfft2_and_literal_double_sum(nx, ny):
             s = (f[0] * np.exp(-2j * np.pi * (kx * i / nx + ky * j / ny))).sum()
             assert abs(s - got[0, ky, kx]) < 1e-12
     assert np.allclose(oracle.dft_xy_forward(f, "fft"), got, atol=1e-12)
+    assert np.allclose(oracle.dft_xy_forward(f, "numpy"), got, atol=1e-12)
 
 
 @pytest.mark.parametrize("nx,ny", [(8, 6), (12, 12), (9, 10)])
@@ -161,9 +162,30 @@ def test_dft_inverse_roundtrip_and_irfft2(nx, ny):
     spec = np.fft.rfft2(f, axes=(-2, -1))
     assert np.allclose(oracle.dft_xy_inverse(spec, nx, "naive"), f, atol=1e-13)
     assert np.allclose(oracle.dft_xy_inverse(spec, nx, "fft"), f, atol=1e-13)
+    assert np.allclose(oracle.dft_xy_inverse(spec, nx, "numpy"), f, atol=1e-13)
     # full-spectrum definition with Hermitian completion
     full = np.fft.fft2(f, axes=(-2, -1))
     i = np.arange(nx)[None, :]
     j = np.arange(ny)[:, None]
     u00 = sum(full[0, ky, kx] * np.exp(2j * np.pi * (kx * 3 / nx + ky * 2 / ny)) for kx in range(nx) for ky in range(ny)) / (nx * ny)
     assert abs(u00.real - oracle.dft_xy_inverse(spec, nx, "naive")[0, 2, 3]) < 1e-13
+
+
+@pytest.mark.parametrize("nx,ny", [(48, 48), (192, 192), (1080, 1080), (50, 28), (34, 22)])
+def test_own_plain_fft_equals_the_naive_dft_sums(nx, ny):
+    """The oracle's own recursive mixed-radix FFT (dft="fft", used where the O(n^2) sums do not finish) against its explicit
+    DFT sums at the grid sizes of configs 1-3 (48, 192, 1080: SURVEY.md §8(d) "validated against its naive DFT to 1e-13 on
+    configs 1-3") and at sizes with prime factors 7, 11, 17 (the prime-length branch); numpy.fft only as a third opinion."""
+    rng = np.random.default_rng(nx + ny)
+    f = rng.standard_normal((1, ny, nx))
+    naive = oracle.dft_xy_forward(f, "naive")
+    own = oracle.dft_xy_forward(f, "fft")
+    scale = np.abs(naive).max()
+    assert np.abs(own - naive).max() < 1e-13 * scale * max(1.0, np.log2(nx * ny) / 8)
+    assert np.abs(oracle.dft_xy_forward(f, "numpy") - own).max() < 1e-13 * scale * max(1.0, np.log2(nx * ny) / 8)
+    spec = naive * (rng.standard_normal(naive.shape) + 0.5)          # a generic Hermitian-completable half spectrum
+    b_naive = oracle.dft_xy_inverse(spec, nx, "naive")
+    b_own = oracle.dft_xy_inverse(spec, nx, "fft")
+    assert np.abs(b_own - b_naive).max() < 1e-13 * np.abs(b_naive).max() * max(1.0, np.log2(nx * ny) / 8)
+    # the imaginary parts of the kx = 0 and kx = nx/2 columns are what Hermitian completion must treat consistently
+    assert np.abs(oracle.dft_xy_inverse(spec, nx, "numpy") - b_own).max() < 1e-12 * np.abs(b_naive).max()
