@@ -402,6 +402,15 @@ template <int NZ> struct SolveSmem {
   static constexpr int DOUBLES = CORR + 12 * LN;
 };
 
+#ifdef DP_SOLVE_TIMING
+// phase timeline of the CTAs that run on a few SMs (development builds only)
+__device__ long long g_tlog[4 * 256 * SOLVE_WARPS * 16];
+__device__ int g_tcount[4];
+#define TMARK(k) do { if (tslot >= 0 && lane == 0) g_tlog[((tsm * 256 + tslot) * SOLVE_WARPS + wid) * 16 + (k)] = clock64(); } while (0)
+#else
+#define TMARK(k) do { } while (0)
+#endif
+
 template <int NZ>
 __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(SolveArgs A) {
   extern __shared__ double smem[];
@@ -416,6 +425,21 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
 
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int mode = lane >> 1, part = lane & 1;
+#ifdef DP_SOLVE_TIMING
+  __shared__ int s_tslot;
+  int tsm = -1, tslot = -1;
+  {
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    if (smid < 4) {
+      tsm = (int)smid;
+      if (tid == 0) { const int c = atomicAdd(&g_tcount[smid], 1); s_tslot = c < 256 ? c : -1; }
+      __syncthreads();
+      tslot = s_tslot;
+    }
+  }
+  TMARK(0);
+#endif
   const int ifast = blockIdx.x * TM + mode, islow = blockIdx.y;
   const bool valid = ifast < A.n_fast;
   const int ix = A.fast_is_x ? ifast : islow;
@@ -465,6 +489,7 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
     }
   }
   cp_async_commit();
+  TMARK(1);
   if (wid == 0) {
     const double ib = factor_chain<NZ, 0>(F + mode, F + NZ * TM + mode, F + 2 * NZ * TM + mode, K.k, K.k2, inv_s, part == 0);
     if (part == 0) s_ibg[mode] = ib;
@@ -478,6 +503,7 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
       C[5 * VS + l * LN + lane] = part ? zl * E : E;
     }
   }
+  TMARK(2);
   cp_async_wait_all();
   __syncwarp();
   if (A.torque) {
@@ -494,6 +520,7 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
       }
     }
   }
+  TMARK(3);
   __syncthreads();
 
   // ---------------- phase 1: Chebyshev analysis, one warp per column: f_x, f_y, f_z, (E, zE) [, t_x, t_y]   (step 2; step 6)
@@ -501,11 +528,13 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
     const int col = wid < 3 ? wid : (wid == 3 ? 5 : wid - 1);          // warps 0-2: C0-C2, warp 3: C5, warps 4, 5: C3, C4
     if (wid < 4 || A.torque) analysis_column<NZ>(C + col * VS + lane);
   }
+  TMARK(4);
   __syncthreads();
 
   // ---------------- phase 2: f_x -= (1/2) D t_y, f_y += (1/2) D t_x (eq 7)
   if (A.torque) {
     if (wid < 2) deriv_column<NZ, true>(C + (wid == 0 ? 4 : 3) * VS + lane, C + wid * VS + lane, inv_s, wid == 0 ? -0.5 : 0.5);
+    TMARK(5);
     __syncthreads();
   }
 
@@ -527,6 +556,7 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
       else Sc = bvp_item<NZ, 0>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], pH, p0, pHo, p0o);
       s_sum[((ph == 0 ? 0 : 1 + comp) * 2 + par) * LN + lane] = Sc;
     }
+    TMARK(6 + ph);
     __syncthreads();
   }
 
@@ -562,14 +592,17 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
       C[c * VS + n * LN + lane] += add;
     }
   }
+  TMARK(8);
   __syncthreads();
 
   // ---------------- phase 7: dz u, dz v of the TOTAL in coefficient space (reading G12) -> C3, C4; synthesis back to the nodes
   if (A.omega) {
     if (wid < 2) deriv_column<NZ, false>(C + wid * VS + lane, C + (3 + wid) * VS + lane, inv_s, 1.0);
+    TMARK(9);
     __syncthreads();
   }
   if (wid < (A.omega ? 5 : 3)) synthesis_column<NZ>(C + wid * VS + lane);
+  TMARK(10);
   __syncthreads();
 
   // ---------------- phase 8: (1/2) curl u (eq 11), scale by 1/(nx ny) for the unnormalised inverse FFT, store
@@ -597,7 +630,21 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
       }
     }
   }
+  TMARK(11);
 }
+
+#ifdef DP_SOLVE_TIMING
+}  // namespace
+extern "C" int dp_debug_solve_timeline(long long* host_log, int* host_count) {   // development builds only
+  cudaDeviceSynchronize();
+  cudaMemcpyFromSymbol(host_log, g_tlog, sizeof(g_tlog));
+  cudaMemcpyFromSymbol(host_count, g_tcount, sizeof(g_tcount));
+  int z[4] = {0, 0, 0, 0};
+  cudaMemcpyToSymbol(g_tcount, z, sizeof(z));
+  return 0;
+}
+namespace {
+#endif
 
 // ---- k = 0 column (paper step 5; eqs 47, 51, 52; (A12) with no slip): one CTA of 64 threads
 //   w = 0;  u'' = -f_x/eta, v'' = -f_y/eta with u(0) = 0 and (bottom wall) u'(H) = 0 / (slit) u(H) = 0.

@@ -8,10 +8,11 @@ configuration bench.py times), through the C ABI, against the CPU oracle.
   stage: oracle spread of ALL particles vs the CUDA grids, plane by plane; sampled planes of the forward and inverse xy
   transforms vs the oracle's FFT; the per-wavenumber solve on sampled (kx, ky) columns (lowest modes, k = 0, both Nyquist
   lines, random interior) vs ``oracle.solve_modes``; oracle interpolation of the CUDA path's real-space u, omega for ALL particles
-  vs the CUDA U, Omega.  The whole oracle product at config 5 (about 60 GB of host memory, several minutes) runs when
-  DP_FULL_ORACLE_CFG5=1.
+  vs the CUDA U, Omega.  The whole oracle product at config 5 (about 60 GB of host memory, two minutes) runs too, unless
+  DP_FULL_ORACLE_CFG5=0.
 """
 import os
+import sys
 
 import numpy as np
 import pytest
@@ -106,7 +107,7 @@ def test_cfg5_full_size_stage_by_stage_against_the_oracle(dp):
         assert plan.fft_backend() == "own"
         # ---- step 1: oracle spread of all 1,048,576 particles vs the CUDA grids, plane by plane
         plan.run_stage(dpos, dF, dT, 1)
-        sample_planes = [(0, nz - 2), (2, nz - 5), (4, nz - 3), (5, nz - 9)]        # (field, l): near the wall, where the monolayer sits
+        sample_planes = [(0, nz - 2), (2, nz - 5), (4, nz - 3), (1, nz - 9)]        # (field, l): near the wall, where the monolayer sits (t_x = t_z = 0 here: torques are +y)
         kept = {}
         for grp, (val, beta) in enumerate(((F, prob.beta_M), (T, prob.beta_D))):
             ref = oracle.spread(prob, pos, val, beta)                               # [3, nz, ny, nx]
@@ -120,7 +121,9 @@ def test_cfg5_full_size_stage_by_stage_against_the_oracle(dp):
                     worst = max(worst, float(np.abs(d).max()))
                     if (3 * grp + c, l) in sample_planes:
                         kept[(3 * grp + c, l)] = g.copy()
-            assert np.sqrt(num / den) < 1e-13 and worst < 1e-12 * float(np.abs(ref).max()), (grp, np.sqrt(num / den), worst)
+            # the two sides differ in summation order and in the rounding of the ES exponent beta (sqrt(1 - q^2) - 1): one ulp in q
+            # (s * (1/alpha) here, s / alpha in the oracle; fused 1 - q q) is amplified by beta / (2 sqrt(1 - q^2)) <~ 100
+            assert np.sqrt(num / den) < 5e-13 and worst < 2e-12 * float(np.abs(ref).max()), (grp, np.sqrt(num / den), worst)
             del ref
         # ---- step 2 (xy): sampled planes of the forward spectrum vs the oracle's FFT of the (verified) grid planes;
         #      the nodal columns of the sampled modes are gathered from all planes for the solve check
@@ -180,8 +183,10 @@ def test_cfg5_full_size_stage_by_stage_against_the_oracle(dp):
         assert rel_max(U, U_o) < 1e-11 and rel_max(Om, Om_o) < 1e-11
 
 
-@pytest.mark.skipif(os.environ.get("DP_FULL_ORACLE_CFG5") != "1", reason="whole oracle product at config 5: ~60 GB host memory, minutes; set DP_FULL_ORACLE_CFG5=1")
+@pytest.mark.skipif(os.environ.get("DP_FULL_ORACLE_CFG5") == "0", reason="whole oracle product at config 5 switched off (DP_FULL_ORACLE_CFG5=0)")
 def test_cfg5_whole_product_against_the_whole_oracle(dp):
+    """Config 5 as bench.py runs it against the WHOLE oracle product (about 60 GB of host memory and two minutes on the 16-core
+    GPU box; DP_FULL_ORACLE_CFG5=0 skips it on a smaller host)."""
     import torch
     prob, pos, F, T = workloads.config(5)
     with dp.Plan(prob, max_particles=len(pos), use_torques=True) as plan:
