@@ -62,6 +62,7 @@ struct dp_plan {
 
   void* host_stage = nullptr;   // device staging buffers of dp_mobility_apply_host (plan.cu), allocated on first use
   double* d_ct_full = nullptr;  // cos(n l pi/(nz-1)) [nz][nz] for the k = 0 kernel (solve.cu), per plan
+  double* d_solve_frag = nullptr;  // DMMA fragment table of the Chebyshev transforms (solve.cu), per plan
 
   cudaStream_t last_stream = nullptr;
   bool profiling = false;
@@ -79,6 +80,7 @@ cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega,
 cudaError_t dp_solve_upload_tables(dp_plan* P);      // per plan: constant tables, k = 0 cosine table, kernel attributes on the plan's device
 void dp_solve_destroy_tables(dp_plan* P);
 bool dp_solve_supports_nz(int nz);
+int dp_solve_nz_list(int* out, int cap);
 // fft.cu: the xy FFTs as two shared-memory passes per direction
 bool dp_fft_own_supported(int nx, int ny);
 cudaError_t dp_fft_own_create(dp_plan* P);

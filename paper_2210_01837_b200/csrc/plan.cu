@@ -271,11 +271,7 @@ double dp_es_radius_over_h(int w, double beta, int dipole) {
   return es_radius_over_h(w, beta, dipole != 0);
 }
 
-int dp_supported_nz(int* out, int cap) {
-  const int all[3] = {16, 32, 48};
-  for (int i = 0; i < 3 && i < cap; ++i) out[i] = all[i];
-  return 3;
-}
+int dp_supported_nz(int* out, int cap) { return dp_solve_nz_list(out, cap); }
 
 const char* dp_strerror(int code) {
   switch (code) {

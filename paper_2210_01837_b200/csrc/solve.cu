@@ -12,15 +12,20 @@
 // chains (n even / n odd), each with one border unknown (c_0 resp. b_0) fixed by one combination of the two
 // boundary rows.  The chains are factored once per mode and reused for p, u, v, w.
 //
-// B200 mapping: one CTA = 16 consecutive modes of one row of the half spectrum, 6 warps.  A lane is (mode, part):
-// lane = 2*mode + part, part 0 = real, 1 = imaginary, so a warp row of a complex column is 256 contiguous bytes in HBM
-// and in shared memory ([column][n][lane], conflict free).  Every real operator of the method (cosine transforms,
-// z-derivative, tridiagonal sweeps) acts on a lane's own 32 numbers only, so a warp that owns a column needs no
-// synchronisation at all; the imaginary unit couples a lane to its neighbour (lane^1).  Work is split into phases of
-// independent column items, one warp per item, sized so that 5-6 of the 6 warps are busy in every long phase; the
-// sweeps run out of registers (all loads hoisted), divisions by constants are compile-time reciprocals, and the
-// transform matrices are warp-uniform constant-bank operands of fully unrolled DFMAs (nz is a template parameter).
-// Shared memory: 6 columns + 3 factor vectors = 61 KB at nz = 32 -> 3 CTAs (18 warps) per SM.
+// B200 mapping: one CTA = 16 consecutive modes of one row of the half spectrum, 6 warps, 4 CTAs per SM at nz = 32.
+// A complex column of the tile is a [nz][32] array of doubles in shared memory: row n = Chebyshev index (or node), the 32
+// entries of a row are (mode, re/im) = "lane" 2*mode + part, stored at position lane ^ swz(n) (an XOR swizzle of the
+// 4-lane groups of a row, see swz()).  Two kinds of work run on this layout:
+//  * the Chebyshev transforms are dense matrix products (cosine table x 32 columns): they run on the fp64 tensor pipe as
+//    mma.sync m8n8k4 (SASS DMMA), folded by the symmetry cos(n (N-l) pi/N) = (-1)^n cos(n l pi/N) into two half-size
+//    products per column; the table fragments come from a small per-plan global table (L1 resident), the data fragments
+//    straight from the swizzled tile (conflict free), 8 columns ("block") at a time so that a column's four blocks can go to
+//    different warps;
+//  * everything else (z-derivative recurrences, tridiagonal sweeps, boundary functionals, the correction) acts on a lane's
+//    own column only; the imaginary unit couples a lane to its neighbour (lane ^ 1), a shuffle or a neighbouring address.
+// Five columns live in shared memory: f_x -> u, f_y -> v, f_z -> f_z - dz p -> w, t_x -> p -> dz u, t_y -> (E, zE) -> dz v.
+// Their rows are stored split by parity (see crow()), which makes each folded transform a square product in place on half the
+// rows and lets a warp keep the table fragments in registers while it walks over the column blocks of a tile.
 #include <cmath>
 #include <vector>
 
@@ -34,21 +39,34 @@ constexpr int SOLVE_WARPS = 6;
 constexpr int SOLVE_THREADS = SOLVE_WARPS * 32;
 static_assert(LN == 32, "a warp row is one complex column row");
 
-// ---- constant tables per compiled nz (N = nz-1, LH = nz/2):
-//   CA[n][l] = cos(n l pi/N), l < LH                       analysis rows (contiguous in l)
-//   SE[l][j] = cos(2j l pi/N), SO[l][j] = cos((2j+1) l pi/N), l, j < LH     synthesis rows (contiguous in j)
-//   P[n], Q[n]: boundary-row functionals of a unit a_n (see chain()), XI[l] = cos(l pi/N)
-template <int NZ> struct Tab {
-  static constexpr int LH = NZ / 2;
-  static constexpr int CA = 0, SE = CA + NZ * LH, SO = SE + LH * LH, P = SO + LH * LH, Q = P + NZ, XI = Q + NZ, SIZE = XI + NZ;
-};
-__constant__ double c_tab16[Tab<16>::SIZE];
-__constant__ double c_tab32[Tab<32>::SIZE];
-__constant__ double c_tab48[Tab<48>::SIZE];
+// ---- shared-memory swizzle: element (row n, lane c) of a column tile lives at n * LN + (c ^ swz(n)).
+// swz(n) is 0, 4, 8 or 12 (it permutes the four 4-lane groups inside each half of a row and keeps (re, im) pairs adjacent),
+// chosen so that the DMMA fragment accesses are bank-conflict free: it is injective on every aligned group of four consecutive
+// rows and on {8m + 2k + p, k < 4}, and rows n, n+1 (n even) and n, n+2 (n = 0, 1 mod 4) differ in its upper bit.
+__host__ __device__ constexpr int swz(int n) { return ((((n ^ (n >> 1)) & 1) << 1) | (((n >> 1) ^ (n >> 2)) & 1)) << 2; }
+// Rows of a tile are "parity split": with NP = ceil(nz/2),
+//   nodal side:        e_l = g_l + g_{N-l} at row l (l < NP; the middle node of an odd nz alone), o_l = g_l - g_{N-l} at row NP + l;
+//   coefficient side:  g^_n at row n/2 for even n, at row NP + (n-1)/2 for odd n.
+// The folded cosine transforms map rows [0, NP) to rows [0, NP) and rows [NP, nz) to rows [NP, nz): each is in place on its
+// own rows and the two never touch the same data.
+template <int NZ> __host__ __device__ constexpr int crow(int n) { return (n & 1) ? (NZ + 1) / 2 + (n >> 1) : (n >> 1); }
+#define EL(tile, n, ln) (tile)[crow<NZ>(n) * LN + ((ln) ^ swz(crow<NZ>(n)))]
+
+// ---- constant tables per compiled nz: P[n], Q[n] = boundary-row functionals of a unit a_n (see chain()), XI[l] = cos(l pi/N)
+template <int NZ> struct Tab { static constexpr int P = 0, Q = NZ, XI = 2 * NZ, SIZE = 3 * NZ; };
+#define DP_SOLVE_NZ_LIST(X) X(16) X(19) X(24) X(26) X(32) X(40) X(48) X(64)
 template <int NZ> __device__ __forceinline__ const double* tab();
-template <> __device__ __forceinline__ const double* tab<16>() { return c_tab16; }
-template <> __device__ __forceinline__ const double* tab<32>() { return c_tab32; }
-template <> __device__ __forceinline__ const double* tab<48>() { return c_tab48; }
+#define X(NZ) __constant__ double c_tab##NZ[Tab<NZ>::SIZE]; \
+  template <> __device__ __forceinline__ const double* tab<NZ>() { return c_tab##NZ; }
+DP_SOLVE_NZ_LIST(X)
+#undef X
+
+// ---- geometry of the folded transforms: NP pairs (l, N-l) of nodes (the middle node pairs with itself when nz is odd),
+// even coefficients n = 2j and odd coefficients n = 2j+1, all padded to LP = a multiple of 8; KB k-blocks of 4, MB m-blocks of 8.
+// Fragment table (global, per plan): [4 kinds][MB][KB][32 lanes]; kind 0, 1: analysis even / odd, 2, 3: synthesis even / odd.
+template <int NZ> struct Tr {
+  static constexpr int N = NZ - 1, NP = (NZ + 1) / 2, LP = (NP + 7) / 8 * 8, KB = LP / 4, MB = LP / 8, FRAGS = 4 * MB * KB;
+};
 
 struct SolveArgs {
   double2* cplx;
@@ -58,79 +76,90 @@ struct SolveArgs {
   int fast_is_x;                 // 1: fast index = kx index (cuFFT layout); 0: fast index = position along ky (transposed layout)
   const int* lmin;               // planes l < *lmin of the input hold zeros that were never written: not read
   const int* ky_of_pos;          // transposed layout: FFT-order ky index stored at each position (digit reversal of the y pass), or null
+  const double* frag;            // transform fragment table (see Tr)
   double Lx, Ly, H, eta;
   int wall_mode, torque, omega;
 };
 
-__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gmem_src) {
+__device__ __forceinline__ void cp_async16(double* smem_dst, const double2* gmem_src) {
   const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ double ldg_stream(const double* p) {
+  double v;
+  asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void named_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+__device__ __forceinline__ void named_arrive(int id, int nthreads) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+
+// D(8x8) += A(8x4) B(4x8) on the fp64 tensor pipe: lane t holds A[t/4][t%4], B[t%4][t/4], D[t/4][2(t%4)], D[t/4][2(t%4)+1]
+__device__ __forceinline__ void dmma(double (&d)[2], double a, double b) {
+  asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d[0]), "+d"(d[1]) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ int swz_rt(int n) { return ((((n ^ (n >> 1)) & 1) << 1) | (((n >> 1) ^ (n >> 2)) & 1)) << 2; }
+
+// ---- one folded cosine transform of one parity, on the fp64 tensor pipe (one warp), in place on that parity's rows:
+//   analysis (kind 0 even, 1 odd):  g^_n = (2/N)(1/c~_n) sum_{l < NP} (1/c~_l) cos(n l pi/N) {e_l | o_l}   (n even | odd),
+//     which is the DCT-I  g^_n = (2/N)(1/c~_n) sum_l (1/c~_l) g_l cos(n l pi/N)  folded with cos(n (N-l) pi/N) = (-1)^n cos(n l pi/N);
+//   synthesis (kind 2 even, 3 odd): E_l = sum_j g^_{2j} cos(2j l pi/N) | O_l = sum_j g^_{2j+1} cos((2j+1) l pi/N), so that
+//     g_l = E_l + O_l, g_{N-l} = E_l - O_l.
+//   NBI 8-column blocks nb0 .. are transformed with the table fragments (all weights are in the table) held in registers.
+template <int NZ, int NBI>
+__device__ __forceinline__ void transform_item(double* __restrict__ tile, int kind, int nb0, const double* __restrict__ frag, int lane) {
+  typedef Tr<NZ> G;
+  constexpr int NP = G::NP, KB = G::KB, MB = G::MB;
+  const int g = lane >> 2, t = lane & 3;
+  const int par = kind & 1;
+  const int row0 = par ? NP : 0, cnt = par ? NZ - NP : NP;
+  const double* __restrict__ fk = frag + (size_t)(kind * MB) * KB * 32 + lane;
+  constexpr bool FRAG_REGS = MB * KB <= 8;  // larger tables are re-read from L1 per block
+  double fa[FRAG_REGS ? MB : 1][FRAG_REGS ? KB : 1];
+  if (FRAG_REGS) {
+#pragma unroll
+    for (int mb = 0; mb < MB; ++mb)
+#pragma unroll
+      for (int kb = 0; kb < KB; ++kb) fa[FRAG_REGS ? mb : 0][FRAG_REGS ? kb : 0] = __ldg(fk + (mb * KB + kb) * 32);
+  }
+  int xo[KB];                                // offsets of this lane's operand rows, swizzle included (column block 0)
+#pragma unroll
+  for (int kb = 0; kb < KB; ++kb) { const int r = row0 + kb * 4 + t; xo[kb] = r * LN + (g ^ swz_rt(r)); }
+#pragma unroll
+  for (int nbi = 0; nbi < NBI; ++nbi) {
+    const int nb = nb0 + nbi;
+    double x[KB];
+#pragma unroll
+    for (int kb = 0; kb < KB; ++kb) x[kb] = (kb * 4 + t < cnt) ? tile[xo[kb] ^ (nb * 8)] : 0.0;
+    double acc[MB][2];
+#pragma unroll
+    for (int mb = 0; mb < MB; ++mb) acc[mb][0] = acc[mb][1] = 0.0;
+#pragma unroll
+    for (int kb = 0; kb < KB; ++kb)
+#pragma unroll
+      for (int mb = 0; mb < MB; ++mb) dmma(acc[mb], FRAG_REGS ? fa[FRAG_REGS ? mb : 0][FRAG_REGS ? kb : 0] : __ldg(fk + (mb * KB + kb) * 32), x[kb]);
+    __syncwarp();                            // every lane has read its operands of this block before the block is overwritten
+#pragma unroll
+    for (int mb = 0; mb < MB; ++mb) {
+      const int m = mb * 8 + g, r = row0 + m;
+      if (m < cnt) *reinterpret_cast<double2*>(&tile[r * LN + ((nb * 8 + 2 * t) ^ swz_rt(r))]) = make_double2(acc[mb][0], acc[mb][1]);
+    }
+  }
+}
 
 // ---- tridiagonal rows of a chain (n >= 1): d_n a_n + l_n a_{n-2} + u_n a_{n+2}; all divisions are compile-time constants
 template <int NZ> __device__ __forceinline__ double row_d(int n, double k2) { return n == 1 ? fma(k2, 0.125, 1.0) : fma(k2, 1.0 / (2.0 * (n * n - 1)), 1.0); }
 template <int NZ> __device__ __forceinline__ double row_l(int n, double k2) { return k2 * (-(n == 2 ? 2.0 : 1.0) / (4.0 * n * (n - 1))); }
 template <int NZ> __device__ __forceinline__ double row_u(int n, double k2) { return (n + 2 <= NZ - 3) ? k2 * (-1.0 / (4.0 * n * (n + 1))) : 0.0; }
 
-// ---- DCT-I analysis of a lane's column, in place:
-//   g^_n = (2/N)(1/c~_n) sum_l (1/c~_l) g_l cos(n l pi/N), folded with cos(n (N-l) pi/N) = (-1)^n cos(n l pi/N)
-template <int NZ> __device__ __forceinline__ void analysis_column(double* __restrict__ v) {
-  constexpr int N = NZ - 1, LH = NZ / 2;
-  const double* __restrict__ T = tab<NZ>() + Tab<NZ>::CA;
-  double e[LH], o[LH];
-#pragma unroll
-  for (int l = 0; l < LH; ++l) {
-    const double a = v[l * LN], b = v[(N - l) * LN];
-    e[l] = a + b; o[l] = a - b;
-  }
-  e[0] *= 0.5; o[0] *= 0.5;
-#pragma unroll
-  for (int j = 0; j < LH; ++j) {
-    double ae0 = 0.0, ae1 = 0.0, ao0 = 0.0, ao1 = 0.0;      // two partial sums per output (see synthesis_column)
-#pragma unroll
-    for (int l = 0; l < LH; l += 2) {
-      ae0 = fma(T[(2 * j) * LH + l], e[l], ae0); ae1 = fma(T[(2 * j) * LH + l + 1], e[l + 1], ae1);
-      ao0 = fma(T[(2 * j + 1) * LH + l], o[l], ao0); ao1 = fma(T[(2 * j + 1) * LH + l + 1], o[l + 1], ao1);
-    }
-    const double ae = ae0 + ae1, ao = ao0 + ao1;
-    v[(2 * j) * LN] = ae * (j == 0 ? 1.0 / N : 2.0 / N);
-    v[(2 * j + 1) * LN] = ao * ((2 * j + 1 == N) ? 1.0 / N : 2.0 / N);
-  }
-}
-
-// ---- DCT-I synthesis of a lane's column, in place: g_l = sum_n g^_n cos(n l pi/N)
-template <int NZ> __device__ __forceinline__ void synthesis_column(double* __restrict__ v) {
-  constexpr int N = NZ - 1, LH = NZ / 2;
-  const double* __restrict__ TE = tab<NZ>() + Tab<NZ>::SE;
-  const double* __restrict__ TO = tab<NZ>() + Tab<NZ>::SO;
-  double ce[LH], co[LH];
-#pragma unroll
-  for (int j = 0; j < LH; ++j) { ce[j] = v[(2 * j) * LN]; co[j] = v[(2 * j + 1) * LN]; }
-  // two partial sums per output: with a single dependent chain per output the compiler interleaves many outputs and then
-  // spends one uniform-register move per DFMA on juggling the table operands
-#pragma unroll
-  for (int l = 0; l < LH; ++l) {
-    double E0 = 0.0, E1 = 0.0, O0 = 0.0, O1 = 0.0;
-#pragma unroll
-    for (int j = 0; j < LH; j += 2) {
-      E0 = fma(TE[l * LH + j], ce[j], E0); E1 = fma(TE[l * LH + j + 1], ce[j + 1], E1);
-      O0 = fma(TO[l * LH + j], co[j], O0); O1 = fma(TO[l * LH + j + 1], co[j + 1], O1);
-    }
-    const double E = E0 + E1, O = O0 + O1;
-    v[l * LN] = E + O;
-    v[(N - l) * LN] = E - O;
-  }
-}
-
 // ---- coefficient-space z-derivative of a lane's column (both parities), top-down recurrence
 //   d_N = 0, d_n = d_{n+2} + 2(n+1) g_{n+1},  (D g)_n = (2/H) d_n (d_0 halved);  dst[n] (+)= scale * (D src)_n
-template <int NZ, bool ACC> __device__ __forceinline__ void deriv_column(const double* __restrict__ src, double* __restrict__ dst, double inv_s, double scale) {
+template <int NZ, bool ACC> __device__ __forceinline__ void deriv_column(const double* __restrict__ src, double* __restrict__ dst, int lane, double inv_s, double scale) {
   constexpr int N = NZ - 1;
   double g[NZ];
 #pragma unroll
-  for (int n = 1; n <= N; ++n) g[n] = src[n * LN];
+  for (int n = 1; n <= N; ++n) g[n] = EL(src, n, lane);
   double d0 = 0.0, d1 = 0.0;          // running sums of the two parities
   const double f = inv_s * scale;
 #pragma unroll
@@ -138,7 +167,7 @@ template <int NZ, bool ACC> __device__ __forceinline__ void deriv_column(const d
     double& d = (n & 1) ? d1 : d0;
     if (n + 1 <= N) d = fma(2.0 * (n + 1), g[n + 1], d);
     const double val = d * (n == 0 ? 0.5 * f : f);
-    if (ACC) dst[n * LN] += val; else dst[n * LN] = val;
+    if (ACC) EL(dst, n, lane) += val; else EL(dst, n, lane) = val;
   }
 }
 
@@ -191,39 +220,33 @@ __device__ __forceinline__ double factor_chain(double* __restrict__ Fm, double* 
 
 // ---- one chain of one BVP for a lane: forward elimination, back substitution with the boundary functional, border
 //      unknown, double integration.  a[j] = (H/2)^2 r_n of row n = n0+2j on entry, rho0 = (H/2)^2 r_0 (even chain).
-//      Writes y's coefficients c_n of parity PAR to col and, if WITH_D, the coefficients of dy/dz of the OTHER parity to
-//      dcol.  Returns S_c = sum of the c_n written (incl. c_0 for the even chain).
+//      Writes y's coefficients c_n of parity PAR to tile `col` and, if SUB_D, SUBTRACTS the coefficients of dy/dz (they have the
+//      OTHER parity) from tile `dcol`.  Returns S_c = sum of the c_n written (incl. c_0 for the even chain).
 template <int NZ, int PAR>
-__device__ __forceinline__ double chain(bool WITH_D, double (&a)[Ch<NZ, PAR>::NR], double rho0, const double* __restrict__ Fm, const double* __restrict__ Fi,
-                                        const double* __restrict__ Fa, double* __restrict__ col, double* __restrict__ dcol, double k,
+__device__ __forceinline__ double chain(bool SUB_D, double (&a)[Ch<NZ, PAR>::NR], double rho0, const double* __restrict__ Fm, const double* __restrict__ Fi,
+                                        const double* __restrict__ Fa, double* __restrict__ col, double* __restrict__ dcol, int lane, double k,
                                         double k2, double inv_s, double beta_bc, double invBg) {
   constexpr int N = NZ - 1, n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR;
   const double* __restrict__ T = tab<NZ>();
-  double mult[NR], invd[NR], ag[NR];
-#pragma unroll
-  for (int j = 0; j < NR; ++j) {
-    const int n = n0 + 2 * j;
-    mult[j] = j > 0 ? Fm[n * TM] : 0.0; invd[j] = Fi[n * TM]; ag[j] = Fa[n * TM];
-  }
   if (!PAR) a[0] = fma(0.25 * k2, rho0, a[0]);               // even chain: row 2 carries (kappa^2/4) rho_0
 #pragma unroll
-  for (int j = 1; j < NR; ++j) a[j] = fma(-mult[j], a[j - 1], a[j]);
+  for (int j = 1; j < NR; ++j) a[j] = fma(-Fm[(n0 + 2 * j) * TM], a[j - 1], a[j]);
   double SP = 0.0, SQ = 0.0, next = 0.0;
 #pragma unroll
   for (int j = NR - 1; j >= 0; --j) {
     const int n = n0 + 2 * j;
-    const double v = (a[j] - row_u<NZ>(n, k2) * next) * invd[j];
+    const double v = (a[j] - row_u<NZ>(n, k2) * next) * Fi[n * TM];
     a[j] = v; next = v;
     SP = fma(T[Tab<NZ>::P + n], v, SP); SQ = fma(T[Tab<NZ>::Q + n], v, SQ);
   }
   if (!PAR) { SP = fma(T[Tab<NZ>::P + 0], rho0, SP); SQ = fma(T[Tab<NZ>::Q + 0], rho0, SQ); }
   const double border = (beta_bc - (inv_s * SP + k * SQ)) * invBg;       // c_0 (even chain) or b_0 (odd chain)
 #pragma unroll
-  for (int j = 0; j < NR; ++j) a[j] = fma(border, ag[j], a[j]);
+  for (int j = 0; j < NR; ++j) a[j] = fma(border, Fa[(n0 + 2 * j) * TM], a[j]);
   // integrate twice:  b_{n+1} = (cbar_n a_n - a_{n+2}) / (2(n+1)),  c_n = (cbar_{n-1} b_{n-1} - b_{n+1}) / (2n)
-  double Sc = 0.0, bprev;
-  if (!PAR) { col[0] = border; Sc = border; bprev = 0.0; }
-  else { bprev = border; if (WITH_D) dcol[0] = border * inv_s; }
+  double Sc0 = 0.0, Sc1 = 0.0, bprev;
+  if (!PAR) { EL(col, 0, lane) = border; Sc0 = border; bprev = 0.0; }
+  else { bprev = border; if (SUB_D) EL(dcol, 0, lane) -= border * inv_s; }
 #pragma unroll
   for (int i = 0; i <= (N - PAR) / 2; ++i) {
     const int n = PAR + 2 * i;
@@ -234,14 +257,13 @@ __device__ __forceinline__ double chain(bool WITH_D, double (&a)[Ch<NZ, PAR>::NR
     const double bn1 = ((n == 0 ? 2.0 : 1.0) * an - ap) * (1.0 / (2.0 * (n + 1)));
     if (n >= 1) {
       const double c = ((n == 1 ? 2.0 : 1.0) * bprev - bn1) * (1.0 / (2.0 * n));
-      col[n * LN] = c;
-      Sc += c;
+      EL(col, n, lane) = c;
+      if (i & 1) Sc1 += c; else Sc0 += c;
     }
-    if (WITH_D && n + 1 <= N - 1) dcol[(n + 1) * LN] = bn1 * inv_s;
+    if (SUB_D && n + 1 <= N - 1) EL(dcol, n + 1, lane) -= bn1 * inv_s;
     bprev = bn1;
   }
-  if (WITH_D && ((N - PAR) & 1) == 1) dcol[N * LN] = 0.0;    // (D y)_N = 0: slot N belongs to the chain whose b's have N's parity
-  return Sc;
+  return Sc0 + Sc1;
 }
 
 // ---- 4x4 real system, one right-hand side per lane, partial pivoting after row equilibration
@@ -288,8 +310,8 @@ struct ModeK {
   double k, k2, kxt, kyt, sgI;       // |k|, (k H/2)^2, derivative multipliers (0 on the unpaired Nyquist index), sign of Re/Im(i z)
 };
 
-// ---- one BVP item of a lane: kind 0 = pressure (eqs 15, 17): right-hand side i k.f + dz f_z, p -> C3, dp/dz -> C4;
-//      kind 1 = u or v (comp 0, 1), kind 2 = w (eq 18 with BCs 22, 24): f_c (column comp) is overwritten by u_c.
+// ---- one BVP item of a lane: kind 0 = pressure (eqs 15, 17): right-hand side i k.f + dz f_z, p -> tile 3, and f_z -= dz p in
+//      tile 2; kind 1 = u or v (comp 0, 1), kind 2 = w (eq 18 with BCs 22, 24): f_c (tile comp) is overwritten by u_c.
 //      One code path per parity so that the chain sweeps exist once in the instruction stream.
 template <int NZ, int PAR>
 __device__ __noinline__ double bvp_item(int kind, int comp, double* __restrict__ C, const double* __restrict__ F, int lane, int mode, ModeK K,
@@ -298,9 +320,9 @@ __device__ __noinline__ double bvp_item(int kind, int comp, double* __restrict__
   double a[NR], rho0 = 0.0, beta_bc = 0.0;
   double* col;
   if (kind == 0) {
-    const double* fxo = C + 0 * VS + (lane ^ 1);          // the OTHER part of f_x, f_y: i k f mixes re and im
-    const double* fyo = C + 1 * VS + (lane ^ 1);
-    const double* fz = C + 2 * VS + lane;
+    const double* fx = C + 0 * VS;                        // read at lane ^ 1: i k f mixes re and im
+    const double* fy = C + 1 * VS;
+    const double* fz = C + 2 * VS;
     double d = 0.0;
     constexpr int ntop = ((N - PAR) & 1) ? N - 1 : N;     // largest n <= N with parity PAR
     const double s2 = s * s;
@@ -308,38 +330,43 @@ __device__ __noinline__ double bvp_item(int kind, int comp, double* __restrict__
     for (int i = 0; i <= ntop / 2; ++i) {
       const int n = ntop - 2 * i;
       if (n < 0) break;
-      if (n + 1 <= N) d = fma(2.0 * (n + 1), fz[(n + 1) * LN], d);
+      if (n + 1 <= N) d = fma(2.0 * (n + 1), EL(fz, n + 1, lane), d);
       if (n <= N - 2) {
-        const double r = fma(K.sgI, fma(K.kxt, fxo[n * LN], K.kyt * fyo[n * LN]), d * (n == 0 ? 0.5 * inv_s : inv_s)) * s2;
+        const double r = fma(K.sgI, fma(K.kxt, EL(fx, n, lane ^ 1), K.kyt * EL(fy, n, lane ^ 1)), d * (n == 0 ? 0.5 * inv_s : inv_s)) * s2;
         if (n >= n0) a[n >= n0 ? (n - n0) / 2 : 0] = r; else rho0 = r;
       }
     }
-    col = C + 3 * VS + lane;
+    col = C + 3 * VS;
   } else {
-    col = C + comp * VS + lane;
+    col = C + comp * VS;
     const double sc = s * s / eta;
     double gH, g0;
-    // kind 1: r = (i k_c p - f_c)/eta ; kind 2: r = (dz p - f_z)/eta
-    const double* src = kind == 1 ? C + 3 * VS + (lane ^ 1) : C + 4 * VS + lane;
     const double kc = comp == 0 ? K.kxt : K.kyt;
-    const double f = kind == 1 ? K.sgI * kc : 1.0;
-#pragma unroll
-    for (int i = 0; i <= (N - 2 - PAR) / 2; ++i) {
-      const int n = PAR + 2 * i;
-      const double r = (f * src[n * LN] - col[n * LN]) * sc;
-      if (n >= n0) a[n >= n0 ? (n - n0) / 2 : 0] = r; else rho0 = r;
-    }
     if (kind == 1) {
-      // (dz + k) u(H) = -(i k_c/(2 k eta)) p(H) ; (dz - k) u(0) = +(i k_c/(2 k eta)) p(0)      (eq 22)
+      // r = (i k_c p - f_c)/eta ; (dz + k) u(H) = -(i k_c/(2 k eta)) p(H) ; (dz - k) u(0) = +(i k_c/(2 k eta)) p(0)      (eqs 18, 22)
+      const double* p = C + 3 * VS;
+      const double f = K.sgI * kc;
+#pragma unroll
+      for (int i = 0; i <= (N - 2 - PAR) / 2; ++i) {
+        const int n = PAR + 2 * i;
+        const double r = (f * EL(p, n, lane ^ 1) - EL(col, n, lane)) * sc;
+        if (n >= n0) a[n >= n0 ? (n - n0) / 2 : 0] = r; else rho0 = r;
+      }
       const double c = kc / (2.0 * K.k * eta);
       gH = -K.sgI * c * pH_oth; g0 = K.sgI * c * p0_oth;
     } else {
-      // (dz + k) w(H) = p(H)/(2 eta) ; (dz - k) w(0) = p(0)/(2 eta)                              (eq 24)
+      // r = (dz p - f_z)/eta = -(f_z - dz p)/eta ; (dz + k) w(H) = p(H)/(2 eta) ; (dz - k) w(0) = p(0)/(2 eta)          (eqs 18, 24)
+#pragma unroll
+      for (int i = 0; i <= (N - 2 - PAR) / 2; ++i) {
+        const int n = PAR + 2 * i;
+        const double r = -EL(col, n, lane) * sc;
+        if (n >= n0) a[n >= n0 ? (n - n0) / 2 : 0] = r; else rho0 = r;
+      }
       gH = pH_own / (2.0 * eta); g0 = p0_own / (2.0 * eta);
     }
     beta_bc = PAR ? 0.5 * (gH + g0) : 0.5 * (gH - g0);
   }
-  return chain<NZ, PAR>(kind == 0, a, rho0, F + 0 * NZ * TM + mode, F + 1 * NZ * TM + mode, F + 2 * NZ * TM + mode, col, C + 4 * VS + lane,
+  return chain<NZ, PAR>(kind == 0, a, rho0, F + 0 * NZ * TM + mode, F + 1 * NZ * TM + mode, F + 2 * NZ * TM + mode, col, C + 2 * VS, lane,
                         K.k, K.k2, inv_s, beta_bc, invBg);
 }
 
@@ -393,13 +420,16 @@ __device__ __forceinline__ void correction_coefficients(const double* __restrict
 }
 
 template <int NZ> struct SolveSmem {
-  static constexpr int VS = NZ * LN;                                   // one complex column [n][lane]
-  static constexpr int COLS = 6 * VS;                                  // C0..C5
+  static constexpr int VS = NZ * LN;                                   // one complex column tile [n][lane ^ swz(n)]
+  static constexpr int COLS = 5 * VS;                                  // tiles 0..4
   static constexpr int FACT = COLS;                                    // [3][NZ][TM]: multipliers, inverse pivots, border solution
   static constexpr int IBG = FACT + 3 * NZ * TM;                       // [2][TM] 1/B_g of the even / odd chain
   static constexpr int SUM = IBG + 2 * TM;                             // [4][2][LN] S_c of (p,u,v,w) x (even, odd chain)
-  static constexpr int CORR = SUM + 8 * LN;                            // [12][LN] correction coefficients (slit)
-  static constexpr int DOUBLES = CORR + 12 * LN;
+  static constexpr int DOUBLES = SUM + 8 * LN;
+  static constexpr int CORR = FACT;                                    // [12][LN] slit correction coefficients: the factors are dead by then
+  static_assert(12 * LN <= 3 * NZ * TM, "correction coefficients fit in the factor area");
+  static constexpr int PER_SM = (227 * 1024) / (DOUBLES * 8 + 1024);   // CTAs that fit an SM's shared memory
+  static constexpr int CTAS = PER_SM >= 4 ? 4 : (PER_SM >= 1 ? PER_SM : 1);
 };
 
 #ifdef DP_SOLVE_TIMING
@@ -412,11 +442,11 @@ __device__ int g_tcount[4];
 #endif
 
 template <int NZ>
-__global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(SolveArgs A) {
-  extern __shared__ double smem[];
-  constexpr int N = NZ - 1, VS = NZ * LN;
+__global__ void __launch_bounds__(SOLVE_THREADS, SolveSmem<NZ>::CTAS) k_solve(SolveArgs A) {
+  extern __shared__ __align__(16) double smem[];
+  constexpr int VS = NZ * LN;
   typedef SolveSmem<NZ> S;
-  double* C = smem;                      // columns: 0 f_x->u, 1 f_y->v, 2 f_z->w, 3 t_x->p->dz u, 4 t_y->dz p->dz v, 5 (E, zE)
+  double* C = smem;                      // tiles: 0 f_x->u, 1 f_y->v, 2 f_z->f_z - dz p->w, 3 t_x->p->dz u, 4 t_y->(E, zE)->dz v
   double* F = smem + S::FACT;
   double* s_ibg = smem + S::IBG;
   double* s_sum = smem + S::SUM;
@@ -460,31 +490,44 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
   const size_t off0 = (size_t)islow * A.pitch + ifast;
   const double* gin = reinterpret_cast<const double*>(A.cplx);
 
-  // ---------------- phase 0: all nodal columns go HBM -> shared memory as 8-byte cp.async (no registers, everything in
-  // flight at once); t_z is only needed for the fold and travels through registers.  While the loads fly: warps 0, 1 factor
-  // the two chains, warps 2-5 evaluate e^{-k z_l} and z_l e^{-k z_l} at the nodes (-> C5).  Then every warp folds the
-  // algebraic part of (1/2) curl t into f for the rows it loaded itself (eq 7).
-  constexpr int ROWS = (NZ + SOLVE_WARPS - 1) / SOLVE_WARPS;
+  // ---------------- phase 0: the nodal columns go HBM -> shared memory as 16-byte cp.async (one (re, im) pair per copy, L1
+  // bypassed, no registers).  A warp takes the node pairs (l, N-l), l = wid, wid + 6, ... < NP: node l lands in row l, node N-l in
+  // row NP + l; its lanes 0-15 copy the modes of tiles 0, 2, 4, its lanes 16-31 those of tiles 1, 3.  t_z is only needed for the
+  // fold below and travels through registers.  While the loads fly, warps 0, 1 factor the two chains.  Then every warp, for the
+  // pairs it loaded itself, folds the algebraic part of (1/2) curl t into f (eq 7) and replaces (g_l, g_{N-l}) by (e_l, o_l).
+  typedef Tr<NZ> G;
+  constexpr int N = NZ - 1, NP = G::NP;
+  constexpr int PAIRS = (NP + SOLVE_WARPS - 1) / SOLVE_WARPS;
   const int lm = __ldg(A.lmin);
-  double tz[ROWS];
+  double tz[PAIRS][2];
+  {
+    const int sub = lane >> 4, m = lane & 15;
+    const int mfast = blockIdx.x * TM + m;
+    const bool mvalid = mfast < A.n_fast;
+    const size_t moff = (size_t)islow * A.pitch + mfast;
+    const int ntile = A.torque ? 5 : 3;
 #pragma unroll
-  for (int r = 0; r < ROWS; ++r) {
-    const int l = wid + r * SOLVE_WARPS;
-    tz[r] = 0.0;
-    if (l < NZ) {
-      const int o = l * LN + lane;
-      if (valid && l >= lm) {
-        const size_t og = 2 * (l * plane + off0) + part;
+    for (int r = 0; r < PAIRS; ++r) {
+      const int lp = wid + r * SOLVE_WARPS;
+      tz[r][0] = tz[r][1] = 0.0;
+      if (lp < NP) {
 #pragma unroll
-        for (int c = 0; c < 3; ++c) cp_async8(&C[c * VS + o], &gin[2 * (c * A.cplx_field) + og]);
-        if (A.torque) {
-          cp_async8(&C[3 * VS + o], &gin[2 * (3 * A.cplx_field) + og]);
-          cp_async8(&C[4 * VS + o], &gin[2 * (4 * A.cplx_field) + og]);
-          tz[r] = __ldg(&gin[2 * (5 * A.cplx_field) + og]);
+        for (int h = 0; h < 2; ++h) {
+          const int l = h ? N - lp : lp, row = h ? NP + lp : lp;          // node, row
+          if (h && l == lp) continue;                                     // the middle node of an odd nz has no partner
+          const int sw = swz_rt(row);
+          const bool live = mvalid && l >= lm;
+#pragma unroll
+          for (int q = 0; q < 3; ++q) {
+            const int c = 2 * q + sub;
+            if (c < ntile) {
+              double* dst = &C[c * VS + row * LN + ((2 * m) ^ sw)];
+              if (live) cp_async16(dst, A.cplx + c * A.cplx_field + l * plane + moff);
+              else *reinterpret_cast<double2*>(dst) = make_double2(0.0, 0.0);
+            }
+          }
+          if (A.torque && valid && l >= lm) tz[r][h] = ldg_stream(&gin[2 * (5 * A.cplx_field + l * plane + off0) + part]);
         }
-      } else {
-#pragma unroll
-        for (int c = 0; c < 5; ++c) C[c * VS + o] = 0.0;
       }
     }
   }
@@ -496,69 +539,111 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
   } else if (wid == 1) {
     const double ib = factor_chain<NZ, 1>(F + mode, F + NZ * TM + mode, F + 2 * NZ * TM + mode, K.k, K.k2, inv_s, part == 0);
     if (part == 0) s_ibg[TM + mode] = ib;
-  } else {
-    for (int l = wid - 2; l < NZ; l += SOLVE_WARPS - 2) {
-      const double zl = s * (1.0 + T[Tab<NZ>::XI + l]);
-      const double E = exp(-K.k * zl);
-      C[5 * VS + l * LN + lane] = part ? zl * E : E;
-    }
   }
   TMARK(2);
   cp_async_wait_all();
   __syncwarp();
-  if (A.torque) {
+  {
+    const int ntile = A.torque ? 5 : 3;
 #pragma unroll
-    for (int r = 0; r < ROWS; ++r) {
-      const int l = wid + r * SOLVE_WARPS;
-      if (l < NZ) {
-        const int o = l * LN + lane, oo = l * LN + (lane ^ 1);
-        const double t2o = __shfl_xor_sync(0xffffffffu, tz[r], 1);
-        const double t0o = C[3 * VS + oo], t1o = C[4 * VS + oo];
-        C[0 * VS + o] = fma(0.5 * K.sgI * K.kyt, t2o, C[0 * VS + o]);                       // f_x += (1/2) i k_y t_z
-        C[1 * VS + o] = fma(-0.5 * K.sgI * K.kxt, t2o, C[1 * VS + o]);                      // f_y -= (1/2) i k_x t_z
-        C[2 * VS + o] = fma(0.5 * K.sgI, K.kxt * t1o - K.kyt * t0o, C[2 * VS + o]);         // f_z += (1/2) i (k_x t_y - k_y t_x)
+    for (int r = 0; r < PAIRS; ++r) {
+      const int lp = wid + r * SOLVE_WARPS;
+      if (lp < NP) {
+        const bool pair = (N - lp) != lp;
+        const int ra = lp, rb = NP + lp;
+        const int oa = ra * LN + (lane ^ swz_rt(ra)), ob = rb * LN + (lane ^ swz_rt(rb));
+        double va[5], vb[5];
+#pragma unroll
+        for (int c = 0; c < 5; ++c) { va[c] = vb[c] = 0.0; if (c < ntile) { va[c] = C[c * VS + oa]; if (pair) vb[c] = C[c * VS + ob]; } }
+        if (A.torque) {
+          // the OTHER part of t: i k x t mixes re and im
+          const double txa = __shfl_xor_sync(0xffffffffu, va[3], 1), tya = __shfl_xor_sync(0xffffffffu, va[4], 1), tza = __shfl_xor_sync(0xffffffffu, tz[r][0], 1);
+          const double txb = __shfl_xor_sync(0xffffffffu, vb[3], 1), tyb = __shfl_xor_sync(0xffffffffu, vb[4], 1), tzb = __shfl_xor_sync(0xffffffffu, tz[r][1], 1);
+          va[0] = fma(0.5 * K.sgI * K.kyt, tza, va[0]);                        // f_x += (1/2) i k_y t_z
+          va[1] = fma(-0.5 * K.sgI * K.kxt, tza, va[1]);                       // f_y -= (1/2) i k_x t_z
+          va[2] = fma(0.5 * K.sgI, K.kxt * tya - K.kyt * txa, va[2]);          // f_z += (1/2) i (k_x t_y - k_y t_x)
+          vb[0] = fma(0.5 * K.sgI * K.kyt, tzb, vb[0]);
+          vb[1] = fma(-0.5 * K.sgI * K.kxt, tzb, vb[1]);
+          vb[2] = fma(0.5 * K.sgI, K.kxt * tyb - K.kyt * txb, vb[2]);
+        }
+#pragma unroll
+        for (int c = 0; c < 5; ++c)
+          if (c < ntile) { C[c * VS + oa] = va[c] + vb[c]; if (pair) C[c * VS + ob] = va[c] - vb[c]; }
       }
     }
   }
   TMARK(3);
   __syncthreads();
 
-  // ---------------- phase 1: Chebyshev analysis, one warp per column: f_x, f_y, f_z, (E, zE) [, t_x, t_y]   (step 2; step 6)
+  // ---------------- phase 1: Chebyshev analysis of f_x, f_y, f_z [, t_x, t_y] on the tensor pipe, one (tile, parity) item per warp   (step 2)
   {
-    const int col = wid < 3 ? wid : (wid == 3 ? 5 : wid - 1);          // warps 0-2: C0-C2, warp 3: C5, warps 4, 5: C3, C4
-    if (wid < 4 || A.torque) analysis_column<NZ>(C + col * VS + lane);
+    const int nitems = (A.torque ? 5 : 3) * 2;
+    for (int i = wid; i < nitems; i += SOLVE_WARPS) transform_item<NZ, 4>(C + (i >> 1) * VS, i & 1, 0, A.frag, lane);
   }
   TMARK(4);
   __syncthreads();
 
-  // ---------------- phase 2: f_x -= (1/2) D t_y, f_y += (1/2) D t_x (eq 7)
-  if (A.torque) {
-    if (wid < 2) deriv_column<NZ, true>(C + (wid == 0 ? 4 : 3) * VS + lane, C + wid * VS + lane, inv_s, wid == 0 ? -0.5 : 0.5);
+  // ---------------- phases 2, 3: warps 0, 1: f_x -= (1/2) D t_y, f_y += (1/2) D t_x (eq 7), then the pressure BVP (eqs 15, 17), one
+  // chain each.  Warps 2-5 meanwhile evaluate e^{-k z_l} and z_l e^{-k z_l} at the nodes, put them into tile 4 once t_y has
+  // been consumed, and transform them (one 8-lane block each); their coefficients are needed for the correction (step 6).
+  if (wid < 2) {
+    if (A.torque) deriv_column<NZ, true>(C + (wid == 0 ? 4 : 3) * VS, C + wid * VS, lane, inv_s, wid == 0 ? -0.5 : 0.5);
     TMARK(5);
-    __syncthreads();
-  }
-
-  // ---------------- phases 3, 4: pressure BVP (eqs 15, 17), one warp per chain; then the velocity BVPs (eq 18) with BCs
-  // (22), (24), one warp per (component, chain)
-#pragma unroll 1
-  for (int ph = 0; ph < 2; ++ph) {
-    if (ph == 1 || wid < 2) {
-      const int comp = wid >> 1, par = wid & 1;
-      const int kind = ph == 0 ? 0 : (comp == 2 ? 2 : 1);
-      double pH = 0.0, p0 = 0.0;
-      if (ph == 1) {
-        const double se = s_sum[0 * LN + lane], so = s_sum[1 * LN + lane];
-        pH = se + so; p0 = se - so;                       // p(H) = sum p_n, p(0) = sum (-1)^n p_n  ("direct summation")
+    named_arrive(2, SOLVE_THREADS);                        // t_y has been read: tile 4 may be overwritten
+    named_sync(1, 64);                                     // f_x and f_y are complete (and t_x consumed) before either chain starts
+    double Sc;
+    if (wid) Sc = bvp_item<NZ, 1>(0, 0, C, F, lane, mode, K, s, inv_s, eta, s_ibg[TM + mode], 0.0, 0.0, 0.0, 0.0);
+    else Sc = bvp_item<NZ, 0>(0, 0, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], 0.0, 0.0, 0.0, 0.0);
+    s_sum[(0 * 2 + wid) * LN + lane] = Sc;
+  } else {
+    constexpr int ER = (NP + 3) / 4;                       // node pairs (l, N-l) per thread
+    double ee[ER], eo[ER];
+#pragma unroll
+    for (int r = 0; r < ER; ++r) {
+      const int lp = (wid - 2) + 4 * r;
+      ee[r] = eo[r] = 0.0;
+      if (lp < NP) {
+        const double za = s * (1.0 + T[Tab<NZ>::XI + lp]);
+        const double Ea = exp(-K.k * za);
+        const double a = part ? za * Ea : Ea;
+        double b = 0.0;
+        if (N - lp != lp) {
+          const double zb = s * (1.0 + T[Tab<NZ>::XI + N - lp]);
+          const double Eb = exp(-K.k * zb);
+          b = part ? zb * Eb : Eb;
+        }
+        ee[r] = a + b; eo[r] = a - b;
       }
-      const double pHo = __shfl_xor_sync(0xffffffffu, pH, 1), p0o = __shfl_xor_sync(0xffffffffu, p0, 1);
-      double Sc;
-      if (par) Sc = bvp_item<NZ, 1>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[TM + mode], pH, p0, pHo, p0o);
-      else Sc = bvp_item<NZ, 0>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], pH, p0, pHo, p0o);
-      s_sum[((ph == 0 ? 0 : 1 + comp) * 2 + par) * LN + lane] = Sc;
     }
-    TMARK(6 + ph);
-    __syncthreads();
+    named_sync(2, SOLVE_THREADS);
+#pragma unroll
+    for (int r = 0; r < ER; ++r) {
+      const int lp = (wid - 2) + 4 * r;
+      if (lp < NP) {
+        C[4 * VS + lp * LN + (lane ^ swz_rt(lp))] = ee[r];
+        if (N - lp != lp) C[4 * VS + (NP + lp) * LN + (lane ^ swz_rt(NP + lp))] = eo[r];
+      }
+    }
+    named_sync(3, 128);
+    transform_item<NZ, 2>(C + 4 * VS, (wid - 2) & 1, ((wid - 2) >> 1) * 2, A.frag, lane);
   }
+  TMARK(6);
+  __syncthreads();
+
+  // ---------------- phase 4: the velocity BVPs (eq 18) with BCs (22), (24), one warp per (component, chain)
+  {
+    const int comp = wid >> 1, par = wid & 1;
+    const int kind = comp == 2 ? 2 : 1;
+    const double se = s_sum[0 * LN + lane], so = s_sum[1 * LN + lane];
+    const double pH = se + so, p0 = se - so;              // p(H) = sum p_n, p(0) = sum (-1)^n p_n  ("direct summation")
+    const double pHo = __shfl_xor_sync(0xffffffffu, pH, 1), p0o = __shfl_xor_sync(0xffffffffu, p0, 1);
+    double Sc;
+    if (par) Sc = bvp_item<NZ, 1>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[TM + mode], pH, p0, pHo, p0o);
+    else Sc = bvp_item<NZ, 0>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], pH, p0, pHo, p0o);
+    s_sum[((1 + comp) * 2 + par) * LN + lane] = Sc;
+  }
+  TMARK(7);
+  __syncthreads();
 
   // ---------------- phase 5: correction coefficients (bottom wall: every warp for itself; slit: warp 0, shared)
   double cf[3][4];
@@ -580,53 +665,70 @@ __global__ void __launch_bounds__(SOLVE_THREADS, (NZ <= 32 ? 3 : 2)) k_solve(Sol
   }
 
   // ---------------- phase 6: total coefficients = DP + correction;  T[z e^{-k(H-z)}]_n = (-1)^n (H e_n - ze_n), T[e^{-k(H-z)}]_n = (-1)^n e_n
-  for (int n = wid; n < NZ; n += SOLVE_WARPS) {
-    const double mine = C[5 * VS + n * LN + lane], other = C[5 * VS + n * LN + (lane ^ 1)];
+  // (rows [0, NP) hold the even coefficients, rows [NP, nz) the odd ones)
+  for (int r = wid; r < NZ; r += SOLVE_WARPS) {
+    const int sw = swz_rt(r);
+    const double mine = C[4 * VS + r * LN + (lane ^ sw)], other = C[4 * VS + r * LN + ((lane ^ 1) ^ sw)];
     const double en = part ? other : mine, zen = part ? mine : other;
-    const double sgn = (n & 1) ? -1.0 : 1.0;
+    const double sgn = (r >= NP) ? -1.0 : 1.0;
     const double b2 = sgn * (A.H * en - zen), b3 = sgn * en;
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
       double add = fma(cf[c][0], zen, cf[c][1] * en);
       if (A.wall_mode == DP_SLIT) add = fma(cf[c][2], b2, fma(cf[c][3], b3, add));
-      C[c * VS + n * LN + lane] += add;
+      C[c * VS + r * LN + (lane ^ sw)] += add;
     }
   }
   TMARK(8);
   __syncthreads();
 
-  // ---------------- phase 7: dz u, dz v of the TOTAL in coefficient space (reading G12) -> C3, C4; synthesis back to the nodes
+  // ---------------- phase 7: dz u, dz v of the TOTAL in coefficient space (reading G12) -> tiles 3, 4 (warps 0, 1) while warps 2-5
+  // bring w back to the nodes; then synthesis of u, v [, dz u, dz v], (tile, parity, half) items dealt to the warps
   if (A.omega) {
-    if (wid < 2) deriv_column<NZ, false>(C + wid * VS + lane, C + (3 + wid) * VS + lane, inv_s, 1.0);
+    if (wid < 2) deriv_column<NZ, false>(C + wid * VS, C + (3 + wid) * VS, lane, inv_s, 1.0);
+    else transform_item<NZ, 2>(C + 2 * VS, 2 + ((wid - 2) & 1), ((wid - 2) >> 1) * 2, A.frag, lane);
     TMARK(9);
     __syncthreads();
+    for (int i = wid; i < 16; i += SOLVE_WARPS) { const int c = i >> 2; transform_item<NZ, 2>(C + (c < 2 ? c : c + 1) * VS, 2 + (i & 1), (i & 2), A.frag, lane); }
+  } else {
+    for (int i = wid; i < 6; i += SOLVE_WARPS) transform_item<NZ, 4>(C + (i >> 1) * VS, 2 + (i & 1), 0, A.frag, lane);
   }
-  if (wid < (A.omega ? 5 : 3)) synthesis_column<NZ>(C + wid * VS + lane);
   TMARK(10);
   __syncthreads();
 
-  // ---------------- phase 8: (1/2) curl u (eq 11), scale by 1/(nx ny) for the unnormalised inverse FFT, store
+  // ---------------- phase 8: back to the nodes g_l = E_l + O_l, g_{N-l} = E_l - O_l; (1/2) curl u (eq 11); scale by 1/(nx ny)
+  // for the unnormalised inverse FFT; store
   const double scl = 1.0 / ((double)A.nx * (double)A.ny);
   double* gout = reinterpret_cast<double*>(A.cplx);
-  for (int l = wid; l < NZ; l += SOLVE_WARPS) {
-    const int o = l * LN + lane;
-    const double u = C[0 * VS + o], v = C[1 * VS + o], w = C[2 * VS + o];
-    double om[3] = {0, 0, 0};
-    if (A.omega) {
-      const double du = C[3 * VS + o], dv = C[4 * VS + o];
-      const double uo = __shfl_xor_sync(0xffffffffu, u, 1), vo = __shfl_xor_sync(0xffffffffu, v, 1), wo = __shfl_xor_sync(0xffffffffu, w, 1);
-      om[0] = 0.5 * (K.sgI * K.kyt * wo - dv);                          // (1/2)(i k_y w - dz v)
-      om[1] = 0.5 * (du - K.sgI * K.kxt * wo);                          // (1/2)(dz u - i k_x w)
-      om[2] = 0.5 * K.sgI * (K.kxt * vo - K.kyt * uo);                  // (1/2)(i k_x v - i k_y u)
-    }
-    if (valid && !zero_mode) {
-      const size_t og = 2 * (l * plane + off0) + part;
-      gout[2 * (0 * A.cplx_field) + og] = u * scl;
-      gout[2 * (1 * A.cplx_field) + og] = v * scl;
-      gout[2 * (2 * A.cplx_field) + og] = w * scl;
-      if (A.omega) {
+  for (int lp = wid; lp < NP; lp += SOLVE_WARPS) {
+    const bool pair = (N - lp) != lp;
+    const int oa = lp * LN + (lane ^ swz_rt(lp)), ob = (NP + lp) * LN + (lane ^ swz_rt(NP + lp));
+    const int nt = A.omega ? 5 : 3;
+    double vE[5], vO[5];
 #pragma unroll
-        for (int c = 0; c < 3; ++c) gout[2 * ((3 + c) * A.cplx_field) + og] = om[c] * scl;
+    for (int c = 0; c < 5; ++c) { vE[c] = vO[c] = 0.0; if (c < nt) { vE[c] = C[c * VS + oa]; if (pair) vO[c] = C[c * VS + ob]; } }
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      if (h && !pair) continue;
+      const int l = h ? N - lp : lp;
+      const double u = h ? vE[0] - vO[0] : vE[0] + vO[0], v = h ? vE[1] - vO[1] : vE[1] + vO[1], w = h ? vE[2] - vO[2] : vE[2] + vO[2];
+      double om[3] = {0, 0, 0};
+      if (A.omega) {
+        const double du = h ? vE[3] - vO[3] : vE[3] + vO[3], dv = h ? vE[4] - vO[4] : vE[4] + vO[4];
+        const double uo = __shfl_xor_sync(0xffffffffu, u, 1), vo = __shfl_xor_sync(0xffffffffu, v, 1), wo = __shfl_xor_sync(0xffffffffu, w, 1);
+        om[0] = 0.5 * (K.sgI * K.kyt * wo - dv);                          // (1/2)(i k_y w - dz v)
+        om[1] = 0.5 * (du - K.sgI * K.kxt * wo);                          // (1/2)(dz u - i k_x w)
+        om[2] = 0.5 * K.sgI * (K.kxt * vo - K.kyt * uo);                  // (1/2)(i k_x v - i k_y u)
+      }
+      if (valid && !zero_mode) {
+        const size_t og = 2 * (l * plane + off0) + part;
+        gout[2 * (0 * A.cplx_field) + og] = u * scl;
+        gout[2 * (1 * A.cplx_field) + og] = v * scl;
+        gout[2 * (2 * A.cplx_field) + og] = w * scl;
+        if (A.omega) {
+#pragma unroll
+          for (int c = 0; c < 3; ++c) gout[2 * ((3 + c) * A.cplx_field) + og] = om[c] * scl;
+        }
       }
     }
   }
@@ -732,19 +834,13 @@ __global__ void k_zero_mode(SolveArgs A, int nz, const double* __restrict__ ct_f
 
 template <int NZ> size_t solve_smem_bytes() { return sizeof(double) * (size_t)SolveSmem<NZ>::DOUBLES; }
 
-template <int NZ> void host_tables(std::vector<double>& out) {
+// P_n, Q_n, XI_l of the constant table, and the transform fragment table of Tr<NZ>
+template <int NZ> void host_tables(std::vector<double>& ctab, std::vector<double>& frag) {
   typedef long double ld;
   const ld PI = 3.141592653589793238462643383279502884L;
-  constexpr int N = NZ - 1, LH = NZ / 2;
-  out.assign(Tab<NZ>::SIZE, 0.0);
-  for (int n = 0; n <= N; ++n)
-    for (int l = 0; l < LH; ++l) out[Tab<NZ>::CA + n * LH + l] = (double)cosl(PI * n * l / N);
-  for (int l = 0; l < LH; ++l)
-    for (int j = 0; j < LH; ++j) {
-      out[Tab<NZ>::SE + l * LH + j] = (double)cosl(PI * (2 * j) * l / N);
-      out[Tab<NZ>::SO + l * LH + j] = (double)cosl(PI * (2 * j + 1) * l / N);
-    }
-  for (int l = 0; l <= N; ++l) out[Tab<NZ>::XI + l] = (double)cosl(PI * l / N);
+  constexpr int N = NZ - 1;
+  ctab.assign(Tab<NZ>::SIZE, 0.0);
+  for (int l = 0; l <= N; ++l) ctab[Tab<NZ>::XI + l] = (double)cosl(PI * l / N);
   // P_n, Q_n: with a = unit vector e_n (n <= N-2), b_m = (cbar_{m-1} a_{m-1} - a_{m+1})/(2m) (1 <= m <= N-1),
   // c_m = (cbar_{m-1} b_{m-1} - b_{m+1})/(2m) (1 <= m <= N), b_0 = 0:  P_n = sum of b_m over m of the other parity,
   // Q_n = sum of c_m over m >= 1 of n's parity.
@@ -755,8 +851,27 @@ template <int NZ> void host_tables(std::vector<double>& out) {
     for (int mm = 1; mm <= N; ++mm) c[mm] = ((mm - 1 == 0 ? 2 : 1) * b[mm - 1] - b[mm + 1]) / (2 * (ld)mm);
     ld p = 0, q = 0;
     for (int mm = 1; mm <= N; ++mm) { if ((mm - n) % 2 != 0) p += b[mm]; else q += c[mm]; }
-    out[Tab<NZ>::P + n] = (double)p; out[Tab<NZ>::Q + n] = (double)q;
+    ctab[Tab<NZ>::P + n] = (double)p; ctab[Tab<NZ>::Q + n] = (double)q;
   }
+  // fragments: lane t of fragment (kind, mb, kb) holds M_kind[mb*8 + t/4][kb*4 + t%4]
+  typedef Tr<NZ> G;
+  frag.assign((size_t)G::FRAGS * 32, 0.0);
+  auto ctil = [&](int i) { return (i == 0 || i == N) ? (ld)2 : (ld)1; };
+  for (int kind = 0; kind < 4; ++kind)
+    for (int mb = 0; mb < G::MB; ++mb)
+      for (int kb = 0; kb < G::KB; ++kb)
+        for (int t = 0; t < 32; ++t) {
+          const int row = mb * 8 + t / 4, col = kb * 4 + t % 4;
+          ld v = 0;
+          if (kind < 2) {                // analysis: row = coefficient index j (n = 2j + kind), col = node pair l
+            const int n = 2 * row + kind, l = col;
+            if (n <= N && l < G::NP) v = (2 / (ld)N) / (ctil(n) * ctil(l)) * cosl(PI * (ld)n * l / N);
+          } else {                       // synthesis: row = node l, col = coefficient index j (n = 2j + kind - 2)
+            const int l = row, n = 2 * col + (kind - 2);
+            if (n <= N && l < G::NP) v = cosl(PI * (ld)n * l / N);
+          }
+          frag[((size_t)(kind * G::MB + mb) * G::KB + kb) * 32 + t] = (double)v;
+        }
 }
 
 template <int NZ> cudaError_t set_attr_nz() {      // per device: called by every plan at creation, on its own device
@@ -770,23 +885,38 @@ template <int NZ> cudaError_t launch_nz(const SolveArgs& A, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-int nz_slot(int nz) { return nz == 16 ? 0 : nz == 32 ? 1 : nz == 48 ? 2 : -1; }
-
 }  // namespace
 
-bool dp_solve_supports_nz(int nz) { return nz_slot(nz) >= 0; }
+bool dp_solve_supports_nz(int nz) {
+#define X(NZ) if (nz == NZ) return true;
+  DP_SOLVE_NZ_LIST(X)
+#undef X
+  return false;
+}
+
+int dp_solve_nz_list(int* out, int cap) {
+  int n = 0;
+#define X(NZ) { if (n < cap) out[n] = NZ; ++n; }
+  DP_SOLVE_NZ_LIST(X)
+#undef X
+  return n;
+}
 
 cudaError_t dp_solve_upload_tables(dp_plan* P) {
-  std::vector<double> t;
-  cudaError_t e = cudaSuccess;
+  std::vector<double> t, frag;
+  cudaError_t e = cudaErrorInvalidValue;
   const int nz = P->p.nz;
-  if (nz == 16) { host_tables<16>(t); e = cudaMemcpyToSymbol(c_tab16, t.data(), sizeof(double) * t.size()); }
-  else if (nz == 32) { host_tables<32>(t); e = cudaMemcpyToSymbol(c_tab32, t.data(), sizeof(double) * t.size()); }
-  else if (nz == 48) { host_tables<48>(t); e = cudaMemcpyToSymbol(c_tab48, t.data(), sizeof(double) * t.size()); }
-  else return cudaErrorInvalidValue;
+#define X(NZ) if (nz == NZ) { host_tables<NZ>(t, frag); e = cudaMemcpyToSymbol(c_tab##NZ, t.data(), sizeof(double) * t.size()); if (e == cudaSuccess) e = set_attr_nz<NZ>(); }
+  DP_SOLVE_NZ_LIST(X)
+#undef X
   if (e != cudaSuccess) return e;
-  if (nz == 16) e = set_attr_nz<16>(); else if (nz == 32) e = set_attr_nz<32>(); else e = set_attr_nz<48>();
-  if (e != cudaSuccess) return e;
+  if (!P->d_solve_frag) {
+    e = cudaMalloc(&P->d_solve_frag, sizeof(double) * frag.size());
+    if (e != cudaSuccess) return e;
+    P->device_bytes += sizeof(double) * frag.size();
+    e = cudaMemcpy(P->d_solve_frag, frag.data(), sizeof(double) * frag.size(), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return e;
+  }
   if (!P->d_ct_full) {
     typedef long double ld;
     const ld PI = 3.141592653589793238462643383279502884L;
@@ -802,6 +932,7 @@ cudaError_t dp_solve_upload_tables(dp_plan* P) {
 
 void dp_solve_destroy_tables(dp_plan* P) {
   if (P->d_ct_full) { cudaFree(P->d_ct_full); P->d_ct_full = nullptr; }
+  if (P->d_solve_frag) { cudaFree(P->d_solve_frag); P->d_solve_frag = nullptr; }
 }
 
 cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega, cudaStream_t st) {
@@ -810,15 +941,13 @@ cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega,
   A.nx = P->p.nx; A.ny = P->p.ny; A.nkx = P->nkx;
   A.n_fast = P->nkx; A.n_slow = P->p.ny; A.pitch = P->nkxp; A.fast_is_x = 1; A.ky_of_pos = nullptr; A.lmin = P->d_lmin;
   if (P->own_fft) { A.n_fast = P->p.ny; A.n_slow = P->nkx; A.pitch = P->p.ny; A.fast_is_x = 0; A.ky_of_pos = dp_fft_own_ky_table(P); }
+  A.frag = P->d_solve_frag;
   A.Lx = P->p.Lx; A.Ly = P->p.Ly; A.H = P->p.H; A.eta = P->p.eta;
   A.wall_mode = P->p.wall_mode; A.torque = with_torque_field ? 1 : 0; A.omega = want_omega ? 1 : 0;
-  cudaError_t e;
-  switch (P->p.nz) {
-    case 16: e = launch_nz<16>(A, st); break;
-    case 32: e = launch_nz<32>(A, st); break;
-    case 48: e = launch_nz<48>(A, st); break;
-    default: return cudaErrorInvalidValue;
-  }
+  cudaError_t e = cudaErrorInvalidValue;
+#define X(NZ) if (P->p.nz == NZ) e = launch_nz<NZ>(A, st);
+  DP_SOLVE_NZ_LIST(X)
+#undef X
   if (e != cudaSuccess) return e;
   k_zero_mode<<<1, 64, 0, st>>>(A, P->p.nz, P->d_ct_full);
   return cudaGetLastError();
