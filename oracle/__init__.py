@@ -55,6 +55,12 @@ def lib():
         L.or_es_norm.argtypes = [d, d]
         L.or_es_phi.restype = d
         L.or_es_phi.argtypes = [d, d, d, d]
+        L.or_es_dphi_cut.restype = d
+        L.or_es_dphi_cut.argtypes = [d]
+        L.or_es_dphi.restype = d
+        L.or_es_dphi.argtypes = [d, d, d, d, d]
+        L.or_spread_curl.argtypes = [p, i, p, p, d, p]
+        L.or_interp_curl.argtypes = [p, i, p, p, d, p]
         L.or_cheb_nodes.argtypes = [i, d, p]
         L.or_cheb_analysis_matrix.argtypes = [i, p]
         L.or_cheb_synthesis_matrix.argtypes = [i, p]
@@ -164,6 +170,37 @@ def interp(prob, pos, grid, beta: float) -> np.ndarray:
     return out
 
 
+def es_dphi_cut(beta: float) -> float:
+    """|s|/alpha beyond which the kernel derivative is truncated to zero (footnote 47)."""
+    return float(lib().or_es_dphi_cut(beta))
+
+
+def es_dphi(s, alpha: float, beta: float, Z: float | None = None, ucut: float | None = None):
+    """Truncated derivative of the ES kernel (footnote 47)."""
+    Z = es_norm(alpha, beta) if Z is None else Z
+    ucut = es_dphi_cut(beta) if ucut is None else ucut
+    f = np.vectorize(lambda x: lib().or_es_dphi(float(x), alpha, beta, Z, ucut))
+    return f(np.asarray(s, dtype=np.float64))
+
+
+def spread_curl(prob, pos, torque, beta: float, grid: np.ndarray) -> np.ndarray:
+    """Kernel-derivative torque spreading: grid += (1/2) curl_x (tau Delta_D^W)   (eq 7, footnotes 47-48)."""
+    pos, torque = _f64(pos), _f64(torque)
+    assert grid.shape == (3, prob.nz, prob.ny, prob.nx) and grid.flags.c_contiguous and grid.dtype == np.float64
+    P = _params(prob)
+    lib().or_spread_curl(ctypes.byref(P), pos.shape[0], _ptr(pos), _ptr(torque), beta, _ptr(grid))
+    return grid
+
+
+def interp_curl(prob, pos, grid, beta: float) -> np.ndarray:
+    """Kernel-derivative angular velocity: Omega = (1/2) sum_g u x grad Delta_D^W h^2 (H/2) w_l   (eq 11 by parts)."""
+    pos, grid = _f64(pos), _f64(grid)
+    P = _params(prob)
+    out = np.empty((pos.shape[0], 3))
+    lib().or_interp_curl(ctypes.byref(P), pos.shape[0], _ptr(pos), _ptr(grid), beta, _ptr(out))
+    return out
+
+
 def dft_xy_forward(real: np.ndarray, dft: str = "naive") -> np.ndarray:
     """Step 2, xy part (O2): unnormalised forward DFT over the last two axes (j, i) -> half spectrum (ny, nx/2+1)."""
     real = _f64(real)
@@ -215,8 +252,11 @@ def solve_modes(prob, ix, iy, fh, th=None, want_omega=False):
     return uh, wh
 
 
-def mobility_apply(prob, pos, force=None, torque=None, want_omega=None, dft="naive", stages=None, timing=None):
+def mobility_apply(prob, pos, force=None, torque=None, want_omega=None, dft="naive", stages=None, timing=None, torque_mode="fourier"):
     """(U, Omega) = M (F, tau): the paper's steps 1-8 in order.
+
+    ``torque_mode``: "fourier" — torques and angular velocities through the curl in Fourier-Chebyshev space (the paper's first
+    way); "kernel" — through the derivative of the ES kernel (its second way: three fields each way).
 
     ``stages`` (dict) receives the intermediate arrays (grid after spread, spectra, ...) when given.
     ``timing`` (dict) receives per-step wall-clock seconds when given.
@@ -231,6 +271,31 @@ def mobility_apply(prob, pos, force=None, torque=None, want_omega=None, dft="nai
     tm = {} if timing is None else timing
     keep = stages is not None
     t0 = time.perf_counter()
+    if torque_mode == "kernel":
+        f = spread(prob, pos, force if force is not None else np.zeros((n, 3)), prob.beta_M)      # step 1
+        if torque is not None:
+            spread_curl(prob, pos, torque, prob.beta_D, f)
+        tm["spread"] = time.perf_counter() - t0; t0 = time.perf_counter()
+        fh = dft_xy_forward(f, dft)                                                                  # step 2 (xy)
+        if keep:
+            stages.update(f=f)
+        del f
+        tm["dft_fwd"] = time.perf_counter() - t0; t0 = time.perf_counter()
+        uh, _, coef = solve(prob, fh, None, want_omega=False, want_coef=keep)                      # steps 2(z)-6
+        if keep:
+            stages.update(fh=fh, ucoef=coef)
+        del fh, coef
+        tm["solve"] = time.perf_counter() - t0; t0 = time.perf_counter()
+        u = dft_xy_inverse(uh, prob.nx, dft)                                                         # step 7
+        if keep:
+            stages.update(uh=uh, u=u)
+        del uh
+        tm["dft_inv"] = time.perf_counter() - t0; t0 = time.perf_counter()
+        U = interp(prob, pos, u, prob.beta_M)                                                        # step 8
+        Om = interp_curl(prob, pos, u, prob.beta_D) if want_omega else None
+        tm["interp"] = time.perf_counter() - t0
+        return U, Om
+    assert torque_mode == "fourier"
     f = spread(prob, pos, force if force is not None else np.zeros((n, 3)), prob.beta_M)          # step 1
     t = spread(prob, pos, torque, prob.beta_D) if torque is not None else None
     tm["spread"] = time.perf_counter() - t0; t0 = time.perf_counter()

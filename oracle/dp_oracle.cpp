@@ -249,6 +249,134 @@ void or_interp(const or_params* P, int n, const double* pos, const double* grid,
     }
 }
 
+// ---- kernel-derivative torque spreading / angular-velocity interpolation (the paper's "second way", PAPER.md:335;
+// footnotes 47, 48; reading G19 in DESIGN.md).  With Delta_D^W the dipole envelope of eqs 9, 53:
+//   f(x_g) += (1/2) curl_x (tau Delta_D^W(x_g - r)) = (1/2) G(x_g) x tau,      G = grad_x Delta_D^W   (eq 7)
+//   Omega   = (1/2) sum_g (u(x_g) x G(x_g)) h^2 (H/2) w_l                       (eq 11 integrated by parts: the adjoint)
+//   G = ( phi'(x) phi(y) zeta(l),  phi(x) phi'(y) zeta(l),  phi(x) phi(y) zeta'(l) ): a different 1-D kernel along each
+//   dimension (footnote 48), zeta'(l; z_p) = d/dz zeta = phi'(z_l - z_p) - phi'(z_l + z_p) - [slit] phi'(z_l - (2H - z_p)),
+//   i.e. the exact z-derivative of eq 9, which makes G vanish with the particle's height ("all components of the mobility
+//   go to zero at a wall", footnote 48; written with the odd kernel phi' evaluated at the mirrored distance this is the
+//   positive image sign of that footnote).
+// phi'(s) = -(beta s / alpha^2) phi(s) / sqrt(1 - (s/alpha)^2) is unbounded at |s| -> alpha; footnote 47: it is truncated to zero
+// for |s| beyond the point where |phi'| has its minimum before it blows up.
+
+// The cut u* = |s|/alpha of footnote 47: the stationary point of log|phi'| = beta sqrt(1-u^2) + log u - (1/2) log(1-u^2) nearest the
+// edge, i.e. the root of  F(u) = -beta u/sqrt(1-u^2) + 1/u + u/(1-u^2)  in (sqrt(2/3), 1), by bisection in long double.
+// Exists for beta > 3 sqrt(3)/2; returns NaN otherwise.
+double or_es_dphi_cut(double beta) {
+    if (!(beta > 2.5980762113533160L)) return NAN;
+    auto F = [&](ld u) { ld q = 1 - u * u; return -(ld)beta * u / sqrtl(q) + 1 / u + u / q; };
+    ld lo = sqrtl(2.0L / 3.0L), hi = 1 - 1e-18L;
+    for (int it = 0; it < 200; ++it) {
+        ld mid = 0.5L * (lo + hi);
+        if (F(mid) < 0) lo = mid; else hi = mid;
+    }
+    return (double)(0.5L * (lo + hi));
+}
+
+// truncated derivative of eq 54's kernel (footnote 47); ucut from or_es_dphi_cut
+double or_es_dphi(double s, double alpha, double beta, double Z, double ucut) {
+    double q = s / alpha;
+    if (fabs(q) > ucut) return 0.0;
+    double r = 1.0 - q * q;
+    return -(beta * s / (alpha * alpha)) * exp(beta * (sqrt(r) - 1.0)) / (sqrt(r) * Z);
+}
+
+}  // extern "C"
+
+struct GradFootprint {
+    Footprint fp;                          // phi(x), phi(y), zeta(l) of the dipole envelope
+    std::vector<double> dpx, dpy, dzeta;   // phi'(x), phi'(y), zeta'(l)
+};
+
+static void grad_footprint(const or_params& P, double beta, double Z, double ucut, const double* z_nodes, const double* r, GradFootprint& g) {
+    footprint(P, beta, Z, z_nodes, r, g.fp);
+    double h = P.Lx / P.nx, alpha = 0.5 * P.w * h;
+    double xw = wrap(r[0], P.Lx), yw = wrap(r[1], P.Ly);
+    g.dpx.resize(P.w); g.dpy.resize(P.w); g.dzeta.resize(P.nz);
+    for (int a = 0; a < P.w; ++a) {
+        g.dpx[a] = or_es_dphi((g.fp.i0 + a) * h - xw, alpha, beta, Z, ucut);
+        g.dpy[a] = or_es_dphi((g.fp.j0 + a) * h - yw, alpha, beta, Z, ucut);
+    }
+    double zp = r[2];
+    for (int l = 0; l < P.nz; ++l) {
+        double v = or_es_dphi(z_nodes[l] - zp, alpha, beta, Z, ucut) - or_es_dphi(z_nodes[l] + zp, alpha, beta, Z, ucut);
+        if (P.wall_mode == 1) v -= or_es_dphi(z_nodes[l] - (2.0 * P.H - zp), alpha, beta, Z, ucut);
+        g.dzeta[l] = v;
+    }
+}
+
+extern "C" {
+
+// grid[c][l][j][i] += (1/2) (G(p; i, j, l) x tau_p)_c   — ADDS to grid (the force field of or_spread is already there)
+void or_spread_curl(const or_params* P, int n, const double* pos, const double* tau, double beta, double* grid) {
+    size_t plane = (size_t)P->nx * P->ny, field = plane * P->nz;
+    double h = P->Lx / P->nx, alpha = 0.5 * P->w * h;
+    double Z = or_es_norm(alpha, beta), ucut = or_es_dphi_cut(beta);
+    std::vector<double> zn(P->nz);
+    or_cheb_nodes(P->nz, P->H, zn.data());
+    GradFootprint g;
+    for (int p = 0; p < n; ++p) {
+        grad_footprint(*P, beta, Z, ucut, zn.data(), pos + 3 * (size_t)p, g);
+        const double* t = tau + 3 * (size_t)p;
+        for (int l = 0; l < P->nz; ++l) {
+            if (g.fp.zeta[l] == 0.0 && g.dzeta[l] == 0.0) continue;
+            for (int b = 0; b < P->w; ++b) {
+                int j = pmod(g.fp.j0 + b, P->ny);
+                for (int a = 0; a < P->w; ++a) {
+                    int i = pmod(g.fp.i0 + a, P->nx);
+                    double Gx = g.dpx[a] * g.fp.py[b] * g.fp.zeta[l];
+                    double Gy = g.fp.px[a] * g.dpy[b] * g.fp.zeta[l];
+                    double Gz = g.fp.px[a] * g.fp.py[b] * g.dzeta[l];
+                    size_t o = l * plane + (size_t)j * P->nx + i;
+                    grid[0 * field + o] += 0.5 * (Gy * t[2] - Gz * t[1]);
+                    grid[1 * field + o] += 0.5 * (Gz * t[0] - Gx * t[2]);
+                    grid[2 * field + o] += 0.5 * (Gx * t[1] - Gy * t[0]);
+                }
+            }
+        }
+    }
+}
+
+// out[p] = (1/2) sum_{i,j,l} (u(i,j,l) x G(p; i, j, l)) h^2 (H/2) w_l,   u = grid[0..2]
+void or_interp_curl(const or_params* P, int n, const double* pos, const double* grid, double beta, double* out) {
+    size_t plane = (size_t)P->nx * P->ny, field = plane * P->nz;
+    double h = P->Lx / P->nx, alpha = 0.5 * P->w * h;
+    double Z = or_es_norm(alpha, beta), ucut = or_es_dphi_cut(beta);
+    std::vector<double> zn(P->nz), wq(P->nz);
+    or_cheb_nodes(P->nz, P->H, zn.data());
+    or_cc_weights(P->nz, wq.data());
+#pragma omp parallel
+    {
+        GradFootprint g;
+#pragma omp for schedule(static)
+        for (int p = 0; p < n; ++p) {
+            grad_footprint(*P, beta, Z, ucut, zn.data(), pos + 3 * (size_t)p, g);
+            double s[3] = {0, 0, 0};
+            for (int l = 0; l < P->nz; ++l) {
+                if (g.fp.zeta[l] == 0.0 && g.dzeta[l] == 0.0) continue;
+                double wl = h * h * (0.5 * P->H) * wq[l];
+                for (int b = 0; b < P->w; ++b) {
+                    int j = pmod(g.fp.j0 + b, P->ny);
+                    for (int a = 0; a < P->w; ++a) {
+                        int i = pmod(g.fp.i0 + a, P->nx);
+                        double Gx = g.dpx[a] * g.fp.py[b] * g.fp.zeta[l];
+                        double Gy = g.fp.px[a] * g.dpy[b] * g.fp.zeta[l];
+                        double Gz = g.fp.px[a] * g.fp.py[b] * g.dzeta[l];
+                        size_t o = l * plane + (size_t)j * P->nx + i;
+                        double u = grid[0 * field + o], v = grid[1 * field + o], w = grid[2 * field + o];
+                        s[0] += 0.5 * (v * Gz - w * Gy) * wl;
+                        s[1] += 0.5 * (w * Gx - u * Gz) * wl;
+                        s[2] += 0.5 * (u * Gy - v * Gx) * wl;
+                    }
+                }
+            }
+            for (int c = 0; c < 3; ++c) out[3 * (size_t)p + c] = s[c];
+        }
+    }
+}
+
 // O2: unnormalised forward DFT in x,y of nplanes real planes [j][i] -> half spectrum [ny][nkx]
 //   f^(n_x, n_y) = sum_{i,j} f(i,j) exp(-2 pi i (n_x i/nx + n_y j/ny)),  n_x = 0..nx/2, n_y = 0..ny-1
 // written as the two nested 1-D sums (x then y).  Explicit O(n^2) per line.
