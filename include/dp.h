@@ -73,6 +73,13 @@ typedef struct {
                            forward transforms are identically zero; the product finds the highest touched plane while
                            binning and skips the spreading stores, forward FFT passes and solve loads of the planes above
                            it (exact: the skipped values are zeros).  1: treat every plane as dense.                        */
+  int torque_mode;      /* how torques enter and Omega leaves.  0: the paper's "first way" — tau is spread as a second
+                           field triple, (1/2) curl in Fourier-Chebyshev space, (1/2) curl u transformed back as a second triple
+                           (6 grid fields each way);  1: its "second way" — the derivative of the ES kernel spreads
+                           (1/2) curl (tau Delta_D^W) into the force field and gathers Omega = (1/2) int (u x grad Delta_D^W) from u
+                           itself (3 fields each way; truncated phi', one kernel per dimension, footnotes 47-48, PAPER.md:797-798;
+                           DESIGN.md reading G19).  The two discretisations agree to the method's 2-3 digits, not to roundoff;
+                           mode 1 needs beta_D > 3 sqrt(3)/2.  Ignored when use_torques = 0.                                     */
 } dp_params;
 
 /* Plan creation for the problem of PAPER.md:74 (box, walls) with the grid of PAPER.md:319 and the ES kernel of eq 54.
@@ -136,6 +143,8 @@ int dp_fft_backend(const dp_plan* plan);       /* 0: own shared-memory FFT passe
 double dp_es_norm(double alpha, double beta);                  /* Z of eq 54, Gauss-Legendre on the host */
 double dp_es_radius_over_h(int w, double beta, int dipole);    /* c(beta) = R_h/h of eq 56 for support w and this
                                                                   beta: what dp_effective_radius divides by h; needs no plan  */
+double dp_es_dphi_cut(double beta);                            /* |s|/alpha beyond which the kernel derivative of torque_mode = 1 is
+                                                                  truncated to zero (footnote 47); < 0: none exists */
 int dp_supported_nz(int* out, int cap);                        /* Chebyshev sizes with a compiled solve kernel; returns how many */
 size_t dp_device_bytes(const dp_plan* plan);                   /* device memory owned by the plan                     */
 const char* dp_strerror(int code);

@@ -15,7 +15,7 @@ _LIBNAME = os.path.join(_HERE, "libdpstokes.so")
 # every symbol include/dp.h declares
 EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_check", "dp_effective_radius", "dp_set_profiling", "dp_stage_ms",
            "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_copy_plane_to_host", "dp_complex_row_pitch", "dp_zero_planes", "dp_fft_backend", "dp_es_norm", "dp_es_radius_over_h",
-           "dp_supported_nz", "dp_device_bytes", "dp_strerror", "dp_last_error", "dp_destroy"]
+           "dp_es_dphi_cut", "dp_supported_nz", "dp_device_bytes", "dp_strerror", "dp_last_error", "dp_destroy"]
 
 
 class DPError(RuntimeError):
@@ -28,7 +28,7 @@ class dp_params(ctypes.Structure):
                 ("beta_M", ctypes.c_double), ("beta_D", ctypes.c_double), ("a", ctypes.c_double), ("eta", ctypes.c_double),
                 ("max_particles", ctypes.c_int), ("transfer_fp32", ctypes.c_int), ("device", ctypes.c_int),
                 # extensions beyond SURVEY.md §8(b)
-                ("use_torques", ctypes.c_int), ("fft_backend", ctypes.c_int), ("dense_planes", ctypes.c_int)]
+                ("use_torques", ctypes.c_int), ("fft_backend", ctypes.c_int), ("dense_planes", ctypes.c_int), ("torque_mode", ctypes.c_int)]
 
 
 _lib = None
@@ -80,6 +80,8 @@ def load_library():
     L.dp_es_norm.restype = d
     L.dp_es_radius_over_h.argtypes = [i, d, i]
     L.dp_es_radius_over_h.restype = d
+    L.dp_es_dphi_cut.argtypes = [d]
+    L.dp_es_dphi_cut.restype = d
     L.dp_supported_nz.argtypes = [ctypes.POINTER(i), i]
     L.dp_supported_nz.restype = i
     L.dp_device_bytes.argtypes = [vp]
@@ -103,6 +105,10 @@ def es_norm(alpha: float, beta: float) -> float:
     return float(load_library().dp_es_norm(alpha, beta))
 
 
+def es_dphi_cut(beta: float) -> float:
+    return float(load_library().dp_es_dphi_cut(beta))
+
+
 def supported_nz():
     buf = (ctypes.c_int * 16)()
     n = load_library().dp_supported_nz(buf, 16)
@@ -116,7 +122,7 @@ class Plan:
     """dp_create / dp_mobility_apply / dp_destroy.  ``prob`` is any object with the fields of ``workloads.Problem``."""
 
     def __init__(self, prob, max_particles: int, use_torques=None, device: int = 0, fft_backend: int = 0, transfer_fp32: bool = False,
-                 dense_planes: bool = False):
+                 dense_planes: bool = False, torque_mode: int = 0):
         self._h = None
         L = load_library()
         if use_torques is None:
@@ -124,14 +130,15 @@ class Plan:
         self.params = dp_params(int(prob.wall_mode), float(prob.Lx), float(prob.Ly), float(prob.H), int(prob.nx), int(prob.ny),
                                 int(prob.nz), int(prob.w), float(prob.beta_M), float(prob.beta_D), float(getattr(prob, "a", 1.0)),
                                 float(prob.eta), int(max_particles), int(bool(transfer_fp32)), int(device),
-                                int(bool(use_torques)), int(fft_backend), int(bool(dense_planes)))
+                                int(bool(use_torques)), int(fft_backend), int(bool(dense_planes)), int(torque_mode))
         h = ctypes.c_void_p()
         rc = L.dp_create(ctypes.byref(self.params), ctypes.byref(h))
         if rc != 0:
             raise DPError("dp_create failed: %s (%d)" % (L.dp_strerror(rc).decode(), rc))
         self._h = h
         self.use_torques = bool(use_torques)
-        self.fields = 6 if use_torques else 3
+        self.torque_mode = int(torque_mode)
+        self.fields = 6 if (use_torques and not torque_mode) else 3
         self.device = device
 
     # -- lifetime

@@ -28,7 +28,11 @@ struct dp_plan {
   // derived
   double h, alpha, ZM, ZD;      // grid spacing, ES half support, ES normalisations (eq 54)
   int nkx, nkxp;                // nx/2+1 and its padded row pitch (complex elements)
-  int fields;                   // 3 or 6
+  int fields;                   // grid fields each way: 6 with torques through the Fourier-Chebyshev curl, else 3
+  bool torques = false;         // torques in / Omega out allowed (dp_params.use_torques)
+  bool kernel_torque = false;   // torques through the derivative of the ES kernel (dp_params.torque_mode = 1): 3 fields
+  int nrec = 1;                 // weight records per particle: Delta_M [, Delta_D [, derivatives of Delta_D]]
+  double ucutD = 1.0;           // |s|/alpha beyond which phi_D' is truncated to zero (footnote 47)
   int nbx, nby, nbins;          // spread tiles / particle bins
   size_t real_field, cplx_field;  // elements per field: nz*ny*nx doubles, nz*ny*nkxp double2
 
@@ -45,7 +49,7 @@ struct dp_plan {
   double* d_trq_s = nullptr;    // [n][3]
   int* d_perm = nullptr;        // sorted slot -> original index
   int4* d_meta = nullptr;       // sorted footprint records: wrapped origin node (i0, j0), plane range [lmin, lmax]
-  double* d_wrec = nullptr;     // sorted 1-D ES weight records [2][max_particles][16 + nz] (transfer.cu)
+  double* d_wrec = nullptr;     // sorted 1-D ES weight records [nrec][max_particles][16 + nz] (transfer.cu)
   int* d_bin_of = nullptr;      // per particle
   int* d_slot_of = nullptr;     // rank within its bin
   int* d_bin_count = nullptr;   // [nbins]

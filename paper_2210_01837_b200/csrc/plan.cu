@@ -138,6 +138,23 @@ double es_radius_over_h(int w, double beta, bool dipole) {
   return (double)(1 / (6 * PI_LD * (2.0L / 3.0L) * integ));
 }
 
+// Truncation point of the ES kernel's derivative (footnote 47): |phi'(s)| ~ e^{beta c} sqrt(1 - c^2)/c with
+// c = sqrt(1 - (s/alpha)^2) is stationary where c (1 - c^2) = 1/beta; of the two roots in (0, 1) the smaller one is the minimum
+// of |phi'| next to the edge of the support, beyond which the derivative blows up.  Newton from c = 1/beta; returns
+// u = |s|/alpha = sqrt(1 - c^2), or a negative number when beta <= 3 sqrt(3)/2 (no interior minimum).
+double es_dphi_cut_host(double beta) {
+  if (!(beta > 2.598076211353316)) return -1.0;
+  const ld rhs = 1 / (ld)beta;
+  ld c = rhs;
+  for (int it = 0; it < 100; ++it) {
+    const ld f = c - c * c * c - rhs, df = 1 - 3 * c * c;
+    const ld dc = f / df;
+    c -= dc;
+    if (fabsl(dc) < 1e-21L) break;
+  }
+  return (double)sqrtl((1 - c) * (1 + c));
+}
+
 void set_err(dp_plan* P, const char* what, const char* detail) {
   if (P) P->last_error = std::string(what) + ": " + (detail ? detail : "");
 }
@@ -198,7 +215,9 @@ int make_fft(dp_plan* P) {
 int run_pipeline(dp_plan* P, int n, const double* pos, const double* force, const double* torque, double* U, double* Omega,
                  cudaStream_t st, int last_stage) {
   const bool with_torque = torque != nullptr;
-  const bool want_omega = Omega != nullptr || (last_stage < 5 && P->fields == 6 && last_stage >= 3);
+  // kernel-derivative torque mode: torques ride in the force field and Omega is gathered from u: three fields throughout
+  const bool torque_field = with_torque && !P->kernel_torque;
+  const bool want_omega = !P->kernel_torque && (Omega != nullptr || (last_stage < 5 && P->fields == 6 && last_stage >= 3));
   const bool prof = P->profiling && P->ev_ok;
   P->last_stream = st;
   P->ev_recorded = false;
@@ -212,15 +231,15 @@ int run_pipeline(dp_plan* P, int n, const double* pos, const double* force, cons
   if (prof) CK(cudaEventRecord(P->ev[2], st));
   if (last_stage >= 2) {
     if (P->own_fft) {
-      CK(dp_fft_own_forward(P, with_torque ? 6 : 3, st));
+      CK(dp_fft_own_forward(P, torque_field ? 6 : 3, st));
     } else {
       CKF(cufftSetStream(P->fft_fwd, st));
       CKF(cufftExecD2Z(P->fft_fwd, P->d_real, (cufftDoubleComplex*)P->d_cplx));
-      if (with_torque) CKF(cufftExecD2Z(P->fft_fwd, P->d_real + 3 * P->real_field, (cufftDoubleComplex*)(P->d_cplx + 3 * P->cplx_field)));
+      if (torque_field) CKF(cufftExecD2Z(P->fft_fwd, P->d_real + 3 * P->real_field, (cufftDoubleComplex*)(P->d_cplx + 3 * P->cplx_field)));
     }
   }
   if (prof) CK(cudaEventRecord(P->ev[3], st));
-  if (last_stage >= 3) CK(dp_launch_solve(P, with_torque, want_omega, st));
+  if (last_stage >= 3) CK(dp_launch_solve(P, torque_field, want_omega, st));
   if (prof) CK(cudaEventRecord(P->ev[4], st));
   if (last_stage >= 4) {
     if (P->own_fft) {
@@ -243,7 +262,7 @@ int check_apply_args(dp_plan* P, int n, const double* pos, const double* force, 
   if (n == 0) return DP_OK;                      // nothing to do; pointers of empty arrays may legitimately be NULL
   if (n > 0 && (!pos || !U)) { set_err(P, "dp_mobility_apply", "pos and U are required"); return DP_EINVAL; }
   if (!force && !torque) { set_err(P, "dp_mobility_apply", "force and torque both NULL"); return DP_EINVAL; }
-  if ((torque || Omega) && P->fields != 6) { set_err(P, "dp_mobility_apply", "plan created with use_torques = 0"); return DP_EINVAL; }
+  if ((torque || Omega) && !P->torques) { set_err(P, "dp_mobility_apply", "plan created with use_torques = 0"); return DP_EINVAL; }
   return DP_OK;
 }
 
@@ -272,6 +291,8 @@ double dp_es_radius_over_h(int w, double beta, int dipole) {
 }
 
 int dp_supported_nz(int* out, int cap) { return dp_solve_nz_list(out, cap); }
+
+double dp_es_dphi_cut(double beta) { return es_dphi_cut_host(beta); }
 
 const char* dp_strerror(int code) {
   switch (code) {
@@ -326,6 +347,8 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   if (p.fft_backend != 0 && p.fft_backend != 1) return DP_EINVAL;
   if (p.transfer_fp32 != 0 && p.transfer_fp32 != 1) return DP_EINVAL;
   if (p.dense_planes != 0 && p.dense_planes != 1) return DP_EINVAL;
+  if (p.torque_mode != 0 && p.torque_mode != 1) return DP_EINVAL;
+  if (p.use_torques && p.torque_mode == 1 && es_dphi_cut_host(p.beta_D) < 0) return DP_EINVAL;   // phi' has no minimum to truncate at
   if (p.transfer_fp32 && !(p.fft_backend == 0 && dp_fft_own_supported(p.nx, p.ny))) return DP_EINVAL;   // fp32 grids are read by the own x passes only
   if (p.wall_mode == DP_SLIT && p.w * hx > p.H) return DP_EINVAL;     // a kernel may overlap one wall, not both
   if ((double)p.nz * p.ny * (p.nx + 16) >= 2.0e9) return DP_EINVAL;    // 32-bit plane indexing inside the kernels
@@ -339,7 +362,11 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   P->ZD = p.use_torques ? es_norm_host(P->alpha, p.beta_D) : 1.0;
   P->nkx = p.nx / 2 + 1;
   P->nkxp = (P->nkx + 7) / 8 * 8;
-  P->fields = p.use_torques ? 6 : 3;
+  P->torques = p.use_torques != 0;
+  P->kernel_torque = P->torques && p.torque_mode == 1;
+  P->fields = (P->torques && !P->kernel_torque) ? 6 : 3;
+  P->nrec = P->torques ? (P->kernel_torque ? 3 : 2) : 1;
+  P->ucutD = P->kernel_torque ? es_dphi_cut_host(p.beta_D) : 1.0;
   P->nbx = (p.nx + DP_TILE_X - 1) / DP_TILE_X;
   P->nby = (p.ny + DP_TILE_Y - 1) / DP_TILE_Y;
   P->nbins = P->nbx * P->nby;
@@ -362,7 +389,7 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   if (p.use_torques) TRY(dev_alloc(P, &P->d_trq_s, 3 * np));
   TRY(dev_alloc(P, &P->d_perm, np));
   TRY(dev_alloc(P, &P->d_meta, np));
-  TRY(dev_alloc(P, &P->d_wrec, np * (p.use_torques ? 2 : 1) * (2 * DP_MAX_W + p.nz)));
+  TRY(dev_alloc(P, &P->d_wrec, np * P->nrec * (2 * DP_MAX_W + p.nz)));
   TRY(dev_alloc(P, &P->d_bin_of, np));
   TRY(dev_alloc(P, &P->d_slot_of, np));
   TRY(dev_alloc(P, &P->d_bin_count, (size_t)P->nbins));
@@ -547,7 +574,7 @@ extern "C" int dp_copy_plane_to_host(dp_plan* P, int which, int field, int l, vo
 
 extern "C" double dp_effective_radius(const dp_plan* P, int dipole) {
   if (!P || (dipole != 0 && dipole != 1)) return -1.0;
-  if (dipole && P->fields != 6) return -1.0;
+  if (dipole && !P->torques) return -1.0;
   return P->h * es_radius_over_h(P->p.w, dipole ? P->p.beta_D : P->p.beta_M, dipole != 0);
 }
 
@@ -563,7 +590,7 @@ extern "C" int dp_mobility_apply_host(dp_plan* P, int n, const double* pos, cons
     dp_host_stage* fresh = new (std::nothrow) dp_host_stage();
     if (!fresh) return DP_ENOMEM;
     const size_t bytes = sizeof(double) * 3 * (size_t)P->p.max_particles;
-    const int nbuf = P->fields == 6 ? 5 : 3;
+    const int nbuf = P->torques ? 5 : 3;
     double** slots[5] = {&fresh->pos, &fresh->frc, &fresh->U, &fresh->trq, &fresh->Om};
     cudaError_t e = cudaSuccess;
     for (int i = 0; i < nbuf && e == cudaSuccess; ++i) e = cudaMalloc((void**)slots[i], bytes);

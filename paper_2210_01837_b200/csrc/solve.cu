@@ -65,7 +65,7 @@ DP_SOLVE_NZ_LIST(X)
 // even coefficients n = 2j and odd coefficients n = 2j+1, all padded to LP = a multiple of 8; KB k-blocks of 4, MB m-blocks of 8.
 // Fragment table (global, per plan): [4 kinds][MB][KB][32 lanes]; kind 0, 1: analysis even / odd, 2, 3: synthesis even / odd.
 template <int NZ> struct Tr {
-  static constexpr int N = NZ - 1, NP = (NZ + 1) / 2, LP = (NP + 7) / 8 * 8, KB = LP / 4, MB = LP / 8, FRAGS = 4 * MB * KB;
+  static constexpr int NP = (NZ + 1) / 2, LP = (NP + 7) / 8 * 8, KB = LP / 4, MB = LP / 8, FRAGS = 4 * MB * KB;
 };
 
 struct SolveArgs {

@@ -4,6 +4,11 @@
 //   Delta^W = phi(x)phi(y)[phi(z - z_j) - phi(z + z_j) - (slit) phi(z - (2H - z_j))]
 // Step 8 (eqs 10, 11): U_j = sum_g u(x_g) Delta_M^W(x_g - r_j) h^2 (H/2) w_l, Omega_j likewise with Delta_D^W.
 //
+// Kernel-derivative torque mode (dp_params.torque_mode = 1; the paper's "second way", footnotes 47-48): the torques
+// are spread into the SAME three fields as the forces, f += (1/2) G x tau with G = grad_x Delta_D^W =
+// (phi'(x)phi(y)zeta(l), phi(x)phi'(y)zeta(l), phi(x)phi(y)zeta'(l)), and Omega_j = (1/2) sum_g (u(x_g) x G(x_g)) h^2 (H/2) w_l is
+// gathered from the velocity field itself (eq 11 integrated by parts), so only three fields are transformed each way.
+//
 // B200 design: particles are counting-sorted by the xy tile (16 x 4 grid columns) that contains the origin of
 // their w x w footprint.  One CTA owns one tile of one field triple and gathers every footprint that touches it into
 // per-thread register accumulators (each thread owns one column and a fixed residue class of the plane index, so no
@@ -58,6 +63,21 @@ __device__ __forceinline__ double es_phi(double s, double inv_alpha, double beta
 __device__ __forceinline__ double zeta_weight(double zl, double zp, double H, int wall_mode, double inv_alpha, double beta, double inv_Z) {
   double v = es_phi(zl - zp, inv_alpha, beta, inv_Z) - es_phi(zl + zp, inv_alpha, beta, inv_Z);
   if (wall_mode == DP_SLIT) v -= es_phi(zl - (2.0 * H - zp), inv_alpha, beta, inv_Z);
+  return v;
+}
+// truncated derivative of eq 54's kernel (footnote 47): phi'(s) = -(beta s/alpha^2) phi(s)/sqrt(1-(s/alpha)^2) for
+// |s| <= ucut alpha, 0 beyond (ucut: where |phi'| is smallest before it blows up at the edge of the support, see plan.cu)
+__device__ __forceinline__ double es_dphi(double s, double inv_alpha, double beta, double inv_Z, double ucut) {
+  const double q = s * inv_alpha;
+  if (!(fabs(q) <= ucut)) return 0.0;
+  const double sr = sqrt(1.0 - q * q);
+  return -(beta * q * inv_alpha) * exp(beta * (sr - 1.0)) * inv_Z / sr;
+}
+// zeta'(l; z_p) = d/dz [phi(z - z_p) - phi(z + z_p) - [slit] phi(z - (2H - z_p))] at z = z_l: the exact z-derivative of eq 9,
+// which vanishes with the particle's height (footnote 48; reading G19)
+__device__ __forceinline__ double dzeta_weight(double zl, double zp, double H, int wall_mode, double inv_alpha, double beta, double inv_Z, double ucut) {
+  double v = es_dphi(zl - zp, inv_alpha, beta, inv_Z, ucut) - es_dphi(zl + zp, inv_alpha, beta, inv_Z, ucut);
+  if (wall_mode == DP_SLIT) v -= es_dphi(zl - (2.0 * H - zp), inv_alpha, beta, inv_Z, ucut);
   return v;
 }
 // node range with z_l in [max(0, zp - alpha), min(H, zp + alpha)] (nodes decrease with l); covers every image term
@@ -151,7 +171,8 @@ __global__ void k_bin_scatter(int n, const double* __restrict__ pos, const doubl
 }
 
 // ---------------------------------------------------------------------------------------------- 1-D ES weights
-// One record per particle and envelope (0: Delta_M, 1: Delta_D), in sorted order, evaluated once per product and used by
+// One record per particle and envelope (0: Delta_M, 1: Delta_D, 2 (kernel-derivative torque mode): the derivatives of record 1,
+// phi'(x), phi'(y), zeta'(l)), in sorted order, evaluated once per product and used by
 // both spreading and interpolation:  rec[0..7] = phi(x_{i0+a} - x), rec[8..15] = phi(y_{j0+b} - y), rec[16+l] = zeta(l; z)
 // (eqs 9, 54).  One thread per record entry.
 struct WeightArgs {
@@ -159,8 +180,9 @@ struct WeightArgs {
   const double* pos_s;
   const int4* meta;
   const double* znodes;
-  double beta[2], Z[2];
-  double* wrec;              // [2][cap][16 + nz]
+  double beta[3], Z[3];      // record 2 uses the dipole envelope's beta and Z
+  double ucut;               // truncation point of phi' (record 2)
+  double* wrec;              // [nrec][cap][16 + nz]
   size_t cap;
 };
 
@@ -178,10 +200,14 @@ __global__ void k_weights(int n, WeightArgs A) {
       const int a = rr & (DP_MAX_W - 1);
       const double xw = A.pos_s[3 * (size_t)p + (rr >= DP_MAX_W ? 1 : 0)];
       const double i0 = ceil((xw - g.alpha) / g.h);            // unwrapped origin: distances use the unwrapped node
-      if (a < g.w) v = es_phi((i0 + a) * g.h - xw, inv_alpha, beta, inv_Z);
+      if (a < g.w) v = k < 2 ? es_phi((i0 + a) * g.h - xw, inv_alpha, beta, inv_Z) : es_dphi((i0 + a) * g.h - xw, inv_alpha, beta, inv_Z, A.ucut);
     } else {
       const int l = rr - 2 * DP_MAX_W;
-      if (l >= m.z && l <= m.w) v = zeta_weight(A.znodes[l], A.pos_s[3 * (size_t)p + 2], g.H, g.wall_mode, inv_alpha, beta, inv_Z);
+      if (l >= m.z && l <= m.w) {
+        const double zp = A.pos_s[3 * (size_t)p + 2];
+        v = k < 2 ? zeta_weight(A.znodes[l], zp, g.H, g.wall_mode, inv_alpha, beta, inv_Z)
+                  : dzeta_weight(A.znodes[l], zp, g.H, g.wall_mode, inv_alpha, beta, inv_Z, A.ucut);
+      }
     }
   }
   A.wrec[((size_t)k * A.cap + p) * wrec + rr] = v;
@@ -209,14 +235,21 @@ struct SpreadArgs {
 // segments per warp).  Dependent global round trips per CTA: bin_start -> candidate records -> stores.
 // GT = double, or float for the optional fp32 variant (accumulators and grid in fp32; the weight records stay fp64 and are
 // rounded when they are used).
-template <int NZ, class GT>
+// MODE 0: field triple blockIdx.z (0: forces with Delta_M, 1: torques with Delta_D) gets sum_j val_j S(j; g)   (eq 7 without the curl,
+//         which the solve kernel takes in Fourier-Chebyshev space);
+// MODE 1 (kernel-derivative torques): ONE triple f = sum_j [F_j S_M(j; g) + (1/2) G_j(g) x tau_j], three records per candidate.
+template <int NZ, class GT, int MODE>
 __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(SpreadArgs A) {
-  constexpr int NL = NZ / ZSPLIT;
-  constexpr int WREC = 2 * DP_MAX_W + NZ;
-  __shared__ double s_w[PCH][WREC];
-  __shared__ double s_val[PCH][3];
-  __shared__ int4 s_meta[PCH];                // i0, j0 (wrapped origin node), lmin, lmax
-  __shared__ int s_src[PCH];                  // index of each staged candidate in the sorted particle arrays
+  constexpr int NL = (NZ + ZSPLIT - 1) / ZSPLIT;
+  constexpr int WREC = 2 * DP_MAX_W + NZ;                 // record length in global memory
+  constexpr int WS = 2 * DP_MAX_W + NL * ZSPLIT;          // staged record length (zero padded to whole z residue classes)
+  constexpr int NREC = MODE ? 3 : 1;
+  constexpr int PC = MODE ? PCH / 2 : PCH;                // candidates per chunk
+  constexpr int NV = MODE ? 6 : 3;
+  __shared__ double s_w[PC][NREC][WS];
+  __shared__ double s_val[PC][NV];
+  __shared__ int4 s_meta[PC];                 // i0, j0 (wrapped origin node), lmin, lmax
+  __shared__ int s_src[PC];                   // index of each staged candidate in the sorted particle arrays
   __shared__ int s_rbeg[MAXR], s_roff[MAXR + 1];   // candidate ranges in the sorted arrays; prefix sums of their lengths
 
   const GridGeom& g = A.g;
@@ -227,8 +260,6 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
   const int ti = t % TX, tj = (t / TX) % TY, tz = t / (TX * TY);
   const int gi = X0 + ti, gj = Y0 + tj;
   const bool in_grid = gi < g.nx && gj < g.ny;
-  const double* __restrict__ val = A.val_s[grp];
-  const double* __restrict__ wrec = A.wrec + (size_t)grp * A.cap * WREC;
 
   GT acc[NL][3];
 #pragma unroll
@@ -263,8 +294,8 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
 
   // Every candidate is staged (no cull pass: the candidates of a range are contiguous, so their records arrive in one
   // batch of independent coalesced loads); the exact footprint test happens per thread in the accumulation loop.
-  for (int c0 = 0; c0 < total; c0 += PCH) {
-    const int nl = min(PCH, total - c0);
+  for (int c0 = 0; c0 < total; c0 += PC) {
+    const int nl = min(PC, total - c0);
     if (t < nl) {                                             // position of candidate c0 + t in the sorted arrays, once
       const int c = c0 + t;
       int r = 0;
@@ -276,12 +307,19 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
     if (t < nl) {
       const int p = s_src[t];
       s_meta[t] = A.meta[p];
-      s_val[t][0] = val[3 * (size_t)p]; s_val[t][1] = val[3 * (size_t)p + 1]; s_val[t][2] = val[3 * (size_t)p + 2];
+      if (MODE) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { s_val[t][c] = A.val_s[0][3 * (size_t)p + c]; s_val[t][3 + c] = A.val_s[1][3 * (size_t)p + c]; }
+      } else {
+        const double* __restrict__ val = A.val_s[grp];
+        s_val[t][0] = val[3 * (size_t)p]; s_val[t][1] = val[3 * (size_t)p + 1]; s_val[t][2] = val[3 * (size_t)p + 2];
+      }
     }
 #pragma unroll 2
-    for (int i = t; i < nl * WREC; i += SPREAD_THREADS) {
-      const int q = i / WREC, e = i - q * WREC;
-      s_w[q][e] = wrec[(size_t)s_src[q] * WREC + e];
+    for (int i = t; i < nl * NREC * WS; i += SPREAD_THREADS) {
+      const int q = i / (NREC * WS), rem = i - q * (NREC * WS), k = rem / WS, e = rem - k * WS;
+      const int kk = MODE ? k : grp;
+      s_w[q][k][e] = e < WREC ? A.wrec[((size_t)kk * A.cap + s_src[q]) * WREC + e] : 0.0;
     }
     __syncthreads();
     // ---- accumulate: each thread adds the particles covering its column to its own planes
@@ -291,28 +329,60 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
         int a = gi - m.x; if (a < 0) a += g.nx;
         int bb = gj - m.y; if (bb < 0) bb += g.ny;
         if (a < w && bb < w && m.z <= m.w) {
-          const GT wxy = (GT)s_w[q][a] * (GT)s_w[q][DP_MAX_W + bb];
-          const GT v0 = (GT)s_val[q][0] * wxy, v1 = (GT)s_val[q][1] * wxy, v2 = (GT)s_val[q][2] * wxy;
-          const double* zt = &s_w[q][2 * DP_MAX_W + tz];
-          // zeta vanishes outside [lmin, lmax]: skipping a half of the planes that lies outside is exact
-          if (m.z < ZSPLIT * (NL / 2)) {
+          if (MODE == 0) {
+            const GT wxy = (GT)s_w[q][0][a] * (GT)s_w[q][0][DP_MAX_W + bb];
+            const GT v0 = (GT)s_val[q][0] * wxy, v1 = (GT)s_val[q][1] * wxy, v2 = (GT)s_val[q][2] * wxy;
+            const double* zt = &s_w[q][0][2 * DP_MAX_W + tz];
+            // zeta vanishes outside [lmin, lmax]: skipping a half of the planes that lies outside is exact
+            if (m.z < ZSPLIT * (NL / 2)) {
 #pragma unroll
-            for (int li = 0; li < NL / 2; ++li) {
-              const GT z = (GT)zt[ZSPLIT * li];
-              acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+              for (int li = 0; li < NL / 2; ++li) {
+                const GT z = (GT)zt[ZSPLIT * li];
+                acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+              }
             }
-          }
-          if (m.w >= ZSPLIT * (NL / 2)) {
+            if (m.w >= ZSPLIT * (NL / 2)) {
 #pragma unroll
-            for (int li = NL / 2; li < NL; ++li) {
-              const GT z = (GT)zt[ZSPLIT * li];
-              acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+              for (int li = NL / 2; li < NL; ++li) {
+                const GT z = (GT)zt[ZSPLIT * li];
+                acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+              }
+            }
+          } else {
+            const double* wM = s_w[q][0]; const double* wD = s_w[q][MODE ? 1 : 0]; const double* wG = s_w[q][MODE ? 2 : 0];
+            const GT pM = (GT)wM[a] * (GT)wM[DP_MAX_W + bb];
+            const GT c0 = (GT)s_val[q][0] * pM, c1 = (GT)s_val[q][1] * pM, c2 = (GT)s_val[q][2] * pM;     // x zeta_M(l)
+            const GT tx = (GT)s_val[q][NV - 3], ty = (GT)s_val[q][NV - 2], tzq = (GT)s_val[q][NV - 1];
+            const GT pxy = (GT)wD[a] * (GT)wD[DP_MAX_W + bb];                   // phi(x) phi(y)
+            const GT dxy = (GT)wG[a] * (GT)wD[DP_MAX_W + bb];                   // phi'(x) phi(y)
+            const GT xdy = (GT)wD[a] * (GT)wG[DP_MAX_W + bb];                   // phi(x) phi'(y)
+            // (1/2) G x tau with G = (dxy zeta, xdy zeta, pxy zeta'):  coefficients of zeta_D(l) and of zeta_D'(l)
+            const GT a0 = (GT)0.5 * tzq * xdy, a1 = -(GT)0.5 * tzq * dxy, a2 = (GT)0.5 * (ty * dxy - tx * xdy);
+            const GT b0 = -(GT)0.5 * ty * pxy, b1 = (GT)0.5 * tx * pxy;
+            const double* zm = &wM[2 * DP_MAX_W + tz]; const double* zd = &wD[2 * DP_MAX_W + tz]; const double* zg = &wG[2 * DP_MAX_W + tz];
+            if (m.z < ZSPLIT * (NL / 2)) {
+#pragma unroll
+              for (int li = 0; li < NL / 2; ++li) {
+                const GT zM = (GT)zm[ZSPLIT * li], zD = (GT)zd[ZSPLIT * li], zG = (GT)zg[ZSPLIT * li];
+                acc[li][0] = fma(c0, zM, fma(a0, zD, fma(b0, zG, acc[li][0])));
+                acc[li][1] = fma(c1, zM, fma(a1, zD, fma(b1, zG, acc[li][1])));
+                acc[li][2] = fma(c2, zM, fma(a2, zD, acc[li][2]));
+              }
+            }
+            if (m.w >= ZSPLIT * (NL / 2)) {
+#pragma unroll
+              for (int li = NL / 2; li < NL; ++li) {
+                const GT zM = (GT)zm[ZSPLIT * li], zD = (GT)zd[ZSPLIT * li], zG = (GT)zg[ZSPLIT * li];
+                acc[li][0] = fma(c0, zM, fma(a0, zD, fma(b0, zG, acc[li][0])));
+                acc[li][1] = fma(c1, zM, fma(a1, zD, fma(b1, zG, acc[li][1])));
+                acc[li][2] = fma(c2, zM, fma(a2, zD, acc[li][2]));
+              }
             }
           }
         }
       }
     }
-    if (c0 + PCH < total) __syncthreads();
+    if (c0 + PC < total) __syncthreads();
   }
   // ---- store: every grid value of the planes that can hold force written exactly once
   if (in_grid) {
@@ -320,7 +390,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
 #pragma unroll
     for (int li = 0; li < NL; ++li) {
       const int l = ZSPLIT * li + tz;
-      if (l < lm) continue;
+      if (l < lm || l >= NZ) continue;
       GT* dst = reinterpret_cast<GT*>(A.grid) + (size_t)A.field0[grp] * A.real_field + ((size_t)l * g.ny + gj) * g.nx + gi;
 #pragma unroll
       for (int c = 0; c < 3; ++c) dst[c * A.real_field] = acc[li][c];
@@ -347,9 +417,12 @@ constexpr int INTERP_WARPS = 8;
 // One warp per particle (sorted order, so neighbouring warps gather from neighbouring columns): the lanes sweep the
 // w x w x (lmax-lmin+1) footprint, weights come from the particle's records, the six sums are reduced by shuffles.
 // W = kernel support (compile-time: the footprint index arithmetic of the inner loop then has no integer division)
-template <class GT, int W>
+// MODE 0: U from fields 0-2 with Delta_M, Omega from fields 3-5 (= (1/2) curl u) with Delta_D   (eqs 10, 11);
+// MODE 1 (kernel-derivative torques): U as before, Omega = (1/2) sum_g (u x G) h^2 (H/2) w_l from the SAME three fields.
+template <class GT, int W, int MODE>
 __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs A) {
-  __shared__ double s_w[INTERP_WARPS][2][2 * DP_MAX_W + DP_MAX_NZ];   // per warp, per envelope: wx[8], wy[8], zeta[nz]
+  constexpr int NREC = MODE ? 3 : 2;
+  __shared__ double s_w[INTERP_WARPS][NREC][2 * DP_MAX_W + DP_MAX_NZ];   // per warp, per record: wx[8], wy[8], zeta[nz]
   __shared__ double s_zw[DP_MAX_NZ];
   const GridGeom& g = A.g;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -357,7 +430,7 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs 
   const int nz = g.nz, wrec = 2 * DP_MAX_W + nz;
   for (int i = threadIdx.x; i < nz; i += blockDim.x) s_zw[i] = A.zweights[i];
   __syncthreads();
-  const int nk = A.Omega ? 2 : 1;
+  const int nk = A.Omega ? NREC : 1;
   for (int p = blockIdx.x * INTERP_WARPS + wid; p < n; p += gridDim.x * INTERP_WARPS) {
     const int4 m = A.meta[p];
     const int dst = A.perm[p];
@@ -378,17 +451,35 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs 
         int j = m.y + b; if (j >= g.ny) j -= g.ny;
         const size_t off = ((size_t)l * g.ny + j) * g.nx + i;
         const GT wl = (GT)s_zw[l];
-        for (int k = 0; k < nk; ++k) {
-          const double* sw = s_w[wid][k];
-          const GT wgt = (GT)sw[a] * (GT)sw[DP_MAX_W + b] * (GT)sw[2 * DP_MAX_W + l];
-          const GT* gp = reinterpret_cast<const GT*>(A.grid) + (size_t)(3 * k) * A.real_field + off;
-          s[3 * k + 0] += __ldg(gp) * wgt * wl;
-          s[3 * k + 1] += __ldg(gp + A.real_field) * wgt * wl;
-          s[3 * k + 2] += __ldg(gp + 2 * A.real_field) * wgt * wl;
+        if (MODE == 0) {
+          for (int k = 0; k < nk; ++k) {
+            const double* sw = s_w[wid][k];
+            const GT wgt = (GT)sw[a] * (GT)sw[DP_MAX_W + b] * (GT)sw[2 * DP_MAX_W + l];
+            const GT* gp = reinterpret_cast<const GT*>(A.grid) + (size_t)(3 * k) * A.real_field + off;
+            s[3 * k + 0] += __ldg(gp) * wgt * wl;
+            s[3 * k + 1] += __ldg(gp + A.real_field) * wgt * wl;
+            s[3 * k + 2] += __ldg(gp + 2 * A.real_field) * wgt * wl;
+          }
+        } else {
+          const GT* gp = reinterpret_cast<const GT*>(A.grid) + off;
+          const GT u = __ldg(gp) * wl, v = __ldg(gp + A.real_field) * wl, ww2 = __ldg(gp + 2 * A.real_field) * wl;
+          const double* wM = s_w[wid][0];
+          const GT wgt = (GT)wM[a] * (GT)wM[DP_MAX_W + b] * (GT)wM[2 * DP_MAX_W + l];
+          s[0] += u * wgt; s[1] += v * wgt; s[2] += ww2 * wgt;
+          if (nk > 1) {
+            const double* wD = s_w[wid][MODE ? 1 : 0]; const double* wG = s_w[wid][MODE ? 2 : 0];
+            const GT zD = (GT)wD[2 * DP_MAX_W + l];
+            const GT Gx = (GT)wG[a] * (GT)wD[DP_MAX_W + b] * zD, Gy = (GT)wD[a] * (GT)wG[DP_MAX_W + b] * zD;
+            const GT Gz = (GT)wD[a] * (GT)wD[DP_MAX_W + b] * (GT)wG[2 * DP_MAX_W + l];
+            s[3] += (GT)0.5 * (v * Gz - ww2 * Gy);                       // (1/2) (u x G)
+            s[4] += (GT)0.5 * (ww2 * Gx - u * Gz);
+            s[5] += (GT)0.5 * (u * Gy - v * Gx);
+          }
         }
       }
     }
-    for (int c = 0; c < 3 * nk; ++c)
+    const int nsum = A.Omega ? 6 : 3;
+    for (int c = 0; c < nsum; ++c)
       for (int o = 16; o > 0; o >>= 1) s[c] += __shfl_xor_sync(0xffffffffu, s[c], o);
     if (lane < 3) A.U[3 * (size_t)dst + lane] = (double)(lane == 0 ? s[0] : (lane == 1 ? s[1] : s[2]));
     if (A.Omega && lane >= 3 && lane < 6) A.Omega[3 * (size_t)dst + lane - 3] = (double)(lane == 3 ? s[3] : (lane == 4 ? s[4] : s[5]));
@@ -418,25 +509,27 @@ cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* fo
   k_bin_count<<<B, T, 0, st>>>(n, pos, g, P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_flag);
   k_scan<<<1, 1024, 0, st>>>(P->nbins, P->d_bin_count, P->d_bin_start);
   k_bin_scatter<<<B, T, 0, st>>>(n, pos, force, torque, g, P->d_bin_of, P->d_slot_of, P->d_bin_start, P->d_znodes, P->d_perm, P->d_meta,
-                                P->d_pos_s, P->d_frc_s, P->fields == 6 ? P->d_trq_s : nullptr, P->d_lmin);
+                                P->d_pos_s, P->d_frc_s, P->torques ? P->d_trq_s : nullptr, P->d_lmin);
   if (dense) { e = cudaMemsetAsync(P->d_lmin, 0, sizeof(int), st); if (e != cudaSuccess) return e; }   // every plane is transformed
   return cudaGetLastError();
 }
 
 cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torque, cudaStream_t st) {
   (void)with_force;
-  const int ngroups = with_torque ? 2 : 1;
+  const bool kt = P->kernel_torque;
+  const int ngroups = (with_torque && !kt) ? 2 : 1;
   {
-    // weight records of both envelopes (the dipole records are also needed when only Omega is wanted: always built on 6-field plans)
+    // weight records of every envelope of the plan (the dipole records are also needed when only Omega is wanted)
     WeightArgs W;
     W.g = make_geom(P);
     W.pos_s = P->d_pos_s; W.meta = P->d_meta; W.znodes = P->d_znodes;
-    W.beta[0] = P->p.beta_M; W.beta[1] = P->p.beta_D;
-    W.Z[0] = P->ZM; W.Z[1] = P->ZD;
+    W.beta[0] = P->p.beta_M; W.beta[1] = P->p.beta_D; W.beta[2] = P->p.beta_D;
+    W.Z[0] = P->ZM; W.Z[1] = P->ZD; W.Z[2] = P->ZD;
+    W.ucut = P->ucutD;
     W.wrec = P->d_wrec; W.cap = (size_t)P->p.max_particles;
     const int wrec = 2 * DP_MAX_W + P->p.nz;
     const size_t items = (size_t)n * wrec;
-    dim3 wg((unsigned)((items + 255) / 256), P->fields == 6 ? 2 : 1);
+    dim3 wg((unsigned)((items + 255) / 256), P->nrec);
     k_weights<<<wg, 256, 0, st>>>(n, W);
   }
   SpreadArgs A;
@@ -451,12 +544,16 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
   A.lmin = P->d_lmin;
   dim3 grid(P->nbx, P->nby, ngroups);
   const bool f32 = P->p.transfer_fp32 != 0;
+#define DP_SPREAD_CASE(NZ)                                                                        \
+  case NZ:                                                                                        \
+    if (kt) { if (f32) k_spread<NZ, float, 1><<<grid, SPREAD_THREADS, 0, st>>>(A); else k_spread<NZ, double, 1><<<grid, SPREAD_THREADS, 0, st>>>(A); } \
+    else    { if (f32) k_spread<NZ, float, 0><<<grid, SPREAD_THREADS, 0, st>>>(A); else k_spread<NZ, double, 0><<<grid, SPREAD_THREADS, 0, st>>>(A); } \
+    break;
   switch (P->p.nz) {
-    case 16: if (f32) k_spread<16, float><<<grid, SPREAD_THREADS, 0, st>>>(A); else k_spread<16, double><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
-    case 32: if (f32) k_spread<32, float><<<grid, SPREAD_THREADS, 0, st>>>(A); else k_spread<32, double><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
-    case 48: if (f32) k_spread<48, float><<<grid, SPREAD_THREADS, 0, st>>>(A); else k_spread<48, double><<<grid, SPREAD_THREADS, 0, st>>>(A); break;
+    DP_SPREAD_CASE(16) DP_SPREAD_CASE(19) DP_SPREAD_CASE(24) DP_SPREAD_CASE(26) DP_SPREAD_CASE(32) DP_SPREAD_CASE(40) DP_SPREAD_CASE(48) DP_SPREAD_CASE(64)
     default: return cudaErrorInvalidValue;
   }
+#undef DP_SPREAD_CASE
   return cudaGetLastError();
 }
 
@@ -472,11 +569,11 @@ cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaSt
   const int maxb = 148 * 64;
   if (blocks > maxb) blocks = maxb;
   if (blocks < 1) blocks = 1;
-  const bool f32 = P->p.transfer_fp32 != 0;
+  const bool f32 = P->p.transfer_fp32 != 0, kt = P->kernel_torque;
 #define DP_INTERP_CASE(WW)                                                              \
   case WW:                                                                              \
-    if (f32) k_interp<float, WW><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A);           \
-    else k_interp<double, WW><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A);              \
+    if (kt) { if (f32) k_interp<float, WW, 1><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A); else k_interp<double, WW, 1><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A); } \
+    else    { if (f32) k_interp<float, WW, 0><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A); else k_interp<double, WW, 0><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A); } \
     break;
   switch (P->p.w) {
     DP_INTERP_CASE(4) DP_INTERP_CASE(5) DP_INTERP_CASE(6) DP_INTERP_CASE(7) DP_INTERP_CASE(8)

@@ -363,3 +363,79 @@ def test_skipping_the_zero_planes_is_exact(dp):
     with dp.Plan(prob, max_particles=len(pos), use_torques=True) as plan:
         plan.mobility_apply(*to_dev(pos, F, T))
         assert plan.zero_planes() == 0
+
+
+# ------------------------------------------------------------------------------------------------ kernel-derivative torques
+@pytest.mark.parametrize("case", ["slit", "bw-monolayer", "cfg2"])
+def test_kernel_derivative_torque_mode_matches_the_oracle(dp, case):
+    """dp_params.torque_mode = 1 (footnotes 47-48): torques spread with the ES kernel's derivative into the force field,
+    Omega gathered from u itself; three grid fields each way.  Against the oracle's own kernel-derivative path."""
+    import dataclasses
+    if case == "slit":
+        prob, pos, F, T = workloads.random_slit(n=300, L=32.0, nxy=48, nz=48, H=8.0, seed=78, name="slit-small")
+        pos = pos.copy(); pos[:5, 2] = [0.0, 0.2, 7.9, 8.0, 4.0]            # on and next to both walls
+    elif case == "bw-monolayer":
+        prob, pos, F, T = small_monolayer("bw", 3000, 41)
+    else:
+        prob, pos, F, T = workloads.config(2)
+    st = {}
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", torque_mode="kernel", stages=st)
+    dpos, dF, dT = to_dev(pos, F, T)
+    with dp.Plan(prob, max_particles=len(pos), use_torques=True, torque_mode=1) as plan:
+        assert plan.fields == 3
+        g = plan.debug_stage(dpos, dF, dT, 1)
+        assert g.shape[0] == 3 and rel_l2(g, st["f"]) < 1e-13 and rel_max(g, st["f"]) < 1e-12
+        ur = plan.debug_stage(dpos, dF, dT, 4)
+        assert rel_l2(ur, st["u"]) < 1e-11
+        U, Om = plan.mobility_apply(dpos, dF, dT)
+        U, Om = U.cpu().numpy(), Om.cpu().numpy()
+        assert plan.check() == 0
+        assert rel_l2(np.concatenate([U, Om], axis=1), np.concatenate([U_o, Om_o], axis=1)) < TOL
+        assert rel_l2(U, U_o) < TOL and rel_max(U, U_o) < TOL_MAX
+        assert rel_l2(Om, Om_o) < TOL and rel_max(Om, Om_o) < TOL_MAX
+        # forces only on the same plan; torques only; Omega not wanted
+        U1, _ = plan.mobility_apply(dpos, dF, None, want_omega=False)
+        U1_o, _ = oracle.mobility_apply(prob, pos, F, None, dft="fft", torque_mode="kernel")
+        assert rel_l2(U1.cpu().numpy(), U1_o) < TOL
+        U2, Om2 = plan.mobility_apply(dpos, None, dT)
+        U2_o, Om2_o = oracle.mobility_apply(prob, pos, None, T, dft="fft", torque_mode="kernel")
+        assert rel_l2(U2.cpu().numpy(), U2_o) < TOL and rel_l2(Om2.cpu().numpy(), Om2_o) < TOL
+        Uh, Omh = plan.mobility_apply_host(pos, F, T)
+        assert rel_l2(Uh, U_o) < TOL and rel_l2(Omh, Om_o) < TOL
+    # and the two ways agree with each other to the method's 2-3 digits (PAPER.md:335, 378), not to roundoff
+    with dp.Plan(prob, max_particles=len(pos), use_torques=True, torque_mode=0) as plan0:
+        U0, Om0 = plan0.mobility_apply(dpos, dF, dT)
+    assert 1e-8 < rel_l2(Om, Om0.cpu().numpy()) < 5e-2 and rel_l2(U, U0.cpu().numpy()) < 5e-2
+
+
+def test_kernel_derivative_mode_fp32_transfer_variant(dp):
+    prob, pos, F, T = small_monolayer("bw", 3000, 43)
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", torque_mode="kernel")
+    with dp.Plan(prob, max_particles=len(pos), use_torques=True, torque_mode=1, transfer_fp32=True) as plan:
+        U, Om = plan.mobility_apply(*to_dev(pos, F, T))
+    eU, eO = rel_l2(U.cpu().numpy(), U_o), rel_l2(Om.cpu().numpy(), Om_o)
+    assert 1e-9 < eU < 1e-5 and 1e-9 < eO < 1e-5, (eU, eO)
+
+
+# ------------------------------------------------------------------------------------------------ other Chebyshev sizes and kernel widths
+@pytest.mark.parametrize("nz,w,wall", [(19, 4, "bw"), (26, 6, "bw"), (24, 5, "slit"), (40, 8, "slit"), (64, 7, "bw"), (16, 4, "slit")])
+def test_every_compiled_chebyshev_size_and_kernel_width(dp, nz, w, wall):
+    """The paper's own performance grids use Nz = 19 (monopole only, m = 4) and Nz = 26 (Table III): every size in
+    dp_supported_nz (odd ones included: the middle Chebyshev node pairs with itself) and every width 4..8, against the oracle."""
+    import dataclasses
+    assert nz in dp.supported_nz()
+    beta_M = {4: 4 * 1.785, 5: 5 * 1.886, 6: 6 * 1.327, 7: 7 * 1.5, 8: 8 * 1.4}[w]
+    beta_D = {4: 4 * 2.4, 5: 5 * 2.232, 6: 6 * 2.216, 7: 7 * 2.1, 8: 8 * 2.0}[w]
+    if wall == "bw":
+        prob, pos, F, _ = workloads.random_bw(n=150, L=40.0, nxy=50, nz=nz, H=9.0, zlo=0.0, zhi=9.0 - 0.5 * w * 0.8, seed=500 + nz, name="nz")
+        T = np.random.default_rng(nz).standard_normal(F.shape)
+    else:
+        prob, pos, F, T = workloads.random_slit(n=150, L=40.0, nxy=50, nz=nz, H=9.0, margin=0.0, seed=500 + nz, name="nz")
+    prob = dataclasses.replace(prob, w=w, beta_M=beta_M, beta_D=beta_D, has_torque=True)
+    for mode, name in ((0, "fourier"), (1, "kernel")):
+        U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", torque_mode=name)
+        with dp.Plan(prob, max_particles=len(pos), use_torques=True, torque_mode=mode) as plan:
+            U, Om = plan.mobility_apply(*to_dev(pos, F, T))
+            assert plan.check() == 0
+        assert rel_l2(U.cpu().numpy(), U_o) < TOL and rel_l2(Om.cpu().numpy(), Om_o) < TOL, (mode, nz, w)
+        assert rel_max(U.cpu().numpy(), U_o) < TOL_MAX and rel_max(Om.cpu().numpy(), Om_o) < TOL_MAX
