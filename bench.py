@@ -33,9 +33,36 @@ METRIC = "ms per DP-wall mobility product M·F at N=1M; particles/s; % of HBM ro
 # kernels of this library launched per product: k_bin_count, k_scan, k_bin_scatter, k_weights, k_spread, k_solve<nz>, k_zero_mode,
 # k_interp, plus k_fft_x_fwd, k_fft_y_fwd, k_fft_y_inv, k_fft_x_inv with the library's own FFT passes (else cuFFT's kernels)
 MY_KERNELS_PER_STEP = {"own": 12, "cufft": 8}
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, one launch, from the committed ncu --set full capture
-# (profiles/r1_d_README.md: 18.83 GB read with 11 of 32 input planes skipped + 29.00 GB written); None where no capture exists
-NCU_TRAFFIC_GB = {("k_solve<32>", 5): 47.83}
+
+
+def ncu_traffic(kernel_prefix: str, cfg: int, torque_mode: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the named kernel, read from the newest committed ncu launch
+    list of this configuration and torque mode (profiles/*_launches_dram_cfg<c>_<mode>.csv, written by the command its .md names).
+    Returns (bytes or None, file name or None): a capture of an older build is evidence for that build, so the file is named."""
+    import csv
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "*_launches_dram_cfg%d_%s.csv" % (cfg, torque_mode))))
+    if not files:
+        return None, None
+    path = files[-1]
+    rd = wr = None
+    try:
+        with open(path, newline="") as f:
+            rows = [r for r in csv.reader(f) if len(r) > 10]
+        h = rows[0]
+        ki, mi, vi, ui = h.index("Kernel Name"), h.index("Metric Name"), h.index("Metric Value"), h.index("Metric Unit")
+        scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+        for r in rows[1:]:
+            if kernel_prefix not in r[ki]:
+                continue
+            v = float(r[vi].replace(",", "")) * scale.get(r[ui], 1.0)
+            if r[mi] == "dram__bytes_read.sum" and rd is None:
+                rd = v
+            if r[mi] == "dram__bytes_write.sum" and wr is None:
+                wr = v
+    except Exception:
+        return None, os.path.basename(path)
+    return (rd + wr if rd is not None and wr is not None else None), os.path.basename(path)
 
 
 def hbm_peak():
@@ -112,25 +139,34 @@ class ClockSampler(threading.Thread):
 
 
 def cpu_sample_problem(cfg: int):
-    """Bounded sample of the same workload recipe for the oracle legs: same kernel, heights, drives and area fraction,
-    fewer particles (the product is linear-time), sized for ~10-30 s of host work."""
-    if cfg in (3, 5):
-        return workloads.monolayer_bw(n=32768, seed=1005, name="cfg5-sample-32k")
+    """Workload of the oracle legs.  Configs 1-3 are timed whole (the oracle finishes them in seconds); configs 4, 5 on a bounded
+    sample of the same recipe — same kernel, heights, drives and area fraction, fewer particles (the product is linear-time,
+    PAPER.md:337) — sized for ~10-30 s of host work.  Returns (problem, pos, F, T, is_whole_config)."""
+    if cfg == 5:
+        return workloads.monolayer_bw(n=32768, seed=1005, name="cfg5-sample-32k") + (False,)
     if cfg == 4:
-        return workloads.monolayer_slit(n=32768, seed=1004, name="cfg4-sample-32k")
-    return workloads.config(cfg)
+        return workloads.monolayer_slit(n=32768, seed=1004, name="cfg4-sample-32k") + (False,)
+    return workloads.config(cfg) + (True,)
 
 
-def time_oracle(cfg: int, reps: int = 1):
+ORACLE_DFT = "fft"       # the oracle's own plain recursive mixed-radix FFT (validated against its explicit O(n^2) sums in tests/)
+
+
+def oracle_sample_text(prob, n, whole):
+    return "%s: N=%d, grid %dx%dx%d%s; xy DFT: the oracle's own plain recursive FFT (dp_oracle.cpp)" % (
+        prob.name, n, prob.nx, prob.ny, prob.nz, " (the whole configuration)" if whole else ", bounded sample of the same recipe")
+
+
+def time_oracle(cfg: int, torque_mode: str, reps: int = 1):
     import oracle
-    prob, pos, F, T = cpu_sample_problem(cfg)
+    prob, pos, F, T, whole = cpu_sample_problem(cfg)
     best = None
     for _ in range(reps):
         t0 = time.perf_counter()
-        oracle.mobility_apply(prob, pos, F, T, dft="fft")
+        oracle.mobility_apply(prob, pos, F, T, dft=ORACLE_DFT, torque_mode=torque_mode)
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
-    return prob, len(pos), best, oracle.num_threads()
+    return prob, len(pos), best, oracle.num_threads(), whole
 
 
 def run_reference(args):
@@ -139,22 +175,22 @@ def run_reference(args):
     if rank != 0:
         return
     import oracle
-    prob, pos, F, T = cpu_sample_problem(args.config)
+    prob, pos, F, T, whole = cpu_sample_problem(args.config)
     for _ in range(args.warmup):
-        oracle.mobility_apply(prob, pos, F, T, dft="fft")
+        oracle.mobility_apply(prob, pos, F, T, dft=ORACLE_DFT, torque_mode=args.torque_mode)
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        oracle.mobility_apply(prob, pos, F, T, dft="fft")
+        oracle.mobility_apply(prob, pos, F, T, dft=ORACLE_DFT, torque_mode=args.torque_mode)
     dt = (time.perf_counter() - t0) / max(args.steps, 1)
     val = len(pos) / dt
     full = workloads_describe(args.config)
+    sample = oracle_sample_text(prob, len(pos), whole)
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": "particles/s", "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": dict(full, note="oracle timed on a bounded sample of this workload"),
-            "cpu_baseline": {"value": val, "unit": "particles/s", "cores": oracle.num_threads(), "kind": "oracle",
-                             "sample": "%s: N=%d, grid %dx%dx%d, same recipe; xy DFT via numpy.fft (library primitive)" % (
-                                 prob.name, len(pos), prob.nx, prob.ny, prob.nz)},
+            "config": dict(full, torque_mode=args.torque_mode, same_config=bool(whole),
+                           note="the oracle timed on " + ("this whole configuration" if whole else "a bounded sample of this workload")),
+            "cpu_baseline": {"value": val, "unit": "particles/s", "cores": oracle.num_threads(), "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": "particles/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 
@@ -163,6 +199,154 @@ def workloads_describe(cfg: int):
     names = {1: "cfg1 bottom wall N=128", 2: "cfg2 slit N=4096", 3: "cfg3 bottom-wall monolayer N=65536",
              4: "cfg4 slit monolayer N=262144", 5: "cfg5 bottom-wall microroller monolayer N=1048576"}
     return {"workload": names[cfg]}
+
+
+def replica_inputs(cfg: int, rank: int):
+    """Rank r of an N-replica run draws its own particles from the configuration's recipe (seed + 17 r); rank 0 is the configuration."""
+    prob, pos, F, T = workloads.config(cfg)
+    if rank == 0:
+        return prob, pos, F, T
+    seed = replica_seed(prob.seed, rank)
+    if cfg == 1:
+        return workloads.random_bw(seed=seed)
+    if cfg == 2:
+        return workloads.random_slit(seed=seed)
+    if cfg in (3, 5):
+        return workloads.monolayer_bw(n=prob.n, seed=seed, name=prob.name)
+    return workloads.monolayer_slit(seed=seed)
+
+
+KERNELS = ("k_spread", "k_fft_x_fwd", "k_fft_y_fwd", "k_solve", "k_fft_y_inv", "k_fft_x_inv", "k_interp")
+
+
+def kernel_bytes(prob, n, fin, fout, zero_planes=0):
+    """Bytes each kernel of the product must itself move (its compulsory reads + writes): R = one real field,
+    C = one half spectrum, a = share of the input planes that can hold force.  The two passes of a 2-D transform each read and
+    write the whole field once, so the two FFT kernels of a stage together move twice SURVEY.md §8(d)'s per-stage figure."""
+    G = prob.nx * prob.ny * prob.nz
+    Kz = (prob.nx // 2 + 1) * prob.ny * prob.nz
+    R, C = 8.0 * G, 16.0 * Kz
+    a = 1.0 - zero_planes / float(prob.nz)
+    return {"k_spread": a * fin * R + 72.0 * n, "k_fft_x_fwd": a * fin * (R + C), "k_fft_y_fwd": a * fin * 2 * C,
+            "k_solve": (a * fin + fout) * C, "k_fft_y_inv": fout * 2 * C, "k_fft_x_inv": fout * (C + R), "k_interp": fout * R + 72.0 * n}
+
+
+def measure(dp, torch, prob, pos, F, T, dev, dist, args, *, torque_mode, transfer_fp32=False, dense_planes=False, fft="own",
+            e2e=False, clocks=False, steps=None):
+    """One timed run: plan, warm-ups, K products between CUDA events on the launching stream (max over ranks), then per-stage and
+    per-FFT-pass times from the plan's own events in a separate pass, then (optionally) the end-to-end run through host buffers."""
+    steps = steps or args.steps
+    n = len(pos)
+    use_t = T is not None
+    tmode = 1 if (torque_mode == "kernel" and use_t) else 0
+    plan = dp.Plan(prob, max_particles=n, use_torques=use_t, device=dev.index, fft_backend=0 if fft == "own" else 1,
+                   transfer_fp32=transfer_fp32, dense_planes=dense_planes, torque_mode=tmode)
+    out = {"torque_mode": (torque_mode if use_t else "none"), "fields": plan.fields, "fft_backend": plan.fft_backend(), "plan_device_GB": plan.device_bytes() / 1e9}
+    dpos = torch.from_numpy(pos).to(dev)
+    dF = torch.from_numpy(F).to(dev)
+    dT = torch.from_numpy(T).to(dev) if use_t else None
+    U = torch.empty((n, 3), dtype=torch.float64, device=dev)
+    Om = torch.empty((n, 3), dtype=torch.float64, device=dev) if use_t else None
+    stream = torch.cuda.current_stream(dev)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    plan.set_profiling(True)
+    for _ in range(args.warmup):
+        plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
+    barrier()
+    sampler = None
+    if clocks:
+        sampler = ClockSampler(dev.index)
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(steps):
+        plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    if sampler is not None:
+        sampler.stop_flag.set()
+        sampler.join(timeout=3)
+        out["clocks"] = sampler.summary()
+    # per-stage / per-pass device times: separately synchronised (dp_stage_ms synchronises, so it stays out of the timed loop)
+    acc = {}
+    for _ in range(max(3, min(steps, 5))):
+        plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
+        d = plan.stage_ms()
+        if out["fft_backend"] == "own":
+            d.update(plan.fft_pass_ms())
+        for k, v in d.items():
+            acc.setdefault(k, []).append(v)
+    out["stage_ms"] = {k: float(np.median(v)) for k, v in acc.items()}
+    assert plan.check() == 0
+    out["zero_planes"] = plan.zero_planes()
+    out["ms_per_step"] = max_over_ranks(dist, ms_total / steps, dev)
+    if e2e:
+        hp = torch.from_numpy(pos).pin_memory(); hF = torch.from_numpy(F).pin_memory()
+        hT = torch.from_numpy(T).pin_memory() if use_t else None
+        hU = torch.empty((n, 3), dtype=torch.float64).pin_memory()
+        hO = torch.empty((n, 3), dtype=torch.float64).pin_memory() if use_t else None
+        npv = lambda t: None if t is None else t.numpy()
+        for _ in range(2):
+            plan.mobility_apply_host(npv(hp), npv(hF), npv(hT), out_U=npv(hU), out_Omega=npv(hO))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            plan.mobility_apply_host(npv(hp), npv(hF), npv(hT), out_U=npv(hU), out_Omega=npv(hO))   # synchronous
+        dt = max_over_ranks(dist, (time.perf_counter() - t0) / steps, dev)
+        world = dist.get_world_size() if dist is not None else 1
+        out["e2e"] = {"value": world * n / dt, "unit": "particles/s", "ms_per_step": dt * 1e3,
+                      "h2d_bytes_per_step": int(24 * n * (3 if use_t else 2)), "d2h_bytes_per_step": int(24 * n * (2 if use_t else 1))}
+    plan.close()
+    del dpos, dF, dT, U, Om
+    return out
+
+
+def kernel_table(prob, n, run, peak):
+    """ms, own compulsory bytes and fraction of the HBM roofline of each of the seven grid kernels of one measured run."""
+    fin = fout = run["fields"]
+    st = run["stage_ms"]
+    ms = {"k_spread": st.get("spread", 0.0), "k_solve": st.get("solve", 0.0), "k_interp": st.get("interp", 0.0),
+          "k_fft_x_fwd": st.get("fft_x_fwd"), "k_fft_y_fwd": st.get("fft_y_fwd"), "k_fft_y_inv": st.get("fft_y_inv"), "k_fft_x_inv": st.get("fft_x_inv")}
+    need = kernel_bytes(prob, n, fin, fout, run["zero_planes"])
+    dense = kernel_bytes(prob, n, fin, fout, 0)
+    tab = {}
+    for k in KERNELS:
+        t = ms[k]
+        if not t:
+            continue
+        gbs = need[k] / (t * 1e-3) / 1e9
+        tab[k] = {"ms": t, "algorithmic_GB": need[k] / 1e9, "GBps": gbs, "frac": gbs / peak, "algorithmic_GB_if_all_planes_dense": dense[k] / 1e9}
+    return tab
+
+
+def summarise(prob, n, run, peak, world):
+    """stage table (SURVEY.md §8(d) bytes: one read + one write per field and stage), the kernel table, the north_star aggregate"""
+    fin = fout = run["fields"]
+    by = stage_bytes(prob, n, fin, fout, run["zero_planes"])
+    by_dense = stage_bytes(prob, n, fin, fout, 0)
+    st = run["stage_ms"]
+    stages = {}
+    for k, b in by.items():
+        t = st.get(k, 0.0)
+        gbs = b / (t * 1e-3) / 1e9 if t > 0 else None
+        stages[k] = {"ms": t, "algorithmic_GB": b / 1e9, "GBps": gbs, "frac": (gbs / peak) if gbs else None}
+    stages["bin"] = {"ms": st.get("bin", 0.0)}
+    mid = sum(by[k] for k in ("fft_fwd", "solve", "fft_inv")) / 1e9
+    mid_ms = sum(st.get(k, 0.0) for k in ("fft_fwd", "solve", "fft_inv"))
+    mid_frac = (mid / (mid_ms * 1e-3) / peak) if mid_ms else None
+    agg = {"fft_chebyshev_solve_stages": {"algorithmic_GB": mid, "ms": mid_ms, "GBps": mid / (mid_ms * 1e-3) if mid_ms else None, "frac": mid_frac,
+                                          "target_frac": 0.5, "target_met": bool(mid_frac is not None and mid_frac >= 0.5)},
+           "whole_product": {"algorithmic_GB": sum(by.values()) / 1e9, "ms": run["ms_per_step"],
+                             "frac": sum(by.values()) / 1e9 / (run["ms_per_step"] * 1e-3) / peak,
+                             "algorithmic_GB_if_all_planes_dense": sum(by_dense.values()) / 1e9}}
+    return stages, agg
 
 
 def main():
@@ -174,9 +358,13 @@ def main():
     ap.add_argument("--impl", default="b200")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-variants", action="store_true", help="skip the extra timings (other torque mode, fp32 transfer variant, dense planes, Fig. 9 workload)")
     ap.add_argument("--transfer-fp32", action="store_true", help="time the fp32 spread/interpolate variant as the main number")
     ap.add_argument("--no-fp32-variant", action="store_true", help="skip the extra timing of the fp32 spread/interpolate variant")
     ap.add_argument("--dense-planes", action="store_true", help="transform every plane (do not skip the planes no footprint reaches)")
+    ap.add_argument("--torque-mode", choices=["fourier", "kernel"], default="kernel",
+                    help="torques / Omega through the ES kernel's derivative (3 grid fields each way; the paper's second way, PAPER.md:335) "
+                         "or through the curl in Fourier-Chebyshev space (6 fields; its first way)")
     ap.add_argument("--fft", choices=["own", "cufft"], default="own", help="xy FFT backend (own shared-memory passes, or cuFFT for comparison)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
@@ -203,109 +391,43 @@ def main():
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
 
-    prob, pos, F, T = workloads.config(args.config)
-    if world > 1:      # replicas: each rank draws its own particles from the same recipe
-        prob, pos, F, T = (workloads.monolayer_bw(n=prob.n, seed=replica_seed(prob.seed, rank), name=prob.name) if args.config in (3, 5)
-                           else workloads.config(args.config))
+    prob, pos, F, T = replica_inputs(args.config, rank)       # replicas: each rank draws its own particles from the same recipe
     n = len(pos)
-    fin = 6 if T is not None else 3
-    fout = fin
-    plan = dp.Plan(prob, max_particles=n, use_torques=T is not None, device=local_rank, fft_backend=0 if args.fft == "own" else 1,
-                   transfer_fp32=args.transfer_fp32, dense_planes=args.dense_planes)
-    fft_backend = plan.fft_backend()
-    dpos = torch.from_numpy(pos).to(dev)
-    dF = torch.from_numpy(F).to(dev)
-    dT = torch.from_numpy(T).to(dev) if T is not None else None
-    U = torch.empty((n, 3), dtype=torch.float64, device=dev)
-    Om = torch.empty((n, 3), dtype=torch.float64, device=dev) if T is not None else None
-    stream = torch.cuda.current_stream(dev)
+    M = lambda **kw: measure(dp, torch, prob, pos, F, T, dev, dist, args, **kw)
 
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize(dev)
-
-    # ---- device-resident timing: inputs already in HBM
-    plan.set_profiling(True)
-    for _ in range(args.warmup):
-        plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
-    barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    stage_acc = {}
-    barrier()
-    e0.record(stream)
-    for _ in range(args.steps):
-        plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
-    e1.record(stream)
-    barrier()
-    ms_total = e0.elapsed_time(e1)
-    sampler.stop_flag.set()
-    sampler.join(timeout=3)
-    # per-stage device times: a second, separately synchronised pass (dp_stage_ms synchronises, so it stays out of the timed loop)
-    for _ in range(max(3, min(args.steps, 5))):
-        plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
-        for k, v in plan.stage_ms().items():
-            stage_acc.setdefault(k, []).append(v)
-    stage_ms = {k: float(np.median(v)) for k, v in stage_acc.items()}
-    assert plan.check() == 0
-    zero_planes = plan.zero_planes()
-    ms_step = max_over_ranks(dist, ms_total / args.steps, dev)
+    # ---- the headline run: device-resident timing, clocks sampled during the timed region, end to end through host buffers
+    main_run = M(torque_mode=args.torque_mode, transfer_fp32=args.transfer_fp32, dense_planes=args.dense_planes, fft=args.fft,
+                 e2e=not args.no_e2e, clocks=True)
+    ms_step = main_run["ms_per_step"]
     value = whole_job_value(n, world, ms_step)
 
-    # ---- end to end: host buffers in (pinned), host buffers out, through dp_mobility_apply_host
-    e2e = None
-    if not args.no_e2e:
-        hp = torch.from_numpy(pos).pin_memory(); hF = torch.from_numpy(F).pin_memory()
-        hT = torch.from_numpy(T).pin_memory() if T is not None else None
-        hU = torch.empty((n, 3), dtype=torch.float64).pin_memory()
-        hO = torch.empty((n, 3), dtype=torch.float64).pin_memory() if T is not None else None
-        npv = lambda t: None if t is None else t.numpy()
-        for _ in range(2):
-            plan.mobility_apply_host(npv(hp), npv(hF), npv(hT), out_U=npv(hU), out_Omega=npv(hO))
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.steps):
-            plan.mobility_apply_host(npv(hp), npv(hF), npv(hT), out_U=npv(hU), out_Omega=npv(hO))   # synchronous
-        dt = max_over_ranks(dist, (time.perf_counter() - t0) / args.steps, dev)
-        e2e = {"value": world * n / dt, "unit": "particles/s", "ms_per_step": dt * 1e3,
-               "h2d_bytes_per_step": int(24 * n * (3 if T is not None else 2)), "d2h_bytes_per_step": int(24 * n * (2 if T is not None else 1))}
-
-    # ---- two more timings of the same product on the same inputs, same rules (3 warm-ups, CUDA events, max over ranks):
-    #      the optional fp32 spread/interpolate variant (north_star: "also timed"), and the product with the zero-plane
-    #      skipping switched off (every plane spread, transformed and loaded)
-    plan_bytes = plan.device_bytes()
-
-    def time_variant(**kw):
-        nonlocal plan
-        plan.close()
-        plan = dp.Plan(prob, max_particles=n, use_torques=T is not None, device=local_rank, **kw)
-        plan.set_profiling(True)
-        for _ in range(args.warmup):
-            plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
-        barrier()
-        v0, v1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        v0.record(stream)
-        for _ in range(args.steps):
-            plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
-        v1.record(stream)
-        barrier()
-        vms = max_over_ranks(dist, v0.elapsed_time(v1) / args.steps, dev)
-        plan.mobility_apply(dpos, dF, dT, out_U=U, out_Omega=Om, stream=stream)
-        vst = plan.stage_ms()
-        return {"ms_per_step": vms, "value": world * n / (vms * 1e-3), "unit": "particles/s",
-                "stage_ms": {k: vst[k] for k in ("spread", "fft_fwd", "solve", "fft_inv", "interp")},
-                "plan_device_GB": plan.device_bytes() / 1e9}
-
-    variant = dense = None
-    if not args.transfer_fp32 and not args.no_fp32_variant and args.fft == "own":
-        variant = time_variant(transfer_fp32=True, dense_planes=args.dense_planes)
-        variant["what"] = ("spreading and interpolation accumulate in fp32, real-space grids stored in fp32; FFTs and solves fp64; "
-                           "matches the oracle to <= 1e-5 (tests)")
-        if not args.dense_planes and zero_planes > 0:
-            dense = time_variant(transfer_fp32=False, dense_planes=True)
-            dense["what"] = "same fp64 product with dense_planes = 1: the %d planes no footprint reaches are spread, transformed and loaded too" % zero_planes
+    # ---- the same product on the same inputs in its other forms, same rules (3 warm-ups, CUDA events, max over ranks)
+    other = variant = dense = fig9 = None
+    if not args.no_variants and args.fft == "own":
+        if T is not None:
+            om = "fourier" if args.torque_mode == "kernel" else "kernel"
+            other = M(torque_mode=om, transfer_fp32=args.transfer_fp32, dense_planes=args.dense_planes)
+            other["what"] = ("the same forces + torques -> U, Omega product with the torques taken through " +
+                             ("the curl in Fourier-Chebyshev space: six grid fields each way (the paper's first way, PAPER.md:335)" if om == "fourier" else
+                              "the derivative of the ES kernel: three grid fields each way (the paper's second way, PAPER.md:335)") +
+                             "; the two discretisations agree to the method's 2-3 digits, each matches its own oracle path to <= 1e-10")
+        if not args.transfer_fp32 and not args.no_fp32_variant:
+            variant = M(torque_mode=args.torque_mode, transfer_fp32=True, dense_planes=args.dense_planes)
+            variant["what"] = ("spreading and interpolation accumulate in fp32, real-space grids stored in fp32; FFTs and solves fp64; "
+                               "matches the oracle to <= 1e-5 (tests)")
+        if not args.dense_planes and main_run["zero_planes"] > 0:
+            dense = M(torque_mode=args.torque_mode, transfer_fp32=args.transfer_fp32, dense_planes=True)
+            dense["what"] = ("same product with dense_planes = 1: the %d planes no footprint reaches are spread, transformed and loaded too"
+                             % main_run["zero_planes"])
+        if world == 1 and args.config == 5:
+            # context for the paper's only published timing (Fig. 9): its own grid and kernel, forces only
+            p9, pos9, F9, T9 = workloads.paper_fig9(18)
+            r9 = measure(dp, torch, p9, pos9, F9, T9, dev, dist, args, torque_mode="kernel")
+            fig9 = {"workload": "paper Fig. 9 / Table III 'M' stand-in: N=%d, forces only, grid %dx%dx%d, m=4, beta/m=1.87, H=9.1 R_h, two-layer heights"
+                                % (len(pos9), p9.nx, p9.ny, p9.nz),
+                    "ms_per_step": r9["ms_per_step"], "value": len(pos9) / (r9["ms_per_step"] * 1e-3), "unit": "particles/s",
+                    "stage_ms": r9["stage_ms"], "plan_device_GB": r9["plan_device_GB"],
+                    "paper": "370 ms per mobility solve on a V100 for this case (PAPER.md:505): another machine's number, context only"}
 
     if rank != 0:
         if dist is not None:
@@ -313,46 +435,60 @@ def main():
         return
 
     peak, peak_src = hbm_peak()
-    by = stage_bytes(prob, n, fin, fout, zero_planes)
-    by_dense = stage_bytes(prob, n, fin, fout, 0)
-    stages = {}
-    for k, b in by.items():
-        t_ms = stage_ms.get(k, 0.0)
-        gbs = b / (t_ms * 1e-3) / 1e9 if t_ms > 0 else None
-        stages[k] = {"ms": t_ms, "algorithmic_GB": b / 1e9, "GBps": gbs, "frac": (gbs / peak) if gbs else None}
-    stages["bin"] = {"ms": stage_ms.get("bin", 0.0)}
-    mine = {k: stages[k] for k in ("spread", "solve", "interp")}
-    dom = max(mine, key=lambda k: mine[k]["ms"])
-    kernel_name = {"spread": "k_spread", "solve": "k_solve<%d>" % prob.nz, "interp": "k_interp"}[dom]
-    mid = sum(by[k] for k in ("fft_fwd", "solve", "fft_inv")) / 1e9
-    mid_ms = sum(stage_ms.get(k, 0.0) for k in ("fft_fwd", "solve", "fft_inv"))
-    traffic = NCU_TRAFFIC_GB.get((kernel_name, args.config))
-    roofline = {"bound": "hbm", "kernel": kernel_name, "achieved": mine[dom]["GBps"], "peak": peak, "unit": "GB/s",
-                "frac": mine[dom]["frac"], "traffic": traffic * 1e9 if traffic else None, "peak_source": peak_src,
-                "note": "k_solve is co-bound by the fp64 pipe and shared memory (profiles/r1_d_README.md); the fraction is of the HBM roofline",
-                "fft_chebyshev_solve_stages": {"algorithmic_GB": mid, "ms": mid_ms, "GBps": mid / (mid_ms * 1e-3) if mid_ms else None,
-                                               "frac": (mid / (mid_ms * 1e-3) / peak) if mid_ms else None},
-                "whole_product": {"algorithmic_GB": sum(by.values()) / 1e9, "ms": ms_step,
-                                  "frac": sum(by.values()) / 1e9 / (ms_step * 1e-3) / peak,
-                                  "algorithmic_GB_if_all_planes_dense": sum(by_dense.values()) / 1e9}}
+    stages, agg = summarise(prob, n, main_run, peak, world)
+    ktab = kernel_table(prob, n, main_run, peak)
+    cand = ktab if ktab else {"k_solve": {"ms": stages["solve"]["ms"], "GBps": stages["solve"]["GBps"], "frac": stages["solve"]["frac"],
+                                          "algorithmic_GB": stages["solve"]["algorithmic_GB"], "algorithmic_GB_if_all_planes_dense": None}}
+    dom = max(cand, key=lambda k: cand[k]["ms"])
+    kname = {"k_solve": "k_solve<%d>" % prob.nz}.get(dom, dom)
+    traffic, traffic_file = ncu_traffic(dom, args.config, main_run["torque_mode"] if T is not None else "kernel")
+    frac_dense = None
+    if dense is not None:
+        dk = kernel_table(prob, n, dense, peak).get(dom)
+        frac_dense = dk["frac"] if dk else None
+    roofline = {"bound": "hbm", "kernel": kname, "achieved": cand[dom]["GBps"], "peak": peak, "unit": "GB/s", "frac": cand[dom]["frac"],
+                "frac_if_all_planes_dense": frac_dense,
+                "traffic": traffic, "traffic_source": ("profiles/%s (ncu capture of the build that file's .md names)" % traffic_file) if traffic_file else None,
+                "peak_source": peak_src,
+                "bytes": "the kernel's own compulsory reads + writes with the planes no footprint reaches left out (algorithmic_GB); "
+                         "frac_if_all_planes_dense: SURVEY.md §8(d)'s dense bytes over the time of the dense_planes = 1 run",
+                "note": "k_solve is co-bound by the fp64 pipe (DFMA + DMMA share it), the shared-memory pipe and instruction issue "
+                        "(profiles/r2_*): the fraction is of the HBM roofline, as the contract asks",
+                "kernels": ktab}
+    roofline.update(agg)
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
-        sprob, sn, sdt, cores = time_oracle(args.config)
-        cpu = {"value": sn / sdt, "unit": "particles/s", "cores": cores, "kind": "oracle", "seconds": sdt,
-               "sample": "%s: N=%d, grid %dx%dx%d, same recipe; xy DFT via numpy.fft (library primitive)" % (sprob.name, sn, sprob.nx, sprob.ny, sprob.nz)}
+        sprob, sn, sdt, cores, whole = time_oracle(args.config, args.torque_mode if T is not None else "fourier")
+        cpu = {"value": sn / sdt, "unit": "particles/s", "cores": cores, "kind": "oracle", "seconds": sdt, "sample": oracle_sample_text(sprob, sn, whole)}
 
+    def brief(r):
+        if r is None:
+            return None
+        keep = ("spread", "fft_fwd", "solve", "fft_inv", "interp", "fft_x_fwd", "fft_y_fwd", "fft_y_inv", "fft_x_inv")
+        d = {"ms_per_step": r["ms_per_step"], "value": world * n / (r["ms_per_step"] * 1e-3), "unit": "particles/s",
+             "fields_each_way": r["fields"], "stage_ms": {k: r["stage_ms"][k] for k in keep if k in r["stage_ms"]},
+             "plan_device_GB": r["plan_device_GB"], "what": r.get("what")}
+        st2, agg2 = summarise(prob, n, r, peak, world)
+        d["fft_chebyshev_solve_stages"] = agg2["fft_chebyshev_solve_stages"]
+        d["whole_product_frac"] = agg2["whole_product"]["frac"]
+        return d
+
+    fin = fout = main_run["fields"]
+    by_total = sum(stage_bytes(prob, n, fin, fout, main_run["zero_planes"]).values())
     line = {"metric": METRIC, "value": value, "unit": "particles/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": dict(workloads_describe(args.config), n_particles=n, grid=[prob.nx, prob.ny, prob.nz], wall_mode=["bottom_wall", "slit"][prob.wall_mode],
-                           fields_in=fin, fields_out=fout, w=prob.w, l2="inputs (%.1f GB of grids per product) far exceed the 126 MB L2" % (sum(by.values()) / 1e9 / 4),
-                           parallelism="replicas" if world > 1 else "single GPU", plan_device_GB=plan_bytes / 1e9,
-                           fft_backend=fft_backend, transfer_fp32=bool(args.transfer_fp32),
-                           zero_planes_skipped=zero_planes, nz=prob.nz),
-            "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": MY_KERNELS_PER_STEP[fft_backend] * args.steps,
-            "stages": stages, "roofline": roofline, "cpu_baseline": cpu, "fp32_transfer_variant": variant, "all_planes_dense": dense}
+                           fields_in=fin, fields_out=fout, w=prob.w, torque_mode=main_run["torque_mode"],
+                           l2="inputs (%.1f GB of grids per product) far exceed the 126 MB L2" % (by_total / 1e9 / 4),
+                           parallelism="replicas" if world > 1 else "single GPU", plan_device_GB=main_run["plan_device_GB"],
+                           fft_backend=main_run["fft_backend"], transfer_fp32=bool(args.transfer_fp32),
+                           zero_planes_skipped=main_run["zero_planes"], nz=prob.nz),
+            "clocks": main_run.get("clocks"), "e2e": main_run.get("e2e"), "gpu_launches": MY_KERNELS_PER_STEP[main_run["fft_backend"]] * args.steps,
+            "stages": stages, "roofline": roofline, "cpu_baseline": cpu,
+            ("fourier_curl_torques" if args.torque_mode == "kernel" else "kernel_derivative_torques"): brief(other),
+            "fp32_transfer_variant": brief(variant), "all_planes_dense": brief(dense), "paper_fig9": fig9}
     print(json.dumps(line), flush=True)
-    plan.close()
     if dist is not None:
         dist.destroy_process_group()
 

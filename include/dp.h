@@ -121,6 +121,9 @@ double dp_effective_radius(const dp_plan* plan, int dipole);
  * Only recorded if dp_set_profiling(plan, 1). */
 int dp_set_profiling(dp_plan* plan, int on);
 int dp_stage_ms(dp_plan* plan, float* ms /* [8] */);
+/* Same, for the four kernels of the library's own xy FFT (step 2 and step 7) of the LAST profiled apply:
+ * ms[0] forward x pass, [1] forward y pass, [2] inverse y pass, [3] inverse x pass.  DP_EINVAL with the cuFFT backend. */
+int dp_fft_pass_ms(dp_plan* plan, float* ms /* [4] */);
 
 /* Test hooks: copy an internal device buffer of the last apply to HOST memory (synchronises).
  *   which = 0: real grid    [fields][nz][ny][nx]       doubles  (after apply: u, (1/2) curl u in real space)

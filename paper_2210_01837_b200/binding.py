@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBNAME = os.path.join(_HERE, "libdpstokes.so")
 
 # every symbol include/dp.h declares
-EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_check", "dp_effective_radius", "dp_set_profiling", "dp_stage_ms",
+EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_check", "dp_effective_radius", "dp_set_profiling", "dp_stage_ms", "dp_fft_pass_ms",
            "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_copy_plane_to_host", "dp_complex_row_pitch", "dp_zero_planes", "dp_fft_backend", "dp_es_norm", "dp_es_radius_over_h",
            "dp_es_dphi_cut", "dp_supported_nz", "dp_device_bytes", "dp_strerror", "dp_last_error", "dp_destroy"]
 
@@ -60,6 +60,8 @@ def load_library():
     L.dp_set_profiling.restype = i
     L.dp_stage_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
     L.dp_stage_ms.restype = i
+    L.dp_fft_pass_ms.argtypes = [vp, ctypes.POINTER(ctypes.c_float)]
+    L.dp_fft_pass_ms.restype = i
     L.dp_debug_run_stage.argtypes = [vp, i, vp, vp, vp, i, vp]
     L.dp_debug_run_stage.restype = i
     L.dp_buffer_bytes.argtypes = [vp, i]
@@ -210,6 +212,11 @@ class Plan:
         buf = (ctypes.c_float * 8)()
         self._ck(load_library().dp_stage_ms(self._h, buf), "dp_stage_ms")
         return {k: float(buf[i]) for i, k in enumerate(STAGE_NAMES)}
+
+    def fft_pass_ms(self) -> dict:
+        buf = (ctypes.c_float * 4)()
+        self._ck(load_library().dp_fft_pass_ms(self._h, buf), "dp_fft_pass_ms")
+        return {k: float(buf[i]) for i, k in enumerate(("fft_x_fwd", "fft_y_fwd", "fft_y_inv", "fft_x_inv"))}
 
     def zero_planes(self) -> int:
         return int(load_library().dp_zero_planes(self._h))

@@ -71,6 +71,7 @@ struct dp_plan {
   cudaStream_t last_stream = nullptr;
   bool profiling = false;
   cudaEvent_t ev[9] = {};
+  cudaEvent_t ev_fft[2] = {};   // between the two passes of the forward / inverse xy FFT (own passes, profiling only)
   bool ev_ok = false;
   bool ev_recorded = false;
   std::string last_error;

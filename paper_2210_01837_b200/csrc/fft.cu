@@ -10,9 +10,10 @@
 //
 // Each pass reads every grid value once and writes it once (4 passes per product and field instead of the ten of the
 // library's multi-kernel plans at 4320 x 4320).  A row (or a batch of short rows) lives in shared memory for its whole
-// transform (fft_engine.cuh).  One persistent CTA per SM holds the small twiddle tables and two independent row slots
-// (256 threads each, named barriers, 128 registers per thread), so that one slot's memory phases overlap the other slot's
-// butterflies.  The stage with the largest stride exchanges its data directly with global memory (coalesced: consecutive
+// transform (fft_engine.cuh).  One persistent CTA per SM holds the small twiddle tables and independent row slots
+// (x passes: two slots of 256 threads; y passes: three slots of 160 threads — 270 / 240 / 288 lines per stage of a 4320-point
+// row waste fewer thread rounds at 160 than at 256; named barriers, 128 registers per thread), so that one slot's memory phases
+// overlap the other slots' butterflies.  The stage with the largest stride exchanges its data directly with global memory (coalesced: consecutive
 // threads take consecutive elements); the other side of the y passes is one bulk asynchronous copy per row
 // (cp.async.bulk + mbarrier), prefetched in the inverse pass; the other side of the x passes is the transposed
 // scatter / gather of 16-byte elements (rb consecutive y per kx).
@@ -30,12 +31,21 @@ namespace {
 
 using namespace dpfft;
 
-constexpr int NSLOT = 2;
-#ifndef DP_FFT_TPS
-#define DP_FFT_TPS 256
+// slots per CTA and threads per slot of the x passes and of the y passes (tuning builds may override them)
+#ifndef DP_FFT_XSLOTS
+#define DP_FFT_XSLOTS 2
 #endif
-constexpr int TPS = DP_FFT_TPS;               // threads per slot
-constexpr int FFT_THREADS = NSLOT * TPS;
+#ifndef DP_FFT_XTPS
+#define DP_FFT_XTPS 256
+#endif
+#ifndef DP_FFT_YSLOTS
+#define DP_FFT_YSLOTS 3
+#endif
+#ifndef DP_FFT_YTPS
+#define DP_FFT_YTPS 160
+#endif
+constexpr int XSLOTS = DP_FFT_XSLOTS, XTPS = DP_FFT_XTPS, XTHREADS = XSLOTS * XTPS;
+constexpr int YSLOTS = DP_FFT_YSLOTS, YTPS = DP_FFT_YTPS, YTHREADS = YSLOTS * YTPS;
 constexpr int SLOT_ELEMS = 4320;               // complex elements a slot can hold (69 120 bytes)
 
 struct dp_fft_own {
@@ -85,7 +95,7 @@ __device__ __forceinline__ void bulk_store(void* gmem_dst, const void* smem_src,
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_async_proxy() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void slot_barrier(int slot) { asm volatile("bar.sync %0, %1;" ::"r"(slot + 1), "r"(TPS) : "memory"); }
+template <int TPS> __device__ __forceinline__ void slot_barrier(int slot) { asm volatile("bar.sync %0, %1;" ::"r"(slot + 1), "n"(TPS) : "memory"); }
 
 struct FftYArgs {
   double2* data;          // rows of n complex numbers, contiguous
@@ -120,7 +130,7 @@ struct MidNone { __device__ __forceinline__ void operator()(int, int) const {} }
 struct MidStoreDrained {      // forward y pass, round 0: the slot's previous bulk store has read the buffer
   int slot, st;
   __device__ __forceinline__ void operator()(int rd, int) const {
-    if (rd == 0) { if (st == 0) bulk_wait_read(); slot_barrier(slot); }
+    if (rd == 0) { if (st == 0) bulk_wait_read(); slot_barrier<YTPS>(slot); }
   }
 };
 struct MidPrefetch {          // inverse y pass, last round: all inputs are in registers, refill the buffer with the next rows
@@ -132,7 +142,7 @@ struct MidPrefetch {          // inverse y pass, last round: all inputs are in r
   __device__ __forceinline__ void operator()(int rd, int nrounds) const {
     if (rd == nrounds - 1) {
       fence_async_proxy();      // generic-proxy accesses of buf (this batch's stages) before the async-proxy refill
-      slot_barrier(slot);
+      slot_barrier<YTPS>(slot);
       if (st == 0 && next) { mbar_expect_tx(mbar, bytes); bulk_load(buf, next, bytes, mbar); }
     }
   }
@@ -141,41 +151,41 @@ struct MidPrefetch {          // inverse y pass, last round: all inputs are in r
 // The kernels are templates on the factorisation <R0, R1, R2> of the hot sizes (no runtime dispatch, every index into the
 // argument arrays static, only three butterflies in the instruction stream); <0, 0, 0> is the general version that
 // reads the radices from its arguments.
-template <int R0, bool INV, class Mid, class TS, class TD>
+template <int TPS, int R0, bool INV, class Mid, class TS, class TD>
 __device__ __forceinline__ void run_edge(int r0, const TS* src, TD* dst, const double2* tw1, int n, int rows, int tid, const Mid& mid) {
   if constexpr (R0 > 0) edge_lines<R0, INV>(src, dst, tw1, n, rows, (size_t)n, (size_t)n, tid, TPS, mid);
   else edge_dispatch<INV>(r0, src, dst, tw1, n, rows, (size_t)n, (size_t)n, tid, TPS, mid);
 }
 // the shared-memory stages after (forward) or before (inverse) the edge stage, with the slot's barrier between stages;
 // LAST_BARRIER: also after the final one
-template <int R0, int R1, int R2, bool INV, bool LAST_BARRIER, class FA>
+template <int TPS, int R0, int R1, int R2, bool INV, bool LAST_BARRIER, class FA>
 __device__ __forceinline__ void run_inner(const FA& A, double2* buf, const double2* tw, int n, int rows, int tid, int slot) {
   if constexpr (R0 > 0) {
     constexpr int S1 = R2;                       // stride of stage 1 (n = R0 R1 R2)
     if (!INV) {
       stage_lines<R1, false>(buf, tw + A.off[1], n, S1, rows, n, tid, TPS);
-      slot_barrier(slot);
+      slot_barrier<TPS>(slot);
       stage_lines<R2, false>(buf, tw + A.off[2], n, 1, rows, n, tid, TPS);
-      if (LAST_BARRIER) slot_barrier(slot);
+      if (LAST_BARRIER) slot_barrier<TPS>(slot);
     } else {
       stage_lines<R2, true>(buf, tw + A.off[2], n, 1, rows, n, tid, TPS);
-      slot_barrier(slot);
+      slot_barrier<TPS>(slot);
       stage_lines<R1, true>(buf, tw + A.off[1], n, S1, rows, n, tid, TPS);
-      if (LAST_BARRIER) slot_barrier(slot);
+      if (LAST_BARRIER) slot_barrier<TPS>(slot);
     }
   } else if (!INV) {
     int S = n / A.F.r[0];
     for (int j = 1; j < A.F.ns; ++j) {
       S /= A.F.r[j];
       stage_dispatch<false>(A.F.r[j], buf, tw + A.off[j], n, S, rows, n, tid, TPS);
-      if (LAST_BARRIER || j + 1 < A.F.ns) slot_barrier(slot);
+      if (LAST_BARRIER || j + 1 < A.F.ns) slot_barrier<TPS>(slot);
     }
   } else {
     int S = 1;
     for (int j = A.F.ns - 1; j >= 1; --j) {
       stage_dispatch<true>(A.F.r[j], buf, tw + A.off[j], n, S, rows, n, tid, TPS);
       S *= A.F.r[j];
-      if (LAST_BARRIER || j > 1) slot_barrier(slot);
+      if (LAST_BARRIER || j > 1) slot_barrier<TPS>(slot);
     }
   }
 }
@@ -185,30 +195,30 @@ __device__ __forceinline__ void run_inner(const FA& A, double2* buf, const doubl
 // result leaves with one bulk store.  While a slot's bulk store drains, its next row's global loads are already in
 // flight; the stage-1 results are written to shared memory only after the store has finished reading it.
 template <int R0, int R1, int R2>
-__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_y_fwd(FftYArgs A) {
+__global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_fwd(FftYArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int n = A.F.n;
   double2* tw = reinterpret_cast<double2*>(smem_raw);
-  const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
+  const int slot = threadIdx.x / YTPS, st = threadIdx.x - slot * YTPS;
   double2* buf = tw + A.ntw + (size_t)slot * A.rb * n;
-  for (int i = threadIdx.x; i < A.ntw; i += FFT_THREADS) tw[i] = A.tw[i];
+  for (int i = threadIdx.x; i < A.ntw; i += YTHREADS) tw[i] = A.tw[i];
   __syncthreads();
   // rows of the planes l >= lm of each field: per field one contiguous range of ra rows, cut into batches of rb
   int lm = A.lmin ? __ldg(A.lmin) : 0;
   lm = lm < 0 ? 0 : (lm > A.nz ? A.nz : lm);
   const long long ra = (long long)(A.nz - lm) * A.nkx, per_field = (ra + A.rb - 1) / A.rb;
   const long long nbatch = per_field * A.fields;
-  for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
+  for (long long b = (long long)blockIdx.x * YSLOTS + slot; b < nbatch; b += (long long)gridDim.x * YSLOTS) {
     const long long f = b / per_field, j = b - f * per_field;
     const long long row0 = (f * A.nz + lm) * A.nkx + j * A.rb;
     const int nr = (int)((ra - j * A.rb) < A.rb ? (ra - j * A.rb) : A.rb);
     double2* g = A.data + row0 * n;
     const MidStoreDrained mid{slot, st};
-    run_edge<R0, false>(A.F.r[0], g, buf, tw + A.off[0], n, nr, st, mid);
-    slot_barrier(slot);
-    run_inner<R0, R1, R2, false, false>(A, buf, tw, n, nr, st, slot);
+    run_edge<YTPS, R0, false>(A.F.r[0], g, buf, tw + A.off[0], n, nr, st, mid);
+    slot_barrier<YTPS>(slot);
+    run_inner<YTPS, R0, R1, R2, false, false>(A, buf, tw, n, nr, st, slot);
     fence_async_proxy();
-    slot_barrier(slot);
+    slot_barrier<YTPS>(slot);
     if (st == 0) bulk_store(g, buf, (unsigned)nr * n * 16u);
   }
   if (st == 0) bulk_wait_all();
@@ -218,21 +228,21 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_y_fwd(FftYArgs A) {
 // stride) stores its results straight to global memory.  As soon as that stage has read the row, the slot's next bulk
 // load is issued, so it flies during the last stage's arithmetic and stores.
 template <int R0, int R1, int R2>
-__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_y_inv(FftYArgs A) {
+__global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_inv(FftYArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int n = A.F.n;
   double2* tw = reinterpret_cast<double2*>(smem_raw);
-  const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
+  const int slot = threadIdx.x / YTPS, st = threadIdx.x - slot * YTPS;
   double2* buf = tw + A.ntw + (size_t)slot * A.rb * n;
-  uint64_t* mbar = reinterpret_cast<uint64_t*>(tw + A.ntw + (size_t)NSLOT * A.rb * n) + slot;
-  for (int i = threadIdx.x; i < A.ntw; i += FFT_THREADS) tw[i] = A.tw[i];
+  uint64_t* mbar = reinterpret_cast<uint64_t*>(tw + A.ntw + (size_t)YSLOTS * A.rb * n) + slot;
+  for (int i = threadIdx.x; i < A.ntw; i += YTHREADS) tw[i] = A.tw[i];
   if (st == 0) mbar_init(mbar, 1);
   fence_async_proxy();
   __syncthreads();
   unsigned phase = 0;
   const long long nbatch = (A.rows + A.rb - 1) / A.rb;
-  const long long stride = (long long)gridDim.x * NSLOT;
-  long long b = (long long)blockIdx.x * NSLOT + slot;
+  const long long stride = (long long)gridDim.x * YSLOTS;
+  long long b = (long long)blockIdx.x * YSLOTS + slot;
   if (st == 0 && b < nbatch) {
     const long long row0 = b * A.rb;
     const int nr = (int)((A.rows - row0) < A.rb ? (A.rows - row0) : A.rb);
@@ -245,28 +255,28 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_y_inv(FftYArgs A) {
     double2* g = A.data + row0 * n;
     mbar_wait(mbar, phase);
     phase ^= 1;
-    run_inner<R0, R1, R2, true, true>(A, buf, tw, n, nr, st, slot);
+    run_inner<YTPS, R0, R1, R2, true, true>(A, buf, tw, n, nr, st, slot);
     const long long nrow0 = (b + stride) * A.rb;
     const bool more = b + stride < nbatch;
     const int nnr = more ? (int)((A.rows - nrow0) < A.rb ? (A.rows - nrow0) : A.rb) : 0;
     const MidPrefetch mid{slot, st, mbar, buf, more ? (const void*)(A.data + nrow0 * n) : nullptr, (unsigned)nnr * n * 16u};
-    run_edge<R0, true>(A.F.r[0], buf, g, tw + A.off[0], n, nr, st, mid);
+    run_edge<YTPS, R0, true>(A.F.r[0], buf, g, tw + A.off[0], n, nr, st, mid);
   }
 }
 
 // ---------------------------------------------------------------------------------------------- pass X forward
 template <int R0, int R1, int R2, bool F32>
-__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
+__global__ void __launch_bounds__(XTHREADS, 1) k_fft_x_fwd(FftXArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int M = A.M, npost = M / 2 + 1;
   double2* tw = reinterpret_cast<double2*>(smem_raw);
   double2* post = tw + A.ntw;
-  const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
+  const int slot = threadIdx.x / XTPS, st = threadIdx.x - slot * XTPS;
   double2* buf = post + npost + (size_t)slot * A.rb * M;
-  unsigned short* pos = reinterpret_cast<unsigned short*>(post + npost + (size_t)NSLOT * A.rb * M);
-  for (int i = threadIdx.x; i < A.ntw; i += FFT_THREADS) tw[i] = A.tw[i];
-  for (int i = threadIdx.x; i < M; i += FFT_THREADS) pos[i] = A.pos[i];
-  for (int i = threadIdx.x; i < npost; i += FFT_THREADS) post[i] = A.post[i];
+  unsigned short* pos = reinterpret_cast<unsigned short*>(post + npost + (size_t)XSLOTS * A.rb * M);
+  for (int i = threadIdx.x; i < A.ntw; i += XTHREADS) tw[i] = A.tw[i];
+  for (int i = threadIdx.x; i < M; i += XTHREADS) pos[i] = A.pos[i];
+  for (int i = threadIdx.x; i < npost; i += XTHREADS) post[i] = A.post[i];
   __syncthreads();
   const int rb = A.rb, ny = A.ny, nkx = M + 1;
   int lm = A.lmin ? __ldg(A.lmin) : 0;
@@ -274,19 +284,19 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
   const int act = A.nz - lm, bpp = ny / rb;              // planes per field that can hold force; batches per plane
   const long long nbatch = (A.planes / A.nz) * act * bpp;
   const MidNone nomid;
-  for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
+  for (long long b = (long long)blockIdx.x * XSLOTS + slot; b < nbatch; b += (long long)gridDim.x * XSLOTS) {
     const long long pa = b / bpp;                        // index among the active planes
     const int y0 = (int)(b - pa * bpp) * rb;
     const long long pl = (pa / act) * A.nz + lm + pa % act;
     const long long row0 = pl * ny + y0;                 // flat row index over (plane, y)
     // a real row of nx doubles is read as M complex numbers z[m] = x[2m] + i x[2m+1]
-    if constexpr (F32) run_edge<R0, false>(A.F.r[0], reinterpret_cast<const float2*>(reinterpret_cast<const float*>(A.real) + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
-    else run_edge<R0, false>(A.F.r[0], reinterpret_cast<const double2*>(A.real + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
-    slot_barrier(slot);
-    run_inner<R0, R1, R2, false, true>(A, buf, tw, M, rb, st, slot);
+    if constexpr (F32) run_edge<XTPS, R0, false>(A.F.r[0], reinterpret_cast<const float2*>(reinterpret_cast<const float*>(A.real) + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
+    else run_edge<XTPS, R0, false>(A.F.r[0], reinterpret_cast<const double2*>(A.real + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
+    slot_barrier<XTPS>(slot);
+    run_inner<XTPS, R0, R1, R2, false, true>(A, buf, tw, M, rb, st, slot);
     // split into the spectra of the real rows and write them transposed: T[pl][kx][y0 + r]
     double2* out = A.cplx + (size_t)pl * nkx * ny + y0;
-    for (int idx = st; idx < npost * rb; idx += TPS) {
+    for (int idx = st; idx < npost * rb; idx += XTPS) {
       const int k = idx / rb, r = idx - k * rb;
       const int km = (k == 0) ? 0 : M - k;
       const double2 z1 = buf[r * M + pos[k]], z2 = buf[r * M + pos[km]];
@@ -296,28 +306,28 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_fwd(FftXArgs A) {
       out[(size_t)k * ny + r] = cadd(E, B);
       if (2 * k != M) out[(size_t)(M - k) * ny + r] = make_double2(E.x - B.x, -(E.y - B.y));
     }
-    slot_barrier(slot);                                  // every read of buf is done before the next batch overwrites it
+    slot_barrier<XTPS>(slot);                                  // every read of buf is done before the next batch overwrites it
   }
 }
 
 // ---------------------------------------------------------------------------------------------- pass X inverse
 template <int R0, int R1, int R2, bool F32>
-__global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_inv(FftXArgs A) {
+__global__ void __launch_bounds__(XTHREADS, 1) k_fft_x_inv(FftXArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int M = A.M, npost = M / 2 + 1;
   double2* tw = reinterpret_cast<double2*>(smem_raw);
   double2* post = tw + A.ntw;
-  const int slot = threadIdx.x / TPS, st = threadIdx.x - slot * TPS;
+  const int slot = threadIdx.x / XTPS, st = threadIdx.x - slot * XTPS;
   double2* buf = post + npost + (size_t)slot * A.rb * M;
-  unsigned short* pos = reinterpret_cast<unsigned short*>(post + npost + (size_t)NSLOT * A.rb * M);
-  for (int i = threadIdx.x; i < A.ntw; i += FFT_THREADS) tw[i] = A.tw[i];
-  for (int i = threadIdx.x; i < M; i += FFT_THREADS) pos[i] = A.pos[i];
-  for (int i = threadIdx.x; i < npost; i += FFT_THREADS) post[i] = A.post[i];
+  unsigned short* pos = reinterpret_cast<unsigned short*>(post + npost + (size_t)XSLOTS * A.rb * M);
+  for (int i = threadIdx.x; i < A.ntw; i += XTHREADS) tw[i] = A.tw[i];
+  for (int i = threadIdx.x; i < M; i += XTHREADS) pos[i] = A.pos[i];
+  for (int i = threadIdx.x; i < npost; i += XTHREADS) post[i] = A.post[i];
   __syncthreads();
   const int rb = A.rb, ny = A.ny, nkx = M + 1;
   const long long nbatch = A.planes * (ny / rb);
   const MidNone nomid;
-  for (long long b = (long long)blockIdx.x * NSLOT + slot; b < nbatch; b += (long long)gridDim.x * NSLOT) {
+  for (long long b = (long long)blockIdx.x * XSLOTS + slot; b < nbatch; b += (long long)gridDim.x * XSLOTS) {
     const long long row0 = b * rb;
     const long long pl = row0 / ny;
     const int y0 = (int)(row0 - pl * ny);
@@ -335,31 +345,31 @@ __global__ void __launch_bounds__(FFT_THREADS, 1) k_fft_x_inv(FftXArgs A) {
       }
     };
     if constexpr (R0 > 0) {
-      constexpr int Ms = R0 * R1 * R2, RB = SLOT_ELEMS / Ms, ITEMS = (Ms / 2 + 1) * RB, NIT = (ITEMS + TPS - 1) / TPS;
+      constexpr int Ms = R0 * R1 * R2, RB = SLOT_ELEMS / Ms, ITEMS = (Ms / 2 + 1) * RB, NIT = (ITEMS + XTPS - 1) / XTPS;
       double2 X1[NIT], X2[NIT];
 #pragma unroll
       for (int i = 0; i < NIT; ++i) {
-        const int idx = st + i * TPS, k = idx / RB, r = idx - k * RB;
+        const int idx = st + i * XTPS, k = idx / RB, r = idx - k * RB;
         if (idx < ITEMS) { X1[i] = __ldg(in + (size_t)k * ny + r); X2[i] = __ldg(in + (size_t)(Ms - k) * ny + r); }
       }
 #pragma unroll
       for (int i = 0; i < NIT; ++i) {
-        const int idx = st + i * TPS, k = idx / RB, r = idx - k * RB;
+        const int idx = st + i * XTPS, k = idx / RB, r = idx - k * RB;
         if (idx < ITEMS) put(k, r, X1[i], X2[i]);
       }
     } else {
 #pragma unroll 4
-      for (int idx = st; idx < npost * rb; idx += TPS) {
+      for (int idx = st; idx < npost * rb; idx += XTPS) {
         const int k = idx / rb, r = idx - k * rb;
         put(k, r, __ldg(in + (size_t)k * ny + r), __ldg(in + (size_t)(M - k) * ny + r));
       }
     }
-    slot_barrier(slot);
-    run_inner<R0, R1, R2, true, true>(A, buf, tw, M, rb, st, slot);
+    slot_barrier<XTPS>(slot);
+    run_inner<XTPS, R0, R1, R2, true, true>(A, buf, tw, M, rb, st, slot);
     // last stage: results go straight to the real grid rows (z[m] = x[2m] + i x[2m+1])
-    if constexpr (F32) run_edge<R0, true>(A.F.r[0], (const double2*)buf, reinterpret_cast<float2*>(reinterpret_cast<float*>(A.real) + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
-    else run_edge<R0, true>(A.F.r[0], (const double2*)buf, reinterpret_cast<double2*>(A.real + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
-    slot_barrier(slot);                                  // the stage has read buf before the next batch refills it
+    if constexpr (F32) run_edge<XTPS, R0, true>(A.F.r[0], (const double2*)buf, reinterpret_cast<float2*>(reinterpret_cast<float*>(A.real) + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
+    else run_edge<XTPS, R0, true>(A.F.r[0], (const double2*)buf, reinterpret_cast<double2*>(A.real + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
+    slot_barrier<XTPS>(slot);                                  // the stage has read buf before the next batch refills it
   }
 }
 
@@ -405,9 +415,9 @@ template <class T> cudaError_t upload(T** dst, const std::vector<T>& v, dp_plan*
   return cudaMemcpy(*dst, v.data(), sizeof(T) * v.size(), cudaMemcpyHostToDevice);
 }
 
-size_t smem_bytes_y(int n, int ntw, int rb) { return sizeof(double2) * ((size_t)ntw + (size_t)NSLOT * rb * n) + 8 * NSLOT; }
+size_t smem_bytes_y(int n, int ntw, int rb) { return sizeof(double2) * ((size_t)ntw + (size_t)YSLOTS * rb * n) + 8 * YSLOTS; }
 size_t smem_bytes_x(int M, int ntw, int rb) {
-  return sizeof(double2) * ((size_t)ntw + (M / 2 + 1) + (size_t)NSLOT * rb * M) + align16(sizeof(unsigned short) * M) + 8 * NSLOT;
+  return sizeof(double2) * ((size_t)ntw + (M / 2 + 1) + (size_t)XSLOTS * rb * M) + align16(sizeof(unsigned short) * M) + 8 * XSLOTS;
 }
 
 #ifdef DP_FFT_TUNING
@@ -518,30 +528,32 @@ static FftYArgs y_args(dp_plan* P, int nfields) {
   for (int j = 0; j < MAX_STAGES; ++j) A.off[j] = O->off_y[j];
   return A;
 }
-static int grid_for(const dp_fft_own* O, long long nbatch) {
-  const long long need = (nbatch + NSLOT - 1) / NSLOT;
+static int grid_for(const dp_fft_own* O, long long nbatch, int nslot) {
+  const long long need = (nbatch + nslot - 1) / nslot;
   return (int)(need < O->grid ? (need < 1 ? 1 : need) : O->grid);
 }
 
 cudaError_t dp_fft_own_forward(dp_plan* P, int nfields, cudaStream_t st) {
   dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
   const FftXArgs X = x_args(P, nfields);
-  O->kx_fwd<<<grid_for(O, X.planes * (X.ny / X.rb)), FFT_THREADS, O->smem_x, st>>>(X);
+  O->kx_fwd<<<grid_for(O, X.planes * (X.ny / X.rb), XSLOTS), XTHREADS, O->smem_x, st>>>(X);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
+  if (P->profiling && P->ev_ok && (e = cudaEventRecord(P->ev_fft[0], st)) != cudaSuccess) return e;
   const FftYArgs Y = y_args(P, nfields);
-  O->ky_fwd<<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb), FFT_THREADS, O->smem_y, st>>>(Y);
+  O->ky_fwd<<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb, YSLOTS), YTHREADS, O->smem_y, st>>>(Y);
   return cudaGetLastError();
 }
 
 cudaError_t dp_fft_own_inverse(dp_plan* P, int nfields, cudaStream_t st) {
   dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
   const FftYArgs Y = y_args(P, nfields);
-  O->ky_inv<<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb), FFT_THREADS, O->smem_y, st>>>(Y);
+  O->ky_inv<<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb, YSLOTS), YTHREADS, O->smem_y, st>>>(Y);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
+  if (P->profiling && P->ev_ok && (e = cudaEventRecord(P->ev_fft[1], st)) != cudaSuccess) return e;
   const FftXArgs X = x_args(P, nfields);
-  O->kx_inv<<<grid_for(O, X.planes * (X.ny / X.rb)), FFT_THREADS, O->smem_x, st>>>(X);
+  O->kx_inv<<<grid_for(O, X.planes * (X.ny / X.rb), XSLOTS), XTHREADS, O->smem_x, st>>>(X);
   return cudaGetLastError();
 }
 

@@ -319,7 +319,7 @@ int dp_destroy(dp_plan* P) {
   void* bufs[] = {P->d_real, P->d_cplx, P->d_fft_work, P->d_znodes, P->d_zweights, P->d_pos_s, P->d_frc_s, P->d_trq_s, P->d_perm, P->d_meta, P->d_wrec,
                   P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_bin_start, P->d_flag, P->d_lmin};
   for (void* b : bufs) if (b) cudaFree(b);
-  if (P->ev_ok) for (auto& e : P->ev) cudaEventDestroy(e);
+  if (P->ev_ok) { for (auto& e : P->ev) cudaEventDestroy(e); for (auto& e : P->ev_fft) cudaEventDestroy(e); }
   if (P->host_stage) {
     dp_host_stage* hs = static_cast<dp_host_stage*>(P->host_stage);
     hs->release();
@@ -426,6 +426,7 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   {
     bool ok = true;
     for (auto& e : P->ev) ok = ok && (cudaEventCreate(&e) == cudaSuccess);
+    for (auto& e : P->ev_fft) ok = ok && (cudaEventCreate(&e) == cudaSuccess);
     P->ev_ok = ok;
   }
   ce = cudaDeviceSynchronize();
@@ -479,6 +480,19 @@ int dp_stage_ms(dp_plan* P, float* ms) {
   for (int i = 0; i < 6; ++i) CK(cudaEventElapsedTime(&ms[i], P->ev[i], P->ev[i + 1]));
   ms[6] = 0.f;   // the k = 0 kernel is launched inside the solve stage
   CK(cudaEventElapsedTime(&ms[7], P->ev[0], P->ev[6]));
+  return DP_OK;
+}
+
+int dp_fft_pass_ms(dp_plan* P, float* ms) {
+  if (!P || !ms) return DP_EINVAL;
+  for (int i = 0; i < 4; ++i) ms[i] = 0.f;
+  if (!P->ev_recorded || !P->own_fft) { set_err(P, "dp_fft_pass_ms", "no profiled apply with the own FFT passes recorded"); return DP_EINVAL; }
+  DeviceGuard guard(P->p.device);
+  CK(cudaEventSynchronize(P->ev[6]));
+  CK(cudaEventElapsedTime(&ms[0], P->ev[2], P->ev_fft[0]));
+  CK(cudaEventElapsedTime(&ms[1], P->ev_fft[0], P->ev[3]));
+  CK(cudaEventElapsedTime(&ms[2], P->ev[4], P->ev_fft[1]));
+  CK(cudaEventElapsedTime(&ms[3], P->ev_fft[1], P->ev[5]));
   return DP_OK;
 }
 

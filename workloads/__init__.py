@@ -138,6 +138,31 @@ def monolayer_slit(n=262144, nz=48, H=6.0, margin=1.2, seed=1004, name="cfg4"):
     return prob, _pack(_xy(seed, n, L, L), z), F, T
 
 
+def paper_fig9(replicas: int = 18, dipole: bool = False, seed: int = 1009, name: str | None = None):
+    """Stand-in for the paper's own performance workload (Fig. 9 and Table III): a tile of 2048 particles of
+    size L = 128.8 R_h, replicated ``replicas`` x ``replicas`` times in the plane (18 x 18 = 663,552 particles is its largest case),
+    area fraction 0.4, two layers of heights above the wall ("bimodal", the inset of Fig. 9), H = 9.1 R_h (M) / 9.2 R_h (M & D).
+    Grid and kernels are Table III's: M (forces only): Nz = 19, Nxy = 150 per tile, m = 4, beta/m = 1.87;  M & D: Nz = 26,
+    Nxy = 216 per tile, m = 6, beta_M/m = 1.38, beta_D/m = 2.3.  R_h = 1.  The tile of ref. [22] itself is not in the container:
+    positions are drawn uniformly (not replicated), heights 1 + Exp(0.3) for two thirds of the particles and N(3.2, 0.3^2) for
+    the rest, clipped to [0.8, H - alpha]."""
+    n = 2048 * replicas * replicas
+    L = 128.8 * replicas
+    if dipole:
+        H, nz, nxy, w, bM, bD = 9.2, 26, 216 * replicas, 6, 6 * 1.38, 6 * 2.3
+    else:
+        H, nz, nxy, w, bM, bD = 9.1, 19, 150 * replicas, 4, 4 * 1.87, 0.0
+    prob = Problem(name or ("fig9-%s-%dx%d" % ("MD" if dipole else "M", replicas, replicas)), BOTTOM_WALL, L, L, H, nxy, nxy, nz, w, bM, bD,
+                   has_torque=dipole, seed=seed, n=n)
+    g = _rng(seed, 1)
+    low = 1.0 + g.exponential(0.3, n)
+    high = g.normal(3.2, 0.3, n)
+    z = np.where(g.uniform(0.0, 1.0, n) < 2.0 / 3.0, low, high)
+    z = np.clip(z, 0.8, H - prob.alpha)
+    F, T = _roller_drive(seed, n)
+    return prob, _pack(_xy(seed, n, L, L), z), F, (T if dipole else None)
+
+
 def config(i: int):
     """BASELINE.json ``configs[i-1]`` (1-based, as SURVEY.md numbers them)."""
     if i == 1:
