@@ -24,6 +24,7 @@ constexpr int SPREAD_THREADS = TX * TY * ZSPLIT;
 constexpr int PCH = 40;                         // candidate particles staged per chunk
 constexpr int MAXB = 6;                         // origin bins per direction that can reach a tile (w <= 8, TY = 4)
 constexpr int MAXR = 2 * MAXB;                  // candidate ranges per tile: one per bin row, two when the x range wraps
+constexpr int MAXKEEP = SPREAD_THREADS;         // survivors of one block of candidates
 
 struct GridGeom {
   int nx, ny, nz, w, wall_mode, nbx, nby;
@@ -230,9 +231,10 @@ struct SpreadArgs {
 // One CTA = one tile of TX x TY grid columns of one field triple.  Thread (ti, tj, tz) owns column (ti, tj) and the
 // planes l = ZSPLIT*li + tz; its 3*NZ/ZSPLIT partial sums live in registers for the whole kernel, so there is no
 // shared-memory tile, no atomic and no memset.  The candidates (the bins whose footprints can reach the tile, merged
-// into contiguous ranges of the sorted arrays) are staged in shared memory with their footprint and weight records;
-// every thread adds the particles covering its column; each grid value is stored to HBM exactly once (128-byte row
-// segments per warp).  Dependent global round trips per CTA: bin_start -> candidate records -> stores.
+// into contiguous ranges of the sorted arrays) are culled by their footprint records; the survivors are staged in shared
+// memory with their weight records; every thread adds the particles covering its column; each grid value is stored to HBM
+// exactly once (128-byte row segments per warp).  Dependent global round trips per CTA: bin_start -> footprint records ->
+// weight records -> stores.
 // GT = double, or float for the optional fp32 variant (accumulators and grid in fp32; the weight records stay fp64 and are
 // rounded when they are used).
 // MODE 0: field triple blockIdx.z (0: forces with Delta_M, 1: torques with Delta_D) gets sum_j val_j S(j; g)   (eq 7 without the curl,
@@ -249,8 +251,9 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
   __shared__ double s_w[PC][NREC][WS];
   __shared__ double s_val[PC][NV];
   __shared__ int4 s_meta[PC];                 // i0, j0 (wrapped origin node), lmin, lmax
-  __shared__ int s_src[PC];                   // index of each staged candidate in the sorted particle arrays
   __shared__ int s_rbeg[MAXR], s_roff[MAXR + 1];   // candidate ranges in the sorted arrays; prefix sums of their lengths
+  __shared__ int s_keep[MAXKEEP];             // candidates whose footprint really touches the tile
+  __shared__ int s_nkeep;
 
   const GridGeom& g = A.g;
   const int w = g.w;
@@ -289,100 +292,125 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
     if (lane < MAXR) { s_rbeg[lane] = beg; s_roff[lane + 1] = incl; }
     if (lane == 0) s_roff[0] = 0;
   }
+  if (t == 0) s_nkeep = 0;
   __syncthreads();
   const int total = s_roff[MAXR];
 
-  // Every candidate is staged (no cull pass: the candidates of a range are contiguous, so their records arrive in one
-  // batch of independent coalesced loads); the exact footprint test happens per thread in the accumulation loop.
-  for (int c0 = 0; c0 < total; c0 += PC) {
-    const int nl = min(PC, total - c0);
-    if (t < nl) {                                             // position of candidate c0 + t in the sorted arrays, once
-      const int c = c0 + t;
-      int r = 0;
+  // Cull: the ranges hold every particle whose footprint ORIGIN lies in a bin that can reach the tile (2-3 times as many as
+  // really touch it).  Blocks of 256 candidates: one pass over their footprint records keeps the ones whose w x w footprint
+  // intersects the tile's columns (warp ballot + one shared-memory counter update per warp; the order of the survivors, hence
+  // the summation order, is not fixed), then the survivors are staged with their weight records in chunks of PC and every
+  // thread adds the ones covering its column to its own planes.
+  const int TXe = min(TX, g.nx - X0), TYe = min(TY, g.ny - Y0);
+  for (int blk = 0; blk < total; blk += SPREAD_THREADS) {
+    {
+      const int c = blk + t;
+      bool keep = false;
+      int src = 0;
+      if (c < total) {
+        int r = 0;
 #pragma unroll
-      for (int q = 1; q < MAXR; ++q) r += (c >= s_roff[q]) ? 1 : 0;
-      s_src[t] = s_rbeg[r] + (c - s_roff[r]);
-    }
-    __syncthreads();
-    if (t < nl) {
-      const int p = s_src[t];
-      s_meta[t] = A.meta[p];
-      if (MODE) {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) { s_val[t][c] = A.val_s[0][3 * (size_t)p + c]; s_val[t][3 + c] = A.val_s[1][3 * (size_t)p + c]; }
-      } else {
-        const double* __restrict__ val = A.val_s[grp];
-        s_val[t][0] = val[3 * (size_t)p]; s_val[t][1] = val[3 * (size_t)p + 1]; s_val[t][2] = val[3 * (size_t)p + 2];
+        for (int q = 1; q < MAXR; ++q) r += (c >= s_roff[q]) ? 1 : 0;
+        src = s_rbeg[r] + (c - s_roff[r]);
+        const int4 m = A.meta[src];
+        int dx = X0 - m.x; if (dx < 0) dx += g.nx;          // tile start seen from the footprint origin
+        int ex = m.x - X0; if (ex < 0) ex += g.nx;          // footprint origin seen from the tile start
+        int dy = Y0 - m.y; if (dy < 0) dy += g.ny;
+        int ey = m.y - Y0; if (ey < 0) ey += g.ny;
+        keep = (m.z <= m.w) && (dx < w || ex < TXe) && (dy < w || ey < TYe);
       }
-    }
-#pragma unroll 2
-    for (int i = t; i < nl * NREC * WS; i += SPREAD_THREADS) {
-      const int q = i / (NREC * WS), rem = i - q * (NREC * WS), k = rem / WS, e = rem - k * WS;
-      const int kk = MODE ? k : grp;
-      s_w[q][k][e] = e < WREC ? A.wrec[((size_t)kk * A.cap + s_src[q]) * WREC + e] : 0.0;
+      const unsigned bal = __ballot_sync(0xffffffffu, keep);
+      int base = 0;
+      if (lane == 0 && bal) base = atomicAdd(&s_nkeep, __popc(bal));
+      base = __shfl_sync(0xffffffffu, base, 0);
+      if (keep) s_keep[base + __popc(bal & ((1u << lane) - 1))] = src;
     }
     __syncthreads();
-    // ---- accumulate: each thread adds the particles covering its column to its own planes
-    if (in_grid) {
-      for (int q = 0; q < nl; ++q) {
-        const int4 m = s_meta[q];
-        int a = gi - m.x; if (a < 0) a += g.nx;
-        int bb = gj - m.y; if (bb < 0) bb += g.ny;
-        if (a < w && bb < w && m.z <= m.w) {
-          if (MODE == 0) {
-            const GT wxy = (GT)s_w[q][0][a] * (GT)s_w[q][0][DP_MAX_W + bb];
-            const GT v0 = (GT)s_val[q][0] * wxy, v1 = (GT)s_val[q][1] * wxy, v2 = (GT)s_val[q][2] * wxy;
-            const double* zt = &s_w[q][0][2 * DP_MAX_W + tz];
-            // zeta vanishes outside [lmin, lmax]: skipping a half of the planes that lies outside is exact
-            if (m.z < ZSPLIT * (NL / 2)) {
+    const int nkeep = s_nkeep;
+    for (int c0 = 0; c0 < nkeep; c0 += PC) {
+      const int nl = min(PC, nkeep - c0);
+      if (t < nl) {
+        const int p = s_keep[c0 + t];
+        s_meta[t] = A.meta[p];
+        if (MODE) {
 #pragma unroll
-              for (int li = 0; li < NL / 2; ++li) {
-                const GT z = (GT)zt[ZSPLIT * li];
-                acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+          for (int c = 0; c < 3; ++c) { s_val[t][c] = A.val_s[0][3 * (size_t)p + c]; s_val[t][3 + c] = A.val_s[1][3 * (size_t)p + c]; }
+        } else {
+          const double* __restrict__ val = A.val_s[grp];
+          s_val[t][0] = val[3 * (size_t)p]; s_val[t][1] = val[3 * (size_t)p + 1]; s_val[t][2] = val[3 * (size_t)p + 2];
+        }
+      }
+#pragma unroll 2
+      for (int i = t; i < nl * NREC * WS; i += SPREAD_THREADS) {
+        const int q = i / (NREC * WS), rem = i - q * (NREC * WS), k = rem / WS, e = rem - k * WS;
+        const int kk = MODE ? k : grp;
+        s_w[q][k][e] = e < WREC ? A.wrec[((size_t)kk * A.cap + s_keep[c0 + q]) * WREC + e] : 0.0;
+      }
+      __syncthreads();
+      // ---- accumulate: each thread adds the particles covering its column to its own planes
+      if (in_grid) {
+        for (int q = 0; q < nl; ++q) {
+          const int4 m = s_meta[q];
+          int a = gi - m.x; if (a < 0) a += g.nx;
+          int bb = gj - m.y; if (bb < 0) bb += g.ny;
+          if (a < w && bb < w) {
+            if (MODE == 0) {
+              const GT wxy = (GT)s_w[q][0][a] * (GT)s_w[q][0][DP_MAX_W + bb];
+              const GT v0 = (GT)s_val[q][0] * wxy, v1 = (GT)s_val[q][1] * wxy, v2 = (GT)s_val[q][2] * wxy;
+              const double* zt = &s_w[q][0][2 * DP_MAX_W + tz];
+              // zeta vanishes outside [lmin, lmax]: skipping a half of the planes that lies outside is exact
+              if (m.z < ZSPLIT * (NL / 2)) {
+#pragma unroll
+                for (int li = 0; li < NL / 2; ++li) {
+                  const GT z = (GT)zt[ZSPLIT * li];
+                  acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+                }
               }
-            }
-            if (m.w >= ZSPLIT * (NL / 2)) {
+              if (m.w >= ZSPLIT * (NL / 2)) {
 #pragma unroll
-              for (int li = NL / 2; li < NL; ++li) {
-                const GT z = (GT)zt[ZSPLIT * li];
-                acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+                for (int li = NL / 2; li < NL; ++li) {
+                  const GT z = (GT)zt[ZSPLIT * li];
+                  acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+                }
               }
-            }
-          } else {
-            const double* wM = s_w[q][0]; const double* wD = s_w[q][MODE ? 1 : 0]; const double* wG = s_w[q][MODE ? 2 : 0];
-            const GT pM = (GT)wM[a] * (GT)wM[DP_MAX_W + bb];
-            const GT c0 = (GT)s_val[q][0] * pM, c1 = (GT)s_val[q][1] * pM, c2 = (GT)s_val[q][2] * pM;     // x zeta_M(l)
-            const GT tx = (GT)s_val[q][NV - 3], ty = (GT)s_val[q][NV - 2], tzq = (GT)s_val[q][NV - 1];
-            const GT pxy = (GT)wD[a] * (GT)wD[DP_MAX_W + bb];                   // phi(x) phi(y)
-            const GT dxy = (GT)wG[a] * (GT)wD[DP_MAX_W + bb];                   // phi'(x) phi(y)
-            const GT xdy = (GT)wD[a] * (GT)wG[DP_MAX_W + bb];                   // phi(x) phi'(y)
-            // (1/2) G x tau with G = (dxy zeta, xdy zeta, pxy zeta'):  coefficients of zeta_D(l) and of zeta_D'(l)
-            const GT a0 = (GT)0.5 * tzq * xdy, a1 = -(GT)0.5 * tzq * dxy, a2 = (GT)0.5 * (ty * dxy - tx * xdy);
-            const GT b0 = -(GT)0.5 * ty * pxy, b1 = (GT)0.5 * tx * pxy;
-            const double* zm = &wM[2 * DP_MAX_W + tz]; const double* zd = &wD[2 * DP_MAX_W + tz]; const double* zg = &wG[2 * DP_MAX_W + tz];
-            if (m.z < ZSPLIT * (NL / 2)) {
+            } else {
+              const double* wM = s_w[q][0]; const double* wD = s_w[q][MODE ? 1 : 0]; const double* wG = s_w[q][MODE ? 2 : 0];
+              const GT pM = (GT)wM[a] * (GT)wM[DP_MAX_W + bb];
+              const GT c0f = (GT)s_val[q][0] * pM, c1f = (GT)s_val[q][1] * pM, c2f = (GT)s_val[q][2] * pM;     // x zeta_M(l)
+              const GT tx = (GT)s_val[q][NV - 3], ty = (GT)s_val[q][NV - 2], tzq = (GT)s_val[q][NV - 1];
+              const GT pxy = (GT)wD[a] * (GT)wD[DP_MAX_W + bb];                   // phi(x) phi(y)
+              const GT dxy = (GT)wG[a] * (GT)wD[DP_MAX_W + bb];                   // phi'(x) phi(y)
+              const GT xdy = (GT)wD[a] * (GT)wG[DP_MAX_W + bb];                   // phi(x) phi'(y)
+              // (1/2) G x tau with G = (dxy zeta, xdy zeta, pxy zeta'):  coefficients of zeta_D(l) and of zeta_D'(l)
+              const GT a0 = (GT)0.5 * tzq * xdy, a1 = -(GT)0.5 * tzq * dxy, a2 = (GT)0.5 * (ty * dxy - tx * xdy);
+              const GT b0 = -(GT)0.5 * ty * pxy, b1 = (GT)0.5 * tx * pxy;
+              const double* zm = &wM[2 * DP_MAX_W + tz]; const double* zd = &wD[2 * DP_MAX_W + tz]; const double* zg = &wG[2 * DP_MAX_W + tz];
+              if (m.z < ZSPLIT * (NL / 2)) {
 #pragma unroll
-              for (int li = 0; li < NL / 2; ++li) {
-                const GT zM = (GT)zm[ZSPLIT * li], zD = (GT)zd[ZSPLIT * li], zG = (GT)zg[ZSPLIT * li];
-                acc[li][0] = fma(c0, zM, fma(a0, zD, fma(b0, zG, acc[li][0])));
-                acc[li][1] = fma(c1, zM, fma(a1, zD, fma(b1, zG, acc[li][1])));
-                acc[li][2] = fma(c2, zM, fma(a2, zD, acc[li][2]));
+                for (int li = 0; li < NL / 2; ++li) {
+                  const GT zM = (GT)zm[ZSPLIT * li], zD = (GT)zd[ZSPLIT * li], zG = (GT)zg[ZSPLIT * li];
+                  acc[li][0] = fma(c0f, zM, fma(a0, zD, fma(b0, zG, acc[li][0])));
+                  acc[li][1] = fma(c1f, zM, fma(a1, zD, fma(b1, zG, acc[li][1])));
+                  acc[li][2] = fma(c2f, zM, fma(a2, zD, acc[li][2]));
+                }
               }
-            }
-            if (m.w >= ZSPLIT * (NL / 2)) {
+              if (m.w >= ZSPLIT * (NL / 2)) {
 #pragma unroll
-              for (int li = NL / 2; li < NL; ++li) {
-                const GT zM = (GT)zm[ZSPLIT * li], zD = (GT)zd[ZSPLIT * li], zG = (GT)zg[ZSPLIT * li];
-                acc[li][0] = fma(c0, zM, fma(a0, zD, fma(b0, zG, acc[li][0])));
-                acc[li][1] = fma(c1, zM, fma(a1, zD, fma(b1, zG, acc[li][1])));
-                acc[li][2] = fma(c2, zM, fma(a2, zD, acc[li][2]));
+                for (int li = NL / 2; li < NL; ++li) {
+                  const GT zM = (GT)zm[ZSPLIT * li], zD = (GT)zd[ZSPLIT * li], zG = (GT)zg[ZSPLIT * li];
+                  acc[li][0] = fma(c0f, zM, fma(a0, zD, fma(b0, zG, acc[li][0])));
+                  acc[li][1] = fma(c1f, zM, fma(a1, zD, fma(b1, zG, acc[li][1])));
+                  acc[li][2] = fma(c2f, zM, fma(a2, zD, acc[li][2]));
+                }
               }
             }
           }
         }
       }
+      __syncthreads();
     }
-    if (c0 + PC < total) __syncthreads();
+    if (t == 0) s_nkeep = 0;
+    __syncthreads();
   }
   // ---- store: every grid value of the planes that can hold force written exactly once
   if (in_grid) {
