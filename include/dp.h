@@ -104,6 +104,15 @@ int dp_mobility_apply(dp_plan* plan, int n, const double* pos, const double* for
 int dp_mobility_apply_host(dp_plan* plan, int n, const double* pos, const double* force, const double* torque,
                            double* U, double* Omega);
 
+/* Brownian "velocities" g = M^{1/2} W (Sec. V B): Lanczos iteration in the Krylov subspace of the mobility
+ * operator, one dp_mobility_apply per iteration, until eps_n = |g_n - g_{n-1}| / |g_{n-1}| < tol (the quantity of Fig. 11,
+ * PAPER.md:527) or max_iter (<= 64) products.  DEVICE pointers [n][3]: W_force required, W_torque or NULL (then the
+ * translational block only: U = M^{tt} F); g_U required, g_Omega given iff W_torque is.  *iters receives the number of products,
+ * eps_hist[0 .. *iters - 2] (HOST, may be NULL) receives eps_2, eps_3, ...  Synchronous (every iteration reads two scalars back);
+ * allocates (max_iter + 2) work vectors for the duration of the call. */
+int dp_lanczos_sqrt(dp_plan* plan, int n, const double* pos, const double* W_force, const double* W_torque, double* g_U,
+                    double* g_Omega, double tol, int max_iter, int* iters, double* eps_hist, void* cuda_stream);
+
 /* Domain check of the last product: "kernels must never extend outside open boundaries" (footnote 44) and
  * 0 <= z <= H.  Synchronises the last stream used; DP_EDOMAIN if any particle of the last apply was out of domain. */
 int dp_check(dp_plan* plan);

@@ -322,3 +322,44 @@ def mobility_apply(prob, pos, force=None, torque=None, want_omega=None, dft="nai
     if keep:
         stages.update(u=u, om=om)
     return U, Om
+
+
+# ---- Lanczos square root (Sec. V B) ------------------------------------------------------------
+def lanczos_sqrt(apply, W, tol: float = 1e-3, max_iter: int = 50):
+    """g ~ M^{1/2} W in the Krylov subspace of the symmetric positive definite operator ``apply`` ("A Lanczos iterative
+    algorithm [37] can be used to estimate g in the Krylov subspace of M"), step by step:
+
+        v_1 = W/|W|;   for n = 1, 2, ...:   w = M v_n - beta_{n-1} v_{n-1};  alpha_n = w.v_n;  w -= alpha_n v_n;
+        beta_n = |w|;  v_{n+1} = w/beta_n;   T_n = tridiag(beta, alpha, beta) (n x n);   g_n = |W| V_n T_n^{1/2} e_1;
+        eps_n = |g_n - g_{n-1}| / |g_{n-1}|   (the quantity of Fig. 11);   stop when eps_n < tol.
+
+    T_n^{1/2} through the symmetric eigendecomposition of T_n (library primitive numpy.linalg.eigh).  No reorthogonalisation.
+    ``apply`` maps a flat vector to a flat vector.  Returns (g, number of products, [eps_2, eps_3, ...])."""
+    W = np.asarray(W, dtype=np.float64).ravel()
+    nrm = float(np.linalg.norm(W))
+    V = [W / nrm]
+    alpha, beta, eps_hist = [], [], []
+    g_prev = None
+    g = None
+    for n in range(1, max_iter + 1):
+        w = np.asarray(apply(V[n - 1]), dtype=np.float64).ravel().copy()
+        if n > 1:
+            w -= beta[n - 2] * V[n - 2]
+        a = float(w @ V[n - 1])
+        w -= a * V[n - 1]
+        b = float(np.linalg.norm(w))
+        alpha.append(a); beta.append(b)
+        T = np.diag(alpha) + np.diag(beta[:n - 1], 1) + np.diag(beta[:n - 1], -1)
+        lam, Q = np.linalg.eigh(T)
+        c = Q @ (np.sqrt(np.maximum(lam, 0.0)) * Q[0, :])            # T^{1/2} e_1
+        g = nrm * sum(ci * vi for ci, vi in zip(c, V))
+        if g_prev is not None:
+            eps = float(np.linalg.norm(g - g_prev) / np.linalg.norm(g_prev))
+            eps_hist.append(eps)
+            if eps < tol:
+                return g, n, eps_hist
+        g_prev = g
+        if b <= 1e-14 * abs(a):                                       # invariant subspace reached: g is exact
+            return g, n, eps_hist
+        V.append(w / b)
+    return g, max_iter, eps_hist

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBNAME = os.path.join(_HERE, "libdpstokes.so")
 
 # every symbol include/dp.h declares
-EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_check", "dp_effective_radius", "dp_set_profiling", "dp_stage_ms", "dp_fft_pass_ms",
+EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_lanczos_sqrt", "dp_check", "dp_effective_radius", "dp_set_profiling", "dp_stage_ms", "dp_fft_pass_ms",
            "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_copy_plane_to_host", "dp_complex_row_pitch", "dp_zero_planes", "dp_fft_backend", "dp_es_norm", "dp_es_radius_over_h",
            "dp_es_dphi_cut", "dp_supported_nz", "dp_device_bytes", "dp_strerror", "dp_last_error", "dp_destroy"]
 
@@ -54,6 +54,8 @@ def load_library():
     L.dp_mobility_apply.restype = i
     L.dp_mobility_apply_host.argtypes = [vp, i, vp, vp, vp, vp, vp]
     L.dp_mobility_apply_host.restype = i
+    L.dp_lanczos_sqrt.argtypes = [vp, i, vp, vp, vp, vp, vp, d, i, ctypes.POINTER(i), ctypes.POINTER(d), vp]
+    L.dp_lanczos_sqrt.restype = i
     L.dp_check.argtypes = [vp]
     L.dp_check.restype = i
     L.dp_set_profiling.argtypes = [vp, i]
@@ -189,6 +191,24 @@ class Plan:
         return U, Om
 
     # -- the product, host arrays (H2D + product + D2H, synchronous)
+    def lanczos_sqrt(self, pos, W_force, W_torque=None, tol: float = 1e-3, max_iter: int = 30, stream=None):
+        """g = M^{1/2} W by the Lanczos iteration.  CUDA tensors [n,3]; returns (g_U, g_Omega or None, iters, eps list)."""
+        import torch
+        n = int(pos.shape[0])
+        for t in (pos, W_force, W_torque):
+            if t is not None:
+                assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == (n, 3)
+        gU = torch.empty((n, 3), dtype=torch.float64, device=pos.device)
+        gO = torch.empty((n, 3), dtype=torch.float64, device=pos.device) if W_torque is not None else None
+        its = ctypes.c_int(0)
+        eps = (ctypes.c_double * max(max_iter, 1))()
+        ptr = lambda t: ctypes.c_void_p(0 if t is None else t.data_ptr())
+        st = torch.cuda.current_stream(pos.device) if stream is None else stream
+        rc = load_library().dp_lanczos_sqrt(self._h, n, ptr(pos), ptr(W_force), ptr(W_torque), ptr(gU), ptr(gO), float(tol), int(max_iter),
+                                            ctypes.byref(its), eps, ctypes.c_void_p(st.cuda_stream))
+        self._ck(rc, "dp_lanczos_sqrt")
+        return gU, gO, int(its.value), [float(eps[k]) for k in range(max(int(its.value) - 1, 0))]
+
     def mobility_apply_host(self, pos, force=None, torque=None, want_omega=None, out_U=None, out_Omega=None):
         if want_omega is None:
             want_omega = torque is not None

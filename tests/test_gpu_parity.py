@@ -439,3 +439,33 @@ def test_every_compiled_chebyshev_size_and_kernel_width(dp, nz, w, wall):
             assert plan.check() == 0
         assert rel_l2(U.cpu().numpy(), U_o) < TOL and rel_l2(Om.cpu().numpy(), Om_o) < TOL, (mode, nz, w)
         assert rel_max(U.cpu().numpy(), U_o) < TOL_MAX and rel_max(Om.cpu().numpy(), Om_o) < TOL_MAX
+
+
+# ------------------------------------------------------------------------------------------------ Lanczos square root
+@pytest.mark.parametrize("with_torque,mode", [(False, 0), (True, 1), (True, 0)])
+def test_lanczos_square_root_matches_the_oracle_iteration(dp, with_torque, mode):
+    """dp_lanczos_sqrt (Sec. V B) against the oracle's Lanczos driven by the oracle's own mobility product: same
+    iteration count, same eps_n history (Fig. 11's quantity), same g."""
+    prob, pos, F, T = small_monolayer("bw", 400, 51)
+    n = len(pos)
+    rng = np.random.default_rng(9)
+    WF = rng.standard_normal((n, 3))
+    WT = rng.standard_normal((n, 3)) if with_torque else None
+    name = "kernel" if mode else "fourier"
+
+    def apply(v):
+        if with_torque:
+            U, Om = oracle.mobility_apply(prob, pos, v[:3 * n].reshape(n, 3), v[3 * n:].reshape(n, 3), dft="fft", torque_mode=name)
+            return np.concatenate([U.ravel(), Om.ravel()])
+        U, _ = oracle.mobility_apply(prob, pos, v.reshape(n, 3), None, dft="fft")
+        return U.ravel()
+
+    W = np.concatenate([WF.ravel(), WT.ravel()]) if with_torque else WF.ravel()
+    g_o, its_o, eps_o = oracle.lanczos_sqrt(apply, W, tol=1e-4, max_iter=40)
+    with dp.Plan(prob, max_particles=n, use_torques=True, torque_mode=mode) as plan:
+        gU, gO, its, eps = plan.lanczos_sqrt(*to_dev(pos, WF, WT), tol=1e-4, max_iter=40)
+    g = np.concatenate([gU.cpu().numpy().ravel()] + ([gO.cpu().numpy().ravel()] if with_torque else []))
+    assert its == its_o and len(eps) == len(eps_o)
+    assert np.allclose(eps, eps_o, rtol=1e-5)
+    assert rel_l2(g, g_o) < 1e-8
+    assert its < 40                                             # converged before max_iter
