@@ -472,7 +472,7 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs 
       __syncwarp();
       constexpr int ww = w * w;
       const int nent = (m.w - m.z + 1) * ww;
-#pragma unroll 2
+#pragma unroll 4
       for (int e = lane; e < nent; e += 32) {
         int l = m.z + e / ww, rem = e % ww, b = rem / w, a = rem % w;
         int i = m.x + a; if (i >= g.nx) i -= g.nx;
