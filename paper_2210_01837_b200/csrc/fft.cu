@@ -127,27 +127,6 @@ __host__ __device__ inline size_t align16(size_t b) { return (b + 15) / 16 * 16;
 
 // hooks of edge_lines (called between the loads of a round and its arithmetic), plain values only
 struct MidNone { __device__ __forceinline__ void operator()(int, int) const {} };
-struct MidStoreDrained {      // forward y pass, round 0: the slot's previous bulk store has read the buffer
-  int slot, st;
-  __device__ __forceinline__ void operator()(int rd, int) const {
-    if (rd == 0) { if (st == 0) bulk_wait_read(); slot_barrier<YTPS>(slot); }
-  }
-};
-struct MidPrefetch {          // inverse y pass, last round: all inputs are in registers, refill the buffer with the next rows
-  int slot, st;
-  uint64_t* mbar;
-  void* buf;
-  const void* next;           // null: nothing left
-  unsigned bytes;
-  __device__ __forceinline__ void operator()(int rd, int nrounds) const {
-    if (rd == nrounds - 1) {
-      fence_async_proxy();      // generic-proxy accesses of buf (this batch's stages) before the async-proxy refill
-      slot_barrier<YTPS>(slot);
-      if (st == 0 && next) { mbar_expect_tx(mbar, bytes); bulk_load(buf, next, bytes, mbar); }
-    }
-  }
-};
-
 // The kernels are templates on the factorisation <R0, R1, R2> of the hot sizes (no runtime dispatch, every index into the
 // argument arrays static, only three butterflies in the instruction stream); <0, 0, 0> is the general version that
 // reads the radices from its arguments.
@@ -192,8 +171,8 @@ __device__ __forceinline__ void run_inner(const FA& A, double2* buf, const doubl
 
 // ---------------------------------------------------------------------------------------------- pass Y (in place)
 // Forward: the first stage reads the row from global memory (edge_lines), the other stages run in shared memory, the
-// result leaves with one bulk store.  While a slot's bulk store drains, its next row's global loads are already in
-// flight; the stage-1 results are written to shared memory only after the store has finished reading it.
+// result leaves with one bulk store; a slot waits for its previous store to have read the buffer before it starts the next
+// row (the CTA's other slots are busy meanwhile).
 template <int R0, int R1, int R2>
 __global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_fwd(FftYArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -213,7 +192,11 @@ __global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_fwd(FftYArgs A) {
     const long long row0 = (f * A.nz + lm) * A.nkx + j * A.rb;
     const int nr = (int)((ra - j * A.rb) < A.rb ? (ra - j * A.rb) : A.rb);
     double2* g = A.data + row0 * n;
-    const MidStoreDrained mid{slot, st};
+    // the slot's previous bulk store must have read the buffer before this row's first stage overwrites it; waiting here (and not
+    // between the loads and the arithmetic of the first round) keeps the first stage's registers free of the barrier: no spills
+    if (st == 0) bulk_wait_read();
+    slot_barrier<YTPS>(slot);
+    const MidNone mid;
     run_edge<YTPS, R0, false>(A.F.r[0], g, buf, tw + A.off[0], n, nr, st, mid);
     slot_barrier<YTPS>(slot);
     run_inner<YTPS, R0, R1, R2, false, false>(A, buf, tw, n, nr, st, slot);
@@ -225,8 +208,7 @@ __global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_fwd(FftYArgs A) {
 }
 
 // Inverse: the row arrives with one bulk load, all stages but the last run in shared memory, the last stage (largest
-// stride) stores its results straight to global memory.  As soon as that stage has read the row, the slot's next bulk
-// load is issued, so it flies during the last stage's arithmetic and stores.
+// stride) stores its results straight to global memory; then the slot's next bulk load is issued.
 template <int R0, int R1, int R2>
 __global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_inv(FftYArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -259,8 +241,12 @@ __global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_inv(FftYArgs A) {
     const long long nrow0 = (b + stride) * A.rb;
     const bool more = b + stride < nbatch;
     const int nnr = more ? (int)((A.rows - nrow0) < A.rb ? (A.rows - nrow0) : A.rb) : 0;
-    const MidPrefetch mid{slot, st, mbar, buf, more ? (const void*)(A.data + nrow0 * n) : nullptr, (unsigned)nnr * n * 16u};
-    run_edge<YTPS, R0, true>(A.F.r[0], buf, g, tw + A.off[0], n, nr, st, mid);
+    // the refill of the buffer is issued after the last stage (issuing it between that stage's loads and its arithmetic costs the
+    // stage 200 bytes of spills per thread; the other slots of the CTA cover the load's latency)
+    run_edge<YTPS, R0, true>(A.F.r[0], buf, g, tw + A.off[0], n, nr, st, MidNone());
+    fence_async_proxy();
+    slot_barrier<YTPS>(slot);
+    if (st == 0 && more) { mbar_expect_tx(mbar, (unsigned)nnr * n * 16u); bulk_load(buf, A.data + nrow0 * n, (unsigned)nnr * n * 16u, mbar); }
   }
 }
 
