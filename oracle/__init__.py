@@ -39,7 +39,8 @@ def build(force: bool = False) -> str:
 class _Params(ctypes.Structure):
     _fields_ = [("wall_mode", ctypes.c_int), ("Lx", ctypes.c_double), ("Ly", ctypes.c_double), ("H", ctypes.c_double),
                 ("nx", ctypes.c_int), ("ny", ctypes.c_int), ("nz", ctypes.c_int), ("w", ctypes.c_int),
-                ("beta_M", ctypes.c_double), ("beta_D", ctypes.c_double), ("eta", ctypes.c_double)]
+                ("beta_M", ctypes.c_double), ("beta_D", ctypes.c_double), ("eta", ctypes.c_double),
+                ("slip_0", ctypes.c_double), ("slip_H", ctypes.c_double), ("uwall_0", ctypes.c_double * 2), ("uwall_H", ctypes.c_double * 2)]
 
 
 _lib = None
@@ -80,9 +81,13 @@ def lib():
 
 
 def _params(prob) -> _Params:
-    """prob: any object with wall_mode, Lx, Ly, H, nx, ny, nz, w, beta_M, beta_D, eta."""
+    """prob: any object with wall_mode, Lx, Ly, H, nx, ny, nz, w, beta_M, beta_D, eta and, optionally, the wall data of App. A /
+    eq 27: slip_0, slip_H (partial slip lengths, slit only), uwall_0, uwall_H (uniform wall velocities (x, y))."""
+    u0 = tuple(float(v) for v in getattr(prob, "uwall_0", (0.0, 0.0)))
+    uH = tuple(float(v) for v in getattr(prob, "uwall_H", (0.0, 0.0)))
     return _Params(int(prob.wall_mode), float(prob.Lx), float(prob.Ly), float(prob.H), int(prob.nx), int(prob.ny),
-                   int(prob.nz), int(prob.w), float(prob.beta_M), float(prob.beta_D), float(prob.eta))
+                   int(prob.nz), int(prob.w), float(prob.beta_M), float(prob.beta_D), float(prob.eta),
+                   float(getattr(prob, "slip_0", 0.0)), float(getattr(prob, "slip_H", 0.0)), (ctypes.c_double * 2)(*u0), (ctypes.c_double * 2)(*uH))
 
 
 def _ptr(a):

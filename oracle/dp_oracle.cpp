@@ -40,6 +40,10 @@ struct or_params {
     int w;                  // ES support in cells (paper's m), alpha = w h / 2
     double beta_M, beta_D;
     double eta;
+    // App. A and eq 27/46/52: partial slip lengths of the bottom / top wall (slit only) and UNIFORM wall
+    // velocities (x, y) of the bottom wall (both geometries) and of the top wall (slit); all zero = the no-slip product
+    double slip_0, slip_H;
+    double uwall_0[2], uwall_H[2];
 };
 
 int or_num_threads() {
@@ -647,15 +651,18 @@ static void bvp_matrix(const ChebOps& C, ld k, std::vector<ld>& M) {
     }
 }
 
-// k = 0 matrix of O9: rows 0..nz-3: D^2; BW: u(0) = 0, du/dz(H) = 0 (eq 52); slit: u(0) = 0, u(H) = 0 ((A12), no slip)
-static void zero_mode_matrix(const ChebOps& C, int wall_mode, std::vector<ld>& M) {
+// k = 0 matrix of O9: rows 0..nz-3: D^2; row nz-2: u(0) - l0 u'(0) (BW: l0 = 0: eq 52; slit: (A12));
+// row nz-1: BW: u'(H) (eq 52); slit: u(H) + lH u'(H)  ((A12))
+static void zero_mode_matrix(const ChebOps& C, int wall_mode, ld l0, ld lH, std::vector<ld>& M) {
     int nz = C.nz;
     M.assign((size_t)nz * nz, 0);
     for (int n = 0; n < nz - 2; ++n) for (int m = 0; m < nz; ++m) M[(size_t)n * nz + m] = C.D2[(size_t)n * nz + m];
     for (int m = 0; m < nz; ++m) {
-        M[(size_t)(nz - 2) * nz + m] = (m % 2 ? -1 : 1);                           // sum (-1)^n u_n = u(z=0)
-        if (wall_mode == 0) { ld s = 0; for (int n = 0; n < nz; ++n) s += C.D[(size_t)n * nz + m]; M[(size_t)(nz - 1) * nz + m] = s; }  // sum (D u)_n
-        else M[(size_t)(nz - 1) * nz + m] = 1;                                       // sum u_n = u(z=H)
+        ld dH = 0, d0 = 0;                                                           // sum (D u)_n = u'(H), sum (-1)^n (D u)_n = u'(0)
+        for (int n = 0; n < nz; ++n) { dH += C.D[(size_t)n * nz + m]; d0 += (n % 2 ? -1 : 1) * C.D[(size_t)n * nz + m]; }
+        M[(size_t)(nz - 2) * nz + m] = (m % 2 ? -1 : 1) - l0 * d0;                   // sum (-1)^n u_n = u(z=0)
+        if (wall_mode == 0) M[(size_t)(nz - 1) * nz + m] = dH;
+        else M[(size_t)(nz - 1) * nz + m] = 1 + lH * dH;                             // sum u_n = u(z=H)
     }
 }
 
@@ -730,11 +737,14 @@ static void solve_columns(const or_params* P, long ncols, const int* ixs, const 
 
             if (ix == 0 && iy == 0) {
                 // O9: k = 0 column (eqs 47, 51, 52, (A12)); no DP/correction split
-                zero_mode_matrix(C, P->wall_mode, M);
+                // the unnormalised xy DFT of a uniform wall velocity U is nx ny U at k = 0 and nothing elsewhere (eqs 46, 52, (A12))
+                zero_mode_matrix(C, P->wall_mode, P->wall_mode == 1 ? (ld)P->slip_0 : 0, P->wall_mode == 1 ? (ld)P->slip_H : 0, M);
                 lu.factor(M, nz);
                 for (int c = 0; c < 2; ++c) {
                     std::vector<cld> b(nz, cld(0));
                     for (int n = 0; n < nz - 2; ++n) b[n] = -fc[c][n] / eta;
+                    b[nz - 2] = (ld)nx * ny * (ld)P->uwall_0[c];
+                    if (P->wall_mode == 1) b[nz - 1] = (ld)nx * ny * (ld)P->uwall_H[c];
                     lu.solve(b);
                     ucoef[c] = b;
                 }
@@ -763,9 +773,18 @@ static void solve_columns(const or_params* P, long ncols, const int* ixs, const 
                 r[nz - 1] = p0 / (2 * eta);
                 uc[2] = r; lu.solve(uc[2]);
 
-                // O7: wall data (eq 27 with u_wall = 0; (A3) with slip length 0)
+                // O7: wall data (eq 27; (A3a-d)): a uniform wall velocity has no k != 0 component;
+                //   u_0 = -u_DP(0) + l0 du_DP/dz(0), u_H = -u_DP(H) - lH du_DP/dz(H) for the tangential components, w unchanged;
+                //   the wall derivatives "by Chebyshev differentiation and direct summation" (footnote 46)
+                const ld l0 = P->wall_mode == 1 ? (ld)P->slip_0 : 0, lH = P->wall_mode == 1 ? (ld)P->slip_H : 0;
                 cld u0[3], uH[3];
                 for (int c = 0; c < 3; ++c) { u0[c] = -ChebOps::at_bottom(uc[c]); uH[c] = -ChebOps::at_top(uc[c]); }
+                if (l0 != 0 || lH != 0)
+                    for (int c = 0; c < 2; ++c) {
+                        C.diff(uc[c], tmp);
+                        u0[c] += l0 * ChebOps::at_bottom(tmp);
+                        uH[c] -= lH * ChebOps::at_top(tmp);
+                    }
 
                 // O8: correction at the nodes
                 for (int c = 0; c < 3; ++c) ucorr[c].assign(nz, cld(0));
@@ -780,19 +799,22 @@ static void solve_columns(const or_params* P, long ncols, const int* ixs, const 
                         ucorr[2][l] = Wc * zl * E + u0[2] * E;
                     }
                 } else {
-                    // App. A with slip lengths 0 ((A5), (A6), (A8), (A10)), unknowns
+                    // App. A ((A5), (A6), (A8), (A10)) with slip lengths l0, lH, unknowns
                     //   x = [C0, D0~, Cx, Dx~, Cy, Dy~, Cz, Dz~],  D~ = D e^{kH}  (basis e^{-k(H-z)})
                     const ld e = expl(-k * H);
                     std::vector<cld> A8(64, cld(0)), b8(8, cld(0));
                     auto at = [&](int r_, int c_) -> cld& { return A8[(size_t)r_ * 8 + c_]; };
                     const ld kcs[2] = {kxt, kyt};
                     for (int c = 0; c < 2; ++c) {
-                        // (A8a): C_c + D_c = u_0
-                        at(2 * c, 2 + 2 * c) = 1; at(2 * c, 3 + 2 * c) = e; b8[2 * c] = u0[c];
-                        // (A8c): -(i k_c H e^{-kH}/(2 eta k)) C0 + (i k_c H e^{kH}/(2 eta k)) D0 + e^{-kH} C_c + e^{kH} D_c = u_H
-                        at(2 * c + 1, 0) = -(I * kcs[c] * H * e) / (2 * eta * k);
-                        at(2 * c + 1, 1) = +(I * kcs[c] * H) / (2 * eta * k);
-                        at(2 * c + 1, 2 + 2 * c) = e; at(2 * c + 1, 3 + 2 * c) = 1; b8[2 * c + 1] = uH[c];
+                        // (A8a): (i k_c l0/(2 eta k)) C0 - (i k_c l0/(2 eta k)) D0 + (1 + k l0) C_c + (1 - k l0) D_c = u_0
+                        at(2 * c, 0) = +(I * kcs[c] * l0) / (2 * eta * k);
+                        at(2 * c, 1) = -(I * kcs[c] * l0 * e) / (2 * eta * k);
+                        at(2 * c, 2 + 2 * c) = 1 + k * l0; at(2 * c, 3 + 2 * c) = (1 - k * l0) * e; b8[2 * c] = u0[c];
+                        // (A8c): (i k_c H e^{-kH}/(2 eta k)) (k lH - lH/H - 1) C0 + (i k_c H e^{kH}/(2 eta k)) (k lH + lH/H + 1) D0
+                        //        + e^{-kH} (1 - k lH) C_c + e^{kH} (1 + k lH) D_c = u_H
+                        at(2 * c + 1, 0) = (I * kcs[c] * H * e) / (2 * eta * k) * (k * lH - lH / H - 1);
+                        at(2 * c + 1, 1) = (I * kcs[c] * H) / (2 * eta * k) * (k * lH + lH / H + 1);
+                        at(2 * c + 1, 2 + 2 * c) = e * (1 - k * lH); at(2 * c + 1, 3 + 2 * c) = 1 + k * lH; b8[2 * c + 1] = uH[c];
                     }
                     // (A8b): Cz + Dz = w_0
                     at(4, 6) = 1; at(4, 7) = e; b8[4] = u0[2];
