@@ -80,6 +80,14 @@ typedef struct {
                            itself (3 fields each way; truncated phi', one kernel per dimension, footnotes 47-48, PAPER.md:797-798;
                            DESIGN.md reading G19).  The two discretisations agree to the method's 2-3 digits, not to roundoff;
                            mode 1 needs beta_D > 3 sqrt(3)/2.  Ignored when use_torques = 0.                                     */
+  double slip_0, slip_H; /* partial slip lengths l_0, l_H >= 0 of the bottom / top wall, slit only (App. A (A1)):
+                           u - u_wall = l_0 du/dz at z = 0, u - u_wall = -l_H du/dz at z = H for the tangential components; 0 = no slip.
+                           The wall derivatives of the DP solution come from Chebyshev differentiation and direct summation
+                           (footnote 46).  Must be 0 for DP_BOTTOM_WALL (the paper gives no slip solution there).       */
+  double uwall_0[2];    /* uniform velocity (x, y) of the bottom wall (eq 27 / eq 46): enters the k = 0 column,
+                           eq 52 / (A12); the product becomes affine, U = M F + (flow driven by the walls)                          */
+  double uwall_H[2];    /* uniform velocity (x, y) of the top wall; slit only ((A1b), (A12)); must be 0 for DP_BOTTOM_WALL.
+                           Non-uniform wall velocity fields u_wall(x, y) are not supported.                                          */
 } dp_params;
 
 /* Plan creation for the problem of PAPER.md:74 (box, walls) with the grid of PAPER.md:319 and the ES kernel of eq 54.

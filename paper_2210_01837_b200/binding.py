@@ -28,7 +28,8 @@ class dp_params(ctypes.Structure):
                 ("beta_M", ctypes.c_double), ("beta_D", ctypes.c_double), ("a", ctypes.c_double), ("eta", ctypes.c_double),
                 ("max_particles", ctypes.c_int), ("transfer_fp32", ctypes.c_int), ("device", ctypes.c_int),
                 # extensions beyond SURVEY.md §8(b)
-                ("use_torques", ctypes.c_int), ("fft_backend", ctypes.c_int), ("dense_planes", ctypes.c_int), ("torque_mode", ctypes.c_int)]
+                ("use_torques", ctypes.c_int), ("fft_backend", ctypes.c_int), ("dense_planes", ctypes.c_int), ("torque_mode", ctypes.c_int),
+                ("slip_0", ctypes.c_double), ("slip_H", ctypes.c_double), ("uwall_0", ctypes.c_double * 2), ("uwall_H", ctypes.c_double * 2)]
 
 
 _lib = None
@@ -134,7 +135,10 @@ class Plan:
         self.params = dp_params(int(prob.wall_mode), float(prob.Lx), float(prob.Ly), float(prob.H), int(prob.nx), int(prob.ny),
                                 int(prob.nz), int(prob.w), float(prob.beta_M), float(prob.beta_D), float(getattr(prob, "a", 1.0)),
                                 float(prob.eta), int(max_particles), int(bool(transfer_fp32)), int(device),
-                                int(bool(use_torques)), int(fft_backend), int(bool(dense_planes)), int(torque_mode))
+                                int(bool(use_torques)), int(fft_backend), int(bool(dense_planes)), int(torque_mode),
+                                float(getattr(prob, "slip_0", 0.0)), float(getattr(prob, "slip_H", 0.0)),
+                                (ctypes.c_double * 2)(*[float(v) for v in getattr(prob, "uwall_0", (0.0, 0.0))]),
+                                (ctypes.c_double * 2)(*[float(v) for v in getattr(prob, "uwall_H", (0.0, 0.0))]))
         h = ctypes.c_void_p()
         rc = L.dp_create(ctypes.byref(self.params), ctypes.byref(h))
         if rc != 0:

@@ -348,6 +348,9 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   if (p.transfer_fp32 != 0 && p.transfer_fp32 != 1) return DP_EINVAL;
   if (p.dense_planes != 0 && p.dense_planes != 1) return DP_EINVAL;
   if (p.torque_mode != 0 && p.torque_mode != 1) return DP_EINVAL;
+  if (!(p.slip_0 >= 0) || !(p.slip_H >= 0) || !std::isfinite(p.slip_0) || !std::isfinite(p.slip_H)) return DP_EINVAL;
+  for (int c = 0; c < 2; ++c) if (!std::isfinite(p.uwall_0[c]) || !std::isfinite(p.uwall_H[c])) return DP_EINVAL;
+  if (p.wall_mode == DP_BOTTOM_WALL && (p.slip_0 != 0 || p.slip_H != 0 || p.uwall_H[0] != 0 || p.uwall_H[1] != 0)) return DP_EINVAL;
   if (p.use_torques && p.torque_mode == 1 && es_dphi_cut_host(p.beta_D) < 0) return DP_EINVAL;   // phi' has no minimum to truncate at
   if (p.transfer_fp32 && !(p.fft_backend == 0 && dp_fft_own_supported(p.nx, p.ny))) return DP_EINVAL;   // fp32 grids are read by the own x passes only
   if (p.wall_mode == DP_SLIT && p.w * hx > p.H) return DP_EINVAL;     // a kernel may overlap one wall, not both

@@ -79,6 +79,9 @@ struct SolveArgs {
   const double* frag;            // transform fragment table (see Tr)
   double Lx, Ly, H, eta;
   int wall_mode, torque, omega;
+  int slip;                      // slit with a non-zero slip length (App. A)
+  double l0, lH;                 // slip lengths of the bottom / top wall
+  double uw0[2], uwH[2];         // uniform wall velocities (x, y): enter the k = 0 column only
 };
 
 __device__ __forceinline__ void cp_async16(double* smem_dst, const double2* gmem_src) {
@@ -225,7 +228,7 @@ __device__ __forceinline__ double factor_chain(double* __restrict__ Fm, double* 
 template <int NZ, int PAR>
 __device__ __forceinline__ double chain(bool SUB_D, double (&a)[Ch<NZ, PAR>::NR], double rho0, const double* __restrict__ Fm, const double* __restrict__ Fi,
                                         const double* __restrict__ Fa, double* __restrict__ col, double* __restrict__ dcol, int lane, double k,
-                                        double k2, double inv_s, double beta_bc, double invBg) {
+                                        double k2, double inv_s, double beta_bc, double invBg, double* __restrict__ sum_b) {
   constexpr int N = NZ - 1, n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR;
   const double* __restrict__ T = tab<NZ>();
   if (!PAR) a[0] = fma(0.25 * k2, rho0, a[0]);               // even chain: row 2 carries (kappa^2/4) rho_0
@@ -245,6 +248,7 @@ __device__ __forceinline__ double chain(bool SUB_D, double (&a)[Ch<NZ, PAR>::NR]
   for (int j = 0; j < NR; ++j) a[j] = fma(border, Fa[(n0 + 2 * j) * TM], a[j]);
   // integrate twice:  b_{n+1} = (cbar_n a_n - a_{n+2}) / (2(n+1)),  c_n = (cbar_{n-1} b_{n-1} - b_{n+1}) / (2n)
   double Sc0 = 0.0, Sc1 = 0.0, bprev;
+  double Sb = PAR ? border : 0.0;            // sum of the b_m this chain produces (m of the other parity): (H/2) dy/dz summed (footnote 46)
   if (!PAR) { EL(col, 0, lane) = border; Sc0 = border; bprev = 0.0; }
   else { bprev = border; if (SUB_D) EL(dcol, 0, lane) -= border * inv_s; }
 #pragma unroll
@@ -261,8 +265,10 @@ __device__ __forceinline__ double chain(bool SUB_D, double (&a)[Ch<NZ, PAR>::NR]
       if (i & 1) Sc1 += c; else Sc0 += c;
     }
     if (SUB_D && n + 1 <= N - 1) EL(dcol, n + 1, lane) -= bn1 * inv_s;
+    if (sum_b && n + 1 <= N - 1) Sb += bn1;
     bprev = bn1;
   }
+  if (sum_b) *sum_b = Sb;
   return Sc0 + Sc1;
 }
 
@@ -315,7 +321,8 @@ struct ModeK {
 //      One code path per parity so that the chain sweeps exist once in the instruction stream.
 template <int NZ, int PAR>
 __device__ __noinline__ double bvp_item(int kind, int comp, double* __restrict__ C, const double* __restrict__ F, int lane, int mode, ModeK K,
-                                        double s, double inv_s, double eta, double invBg, double pH_own, double p0_own, double pH_oth, double p0_oth) {
+                                        double s, double inv_s, double eta, double invBg, double pH_own, double p0_own, double pH_oth, double p0_oth,
+                                        double* __restrict__ sum_b) {
   constexpr int N = NZ - 1, n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR, VS = NZ * LN;
   double a[NR], rho0 = 0.0, beta_bc = 0.0;
   double* col;
@@ -367,20 +374,33 @@ __device__ __noinline__ double bvp_item(int kind, int comp, double* __restrict__
     beta_bc = PAR ? 0.5 * (gH + g0) : 0.5 * (gH - g0);
   }
   return chain<NZ, PAR>(kind == 0, a, rho0, F + 0 * NZ * TM + mode, F + 1 * NZ * TM + mode, F + 2 * NZ * TM + mode, col, C + 2 * VS, lane,
-                        K.k, K.k2, inv_s, beta_bc, invBg);
+                        K.k, K.k2, inv_s, beta_bc, invBg, sum_b);
 }
 
 // ---- wall correction coefficients of a lane (own part), basis: 0 = z e^{-kz}, 1 = e^{-kz}, 2 = z e^{-k(H-z)}, 3 = e^{-k(H-z)}
-//   wall data (eq 27 / (A3) with no slip, u_wall = 0): u_0 = -u_DP(z=0) = -(S_even - S_odd), u_H = -u_DP(z=H) = -(S_even + S_odd)
-__device__ __forceinline__ void correction_coefficients(const double* __restrict__ s_sum, int lane, const ModeK& K, double H, int wall_mode,
-                                                        double cf[3][4]) {
+//   wall data (eq 27 / (A3), u_wall uniform, i.e. absent for k != 0): u_0 = -u_DP(0) + l0 du_DP/dz(0), u_H = -u_DP(H) - lH du_DP/dz(H)
+//   for the tangential components (slit; l0 = lH = 0 is no slip), w_0 = -w_DP(0), w_H = -w_DP(H); end values by direct summation:
+//   y(0) = S_even - S_odd, y(H) = S_even + S_odd, (H/2) dy/dz likewise from the sums of the first-integral coefficients b_m
+//   (even m come from the odd chain, odd m from the even chain; footnote 46).
+__device__ __forceinline__ void correction_coefficients(const double* __restrict__ s_sum, const double* __restrict__ s_sumb, int lane, const ModeK& K,
+                                                        double H, int wall_mode, double l0, double lH, double cf[3][4]) {
   double u0[3], uH[3], u0o[3], uHo[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
     const double se = s_sum[((1 + c) * 2 + 0) * LN + lane], so = s_sum[((1 + c) * 2 + 1) * LN + lane];
     u0[c] = -(se - so); uH[c] = -(se + so);
-    u0o[c] = __shfl_xor_sync(0xffffffffu, u0[c], 1); uHo[c] = __shfl_xor_sync(0xffffffffu, uH[c], 1);
   }
+  if (wall_mode == DP_SLIT && (l0 != 0.0 || lH != 0.0)) {
+    const double inv_s = 2.0 / H;
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+      const double b_odd = s_sumb[(c * 2 + 0) * LN + lane], b_even = s_sumb[(c * 2 + 1) * LN + lane];   // from the even / odd chain
+      u0[c] = fma(l0 * inv_s, b_even - b_odd, u0[c]);
+      uH[c] = fma(-lH * inv_s, b_even + b_odd, uH[c]);
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < 3; ++c) { u0o[c] = __shfl_xor_sync(0xffffffffu, u0[c], 1); uHo[c] = __shfl_xor_sync(0xffffffffu, uH[c], 1); }
   const double k = K.k, kxt = K.kxt, kyt = K.kyt, sgI = K.sgI;
 #pragma unroll
   for (int c = 0; c < 3; ++c) { cf[c][0] = cf[c][1] = cf[c][2] = cf[c][3] = 0.0; }
@@ -392,24 +412,37 @@ __device__ __forceinline__ void correction_coefficients(const double* __restrict
     cf[0][0] = -(kxt * ik) * Q; cf[1][0] = -(kyt * ik) * Q; cf[2][0] = Wc;
     cf[0][1] = u0[0]; cf[1][1] = u0[1]; cf[2][1] = u0[2];
   } else {
-    // App. A, no slip.  Unknowns [C0', D0', Cz, Dz] with C0' = C0/(2 eta), D0' = D0 e^{kH}/(2 eta) (basis e^{-k(H-z)}):
-    // (A8b), (A8d), (A10a), (A10b) after eliminating Cx+e Dx, e Cx+Dx (and y) with (A8a), (A8c); e = e^{-kH}.
+    // App. A.  Unknowns C0' = C0/(2 eta), D0' = D0 e^{kH}/(2 eta), C_c, D~_c = D_c e^{kH} (basis e^{-k(H-z)}, reading G13); e = e^{-kH}.
+    // Tangential pairs, c = x, y ((A8a), (A8c)):
+    //   a1 C_c + a2 D~_c = u0_c - i k_c (p1 C0' + p2 D0'),   a3 C_c + a4 D~_c = uH_c - i k_c (p3 C0' + p4 D0')
+    //   a1 = 1 + k l0, a2 = (1 - k l0) e, a3 = (1 - k lH) e, a4 = 1 + k lH, p1 = l0/k, p2 = -l0 e/k,
+    //   p3 = (H e/k)(k lH - lH/H - 1), p4 = (H/k)(k lH + lH/H + 1).
+    // Eliminating them from the two continuity rows (A10a), (A10b) leaves a REAL 4x4 system for [C0', D0', Cz, D~z] with the rows
+    // (A8b), (A8d), (A10a), (A10b); its right-hand sides are complex, one part per lane.
     const double e = exp(-k * H), ik = 1.0 / k;
-    const double g = (kxt * kxt + kyt * kyt) * H * ik;
-    double M[4][4] = {{0.0, 0.0, 1.0, e}, {H * e, H, e, 1.0}, {1.0, e, -k, k * e}, {e * (1.0 - g), 1.0 + g, -k * e, k}};
-    // right-hand sides: [w0, wH, -i(kx u0 + ky v0), -i(kx uH + ky vH)]  ->  own part of -i z = -sgI * other part of z
-    double b[4] = {u0[2], uH[2], -sgI * fma(kxt, u0o[0], kyt * u0o[1]), -sgI * fma(kxt, uHo[0], kyt * uHo[1])};
+    const double a1 = 1.0 + k * l0, a2 = (1.0 - k * l0) * e, a3 = (1.0 - k * lH) * e, a4 = 1.0 + k * lH;
+    const double p1 = l0 * ik, p2 = -l0 * e * ik, p3 = H * e * ik * (k * lH - lH / H - 1.0), p4 = H * ik * (k * lH + lH / H + 1.0);
+    const double idet = 1.0 / (a1 * a4 - a2 * a3);
+    const double g1a = (a4 - e * a3) * idet, g2a = (e * a1 - a2) * idet, g1b = (e * a4 - a3) * idet, g2b = (a1 - e * a2) * idet;
+    const double kk = kxt * kxt + kyt * kyt;
+    double M[4][4] = {{0.0, 0.0, 1.0, e},
+                      {H * e, H, e, 1.0},
+                      {1.0 + kk * (g1a * p1 + g2a * p3), e + kk * (g1a * p2 + g2a * p4), -k, k * e},
+                      {e + kk * (g1b * p1 + g2b * p3), 1.0 + kk * (g1b * p2 + g2b * p4), -k * e, k}};
+    // right-hand sides: [w0, wH, -i (g1a q0 + g2a qH), -i (g1b q0 + g2b qH)], q = kx u + ky v;  own part of -i z = -sgI * other part of z
+    const double q0o = fma(kxt, u0o[0], kyt * u0o[1]), qHo = fma(kxt, uHo[0], kyt * uHo[1]);
+    double b[4] = {u0[2], uH[2], -sgI * (g1a * q0o + g2a * qHo), -sgI * (g1b * q0o + g2b * qHo)};
     solve4(M, b);
     const double C0 = b[0], D0 = b[1];
     const double C0o = __shfl_xor_sync(0xffffffffu, C0, 1), D0o = __shfl_xor_sync(0xffffffffu, D0, 1);
-    const double iom = 1.0 / (-expm1(-k * H) * (1.0 + e));       // 1/(1 - e^2)
 #pragma unroll
     for (int c = 0; c < 2; ++c) {
-      const double kc = c == 0 ? kxt : kyt, q = kc * H * ik;
-      // C_c + e D_c = u0 ; e C_c + D_c = uH + i q (e C0' - D0')
-      const double r2 = fma(sgI * q, e * C0o - D0o, uH[c]);
-      cf[c][1] = (u0[c] - e * r2) * iom;
-      cf[c][3] = (r2 - e * u0[c]) * iom;
+      const double kc = c == 0 ? kxt : kyt;
+      // own part of -i k_c X = -k_c sgI other(X)
+      const double r1 = fma(-kc * sgI, p1 * C0o + p2 * D0o, u0[c]);
+      const double r2 = fma(-kc * sgI, p3 * C0o + p4 * D0o, uH[c]);
+      cf[c][1] = (a4 * r1 - a2 * r2) * idet;
+      cf[c][3] = (a1 * r2 - a3 * r1) * idet;
       // (A5): -i (k_c/k) C0' z e^{-kz} + i (k_c/k) D0' z e^{-k(H-z)}
       cf[c][0] = -sgI * (kc * ik) * C0o;
       cf[c][2] = sgI * (kc * ik) * D0o;
@@ -425,7 +458,8 @@ template <int NZ> struct SolveSmem {
   static constexpr int FACT = COLS;                                    // [3][NZ][TM]: multipliers, inverse pivots, border solution
   static constexpr int IBG = FACT + 3 * NZ * TM;                       // [2][TM] 1/B_g of the even / odd chain
   static constexpr int SUM = IBG + 2 * TM;                             // [4][2][LN] S_c of (p,u,v,w) x (even, odd chain)
-  static constexpr int DOUBLES = SUM + 8 * LN;
+  static constexpr int SUMB = SUM + 8 * LN;                            // [2][2][LN] S_b of (u,v) x (even, odd chain): wall derivatives (partial slip)
+  static constexpr int DOUBLES = SUMB + 4 * LN;
   static constexpr int CORR = FACT;                                    // [12][LN] slit correction coefficients: the factors are dead by then
   static_assert(12 * LN <= 3 * NZ * TM, "correction coefficients fit in the factor area");
   static constexpr int PER_SM = (227 * 1024) / (DOUBLES * 8 + 1024);   // CTAs that fit an SM's shared memory
@@ -450,6 +484,7 @@ __global__ void __launch_bounds__(SOLVE_THREADS, SolveSmem<NZ>::CTAS) k_solve(So
   double* F = smem + S::FACT;
   double* s_ibg = smem + S::IBG;
   double* s_sum = smem + S::SUM;
+  double* s_sumb = smem + S::SUMB;
   double* s_corr = smem + S::CORR;
   const double* T = tab<NZ>();
 
@@ -592,8 +627,8 @@ __global__ void __launch_bounds__(SOLVE_THREADS, SolveSmem<NZ>::CTAS) k_solve(So
     named_arrive(2, SOLVE_THREADS);                        // t_y has been read: tile 4 may be overwritten
     named_sync(1, 64);                                     // f_x and f_y are complete (and t_x consumed) before either chain starts
     double Sc;
-    if (wid) Sc = bvp_item<NZ, 1>(0, 0, C, F, lane, mode, K, s, inv_s, eta, s_ibg[TM + mode], 0.0, 0.0, 0.0, 0.0);
-    else Sc = bvp_item<NZ, 0>(0, 0, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], 0.0, 0.0, 0.0, 0.0);
+    if (wid) Sc = bvp_item<NZ, 1>(0, 0, C, F, lane, mode, K, s, inv_s, eta, s_ibg[TM + mode], 0.0, 0.0, 0.0, 0.0, nullptr);
+    else Sc = bvp_item<NZ, 0>(0, 0, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], 0.0, 0.0, 0.0, 0.0, nullptr);
     s_sum[(0 * 2 + wid) * LN + lane] = Sc;
   } else {
     constexpr int ER = (NP + 3) / 4;                       // node pairs (l, N-l) per thread
@@ -637,10 +672,12 @@ __global__ void __launch_bounds__(SOLVE_THREADS, SolveSmem<NZ>::CTAS) k_solve(So
     const double se = s_sum[0 * LN + lane], so = s_sum[1 * LN + lane];
     const double pH = se + so, p0 = se - so;              // p(H) = sum p_n, p(0) = sum (-1)^n p_n  ("direct summation")
     const double pHo = __shfl_xor_sync(0xffffffffu, pH, 1), p0o = __shfl_xor_sync(0xffffffffu, p0, 1);
-    double Sc;
-    if (par) Sc = bvp_item<NZ, 1>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[TM + mode], pH, p0, pHo, p0o);
-    else Sc = bvp_item<NZ, 0>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], pH, p0, pHo, p0o);
+    double Sc, Sb = 0.0;
+    double* want_sb = (A.slip && comp < 2) ? &Sb : nullptr;        // partial slip needs du/dz, dv/dz of the DP solution on the walls
+    if (par) Sc = bvp_item<NZ, 1>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[TM + mode], pH, p0, pHo, p0o, want_sb);
+    else Sc = bvp_item<NZ, 0>(kind, comp, C, F, lane, mode, K, s, inv_s, eta, s_ibg[mode], pH, p0, pHo, p0o, want_sb);
     s_sum[((1 + comp) * 2 + par) * LN + lane] = Sc;
+    if (want_sb) s_sumb[(comp * 2 + par) * LN + lane] = Sb;
   }
   TMARK(7);
   __syncthreads();
@@ -648,10 +685,10 @@ __global__ void __launch_bounds__(SOLVE_THREADS, SolveSmem<NZ>::CTAS) k_solve(So
   // ---------------- phase 5: correction coefficients (bottom wall: every warp for itself; slit: warp 0, shared)
   double cf[3][4];
   if (A.wall_mode == DP_BOTTOM_WALL) {
-    correction_coefficients(s_sum, lane, K, A.H, DP_BOTTOM_WALL, cf);
+    correction_coefficients(s_sum, s_sumb, lane, K, A.H, DP_BOTTOM_WALL, 0.0, 0.0, cf);
   } else {
     if (wid == 0) {
-      correction_coefficients(s_sum, lane, K, A.H, DP_SLIT, cf);
+      correction_coefficients(s_sum, s_sumb, lane, K, A.H, DP_SLIT, A.l0, A.lH, cf);
 #pragma unroll
       for (int c = 0; c < 3; ++c)
 #pragma unroll
@@ -749,7 +786,8 @@ namespace {
 #endif
 
 // ---- k = 0 column (paper step 5; eqs 47, 51, 52; (A12) with no slip): one CTA of 64 threads
-//   w = 0;  u'' = -f_x/eta, v'' = -f_y/eta with u(0) = 0 and (bottom wall) u'(H) = 0 / (slit) u(H) = 0.
+//   w = 0;  u'' = -f_x/eta, v'' = -f_y/eta with u(0) = u_wall and (bottom wall) u'(H) = 0, or (slit, (A12)) u(0) - l0 u'(0) = u_wall_0,
+//   u(H) + lH u'(H) = u_wall_H (uniform wall velocities; slip lengths l0, lH).
 //   With torques the k = 0 force is f_x - (1/2) dz t_y, f_y + (1/2) dz t_x (eq 7).
 __global__ void k_zero_mode(SolveArgs A, int nz, const double* __restrict__ ct_full /* cos(n l pi/N) [nz][nz] */) {
   __shared__ double fc[4][2][DP_MAX_NZ];     // coefficients: f_x, f_y, t_x, t_y (re, im)
@@ -776,6 +814,9 @@ __global__ void k_zero_mode(SolveArgs A, int nz, const double* __restrict__ ct_f
   __syncthreads();
   if (t < 4) {
     const int comp = t >> 1, part = t & 1;          // u or v, re or im
+    // the unnormalised xy DFT of a uniform wall velocity U is nx ny U at k = 0 (real), and nothing at any other wavenumber
+    const double Uw0 = part ? 0.0 : (double)A.nx * (double)A.ny * A.uw0[comp];
+    const double UwH = part ? 0.0 : (double)A.nx * (double)A.ny * A.uwH[comp];
     // total force coefficients: f_x - (1/2) D t_y ; f_y + (1/2) D t_x
     double a[DP_MAX_NZ + 2], b[DP_MAX_NZ + 2], c[DP_MAX_NZ + 2];
     {
@@ -799,12 +840,19 @@ __global__ void k_zero_mode(SolveArgs A, int nz, const double* __restrict__ ct_f
       for (int n = 1; n <= N; ++n) c[n] = ((n == 1 ? 2.0 : 1.0) * b[n - 1] - b[n + 1]) / (2.0 * n);
       double sc = 0.0;
       for (int n = N; n >= 1; --n) sc += (n & 1) ? -c[n] : c[n];
-      c[0] = -sc;                                                // u(0) = sum (-1)^n c_n = 0
+      c[0] = Uw0 - sc;                                           // u(0) = sum (-1)^n c_n = u_wall (eqs 46, 52; 0 for a wall at rest)
     } else {
       for (int n = 2; n <= N; ++n) c[n] = (b[n - 1] - b[n + 1]) / (2.0 * n);
-      double so = 0.0, se = 0.0;
+      double so = 0.0, se = 0.0, sbH = 0.0, sb0 = 0.0;
       for (int n = N; n >= 2; --n) { if (n & 1) so += c[n]; else se += c[n]; }
-      c[1] = -so; c[0] = -se;                                    // u(0) = u(H) = 0   ((A12), no slip)
+      for (int n = N - 1; n >= 1; --n) { sbH += b[n]; sb0 += (n & 1) ? -b[n] : b[n]; }
+      // (A12): u(H) + lH u'(H) = U_H, u(0) - l0 u'(0) = U_0 with u' = (1/s) sum b_n, b_0 = c_1 + b_2/2:
+      //   c_0 + c_1 (1 + lH/s) = T,   c_0 - c_1 (1 + l0/s) = B
+      const double rH = A.lH / s, r0 = A.l0 / s;
+      const double Tt = UwH - se - so - rH * (0.5 * b[2] + sbH);
+      const double Bb = Uw0 - se + so + r0 * (0.5 * b[2] + sb0);
+      c[1] = (Tt - Bb) / (2.0 + rH + r0);
+      c[0] = Tt - c[1] * (1.0 + rH);
       b[0] = c[1] + 0.5 * b[2];                                  // c_1 = b_0 - b_2/2
     }
     for (int n = 0; n <= N; ++n) { uc[comp][part][n] = c[n]; ub[comp][part][n] = n <= N - 1 ? b[n] / s : 0.0; }
@@ -944,6 +992,9 @@ cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega,
   A.frag = P->d_solve_frag;
   A.Lx = P->p.Lx; A.Ly = P->p.Ly; A.H = P->p.H; A.eta = P->p.eta;
   A.wall_mode = P->p.wall_mode; A.torque = with_torque_field ? 1 : 0; A.omega = want_omega ? 1 : 0;
+  A.l0 = P->p.slip_0; A.lH = P->p.slip_H;
+  A.slip = (P->p.wall_mode == DP_SLIT && (A.l0 != 0.0 || A.lH != 0.0)) ? 1 : 0;
+  for (int c = 0; c < 2; ++c) { A.uw0[c] = P->p.uwall_0[c]; A.uwH[c] = P->p.uwall_H[c]; }
   cudaError_t e = cudaErrorInvalidValue;
 #define X(NZ) if (P->p.nz == NZ) e = launch_nz<NZ>(A, st);
   DP_SOLVE_NZ_LIST(X)

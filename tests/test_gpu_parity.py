@@ -469,3 +469,50 @@ def test_lanczos_square_root_matches_the_oracle_iteration(dp, with_torque, mode)
     assert np.allclose(eps, eps_o, rtol=1e-5)
     assert rel_l2(g, g_o) < 1e-8
     assert its < 40                                             # converged before max_iter
+
+
+# ------------------------------------------------------------------------------------------------ partial slip, moving walls
+@pytest.mark.parametrize("case", ["slit-slip", "slit-slip-top-only", "slit-moving-walls", "bw-moving-wall", "slit-all-kernel-mode"])
+def test_partial_slip_and_moving_walls_match_the_oracle(dp, case):
+    """Appendix A: slip lengths l_0, l_H in the slit ((A8), (A12)) and uniform wall velocities (eqs 27, 46, 52),
+    against the oracle's general 8 x 8 correction solve and its k = 0 system with slip rows."""
+    import dataclasses
+    mode = 0
+    if case.startswith("slit"):
+        prob, pos, F, T = workloads.random_slit(n=300, L=32.0, nxy=48, nz=48, H=8.0, seed=91, name=case)
+        pos = pos.copy(); pos[:4, 2] = [0.0, 0.3, 7.8, 8.0]
+        if case == "slit-slip":
+            prob = dataclasses.replace(prob, slip_0=0.7, slip_H=0.25)
+        elif case == "slit-slip-top-only":
+            prob = dataclasses.replace(prob, slip_H=3.0)
+        elif case == "slit-moving-walls":
+            prob = dataclasses.replace(prob, uwall_0=(0.3, -0.1), uwall_H=(-1.2, 0.4))
+        else:
+            prob = dataclasses.replace(prob, slip_0=0.4, slip_H=1.1, uwall_0=(0.3, -0.1), uwall_H=(-1.2, 0.4))
+            mode = 1
+    else:
+        prob, pos, F, T = small_monolayer("bw", 1500, 93)
+        prob = dataclasses.replace(prob, uwall_0=(0.8, 0.5))
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", torque_mode="kernel" if mode else "fourier")
+    with dp.Plan(prob, max_particles=len(pos), use_torques=True, torque_mode=mode) as plan:
+        U, Om = plan.mobility_apply(*to_dev(pos, F, T))
+        assert plan.check() == 0
+    U, Om = U.cpu().numpy(), Om.cpu().numpy()
+    assert rel_l2(U, U_o) < TOL and rel_max(U, U_o) < TOL_MAX
+    assert rel_l2(Om, Om_o) < TOL and rel_max(Om, Om_o) < TOL_MAX
+    # the wall data really matter: the no-slip, resting-wall product differs
+    base = dataclasses.replace(prob, slip_0=0.0, slip_H=0.0, uwall_0=(0.0, 0.0), uwall_H=(0.0, 0.0))
+    with dp.Plan(base, max_particles=len(pos), use_torques=True, torque_mode=mode) as plan0:
+        U0, _ = plan0.mobility_apply(*to_dev(pos, F, T))
+    assert rel_l2(U, U0.cpu().numpy()) > 1e-3
+
+
+def test_wall_data_that_the_paper_gives_no_solution_for_are_rejected(dp):
+    import dataclasses
+    prob, pos, F, T = small_monolayer("bw", 100, 94)
+    for bad in (dict(slip_0=0.1), dict(slip_H=0.1), dict(uwall_H=(0.1, 0.0))):
+        with pytest.raises(dp.DPError):
+            dp.Plan(dataclasses.replace(prob, **bad), max_particles=len(pos))
+    probS, *_ = workloads.random_slit(n=10, L=32.0, nxy=48, nz=32, H=8.0, seed=1, name="s")
+    with pytest.raises(dp.DPError):
+        dp.Plan(dataclasses.replace(probS, slip_0=-0.1), max_particles=10)

@@ -47,6 +47,11 @@ class Problem:
     has_torque: bool = True     # torques in, Omega out
     seed: int = 0
     n: int = 0
+    # wall data of Appendix A / eq 27: partial slip lengths (slit only) and uniform wall velocities (x, y)
+    slip_0: float = 0.0
+    slip_H: float = 0.0
+    uwall_0: tuple = (0.0, 0.0)
+    uwall_H: tuple = (0.0, 0.0)
 
     @property
     def h(self) -> float:
