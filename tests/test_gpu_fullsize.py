@@ -57,21 +57,22 @@ def check_product(U, Om, U_o, Om_o):
     return stacked
 
 
-@pytest.mark.parametrize("cfg", [3, 4])
-def test_cfg3_cfg4_full_size_against_the_oracle(dp, cfg):
+@pytest.mark.parametrize("cfg,torque_mode", [(3, "fourier"), (4, "fourier"), (3, "kernel"), (4, "kernel")])
+def test_cfg3_cfg4_full_size_against_the_oracle(dp, cfg, torque_mode):
+    """torque_mode: "fourier" = curl in Fourier-Chebyshev space (6 fields), "kernel" = ES kernel derivative (3 fields, bench.py's default)"""
     import torch
     prob, pos, F, T = workloads.config(cfg)
     assert len(pos) == {3: 65536, 4: 262144}[cfg] and prob.nx == {3: 1080, 4: 2160}[cfg] and prob.nz == {3: 32, 4: 48}[cfg]
-    with dp.Plan(prob, max_particles=len(pos), use_torques=True) as plan:
+    with dp.Plan(prob, max_particles=len(pos), use_torques=True, torque_mode=1 if torque_mode == "kernel" else 0) as plan:
         assert plan.fft_backend() == "own"
         U, Om = plan.mobility_apply(*to_dev(pos, F, T))
         torch.cuda.synchronize()
         assert plan.check() == 0
         U, Om = U.cpu().numpy(), Om.cpu().numpy()
     torch.cuda.empty_cache()
-    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft")
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", torque_mode=torque_mode)
     err = check_product(U, Om, U_o, Om_o)
-    print("cfg%d full size: stacked rel L2 %.2e, per-particle max %.2e / %.2e" % (cfg, err, rel_max(U, U_o), rel_max(Om, Om_o)))
+    print("cfg%d (%s) full size: stacked rel L2 %.2e, per-particle max %.2e / %.2e" % (cfg, torque_mode, err, rel_max(U, U_o), rel_max(Om, Om_o)))
 
 
 def _sample_modes(prob, rng, n_random=3000):
@@ -184,19 +185,20 @@ def test_cfg5_full_size_stage_by_stage_against_the_oracle(dp):
 
 
 @pytest.mark.skipif(os.environ.get("DP_FULL_ORACLE_CFG5") == "0", reason="whole oracle product at config 5 switched off (DP_FULL_ORACLE_CFG5=0)")
-def test_cfg5_whole_product_against_the_whole_oracle(dp):
-    """Config 5 as bench.py runs it against the WHOLE oracle product (about 60 GB of host memory and two minutes on the 16-core
-    GPU box; DP_FULL_ORACLE_CFG5=0 skips it on a smaller host)."""
+@pytest.mark.parametrize("torque_mode", ["kernel", "fourier"])
+def test_cfg5_whole_product_against_the_whole_oracle(dp, torque_mode):
+    """Config 5 as bench.py runs it (default torque mode "kernel"; "fourier" is its second timed form) against the WHOLE oracle
+    product (up to about 60 GB of host memory and two minutes on the 16-core GPU box; DP_FULL_ORACLE_CFG5=0 skips it on a smaller host)."""
     import torch
     prob, pos, F, T = workloads.config(5)
-    with dp.Plan(prob, max_particles=len(pos), use_torques=True) as plan:
+    with dp.Plan(prob, max_particles=len(pos), use_torques=True, torque_mode=1 if torque_mode == "kernel" else 0) as plan:
         U, Om = plan.mobility_apply(*to_dev(pos, F, T))
         torch.cuda.synchronize()
         assert plan.check() == 0
         U, Om = U.cpu().numpy(), Om.cpu().numpy()
     torch.cuda.empty_cache()
     tm = {}
-    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", timing=tm)
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", timing=tm, torque_mode=torque_mode)
     err = check_product(U, Om, U_o, Om_o)
-    print("cfg5 whole oracle: stacked rel L2 %.2e, per-particle max %.2e / %.2e, oracle seconds %s" % (
+    print("cfg5 (" + torque_mode + ") whole oracle: stacked rel L2 %.2e, per-particle max %.2e / %.2e, oracle seconds %s" % (
         err, rel_max(U, U_o), rel_max(Om, Om_o), {k: round(v, 1) for k, v in tm.items()}))
