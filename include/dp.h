@@ -88,6 +88,11 @@ typedef struct {
                            eq 52 / (A12); the product becomes affine, U = M F + (flow driven by the walls)                          */
   double uwall_H[2];    /* uniform velocity (x, y) of the top wall; slit only ((A1b), (A12)); must be 0 for DP_BOTTOM_WALL.
                            Non-uniform wall velocity fields u_wall(x, y) are not supported.                                          */
+  int solve_kernel;     /* which kernel runs steps 2(z)-6 of products with three grid fields each way (forces only, or
+                           torque_mode = 1).  0 (default): the register-resident warp-pair kernel (solve_pair.cu) where it is compiled
+                           (nz in {16, 19, 24, 26, 32, 40, 48}), else the tile kernel;  1: always the tile kernel (solve.cu; kept for
+                           comparison).  Products with six fields (torque_mode = 0 with torques) always use the tile kernel.  Both solve
+                           the same discrete problem; results agree to roundoff.                                                      */
 } dp_params;
 
 /* Plan creation for the problem of PAPER.md:74 (box, walls) with the grid of PAPER.md:319 and the ES kernel of eq 54.

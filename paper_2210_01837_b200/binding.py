@@ -29,7 +29,8 @@ class dp_params(ctypes.Structure):
                 ("max_particles", ctypes.c_int), ("transfer_fp32", ctypes.c_int), ("device", ctypes.c_int),
                 # extensions beyond SURVEY.md §8(b)
                 ("use_torques", ctypes.c_int), ("fft_backend", ctypes.c_int), ("dense_planes", ctypes.c_int), ("torque_mode", ctypes.c_int),
-                ("slip_0", ctypes.c_double), ("slip_H", ctypes.c_double), ("uwall_0", ctypes.c_double * 2), ("uwall_H", ctypes.c_double * 2)]
+                ("slip_0", ctypes.c_double), ("slip_H", ctypes.c_double), ("uwall_0", ctypes.c_double * 2), ("uwall_H", ctypes.c_double * 2),
+                ("solve_kernel", ctypes.c_int)]
 
 
 _lib = None
@@ -127,7 +128,7 @@ class Plan:
     """dp_create / dp_mobility_apply / dp_destroy.  ``prob`` is any object with the fields of ``workloads.Problem``."""
 
     def __init__(self, prob, max_particles: int, use_torques=None, device: int = 0, fft_backend: int = 0, transfer_fp32: bool = False,
-                 dense_planes: bool = False, torque_mode: int = 0):
+                 dense_planes: bool = False, torque_mode: int = 0, solve_kernel: int = 0):
         self._h = None
         L = load_library()
         if use_torques is None:
@@ -138,7 +139,8 @@ class Plan:
                                 int(bool(use_torques)), int(fft_backend), int(bool(dense_planes)), int(torque_mode),
                                 float(getattr(prob, "slip_0", 0.0)), float(getattr(prob, "slip_H", 0.0)),
                                 (ctypes.c_double * 2)(*[float(v) for v in getattr(prob, "uwall_0", (0.0, 0.0))]),
-                                (ctypes.c_double * 2)(*[float(v) for v in getattr(prob, "uwall_H", (0.0, 0.0))]))
+                                (ctypes.c_double * 2)(*[float(v) for v in getattr(prob, "uwall_H", (0.0, 0.0))]),
+                                int(solve_kernel))
         h = ctypes.c_void_p()
         rc = L.dp_create(ctypes.byref(self.params), ctypes.byref(h))
         if rc != 0:

@@ -8,8 +8,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libdpstokes.so")
-SOURCES = ["plan.cu", "transfer.cu", "solve.cu", "fft.cu", "lanczos.cu"]
-HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "fft_engine.cuh"), os.path.join(CSRC, "fft_radix.cuh"), os.path.join(os.path.dirname(HERE), "include", "dp.h")]
+SOURCES = ["plan.cu", "transfer.cu", "solve.cu", "solve_pair.cu", "fft.cu", "lanczos.cu"]
+HEADERS = [os.path.join(CSRC, "common.cuh"), os.path.join(CSRC, "solve_common.cuh"), os.path.join(CSRC, "fft_engine.cuh"), os.path.join(CSRC, "fft_radix.cuh"), os.path.join(os.path.dirname(HERE), "include", "dp.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--extended-lambda", "-Xcompiler", "-fPIC"]
 
 

@@ -67,6 +67,8 @@ struct dp_plan {
   void* host_stage = nullptr;   // device staging buffers of dp_mobility_apply_host (plan.cu), allocated on first use
   double* d_ct_full = nullptr;  // cos(n l pi/(nz-1)) [nz][nz] for the k = 0 kernel (solve.cu), per plan
   double* d_solve_frag = nullptr;  // DMMA fragment table of the Chebyshev transforms (solve.cu), per plan
+  bool solve_force_tile = false;   // dp_params.solve_kernel = 1: keep the tile kernel of solve.cu for every product (comparison runs)
+  void* solve_pair_tab = nullptr;  // host copy of the tables the warp-pair solve kernel takes as a kernel parameter (solve_pair.cu)
 
   cudaStream_t last_stream = nullptr;
   bool profiling = false;
@@ -85,6 +87,10 @@ cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega,
 cudaError_t dp_solve_upload_tables(dp_plan* P);      // per plan: constant tables, k = 0 cosine table, kernel attributes on the plan's device
 void dp_solve_destroy_tables(dp_plan* P);
 bool dp_solve_supports_nz(int nz);
+// solve_pair.cu: the solve kernel of products with three grid fields each way (forces only / kernel-derivative torques)
+bool dp_solve_pair_supports_nz(int nz);
+cudaError_t dp_solve_pair_create(dp_plan* P);
+void dp_solve_pair_destroy(dp_plan* P);
 int dp_solve_nz_list(int* out, int cap);
 // fft.cu: the xy FFTs as two shared-memory passes per direction
 bool dp_fft_own_supported(int nx, int ny);

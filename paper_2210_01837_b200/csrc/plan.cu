@@ -348,6 +348,7 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   if (p.transfer_fp32 != 0 && p.transfer_fp32 != 1) return DP_EINVAL;
   if (p.dense_planes != 0 && p.dense_planes != 1) return DP_EINVAL;
   if (p.torque_mode != 0 && p.torque_mode != 1) return DP_EINVAL;
+  if (p.solve_kernel != 0 && p.solve_kernel != 1) return DP_EINVAL;
   if (!(p.slip_0 >= 0) || !(p.slip_H >= 0) || !std::isfinite(p.slip_0) || !std::isfinite(p.slip_H)) return DP_EINVAL;
   for (int c = 0; c < 2; ++c) if (!std::isfinite(p.uwall_0[c]) || !std::isfinite(p.uwall_H[c])) return DP_EINVAL;
   if (p.wall_mode == DP_BOTTOM_WALL && (p.slip_0 != 0 || p.slip_H != 0 || p.uwall_H[0] != 0 || p.uwall_H[1] != 0)) return DP_EINVAL;
@@ -367,6 +368,7 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   P->nkxp = (P->nkx + 7) / 8 * 8;
   P->torques = p.use_torques != 0;
   P->kernel_torque = P->torques && p.torque_mode == 1;
+  P->solve_force_tile = p.solve_kernel == 1;
   P->fields = (P->torques && !P->kernel_torque) ? 6 : 3;
   P->nrec = P->torques ? (P->kernel_torque ? 3 : 2) : 1;
   P->ucutD = P->kernel_torque ? es_dphi_cut_host(p.beta_D) : 1.0;
