@@ -39,9 +39,10 @@ template <int NZ> struct PG {
 // tables of one plan: analysis A[par][l][j] (times 1/(nx ny): the inverse FFT is unnormalised; j = output index runs fastest, so the
 // sixteen entries an input value meets are adjacent in the constant bank), synthesis S[par][l][j] (the coefficient index j fastest: an output value is a dot product with one row), boundary-row functionals
 // P_n, Q_n (see chains()), nodes xi_l = cos(l pi/N)
-template <int NZ> struct PairTab {
-  double A[2][PG<NZ>::NE][PG<NZ>::NE];
-  double S[2][PG<NZ>::NE][PG<NZ>::NE];
+template <int NZ> struct alignas(16) PairTab {
+  static constexpr int NEP = (PG<NZ>::NE + 1) & ~1;      // rows padded to whole 16-byte pairs (LDCU.128)
+  double A[2][PG<NZ>::NE][NEP];
+  double S[2][PG<NZ>::NE][NEP];
   double P[NZ], Q[NZ], XI[NZ];
 };
 struct PairConst { double s, inv_s, sc, inv_2eta; };      // H/2, 2/H, (H/2)^2 / eta, 1/(2 eta): computed once on the host
@@ -64,8 +65,8 @@ template <int NZ> struct PairSmem {
   // cover each other's loads and barrier waits.
   static constexpr int PAIRS_SM = (227 * 1024 - 2048) / (DOUBLES * 8);       // pairs whose shared memory fits one SM
 #ifndef DP_PAIR_CTAS
-#define DP_PAIR_CTAS 2
-#define DP_PAIR_NPAIR 3
+#define DP_PAIR_CTAS 1
+#define DP_PAIR_NPAIR 6
 #endif
   static constexpr int CTAS = PAIRS_SM >= DP_PAIR_CTAS ? DP_PAIR_CTAS : 1;
   static constexpr int NPAIR = PAIRS_SM / CTAS >= DP_PAIR_NPAIR ? DP_PAIR_NPAIR : (PAIRS_SM / CTAS >= 1 ? PAIRS_SM / CTAS : 1);
@@ -270,11 +271,15 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
       const double gb = alone ? 0.0 : NB[c * VS + (N - l) * LN + lane];
       x[c] = PAR ? ga - gb : ga + gb;
     }
-    const double* t = &T.A[PAR][l][0];
+    const double2* t = reinterpret_cast<const double2*>(&T.A[PAR][l][0]);
 #pragma unroll
-    for (int j = 0; j < NH; ++j) {
+    for (int j = 0; j < NH; j += 2) {
+      const double2 tt = t[j >> 1];
 #pragma unroll
-      for (int c = 0; c < 3; ++c) f[c][j] = fma(t[j], x[c], f[c][j]);
+      for (int c = 0; c < 3; ++c) {
+        f[c][j] = fma(tt.x, x[c], f[c][j]);
+        if (j + 1 < NH) f[c][j + 1] = fma(tt.y, x[c], f[c][j + 1]);
+      }
     }
   }
   pair_sync<NZ>();                                   // both warps have read the nodal columns: the buffer now carries the hand-overs
@@ -332,61 +337,47 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
   }
   pair_sync<NZ>();
 
-  // ---- 4. velocity BVPs (eq 18) with BCs (22), (24): w first (f^z - dz p is its right-hand side; frees f^z), then u and v together
+  // ---- 4. velocity BVPs (eq 18) with BCs (22), (24), the three components together (one load of the factors, three independent
+  // dependency chains per lane)
   double uc[3][NH];
   {
     const ModeK K = load_modek(SUM, lane);
     const double se = SUM[(0 * 8 + 0) * LN + lane], so = SUM[(1 * 8 + 0) * LN + lane];
     const double pH = se + so, p0 = se - so;               // p(H) = sum p_n, p(0) = sum (-1)^n p_n ("direct summation")
+    const double pHo = __shfl_xor_sync(0xffffffffu, pH, 1), p0o = __shfl_xor_sync(0xffffffffu, p0, 1);
     const double sc = PA.c.sc, inv_2eta = PA.c.inv_2eta;
-    {
-      // r = (dz p - f_z)/eta;  (dz +- k) w = p/(2 eta) at z = H, 0 (eq 24)
-      double a[1][NR], rho0[1] = {0.0}, bbc[1];
+    double a[3][NR], rho0[3] = {0.0, 0.0, 0.0}, bbc[3];
+    const double fu = K.sgI * K.kxt, fv = K.sgI * K.kyt;
 #pragma unroll
-      for (int j = 0; j < NH; ++j) {
-        const int n = 2 * j + PAR;
-        if (n <= N - 2) {
-          const double dzp = X2[((PAR ? 0 : NO) + j) * LN + lane] * inv_s;
-          const double rw = (dzp - f[2][j]) * sc;
-          if (n >= n0) a[0][(n - n0) / 2] = rw; else rho0[0] = rw;
-        }
+    for (int j = 0; j < NH; ++j) {
+      const int n = 2 * j + PAR;
+      if (n <= N - 2) {
+        // r = (i k_c p - f_c)/eta (c = x, y);  r = (dz p - f_z)/eta
+        const double po = __shfl_xor_sync(0xffffffffu, pc[0][j], 1);
+        const double dzp = X2[((PAR ? 0 : NO) + j) * LN + lane] * inv_s;
+        const double ru = fma(fu, po, -f[0][j]) * sc, rv = fma(fv, po, -ST[j * LN + lane]) * sc, rw = (dzp - f[2][j]) * sc;
+        if (n >= n0) { a[0][(n - n0) / 2] = ru; a[1][(n - n0) / 2] = rv; a[2][(n - n0) / 2] = rw; }
+        else { rho0[0] = ru; rho0[1] = rv; rho0[2] = rw; }
       }
-      const double gH = pH * inv_2eta, g0 = p0 * inv_2eta;
-      bbc[0] = PAR ? 0.5 * (gH + g0) : 0.5 * (gH - g0);
-      double bo[1][NH], border[1], Sc[1], Sb[1];
-      double (&wc)[1][NH] = *reinterpret_cast<double (*)[1][NH]>(&uc[2]);
-      chains<NZ, PAR, 1>(A, T, a, rho0, bbc, Fi, Fa, K.k, K.k2, inv_s, invBg, wc, bo, border, Sc, Sb);
-      SUM[(PAR * 8 + 3) * LN + lane] = Sc[0];
     }
-    DP_SPLIT(A, 7);
-    {
-      // r = (i k_c p - f_c)/eta;  (dz + k) u(H) = -(i k_c/(2 k eta)) p(H), (dz - k) u(0) = +(i k_c/(2 k eta)) p(0) (eq 22)
-      const double pHo = __shfl_xor_sync(0xffffffffu, pH, 1), p0o = __shfl_xor_sync(0xffffffffu, p0, 1);
-      double a[2][NR], rho0[2] = {0.0, 0.0}, bbc[2];
+    // (dz + k) u(H) = -(i k_c/(2 k eta)) p(H), (dz - k) u(0) = +(i k_c/(2 k eta)) p(0) (eq 22); (dz +- k) w = p/(2 eta) at z = H, 0 (eq 24)
+    const double inv_k = dp_rcp(K.k);
 #pragma unroll
-      for (int j = 0; j < NH; ++j) {
-        const int n = 2 * j + PAR;
-        if (n <= N - 2) {
-          const double po = __shfl_xor_sync(0xffffffffu, pc[0][j], 1);
-          const double ru = (K.sgI * K.kxt * po - f[0][j]) * sc, rv = (K.sgI * K.kyt * po - ST[j * LN + lane]) * sc;
-          if (n >= n0) { a[0][(n - n0) / 2] = ru; a[1][(n - n0) / 2] = rv; }
-          else { rho0[0] = ru; rho0[1] = rv; }
-        }
+    for (int c = 0; c < 3; ++c) {
+      double gH, g0;
+      if (c < 2) {
+        const double cfc = (c == 0 ? K.kxt : K.kyt) * inv_k * inv_2eta;
+        gH = -K.sgI * cfc * pHo; g0 = K.sgI * cfc * p0o;
+      } else {
+        gH = pH * inv_2eta; g0 = p0 * inv_2eta;
       }
-#pragma unroll
-      const double inv_k = dp_rcp(K.k);
-#pragma unroll
-      for (int c = 0; c < 2; ++c) {
-        const double cf = (c == 0 ? K.kxt : K.kyt) * inv_k * inv_2eta;
-        const double gH = -K.sgI * cf * pHo, g0 = K.sgI * cf * p0o;
-        bbc[c] = PAR ? 0.5 * (gH + g0) : 0.5 * (gH - g0);
-      }
-      double bo[2][NH], border[2], Sc[2], Sb[2];
-      double (&uvc)[2][NH] = *reinterpret_cast<double (*)[2][NH]>(&uc[0]);
-      chains<NZ, PAR, 2>(A, T, a, rho0, bbc, Fi, Fa, K.k, K.k2, inv_s, invBg, uvc, bo, border, Sc, Sb);
-      SUM[(PAR * 8 + 1) * LN + lane] = Sc[0]; SUM[(PAR * 8 + 2) * LN + lane] = Sc[1];
-      if (A.slip) { SUM[(PAR * 8 + 4) * LN + lane] = Sb[0]; SUM[(PAR * 8 + 5) * LN + lane] = Sb[1]; }
+      bbc[c] = PAR ? 0.5 * (gH + g0) : 0.5 * (gH - g0);
     }
+    double bo[3][NH], border[3], Sc[3], Sb[3];
+    chains<NZ, PAR, 3>(A, T, a, rho0, bbc, Fi, Fa, K.k, K.k2, inv_s, invBg, uc, bo, border, Sc, Sb);
+#pragma unroll
+    for (int c = 0; c < 3; ++c) SUM[(PAR * 8 + 1 + c) * LN + lane] = Sc[c];
+    if (A.slip) { SUM[(PAR * 8 + 4) * LN + lane] = Sb[0]; SUM[(PAR * 8 + 5) * LN + lane] = Sb[1]; }
   }
   DP_SPLIT(A, 8);
 
@@ -398,13 +389,17 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
     constexpr int LE = NH & ~1;
 #pragma unroll 1
     for (int l = 0; l < LE; l += 2) {
-      const double* t0 = &T.S[PAR][l][0];
-      const double* t1 = &T.S[PAR][l + 1][0];
+      const double2* t0 = reinterpret_cast<const double2*>(&T.S[PAR][l][0]);
+      const double2* t1 = reinterpret_cast<const double2*>(&T.S[PAR][l + 1][0]);
       double g0[3] = {0.0, 0.0, 0.0}, g1[3] = {0.0, 0.0, 0.0};
 #pragma unroll
-      for (int j = 0; j < NH; ++j) {
+      for (int j = 0; j < NH; j += 2) {
+        const double2 ta = t0[j >> 1], tb = t1[j >> 1];
 #pragma unroll
-        for (int c = 0; c < 3; ++c) { g0[c] = fma(t0[j], uc[c][j], g0[c]); g1[c] = fma(t1[j], uc[c][j], g1[c]); }
+        for (int c = 0; c < 3; ++c) {
+          g0[c] = fma(ta.x, uc[c][j], g0[c]); g1[c] = fma(tb.x, uc[c][j], g1[c]);
+          if (j + 1 < NH) { g0[c] = fma(ta.y, uc[c][j + 1], g0[c]); g1[c] = fma(tb.y, uc[c][j + 1], g1[c]); }
+        }
       }
 #pragma unroll
       for (int c = 0; c < 3; ++c) {
