@@ -441,6 +441,41 @@ def test_every_compiled_chebyshev_size_and_kernel_width(dp, nz, w, wall):
         assert rel_max(U.cpu().numpy(), U_o) < TOL_MAX and rel_max(Om.cpu().numpy(), Om_o) < TOL_MAX
 
 
+# ------------------------------------------------------------------------------------------------ the two solve kernels
+@pytest.mark.parametrize("case", ["bw-forces", "slit-forces-nz26", "slit-kernel-torques-slip", "bw-kernel-torques-ragged-nz19"])
+def test_both_solve_kernels_match_the_oracle_and_each_other(dp, case):
+    """Products with three grid fields each way run steps 2(z)-6 (PAPER.md:326-331) in the warp-pair kernel (solve_pair.cu) by default;
+    dp_params.solve_kernel = 1 keeps the tile kernel (solve.cu).  Both solve the oracle's discrete problem: each <= 1e-10 from the
+    oracle, and they agree with one another to roundoff (the nodal correction equals the coefficient-space one)."""
+    import dataclasses
+    if case == "bw-forces":
+        prob, pos, F, T = workloads.random_bw(n=300, L=40.0, nxy=60, nz=32, H=9.0, seed=811, name=case)
+        T = None; mode = 0
+    elif case == "slit-forces-nz26":
+        prob, pos, F, T = workloads.random_slit(n=300, L=36.0, nxy=54, nz=26, H=8.0, seed=812, name=case)
+        prob = dataclasses.replace(prob, has_torque=False); T = None; mode = 0
+    elif case == "slit-kernel-torques-slip":
+        prob, pos, F, T = workloads.random_slit(n=300, L=32.0, nxy=48, nz=40, H=8.0, seed=813, name=case)
+        prob = dataclasses.replace(prob, slip_0=0.3, slip_H=0.7); mode = 1
+    else:
+        prob, pos, F, _ = workloads.random_bw(n=200, L=40.0, nxy=50, nz=19, H=9.0, zlo=0.0, zhi=6.0, seed=814, name=case)   # 50 = 3 tiles of 16 + 2
+        T = np.random.default_rng(814).standard_normal(F.shape); prob = dataclasses.replace(prob, has_torque=True, beta_M=6 * 1.327, beta_D=6 * 2.216); mode = 1
+    use_t = T is not None
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", torque_mode="kernel" if mode else "fourier")
+    out = {}
+    for sk in (0, 1):
+        with dp.Plan(prob, max_particles=len(pos), use_torques=use_t, torque_mode=mode, solve_kernel=sk) as plan:
+            U, Om = plan.mobility_apply(*to_dev(pos, F, T))
+            assert plan.check() == 0
+            out[sk] = (U.cpu().numpy(), None if Om is None else Om.cpu().numpy())
+        assert rel_l2(out[sk][0], U_o) < TOL and rel_max(out[sk][0], U_o) < TOL_MAX, (case, sk)
+        if use_t:
+            assert rel_l2(out[sk][1], Om_o) < TOL and rel_max(out[sk][1], Om_o) < TOL_MAX, (case, sk)
+    assert rel_l2(out[0][0], out[1][0]) < 1e-12
+    if use_t:
+        assert rel_l2(out[0][1], out[1][1]) < 1e-12
+
+
 # ------------------------------------------------------------------------------------------------ Lanczos square root (SURVEY.md §8 f-2)
 @pytest.mark.parametrize("with_torque,mode", [(False, 0), (True, 1), (True, 0)])
 def test_lanczos_square_root_matches_the_oracle_iteration(dp, with_torque, mode):
