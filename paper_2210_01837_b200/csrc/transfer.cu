@@ -215,6 +215,12 @@ __global__ void k_weights(int n, WeightArgs A) {
 }
 
 // ---------------------------------------------------------------------------------------------- spread
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all_groups() { asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory"); }
+
 struct SpreadArgs {
   GridGeom g;
   const double* val_s[2];    // forces, torques (sorted)
@@ -340,12 +346,15 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
           s_val[t][0] = val[3 * (size_t)p]; s_val[t][1] = val[3 * (size_t)p + 1]; s_val[t][2] = val[3 * (size_t)p + 2];
         }
       }
-#pragma unroll 2
+      // the weight records travel as asynchronous 8-byte copies: all of a thread's entries are in flight at once (one round of
+      // global latency per chunk instead of one per two entries)
       for (int i = t; i < nl * NREC * WS; i += SPREAD_THREADS) {
         const int q = i / (NREC * WS), rem = i - q * (NREC * WS), k = rem / WS, e = rem - k * WS;
         const int kk = MODE ? k : grp;
-        s_w[q][k][e] = e < WREC ? A.wrec[((size_t)kk * A.cap + s_keep[c0 + q]) * WREC + e] : 0.0;
+        if (e < WREC) cp_async8(&s_w[q][k][e], A.wrec + ((size_t)kk * A.cap + s_keep[c0 + q]) * WREC + e);
+        else s_w[q][k][e] = 0.0;
       }
+      cp_async_wait_all_groups();
       __syncthreads();
       // ---- accumulate: each thread adds the particles covering its column to its own planes
       if (in_grid) {
