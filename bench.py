@@ -30,8 +30,9 @@ import numpy as np
 import workloads
 
 METRIC = "ms per DP-wall mobility product M·F at N=1M; particles/s; % of HBM roofline"
-# kernels of this library launched per product: k_bin_count, k_scan, k_bin_scatter, k_weights, k_spread, k_solve<nz>, k_zero_mode,
-# k_interp, plus k_fft_x_fwd, k_fft_y_fwd, k_fft_y_inv, k_fft_x_inv with the library's own FFT passes (else cuFFT's kernels)
+# kernels of this library launched per product: k_bin_count, k_scan, k_bin_scatter, k_weights, k_spread, k_solve_pair<nz> (three grid
+# fields each way) or k_solve<nz> (six), k_zero_mode, k_interp, plus k_fft_x_fwd, k_fft_y_fwd, k_fft_y_inv, k_fft_x_inv with the
+# library's own FFT passes (else cuFFT's kernels)
 MY_KERNELS_PER_STEP = {"own": 12, "cufft": 8}
 
 
@@ -232,7 +233,7 @@ def kernel_bytes(prob, n, fin, fout, zero_planes=0):
 
 
 def measure(dp, torch, prob, pos, F, T, dev, dist, args, *, torque_mode, transfer_fp32=False, dense_planes=False, fft="own",
-            e2e=False, clocks=False, steps=None):
+            e2e=False, clocks=False, steps=None, solve_kernel=0):
     """One timed run: plan, warm-ups, K products between CUDA events on the launching stream (max over ranks), then per-stage and
     per-FFT-pass times from the plan's own events in a separate pass, then (optionally) the end-to-end run through host buffers."""
     steps = steps or args.steps
@@ -240,8 +241,9 @@ def measure(dp, torch, prob, pos, F, T, dev, dist, args, *, torque_mode, transfe
     use_t = T is not None
     tmode = 1 if (torque_mode == "kernel" and use_t) else 0
     plan = dp.Plan(prob, max_particles=n, use_torques=use_t, device=dev.index, fft_backend=0 if fft == "own" else 1,
-                   transfer_fp32=transfer_fp32, dense_planes=dense_planes, torque_mode=tmode)
-    out = {"torque_mode": (torque_mode if use_t else "none"), "fields": plan.fields, "fft_backend": plan.fft_backend(), "plan_device_GB": plan.device_bytes() / 1e9}
+                   transfer_fp32=transfer_fp32, dense_planes=dense_planes, torque_mode=tmode, solve_kernel=solve_kernel)
+    out = {"torque_mode": (torque_mode if use_t else "none"), "fields": plan.fields, "fft_backend": plan.fft_backend(), "plan_device_GB": plan.device_bytes() / 1e9,
+           "solve_kernel": ("k_solve_pair<%d>" if (plan.fields == 3 and plan.solve_kernel() == "pair") else "k_solve<%d>") % prob.nz}
     dpos = torch.from_numpy(pos).to(dev)
     dF = torch.from_numpy(F).to(dev)
     dT = torch.from_numpy(T).to(dev) if use_t else None
@@ -366,6 +368,9 @@ def main():
                     help="torques / Omega through the ES kernel's derivative (3 grid fields each way; the paper's second way, PAPER.md:335) "
                          "or through the curl in Fourier-Chebyshev space (6 fields; its first way)")
     ap.add_argument("--fft", choices=["own", "cufft"], default="own", help="xy FFT backend (own shared-memory passes, or cuFFT for comparison)")
+    ap.add_argument("--solve-kernel", choices=["pair", "tile"], default="pair",
+                    help="kernel of the per-wavenumber solve for products with three grid fields each way: the register-resident warp-pair "
+                         "kernel (default) or the tile kernel (dp_params.solve_kernel = 1; always used with six fields)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl != "reference" else args.warmup
 
@@ -396,14 +401,18 @@ def main():
     M = lambda **kw: measure(dp, torch, prob, pos, F, T, dev, dist, args, **kw)
 
     # ---- the headline run: device-resident timing, clocks sampled during the timed region, end to end through host buffers
+    sk = 0 if args.solve_kernel == "pair" else 1
     main_run = M(torque_mode=args.torque_mode, transfer_fp32=args.transfer_fp32, dense_planes=args.dense_planes, fft=args.fft,
-                 e2e=not args.no_e2e, clocks=True)
+                 e2e=not args.no_e2e, clocks=True, solve_kernel=sk)
     ms_step = main_run["ms_per_step"]
     value = whole_job_value(n, world, ms_step)
 
     # ---- the same product on the same inputs in its other forms, same rules (3 warm-ups, CUDA events, max over ranks)
-    other = variant = dense = fig9 = None
+    other = variant = dense = fig9 = tile = None
     if not args.no_variants and args.fft == "own":
+        if main_run["solve_kernel"].startswith("k_solve_pair"):
+            tile = M(torque_mode=args.torque_mode, transfer_fp32=args.transfer_fp32, dense_planes=args.dense_planes, solve_kernel=1)
+            tile["what"] = "same product with dp_params.solve_kernel = 1: the tile kernel (solve.cu) instead of the warp-pair kernel (solve_pair.cu) in the solve stage"
         if T is not None:
             om = "fourier" if args.torque_mode == "kernel" else "kernel"
             other = M(torque_mode=om, transfer_fp32=args.transfer_fp32, dense_planes=args.dense_planes)
@@ -440,7 +449,7 @@ def main():
     cand = ktab if ktab else {"k_solve": {"ms": stages["solve"]["ms"], "GBps": stages["solve"]["GBps"], "frac": stages["solve"]["frac"],
                                           "algorithmic_GB": stages["solve"]["algorithmic_GB"], "algorithmic_GB_if_all_planes_dense": None}}
     dom = max(cand, key=lambda k: cand[k]["ms"])
-    kname = {"k_solve": "k_solve<%d>" % prob.nz}.get(dom, dom)
+    kname = {"k_solve": main_run["solve_kernel"]}.get(dom, dom)
     traffic, traffic_file = ncu_traffic(dom, args.config, main_run["torque_mode"] if T is not None else "kernel")
     frac_dense = None
     if dense is not None:
@@ -452,8 +461,8 @@ def main():
                 "peak_source": peak_src,
                 "bytes": "the kernel's own compulsory reads + writes with the planes no footprint reaches left out (algorithmic_GB); "
                          "frac_if_all_planes_dense: SURVEY.md §8(d)'s dense bytes over the time of the dense_planes = 1 run",
-                "note": "k_solve is co-bound by the fp64 pipe (DFMA + DMMA share it), the shared-memory pipe and instruction issue "
-                        "(profiles/r2_*): the fraction is of the HBM roofline, as the contract asks",
+                "note": "the solve kernel is bound by the fp64 pipe and instruction issue, not by HBM (k_solve_pair: about 3.7 k fp64 instructions per "
+                        "warp and 16 modes against 64 FMA lanes per clock and SM; profiles/r2_*): the fraction is of the HBM roofline, as the contract asks",
                 "kernels": ktab}
     roofline.update(agg)
 
@@ -482,12 +491,12 @@ def main():
                            fields_in=fin, fields_out=fout, w=prob.w, torque_mode=main_run["torque_mode"],
                            l2="inputs (%.1f GB of grids per product) far exceed the 126 MB L2" % (by_total / 1e9 / 4),
                            parallelism="replicas" if world > 1 else "single GPU", plan_device_GB=main_run["plan_device_GB"],
-                           fft_backend=main_run["fft_backend"], transfer_fp32=bool(args.transfer_fp32),
+                           fft_backend=main_run["fft_backend"], solve_kernel=main_run["solve_kernel"], transfer_fp32=bool(args.transfer_fp32),
                            zero_planes_skipped=main_run["zero_planes"], nz=prob.nz),
             "clocks": main_run.get("clocks"), "e2e": main_run.get("e2e"), "gpu_launches": MY_KERNELS_PER_STEP[main_run["fft_backend"]] * args.steps,
             "stages": stages, "roofline": roofline, "cpu_baseline": cpu,
             ("fourier_curl_torques" if args.torque_mode == "kernel" else "kernel_derivative_torques"): brief(other),
-            "fp32_transfer_variant": brief(variant), "all_planes_dense": brief(dense), "paper_fig9": fig9}
+            "fp32_transfer_variant": brief(variant), "all_planes_dense": brief(dense), "tile_solve_kernel": brief(tile), "paper_fig9": fig9}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

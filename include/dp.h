@@ -163,6 +163,8 @@ int dp_copy_plane_to_host(dp_plan* plan, int which, int field, int l, void* host
 int dp_complex_row_pitch(const dp_plan* plan); /* nkxp: padded row length (in complex numbers) of the half spectrum */
 int dp_zero_planes(dp_plan* plan);             /* synchronises; number of leading planes (l = 0 is z = H) the last apply skipped */
 int dp_fft_backend(const dp_plan* plan);       /* 0: own shared-memory FFT passes in use, 1: cuFFT                    */
+int dp_solve_kernel(const dp_plan* plan);      /* kernel of steps 2(z)-6 for products with three grid fields each way:
+                                                  0: warp-pair kernel (solve_pair.cu), 1: tile kernel (solve.cu; always used with six fields) */
 
 /* Introspection */
 double dp_es_norm(double alpha, double beta);                  /* Z of eq 54, Gauss-Legendre on the host */

@@ -14,7 +14,7 @@ _LIBNAME = os.path.join(_HERE, "libdpstokes.so")
 
 # every symbol include/dp.h declares
 EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_lanczos_sqrt", "dp_check", "dp_effective_radius", "dp_set_profiling", "dp_stage_ms", "dp_fft_pass_ms",
-           "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_copy_plane_to_host", "dp_complex_row_pitch", "dp_zero_planes", "dp_fft_backend", "dp_es_norm", "dp_es_radius_over_h",
+           "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_copy_plane_to_host", "dp_complex_row_pitch", "dp_zero_planes", "dp_fft_backend", "dp_solve_kernel", "dp_es_norm", "dp_es_radius_over_h",
            "dp_es_dphi_cut", "dp_supported_nz", "dp_device_bytes", "dp_strerror", "dp_last_error", "dp_destroy"]
 
 
@@ -82,6 +82,8 @@ def load_library():
     L.dp_zero_planes.restype = i
     L.dp_fft_backend.argtypes = [vp]
     L.dp_fft_backend.restype = i
+    L.dp_solve_kernel.argtypes = [vp]
+    L.dp_solve_kernel.restype = i
     L.dp_es_norm.argtypes = [d, d]
     L.dp_es_norm.restype = d
     L.dp_es_radius_over_h.argtypes = [i, d, i]
@@ -249,6 +251,10 @@ class Plan:
 
     def fft_backend(self) -> str:
         return ["own", "cufft"][int(load_library().dp_fft_backend(self._h))]
+
+    def solve_kernel(self) -> str:
+        """Kernel that runs steps 2(z)-6 of a product with three grid fields each way: "pair" (solve_pair.cu) or "tile" (solve.cu)."""
+        return ["pair", "tile"][int(load_library().dp_solve_kernel(self._h))]
 
     def device_bytes(self) -> int:
         return int(load_library().dp_device_bytes(self._h))

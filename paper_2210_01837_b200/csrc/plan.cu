@@ -509,6 +509,7 @@ size_t dp_buffer_bytes(const dp_plan* P, int which) {
 }
 
 int dp_fft_backend(const dp_plan* P) { return P ? (P->own_fft ? 0 : 1) : -1; }
+int dp_solve_kernel(const dp_plan* P) { return P ? ((P->solve_pair_tab && !P->solve_force_tile) ? 0 : 1) : -1; }
 
 int dp_zero_planes(dp_plan* P) {
   if (!P) return DP_EINVAL;
