@@ -77,14 +77,15 @@ def hbm_peak():
 
 def stage_bytes(prob, n, fin, fout, zero_planes=0):
     """Algorithmic (compulsory) bytes per product and stage: every grid value read once and
-    written once per stage.  Planes above every footprint hold no force (exactly zero): with ``zero_planes`` of the nz input
-    planes skipped, the input side of spread / forward FFT / solve shrinks by that share — the bytes really needed."""
+    written once per stage.  Planes above every footprint hold no force (exactly zero) and are never interpolated from: with
+    ``zero_planes`` of the nz planes skipped, spread / forward FFT / solve loads shrink by that share on the input side and
+    solve stores / inverse FFT / interpolation on the output side — the bytes really needed."""
     G = prob.nx * prob.ny * prob.nz
     Kz = (prob.nx // 2 + 1) * prob.ny * prob.nz
     R, C = 8.0 * G, 16.0 * Kz
     a = 1.0 - zero_planes / float(prob.nz)
-    return {"spread": a * fin * R + 72.0 * n, "fft_fwd": a * fin * (R + C), "solve": (a * fin + fout) * C,
-            "fft_inv": fout * (C + R), "interp": fout * R + 72.0 * n}
+    return {"spread": a * fin * R + 72.0 * n, "fft_fwd": a * fin * (R + C), "solve": a * (fin + fout) * C,
+            "fft_inv": a * fout * (C + R), "interp": a * fout * R + 72.0 * n}
 
 
 def replica_seed(base_seed: int, rank: int) -> int:
@@ -222,14 +223,14 @@ KERNELS = ("k_spread", "k_fft_x_fwd", "k_fft_y_fwd", "k_solve", "k_fft_y_inv", "
 
 def kernel_bytes(prob, n, fin, fout, zero_planes=0):
     """Bytes each kernel of the product must itself move (its compulsory reads + writes): R = one real field,
-    C = one half spectrum, a = share of the input planes that can hold force.  The two passes of a 2-D transform each read and
+    C = one half spectrum, a = share of the planes that a footprint reaches (the others hold no force and are never interpolated from).  The two passes of a 2-D transform each read and
     write the whole field once, so the two FFT kernels of a stage together move twice SURVEY.md §8(d)'s per-stage figure."""
     G = prob.nx * prob.ny * prob.nz
     Kz = (prob.nx // 2 + 1) * prob.ny * prob.nz
     R, C = 8.0 * G, 16.0 * Kz
     a = 1.0 - zero_planes / float(prob.nz)
     return {"k_spread": a * fin * R + 72.0 * n, "k_fft_x_fwd": a * fin * (R + C), "k_fft_y_fwd": a * fin * 2 * C,
-            "k_solve": (a * fin + fout) * C, "k_fft_y_inv": fout * 2 * C, "k_fft_x_inv": fout * (C + R), "k_interp": fout * R + 72.0 * n}
+            "k_solve": a * (fin + fout) * C, "k_fft_y_inv": a * fout * 2 * C, "k_fft_x_inv": a * fout * (C + R), "k_interp": a * fout * R + 72.0 * n}
 
 
 def measure(dp, torch, prob, pos, F, T, dev, dist, args, *, torque_mode, transfer_fp32=False, dense_planes=False, fft="own",
@@ -426,7 +427,7 @@ def main():
                                "matches the oracle to <= 1e-5 (tests)")
         if not args.dense_planes and main_run["zero_planes"] > 0:
             dense = M(torque_mode=args.torque_mode, transfer_fp32=args.transfer_fp32, dense_planes=True)
-            dense["what"] = ("same product with dense_planes = 1: the %d planes no footprint reaches are spread, transformed and loaded too"
+            dense["what"] = ("same product with dense_planes = 1: the %d planes no footprint reaches are spread, transformed, solved for and transformed back too"
                              % main_run["zero_planes"])
         if world == 1 and args.config == 5:
             # context for the paper's only published timing (Fig. 9): its own grid and kernel, forces only

@@ -222,25 +222,35 @@ __global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_inv(FftYArgs A) {
   fence_async_proxy();
   __syncthreads();
   unsigned phase = 0;
-  const long long nbatch = (A.rows + A.rb - 1) / A.rb;
+  // rows of the planes l >= lm of each field (the planes above every footprint are never interpolated from: their inverse transform
+  // is skipped, as their forward transform was): per field one contiguous range of ra rows, cut into batches of rb
+  int lm = A.lmin ? __ldg(A.lmin) : 0;
+  lm = lm < 0 ? 0 : (lm > A.nz ? A.nz : lm);
+  const long long ra = (long long)(A.nz - lm) * A.nkx, per_field = (ra + A.rb - 1) / A.rb;
+  const long long nbatch = per_field * A.fields;
   const long long stride = (long long)gridDim.x * YSLOTS;
+  auto batch = [&](long long bb, long long& row0, int& nr) {
+    const long long f = bb / per_field, j = bb - f * per_field;
+    row0 = (f * A.nz + lm) * A.nkx + j * A.rb;
+    nr = (int)((ra - j * A.rb) < A.rb ? (ra - j * A.rb) : A.rb);
+  };
   long long b = (long long)blockIdx.x * YSLOTS + slot;
   if (st == 0 && b < nbatch) {
-    const long long row0 = b * A.rb;
-    const int nr = (int)((A.rows - row0) < A.rb ? (A.rows - row0) : A.rb);
+    long long row0; int nr;
+    batch(b, row0, nr);
     mbar_expect_tx(mbar, (unsigned)nr * n * 16u);
     bulk_load(buf, A.data + row0 * n, (unsigned)nr * n * 16u, mbar);
   }
   for (; b < nbatch; b += stride) {
-    const long long row0 = b * A.rb;
-    const int nr = (int)((A.rows - row0) < A.rb ? (A.rows - row0) : A.rb);
+    long long row0; int nr;
+    batch(b, row0, nr);
     double2* g = A.data + row0 * n;
     mbar_wait(mbar, phase);
     phase ^= 1;
     run_inner<YTPS, R0, R1, R2, true, true>(A, buf, tw, n, nr, st, slot);
-    const long long nrow0 = (b + stride) * A.rb;
     const bool more = b + stride < nbatch;
-    const int nnr = more ? (int)((A.rows - nrow0) < A.rb ? (A.rows - nrow0) : A.rb) : 0;
+    long long nrow0 = 0; int nnr = 0;
+    if (more) batch(b + stride, nrow0, nnr);
     // the refill of the buffer is issued after the last stage (issuing it between that stage's loads and its arithmetic costs the
     // stage 200 bytes of spills per thread; the other slots of the CTA cover the load's latency)
     run_edge<YTPS, R0, true>(A.F.r[0], buf, g, tw + A.off[0], n, nr, st, MidNone());
@@ -311,12 +321,16 @@ __global__ void __launch_bounds__(XTHREADS, 1) k_fft_x_inv(FftXArgs A) {
   for (int i = threadIdx.x; i < npost; i += XTHREADS) post[i] = A.post[i];
   __syncthreads();
   const int rb = A.rb, ny = A.ny, nkx = M + 1;
-  const long long nbatch = A.planes * (ny / rb);
+  int lm = A.lmin ? __ldg(A.lmin) : 0;                   // planes l < lm are never interpolated from: not transformed back
+  lm = lm < 0 ? 0 : (lm > A.nz ? A.nz : lm);
+  const int act = A.nz - lm, bpp = ny / rb;
+  const long long nbatch = (A.planes / A.nz) * act * bpp;
   const MidNone nomid;
   for (long long b = (long long)blockIdx.x * XSLOTS + slot; b < nbatch; b += (long long)gridDim.x * XSLOTS) {
-    const long long row0 = b * rb;
-    const long long pl = row0 / ny;
-    const int y0 = (int)(row0 - pl * ny);
+    const long long pa = b / bpp;                        // index among the active planes
+    const int y0 = (int)(b - pa * bpp) * rb;
+    const long long pl = (pa / act) * A.nz + lm + pa % act;
+    const long long row0 = pl * ny + y0;
     const double2* in = A.cplx + (size_t)pl * nkx * ny + y0;
     // Z'[k] = (X[k] + conj X[M-k]) + i conj(W^k) (X[k] - conj X[M-k]) at its digit-reversed position (unnormalised C2R).
     // All of a thread's gathered values are loaded before any is used: one round of global latency per batch.

@@ -609,7 +609,7 @@ __global__ void __launch_bounds__(SOLVE_THREADS, SolveSmem<NZ>::CTAS) k_solve(So
         om[1] = 0.5 * (du - K.sgI * K.kxt * wo);                          // (1/2)(dz u - i k_x w)
         om[2] = 0.5 * K.sgI * (K.kxt * vo - K.kyt * uo);                  // (1/2)(i k_x v - i k_y u)
       }
-      if (valid && !zero_mode) {
+      if (valid && !zero_mode && l >= lm) {                // planes above every footprint are never interpolated from: not stored
         const size_t og = 2 * (l * plane + off0) + part;
         gout[2 * (0 * A.cplx_field) + og] = u * scl;
         gout[2 * (1 * A.cplx_field) + og] = v * scl;

@@ -201,7 +201,7 @@ __device__ __forceinline__ void chains(const SolveArgs& A, const PairTab<NZ>& T,
 // buffer, plus the correction evaluated at the node, to global memory
 template <int NZ, int PAR, bool SLIT>
 __device__ __forceinline__ void store_nodes(const PairTab<NZ>& T, const double* NB, const double* EXP, const double (&cf)[3][4], double* gout,
-                                            size_t cplx_field, size_t plane, double s, int lane, bool store_ok) {
+                                            size_t cplx_field, size_t plane, double s, int lane, bool store_ok, int lm) {
   typedef PG<NZ> G;
   constexpr int N = G::N, NE = G::NE, NO = G::NO, NH = PAR ? NO : NE, VS = NZ * LN;
   const int mode = lane >> 1;
@@ -221,7 +221,7 @@ __device__ __forceinline__ void store_nodes(const PairTab<NZ>& T, const double* 
       double v = PAR ? ve - vo : ve + vo;
       v = fma(fma(cf[c][0], z, cf[c][1]), e1, v);
       if (SLIT) v = fma(fma(cf[c][2], z, cf[c][3]), e2, v);
-      if (store_ok) go[2 * (size_t)c * cplx_field] = v;
+      if (store_ok && node >= lm) go[2 * (size_t)c * cplx_field] = v;       // planes above every footprint are never interpolated from
     }
   }
 }
@@ -449,8 +449,9 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
   // ---- 7. back to the nodes g_l = E_l + O_l (even warp, l < NE), g_{N-l} = E_l - O_l (odd warp, l < NO); correction at the node
   // (basis z e^{-kz}, e^{-kz}, z e^{-k(H-z)}, e^{-k(H-z)}); store.  A rolled loop per geometry.
   double* gout = reinterpret_cast<double*>(A.cplx) + 2 * off0 + part;
-  if (A.wall_mode == DP_SLIT) store_nodes<NZ, PAR, true>(T, NB, EXP, cf, gout, A.cplx_field, plane, s, lane, store_ok);
-  else store_nodes<NZ, PAR, false>(T, NB, EXP, cf, gout, A.cplx_field, plane, s, lane, store_ok);
+  const int lm = __ldg(A.lmin);
+  if (A.wall_mode == DP_SLIT) store_nodes<NZ, PAR, true>(T, NB, EXP, cf, gout, A.cplx_field, plane, s, lane, store_ok, lm);
+  else store_nodes<NZ, PAR, false>(T, NB, EXP, cf, gout, A.cplx_field, plane, s, lane, store_ok, lm);
 }
 
 template <int NZ>
