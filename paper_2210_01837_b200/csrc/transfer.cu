@@ -181,37 +181,43 @@ struct WeightArgs {
   const double* pos_s;
   const int4* meta;
   const double* znodes;
-  double beta[3], Z[3];      // record 2 uses the dipole envelope's beta and Z
+  double beta[3], inv_Z[3];  // record 2 uses the dipole envelope's beta and Z
+  double inv_alpha;
   double ucut;               // truncation point of phi' (record 2)
   double* wrec;              // [nrec][cap][16 + nz]
   size_t cap;
 };
 
-__global__ void k_weights(int n, WeightArgs A) {
+// One warp per (particle, record).  Only about 22 of the 16 + nz entries of a record are not zero (w + w in x, y and the planes
+// lmin..lmax in z), and every evaluation of the kernel costs an exp and a square root: the warp first stores zeros over the whole
+// record, then lanes 0-7 take the x entries, 8-15 the y entries and lanes 16-31 the planes lmin, lmin + 1, ... sixteen at a time, so a
+// warp evaluates the kernel once (plus once per image term of eq 9 that reaches some plane) instead of once per 32 record entries.
+constexpr int WEIGHT_WARPS = 8;
+__global__ void __launch_bounds__(WEIGHT_WARPS * 32) k_weights(int n, WeightArgs A) {
   const GridGeom& g = A.g;
   const int wrec = 2 * DP_MAX_W + g.nz;
-  const size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
-  if (i >= (size_t)n * wrec) return;
-  const int p = (int)(i / wrec), rr = (int)(i % wrec), k = blockIdx.y;
-  const double beta = A.beta[k], inv_Z = 1.0 / A.Z[k], inv_alpha = 1.0 / g.alpha;
+  const int lane = threadIdx.x & 31, p = blockIdx.x * WEIGHT_WARPS + (threadIdx.x >> 5), k = blockIdx.y;
+  if (p >= n) return;
+  const double beta = A.beta[k], inv_Z = A.inv_Z[k], inv_alpha = A.inv_alpha;
   const int4 m = A.meta[p];
-  double v = 0.0;
-  if (m.z <= m.w) {
-    if (rr < 2 * DP_MAX_W) {
-      const int a = rr & (DP_MAX_W - 1);
-      const double xw = A.pos_s[3 * (size_t)p + (rr >= DP_MAX_W ? 1 : 0)];
-      const double i0 = ceil((xw - g.alpha) / g.h);            // unwrapped origin: distances use the unwrapped node
-      if (a < g.w) v = k < 2 ? es_phi((i0 + a) * g.h - xw, inv_alpha, beta, inv_Z) : es_dphi((i0 + a) * g.h - xw, inv_alpha, beta, inv_Z, A.ucut);
-    } else {
-      const int l = rr - 2 * DP_MAX_W;
-      if (l >= m.z && l <= m.w) {
-        const double zp = A.pos_s[3 * (size_t)p + 2];
-        v = k < 2 ? zeta_weight(A.znodes[l], zp, g.H, g.wall_mode, inv_alpha, beta, inv_Z)
-                  : dzeta_weight(A.znodes[l], zp, g.H, g.wall_mode, inv_alpha, beta, inv_Z, A.ucut);
-      }
+  double* rec = A.wrec + ((size_t)k * A.cap + p) * wrec;
+  for (int e = lane; e < wrec; e += 32) rec[e] = 0.0;
+  if (m.z > m.w) return;                                         // skipped particle: an all-zero record
+  __syncwarp();
+  const double zp = A.pos_s[3 * (size_t)p + 2];
+  if (lane < 2 * DP_MAX_W) {
+    const int a = lane & (DP_MAX_W - 1);
+    if (a < g.w) {
+      const double xw = A.pos_s[3 * (size_t)p + (lane >= DP_MAX_W ? 1 : 0)];
+      const double i0 = ceil((xw - g.alpha) / g.h);              // unwrapped origin: distances use the unwrapped node (same expression as origin_cell)
+      rec[lane] = k < 2 ? es_phi((i0 + a) * g.h - xw, inv_alpha, beta, inv_Z) : es_dphi((i0 + a) * g.h - xw, inv_alpha, beta, inv_Z, A.ucut);
+    }
+  } else {
+    for (int l = m.z + (lane - 2 * DP_MAX_W); l <= m.w; l += 32 - 2 * DP_MAX_W) {
+      rec[2 * DP_MAX_W + l] = k < 2 ? zeta_weight(A.znodes[l], zp, g.H, g.wall_mode, inv_alpha, beta, inv_Z)
+                                    : dzeta_weight(A.znodes[l], zp, g.H, g.wall_mode, inv_alpha, beta, inv_Z, A.ucut);
     }
   }
-  A.wrec[((size_t)k * A.cap + p) * wrec + rr] = v;
 }
 
 // ---------------------------------------------------------------------------------------------- spread
@@ -561,13 +567,11 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
     W.g = make_geom(P);
     W.pos_s = P->d_pos_s; W.meta = P->d_meta; W.znodes = P->d_znodes;
     W.beta[0] = P->p.beta_M; W.beta[1] = P->p.beta_D; W.beta[2] = P->p.beta_D;
-    W.Z[0] = P->ZM; W.Z[1] = P->ZD; W.Z[2] = P->ZD;
+    W.inv_Z[0] = 1.0 / P->ZM; W.inv_Z[1] = 1.0 / P->ZD; W.inv_Z[2] = 1.0 / P->ZD; W.inv_alpha = 1.0 / P->alpha;
     W.ucut = P->ucutD;
     W.wrec = P->d_wrec; W.cap = (size_t)P->p.max_particles;
-    const int wrec = 2 * DP_MAX_W + P->p.nz;
-    const size_t items = (size_t)n * wrec;
-    dim3 wg((unsigned)((items + 255) / 256), P->nrec);
-    k_weights<<<wg, 256, 0, st>>>(n, W);
+    dim3 wg((unsigned)((n + WEIGHT_WARPS - 1) / WEIGHT_WARPS), P->nrec);
+    if (n > 0) k_weights<<<wg, WEIGHT_WARPS * 32, 0, st>>>(n, W);
   }
   SpreadArgs A;
   A.g = make_geom(P);
