@@ -45,7 +45,7 @@ template <int NZ> struct alignas(16) PairTab {
   double S[2][PG<NZ>::NE][NEP];
   double P[NZ], Q[NZ], XI[NZ];
 };
-struct PairConst { double s, inv_s, sc, inv_2eta; };      // H/2, 2/H, (H/2)^2 / eta, 1/(2 eta): computed once on the host
+struct PairConst { double s, inv_s, sc, inv_2eta, dkx, dky; };   // H/2, 2/H, (H/2)^2 / eta, 1/(2 eta), 2 pi / Lx, 2 pi / Ly: computed once on the host
 template <int NZ> struct PairArgs {
   SolveArgs a;
   PairConst c;
@@ -475,7 +475,7 @@ __global__ void __launch_bounds__(PairSmem<NZ>::THREADS, PairSmem<NZ>::CTAS) k_s
   K.k = 1.0; K.kxt = 0.0; K.kyt = 0.0; K.sgI = part ? 1.0 : -1.0;
   if (valid && !zero_mode) {
     const int nyq = (iy <= A.ny / 2) ? iy : iy - A.ny;
-    const double kx = 2.0 * M_PI * ix / A.Lx, ky = 2.0 * M_PI * nyq / A.Ly;
+    const double kx = PA.c.dkx * ix, ky = PA.c.dky * nyq;
     K.k = sqrt(kx * kx + ky * ky);                         // magnitude: always the full values (reading G5)
     K.kxt = (ix == A.nx / 2) ? 0.0 : kx;                   // component multipliers vanish on the unpaired Nyquist index
     K.kyt = (iy == A.ny / 2) ? 0.0 : ky;
@@ -491,12 +491,21 @@ __global__ void __launch_bounds__(PairSmem<NZ>::THREADS, PairSmem<NZ>::CTAS) k_s
     const int mfast = fast0 + m;
     const bool mvalid = mfast < A.n_fast;
     const size_t moff = (size_t)islow * A.pitch + mfast;
+    // half warp (wid, sub) takes the nodes l = 2 wid + sub, + 4, ... of every field: pointers advance by constant strides
+    const int l0 = 2 * wid + sub;
+    const double2* src = A.cplx + (size_t)l0 * plane + moff;
+    double* dst = &smem[S::NB + l0 * LN + 2 * m];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const double2* sp = src;
+      double* dp = dst;
 #pragma unroll 4
-    for (int r = 2 * wid + sub; r < 3 * NZ; r += 4) {
-      const int c = r / NZ, l = r - c * NZ;
-      double* dst = &smem[S::NB + c * VS + l * LN + 2 * m];
-      if (mvalid && l >= lm) cp_async16(dst, A.cplx + c * A.cplx_field + (size_t)l * plane + moff);
-      else *reinterpret_cast<double2*>(dst) = make_double2(0.0, 0.0);
+      for (int l = l0; l < NZ; l += 4) {
+        if (mvalid && l >= lm) cp_async16(dp, sp);
+        else *reinterpret_cast<double2*>(dp) = make_double2(0.0, 0.0);
+        sp += 4 * plane; dp += 4 * LN;
+      }
+      src += A.cplx_field; dst += VS;
     }
     cp_async_commit();
   }
@@ -585,7 +594,7 @@ void dp_solve_pair_destroy(dp_plan* P) {
 
 cudaError_t dp_launch_solve_pair(dp_plan* P, const SolveArgs& A, cudaStream_t st) {
   cudaError_t e = cudaErrorInvalidValue;
-#define X(NZ) if (P->p.nz == NZ) { PairArgs<NZ> PA; PA.a = A; PA.c.s = 0.5 * A.H; PA.c.inv_s = 2.0 / A.H; PA.c.sc = 0.25 * A.H * A.H / A.eta; PA.c.inv_2eta = 0.5 / A.eta; PA.t = *static_cast<const PairTab<NZ>*>(P->solve_pair_tab); \
+#define X(NZ) if (P->p.nz == NZ) { PairArgs<NZ> PA; PA.a = A; PA.c.s = 0.5 * A.H; PA.c.inv_s = 2.0 / A.H; PA.c.sc = 0.25 * A.H * A.H / A.eta; PA.c.inv_2eta = 0.5 / A.eta; PA.c.dkx = 2.0 * M_PI / A.Lx; PA.c.dky = 2.0 * M_PI / A.Ly; PA.t = *static_cast<const PairTab<NZ>*>(P->solve_pair_tab); \
     constexpr int CM = TM * PairSmem<NZ>::NPAIR; dim3 grid((A.n_fast + CM - 1) / CM, A.n_slow); \
     k_solve_pair<NZ><<<grid, PairSmem<NZ>::THREADS, pair_smem_bytes<NZ>(), st>>>(PA); e = cudaGetLastError(); }
   DP_PAIR_NZ_LIST(X)

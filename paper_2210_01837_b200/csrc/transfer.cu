@@ -109,17 +109,20 @@ __global__ void k_bin_count(int n, const double* __restrict__ pos, GridGeom g, i
   slot_of[p] = atomicAdd(&bin_count[b], 1);
 }
 
-// exclusive scan of bin_count -> bin_start[0..nbins]; one CTA, chunked
+// exclusive scan of bin_count -> bin_start[0..nbins]; one CTA, chunks of blockDim * 8 elements (eight consecutive bins per thread)
 __global__ void k_scan(int nbins, const int* __restrict__ cnt, int* __restrict__ start) {
+  constexpr int E = 8;
   __shared__ int warp_sums[32];
   __shared__ int carry;
   if (threadIdx.x == 0) carry = 0;
   __syncthreads();
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  for (int base = 0; base < nbins; base += blockDim.x) {
-    int i = base + threadIdx.x;
-    int v = i < nbins ? cnt[i] : 0;
-    int s = v;
+  for (int base = 0; base < nbins; base += blockDim.x * E) {
+    const int i0 = base + threadIdx.x * E;
+    int v[E], tot = 0;
+#pragma unroll
+    for (int e = 0; e < E; ++e) { v[e] = (i0 + e < nbins) ? cnt[i0 + e] : 0; tot += v[e]; }
+    int s = tot;
     for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += t; }
     if (lane == 31) warp_sums[wid] = s;
     __syncthreads();
@@ -129,10 +132,11 @@ __global__ void k_scan(int nbins, const int* __restrict__ cnt, int* __restrict__
       warp_sums[lane] = ws;
     }
     __syncthreads();
-    int excl = carry + (wid > 0 ? warp_sums[wid - 1] : 0) + s - v;
-    if (i < nbins) start[i] = excl;
+    int run = carry + (wid > 0 ? warp_sums[wid - 1] : 0) + s - tot;        // exclusive prefix of this thread's first bin
+#pragma unroll
+    for (int e = 0; e < E; ++e) { if (i0 + e < nbins) start[i0 + e] = run; run += v[e]; }
     __syncthreads();
-    if (threadIdx.x == blockDim.x - 1) carry = excl + v;
+    if (threadIdx.x == blockDim.x - 1) carry = run;
     __syncthreads();
   }
   if (threadIdx.x == 0) start[nbins] = carry;
