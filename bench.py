@@ -466,6 +466,19 @@ def main():
                         "warp and 16 modes against 64 FMA lanes per clock and SM; profiles/r2_*): the fraction is of the HBM roofline, as the contract asks",
                 "kernels": ktab}
     roofline.update(agg)
+    # the solve kernel against the fp64 pipe (it is bound by plain fp64 arithmetic, not by HBM): algorithmic FMAs per mode of
+    # a product with F fields each way = the folded Chebyshev transforms, 2 (directions) x 2F (real columns) x (NE^2 + NO^2), plus the
+    # 2(F + 1) real boundary-value problems of nz - 2 rows at 9 FMAs per row (elimination, back substitution with the two boundary
+    # functionals, border update, two integrations); peak = 148 SMs x 64 FMA lanes per clock x 1.965 GHz
+    ne, no, fin = (prob.nz + 1) // 2, prob.nz // 2, main_run["fields"]
+    fma_mode = 2 * 2 * fin * (ne * ne + no * no) + 2 * (fin + 1) * (prob.nz - 2) * 9
+    modes = (prob.nx // 2 + 1) * prob.ny - 1
+    t_solve = stages["solve"]["ms"] * 1e-3
+    if t_solve > 0:
+        ach = 2.0 * fma_mode * modes / t_solve / 1e12
+        roofline["solve_fp64"] = {"bound": "alu", "kernel": main_run["solve_kernel"], "achieved": ach, "peak": 2 * 148 * 64 * 1.965e9 / 1e12, "unit": "TFLOP/s",
+                                  "frac": ach / (2 * 148 * 64 * 1.965e9 / 1e12), "algorithmic_fma_per_mode": fma_mode, "modes": modes,
+                                  "peak_source": "148 SMs x 64 fp64 FMA lanes per clock x 1.965 GHz (B200_PROFILING.md unit counts; a DFMA-only probe reaches 0.92 of it)"}
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
