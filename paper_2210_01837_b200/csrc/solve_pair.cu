@@ -205,8 +205,11 @@ __device__ __forceinline__ void store_nodes(const PairTab<NZ>& T, const double* 
   typedef PG<NZ> G;
   constexpr int N = G::N, NE = G::NE, NO = G::NO, NH = PAR ? NO : NE, VS = NZ * LN;
   const int mode = lane >> 1;
+  // own nodes that are stored: l >= lm for the even warp, N - l >= lm for the odd one
+  const int lmc = lm < 0 ? 0 : lm;
+  const int lbeg = PAR ? 0 : (lmc < NH ? lmc : NH), lend = PAR ? ((N - lmc + 1) < NH ? (N - lmc + 1 > 0 ? N - lmc + 1 : 0) : NH) : NH;
 #pragma unroll 2
-  for (int l = 0; l < NH; ++l) {
+  for (int l = lbeg; l < lend; ++l) {
     const int node = PAR ? N - l : l;
     const bool mid = (!PAR && l >= NO);                  // the middle node of an odd nz: no O row, and it mirrors itself
     const double z = s * (1.0 + T.XI[node]);
@@ -422,14 +425,16 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
   // e^{-k z} at this warp's own nodes, z_l (even warp) or z_{N-l} = H - z_l (odd warp): the two parts of a mode share the work and
   // leave the values in shared memory (the chain factors are dead); the slit also needs those of the mirrored nodes = the partner's
   double* EXP = smem + S::FAC;
+  const int lm = __ldg(A.lmin);                  // nodes l < lm are not stored (no footprint reaches them)
   {
     constexpr int HALF = (NH + 1) / 2;
 #pragma unroll
-    for (int i = 0; i < HALF; ++i) {
+    for (int i = 0; i < HALF; ++i) {             // unrolled: the exponentials are independent dependency chains
       const int l = 2 * i + part;
       if (l < NH) {
-        const double z = s * (PAR ? 1.0 - T.XI[2 * i] : 1.0 + T.XI[2 * i]), z1 = s * (PAR ? 1.0 - T.XI[2 * i + 1 < NH ? 2 * i + 1 : 0] : 1.0 + T.XI[2 * i + 1 < NH ? 2 * i + 1 : 0]);
-        EXP[(PAR * NE + l) * TM + mode] = dp_exp_neg(-K.k * (part ? z1 : z));
+        const double xi = part ? T.XI[2 * i + 1 < NH ? 2 * i + 1 : 0] : T.XI[2 * i];
+        const double z = s * (PAR ? 1.0 - xi : 1.0 + xi);
+        EXP[(PAR * NE + l) * TM + mode] = dp_exp_neg(-K.k * z);
       }
     }
   }
@@ -449,7 +454,6 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
   // ---- 7. back to the nodes g_l = E_l + O_l (even warp, l < NE), g_{N-l} = E_l - O_l (odd warp, l < NO); correction at the node
   // (basis z e^{-kz}, e^{-kz}, z e^{-k(H-z)}, e^{-k(H-z)}); store.  A rolled loop per geometry.
   double* gout = reinterpret_cast<double*>(A.cplx) + 2 * off0 + part;
-  const int lm = __ldg(A.lmin);
   if (A.wall_mode == DP_SLIT) store_nodes<NZ, PAR, true>(T, NB, EXP, cf, gout, A.cplx_field, plane, s, lane, store_ok, lm);
   else store_nodes<NZ, PAR, false>(T, NB, EXP, cf, gout, A.cplx_field, plane, s, lane, store_ok, lm);
 }
