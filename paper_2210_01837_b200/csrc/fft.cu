@@ -130,9 +130,11 @@ struct MidNone { __device__ __forceinline__ void operator()(int, int) const {} }
 // The kernels are templates on the factorisation <R0, R1, R2> of the hot sizes (no runtime dispatch, every index into the
 // argument arrays static, only three butterflies in the instruction stream); <0, 0, 0> is the general version that
 // reads the radices from its arguments.
-template <int TPS, int R0, bool INV, class Mid, class TS, class TD>
+// (NN = R0 R1 R2, the transform length, is a compile-time constant there too: the index arithmetic of every line — id / (n / R) — then
+// compiles to a multiplication instead of an integer division)
+template <int TPS, int R0, int NN, bool INV, class Mid, class TS, class TD>
 __device__ __forceinline__ void run_edge(int r0, const TS* src, TD* dst, const double2* tw1, int n, int rows, int tid, const Mid& mid) {
-  if constexpr (R0 > 0) edge_lines<R0, INV>(src, dst, tw1, n, rows, (size_t)n, (size_t)n, tid, TPS, mid);
+  if constexpr (R0 > 0) edge_lines<R0, INV>(src, dst, tw1, NN, rows, (size_t)NN, (size_t)NN, tid, TPS, mid);
   else edge_dispatch<INV>(r0, src, dst, tw1, n, rows, (size_t)n, (size_t)n, tid, TPS, mid);
 }
 // the shared-memory stages after (forward) or before (inverse) the edge stage, with the slot's barrier between stages;
@@ -140,16 +142,16 @@ __device__ __forceinline__ void run_edge(int r0, const TS* src, TD* dst, const d
 template <int TPS, int R0, int R1, int R2, bool INV, bool LAST_BARRIER, class FA>
 __device__ __forceinline__ void run_inner(const FA& A, double2* buf, const double2* tw, int n, int rows, int tid, int slot) {
   if constexpr (R0 > 0) {
-    constexpr int S1 = R2;                       // stride of stage 1 (n = R0 R1 R2)
+    constexpr int S1 = R2, NN = R0 * R1 * R2;    // stride of stage 1; n = R0 R1 R2 as a compile-time constant
     if (!INV) {
-      stage_lines<R1, false>(buf, tw + A.off[1], n, S1, rows, n, tid, TPS);
+      stage_lines<R1, false>(buf, tw + A.off[1], NN, S1, rows, NN, tid, TPS);
       slot_barrier<TPS>(slot);
-      stage_lines<R2, false>(buf, tw + A.off[2], n, 1, rows, n, tid, TPS);
+      stage_lines<R2, false>(buf, tw + A.off[2], NN, 1, rows, NN, tid, TPS);
       if (LAST_BARRIER) slot_barrier<TPS>(slot);
     } else {
-      stage_lines<R2, true>(buf, tw + A.off[2], n, 1, rows, n, tid, TPS);
+      stage_lines<R2, true>(buf, tw + A.off[2], NN, 1, rows, NN, tid, TPS);
       slot_barrier<TPS>(slot);
-      stage_lines<R1, true>(buf, tw + A.off[1], n, S1, rows, n, tid, TPS);
+      stage_lines<R1, true>(buf, tw + A.off[1], NN, S1, rows, NN, tid, TPS);
       if (LAST_BARRIER) slot_barrier<TPS>(slot);
     }
   } else if (!INV) {
@@ -197,7 +199,7 @@ __global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_fwd(FftYArgs A) {
     if (st == 0) bulk_wait_read();
     slot_barrier<YTPS>(slot);
     const MidNone mid;
-    run_edge<YTPS, R0, false>(A.F.r[0], g, buf, tw + A.off[0], n, nr, st, mid);
+    run_edge<YTPS, R0, R0 * R1 * R2, false>(A.F.r[0], g, buf, tw + A.off[0], n, nr, st, mid);
     slot_barrier<YTPS>(slot);
     run_inner<YTPS, R0, R1, R2, false, false>(A, buf, tw, n, nr, st, slot);
     fence_async_proxy();
@@ -253,7 +255,7 @@ __global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_inv(FftYArgs A) {
     if (more) batch(b + stride, nrow0, nnr);
     // the refill of the buffer is issued after the last stage (issuing it between that stage's loads and its arithmetic costs the
     // stage 200 bytes of spills per thread; the other slots of the CTA cover the load's latency)
-    run_edge<YTPS, R0, true>(A.F.r[0], buf, g, tw + A.off[0], n, nr, st, MidNone());
+    run_edge<YTPS, R0, R0 * R1 * R2, true>(A.F.r[0], buf, g, tw + A.off[0], n, nr, st, MidNone());
     fence_async_proxy();
     slot_barrier<YTPS>(slot);
     if (st == 0 && more) { mbar_expect_tx(mbar, (unsigned)nnr * n * 16u); bulk_load(buf, A.data + nrow0 * n, (unsigned)nnr * n * 16u, mbar); }
@@ -286,21 +288,26 @@ __global__ void __launch_bounds__(XTHREADS, 1) k_fft_x_fwd(FftXArgs A) {
     const long long pl = (pa / act) * A.nz + lm + pa % act;
     const long long row0 = pl * ny + y0;                 // flat row index over (plane, y)
     // a real row of nx doubles is read as M complex numbers z[m] = x[2m] + i x[2m+1]
-    if constexpr (F32) run_edge<XTPS, R0, false>(A.F.r[0], reinterpret_cast<const float2*>(reinterpret_cast<const float*>(A.real) + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
-    else run_edge<XTPS, R0, false>(A.F.r[0], reinterpret_cast<const double2*>(A.real + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
+    if constexpr (F32) run_edge<XTPS, R0, R0 * R1 * R2, false>(A.F.r[0], reinterpret_cast<const float2*>(reinterpret_cast<const float*>(A.real) + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
+    else run_edge<XTPS, R0, R0 * R1 * R2, false>(A.F.r[0], reinterpret_cast<const double2*>(A.real + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
     slot_barrier<XTPS>(slot);
     run_inner<XTPS, R0, R1, R2, false, true>(A, buf, tw, M, rb, st, slot);
     // split into the spectra of the real rows and write them transposed: T[pl][kx][y0 + r]
     double2* out = A.cplx + (size_t)pl * nkx * ny + y0;
-    for (int idx = st; idx < npost * rb; idx += XTPS) {
-      const int k = idx / rb, r = idx - k * rb;
-      const int km = (k == 0) ? 0 : M - k;
-      const double2 z1 = buf[r * M + pos[k]], z2 = buf[r * M + pos[km]];
+    auto split = [&](int k, int r, int Mc) {
+      const int km = (k == 0) ? 0 : Mc - k;
+      const double2 z1 = buf[r * Mc + pos[k]], z2 = buf[r * Mc + pos[km]];
       const double2 E = make_double2(0.5 * (z1.x + z2.x), 0.5 * (z1.y - z2.y));
       const double2 O = make_double2(0.5 * (z1.y + z2.y), -0.5 * (z1.x - z2.x));
       const double2 B = cmul(O, post[k]);
       out[(size_t)k * ny + r] = cadd(E, B);
-      if (2 * k != M) out[(size_t)(M - k) * ny + r] = make_double2(E.x - B.x, -(E.y - B.y));
+      if (2 * k != Mc) out[(size_t)(Mc - k) * ny + r] = make_double2(E.x - B.x, -(E.y - B.y));
+    };
+    if constexpr (R0 > 0) {                     // static kernels: M and the rows per batch are compile-time constants (no integer division)
+      constexpr int Ms = R0 * R1 * R2, RB = SLOT_ELEMS / Ms > 0 ? SLOT_ELEMS / Ms : 1;
+      for (int idx = st; idx < (Ms / 2 + 1) * RB; idx += XTPS) split(idx / RB, idx % RB, Ms);
+    } else {
+      for (int idx = st; idx < npost * rb; idx += XTPS) { const int k = idx / rb; split(k, idx - k * rb, M); }
     }
     slot_barrier<XTPS>(slot);                                  // every read of buf is done before the next batch overwrites it
   }
@@ -367,8 +374,8 @@ __global__ void __launch_bounds__(XTHREADS, 1) k_fft_x_inv(FftXArgs A) {
     slot_barrier<XTPS>(slot);
     run_inner<XTPS, R0, R1, R2, true, true>(A, buf, tw, M, rb, st, slot);
     // last stage: results go straight to the real grid rows (z[m] = x[2m] + i x[2m+1])
-    if constexpr (F32) run_edge<XTPS, R0, true>(A.F.r[0], (const double2*)buf, reinterpret_cast<float2*>(reinterpret_cast<float*>(A.real) + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
-    else run_edge<XTPS, R0, true>(A.F.r[0], (const double2*)buf, reinterpret_cast<double2*>(A.real + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
+    if constexpr (F32) run_edge<XTPS, R0, R0 * R1 * R2, true>(A.F.r[0], (const double2*)buf, reinterpret_cast<float2*>(reinterpret_cast<float*>(A.real) + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
+    else run_edge<XTPS, R0, R0 * R1 * R2, true>(A.F.r[0], (const double2*)buf, reinterpret_cast<double2*>(A.real + row0 * A.nx), tw + A.off[0], M, rb, st, nomid);
     slot_barrier<XTPS>(slot);                                  // the stage has read buf before the next batch refills it
   }
 }
