@@ -75,6 +75,21 @@ __device__ __forceinline__ double dp_exp_neg(double x) {      // e^x for x <= 0 
   return p * __hiloint2double((1023 + (int)t) << 20, 0);      // 2^t, t in [-1010, 0]
 }
 
+// the same with the Taylor coefficients 1/13!, ..., 1/2! read from a table `ec` (a kernel-parameter array: one uniform load per coefficient
+// instead of two immediate moves)
+__device__ __forceinline__ double dp_exp_neg_tab(double x, const double (&ec)[12]) {
+  x = fmax(x, -700.0);
+  const double t = rint(x * 1.4426950408889634074);
+  double r = fma(t, -6.93147180369123816490e-01, x);
+  r = fma(t, -1.90821492927058770002e-10, r);
+  double p = ec[0];
+#pragma unroll
+  for (int q = 1; q < 12; ++q) p = fma(p, r, ec[q]);
+  p = fma(p, r, 1.0);
+  p = fma(p, r, 1.0);
+  return p * __hiloint2double((1023 + (int)t) << 20, 0);
+}
+
 // ---- tridiagonal rows of a chain (n >= 1): d_n a_n + l_n a_{n-2} + u_n a_{n+2}; all divisions are compile-time constants
 template <int NZ> __device__ __forceinline__ double row_d(int n, double k2) { return n == 1 ? fma(k2, 0.125, 1.0) : fma(k2, 1.0 / (2.0 * (n * n - 1)), 1.0); }
 template <int NZ> __device__ __forceinline__ double row_l(int n, double k2) { return k2 * (-(n == 2 ? 2.0 : 1.0) / (4.0 * n * (n - 1))); }

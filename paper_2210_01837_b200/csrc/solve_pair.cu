@@ -44,6 +44,10 @@ template <int NZ> struct alignas(16) PairTab {
   double A[2][PG<NZ>::NE][NEP];
   double S[2][PG<NZ>::NE][NEP];
   double P[NZ], Q[NZ], XI[NZ];
+  // per-row constants of the chains (n = row index): rows d_n = 1 + kappa^2 RD[n], l_n = kappa^2 RL[n], u_n = kappa^2 RU[n] (0 beyond the last
+  // row), and 1/(2n) for the integrations — one LDCU each instead of a pair of immediate moves
+  double RD[NZ], RL[NZ], RU[NZ], IH[NZ + 1];
+  double EC[12];                                        // 1/13! ... 1/2!: Taylor coefficients of dp_exp_neg's polynomial
 };
 struct PairConst { double s, inv_s, sc, inv_2eta, dkx, dky; };   // H/2, 2/H, (H/2)^2 / eta, 1/(2 eta), 2 pi / Lx, 2 pi / Ly: computed once on the host
 template <int NZ> struct PairArgs {
@@ -57,7 +61,8 @@ template <int NZ> struct PairSmem {
   static constexpr int NB = 0;                            // [3][NZ][32] nodal columns; later the hand-over rows (see the kernel)
   static constexpr int FAC = NB + 3 * NZ * ROW;           // [2][NZ][TM] inverse pivots, border solution (by row n); later e^{-k z}
   static constexpr int IBG = FAC + 2 * NZ * TM;           // [2][TM] 1 / B_g of the even / odd chain
-  static constexpr int SUM = IBG + 2 * TM;                // [2][8][32] sums handed over: S_c of p, u, v, w and S_b of u, v per parity
+  static constexpr int GPQ = IBG + 2 * TM;                // [2][2][TM] sums of b_m and of c_n of the unit border solution (even / odd chain)
+  static constexpr int SUM = GPQ + 4 * TM;                // [2][8][32] sums handed over: S_c of p, u, v, w and S_b of u, v per parity
   static constexpr int DOUBLES = SUM + 2 * 8 * ROW;
   // pairs per CTA and CTAs per SM.  Every warp runs ~9 k straight-line instructions per 16 modes, far more than the instruction
   // caches hold, and an SM fetches only ~20 bytes of code per clock from L2: the warps of one parity must therefore run the SAME
@@ -83,7 +88,7 @@ __device__ __forceinline__ void sched_fence() { __syncwarp(); }
 // ---- factorisation of the chain of parity PAR for this lane's mode (depends on |k| only): inverse pivots Fi[n], the solution Fa[n]
 // with unit border unknown, and 1/B_g (B_g = boundary functional of that solution).  Rows are indexed by n with stride TM.
 template <int NZ, int PAR>
-__device__ __forceinline__ double factor_chain(const PairTab<NZ>& T, double* __restrict__ Fi, double* __restrict__ Fa, double k, double k2,
+__device__ __forceinline__ double factor_chain(const PairTab<NZ>& T, double* __restrict__ Fi, double* __restrict__ Fa, double* __restrict__ Gpq, double k, double k2,
                                                double inv_s, bool store) {
   constexpr int n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR;
   double invd[NR], ag[NR];
@@ -91,10 +96,10 @@ __device__ __forceinline__ double factor_chain(const PairTab<NZ>& T, double* __r
 #pragma unroll
   for (int j = 0; j < NR; ++j) {
     const int n = n0 + 2 * j;
-    double d = row_d<NZ>(n, k2);
+    double d = fma(k2, T.RD[n], 1.0);
     if (j > 0) {
-      const double mu = row_l<NZ>(n, k2) * invd[j - 1];
-      d = fma(-mu, row_u<NZ>(n - 2, k2), d);
+      const double mu = k2 * T.RL[n] * invd[j - 1];
+      d = fma(-mu, k2 * T.RU[n - 2], d);
       g = -mu * g;
     }
     invd[j] = dp_rcp(d);
@@ -104,19 +109,17 @@ __device__ __forceinline__ double factor_chain(const PairTab<NZ>& T, double* __r
 #pragma unroll
   for (int j = NR - 1; j >= 0; --j) {
     const int n = n0 + 2 * j;
-    const double a = (ag[j] - row_u<NZ>(n, k2) * next) * invd[j];
+    const double a = (ag[j] - k2 * T.RU[n] * next) * invd[j];
     next = a;
     if (store) { Fa[n * TM] = a; Fi[n * TM] = invd[j]; }
     SP = fma(T.P[n], a, SP); SQ = fma(T.Q[n], a, SQ);
   }
-  double Bg;
-  if (!PAR) {                                                // a_0 = rho_0 + kappa^2 c_0 ; c_0 = 1 also enters sum c_n directly
-    SP = fma(T.P[0], k2, SP); SQ = fma(T.Q[0], k2, SQ);
-    Bg = inv_s * SP + k * (1.0 + SQ);
-  } else {                                                   // b_0 = 1 enters sum b_n and c_1
-    Bg = inv_s * (1.0 + SP) + k * (1.0 + SQ);
-  }
-  return dp_rcp(Bg);
+  // sums of the first-integral coefficients b_m and of the coefficients c_n of this unit-border solution: a_0 = kappa^2 c_0 and c_0 = 1
+  // itself (even chain); b_0 = 1, which is also c_1's leading term (odd chain)
+  if (!PAR) { SP = fma(T.P[0], k2, SP); SQ = fma(T.Q[0], k2, SQ); }
+  const double GP = PAR ? 1.0 + SP : SP, GQ = 1.0 + SQ;
+  if (store) { Gpq[0] = GP; Gpq[TM] = GQ; }
+  return dp_rcp(inv_s * GP + k * GQ);
 }
 
 // ---- NC BVPs at once on the chain of parity PAR of this lane (the factors are loaded once): forward elimination, back substitution
@@ -127,7 +130,7 @@ __device__ __forceinline__ double factor_chain(const PairTab<NZ>& T, double* __r
 //        Sb[c] = sum of the b_m this chain produces (wall derivatives for partial slip, footnote 46)
 template <int NZ, int PAR, int NC>
 __device__ __forceinline__ void chains(const SolveArgs& A, const PairTab<NZ>& T, double (&a)[NC][Ch<NZ, PAR>::NR], const double (&rho0)[NC], const double (&beta_bc)[NC],
-                                       const double* Fi, const double* Fa, double k, double k2, double inv_s, double invBg,
+                                       const double* Fi, const double* Fa, const double* Gpq, double k, double k2, double inv_s, double invBg,
                                        double (&cc)[NC][PAR ? PG<NZ>::NO : PG<NZ>::NE], double (&bo)[NC][PAR ? PG<NZ>::NO : PG<NZ>::NE],
                                        double (&border)[NC], double (&Sc)[NC], double (&Sb)[NC]) {
   constexpr int N = NZ - 1, n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR;
@@ -137,7 +140,7 @@ __device__ __forceinline__ void chains(const SolveArgs& A, const PairTab<NZ>& T,
   }
 #pragma unroll
   for (int j = 1; j < NR; ++j) {
-    const double mu = row_l<NZ>(n0 + 2 * j, k2) * Fi[(n0 + 2 * j - 2) * TM];
+    const double mu = k2 * T.RL[n0 + 2 * j] * Fi[(n0 + 2 * j - 2) * TM];
 #pragma unroll
     for (int c = 0; c < NC; ++c) a[c][j] = fma(-mu, a[c][j - 1], a[c][j]);
   }
@@ -148,7 +151,7 @@ __device__ __forceinline__ void chains(const SolveArgs& A, const PairTab<NZ>& T,
 #pragma unroll
   for (int j = NR - 1; j >= 0; --j) {
     const int n = n0 + 2 * j;
-    const double ru = row_u<NZ>(n, k2), fi = Fi[n * TM];
+    const double ru = k2 * T.RU[n], fi = Fi[n * TM];
 #pragma unroll
     for (int c = 0; c < NC; ++c) {
       const double v = fma(-ru, next[c], a[c][j]) * fi;
@@ -156,10 +159,15 @@ __device__ __forceinline__ void chains(const SolveArgs& A, const PairTab<NZ>& T,
       SP[c] = fma(T.P[n], v, SP[c]); SQ[c] = fma(T.Q[n], v, SQ[c]);
     }
   }
+  // border unknown from the boundary row; the sums of the b_m and of the c_n of the solution follow from the same functionals
+  // (S_b = SP + border G_P, S_c = SQ + border G_Q with the unit border solution's sums G_P, G_Q): no summation of the results
+  const double GP = Gpq[0], GQ = Gpq[TM];
 #pragma unroll
   for (int c = 0; c < NC; ++c) {
     if (!PAR) { SP[c] = fma(T.P[0], rho0[c], SP[c]); SQ[c] = fma(T.Q[0], rho0[c], SQ[c]); }
     border[c] = (beta_bc[c] - (inv_s * SP[c] + k * SQ[c])) * invBg;               // c_0 (even chain) or b_0 (odd chain)
+    Sb[c] = fma(border[c], GP, SP[c]);
+    Sc[c] = fma(border[c], GQ, SQ[c]);
   }
   DP_SPLIT(A, 2);
 #pragma unroll
@@ -172,8 +180,8 @@ __device__ __forceinline__ void chains(const SolveArgs& A, const PairTab<NZ>& T,
 #pragma unroll
   for (int c = 0; c < NC; ++c) {
     DP_SPLIT(A, 3 + c);
-    double Sc0 = 0.0, Sc1 = 0.0, bprev, sb = PAR ? border[c] : 0.0;
-    if (!PAR) { cc[c][0] = border[c]; Sc0 = border[c]; bprev = 0.0; }
+    double bprev;
+    if (!PAR) { cc[c][0] = border[c]; bprev = 0.0; }
     else bprev = border[c];
 #pragma unroll
     for (int i = 0; i <= (N - PAR) / 2; ++i) {
@@ -182,21 +190,14 @@ __device__ __forceinline__ void chains(const SolveArgs& A, const PairTab<NZ>& T,
       double an = 0.0, ap = 0.0;
       if (n <= N - 2) an = (!PAR && n == 0) ? fma(border[c], k2, rho0[c]) : a[c][n >= n0 ? (n - n0) / 2 : 0];
       if (n + 2 <= N - 2) ap = a[c][(n + 2 - n0) / 2];
-      const double bn1 = ((n == 0 ? 2.0 : 1.0) * an - ap) * (1.0 / (2.0 * (n + 1)));
-      if (n >= 1) {
-        const double v = ((n == 1 ? 2.0 : 1.0) * bprev - bn1) * (1.0 / (2.0 * n));
-        cc[c][i] = v;
-        if (i & 1) Sc1 += v; else Sc0 += v;
-      }
+      const double bn1 = ((n == 0 ? 2.0 : 1.0) * an - ap) * T.IH[n + 1];
+      if (n >= 1) cc[c][i] = ((n == 1 ? 2.0 : 1.0) * bprev - bn1) * T.IH[n];
       bo[c][i] = (n + 1 <= N - 1) ? bn1 : 0.0;
-      if (n + 1 <= N - 1) sb += bn1;
       bprev = bn1;
     }
-    Sc[c] = Sc0 + Sc1; Sb[c] = sb;
   }
 }
 
-// ---- everything after the loads for the warp that owns the coefficients of parity PAR
 // ---- last step for the warp of parity PAR: its own nodes (l for the even warp, N - l for the odd one) from E_l, O_l in the
 // buffer, plus the correction evaluated at the node, to global memory
 template <int NZ, int PAR, bool SLIT>
@@ -252,6 +253,7 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
   double* NB = smem + S::NB;
   const double* Fi = smem + S::FAC + mode;
   const double* Fa = smem + S::FAC + NZ * TM + mode;
+  const double* Gpq = smem + S::GPQ + PAR * 2 * TM + mode;
   double* SUM = smem + S::SUM;
   const double invBg = smem[S::IBG + PAR * TM + mode];
 
@@ -326,7 +328,7 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
       }
     }
     double bo[1][NH], border[1], Sc[1], Sb[1];
-    chains<NZ, PAR, 1>(A, T, a, rho0, bbc, Fi, Fa, K.k, K.k2, inv_s, invBg, pc, bo, border, Sc, Sb);
+    chains<NZ, PAR, 1>(A, T, a, rho0, bbc, Fi, Fa, Gpq, K.k, K.k2, inv_s, invBg, pc, bo, border, Sc, Sb);
     // (H/2) dp/dz: the even chain yields b_m for odd m = 2i + 1 (reader index i), the odd chain b_0 = border and b_m for even m = 2i + 2
     if (!PAR) {
 #pragma unroll
@@ -377,7 +379,7 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
       bbc[c] = PAR ? 0.5 * (gH + g0) : 0.5 * (gH - g0);
     }
     double bo[3][NH], border[3], Sc[3], Sb[3];
-    chains<NZ, PAR, 3>(A, T, a, rho0, bbc, Fi, Fa, K.k, K.k2, inv_s, invBg, uc, bo, border, Sc, Sb);
+    chains<NZ, PAR, 3>(A, T, a, rho0, bbc, Fi, Fa, Gpq, K.k, K.k2, inv_s, invBg, uc, bo, border, Sc, Sb);
 #pragma unroll
     for (int c = 0; c < 3; ++c) SUM[(PAR * 8 + 1 + c) * LN + lane] = Sc[c];
     if (A.slip) { SUM[(PAR * 8 + 4) * LN + lane] = Sb[0]; SUM[(PAR * 8 + 5) * LN + lane] = Sb[1]; }
@@ -434,7 +436,7 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
       if (l < NH) {
         const double xi = part ? T.XI[2 * i + 1 < NH ? 2 * i + 1 : 0] : T.XI[2 * i];
         const double z = s * (PAR ? 1.0 - xi : 1.0 + xi);
-        EXP[(PAR * NE + l) * TM + mode] = dp_exp_neg(-K.k * z);
+        EXP[(PAR * NE + l) * TM + mode] = dp_exp_neg_tab(-K.k * z, T.EC);
       }
     }
   }
@@ -518,8 +520,9 @@ __global__ void __launch_bounds__(PairSmem<NZ>::THREADS, PairSmem<NZ>::CTAS) k_s
     double* Fi = smem + S::FAC + mode;
     double* Fa = smem + S::FAC + NZ * TM + mode;
     double ib;
-    if (wid == 0) ib = factor_chain<NZ, 0>(PA.t, Fi, Fa, K.k, K.k2, inv_s, part == 0);
-    else ib = factor_chain<NZ, 1>(PA.t, Fi, Fa, K.k, K.k2, inv_s, part == 0);
+    double* Gpq = smem + S::GPQ + wid * 2 * TM + mode;
+    if (wid == 0) ib = factor_chain<NZ, 0>(PA.t, Fi, Fa, Gpq, K.k, K.k2, inv_s, part == 0);
+    else ib = factor_chain<NZ, 1>(PA.t, Fi, Fa, Gpq, K.k, K.k2, inv_s, part == 0);
     if (part == 0) smem[S::IBG + wid * TM + mode] = ib;
     if (wid == 0) { smem[S::SUM + 6 * LN + lane] = K.k; smem[S::SUM + 7 * LN + lane] = K.k2; }
     else { smem[S::SUM + 14 * LN + lane] = K.kxt; smem[S::SUM + 15 * LN + lane] = K.kyt; }
@@ -548,6 +551,13 @@ template <int NZ> void host_pair_tab(PairTab<NZ>& T, double scale) {
       }
   }
   for (int l = 0; l <= N; ++l) T.XI[l] = (double)cosl(PI * l / N);
+  for (int n = 1; n <= N; ++n) {             // the chain rows of solve_common.cuh's row_d / row_l / row_u, without the factor kappa^2
+    T.RD[n] = n == 1 ? 0.125 : 1.0 / (2.0 * (n * n - 1));
+    T.RL[n] = n >= 2 ? -(n == 2 ? 2.0 : 1.0) / (4.0 * n * (n - 1)) : 0.0;
+    T.RU[n] = (n + 2 <= NZ - 3) ? -1.0 / (4.0 * n * (n + 1)) : 0.0;
+  }
+  for (int n = 1; n <= N + 1; ++n) T.IH[n] = 1.0 / (2.0 * n);
+  { double f = 2.0; for (int q = 2; q <= 13; ++q) { T.EC[13 - q] = 1.0 / f; f *= (q + 1); } }   // EC[0] = 1/13!, ..., EC[11] = 1/2!
   // P_n, Q_n: with a = unit vector e_n (n <= N-2), b_m = (cbar_{m-1} a_{m-1} - a_{m+1})/(2m) (1 <= m <= N-1),
   // c_m = (cbar_{m-1} b_{m-1} - b_{m+1})/(2m) (1 <= m <= N), b_0 = 0:  P_n = sum of b_m over m of the other parity,
   // Q_n = sum of c_m over m >= 1 of n's parity.
