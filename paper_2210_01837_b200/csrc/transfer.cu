@@ -229,6 +229,10 @@ __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gmem_s
   const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
 }
+__device__ __forceinline__ void cp_async16(double* smem_dst, const double* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
 __device__ __forceinline__ void cp_async_wait_all_groups() { asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory"); }
 
 struct SpreadArgs {
@@ -264,7 +268,7 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
   constexpr int NREC = MODE ? 3 : 1;
   constexpr int PC = MODE ? PCH / 2 : PCH;                // candidates per chunk
   constexpr int NV = MODE ? 6 : 3;
-  __shared__ double s_w[PC][NREC][WS];
+  __shared__ __align__(16) double s_w[PC][NREC][WS];
   __shared__ double s_val[PC][NV];
   __shared__ int4 s_meta[PC];                 // i0, j0 (wrapped origin node), lmin, lmax
   __shared__ int s_rbeg[MAXR], s_roff[MAXR + 1];   // candidate ranges in the sorted arrays; prefix sums of their lengths
@@ -358,11 +362,22 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
       }
       // the weight records travel as asynchronous 8-byte copies: all of a thread's entries are in flight at once (one round of
       // global latency per chunk instead of one per two entries)
-      for (int i = t; i < nl * NREC * WS; i += SPREAD_THREADS) {
-        const int q = i / (NREC * WS), rem = i - q * (NREC * WS), k = rem / WS, e = rem - k * WS;
-        const int kk = MODE ? k : grp;
-        if (e < WREC) cp_async8(&s_w[q][k][e], A.wrec + ((size_t)kk * A.cap + s_keep[c0 + q]) * WREC + e);
-        else s_w[q][k][e] = 0.0;
+      // (16 bytes per copy where the record length is even, i.e. every record starts on a 16-byte boundary)
+      if constexpr (WREC % 2 == 0) {
+        constexpr int WH = WS / 2;
+        for (int i = t; i < nl * NREC * WH; i += SPREAD_THREADS) {
+          const int q = i / (NREC * WH), rem = i - q * (NREC * WH), k = rem / WH, e = 2 * (rem - k * WH);
+          const int kk = MODE ? k : grp;
+          if (e < WREC) cp_async16(&s_w[q][k][e], A.wrec + ((size_t)kk * A.cap + s_keep[c0 + q]) * WREC + e);
+          else { s_w[q][k][e] = 0.0; s_w[q][k][e + 1] = 0.0; }
+        }
+      } else {
+        for (int i = t; i < nl * NREC * WS; i += SPREAD_THREADS) {
+          const int q = i / (NREC * WS), rem = i - q * (NREC * WS), k = rem / WS, e = rem - k * WS;
+          const int kk = MODE ? k : grp;
+          if (e < WREC) cp_async8(&s_w[q][k][e], A.wrec + ((size_t)kk * A.cap + s_keep[c0 + q]) * WREC + e);
+          else s_w[q][k][e] = 0.0;
+        }
       }
       cp_async_wait_all_groups();
       __syncthreads();
@@ -434,13 +449,16 @@ __global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(S
   // ---- store: every grid value of the planes that can hold force written exactly once
   if (in_grid) {
     const int lm = __ldg(A.lmin);
+    GT* dst = reinterpret_cast<GT*>(A.grid) + (size_t)A.field0[grp] * A.real_field + ((size_t)tz * g.ny + gj) * g.nx + gi;
+    const size_t step = (size_t)ZSPLIT * g.ny * g.nx;             // from plane l to plane l + ZSPLIT
 #pragma unroll
     for (int li = 0; li < NL; ++li) {
       const int l = ZSPLIT * li + tz;
-      if (l < lm || l >= NZ) continue;
-      GT* dst = reinterpret_cast<GT*>(A.grid) + (size_t)A.field0[grp] * A.real_field + ((size_t)l * g.ny + gj) * g.nx + gi;
+      if (l >= lm && l < NZ) {
 #pragma unroll
-      for (int c = 0; c < 3; ++c) dst[c * A.real_field] = acc[li][c];
+        for (int c = 0; c < 3; ++c) dst[c * A.real_field] = acc[li][c];
+      }
+      dst += step;
     }
   }
 }
