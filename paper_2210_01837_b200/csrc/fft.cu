@@ -44,7 +44,13 @@ using namespace dpfft;
 #ifndef DP_FFT_YTPS
 #define DP_FFT_YTPS 160
 #endif
+#ifndef DP_FFT_XTPS_FWD
+#define DP_FFT_XTPS_FWD 320
+#endif
+// the forward x pass runs best with 320 threads per slot (its loads are one contiguous row per slot: more lines in flight), the
+// inverse with 256 (its gather keeps 2 x 9 values per thread in registers at 256 threads; measured 4.7 / 5.1 ms and 6.4 / 5.5 ms at cfg 5)
 constexpr int XSLOTS = DP_FFT_XSLOTS, XTPS = DP_FFT_XTPS, XTHREADS = XSLOTS * XTPS;
+constexpr int XFTPS = DP_FFT_XTPS_FWD, XFTHREADS = XSLOTS * XFTPS;
 constexpr int YSLOTS = DP_FFT_YSLOTS, YTPS = DP_FFT_YTPS, YTHREADS = YSLOTS * YTPS;
 constexpr int SLOT_ELEMS = 4320;               // complex elements a slot can hold (69 120 bytes)
 
@@ -264,17 +270,17 @@ __global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_inv(FftYArgs A) {
 
 // ---------------------------------------------------------------------------------------------- pass X forward
 template <int R0, int R1, int R2, bool F32>
-__global__ void __launch_bounds__(XTHREADS, 1) k_fft_x_fwd(FftXArgs A) {
+__global__ void __launch_bounds__(XFTHREADS, 1) k_fft_x_fwd(FftXArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int M = A.M, npost = M / 2 + 1;
   double2* tw = reinterpret_cast<double2*>(smem_raw);
   double2* post = tw + A.ntw;
-  const int slot = threadIdx.x / XTPS, st = threadIdx.x - slot * XTPS;
+  const int slot = threadIdx.x / XFTPS, st = threadIdx.x - slot * XFTPS;
   double2* buf = post + npost + (size_t)slot * A.rb * M;
   unsigned short* pos = reinterpret_cast<unsigned short*>(post + npost + (size_t)XSLOTS * A.rb * M);
-  for (int i = threadIdx.x; i < A.ntw; i += XTHREADS) tw[i] = A.tw[i];
-  for (int i = threadIdx.x; i < M; i += XTHREADS) pos[i] = A.pos[i];
-  for (int i = threadIdx.x; i < npost; i += XTHREADS) post[i] = A.post[i];
+  for (int i = threadIdx.x; i < A.ntw; i += XFTHREADS) tw[i] = A.tw[i];
+  for (int i = threadIdx.x; i < M; i += XFTHREADS) pos[i] = A.pos[i];
+  for (int i = threadIdx.x; i < npost; i += XFTHREADS) post[i] = A.post[i];
   __syncthreads();
   const int rb = A.rb, ny = A.ny, nkx = M + 1;
   int lm = A.lmin ? __ldg(A.lmin) : 0;
@@ -288,10 +294,10 @@ __global__ void __launch_bounds__(XTHREADS, 1) k_fft_x_fwd(FftXArgs A) {
     const long long pl = (pa / act) * A.nz + lm + pa % act;
     const long long row0 = pl * ny + y0;                 // flat row index over (plane, y)
     // a real row of nx doubles is read as M complex numbers z[m] = x[2m] + i x[2m+1]
-    if constexpr (F32) run_edge<XTPS, R0, R0 * R1 * R2, false>(A.F.r[0], reinterpret_cast<const float2*>(reinterpret_cast<const float*>(A.real) + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
-    else run_edge<XTPS, R0, R0 * R1 * R2, false>(A.F.r[0], reinterpret_cast<const double2*>(A.real + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
-    slot_barrier<XTPS>(slot);
-    run_inner<XTPS, R0, R1, R2, false, true>(A, buf, tw, M, rb, st, slot);
+    if constexpr (F32) run_edge<XFTPS, R0, R0 * R1 * R2, false>(A.F.r[0], reinterpret_cast<const float2*>(reinterpret_cast<const float*>(A.real) + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
+    else run_edge<XFTPS, R0, R0 * R1 * R2, false>(A.F.r[0], reinterpret_cast<const double2*>(A.real + row0 * A.nx), buf, tw + A.off[0], M, rb, st, nomid);
+    slot_barrier<XFTPS>(slot);
+    run_inner<XFTPS, R0, R1, R2, false, true>(A, buf, tw, M, rb, st, slot);
     // split into the spectra of the real rows and write them transposed: T[pl][kx][y0 + r]
     double2* out = A.cplx + (size_t)pl * nkx * ny + y0;
     auto split = [&](int k, int r, int Mc) {
@@ -305,11 +311,11 @@ __global__ void __launch_bounds__(XTHREADS, 1) k_fft_x_fwd(FftXArgs A) {
     };
     if constexpr (R0 > 0) {                     // static kernels: M and the rows per batch are compile-time constants (no integer division)
       constexpr int Ms = R0 * R1 * R2, RB = SLOT_ELEMS / Ms > 0 ? SLOT_ELEMS / Ms : 1;
-      for (int idx = st; idx < (Ms / 2 + 1) * RB; idx += XTPS) split(idx / RB, idx % RB, Ms);
+      for (int idx = st; idx < (Ms / 2 + 1) * RB; idx += XFTPS) split(idx / RB, idx % RB, Ms);
     } else {
-      for (int idx = st; idx < npost * rb; idx += XTPS) { const int k = idx / rb; split(k, idx - k * rb, M); }
+      for (int idx = st; idx < npost * rb; idx += XFTPS) { const int k = idx / rb; split(k, idx - k * rb, M); }
     }
-    slot_barrier<XTPS>(slot);                                  // every read of buf is done before the next batch overwrites it
+    slot_barrier<XFTPS>(slot);                                  // every read of buf is done before the next batch overwrites it
   }
 }
 
@@ -543,7 +549,7 @@ static int grid_for(const dp_fft_own* O, long long nbatch, int nslot) {
 cudaError_t dp_fft_own_forward(dp_plan* P, int nfields, cudaStream_t st) {
   dp_fft_own* O = static_cast<dp_fft_own*>(P->fft_own);
   const FftXArgs X = x_args(P, nfields);
-  O->kx_fwd<<<grid_for(O, X.planes * (X.ny / X.rb), XSLOTS), XTHREADS, O->smem_x, st>>>(X);
+  O->kx_fwd<<<grid_for(O, X.planes * (X.ny / X.rb), XSLOTS), XFTHREADS, O->smem_x, st>>>(X);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
   if (P->profiling && P->ev_ok && (e = cudaEventRecord(P->ev_fft[0], st)) != cudaSuccess) return e;
