@@ -51,7 +51,17 @@ using namespace dpfft;
 // inverse with 256 (its gather keeps 2 x 9 values per thread in registers at 256 threads; measured 4.7 / 5.1 ms and 6.4 / 5.5 ms at cfg 5)
 constexpr int XSLOTS = DP_FFT_XSLOTS, XTPS = DP_FFT_XTPS, XTHREADS = XSLOTS * XTPS;
 constexpr int XFTPS = DP_FFT_XTPS_FWD, XFTHREADS = XSLOTS * XFTPS;
+#ifndef DP_FFT_YSLOTS_FWD
+#define DP_FFT_YSLOTS_FWD 2
+#endif
+#ifndef DP_FFT_YTPS_FWD
+#define DP_FFT_YTPS_FWD 288
+#endif
+// the forward y pass (whose first stage loads its lines from global memory into registers) runs best with two slots of 288 threads:
+// every stage of a 4320-point row (270 / 240 / 288 lines) is then ONE round of its slot; measured 3.9 against 4.6 ms at cfg 5, while
+// the inverse (bulk-load prefetch, stores straight to global) loses with that shape (4.2 against 3.4 ms)
 constexpr int YSLOTS = DP_FFT_YSLOTS, YTPS = DP_FFT_YTPS, YTHREADS = YSLOTS * YTPS;
+constexpr int YFSLOTS = DP_FFT_YSLOTS_FWD, YFTPS = DP_FFT_YTPS_FWD, YFTHREADS = YFSLOTS * YFTPS;
 constexpr int SLOT_ELEMS = 4320;               // complex elements a slot can hold (69 120 bytes)
 
 struct dp_fft_own {
@@ -63,7 +73,7 @@ struct dp_fft_own {
   double2* d_tw_y = nullptr;   // stage tables of the length-ny transform
   unsigned short* d_pos_x = nullptr;   // position of Z[k] after the forward x transform
   int* d_ky_of_pos = nullptr;          // FFT-order ky index held at position p of a transformed y row
-  size_t smem_x = 0, smem_y = 0;
+  size_t smem_x = 0, smem_y = 0, smem_y_fwd = 0;
   int grid = 148;
   void (*ky_fwd)(struct FftYArgs) = nullptr;
   void (*ky_inv)(struct FftYArgs) = nullptr;
@@ -182,20 +192,20 @@ __device__ __forceinline__ void run_inner(const FA& A, double2* buf, const doubl
 // result leaves with one bulk store; a slot waits for its previous store to have read the buffer before it starts the next
 // row (the CTA's other slots are busy meanwhile).
 template <int R0, int R1, int R2>
-__global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_fwd(FftYArgs A) {
+__global__ void __launch_bounds__(YFTHREADS, 1) k_fft_y_fwd(FftYArgs A) {
   extern __shared__ __align__(128) unsigned char smem_raw[];
   const int n = A.F.n;
   double2* tw = reinterpret_cast<double2*>(smem_raw);
-  const int slot = threadIdx.x / YTPS, st = threadIdx.x - slot * YTPS;
+  const int slot = threadIdx.x / YFTPS, st = threadIdx.x - slot * YFTPS;
   double2* buf = tw + A.ntw + (size_t)slot * A.rb * n;
-  for (int i = threadIdx.x; i < A.ntw; i += YTHREADS) tw[i] = A.tw[i];
+  for (int i = threadIdx.x; i < A.ntw; i += YFTHREADS) tw[i] = A.tw[i];
   __syncthreads();
   // rows of the planes l >= lm of each field: per field one contiguous range of ra rows, cut into batches of rb
   int lm = A.lmin ? __ldg(A.lmin) : 0;
   lm = lm < 0 ? 0 : (lm > A.nz ? A.nz : lm);
   const long long ra = (long long)(A.nz - lm) * A.nkx, per_field = (ra + A.rb - 1) / A.rb;
   const long long nbatch = per_field * A.fields;
-  for (long long b = (long long)blockIdx.x * YSLOTS + slot; b < nbatch; b += (long long)gridDim.x * YSLOTS) {
+  for (long long b = (long long)blockIdx.x * YFSLOTS + slot; b < nbatch; b += (long long)gridDim.x * YFSLOTS) {
     const long long f = b / per_field, j = b - f * per_field;
     const long long row0 = (f * A.nz + lm) * A.nkx + j * A.rb;
     const int nr = (int)((ra - j * A.rb) < A.rb ? (ra - j * A.rb) : A.rb);
@@ -203,13 +213,13 @@ __global__ void __launch_bounds__(YTHREADS, 1) k_fft_y_fwd(FftYArgs A) {
     // the slot's previous bulk store must have read the buffer before this row's first stage overwrites it; waiting here (and not
     // between the loads and the arithmetic of the first round) keeps the first stage's registers free of the barrier: no spills
     if (st == 0) bulk_wait_read();
-    slot_barrier<YTPS>(slot);
+    slot_barrier<YFTPS>(slot);
     const MidNone mid;
-    run_edge<YTPS, R0, R0 * R1 * R2, false>(A.F.r[0], g, buf, tw + A.off[0], n, nr, st, mid);
-    slot_barrier<YTPS>(slot);
-    run_inner<YTPS, R0, R1, R2, false, false>(A, buf, tw, n, nr, st, slot);
+    run_edge<YFTPS, R0, R0 * R1 * R2, false>(A.F.r[0], g, buf, tw + A.off[0], n, nr, st, mid);
+    slot_barrier<YFTPS>(slot);
+    run_inner<YFTPS, R0, R1, R2, false, false>(A, buf, tw, n, nr, st, slot);
     fence_async_proxy();
-    slot_barrier<YTPS>(slot);
+    slot_barrier<YFTPS>(slot);
     if (st == 0) bulk_store(g, buf, (unsigned)nr * n * 16u);
   }
   if (st == 0) bulk_wait_all();
@@ -428,7 +438,7 @@ template <class T> cudaError_t upload(T** dst, const std::vector<T>& v, dp_plan*
   return cudaMemcpy(*dst, v.data(), sizeof(T) * v.size(), cudaMemcpyHostToDevice);
 }
 
-size_t smem_bytes_y(int n, int ntw, int rb) { return sizeof(double2) * ((size_t)ntw + (size_t)YSLOTS * rb * n) + 8 * YSLOTS; }
+size_t smem_bytes_y(int n, int ntw, int rb, int slots) { return sizeof(double2) * ((size_t)ntw + (size_t)slots * rb * n) + 8 * slots; }
 size_t smem_bytes_x(int M, int ntw, int rb) {
   return sizeof(double2) * ((size_t)ntw + (M / 2 + 1) + (size_t)XSLOTS * rb * M) + align16(sizeof(unsigned short) * M) + 8 * XSLOTS;
 }
@@ -508,11 +518,12 @@ cudaError_t dp_fft_own_create(dp_plan* P) {
   if ((e = upload(&O->d_pos_x, posx, P)) != cudaSuccess) return e;
   if ((e = upload(&O->d_ky_of_pos, kyp, P)) != cudaSuccess) return e;
   O->smem_x = smem_bytes_x(M, O->ntw_x, O->rbx);
-  O->smem_y = smem_bytes_y(ny, O->ntw_y, O->rby);
+  O->smem_y = smem_bytes_y(ny, O->ntw_y, O->rby, YSLOTS);
+  O->smem_y_fwd = smem_bytes_y(ny, O->ntw_y, O->rby, YFSLOTS);   // its own size: what the slots do not need stays L1 cache for the first stage's loads
   if (O->smem_x > 227 * 1024 || O->smem_y > 227 * 1024) return cudaErrorInvalidValue;
   O->ky_fwd = pick_y(O->Fy, false); O->ky_inv = pick_y(O->Fy, true);
   O->kx_fwd = pick_x(O->Fx, false, O->rbx, P->p.transfer_fp32 != 0); O->kx_inv = pick_x(O->Fx, true, O->rbx, P->p.transfer_fp32 != 0);
-  if ((e = cudaFuncSetAttribute(O->ky_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(O->ky_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y_fwd)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(O->ky_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(O->kx_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;
   if ((e = cudaFuncSetAttribute(O->kx_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;
@@ -554,7 +565,7 @@ cudaError_t dp_fft_own_forward(dp_plan* P, int nfields, cudaStream_t st) {
   if (e != cudaSuccess) return e;
   if (P->profiling && P->ev_ok && (e = cudaEventRecord(P->ev_fft[0], st)) != cudaSuccess) return e;
   const FftYArgs Y = y_args(P, nfields);
-  O->ky_fwd<<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb, YSLOTS), YTHREADS, O->smem_y, st>>>(Y);
+  O->ky_fwd<<<grid_for(O, (Y.rows + Y.rb - 1) / Y.rb, YFSLOTS), YFTHREADS, O->smem_y_fwd, st>>>(Y);
   return cudaGetLastError();
 }
 
