@@ -477,7 +477,10 @@ struct InterpArgs {
   double* Omega;             // may be NULL
 };
 
-constexpr int INTERP_WARPS = 8;
+#ifndef DP_INTERP_WARPS
+#define DP_INTERP_WARPS 16
+#endif
+constexpr int INTERP_WARPS = DP_INTERP_WARPS;
 
 // One warp per particle (sorted order, so neighbouring warps gather from neighbouring columns): the lanes sweep the
 // w x w x (lmax-lmin+1) footprint, weights come from the particle's records, the six sums are reduced by shuffles.
@@ -629,7 +632,10 @@ cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaSt
   A.grid = P->d_real; A.real_field = P->real_field;
   A.U = U; A.Omega = Omega;
   int blocks = (n + INTERP_WARPS - 1) / INTERP_WARPS;
-  const int maxb = 148 * 64;
+#ifndef DP_INTERP_MAXB
+#define DP_INTERP_MAXB 32
+#endif
+  const int maxb = 148 * DP_INTERP_MAXB;
   if (blocks > maxb) blocks = maxb;
   if (blocks < 1) blocks = 1;
   const bool f32 = P->p.transfer_fp32 != 0, kt = P->kernel_torque;
