@@ -196,7 +196,10 @@ struct WeightArgs {
 // lmin..lmax in z), and every evaluation of the kernel costs an exp and a square root: the warp first stores zeros over the whole
 // record, then lanes 0-7 take the x entries, 8-15 the y entries and lanes 16-31 the planes lmin, lmin + 1, ... sixteen at a time, so a
 // warp evaluates the kernel once (plus once per image term of eq 9 that reaches some plane) instead of once per 32 record entries.
-constexpr int WEIGHT_WARPS = 8;
+#ifndef DP_WEIGHT_WARPS
+#define DP_WEIGHT_WARPS 8
+#endif
+constexpr int WEIGHT_WARPS = DP_WEIGHT_WARPS;
 __global__ void __launch_bounds__(WEIGHT_WARPS * 32) k_weights(int n, WeightArgs A) {
   const GridGeom& g = A.g;
   const int wrec = 2 * DP_MAX_W + g.nz;
