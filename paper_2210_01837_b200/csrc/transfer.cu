@@ -109,37 +109,46 @@ __global__ void k_bin_count(int n, const double* __restrict__ pos, GridGeom g, i
   slot_of[p] = atomicAdd(&bin_count[b], 1);
 }
 
-// exclusive scan of bin_count -> bin_start[0..nbins]; one CTA, chunks of blockDim * 8 elements (eight consecutive bins per thread)
-__global__ void k_scan(int nbins, const int* __restrict__ cnt, int* __restrict__ start) {
-  constexpr int E = 8;
+// exclusive scan of bin_count -> bin_start[0..nbins] in two launches: k_scan_local scans chunks of SCAN_CHUNK bins (one CTA each, eight
+// consecutive bins per thread) and leaves each chunk's total in block_sum; k_scan_add adds the totals of the preceding chunks
+constexpr int SCAN_THREADS = 1024, SCAN_E = 8, SCAN_CHUNK = SCAN_THREADS * SCAN_E;
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_local(int nbins, const int* __restrict__ cnt, int* __restrict__ start, int* __restrict__ block_sum) {
   __shared__ int warp_sums[32];
-  __shared__ int carry;
-  if (threadIdx.x == 0) carry = 0;
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const int i0 = blockIdx.x * SCAN_CHUNK + threadIdx.x * SCAN_E;
+  int v[SCAN_E], tot = 0;
+#pragma unroll
+  for (int e = 0; e < SCAN_E; ++e) { v[e] = (i0 + e < nbins) ? cnt[i0 + e] : 0; tot += v[e]; }
+  int s = tot;
+  for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += t; }
+  if (lane == 31) warp_sums[wid] = s;
   __syncthreads();
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5;
-  for (int base = 0; base < nbins; base += blockDim.x * E) {
-    const int i0 = base + threadIdx.x * E;
-    int v[E], tot = 0;
-#pragma unroll
-    for (int e = 0; e < E; ++e) { v[e] = (i0 + e < nbins) ? cnt[i0 + e] : 0; tot += v[e]; }
-    int s = tot;
-    for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += t; }
-    if (lane == 31) warp_sums[wid] = s;
-    __syncthreads();
-    if (wid == 0) {
-      int ws = lane < nw ? warp_sums[lane] : 0;
-      for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(0xffffffffu, ws, o); if (lane >= o) ws += t; }
-      warp_sums[lane] = ws;
-    }
-    __syncthreads();
-    int run = carry + (wid > 0 ? warp_sums[wid - 1] : 0) + s - tot;        // exclusive prefix of this thread's first bin
-#pragma unroll
-    for (int e = 0; e < E; ++e) { if (i0 + e < nbins) start[i0 + e] = run; run += v[e]; }
-    __syncthreads();
-    if (threadIdx.x == blockDim.x - 1) carry = run;
-    __syncthreads();
+  if (wid == 0) {
+    int ws = warp_sums[lane];
+    for (int o = 1; o < 32; o <<= 1) { int t = __shfl_up_sync(0xffffffffu, ws, o); if (lane >= o) ws += t; }
+    warp_sums[lane] = ws;
   }
-  if (threadIdx.x == 0) start[nbins] = carry;
+  __syncthreads();
+  int run = (wid > 0 ? warp_sums[wid - 1] : 0) + s - tot;                 // exclusive prefix of this thread's first bin within the chunk
+#pragma unroll
+  for (int e = 0; e < SCAN_E; ++e) { if (i0 + e < nbins) start[i0 + e] = run; run += v[e]; }
+  if (threadIdx.x == SCAN_THREADS - 1) block_sum[blockIdx.x] = run;
+}
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_add(int nbins, int nblocks, int* __restrict__ start, const int* __restrict__ block_sum) {
+  __shared__ int s_off, s_part[32];
+  // offset of this chunk = sum of the totals of the chunks before it (a few dozen values: one warp-shuffle reduction per 1024)
+  int acc = 0;
+  for (int b = threadIdx.x; b < (int)blockIdx.x; b += SCAN_THREADS) acc += block_sum[b];
+  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+  if ((threadIdx.x & 31) == 0) s_part[threadIdx.x >> 5] = acc;
+  __syncthreads();
+  if (threadIdx.x == 0) { int t = 0; for (int w = 0; w < SCAN_THREADS / 32; ++w) t += s_part[w]; s_off = t; }
+  __syncthreads();
+  const int off = s_off;
+  const int i0 = blockIdx.x * SCAN_CHUNK + threadIdx.x * SCAN_E;
+#pragma unroll
+  for (int e = 0; e < SCAN_E; ++e) if (i0 + e < nbins) start[i0 + e] += off;
+  if ((int)blockIdx.x == nblocks - 1 && threadIdx.x == 0) start[nbins] = off + block_sum[blockIdx.x];
 }
 
 __global__ void k_bin_scatter(int n, const double* __restrict__ pos, const double* __restrict__ force,
@@ -578,7 +587,9 @@ cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* fo
   if (e != cudaSuccess) return e;
   const int T = 256, B = (n + T - 1) / T;
   k_bin_count<<<B, T, 0, st>>>(n, pos, g, P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_flag);
-  k_scan<<<1, 1024, 0, st>>>(P->nbins, P->d_bin_count, P->d_bin_start);
+  const int nsb = (P->nbins + SCAN_CHUNK - 1) / SCAN_CHUNK;      // P->d_scan_sums holds nsb ints (plan.cu)
+  k_scan_local<<<nsb, SCAN_THREADS, 0, st>>>(P->nbins, P->d_bin_count, P->d_bin_start, P->d_scan_sums);
+  k_scan_add<<<nsb, SCAN_THREADS, 0, st>>>(P->nbins, nsb, P->d_bin_start, P->d_scan_sums);
   k_bin_scatter<<<B, T, 0, st>>>(n, pos, force, torque, g, P->d_bin_of, P->d_slot_of, P->d_bin_start, P->d_znodes, P->d_perm, P->d_meta,
                                 P->d_pos_s, P->d_frc_s, P->torques ? P->d_trq_s : nullptr, P->d_lmin);
   if (dense) { e = cudaMemsetAsync(P->d_lmin, 0, sizeof(int), st); if (e != cudaSuccess) return e; }   // every plane is transformed
