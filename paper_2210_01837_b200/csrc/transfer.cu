@@ -272,8 +272,11 @@ struct SpreadArgs {
 // MODE 0: field triple blockIdx.z (0: forces with Delta_M, 1: torques with Delta_D) gets sum_j val_j S(j; g)   (eq 7 without the curl,
 //         which the solve kernel takes in Fourier-Chebyshev space);
 // MODE 1 (kernel-derivative torques): ONE triple f = sum_j [F_j S_M(j; g) + (1/2) G_j(g) x tau_j], three records per candidate.
+#ifndef DP_SPREAD_MINB
+#define DP_SPREAD_MINB (NZ <= 32 ? 3 : 2)
+#endif
 template <int NZ, class GT, int MODE>
-__global__ void __launch_bounds__(SPREAD_THREADS, (NZ <= 32 ? 3 : 2)) k_spread(SpreadArgs A) {
+__global__ void __launch_bounds__(SPREAD_THREADS, DP_SPREAD_MINB) k_spread(SpreadArgs A) {
   constexpr int NL = (NZ + ZSPLIT - 1) / ZSPLIT;
   constexpr int WREC = 2 * DP_MAX_W + NZ;                 // record length in global memory
   constexpr int WS = 2 * DP_MAX_W + NL * ZSPLIT;          // staged record length (zero padded to whole z residue classes)
