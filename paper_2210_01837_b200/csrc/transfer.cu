@@ -275,17 +275,112 @@ struct SpreadArgs {
 #ifndef DP_SPREAD_MINB
 #define DP_SPREAD_MINB (NZ <= 32 ? 3 : 2)
 #endif
+// staged candidates of one chunk: weight records (zero padded to whole z residue classes), values, footprint records
+template <int NZ, int MODE> struct SpreadBuf {
+  static constexpr int NL = (NZ + ZSPLIT - 1) / ZSPLIT;
+  static constexpr int WREC = 2 * DP_MAX_W + NZ;                 // record length in global memory
+  static constexpr int WS = 2 * DP_MAX_W + NL * ZSPLIT;          // staged record length
+  static constexpr int NREC = MODE ? 3 : 1;
+  static constexpr int PC = MODE ? PCH / 2 : PCH;                // candidates per chunk
+  static constexpr int NV = MODE ? 6 : 3;
+  double w[PC][NREC][WS];
+  double val[PC][NV];
+  int4 meta[PC];                                                 // i0, j0 (wrapped origin node), lmin, lmax
+};
+
+// every thread adds the nl staged particles that cover its column (gi, gj) to its own planes l = ZSPLIT li + tz
+template <int NZ, class GT, int MODE>
+__device__ __forceinline__ void accumulate_chunk(GT (&acc)[(NZ + ZSPLIT - 1) / ZSPLIT][3], const SpreadBuf<NZ, MODE>& B, int nl, const GridGeom& g, int gi, int gj, int tz,
+                                                 bool in_grid) {
+  constexpr int NL = SpreadBuf<NZ, MODE>::NL, NV = SpreadBuf<NZ, MODE>::NV;
+  const int w = g.w;
+  if (in_grid) {
+    for (int q = 0; q < nl; ++q) {
+      const int4 m = B.meta[q];
+      int a = gi - m.x; if (a < 0) a += g.nx;
+      int bb = gj - m.y; if (bb < 0) bb += g.ny;
+      if (a < w && bb < w) {
+        if (MODE == 0) {
+          const GT wxy = (GT)B.w[q][0][a] * (GT)B.w[q][0][DP_MAX_W + bb];
+          const GT v0 = (GT)B.val[q][0] * wxy, v1 = (GT)B.val[q][1] * wxy, v2 = (GT)B.val[q][2] * wxy;
+          const double* zt = &B.w[q][0][2 * DP_MAX_W + tz];
+          // zeta vanishes outside [lmin, lmax]: skipping a half of the planes that lies outside is exact
+          if (m.z < ZSPLIT * (NL / 2)) {
+#pragma unroll
+            for (int li = 0; li < NL / 2; ++li) {
+              const GT z = (GT)zt[ZSPLIT * li];
+              acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+            }
+          }
+          if (m.w >= ZSPLIT * (NL / 2)) {
+#pragma unroll
+            for (int li = NL / 2; li < NL; ++li) {
+              const GT z = (GT)zt[ZSPLIT * li];
+              acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
+            }
+          }
+        } else {
+          const double* wM = B.w[q][0]; const double* wD = B.w[q][MODE ? 1 : 0]; const double* wG = B.w[q][MODE ? 2 : 0];
+          const GT pM = (GT)wM[a] * (GT)wM[DP_MAX_W + bb];
+          const GT c0f = (GT)B.val[q][0] * pM, c1f = (GT)B.val[q][1] * pM, c2f = (GT)B.val[q][2] * pM;     // x zeta_M(l)
+          const GT tx = (GT)B.val[q][NV - 3], ty = (GT)B.val[q][NV - 2], tzq = (GT)B.val[q][NV - 1];
+          const GT pxy = (GT)wD[a] * (GT)wD[DP_MAX_W + bb];                   // phi(x) phi(y)
+          const GT dxy = (GT)wG[a] * (GT)wD[DP_MAX_W + bb];                   // phi'(x) phi(y)
+          const GT xdy = (GT)wD[a] * (GT)wG[DP_MAX_W + bb];                   // phi(x) phi'(y)
+          // (1/2) G x tau with G = (dxy zeta, xdy zeta, pxy zeta'):  coefficients of zeta_D(l) and of zeta_D'(l)
+          const GT a0 = (GT)0.5 * tzq * xdy, a1 = -(GT)0.5 * tzq * dxy, a2 = (GT)0.5 * (ty * dxy - tx * xdy);
+          const GT b0 = -(GT)0.5 * ty * pxy, b1 = (GT)0.5 * tx * pxy;
+          const double* zm = &wM[2 * DP_MAX_W + tz]; const double* zd = &wD[2 * DP_MAX_W + tz]; const double* zg = &wG[2 * DP_MAX_W + tz];
+          if (m.z < ZSPLIT * (NL / 2)) {
+#pragma unroll
+            for (int li = 0; li < NL / 2; ++li) {
+              const GT zM = (GT)zm[ZSPLIT * li], zD = (GT)zd[ZSPLIT * li], zG = (GT)zg[ZSPLIT * li];
+              acc[li][0] = fma(c0f, zM, fma(a0, zD, fma(b0, zG, acc[li][0])));
+              acc[li][1] = fma(c1f, zM, fma(a1, zD, fma(b1, zG, acc[li][1])));
+              acc[li][2] = fma(c2f, zM, fma(a2, zD, acc[li][2]));
+            }
+          }
+          if (m.w >= ZSPLIT * (NL / 2)) {
+#pragma unroll
+            for (int li = NL / 2; li < NL; ++li) {
+              const GT zM = (GT)zm[ZSPLIT * li], zD = (GT)zd[ZSPLIT * li], zG = (GT)zg[ZSPLIT * li];
+              acc[li][0] = fma(c0f, zM, fma(a0, zD, fma(b0, zG, acc[li][0])));
+              acc[li][1] = fma(c1f, zM, fma(a1, zD, fma(b1, zG, acc[li][1])));
+              acc[li][2] = fma(c2f, zM, fma(a2, zD, acc[li][2]));
+            }
+          }
+        }
+      }
+    }
+  }
+}
+
+// every grid value of the tile's planes that can hold force is written exactly once
+template <int NZ, class GT>
+__device__ __forceinline__ void store_tile(const GT (&acc)[(NZ + ZSPLIT - 1) / ZSPLIT][3], const SpreadArgs& A, const GridGeom& g, int grp, int gi, int gj, int tz, bool in_grid) {
+  constexpr int NL = (NZ + ZSPLIT - 1) / ZSPLIT;
+  if (in_grid) {
+    const int lm = __ldg(A.lmin);
+    GT* dst = reinterpret_cast<GT*>(A.grid) + (size_t)A.field0[grp] * A.real_field + ((size_t)tz * g.ny + gj) * g.nx + gi;
+    const size_t step = (size_t)ZSPLIT * g.ny * g.nx;             // from plane l to plane l + ZSPLIT
+#pragma unroll
+    for (int li = 0; li < NL; ++li) {
+      const int l = ZSPLIT * li + tz;
+      if (l >= lm && l < NZ) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) dst[c * A.real_field] = acc[li][c];
+      }
+      dst += step;
+    }
+  }
+
+}
+
 template <int NZ, class GT, int MODE>
 __global__ void __launch_bounds__(SPREAD_THREADS, DP_SPREAD_MINB) k_spread(SpreadArgs A) {
-  constexpr int NL = (NZ + ZSPLIT - 1) / ZSPLIT;
-  constexpr int WREC = 2 * DP_MAX_W + NZ;                 // record length in global memory
-  constexpr int WS = 2 * DP_MAX_W + NL * ZSPLIT;          // staged record length (zero padded to whole z residue classes)
-  constexpr int NREC = MODE ? 3 : 1;
-  constexpr int PC = MODE ? PCH / 2 : PCH;                // candidates per chunk
-  constexpr int NV = MODE ? 6 : 3;
-  __shared__ __align__(16) double s_w[PC][NREC][WS];
-  __shared__ double s_val[PC][NV];
-  __shared__ int4 s_meta[PC];                 // i0, j0 (wrapped origin node), lmin, lmax
+  typedef SpreadBuf<NZ, MODE> SB;
+  constexpr int NL = SB::NL, WREC = SB::WREC, WS = SB::WS, NREC = SB::NREC, PC = SB::PC;
+  __shared__ __align__(16) SB B;
   __shared__ int s_rbeg[MAXR], s_roff[MAXR + 1];   // candidate ranges in the sorted arrays; prefix sums of their lengths
   __shared__ int s_keep[MAXKEEP];             // candidates whose footprint really touches the tile
   __shared__ int s_nkeep;
@@ -366,13 +461,13 @@ __global__ void __launch_bounds__(SPREAD_THREADS, DP_SPREAD_MINB) k_spread(Sprea
       const int nl = min(PC, nkeep - c0);
       if (t < nl) {
         const int p = s_keep[c0 + t];
-        s_meta[t] = A.meta[p];
+        B.meta[t] = A.meta[p];
         if (MODE) {
 #pragma unroll
-          for (int c = 0; c < 3; ++c) { s_val[t][c] = A.val_s[0][3 * (size_t)p + c]; s_val[t][3 + c] = A.val_s[1][3 * (size_t)p + c]; }
+          for (int c = 0; c < 3; ++c) { B.val[t][c] = A.val_s[0][3 * (size_t)p + c]; B.val[t][3 + c] = A.val_s[1][3 * (size_t)p + c]; }
         } else {
           const double* __restrict__ val = A.val_s[grp];
-          s_val[t][0] = val[3 * (size_t)p]; s_val[t][1] = val[3 * (size_t)p + 1]; s_val[t][2] = val[3 * (size_t)p + 2];
+          B.val[t][0] = val[3 * (size_t)p]; B.val[t][1] = val[3 * (size_t)p + 1]; B.val[t][2] = val[3 * (size_t)p + 2];
         }
       }
       // the weight records travel as asynchronous 8-byte copies: all of a thread's entries are in flight at once (one round of
@@ -383,99 +478,26 @@ __global__ void __launch_bounds__(SPREAD_THREADS, DP_SPREAD_MINB) k_spread(Sprea
         for (int i = t; i < nl * NREC * WH; i += SPREAD_THREADS) {
           const int q = i / (NREC * WH), rem = i - q * (NREC * WH), k = rem / WH, e = 2 * (rem - k * WH);
           const int kk = MODE ? k : grp;
-          if (e < WREC) cp_async16(&s_w[q][k][e], A.wrec + ((size_t)kk * A.cap + s_keep[c0 + q]) * WREC + e);
-          else { s_w[q][k][e] = 0.0; s_w[q][k][e + 1] = 0.0; }
+          if (e < WREC) cp_async16(&B.w[q][k][e], A.wrec + ((size_t)kk * A.cap + s_keep[c0 + q]) * WREC + e);
+          else { B.w[q][k][e] = 0.0; B.w[q][k][e + 1] = 0.0; }
         }
       } else {
         for (int i = t; i < nl * NREC * WS; i += SPREAD_THREADS) {
           const int q = i / (NREC * WS), rem = i - q * (NREC * WS), k = rem / WS, e = rem - k * WS;
           const int kk = MODE ? k : grp;
-          if (e < WREC) cp_async8(&s_w[q][k][e], A.wrec + ((size_t)kk * A.cap + s_keep[c0 + q]) * WREC + e);
-          else s_w[q][k][e] = 0.0;
+          if (e < WREC) cp_async8(&B.w[q][k][e], A.wrec + ((size_t)kk * A.cap + s_keep[c0 + q]) * WREC + e);
+          else B.w[q][k][e] = 0.0;
         }
       }
       cp_async_wait_all_groups();
       __syncthreads();
-      // ---- accumulate: each thread adds the particles covering its column to its own planes
-      if (in_grid) {
-        for (int q = 0; q < nl; ++q) {
-          const int4 m = s_meta[q];
-          int a = gi - m.x; if (a < 0) a += g.nx;
-          int bb = gj - m.y; if (bb < 0) bb += g.ny;
-          if (a < w && bb < w) {
-            if (MODE == 0) {
-              const GT wxy = (GT)s_w[q][0][a] * (GT)s_w[q][0][DP_MAX_W + bb];
-              const GT v0 = (GT)s_val[q][0] * wxy, v1 = (GT)s_val[q][1] * wxy, v2 = (GT)s_val[q][2] * wxy;
-              const double* zt = &s_w[q][0][2 * DP_MAX_W + tz];
-              // zeta vanishes outside [lmin, lmax]: skipping a half of the planes that lies outside is exact
-              if (m.z < ZSPLIT * (NL / 2)) {
-#pragma unroll
-                for (int li = 0; li < NL / 2; ++li) {
-                  const GT z = (GT)zt[ZSPLIT * li];
-                  acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
-                }
-              }
-              if (m.w >= ZSPLIT * (NL / 2)) {
-#pragma unroll
-                for (int li = NL / 2; li < NL; ++li) {
-                  const GT z = (GT)zt[ZSPLIT * li];
-                  acc[li][0] = fma(v0, z, acc[li][0]); acc[li][1] = fma(v1, z, acc[li][1]); acc[li][2] = fma(v2, z, acc[li][2]);
-                }
-              }
-            } else {
-              const double* wM = s_w[q][0]; const double* wD = s_w[q][MODE ? 1 : 0]; const double* wG = s_w[q][MODE ? 2 : 0];
-              const GT pM = (GT)wM[a] * (GT)wM[DP_MAX_W + bb];
-              const GT c0f = (GT)s_val[q][0] * pM, c1f = (GT)s_val[q][1] * pM, c2f = (GT)s_val[q][2] * pM;     // x zeta_M(l)
-              const GT tx = (GT)s_val[q][NV - 3], ty = (GT)s_val[q][NV - 2], tzq = (GT)s_val[q][NV - 1];
-              const GT pxy = (GT)wD[a] * (GT)wD[DP_MAX_W + bb];                   // phi(x) phi(y)
-              const GT dxy = (GT)wG[a] * (GT)wD[DP_MAX_W + bb];                   // phi'(x) phi(y)
-              const GT xdy = (GT)wD[a] * (GT)wG[DP_MAX_W + bb];                   // phi(x) phi'(y)
-              // (1/2) G x tau with G = (dxy zeta, xdy zeta, pxy zeta'):  coefficients of zeta_D(l) and of zeta_D'(l)
-              const GT a0 = (GT)0.5 * tzq * xdy, a1 = -(GT)0.5 * tzq * dxy, a2 = (GT)0.5 * (ty * dxy - tx * xdy);
-              const GT b0 = -(GT)0.5 * ty * pxy, b1 = (GT)0.5 * tx * pxy;
-              const double* zm = &wM[2 * DP_MAX_W + tz]; const double* zd = &wD[2 * DP_MAX_W + tz]; const double* zg = &wG[2 * DP_MAX_W + tz];
-              if (m.z < ZSPLIT * (NL / 2)) {
-#pragma unroll
-                for (int li = 0; li < NL / 2; ++li) {
-                  const GT zM = (GT)zm[ZSPLIT * li], zD = (GT)zd[ZSPLIT * li], zG = (GT)zg[ZSPLIT * li];
-                  acc[li][0] = fma(c0f, zM, fma(a0, zD, fma(b0, zG, acc[li][0])));
-                  acc[li][1] = fma(c1f, zM, fma(a1, zD, fma(b1, zG, acc[li][1])));
-                  acc[li][2] = fma(c2f, zM, fma(a2, zD, acc[li][2]));
-                }
-              }
-              if (m.w >= ZSPLIT * (NL / 2)) {
-#pragma unroll
-                for (int li = NL / 2; li < NL; ++li) {
-                  const GT zM = (GT)zm[ZSPLIT * li], zD = (GT)zd[ZSPLIT * li], zG = (GT)zg[ZSPLIT * li];
-                  acc[li][0] = fma(c0f, zM, fma(a0, zD, fma(b0, zG, acc[li][0])));
-                  acc[li][1] = fma(c1f, zM, fma(a1, zD, fma(b1, zG, acc[li][1])));
-                  acc[li][2] = fma(c2f, zM, fma(a2, zD, acc[li][2]));
-                }
-              }
-            }
-          }
-        }
-      }
+      accumulate_chunk<NZ, GT, MODE>(acc, B, nl, g, gi, gj, tz, in_grid);
       __syncthreads();
     }
     if (t == 0) s_nkeep = 0;
     __syncthreads();
   }
-  // ---- store: every grid value of the planes that can hold force written exactly once
-  if (in_grid) {
-    const int lm = __ldg(A.lmin);
-    GT* dst = reinterpret_cast<GT*>(A.grid) + (size_t)A.field0[grp] * A.real_field + ((size_t)tz * g.ny + gj) * g.nx + gi;
-    const size_t step = (size_t)ZSPLIT * g.ny * g.nx;             // from plane l to plane l + ZSPLIT
-#pragma unroll
-    for (int li = 0; li < NL; ++li) {
-      const int l = ZSPLIT * li + tz;
-      if (l >= lm && l < NZ) {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) dst[c * A.real_field] = acc[li][c];
-      }
-      dst += step;
-    }
-  }
+  store_tile<NZ, GT>(acc, A, g, grp, gi, gj, tz, in_grid);
 }
 
 // ---------------------------------------------------------------------------------------------- interpolate
