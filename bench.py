@@ -30,10 +30,10 @@ import numpy as np
 import workloads
 
 METRIC = "ms per DP-wall mobility product M·F at N=1M; particles/s; % of HBM roofline"
-# kernels of this library launched per product: k_bin_count, k_scan_local, k_scan_add, k_bin_scatter, k_weights, k_spread, k_solve_pair<nz> (three grid
+# kernels of this library launched per product: k_bin_count, k_scan_local, k_scan_add, k_bin_scatter, k_weights, k_tile_lists, k_spread_pipe, k_spread (the tiles that overflow a staged chunk), k_solve_pair<nz> (three grid
 # fields each way) or k_solve<nz> (six), k_zero_mode, k_interp, plus k_fft_x_fwd, k_fft_y_fwd, k_fft_y_inv, k_fft_x_inv with the
 # library's own FFT passes (else cuFFT's kernels)
-MY_KERNELS_PER_STEP = {"own": 13, "cufft": 9}
+MY_KERNELS_PER_STEP = {"own": 15, "cufft": 11}
 
 
 def ncu_traffic(kernel_prefix: str, cfg: int, torque_mode: str):

@@ -54,6 +54,10 @@ struct dp_plan {
   int* d_slot_of = nullptr;     // rank within its bin
   int* d_bin_count = nullptr;   // [nbins]
   int* d_bin_start = nullptr;   // [nbins+1]
+  int* d_tile_cnt = nullptr;    // [nbins] survivors per spread tile (transfer.cu: k_tile_lists)
+  int* d_tile_list = nullptr;   // [nbins][40] their indices in the sorted particle arrays (the first 40)
+  int* d_ov_tiles = nullptr;    // [nbins] tiles with more survivors than a staged chunk holds
+  int* d_ov_count = nullptr;    // [1]
   int* d_scan_sums = nullptr;   // [ceil(nbins / 8192)] chunk totals of the two-launch scan (transfer.cu)
   int* d_flag = nullptr;        // out-of-domain flag
   int* d_lmin = nullptr;        // lowest plane index touched by any footprint of the current apply (planes below it are zero)

@@ -317,7 +317,7 @@ int dp_destroy(dp_plan* P) {
   if (P->fft_ok) { cufftDestroy(P->fft_fwd); cufftDestroy(P->fft_inv); }
   dp_fft_own_destroy(P);
   void* bufs[] = {P->d_real, P->d_cplx, P->d_fft_work, P->d_znodes, P->d_zweights, P->d_pos_s, P->d_frc_s, P->d_trq_s, P->d_perm, P->d_meta, P->d_wrec,
-                  P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_bin_start, P->d_scan_sums, P->d_flag, P->d_lmin};
+                  P->d_bin_of, P->d_slot_of, P->d_bin_count, P->d_bin_start, P->d_scan_sums, P->d_tile_cnt, P->d_tile_list, P->d_ov_tiles, P->d_ov_count, P->d_flag, P->d_lmin};
   for (void* b : bufs) if (b) cudaFree(b);
   if (P->ev_ok) { for (auto& e : P->ev) cudaEventDestroy(e); for (auto& e : P->ev_fft) cudaEventDestroy(e); }
   if (P->host_stage) {
@@ -400,6 +400,10 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   TRY(dev_alloc(P, &P->d_bin_count, (size_t)P->nbins));
   TRY(dev_alloc(P, &P->d_bin_start, (size_t)P->nbins + 1));
   TRY(dev_alloc(P, &P->d_scan_sums, (size_t)P->nbins / 8192 + 1));
+  TRY(dev_alloc(P, &P->d_tile_cnt, (size_t)P->nbins));
+  TRY(dev_alloc(P, &P->d_tile_list, (size_t)P->nbins * 40));
+  TRY(dev_alloc(P, &P->d_ov_tiles, (size_t)P->nbins));
+  TRY(dev_alloc(P, &P->d_ov_count, (size_t)1));
   TRY(dev_alloc(P, &P->d_flag, (size_t)1));
   TRY(dev_alloc(P, &P->d_lmin, (size_t)1));
   if (P->own_fft) {

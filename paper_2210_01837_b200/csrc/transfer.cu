@@ -376,8 +376,10 @@ __device__ __forceinline__ void store_tile(const GT (&acc)[(NZ + ZSPLIT - 1) / Z
 
 }
 
+// With a tile list (ov_tiles, *ov_count) the CTAs walk that list instead of taking the tile from blockIdx: the tiles the pipelined
+// kernel below leaves to this one (more survivors than a staged chunk holds).
 template <int NZ, class GT, int MODE>
-__global__ void __launch_bounds__(SPREAD_THREADS, DP_SPREAD_MINB) k_spread(SpreadArgs A) {
+__global__ void __launch_bounds__(SPREAD_THREADS, DP_SPREAD_MINB) k_spread(SpreadArgs A, const int* __restrict__ ov_tiles, const int* __restrict__ ov_count) {
   typedef SpreadBuf<NZ, MODE> SB;
   constexpr int NL = SB::NL, WREC = SB::WREC, WS = SB::WS, NREC = SB::NREC, PC = SB::PC;
   __shared__ __align__(16) SB B;
@@ -388,9 +390,12 @@ __global__ void __launch_bounds__(SPREAD_THREADS, DP_SPREAD_MINB) k_spread(Sprea
   const GridGeom& g = A.g;
   const int w = g.w;
   const int grp = blockIdx.z;
-  const int X0 = blockIdx.x * TX, Y0 = blockIdx.y * TY;
   const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
   const int ti = t % TX, tj = (t / TX) % TY, tz = t / (TX * TY);
+  const int nlist = ov_tiles ? __ldg(ov_count) : 1;
+  for (int it = ov_tiles ? (int)blockIdx.x : 0; it < nlist; it += ov_tiles ? (int)gridDim.x : 1) {
+  const int tile = ov_tiles ? __ldg(ov_tiles + it) : -1;
+  const int X0 = (tile >= 0 ? tile % g.nbx : (int)blockIdx.x) * TX, Y0 = (tile >= 0 ? tile / g.nbx : (int)blockIdx.y) * TY;
   const int gi = X0 + ti, gj = Y0 + tj;
   const bool in_grid = gi < g.nx && gj < g.ny;
 
@@ -498,6 +503,163 @@ __global__ void __launch_bounds__(SPREAD_THREADS, DP_SPREAD_MINB) k_spread(Sprea
     __syncthreads();
   }
   store_tile<NZ, GT>(acc, A, g, grp, gi, gj, tz, in_grid);
+  __syncthreads();                             // the shared state is reused by the next tile of the list
+  }
+}
+
+// ---------------------------------------------------------------------------------------------- spread, pipelined
+// Per-tile survivor lists, built once per product by one warp per tile (k_tile_lists): the particles whose w x w footprint touches
+// the tile's columns, at most LMAX stored, the true count beside them; tiles with more survivors than a staged chunk holds go to an
+// overflow list that k_spread (above) works through.
+constexpr int LMAX = PCH;
+constexpr int LIST_WARPS = 8;
+__global__ void __launch_bounds__(LIST_WARPS * 32) k_tile_lists(GridGeom g, const int* __restrict__ bin_start, const int4* __restrict__ meta, int pc_limit,
+                                                                  int* __restrict__ tile_cnt, int* __restrict__ tile_list, int* __restrict__ ov_tiles, int* __restrict__ ov_count) {
+  const int lane = threadIdx.x & 31, tile = blockIdx.x * LIST_WARPS + (threadIdx.x >> 5);
+  if (tile >= g.nbx * g.nby) return;
+  const int w = g.w, X0 = (tile % g.nbx) * TX, Y0 = (tile / g.nbx) * TY;
+  // candidate ranges, exactly as in k_spread
+  int o = X0 - (w - 1); o %= g.nx; if (o < 0) o += g.nx;
+  const int len = min(TX, g.nx - X0) + w - 1;
+  const int b0 = o / TX, b1 = (o + len - 1 < g.nx) ? (o + len - 1) / TX : g.nbx - 1;
+  const int wrap_b1 = (o + len - 1 < g.nx) ? -1 : (o + len - 1 - g.nx) / TX;
+  int bys[MAXB];
+  const int ncy = origin_bins(Y0, min(TY, g.ny - Y0), TY, w, g.ny, bys);
+  const int per_row = wrap_b1 >= 0 ? 2 : 1;
+  const int nr = ncy * per_row;
+  int beg = 0, cnt = 0;
+  if (lane < nr) {
+    const int row = bys[lane / per_row], piece = lane % per_row;
+    const int ba = piece == 0 ? b0 : 0, bb = piece == 0 ? b1 : min(wrap_b1, b0 - 1);
+    beg = bin_start[row * g.nbx + ba];
+    cnt = bb >= ba ? bin_start[row * g.nbx + bb + 1] - beg : 0;
+  }
+  int incl = cnt;
+#pragma unroll
+  for (int o2 = 1; o2 < 16; o2 <<= 1) { const int v = __shfl_up_sync(0xffffffffu, incl, o2); if (lane >= o2) incl += v; }
+  const int total = __shfl_sync(0xffffffffu, incl, MAXR - 1);
+  const int excl = incl - cnt;
+  const int TXe = min(TX, g.nx - X0), TYe = min(TY, g.ny - Y0);
+  int nk = 0;
+  for (int c0 = 0; c0 < total; c0 += 32) {
+    const int c = c0 + lane;
+    int r = 0;
+#pragma unroll
+    for (int q = 0; q < MAXR; ++q) { const int iq = __shfl_sync(0xffffffffu, incl, q); r += (c >= iq) ? 1 : 0; }
+    r = r < MAXR ? r : MAXR - 1;
+    const int rb = __shfl_sync(0xffffffffu, beg, r), re = __shfl_sync(0xffffffffu, excl, r);
+    bool keep = false;
+    int src = 0;
+    if (c < total) {
+      src = rb + (c - re);
+      const int4 m = meta[src];
+      int dx = X0 - m.x; if (dx < 0) dx += g.nx;
+      int ex = m.x - X0; if (ex < 0) ex += g.nx;
+      int dy = Y0 - m.y; if (dy < 0) dy += g.ny;
+      int ey = m.y - Y0; if (ey < 0) ey += g.ny;
+      keep = (m.z <= m.w) && (dx < w || ex < TXe) && (dy < w || ey < TYe);
+    }
+    const unsigned bal = __ballot_sync(0xffffffffu, keep);
+    const int slot = nk + __popc(bal & ((1u << lane) - 1));
+    if (keep && slot < LMAX) tile_list[(size_t)tile * LMAX + slot] = src;
+    nk += __popc(bal);
+  }
+  if (lane == 0) {
+    tile_cnt[tile] = nk;
+    if (nk > pc_limit) ov_tiles[atomicAdd(ov_count, 1)] = tile;
+  }
+}
+
+__device__ __forceinline__ void cp_async4(int* smem_dst, const int* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async16v(void* smem_dst, const void* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+
+// Persistent CTAs (DP_SPREAD_MINB per SM) walk the tiles b, b + G, ... with everything that comes from global memory two steps ahead:
+// while tile k is accumulated from one staging buffer, the records, values and footprints of tile k + 1 arrive in the other one
+// (cp.async) and the survivor list of tile k + 2 in a third small slot — one __syncthreads per tile, no global latency on the
+// critical path.  Tiles whose list does not fit a chunk are skipped (k_spread takes them from the overflow list).
+template <int NZ, class GT, int MODE>
+__global__ void __launch_bounds__(SPREAD_THREADS, DP_SPREAD_MINB) k_spread_pipe(SpreadArgs A, const int* __restrict__ tile_cnt, const int* __restrict__ tile_list) {
+  typedef SpreadBuf<NZ, MODE> SB;
+  constexpr int NL = SB::NL, WREC = SB::WREC, WS = SB::WS, NREC = SB::NREC, PC = SB::PC, LS = LMAX + 1;
+  extern __shared__ __align__(16) unsigned char spread_smem[];
+  SB* B = reinterpret_cast<SB*>(spread_smem);                 // two staging buffers
+  int* s_list = reinterpret_cast<int*>(B + 2);                // three list slots: LMAX indices + the count
+
+  const GridGeom& g = A.g;
+  const int grp = blockIdx.y, ntiles = g.nbx * g.nby, G = gridDim.x;
+  const int t = threadIdx.x;
+  const int ti = t % TX, tj = (t / TX) % TY, tz = t / (TX * TY);
+
+  auto load_list = [&](int k, int tile) {
+    if (tile >= ntiles) return;
+    int* L = s_list + (k % 3) * LS;
+    if (t < LMAX) cp_async4(L + t, tile_list + (size_t)tile * LMAX + t);
+    else if (t == LMAX) cp_async4(L + LMAX, tile_cnt + tile);
+  };
+  auto stage = [&](int k, int tile) {
+    if (tile >= ntiles) return;
+    const int* L = s_list + (k % 3) * LS;
+    const int nl = L[LMAX];
+    if (nl > PC) return;
+    SB& b = B[k & 1];
+    if (t < nl) {
+      const int p = L[t];
+      cp_async16v(&b.meta[t], A.meta + p);
+      if (MODE) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) { cp_async8(&b.val[t][c], A.val_s[0] + 3 * (size_t)p + c); cp_async8(&b.val[t][3 + c], A.val_s[1] + 3 * (size_t)p + c); }
+      } else {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) cp_async8(&b.val[t][c], A.val_s[grp] + 3 * (size_t)p + c);
+      }
+    }
+    if constexpr (WREC % 2 == 0) {
+      constexpr int WH = WS / 2;
+      for (int i = t; i < nl * NREC * WH; i += SPREAD_THREADS) {
+        const int q = i / (NREC * WH), rem = i - q * (NREC * WH), k2 = rem / WH, e = 2 * (rem - k2 * WH);
+        const int kk = MODE ? k2 : grp;
+        if (e < WREC) cp_async16(&b.w[q][k2][e], A.wrec + ((size_t)kk * A.cap + L[q]) * WREC + e);
+        else { b.w[q][k2][e] = 0.0; b.w[q][k2][e + 1] = 0.0; }
+      }
+    } else {
+      for (int i = t; i < nl * NREC * WS; i += SPREAD_THREADS) {
+        const int q = i / (NREC * WS), rem = i - q * (NREC * WS), k2 = rem / WS, e = rem - k2 * WS;
+        const int kk = MODE ? k2 : grp;
+        if (e < WREC) cp_async8(&b.w[q][k2][e], A.wrec + ((size_t)kk * A.cap + L[q]) * WREC + e);
+        else b.w[q][k2][e] = 0.0;
+      }
+    }
+  };
+
+  const int tile0 = blockIdx.x;
+  load_list(0, tile0);
+  load_list(1, tile0 + G);
+  cp_async_wait_all_groups();
+  __syncthreads();
+  stage(0, tile0);
+  for (int k = 0, tile = tile0; tile < ntiles; ++k, tile += G) {
+    cp_async_wait_all_groups();                               // records of tile k, list of tile k + 1
+    __syncthreads();                                          // ... visible to all; every thread is done with tile k - 1
+    load_list(k + 2, tile + 2 * G);
+    stage(k + 1, tile + G);
+    const int nl = s_list[(k % 3) * LS + LMAX];
+    if (nl > PC) continue;                                    // overflow tile: left to k_spread
+    const int X0 = (tile % g.nbx) * TX, Y0 = (tile / g.nbx) * TY;
+    const int gi = X0 + ti, gj = Y0 + tj;
+    const bool in_grid = gi < g.nx && gj < g.ny;
+    GT acc[NL][3];
+#pragma unroll
+    for (int li = 0; li < NL; ++li) { acc[li][0] = 0; acc[li][1] = 0; acc[li][2] = 0; }
+    accumulate_chunk<NZ, GT, MODE>(acc, B[k & 1], nl, g, gi, gj, tz, in_grid);
+    store_tile<NZ, GT>(acc, A, g, grp, gi, gj, tz, in_grid);
+  }
+  cp_async_wait_all_groups();
 }
 
 // ---------------------------------------------------------------------------------------------- interpolate
@@ -647,18 +809,37 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
   A.grid = P->d_real;
   A.real_field = P->real_field;
   A.lmin = P->d_lmin;
-  dim3 grid(P->nbx, P->nby, ngroups);
   const bool f32 = P->p.transfer_fp32 != 0;
+  // survivor lists per tile, then the pipelined kernel over the tiles whose list fits a staged chunk, then the culling kernel over the rest
+  const int ntiles = P->nbx * P->nby;
+  const int pc_limit = kt ? PCH / 2 : PCH;
+  cudaError_t e = cudaMemsetAsync(P->d_ov_count, 0, sizeof(int), st);
+  if (e != cudaSuccess) return e;
+  k_tile_lists<<<(ntiles + LIST_WARPS - 1) / LIST_WARPS, LIST_WARPS * 32, 0, st>>>(A.g, P->d_bin_start, P->d_meta, pc_limit, P->d_tile_cnt, P->d_tile_list,
+                                                                                    P->d_ov_tiles, P->d_ov_count);
+  int sms = 148;
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->p.device);
+#define DP_SPREAD_LAUNCH(NZ, GT, MODE)                                                                                                   \
+  {                                                                                                                                      \
+    const int per_sm = (NZ <= 32 ? 3 : 2);                                                                                               \
+    const size_t smem = 2 * sizeof(SpreadBuf<NZ, MODE>) + 3 * (LMAX + 1) * sizeof(int);                                                  \
+    e = cudaFuncSetAttribute(k_spread_pipe<NZ, GT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                       \
+    if (e != cudaSuccess) return e;                                                                                                      \
+    const int gp = ntiles < sms * per_sm ? ntiles : sms * per_sm;                                                                        \
+    k_spread_pipe<NZ, GT, MODE><<<dim3(gp, ngroups), SPREAD_THREADS, smem, st>>>(A, P->d_tile_cnt, P->d_tile_list);                      \
+    k_spread<NZ, GT, MODE><<<dim3(gp, 1, ngroups), SPREAD_THREADS, 0, st>>>(A, P->d_ov_tiles, P->d_ov_count);                            \
+  }
 #define DP_SPREAD_CASE(NZ)                                                                        \
   case NZ:                                                                                        \
-    if (kt) { if (f32) k_spread<NZ, float, 1><<<grid, SPREAD_THREADS, 0, st>>>(A); else k_spread<NZ, double, 1><<<grid, SPREAD_THREADS, 0, st>>>(A); } \
-    else    { if (f32) k_spread<NZ, float, 0><<<grid, SPREAD_THREADS, 0, st>>>(A); else k_spread<NZ, double, 0><<<grid, SPREAD_THREADS, 0, st>>>(A); } \
+    if (kt) { if (f32) DP_SPREAD_LAUNCH(NZ, float, 1) else DP_SPREAD_LAUNCH(NZ, double, 1) }      \
+    else    { if (f32) DP_SPREAD_LAUNCH(NZ, float, 0) else DP_SPREAD_LAUNCH(NZ, double, 0) }      \
     break;
   switch (P->p.nz) {
     DP_SPREAD_CASE(16) DP_SPREAD_CASE(19) DP_SPREAD_CASE(24) DP_SPREAD_CASE(26) DP_SPREAD_CASE(32) DP_SPREAD_CASE(40) DP_SPREAD_CASE(48) DP_SPREAD_CASE(64)
     default: return cudaErrorInvalidValue;
   }
 #undef DP_SPREAD_CASE
+#undef DP_SPREAD_LAUNCH
   return cudaGetLastError();
 }
 
