@@ -201,7 +201,7 @@ struct WeightArgs {
   size_t cap;
 };
 
-// One warp per (particle, record).  Only about 22 of the 16 + nz entries of a record are not zero (w + w in x, y and the planes
+// One warp per particle, all of its records.  Only about 22 of the 16 + nz entries of a record are not zero (w + w in x, y and the planes
 // lmin..lmax in z), and every evaluation of the kernel costs an exp and a square root: the warp first stores zeros over the whole
 // record, then lanes 0-7 take the x entries, 8-15 the y entries and lanes 16-31 the planes lmin, lmin + 1, ... sixteen at a time, so a
 // warp evaluates the kernel once (plus once per image term of eq 9 that reaches some plane) instead of once per 32 record entries.
@@ -209,29 +209,48 @@ struct WeightArgs {
 #define DP_WEIGHT_WARPS 8
 #endif
 constexpr int WEIGHT_WARPS = DP_WEIGHT_WARPS;
-__global__ void __launch_bounds__(WEIGHT_WARPS * 32) k_weights(int n, WeightArgs A) {
+__global__ void __launch_bounds__(WEIGHT_WARPS * 32) k_weights(int n, WeightArgs A, int nrec) {
   const GridGeom& g = A.g;
   const int wrec = 2 * DP_MAX_W + g.nz;
-  const int lane = threadIdx.x & 31, p = blockIdx.x * WEIGHT_WARPS + (threadIdx.x >> 5), k = blockIdx.y;
+  const int lane = threadIdx.x & 31, p = blockIdx.x * WEIGHT_WARPS + (threadIdx.x >> 5);
   if (p >= n) return;
-  const double beta = A.beta[k], inv_Z = A.inv_Z[k], inv_alpha = A.inv_alpha;
   const int4 m = A.meta[p];
-  double* rec = A.wrec + ((size_t)k * A.cap + p) * wrec;
-  for (int e = lane; e < wrec; e += 32) rec[e] = 0.0;
-  if (m.z > m.w) return;                                         // skipped particle: an all-zero record
+  const double inv_alpha = A.inv_alpha;
+  // the particle's coordinate this lane works with: x for lanes 0-7, y for 8-15, z for the rest (one load for all of its records)
+  const double c = A.pos_s[3 * (size_t)p + (lane < DP_MAX_W ? 0 : (lane < 2 * DP_MAX_W ? 1 : 2))];
+  for (int k = 0; k < nrec; ++k) {
+    double* rec = A.wrec + ((size_t)k * A.cap + p) * wrec;
+    for (int e = lane; e < wrec; e += 32) rec[e] = 0.0;
+  }
+  if (m.z > m.w) return;                                         // skipped particle: all-zero records
   __syncwarp();
-  const double zp = A.pos_s[3 * (size_t)p + 2];
-  if (lane < 2 * DP_MAX_W) {
-    const int a = lane & (DP_MAX_W - 1);
-    if (a < g.w) {
-      const double xw = A.pos_s[3 * (size_t)p + (lane >= DP_MAX_W ? 1 : 0)];
-      const double i0 = ceil((xw - g.alpha) / g.h);              // unwrapped origin: distances use the unwrapped node (same expression as origin_cell)
-      rec[lane] = k < 2 ? es_phi((i0 + a) * g.h - xw, inv_alpha, beta, inv_Z) : es_dphi((i0 + a) * g.h - xw, inv_alpha, beta, inv_Z, A.ucut);
-    }
-  } else {
-    for (int l = m.z + (lane - 2 * DP_MAX_W); l <= m.w; l += 32 - 2 * DP_MAX_W) {
-      rec[2 * DP_MAX_W + l] = k < 2 ? zeta_weight(A.znodes[l], zp, g.H, g.wall_mode, inv_alpha, beta, inv_Z)
-                                    : dzeta_weight(A.znodes[l], zp, g.H, g.wall_mode, inv_alpha, beta, inv_Z, A.ucut);
+  const int a = lane & (DP_MAX_W - 1);
+  const double i0 = ceil((c - g.alpha) / g.h);                   // unwrapped origin: distances use the unwrapped node (same expression as origin_cell)
+  const bool is_xy = lane < 2 * DP_MAX_W;
+  const double far = 4.0 * g.alpha;                              // a distance outside every support
+  for (int k = 0; k < nrec; ++k) {
+    const double beta = A.beta[k], inv_Z = A.inv_Z[k];
+    double* rec = A.wrec + ((size_t)k * A.cap + p) * wrec;
+    // every lane evaluates the kernel ONCE per round at its own distance (x, y entries: node minus particle; z entries: z_l - z_p, sixteen
+    // planes per round); the image terms of eq 9 follow for the z lanes only where some lane of the warp is inside their support
+    for (int l0 = m.z; l0 <= m.w || l0 == m.z; l0 += 32 - 2 * DP_MAX_W) {
+      const int l = l0 + (lane - 2 * DP_MAX_W);
+      const bool zon = !is_xy && l <= m.w, xyon = is_xy && a < g.w && l0 == m.z;
+      const double zl = zon ? A.znodes[l] : 0.0;
+      const double s1 = xyon ? (i0 + a) * g.h - c : (zon ? zl - c : far);
+      const double s2 = zon ? zl + c : far, s3 = (zon && g.wall_mode == DP_SLIT) ? zl - (2.0 * g.H - c) : far;
+      double v;
+      if (k < 2) {
+        v = es_phi(s1, inv_alpha, beta, inv_Z);
+        if (__any_sync(0xffffffffu, fabs(s2) <= g.alpha)) v -= es_phi(s2, inv_alpha, beta, inv_Z);
+        if (__any_sync(0xffffffffu, fabs(s3) <= g.alpha)) v -= es_phi(s3, inv_alpha, beta, inv_Z);
+      } else {
+        v = es_dphi(s1, inv_alpha, beta, inv_Z, A.ucut);
+        if (__any_sync(0xffffffffu, fabs(s2) <= g.alpha)) v -= es_dphi(s2, inv_alpha, beta, inv_Z, A.ucut);
+        if (__any_sync(0xffffffffu, fabs(s3) <= g.alpha)) v -= es_dphi(s3, inv_alpha, beta, inv_Z, A.ucut);
+      }
+      if (xyon) rec[lane] = v;
+      else if (zon) rec[2 * DP_MAX_W + l] = v;
     }
   }
 }
@@ -796,8 +815,7 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
     W.inv_Z[0] = 1.0 / P->ZM; W.inv_Z[1] = 1.0 / P->ZD; W.inv_Z[2] = 1.0 / P->ZD; W.inv_alpha = 1.0 / P->alpha;
     W.ucut = P->ucutD;
     W.wrec = P->d_wrec; W.cap = (size_t)P->p.max_particles;
-    dim3 wg((unsigned)((n + WEIGHT_WARPS - 1) / WEIGHT_WARPS), P->nrec);
-    if (n > 0) k_weights<<<wg, WEIGHT_WARPS * 32, 0, st>>>(n, W);
+    if (n > 0) k_weights<<<(unsigned)((n + WEIGHT_WARPS - 1) / WEIGHT_WARPS), WEIGHT_WARPS * 32, 0, st>>>(n, W, P->nrec);
   }
   SpreadArgs A;
   A.g = make_geom(P);
