@@ -705,8 +705,11 @@ constexpr int INTERP_WARPS = DP_INTERP_WARPS;
 // W = kernel support (compile-time: the footprint index arithmetic of the inner loop then has no integer division)
 // MODE 0: U from fields 0-2 with Delta_M, Omega from fields 3-5 (= (1/2) curl u) with Delta_D   (eqs 10, 11);
 // MODE 1 (kernel-derivative torques): U as before, Omega = (1/2) sum_g (u x G) h^2 (H/2) w_l from the SAME three fields.
+#ifndef DP_INTERP_MINB
+#define DP_INTERP_MINB 1
+#endif
 template <class GT, int W, int MODE>
-__global__ void __launch_bounds__(INTERP_WARPS * 32) k_interp(int n, InterpArgs A) {
+__global__ void __launch_bounds__(INTERP_WARPS * 32, DP_INTERP_MINB) k_interp(int n, InterpArgs A) {
   constexpr int NREC = MODE ? 3 : 2;
   __shared__ double s_w[INTERP_WARPS][NREC][2 * DP_MAX_W + DP_MAX_NZ];   // per warp, per record: wx[8], wy[8], zeta[nz]
   __shared__ double s_zw[DP_MAX_NZ];
