@@ -264,6 +264,8 @@ __device__ __forceinline__ void cp_async16(double* smem_dst, const double* gmem_
   const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
 }
+__device__ __forceinline__ void cp_async_commit_only() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_only() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all_groups() { asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;" ::: "memory"); }
 
 struct SpreadArgs {
@@ -711,26 +713,43 @@ constexpr int INTERP_WARPS = DP_INTERP_WARPS;
 template <class GT, int W, int MODE>
 __global__ void __launch_bounds__(INTERP_WARPS * 32, DP_INTERP_MINB) k_interp(int n, InterpArgs A) {
   constexpr int NREC = MODE ? 3 : 2;
-  __shared__ double s_w[INTERP_WARPS][NREC][2 * DP_MAX_W + DP_MAX_NZ];   // per warp, per record: wx[8], wy[8], zeta[nz]
-  __shared__ double s_zw[DP_MAX_NZ];
+  // dynamic shared memory: quadrature weights [DP_MAX_NZ], then two sets of per-warp weight records [2][INTERP_WARPS][NREC][WR]: while a
+  // warp gathers for one particle, the records (and the footprint record, in registers) of its next particle are already on their way
+  extern __shared__ __align__(16) double interp_smem[];
+  double* s_zw = interp_smem;
   const GridGeom& g = A.g;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
   constexpr int w = W;
-  const int nz = g.nz, wrec = 2 * DP_MAX_W + nz;
+  const int nz = g.nz, wrec = 2 * DP_MAX_W + nz, WR = (wrec + 1) & ~1;
+  double* s_wb = interp_smem + DP_MAX_NZ;
   for (int i = threadIdx.x; i < nz; i += blockDim.x) s_zw[i] = A.zweights[i];
   __syncthreads();
   const int nk = A.Omega ? NREC : 1;
-  for (int p = blockIdx.x * INTERP_WARPS + wid; p < n; p += gridDim.x * INTERP_WARPS) {
-    const int4 m = A.meta[p];
-    const int dst = A.perm[p];
+  auto wbuf = [&](int b) { return s_wb + (size_t)((b * INTERP_WARPS + wid) * NREC) * WR; };
+  auto prefetch = [&](int b, int pp) {
+    double* d = wbuf(b);
+    for (int k = 0; k < nk; ++k) {
+      const double* rec = A.wrec + ((size_t)k * A.cap + pp) * wrec;
+      for (int e = lane; e < wrec; e += 32) cp_async8(d + k * WR + e, rec + e);
+    }
+    cp_async_commit_only();
+  };
+  const int stride = gridDim.x * INTERP_WARPS;
+  int p = blockIdx.x * INTERP_WARPS + wid, cur = 0;
+  int4 m = make_int4(0, 0, 1, 0);
+  int dst = 0;
+  if (p < n) { m = A.meta[p]; dst = A.perm[p]; prefetch(0, p); }
+  for (; p < n; p += stride) {
+    const int pn = p + stride;
+    int4 mn = make_int4(0, 0, 1, 0);
+    int dstn = 0;
+    if (pn < n) { mn = A.meta[pn]; dstn = A.perm[pn]; }
+    cp_async_wait_only();
+    __syncwarp();                                  // this particle's records are in buffer cur; every lane is done with the other buffer
+    if (pn < n) prefetch(cur ^ 1, pn);
+    const double* swb = wbuf(cur);
     GT s[6] = {0, 0, 0, 0, 0, 0};
     if (m.z <= m.w) {
-      __syncwarp();
-      for (int k = 0; k < nk; ++k) {
-        const double* rec = A.wrec + ((size_t)k * A.cap + p) * wrec;
-        for (int e = lane; e < wrec; e += 32) s_w[wid][k][e] = rec[e];
-      }
-      __syncwarp();
       constexpr int ww = w * w;
       const int nent = (m.w - m.z + 1) * ww;
 #pragma unroll 4
@@ -742,7 +761,7 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32, DP_INTERP_MINB) k_interp(in
         const GT wl = (GT)s_zw[l];
         if (MODE == 0) {
           for (int k = 0; k < nk; ++k) {
-            const double* sw = s_w[wid][k];
+            const double* sw = swb + k * WR;
             const GT wgt = (GT)sw[a] * (GT)sw[DP_MAX_W + b] * (GT)sw[2 * DP_MAX_W + l];
             const GT* gp = reinterpret_cast<const GT*>(A.grid) + (size_t)(3 * k) * A.real_field + off;
             s[3 * k + 0] += __ldg(gp) * wgt * wl;
@@ -752,11 +771,11 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32, DP_INTERP_MINB) k_interp(in
         } else {
           const GT* gp = reinterpret_cast<const GT*>(A.grid) + off;
           const GT u = __ldg(gp) * wl, v = __ldg(gp + A.real_field) * wl, ww2 = __ldg(gp + 2 * A.real_field) * wl;
-          const double* wM = s_w[wid][0];
+          const double* wM = swb;
           const GT wgt = (GT)wM[a] * (GT)wM[DP_MAX_W + b] * (GT)wM[2 * DP_MAX_W + l];
           s[0] += u * wgt; s[1] += v * wgt; s[2] += ww2 * wgt;
           if (nk > 1) {
-            const double* wD = s_w[wid][MODE ? 1 : 0]; const double* wG = s_w[wid][MODE ? 2 : 0];
+            const double* wD = swb + (MODE ? 1 : 0) * WR; const double* wG = swb + (MODE ? 2 : 0) * WR;
             const GT zD = (GT)wD[2 * DP_MAX_W + l];
             const GT Gx = (GT)wG[a] * (GT)wD[DP_MAX_W + b] * zD, Gy = (GT)wD[a] * (GT)wG[DP_MAX_W + b] * zD;
             const GT Gz = (GT)wD[a] * (GT)wD[DP_MAX_W + b] * (GT)wG[2 * DP_MAX_W + l];
@@ -772,7 +791,7 @@ __global__ void __launch_bounds__(INTERP_WARPS * 32, DP_INTERP_MINB) k_interp(in
       for (int o = 16; o > 0; o >>= 1) s[c] += __shfl_xor_sync(0xffffffffu, s[c], o);
     if (lane < 3) A.U[3 * (size_t)dst + lane] = (double)(lane == 0 ? s[0] : (lane == 1 ? s[1] : s[2]));
     if (A.Omega && lane >= 3 && lane < 6) A.Omega[3 * (size_t)dst + lane - 3] = (double)(lane == 3 ? s[3] : (lane == 4 ? s[4] : s[5]));
-    __syncwarp();
+    m = mn; dst = dstn; cur ^= 1;
   }
 }
 
@@ -880,15 +899,23 @@ cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaSt
   if (blocks > maxb) blocks = maxb;
   if (blocks < 1) blocks = 1;
   const bool f32 = P->p.transfer_fp32 != 0, kt = P->kernel_torque;
+  const int wr_even = (2 * DP_MAX_W + P->p.nz + 1) & ~1;
+  const size_t ismem = sizeof(double) * (DP_MAX_NZ + (size_t)2 * INTERP_WARPS * (kt ? 3 : 2) * wr_even);
+  cudaError_t ie = cudaSuccess;
+#define DP_INTERP_LAUNCH(GT, WW, MODE)                                                                                           \
+  { ie = cudaFuncSetAttribute(k_interp<GT, WW, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ismem);                  \
+    if (ie != cudaSuccess) return ie;                                                                                            \
+    k_interp<GT, WW, MODE><<<blocks, INTERP_WARPS * 32, ismem, st>>>(n, A); }
 #define DP_INTERP_CASE(WW)                                                              \
   case WW:                                                                              \
-    if (kt) { if (f32) k_interp<float, WW, 1><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A); else k_interp<double, WW, 1><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A); } \
-    else    { if (f32) k_interp<float, WW, 0><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A); else k_interp<double, WW, 0><<<blocks, INTERP_WARPS * 32, 0, st>>>(n, A); } \
+    if (kt) { if (f32) DP_INTERP_LAUNCH(float, WW, 1) else DP_INTERP_LAUNCH(double, WW, 1) } \
+    else    { if (f32) DP_INTERP_LAUNCH(float, WW, 0) else DP_INTERP_LAUNCH(double, WW, 0) } \
     break;
   switch (P->p.w) {
     DP_INTERP_CASE(4) DP_INTERP_CASE(5) DP_INTERP_CASE(6) DP_INTERP_CASE(7) DP_INTERP_CASE(8)
     default: return cudaErrorInvalidValue;
   }
 #undef DP_INTERP_CASE
+#undef DP_INTERP_LAUNCH
   return cudaGetLastError();
 }
