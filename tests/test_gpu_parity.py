@@ -194,6 +194,30 @@ def test_edge_cases(dp):
         assert rel_l2(U1.cpu().numpy(), U2.cpu().numpy()) < 1e-13
 
 
+@pytest.mark.parametrize("mode", ["fourier", "kernel", "forces"])
+def test_clustered_particles_take_both_spreading_paths(dp, mode):
+    """Spreading runs per-tile survivor lists through a pipelined kernel and leaves tiles whose list does not fit a staged chunk (20 particles
+    with kernel-derivative torques, 40 otherwise) to the culling kernel: a cluster of 300 particles inside a 6 x 6 patch (every tile it
+    touches overflows, hundreds of survivors per tile = several chunks) plus a dilute background (lists of 0..5) exercises both, and the
+    interpolation of many particles from the same columns.  Result against the oracle."""
+    import dataclasses
+    prob, pos, F, T = workloads.random_slit(n=700, L=40.0, nxy=60, nz=24, H=8.0, seed=4242, name="cluster")
+    rng = np.random.default_rng(4243)
+    pos = pos.copy()
+    pos[:300, 0] = 11.0 + 6.0 * rng.random(300)
+    pos[:300, 1] = 23.0 + 6.0 * rng.random(300)
+    if mode == "forces":
+        prob = dataclasses.replace(prob, has_torque=False); T = None
+    tm = 1 if mode == "kernel" else 0
+    U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", torque_mode="kernel" if tm else "fourier")
+    with dp.Plan(prob, max_particles=len(pos), use_torques=T is not None, torque_mode=tm) as plan:
+        U, Om = plan.mobility_apply(*to_dev(pos, F, T))
+        assert plan.check() == 0
+    assert rel_l2(U.cpu().numpy(), U_o) < TOL and rel_max(U.cpu().numpy(), U_o) < TOL_MAX
+    if T is not None:
+        assert rel_l2(Om.cpu().numpy(), Om_o) < TOL and rel_max(Om.cpu().numpy(), Om_o) < TOL_MAX
+
+
 def test_host_entry_point_matches_device_entry_point(dp):
     prob, pos, F, T = workloads.random_slit(n=500, L=32.0, nxy=48, nz=32, H=8.0, seed=12, name="host")
     with dp.Plan(prob, max_particles=len(pos)) as plan:
