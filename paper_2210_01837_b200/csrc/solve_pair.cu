@@ -266,7 +266,7 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
     for (int j = 0; j < NH; ++j) f[c][j] = 0.0;
   // a rolled loop over the input index l (the accumulators f are indexed statically): ~75 instructions that stay in the L0
   // instruction cache instead of 1500 fetched once
-#pragma unroll 1
+#pragma unroll 2
   for (int l = 0; l < NH; ++l) {
     double x[3];
     const bool alone = (N - l == l);                     // the middle node of an odd nz
@@ -392,7 +392,7 @@ __device__ __forceinline__ void pair_body(const PairArgs<NZ>& PA, double* smem, 
   // rolled over the OUTPUT index l, two at a time (six independent sums); the coefficients stay in registers
   {
     constexpr int LE = NH & ~1;
-#pragma unroll 1
+#pragma unroll 2
     for (int l = 0; l < LE; l += 2) {
       const double2* t0 = reinterpret_cast<const double2*>(&T.S[PAR][l][0]);
       const double2* t1 = reinterpret_cast<const double2*>(&T.S[PAR][l + 1][0]);
