@@ -5,21 +5,25 @@
 //   0..nz-3 of (D^2 - k^2) y = r plus the two Dirichlet-to-Neumann rows, solved in Greengard's integration form as two parity-decoupled
 //   tridiagonal chains with one border unknown each.
 //
-// B200 mapping: the fp64 pipe bounds this kernel (≈ 9 k DFMA per mode against 23.7 GB of traffic), so everything is arranged for it
-// to issue DFMAs and nothing else:
-//  * one CTA = 16 consecutive modes of one spectrum row = TWO warps; a lane is (mode, re/im); warp 0 owns the EVEN Chebyshev
+// B200 mapping: the fp64 pipe bounds this kernel (8.3 k algorithmic FMAs per mode against 18.8 GB of traffic at cfg 5), so everything
+// is arranged for it to issue fp64 instructions and little else:
+//  * a warp PAIR owns 16 consecutive modes of one spectrum row; a lane is (mode, re/im); warp 0 of the pair owns the EVEN Chebyshev
 //    coefficients of every column, warp 1 the ODD ones.  With the fold cos(n (N-l) pi/N) = (-1)^n cos(n l pi/N) the transforms, the
 //    chain factorisation and the four BVPs split exactly along that line, so each warp keeps its half of f_x, f_y, f_z (then p, then
 //    u, v, w) in REGISTERS from the analysis to the synthesis;
 //  * the transforms are 16 x 16 (nz = 32) matrix-vector products per lane whose matrix entries are the same for all lanes of a warp:
-//    they come straight from the constant bank (the tables travel as a __grid_constant__ kernel parameter), one DFMA per entry, no
-//    shared-memory traffic, sixteen independent accumulators;
+//    the tables travel as a __grid_constant__ kernel parameter and are read into uniform registers (LDCU; sm_100a has no constant-bank
+//    operand on DFMA), each entry feeding the DFMAs of all three fields; the loops over the input (analysis) and output (synthesis)
+//    index are ROLLED (unrolled by two): ~150 instructions that stay in the L0 instruction cache;
 //  * the two parities meet in five places only — d/dz of f_z for the pressure right-hand side, d/dz of p for the w right-hand side, the
 //    end-point sums (p(0), p(H), u_DP on the walls), and the un-fold g_l = E_l + O_l, g_{N-l} = E_l - O_l after the synthesis — each a
-//    few rows handed over through shared memory behind a 64-thread named barrier;
+//    few rows handed over through shared memory behind a barrier;
 //  * the nodal columns come in by cp.async (16 bytes per (mode, re/im) pair) while the warps factor their chains; the correction is
-//    added at the nodes (analysis and synthesis are exact inverses of one another, so this equals adding its coefficients).
-// Six CTAs (12 warps) per SM at nz = 32; no CTA-wide phase structure: CTAs drift apart and cover each other's loads and barriers.
+//    added at the nodes (analysis and synthesis are exact inverses of one another, so this equals adding its coefficients);
+//  * one CTA = six pairs (12 warps, one CTA per SM at nz = 32) that step through the phases behind CTA-wide barriers: the chain sweeps
+//    are ~3 k straight-line instructions per warp, executed once per 16 modes, and an SM cannot fetch that much code for warps that
+//    are at different places in it (profiles/r2_b_fetch_microbenchmarks.md) — in step, the six warps of a parity share one fetch
+//    stream; reciprocals and exponentials are branch-free for the same reason (no BSSY / BSYNC around library slow paths).
 #include <cmath>
 #include <cstring>
 #include <vector>
@@ -64,10 +68,8 @@ template <int NZ> struct PairSmem {
   static constexpr int GPQ = IBG + 2 * TM;                // [2][2][TM] sums of b_m and of c_n of the unit border solution (even / odd chain)
   static constexpr int SUM = GPQ + 4 * TM;                // [2][8][32] sums handed over: S_c of p, u, v, w and S_b of u, v per parity
   static constexpr int DOUBLES = SUM + 2 * 8 * ROW;
-  // pairs per CTA and CTAs per SM.  Every warp runs ~9 k straight-line instructions per 16 modes, far more than the instruction
-  // caches hold, and an SM fetches only ~20 bytes of code per clock from L2: the warps of one parity must therefore run the SAME
-  // stretch of code at the same time.  A CTA is NPAIR pairs stepping through the phases behind CTA-wide barriers; two CTAs per SM
-  // cover each other's loads and barrier waits.
+  // pairs per CTA and CTAs per SM: one CTA of six pairs (measured: two CTAs of three pairs 12.6 ms, three of two 11.9 ms, one of six
+  // 10.9 ms at cfg 5 — the warps of one parity must run the SAME stretch of straight-line code at the same time, see the header)
   static constexpr int PAIRS_SM = (227 * 1024 - 2048) / (DOUBLES * 8);       // pairs whose shared memory fits one SM
 #ifndef DP_PAIR_CTAS
 #define DP_PAIR_CTAS 1
