@@ -15,8 +15,12 @@
 #define DP_MAX_W 8
 
 // xy tile of the spread kernel (grid columns per CTA); particles are binned by the tile of their footprint origin.
+#ifndef DP_TILE_X
 #define DP_TILE_X 16
+#endif
+#ifndef DP_TILE_Y
 #define DP_TILE_Y 4
+#endif
 
 // modes per CTA in the solve kernel (consecutive modes of one row of the half spectrum); a lane is (mode, re/im)
 #define DP_SOLVE_TM 16

@@ -19,12 +19,22 @@
 namespace {
 
 constexpr int TX = DP_TILE_X, TY = DP_TILE_Y;
-constexpr int ZSPLIT = 4;                       // z residue classes per column
-constexpr int SPREAD_THREADS = TX * TY * ZSPLIT;
-constexpr int PCH = 40;                         // candidate particles staged per chunk
+// z residue classes per grid column = threads per column of the spread kernels, by compiled nz: with the pipelined kernel hiding the global
+// latency, ONE thread per column (all of its planes in registers: no per-column set-up repeated by several threads) is fastest up to nz = 32
+// (measured at cfg 5: 4.7 ms against 5.0 with two and 6.0 with four); larger nz need two to keep the accumulators in registers.
+// ZSPLIT / SPREAD_THREADS are usable wherever a template parameter (or macro argument) NZ is in scope.
+#ifndef DP_ZSPLIT_OF
+#define DP_ZSPLIT_OF(NZ) ((NZ) <= 32 ? 1 : 2)
+#endif
+#define ZSPLIT (DP_ZSPLIT_OF(NZ))
+#define SPREAD_THREADS (TX * TY * ZSPLIT)
+#ifndef DP_PCH
+#define DP_PCH 40
+#endif
+constexpr int PCH = DP_PCH;                     // candidate particles staged per chunk
 constexpr int MAXB = 6;                         // origin bins per direction that can reach a tile (w <= 8, TY = 4)
 constexpr int MAXR = 2 * MAXB;                  // candidate ranges per tile: one per bin row, two when the x range wraps
-constexpr int MAXKEEP = SPREAD_THREADS;         // survivors of one block of candidates
+#define MAXKEEP SPREAD_THREADS                  // survivors of one block of candidates
 
 struct GridGeom {
   int nx, ny, nz, w, wall_mode, nbx, nby;
@@ -294,7 +304,7 @@ struct SpreadArgs {
 //         which the solve kernel takes in Fourier-Chebyshev space);
 // MODE 1 (kernel-derivative torques): ONE triple f = sum_j [F_j S_M(j; g) + (1/2) G_j(g) x tau_j], three records per candidate.
 #ifndef DP_SPREAD_MINB
-#define DP_SPREAD_MINB (NZ <= 32 ? 3 : 2)
+#define DP_SPREAD_MINB (NZ <= 32 ? 4 : 2)
 #endif
 // staged candidates of one chunk: weight records (zero padded to whole z residue classes), values, footprint records
 template <int NZ, int MODE> struct SpreadBuf {
@@ -859,9 +869,10 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
                                                                                     P->d_ov_tiles, P->d_ov_count);
   int sms = 148;
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->p.device);
-#define DP_SPREAD_LAUNCH(NZ, GT, MODE)                                                                                                   \
+#define DP_SPREAD_LAUNCH(NZV, GT, MODE)                                                                                                   \
   {                                                                                                                                      \
-    const int per_sm = (NZ <= 32 ? 3 : 2);                                                                                               \
+    constexpr int NZ = NZV;                                                                                                              \
+    const int per_sm = DP_SPREAD_MINB;                                                                                                   \
     const size_t smem = 2 * sizeof(SpreadBuf<NZ, MODE>) + 3 * (LMAX + 1) * sizeof(int);                                                  \
     e = cudaFuncSetAttribute(k_spread_pipe<NZ, GT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                       \
     if (e != cudaSuccess) return e;                                                                                                      \
