@@ -42,7 +42,8 @@ extern "C" {
 typedef struct dp_plan dp_plan; /* opaque: owns grids, FFT tables (or cuFFT plans), solver tables, workspace */
 
 enum { DP_BOTTOM_WALL = 0, DP_SLIT = 1 };
-enum { DP_OK = 0, DP_EINVAL = -1, DP_ENOMEM = -2, DP_ECUDA = -3, DP_ECUFFT = -4, DP_EDOMAIN = -5 };
+enum { DP_OK = 0, DP_EINVAL = -1, DP_ENOMEM = -2, DP_ECUDA = -3, DP_ECUFFT = -4, DP_EDOMAIN = -5,
+       DP_ETOOBIG = -6 /* problem larger than the fixed work array of dp_bin_particles_static */ };
 
 /* Problem statement of the paper: box doubly periodic in xy with wall(s), ES kernel (w, beta) per envelope
  * (eqs 53-54), viscosity.  The first block of fields is SURVEY.md §8(b)'s struct; the second block
@@ -125,6 +126,39 @@ int dp_mobility_apply_host(dp_plan* plan, int n, const double* pos, const double
  * allocates (max_iter + 2) work vectors for the duration of the call. */
 int dp_lanczos_sqrt(dp_plan* plan, int n, const double* pos, const double* W_force, const double* W_torque, double* g_U,
                     double* g_Omega, double tol, int max_iter, int* iters, double* eps_hist, void* cuda_stream);
+
+/* Particle binning (step a0 of the product: the counting sort by xy tile that spreading and interpolation rely on; the build's
+ * own step, it is how step 1, reaches the grid without global atomics) for callers that MUST NOT ALLOCATE device
+ * memory while they run.  Who that is: code living inside a host application that took all of HBM for its own memory pool when
+ * it started, so that a later cudaMalloc fails or fragments the pool; a plug-in or a latency-bound loop whose host forbids driver
+ * allocations after initialisation, because cudaMalloc / cudaFree may synchronise the whole device; a worker that is only ever
+ * handed buffers.  dp_create gives a plan its work arrays with cudaMalloc; this entry point needs no plan and calls neither
+ * cudaMalloc, cudaFree nor any library routine that allocates: the work arrays of the sort (tile and rank of every particle, tile
+ * counters, scan totals; 2.5 MiB) are a fixed array inside libdpstokes.so itself, which every GPU that loads the library holds
+ * until the process exits.
+ *   prm         box and grid: wall_mode, Lx, Ly, H, nx, ny, w and device are used (checked as dp_create checks them), the rest ignored
+ *   pos         [n][3]  DEVICE, positions (x, y wrapped periodically; a particle outside the domain in z is filed under tile 0,
+ *                       as the product does before it skips it)
+ *   perm        [n]     DEVICE, out: particle indices ordered by tile; the order of the particles WITHIN one tile is not fixed
+ *                       (it comes from atomic counters) and may differ from call to call
+ *   tile_start  [T+1]   DEVICE, out: perm[tile_start[t] .. tile_start[t+1]-1] are the particles whose w x w footprint has its
+ *                       first node in tile t = ty * ceil(nx / DP_BIN_TILE_X) + tx;  T = ceil(nx/DP_BIN_TILE_X) * ceil(ny/DP_BIN_TILE_Y)
+ * Limits: n <= DP_STATIC_BIN_MAX_PARTICLES and T <= DP_STATIC_BIN_MAX_TILES, else DP_ETOOBIG and nothing is launched (configs 1-4
+ * fit; config 5 does not: use a plan).  Asynchronous on `cuda_stream`; inputs are read-only, outputs fully overwritten.
+ * Set-up: the FIRST call on each device looks up the device address of the fixed array (cudaGetSymbolAddress, with that device
+ * current) and keeps it; make that first call during your own initialisation, before any stream capture is begun.
+ * Sharing: every call on a device uses the same array, which still holds the previous call's contents — the entry point clears the
+ * parts that must start at zero itself (on the stream), so back-to-back calls on ONE stream are fine, but two calls that can run at
+ * the same time on the GPU (different streams, different host threads) race on it and give garbage: serialise them. */
+#define DP_BIN_TILE_X 16
+#define DP_BIN_TILE_Y 4
+#define DP_STATIC_BIN_MAX_PARTICLES 262144
+#define DP_STATIC_BIN_MAX_TILES 131072
+int dp_bin_particles_static(const dp_params* prm, int n, const double* pos, int* perm, int* tile_start, void* cuda_stream);
+
+/* Test hook: the same two arrays as the LAST product of `plan` left them in the plan's own work arrays (HOST pointers; perm [n],
+ * tile_start [T+1]; synchronises the last stream).  n must be the particle count of that product. */
+int dp_copy_bins_to_host(dp_plan* plan, int n, int* perm, int* tile_start);
 
 /* Domain check of the last product: "kernels must never extend outside open boundaries" (footnote 44) and
  * 0 <= z <= H.  Synchronises the last stream used; DP_EDOMAIN if any particle of the last apply was out of domain. */

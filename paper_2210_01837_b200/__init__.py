@@ -4,8 +4,8 @@ Every step of the path runs in the CUDA library (``csrc/`` -> ``libdpstokes.so``
 this package only marshals arguments.  PyTorch is used for device memory and streams, nothing else.
 There is no CPU fallback: if the library is missing or no CUDA device is present, calls fail loudly.
 """
-from .binding import (BOTTOM_WALL, SLIT, DPError, Plan, es_dphi_cut, es_norm, exported_symbols, library_path, load_library,
+from .binding import (BOTTOM_WALL, SLIT, DPError, Plan, bin_particles_static, es_dphi_cut, es_norm, exported_symbols, library_path, load_library,
                       supported_nz)
 
-__all__ = ["BOTTOM_WALL", "SLIT", "DPError", "Plan", "es_dphi_cut", "es_norm", "exported_symbols", "library_path", "load_library",
+__all__ = ["BOTTOM_WALL", "SLIT", "DPError", "Plan", "bin_particles_static", "es_dphi_cut", "es_norm", "exported_symbols", "library_path", "load_library",
            "supported_nz"]

@@ -13,7 +13,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIBNAME = os.path.join(_HERE, "libdpstokes.so")
 
 # every symbol include/dp.h declares
-EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_lanczos_sqrt", "dp_check", "dp_effective_radius", "dp_set_profiling", "dp_stage_ms", "dp_fft_pass_ms",
+EXPORTS = ["dp_create", "dp_mobility_apply", "dp_mobility_apply_host", "dp_lanczos_sqrt", "dp_bin_particles_static", "dp_copy_bins_to_host", "dp_check", "dp_effective_radius", "dp_set_profiling", "dp_stage_ms", "dp_fft_pass_ms",
            "dp_debug_run_stage", "dp_buffer_bytes", "dp_copy_buffer_to_host", "dp_copy_plane_to_host", "dp_complex_row_pitch", "dp_zero_planes", "dp_fft_backend", "dp_solve_kernel", "dp_es_norm", "dp_es_radius_over_h",
            "dp_es_dphi_cut", "dp_supported_nz", "dp_device_bytes", "dp_strerror", "dp_last_error", "dp_destroy"]
 
@@ -58,6 +58,10 @@ def load_library():
     L.dp_mobility_apply_host.restype = i
     L.dp_lanczos_sqrt.argtypes = [vp, i, vp, vp, vp, vp, vp, d, i, ctypes.POINTER(i), ctypes.POINTER(d), vp]
     L.dp_lanczos_sqrt.restype = i
+    L.dp_bin_particles_static.argtypes = [ctypes.POINTER(dp_params), i, vp, vp, vp, vp]
+    L.dp_bin_particles_static.restype = i
+    L.dp_copy_bins_to_host.argtypes = [vp, i, vp, vp]
+    L.dp_copy_bins_to_host.restype = i
     L.dp_check.argtypes = [vp]
     L.dp_check.restype = i
     L.dp_set_profiling.argtypes = [vp, i]
@@ -121,6 +125,38 @@ def supported_nz():
     buf = (ctypes.c_int * 16)()
     n = load_library().dp_supported_nz(buf, 16)
     return [int(buf[k]) for k in range(n)]
+
+
+BIN_TILE_X, BIN_TILE_Y = 16, 4                                      # DP_BIN_TILE_X, DP_BIN_TILE_Y
+STATIC_BIN_MAX_PARTICLES, STATIC_BIN_MAX_TILES = 262144, 131072     # DP_STATIC_BIN_MAX_PARTICLES, DP_STATIC_BIN_MAX_TILES
+ETOOBIG = -6
+
+
+def bin_particles_static(params: dp_params, pos, perm=None, tile_start=None, stream=None):
+    """dp_bin_particles_static: the product's counting sort of the particles by xy tile for callers that may not allocate device
+    memory (see include/dp.h: its work arrays are a fixed array inside the library, at most 262,144 particles and 131,072 tiles).
+    ``pos`` float64 CUDA tensor [n,3]; ``perm`` [n] and ``tile_start`` [tiles+1] int32 CUDA tensors are the caller's outputs (made
+    here with torch only when not given — pass your own if you cannot allocate).  Asynchronous on ``stream``.  Calls that overlap on
+    the GPU race on the shared array; the first call on a device should come before any stream capture."""
+    import torch
+    n = int(pos.shape[0])
+    if not (pos.is_cuda and pos.dtype == torch.float64 and pos.is_contiguous() and tuple(pos.shape) == (n, 3)):
+        raise DPError("pos must be a contiguous float64 CUDA tensor of shape [n,3]")
+    tiles = -(-int(params.nx) // BIN_TILE_X) * -(-int(params.ny) // BIN_TILE_Y)
+    if perm is None:
+        perm = torch.empty((n,), dtype=torch.int32, device=pos.device)
+    if tile_start is None:
+        tile_start = torch.empty((tiles + 1,), dtype=torch.int32, device=pos.device)
+    for t, m in ((perm, n), (tile_start, tiles + 1)):
+        if not (t.is_cuda and t.dtype == torch.int32 and t.is_contiguous() and t.numel() == m):
+            raise DPError("perm / tile_start must be contiguous int32 CUDA tensors of n resp. tiles + 1 elements")
+    st = stream if stream is not None else torch.cuda.current_stream(pos.device)
+    L = load_library()
+    rc = L.dp_bin_particles_static(ctypes.byref(params), n, ctypes.c_void_p(pos.data_ptr()), ctypes.c_void_p(perm.data_ptr()),
+                                   ctypes.c_void_p(tile_start.data_ptr()), ctypes.c_void_p(st.cuda_stream))
+    if rc != 0:
+        raise DPError("dp_bin_particles_static failed: %s (%d)" % (L.dp_strerror(rc).decode(), rc))
+    return perm, tile_start
 
 
 STAGE_NAMES = ["bin", "spread", "fft_fwd", "solve", "fft_inv", "interp", "k0", "total"]
@@ -245,6 +281,15 @@ class Plan:
         buf = (ctypes.c_float * 4)()
         self._ck(load_library().dp_fft_pass_ms(self._h, buf), "dp_fft_pass_ms")
         return {k: float(buf[i]) for i, k in enumerate(("fft_x_fwd", "fft_y_fwd", "fft_y_inv", "fft_x_inv"))}
+
+    def copy_bins(self, n: int):
+        """Test hook (dp_copy_bins_to_host): (perm [n], tile_start [tiles+1]) of the last product's own sort, as numpy int32."""
+        p = self.params
+        tiles = -(-int(p.nx) // BIN_TILE_X) * -(-int(p.ny) // BIN_TILE_Y)
+        perm, start = np.empty((n,), dtype=np.int32), np.empty((tiles + 1,), dtype=np.int32)
+        self._ck(load_library().dp_copy_bins_to_host(self._h, int(n), perm.ctypes.data_as(ctypes.c_void_p), start.ctypes.data_as(ctypes.c_void_p)),
+                 "dp_copy_bins_to_host")
+        return perm, start
 
     def zero_planes(self) -> int:
         return int(load_library().dp_zero_planes(self._h))

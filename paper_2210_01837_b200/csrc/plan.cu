@@ -302,6 +302,7 @@ const char* dp_strerror(int code) {
     case DP_ECUDA: return "CUDA error";
     case DP_ECUFFT: return "cuFFT error";
     case DP_EDOMAIN: return "particle outside the domain";
+    case DP_ETOOBIG: return "problem larger than the fixed work array (dp_bin_particles_static: use a plan)";
     default: return "unknown error";
   }
 }
@@ -515,6 +516,16 @@ size_t dp_buffer_bytes(const dp_plan* P, int which) {
 
 int dp_fft_backend(const dp_plan* P) { return P ? (P->own_fft ? 0 : 1) : -1; }
 int dp_solve_kernel(const dp_plan* P) { return P ? ((P->solve_pair_tab && !P->solve_force_tile) ? 0 : 1) : -1; }
+
+// ---- the sort of the last product (test hook: what dp_bin_particles_static is compared with)
+int dp_copy_bins_to_host(dp_plan* P, int n, int* perm, int* tile_start) {
+  if (!P || !tile_start || n < 0 || n > P->p.max_particles || (n > 0 && !perm)) return DP_EINVAL;
+  DeviceGuard guard(P->p.device);
+  CK(cudaStreamSynchronize(P->last_stream));
+  if (n > 0) CK(cudaMemcpy(perm, P->d_perm, sizeof(int) * (size_t)n, cudaMemcpyDeviceToHost));
+  CK(cudaMemcpy(tile_start, P->d_bin_start, sizeof(int) * ((size_t)P->nbins + 1), cudaMemcpyDeviceToHost));
+  return DP_OK;
+}
 
 int dp_zero_planes(dp_plan* P) {
   if (!P) return DP_EINVAL;

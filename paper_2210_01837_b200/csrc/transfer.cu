@@ -930,3 +930,88 @@ cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaSt
 #undef DP_INTERP_LAUNCH
   return cudaGetLastError();
 }
+
+// ---------------------------------------------------------------------------------------------- binning with no allocation (dp_bin_particles_static)
+#include <mutex>
+// Step a0 for callers that must not allocate device memory: code running inside a framework that reserved all of HBM for its own pool at start-up,
+// a plug-in whose host forbids driver allocations after initialisation (each one may synchronise the device, and the hot loop must not stall or
+// fail with "out of memory" half way), or a worker that only ever gets buffers handed to it.  The product path keeps the work arrays of its
+// counting sort in the plan (cudaMalloc in dp_create); here the same kernels run on a fixed array that is part of the loaded library image.
+namespace {
+
+static_assert(DP_BIN_TILE_X == TX && DP_BIN_TILE_Y == TY, "dp.h states the tile of the sort");
+constexpr int SB_MAX_N = DP_STATIC_BIN_MAX_PARTICLES, SB_MAX_BINS = DP_STATIC_BIN_MAX_TILES;
+constexpr int SB_SCAN = SB_MAX_BINS / SCAN_CHUNK + 1;
+// layout (ints): tile of each particle [SB_MAX_N] | rank within its tile [SB_MAX_N] | tile counters [SB_MAX_BINS] | chunk totals of the scan [SB_SCAN] | flag [1]
+constexpr size_t SB_OFF_SLOT = SB_MAX_N, SB_OFF_COUNT = 2 * (size_t)SB_MAX_N, SB_OFF_SUMS = SB_OFF_COUNT + SB_MAX_BINS, SB_OFF_FLAG = SB_OFF_SUMS + SB_SCAN;
+constexpr size_t SB_INTS = SB_OFF_FLAG + 1;
+// 2.5 MiB that every GPU which loads libdpstokes.so holds until the process exits.  In host code this name is only a handle for
+// cudaGetSymbolAddress — it is NOT a device address and must never be passed to a kernel as it stands.
+static __device__ __align__(256) int g_static_bin_scratch[SB_INTS];
+
+constexpr int SB_MAX_DEVICES = 64;
+std::mutex g_sb_mutex;
+int* g_sb_addr[SB_MAX_DEVICES] = {};            // device address of g_static_bin_scratch on each device, resolved once per device
+
+// `dev` must be the current device: the symbol is looked up in the current device's copy of the module
+cudaError_t static_bin_scratch(int dev, int** out) {
+  std::lock_guard<std::mutex> lock(g_sb_mutex);
+  if (!g_sb_addr[dev]) {
+    void* a = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&a, g_static_bin_scratch);
+    if (e != cudaSuccess) return e;
+    g_sb_addr[dev] = static_cast<int*>(a);
+  }
+  *out = g_sb_addr[dev];
+  return cudaSuccess;
+}
+
+// the part of k_bin_scatter that a caller of the sort alone needs: sorted slot -> original particle index
+__global__ void k_bin_perm(int n, const int* __restrict__ bin_of, const int* __restrict__ slot_of, const int* __restrict__ bin_start, int* __restrict__ perm) {
+  const int p = blockIdx.x * blockDim.x + threadIdx.x;
+  if (p < n) perm[bin_start[bin_of[p]] + slot_of[p]] = p;
+}
+
+}  // namespace
+
+extern "C" int dp_bin_particles_static(const dp_params* prm, int n, const double* pos, int* perm, int* tile_start, void* cuda_stream) {
+  if (!prm || !tile_start || n < 0 || (n > 0 && (!pos || !perm))) return DP_EINVAL;
+  const dp_params& p = *prm;
+  // the geometry checks of dp_create that binning depends on
+  if (p.wall_mode != DP_BOTTOM_WALL && p.wall_mode != DP_SLIT) return DP_EINVAL;
+  if (!(p.Lx > 0) || !(p.Ly > 0) || !(p.H > 0) || p.w < 4 || p.w > DP_MAX_W) return DP_EINVAL;
+  if (p.nx < TX + p.w || p.ny < TY + p.w || (p.nx & 1) || (p.ny & 1)) return DP_EINVAL;
+  const double h = p.Lx / p.nx;
+  if (fabs(h - p.Ly / p.ny) > 1e-12 * h) return DP_EINVAL;
+  if (p.device < 0 || p.device >= SB_MAX_DEVICES) return DP_EINVAL;
+  GridGeom g;
+  g.nx = p.nx; g.ny = p.ny; g.nz = p.nz; g.w = p.w; g.wall_mode = p.wall_mode;
+  g.nbx = (p.nx + TX - 1) / TX; g.nby = (p.ny + TY - 1) / TY;
+  g.Lx = p.Lx; g.Ly = p.Ly; g.H = p.H; g.h = h; g.alpha = 0.5 * p.w * h;
+  const long long nbins_ll = (long long)g.nbx * g.nby;
+  if (n > SB_MAX_N || nbins_ll > SB_MAX_BINS) return DP_ETOOBIG;      // beyond the fixed work array: use a plan (dp_create) instead
+  const int nbins = (int)nbins_ll;
+
+  int prev = -1;
+  if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return DP_ECUDA; }
+  if (prev != p.device && cudaSetDevice(p.device) != cudaSuccess) { cudaGetLastError(); return DP_ECUDA; }
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int* S = nullptr;
+  cudaError_t e = static_bin_scratch(p.device, &S);
+  // The array still holds what the previous call left in it: the tile counters and the flag are the two parts that must start at zero
+  // (everything else is written before it is read).  A memset on the stream allocates nothing.
+  if (e == cudaSuccess) e = cudaMemsetAsync(S + SB_OFF_COUNT, 0, sizeof(int) * (size_t)nbins, st);
+  if (e == cudaSuccess) e = cudaMemsetAsync(S + SB_OFF_FLAG, 0, sizeof(int), st);
+  if (e == cudaSuccess) {
+    const int T = 256, B = (n + T - 1) / T;
+    if (n > 0) k_bin_count<<<B, T, 0, st>>>(n, pos, g, S, S + SB_OFF_SLOT, S + SB_OFF_COUNT, S + SB_OFF_FLAG);
+    const int nsb = (nbins + SCAN_CHUNK - 1) / SCAN_CHUNK;
+    k_scan_local<<<nsb, SCAN_THREADS, 0, st>>>(nbins, S + SB_OFF_COUNT, tile_start, S + SB_OFF_SUMS);
+    k_scan_add<<<nsb, SCAN_THREADS, 0, st>>>(nbins, nsb, tile_start, S + SB_OFF_SUMS);
+    if (n > 0) k_bin_perm<<<B, T, 0, st>>>(n, S, S + SB_OFF_SLOT, tile_start, perm);
+    e = cudaGetLastError();
+  }
+  if (prev != p.device) cudaSetDevice(prev);
+  if (e != cudaSuccess) { cudaGetLastError(); return DP_ECUDA; }
+  return DP_OK;
+}
