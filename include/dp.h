@@ -53,7 +53,8 @@ typedef struct {
   double Lx, Ly, H;     /* FULL periods in x, y (reading G1); top of the Chebyshev grid                       */
   int nx, ny, nz;       /* grid: uniform in x,y (h = Lx/nx = Ly/ny to 1e-12 relative; nx, ny even), nz type-2
                            Chebyshev nodes z_l = (H/2)(1+cos(l pi/(nz-1))) including both ends;
-                           8 <= nz <= 64 (dp_supported_nz lists the sizes with a compiled fast path)                     */
+                           only the sizes dp_supported_nz lists ({16, 19, 24, 26, 32, 40, 48, 64}: one compiled kernel set each)
+                           are accepted; any other nz is DP_EINVAL                                                       */
   int w;                /* ES kernel support in cells (paper's m), 4..8; alpha = w h/2                   */
   double beta_M;        /* ES beta of the monopole envelope Delta_M (eq 54; beta, not beta/w)                            */
   double beta_D;        /* ES beta of the dipole envelope Delta_D; ignored if torques/Omega are never used               */
@@ -123,7 +124,9 @@ int dp_mobility_apply_host(dp_plan* plan, int n, const double* pos, const double
  * PAPER.md:527) or max_iter (<= 64) products.  DEVICE pointers [n][3]: W_force required, W_torque or NULL (then the
  * translational block only: U = M^{tt} F); g_U required, g_Omega given iff W_torque is.  *iters receives the number of products,
  * eps_hist[0 .. *iters - 2] (HOST, may be NULL) receives eps_2, eps_3, ...  Synchronous (every iteration reads two scalars back);
- * allocates (max_iter + 2) work vectors for the duration of the call. */
+ * allocates (max_iter + 2) work vectors for the duration of the call.
+ * Needs n >= 1 (n == 0 is DP_EINVAL here, unlike dp_mobility_apply's no-op) and a LINEAR product: a plan with a non-zero uwall_0 / uwall_H
+ * (whose product is affine, U = M F + wall-driven flow) is refused with DP_EINVAL and a dp_last_error message. */
 int dp_lanczos_sqrt(dp_plan* plan, int n, const double* pos, const double* W_force, const double* W_torque, double* g_U,
                     double* g_Omega, double tol, int max_iter, int* iters, double* eps_hist, void* cuda_stream);
 

@@ -15,12 +15,8 @@
 #define DP_MAX_W 8
 
 // xy tile of the spread kernel (grid columns per CTA); particles are binned by the tile of their footprint origin.
-#ifndef DP_TILE_X
 #define DP_TILE_X 16
-#endif
-#ifndef DP_TILE_Y
 #define DP_TILE_Y 4
-#endif
 
 // modes per CTA in the solve kernel (consecutive modes of one row of the half spectrum); a lane is (mode, re/im)
 #define DP_SOLVE_TM 16
@@ -66,6 +62,8 @@ struct dp_plan {
   int* d_flag = nullptr;        // out-of-domain flag
   int* d_lmin = nullptr;        // lowest plane index touched by any footprint of the current apply (planes below it are zero)
   size_t device_bytes = 0;
+  int sm_count = 148;           // multiprocessors of the plan's device (queried once in dp_create): grid sizes of the persistent kernels
+  int smem_optin = 0;           // opt-in maximum of dynamic shared memory per CTA on the plan's device
 
   cufftHandle fft_fwd = 0, fft_inv = 0;
   bool fft_ok = false;
@@ -92,6 +90,7 @@ struct dp_plan {
 cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* force, const double* torque, bool dense, cudaStream_t st);
 cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torque, cudaStream_t st);
 cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaStream_t st);
+cudaError_t dp_transfer_setup(dp_plan* P);          // per plan, from dp_create: kernel attributes of the plan's spread / interpolation kernels
 cudaError_t dp_launch_solve(dp_plan* P, bool with_torque_field, bool want_omega, cudaStream_t st);
 cudaError_t dp_solve_upload_tables(dp_plan* P);      // per plan: constant tables, k = 0 cosine table, kernel attributes on the plan's device
 void dp_solve_destroy_tables(dp_plan* P);

@@ -31,32 +31,18 @@ namespace {
 
 using namespace dpfft;
 
-// slots per CTA and threads per slot of the x passes and of the y passes (tuning builds may override them)
-#ifndef DP_FFT_XSLOTS
+// slots per CTA and threads per slot of the x passes and of the y passes
 #define DP_FFT_XSLOTS 2
-#endif
-#ifndef DP_FFT_XTPS
 #define DP_FFT_XTPS 256
-#endif
-#ifndef DP_FFT_YSLOTS
 #define DP_FFT_YSLOTS 3
-#endif
-#ifndef DP_FFT_YTPS
 #define DP_FFT_YTPS 160
-#endif
-#ifndef DP_FFT_XTPS_FWD
 #define DP_FFT_XTPS_FWD 320
-#endif
 // the forward x pass runs best with 320 threads per slot (its loads are one contiguous row per slot: more lines in flight), the
 // inverse with 256 (its gather keeps 2 x 9 values per thread in registers at 256 threads; measured 4.7 / 5.1 ms and 6.4 / 5.5 ms at cfg 5)
 constexpr int XSLOTS = DP_FFT_XSLOTS, XTPS = DP_FFT_XTPS, XTHREADS = XSLOTS * XTPS;
 constexpr int XFTPS = DP_FFT_XTPS_FWD, XFTHREADS = XSLOTS * XFTPS;
-#ifndef DP_FFT_YSLOTS_FWD
 #define DP_FFT_YSLOTS_FWD 2
-#endif
-#ifndef DP_FFT_YTPS_FWD
 #define DP_FFT_YTPS_FWD 288
-#endif
 // the forward y pass (whose first stage loads its lines from global memory into registers) runs best with two slots of 288 threads:
 // every stage of a 4320-point row (270 / 240 / 288 lines) is then ONE round of its slot; measured 3.9 against 4.6 ms at cfg 5, while
 // the inverse (bulk-load prefetch, stores straight to global) loses with that shape (4.2 against 3.4 ms)
@@ -443,25 +429,6 @@ size_t smem_bytes_x(int M, int ntw, int rb) {
   return sizeof(double2) * ((size_t)ntw + (M / 2 + 1) + (size_t)XSLOTS * rb * M) + align16(sizeof(unsigned short) * M) + 8 * XSLOTS;
 }
 
-#ifdef DP_FFT_TUNING
-// tuning override: DP_FFT_FACTORS_X / DP_FFT_FACTORS_Y = comma-separated radices (product must equal the length)
-bool factors_from_env(const char* name, int n, Factors* F) {
-  const char* e = getenv(name);
-  if (!e || !*e) return false;
-  Factors G; G.n = n; G.ns = 0;
-  long prod = 1;
-  while (*e && G.ns < MAX_STAGES) {
-    char* end = nullptr;
-    const long r = strtol(e, &end, 10);
-    if (end == e || !radix_supported((int)r)) return false;
-    G.r[G.ns++] = (int)r; prod *= r;
-    e = (*end == ',') ? end + 1 : end;
-  }
-  if (prod != n || *e) return false;
-  *F = G;
-  return true;
-}
-#endif
 
 }  // namespace
 
@@ -490,10 +457,6 @@ cudaError_t dp_fft_own_create(dp_plan* P) {
   dp_fft_own* O = new dp_fft_own();
   P->fft_own = O;
   if (!factorize(M, &O->Fx) || !factorize(ny, &O->Fy)) return cudaErrorInvalidValue;
-#ifdef DP_FFT_TUNING              // tuning builds only: override the factorisation from the environment
-  factors_from_env("DP_FFT_FACTORS_X", M, &O->Fx);
-  factors_from_env("DP_FFT_FACTORS_Y", ny, &O->Fy);
-#endif
   // rows per slot batch: as many as fit the slot; in the x passes the batch must tile a plane's ny rows
   O->rby = SLOT_ELEMS / ny < 1 ? 1 : SLOT_ELEMS / ny;
   int rbmax = SLOT_ELEMS / M;                // <= 2 rows at nx = 4320: a batch is rb * nx doubles = rb * M complex
@@ -523,10 +486,16 @@ cudaError_t dp_fft_own_create(dp_plan* P) {
   if (O->smem_x > 227 * 1024 || O->smem_y > 227 * 1024) return cudaErrorInvalidValue;
   O->ky_fwd = pick_y(O->Fy, false); O->ky_inv = pick_y(O->Fy, true);
   O->kx_fwd = pick_x(O->Fx, false, O->rbx, P->p.transfer_fp32 != 0); O->kx_inv = pick_x(O->Fx, true, O->rbx, P->p.transfer_fp32 != 0);
-  if ((e = cudaFuncSetAttribute(O->ky_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y_fwd)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(O->ky_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_y)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(O->kx_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;
-  if ((e = cudaFuncSetAttribute(O->kx_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)O->smem_x)) != cudaSuccess) return e;
+  // The limit is a property of the FUNCTION on this device, not of the plan, and plans of different grid sizes share the general kernels
+  // k_fft_*<0,0,0>: every plan raises it to the device's opt-in maximum, so a plan created later with a smaller grid cannot lower it under
+  // a live plan that needs more (the size a launch actually asks for is what decides the shared-memory carve-out).
+  int smem_optin = 0;
+  if ((e = cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, P->p.device)) != cudaSuccess) return e;
+  if ((size_t)smem_optin < O->smem_x || (size_t)smem_optin < O->smem_y) return cudaErrorInvalidValue;
+  if ((e = cudaFuncSetAttribute(O->ky_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(O->ky_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(O->kx_fwd, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
+  if ((e = cudaFuncSetAttribute(O->kx_inv, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_optin)) != cudaSuccess) return e;
   int sms = 0;
   if ((e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->p.device)) != cudaSuccess) return e;
   O->grid = sms > 0 ? sms : 148;

@@ -125,6 +125,11 @@ extern "C" int dp_lanczos_sqrt(dp_plan* P, int n, const double* pos, const doubl
   if (!P || n < 1 || n > P->p.max_particles || !pos || !W_force || !g_U || !(tol > 0) || max_iter < 1 || max_iter > 64) return DP_EINVAL;
   if ((W_torque != nullptr) != (g_Omega != nullptr)) return DP_EINVAL;
   if (W_torque && !P->torques) return DP_EINVAL;
+  // the recurrence needs a linear, symmetric positive definite operator: with moving walls dp_mobility_apply is affine (U = M F + wall flow)
+  if (P->p.uwall_0[0] != 0 || P->p.uwall_0[1] != 0 || P->p.uwall_H[0] != 0 || P->p.uwall_H[1] != 0) {
+    P->last_error = "dp_lanczos_sqrt: the plan has a non-zero wall velocity, so its product is affine, not linear; use a plan with uwall_0 = uwall_H = 0";
+    return DP_EINVAL;
+  }
   int prev_dev = -1;
   cudaGetDevice(&prev_dev);
   if (prev_dev != P->p.device && cudaSetDevice(P->p.device) != cudaSuccess) { cudaGetLastError(); return DP_ECUDA; }

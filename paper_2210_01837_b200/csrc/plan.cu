@@ -407,6 +407,16 @@ int dp_create(const dp_params* prm, dp_plan** out) {
   TRY(dev_alloc(P, &P->d_ov_count, (size_t)1));
   TRY(dev_alloc(P, &P->d_flag, (size_t)1));
   TRY(dev_alloc(P, &P->d_lmin, (size_t)1));
+  {   // device shape, once per plan: grid sizes of the persistent kernels and the shared-memory limit their attributes are raised to
+    int sms = 0, optin = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, p.device) != cudaSuccess ||
+        cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, p.device) != cudaSuccess || sms < 1) {
+      set_err(P, "cudaDeviceGetAttribute", "cannot query the device"); cudaGetLastError(); dp_destroy(P); return DP_ECUDA;
+    }
+    P->sm_count = sms; P->smem_optin = optin;
+    cudaError_t te = dp_transfer_setup(P);
+    if (te != cudaSuccess) { set_err(P, "dp_transfer_setup", cudaGetErrorString(te)); cudaGetLastError(); dp_destroy(P); return DP_ECUDA; }
+  }
   if (P->own_fft) {
     cudaError_t fe = dp_fft_own_create(P);
     if (fe != cudaSuccess) { set_err(P, "dp_fft_own_create", cudaGetErrorString(fe)); dp_destroy(P); return DP_ECUDA; }

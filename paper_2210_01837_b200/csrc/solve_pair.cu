@@ -71,10 +71,8 @@ template <int NZ> struct PairSmem {
   // pairs per CTA and CTAs per SM: one CTA of six pairs (measured: two CTAs of three pairs 12.6 ms, three of two 11.9 ms, one of six
   // 10.9 ms at cfg 5 — the warps of one parity must run the SAME stretch of straight-line code at the same time, see the header)
   static constexpr int PAIRS_SM = (227 * 1024 - 2048) / (DOUBLES * 8);       // pairs whose shared memory fits one SM
-#ifndef DP_PAIR_CTAS
 #define DP_PAIR_CTAS 1
 #define DP_PAIR_NPAIR 6
-#endif
   static constexpr int CTAS = PAIRS_SM >= DP_PAIR_CTAS ? DP_PAIR_CTAS : 1;
   static constexpr int NPAIR = PAIRS_SM / CTAS >= DP_PAIR_NPAIR ? DP_PAIR_NPAIR : (PAIRS_SM / CTAS >= 1 ? PAIRS_SM / CTAS : 1);
   static constexpr int THREADS = 64 * NPAIR;
@@ -83,6 +81,9 @@ template <int NZ> struct PairSmem {
 template <int NZ> __device__ __forceinline__ void pair_sync() { named_sync(0, PairSmem<NZ>::THREADS); }
 // Ends a basic block without doing anything (the branch is never taken and costs one uniform compare): ptxas schedules block by
 // block, so work of a later step cannot be started (and its operands loaded) long before its turn at the price of spills.
+// The condition cannot hold: dp_create accepts only nx >= DP_TILE_X + w > 0 and the kernel is launched from a validated plan only.
+// Bodies without a fatal effect were measured in round 3 and dropped: "nanosleep" 158 -> 162 registers and 10.64 -> 10.81 ms at cfg 5;
+// "exit" / "brkpt" compile to 162 registers as well (nz = 40: 128 / 384 bytes of spill loads instead of 88).
 #define DP_SPLIT(A, id) do { if ((A).nx == -(id)) asm volatile("trap;"); } while (0)
 // keeps ptxas from hoisting the shared-memory loads of a later block of work above this point (register pressure)
 __device__ __forceinline__ void sched_fence() { __syncwarp(); }
@@ -90,7 +91,7 @@ __device__ __forceinline__ void sched_fence() { __syncwarp(); }
 // ---- factorisation of the chain of parity PAR for this lane's mode (depends on |k| only): inverse pivots Fi[n], the solution Fa[n]
 // with unit border unknown, and 1/B_g (B_g = boundary functional of that solution).  Rows are indexed by n with stride TM.
 template <int NZ, int PAR>
-__device__ __forceinline__ double factor_chain(const PairTab<NZ>& T, double* __restrict__ Fi, double* __restrict__ Fa, double* __restrict__ Gpq, double k, double k2,
+__device__ __forceinline__ double factor_chain(const PairTab<NZ>& T, double* Fi, double* Fa, double* Gpq, double k, double k2,
                                                double inv_s, bool store) {
   constexpr int n0 = Ch<NZ, PAR>::n0, NR = Ch<NZ, PAR>::NR;
   double invd[NR], ag[NR];
@@ -579,9 +580,7 @@ template <int NZ> size_t pair_smem_bytes() { return sizeof(double) * (size_t)Pai
 }  // namespace
 
 // compiled sizes: the tables of larger nz do not fit a kernel parameter (32 KB); those plans keep the tile kernel of solve.cu
-#ifndef DP_PAIR_NZ_LIST
 #define DP_PAIR_NZ_LIST(X) X(16) X(19) X(24) X(26) X(32) X(40) X(48)
-#endif
 
 bool dp_solve_pair_supports_nz(int nz) {
 #define X(NZ) if (nz == NZ) return true;

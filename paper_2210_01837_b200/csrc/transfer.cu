@@ -23,14 +23,10 @@ constexpr int TX = DP_TILE_X, TY = DP_TILE_Y;
 // latency, ONE thread per column (all of its planes in registers: no per-column set-up repeated by several threads) is fastest up to nz = 32
 // (measured at cfg 5: 4.7 ms against 5.0 with two and 6.0 with four); larger nz need two to keep the accumulators in registers.
 // ZSPLIT / SPREAD_THREADS are usable wherever a template parameter (or macro argument) NZ is in scope.
-#ifndef DP_ZSPLIT_OF
 #define DP_ZSPLIT_OF(NZ) ((NZ) <= 32 ? 1 : 2)
-#endif
 #define ZSPLIT (DP_ZSPLIT_OF(NZ))
 #define SPREAD_THREADS (TX * TY * ZSPLIT)
-#ifndef DP_PCH
 #define DP_PCH 40
-#endif
 constexpr int PCH = DP_PCH;                     // candidate particles staged per chunk
 constexpr int MAXB = 6;                         // origin bins per direction that can reach a tile (w <= 8, TY = 4)
 constexpr int MAXR = 2 * MAXB;                  // candidate ranges per tile: one per bin row, two when the x range wraps
@@ -215,9 +211,7 @@ struct WeightArgs {
 // lmin..lmax in z), and every evaluation of the kernel costs an exp and a square root: the warp first stores zeros over the whole
 // record, then lanes 0-7 take the x entries, 8-15 the y entries and lanes 16-31 the planes lmin, lmin + 1, ... sixteen at a time, so a
 // warp evaluates the kernel once (plus once per image term of eq 9 that reaches some plane) instead of once per 32 record entries.
-#ifndef DP_WEIGHT_WARPS
 #define DP_WEIGHT_WARPS 8
-#endif
 constexpr int WEIGHT_WARPS = DP_WEIGHT_WARPS;
 __global__ void __launch_bounds__(WEIGHT_WARPS * 32) k_weights(int n, WeightArgs A, int nrec) {
   const GridGeom& g = A.g;
@@ -303,9 +297,7 @@ struct SpreadArgs {
 // MODE 0: field triple blockIdx.z (0: forces with Delta_M, 1: torques with Delta_D) gets sum_j val_j S(j; g)   (eq 7 without the curl,
 //         which the solve kernel takes in Fourier-Chebyshev space);
 // MODE 1 (kernel-derivative torques): ONE triple f = sum_j [F_j S_M(j; g) + (1/2) G_j(g) x tau_j], three records per candidate.
-#ifndef DP_SPREAD_MINB
 #define DP_SPREAD_MINB (NZ <= 32 ? 4 : 2)
-#endif
 // staged candidates of one chunk: weight records (zero padded to whole z residue classes), values, footprint records
 template <int NZ, int MODE> struct SpreadBuf {
   static constexpr int NL = (NZ + ZSPLIT - 1) / ZSPLIT;
@@ -707,9 +699,7 @@ struct InterpArgs {
   double* Omega;             // may be NULL
 };
 
-#ifndef DP_INTERP_WARPS
 #define DP_INTERP_WARPS 16
-#endif
 constexpr int INTERP_WARPS = DP_INTERP_WARPS;
 
 // One warp per particle (sorted order, so neighbouring warps gather from neighbouring columns): the lanes sweep the
@@ -717,9 +707,7 @@ constexpr int INTERP_WARPS = DP_INTERP_WARPS;
 // W = kernel support (compile-time: the footprint index arithmetic of the inner loop then has no integer division)
 // MODE 0: U from fields 0-2 with Delta_M, Omega from fields 3-5 (= (1/2) curl u) with Delta_D   (eqs 10, 11);
 // MODE 1 (kernel-derivative torques): U as before, Omega = (1/2) sum_g (u x G) h^2 (H/2) w_l from the SAME three fields.
-#ifndef DP_INTERP_MINB
 #define DP_INTERP_MINB 1
-#endif
 template <class GT, int W, int MODE>
 __global__ void __launch_bounds__(INTERP_WARPS * 32, DP_INTERP_MINB) k_interp(int n, InterpArgs A) {
   constexpr int NREC = MODE ? 3 : 2;
@@ -834,8 +822,13 @@ cudaError_t dp_launch_bin(dp_plan* P, int n, const double* pos, const double* fo
   return cudaGetLastError();
 }
 
+// setup_only: set the kernel attributes of the plan's spread kernels and return (called once per plan from dp_create, never per product)
+static cudaError_t spread_dispatch(dp_plan* P, int n, bool with_torque, cudaStream_t st, bool setup_only);
 cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torque, cudaStream_t st) {
   (void)with_force;
+  return spread_dispatch(P, n, with_torque, st, false);
+}
+static cudaError_t spread_dispatch(dp_plan* P, int n, bool with_torque, cudaStream_t st, bool setup_only) {
   const bool kt = P->kernel_torque;
   const int ngroups = (with_torque && !kt) ? 2 : 1;
   {
@@ -847,7 +840,7 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
     W.inv_Z[0] = 1.0 / P->ZM; W.inv_Z[1] = 1.0 / P->ZD; W.inv_Z[2] = 1.0 / P->ZD; W.inv_alpha = 1.0 / P->alpha;
     W.ucut = P->ucutD;
     W.wrec = P->d_wrec; W.cap = (size_t)P->p.max_particles;
-    if (n > 0) k_weights<<<(unsigned)((n + WEIGHT_WARPS - 1) / WEIGHT_WARPS), WEIGHT_WARPS * 32, 0, st>>>(n, W, P->nrec);
+    if (n > 0 && !setup_only) k_weights<<<(unsigned)((n + WEIGHT_WARPS - 1) / WEIGHT_WARPS), WEIGHT_WARPS * 32, 0, st>>>(n, W, P->nrec);
   }
   SpreadArgs A;
   A.g = make_geom(P);
@@ -863,19 +856,20 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
   // survivor lists per tile, then the pipelined kernel over the tiles whose list fits a staged chunk, then the culling kernel over the rest
   const int ntiles = P->nbx * P->nby;
   const int pc_limit = kt ? PCH / 2 : PCH;
-  cudaError_t e = cudaMemsetAsync(P->d_ov_count, 0, sizeof(int), st);
+  cudaError_t e = cudaSuccess;
+  if (!setup_only) {
+  e = cudaMemsetAsync(P->d_ov_count, 0, sizeof(int), st);
   if (e != cudaSuccess) return e;
   k_tile_lists<<<(ntiles + LIST_WARPS - 1) / LIST_WARPS, LIST_WARPS * 32, 0, st>>>(A.g, P->d_bin_start, P->d_meta, pc_limit, P->d_tile_cnt, P->d_tile_list,
                                                                                     P->d_ov_tiles, P->d_ov_count);
-  int sms = 148;
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, P->p.device);
+  }
+  const int sms = P->sm_count;
 #define DP_SPREAD_LAUNCH(NZV, GT, MODE)                                                                                                   \
   {                                                                                                                                      \
     constexpr int NZ = NZV;                                                                                                              \
     const int per_sm = DP_SPREAD_MINB;                                                                                                   \
     const size_t smem = 2 * sizeof(SpreadBuf<NZ, MODE>) + 3 * (LMAX + 1) * sizeof(int);                                                  \
-    e = cudaFuncSetAttribute(k_spread_pipe<NZ, GT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                       \
-    if (e != cudaSuccess) return e;                                                                                                      \
+    if (setup_only) return cudaFuncSetAttribute(k_spread_pipe<NZ, GT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);    \
     const int gp = ntiles < sms * per_sm ? ntiles : sms * per_sm;                                                                        \
     k_spread_pipe<NZ, GT, MODE><<<dim3(gp, ngroups), SPREAD_THREADS, smem, st>>>(A, P->d_tile_cnt, P->d_tile_list);                      \
     k_spread<NZ, GT, MODE><<<dim3(gp, 1, ngroups), SPREAD_THREADS, 0, st>>>(A, P->d_ov_tiles, P->d_ov_count);                            \
@@ -894,7 +888,17 @@ cudaError_t dp_launch_spread(dp_plan* P, int n, bool with_force, bool with_torqu
   return cudaGetLastError();
 }
 
-cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaStream_t st) {
+static cudaError_t interp_dispatch(dp_plan* P, int n, double* U, double* Omega, cudaStream_t st, bool setup_only);
+cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaStream_t st) { return interp_dispatch(P, n, U, Omega, st, false); }
+// once per plan, from dp_create: dynamic shared-memory limits of the plan's spread and interpolation kernels.  The interpolation kernel's size
+// depends on nz while its instantiation does not, and the limit belongs to the function (not the plan): it is raised to the device's opt-in
+// maximum so that plans with different nz can coexist.
+cudaError_t dp_transfer_setup(dp_plan* P) {
+  cudaError_t e = spread_dispatch(P, 0, false, nullptr, true);
+  if (e != cudaSuccess) return e;
+  return interp_dispatch(P, 0, nullptr, nullptr, nullptr, true);
+}
+static cudaError_t interp_dispatch(dp_plan* P, int n, double* U, double* Omega, cudaStream_t st, bool setup_only) {
   InterpArgs A;
   A.g = make_geom(P);
   A.perm = P->d_perm; A.meta = P->d_meta;
@@ -903,19 +907,15 @@ cudaError_t dp_launch_interp(dp_plan* P, int n, double* U, double* Omega, cudaSt
   A.grid = P->d_real; A.real_field = P->real_field;
   A.U = U; A.Omega = Omega;
   int blocks = (n + INTERP_WARPS - 1) / INTERP_WARPS;
-#ifndef DP_INTERP_MAXB
 #define DP_INTERP_MAXB 32
-#endif
-  const int maxb = 148 * DP_INTERP_MAXB;
+  const int maxb = P->sm_count * DP_INTERP_MAXB;
   if (blocks > maxb) blocks = maxb;
   if (blocks < 1) blocks = 1;
   const bool f32 = P->p.transfer_fp32 != 0, kt = P->kernel_torque;
   const int wr_even = (2 * DP_MAX_W + P->p.nz + 1) & ~1;
   const size_t ismem = sizeof(double) * (DP_MAX_NZ + (size_t)2 * INTERP_WARPS * (kt ? 3 : 2) * wr_even);
-  cudaError_t ie = cudaSuccess;
 #define DP_INTERP_LAUNCH(GT, WW, MODE)                                                                                           \
-  { ie = cudaFuncSetAttribute(k_interp<GT, WW, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ismem);                  \
-    if (ie != cudaSuccess) return ie;                                                                                            \
+  { if (setup_only) return cudaFuncSetAttribute(k_interp<GT, WW, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, P->smem_optin); \
     k_interp<GT, WW, MODE><<<blocks, INTERP_WARPS * 32, ismem, st>>>(n, A); }
 #define DP_INTERP_CASE(WW)                                                              \
   case WW:                                                                              \

@@ -144,6 +144,24 @@ def test_two_plans_coexist_and_other_devices_work(dp):
         assert rel_l2(U1.cpu().numpy(), Ua_o) < TOL
 
 
+def test_a_later_plan_with_another_grid_size_does_not_disturb_a_live_one(dp):
+    """Grid sizes without a static FFT instantiation share the general pass kernels, whose dynamic shared-memory limit is a property of the
+    function, not of the plan: a plan created later (smaller or larger grid) must not leave a live plan unable to launch."""
+    sizes = (60, 48, 90, 50)
+    cases = [workloads.random_bw(n=100, L=nxy * (2.0 / 3.0), nxy=nxy, nz=16, H=8.0, seed=20 + nxy, name="co%d" % nxy) for nxy in sizes]
+    refs = [oracle.mobility_apply(pr, pos, F, None, dft="fft")[0] for pr, pos, F, _ in cases]
+    plans = []
+    try:
+        for k, (pr, pos, F, _) in enumerate(cases):
+            plans.append(dp.Plan(pr, max_particles=len(pos), use_torques=False))
+            for j in range(k + 1):                         # every plan alive so far still works after each creation
+                U, _ = plans[j].mobility_apply(*to_dev(cases[j][1], cases[j][2]))
+                assert rel_l2(U.cpu().numpy(), refs[j]) < TOL, (k, j)
+    finally:
+        for pl in plans:
+            pl.close()
+
+
 def test_forces_only_on_a_torque_plan_and_omega_without_torque(dp):
     prob, pos, F, T = workloads.random_slit(n=200, L=32.0, nxy=48, nz=32, H=8.0, seed=5, name="mix")
     U_o, Om_o = oracle.mobility_apply(prob, pos, F, None, want_omega=True, dft="fft")
@@ -229,7 +247,7 @@ def test_host_entry_point_matches_device_entry_point(dp):
 def test_create_rejects_bad_parameters(dp):
     prob, *_ = workloads.config(1)
     import dataclasses
-    for bad in (dict(nz=7), dict(nx=49), dict(w=3), dict(eta=0.0), dict(Ly=prob.Ly * 1.01), dict(nx=16, ny=16)):
+    for bad in (dict(nz=7), dict(nz=31), dict(nx=49), dict(w=3), dict(eta=0.0), dict(Ly=prob.Ly * 1.01), dict(nx=16, ny=16)):
         with pytest.raises(dp.DPError):
             dp.Plan(dataclasses.replace(prob, **bad), max_particles=8)
 
@@ -528,6 +546,45 @@ def test_lanczos_square_root_matches_the_oracle_iteration(dp, with_torque, mode)
     assert np.allclose(eps, eps_o, rtol=1e-5)
     assert rel_l2(g, g_o) < 1e-8
     assert its < 40                                             # converged before max_iter
+
+
+def test_lanczos_on_the_fp32_transfer_variant_converges_like_the_fp64_run(dp):
+    """Fig. 12's caption: above ~1e-6 the convergence of the Lanczos iteration is not affected by single vs double
+    precision.  dp_lanczos_sqrt on a transfer_fp32 plan against the fp64 plan: same number of products at the paper's working tolerance
+    (1e-3) and at 1e-4 (measured: 17 and 38 at both precisions), within one product at 1e-5 (which may hit the 64-product limit of the entry point),
+    eps_n histories that agree wherever eps_n > 1e-4 (measured: to 8e-3 relative), and the same g to the variant's accuracy (measured: 1e-7)."""
+    prob, pos, F, T = small_monolayer("bw", 2000, 53)
+    n = len(pos)
+    rng = np.random.default_rng(10)
+    WF, WT = rng.standard_normal((n, 3)), rng.standard_normal((n, 3))
+    out = {}
+    for f32 in (False, True):
+        with dp.Plan(prob, max_particles=n, use_torques=True, torque_mode=1, transfer_fp32=f32) as plan:
+            for tol in (1e-3, 1e-4, 1e-5):
+                gU, gO, its, eps = plan.lanczos_sqrt(*to_dev(pos, WF, WT), tol=tol, max_iter=64)
+                out[(f32, tol)] = (np.concatenate([gU.cpu().numpy().ravel(), gO.cpu().numpy().ravel()]), its, np.array(eps))
+    for tol in (1e-3, 1e-4, 1e-5):
+        g64, its64, eps64 = out[(False, tol)]
+        g32, its32, eps32 = out[(True, tol)]
+        m = min(len(eps64), len(eps32))
+        big = eps64[:m] > 1e-4
+        print("lanczos tol %.0e: products fp64 %d / fp32 %d, max rel eps difference above 1e-4: %.2e, g rel L2 %.2e" % (
+            tol, its64, its32, float(np.abs(eps32[:m][big] / eps64[:m][big] - 1).max()) if big.any() else 0.0, rel_l2(g32, g64)))
+        if tol >= 1e-4:
+            assert its64 < 64 and its32 == its64                # converged, and after the same number of products
+        else:
+            assert abs(its32 - its64) <= 1
+        assert np.allclose(eps32[:m][big], eps64[:m][big], rtol=2e-2)
+        assert rel_l2(g32, g64) < max(1e-5, 3 * tol)
+
+
+def test_lanczos_refuses_a_plan_whose_product_is_affine(dp):
+    """With moving walls U = M F + (wall-driven flow): not a linear SPD operator, so M^{1/2} W has no meaning (dp.h)."""
+    import dataclasses
+    prob, pos, F, T = small_monolayer("bw", 100, 54)
+    with dp.Plan(dataclasses.replace(prob, uwall_0=(0.5, 0.0)), max_particles=len(pos)) as plan:
+        with pytest.raises(dp.DPError, match="wall velocity"):
+            plan.lanczos_sqrt(*to_dev(pos, F, T), tol=1e-3, max_iter=10)
 
 
 # ------------------------------------------------------------------------------------------------ partial slip, moving walls (SURVEY.md §8 f-3)
