@@ -10,6 +10,8 @@ configuration bench.py times), through the C ABI, against the CPU oracle.
   lines, random interior) vs ``oracle.solve_modes``; oracle interpolation of the CUDA path's real-space u, omega for ALL particles
   vs the CUDA U, Omega.  The whole oracle product at config 5 (about 60 GB of host memory, two minutes) runs too, unless
   DP_FULL_ORACLE_CFG5=0.
+* the fp32 spread / interpolate variant (transfer_fp32 = 1, north_star: <= 1e-5) at configs 3, 4 and 5 in the torque mode bench.py times,
+  against the same whole-oracle results.
 """
 import os
 import sys
@@ -57,6 +59,30 @@ def check_product(U, Om, U_o, Om_o):
     return stacked
 
 
+TOL_FP32 = 1e-5      # north_star: the optional fp32 spread / interpolate variant, relative L2
+TOL_FP32_MAX = 1e-4  # per particle, of max |reference| (fp32 rounding, 6e-8, of ~10^3 accumulated terms each way; measured: see the printed line)
+
+
+def run_fp32_variant(dp, prob, pos, F, T, torque_mode):
+    """The same product on a transfer_fp32 plan (fp32 spreading, interpolation and real-space grids; transforms and solves fp64)."""
+    import torch
+    with dp.Plan(prob, max_particles=len(pos), use_torques=True, torque_mode=1 if torque_mode == "kernel" else 0, transfer_fp32=True) as plan:
+        U, Om = plan.mobility_apply(*to_dev(pos, F, T))
+        torch.cuda.synchronize()
+        assert plan.check() == 0
+        U, Om = U.cpu().numpy(), Om.cpu().numpy()
+    torch.cuda.empty_cache()
+    return U, Om
+
+
+def check_fp32_product(tag, U, Om, U_o, Om_o):
+    stacked = rel_l2(np.concatenate([U, Om], axis=1), np.concatenate([U_o, Om_o], axis=1))
+    print("%s fp32 transfer variant: stacked rel L2 %.2e, per-particle max %.2e / %.2e" % (tag, stacked, rel_max(U, U_o), rel_max(Om, Om_o)))
+    assert stacked < TOL_FP32, stacked
+    assert rel_l2(U, U_o) < TOL_FP32 and rel_l2(Om, Om_o) < TOL_FP32
+    assert rel_max(U, U_o) < TOL_FP32_MAX and rel_max(Om, Om_o) < TOL_FP32_MAX, (rel_max(U, U_o), rel_max(Om, Om_o))
+
+
 @pytest.mark.parametrize("cfg,torque_mode", [(3, "fourier"), (4, "fourier"), (3, "kernel"), (4, "kernel")])
 def test_cfg3_cfg4_full_size_against_the_oracle(dp, cfg, torque_mode):
     """torque_mode: "fourier" = curl in Fourier-Chebyshev space (6 fields), "kernel" = ES kernel derivative (3 fields, bench.py's default)"""
@@ -70,7 +96,10 @@ def test_cfg3_cfg4_full_size_against_the_oracle(dp, cfg, torque_mode):
         assert plan.check() == 0
         U, Om = U.cpu().numpy(), Om.cpu().numpy()
     torch.cuda.empty_cache()
+    fp32 = run_fp32_variant(dp, prob, pos, F, T, torque_mode) if torque_mode == "kernel" else None   # the variant bench.py times, same oracle run
     U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", torque_mode=torque_mode)
+    if fp32 is not None:
+        check_fp32_product("cfg%d (%s)" % (cfg, torque_mode), fp32[0], fp32[1], U_o, Om_o)
     err = check_product(U, Om, U_o, Om_o)
     print("cfg%d (%s) full size: stacked rel L2 %.2e, per-particle max %.2e / %.2e" % (cfg, torque_mode, err, rel_max(U, U_o), rel_max(Om, Om_o)))
 
@@ -197,8 +226,11 @@ def test_cfg5_whole_product_against_the_whole_oracle(dp, torque_mode):
         assert plan.check() == 0
         U, Om = U.cpu().numpy(), Om.cpu().numpy()
     torch.cuda.empty_cache()
+    fp32 = run_fp32_variant(dp, prob, pos, F, T, torque_mode) if torque_mode == "kernel" else None   # bench.py's fp32_transfer_variant at the size it is timed
     tm = {}
     U_o, Om_o = oracle.mobility_apply(prob, pos, F, T, dft="fft", timing=tm, torque_mode=torque_mode)
+    if fp32 is not None:
+        check_fp32_product("cfg5 (kernel)", fp32[0], fp32[1], U_o, Om_o)
     err = check_product(U, Om, U_o, Om_o)
     print("cfg5 (" + torque_mode + ") whole oracle: stacked rel L2 %.2e, per-particle max %.2e / %.2e, oracle seconds %s" % (
         err, rel_max(U, U_o), rel_max(Om, Om_o), {k: round(v, 1) for k, v in tm.items()}))
