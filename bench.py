@@ -439,6 +439,27 @@ def main():
                     "stage_ms": r9["stage_ms"], "plan_device_GB": r9["plan_device_GB"],
                     "paper": "370 ms per mobility solve on a V100 for this case (PAPER.md:505): another machine's number, context only"}
 
+    # ---- other workloads of the same path, same timing rules: what has full-size parity tests but would otherwise have no time
+    #      (each: problem, particle count, measured run, description); single GPU, default configuration only
+    extras = {}
+    if not args.no_variants and args.fft == "own" and world == 1 and args.config == 5:
+        def X(key, what, pX, posX, FX, TX, tm):
+            extras[key] = (pX, len(posX), measure(dp, torch, pX, posX, FX, TX, dev, dist, args, torque_mode=tm), what)
+        p4, pos4, F4, T4 = workloads.config(4)
+        for tm in ("kernel", "fourier"):
+            X("slit_cfg4_" + tm, "BASELINE.json configs[3]: slit channel H = 6 (two walls, App. A correction, no empty planes), N = 262,144, grid %dx%dx%d, forces + torques, torque mode %s"
+              % (p4.nx, p4.ny, p4.nz, tm), p4, pos4, F4, T4, tm)
+        del pos4, F4, T4
+        pj, posj, Fj, Tj = workloads.monolayer_bw(n=n, seed=prob.seed, name="cfg5-jittered", xy="jittered")
+        X("cfg5_jittered_lattice", "config 5 with non-overlapping in-plane positions (jittered square lattice at area fraction 0.4, SURVEY.md §8(d): the closer stand-in "
+          "for the paper's hard-sphere tile, PAPER.md:492); same box, grid, heights, drives and torque mode as the headline", pj, posj, Fj, Tj, args.torque_mode)
+        del posj, Fj, Tj
+        p9d, pos9d, F9d, T9d = workloads.paper_fig9(18, dipole=True)
+        for tm in ("kernel", "fourier"):
+            X("paper_fig9_MD_" + tm, "paper Table III 'M & D' stand-in (PAPER.md:492-501): N = %d, forces + torques, grid %dx%dx%d, m = 6, beta_M/m = 1.38, beta_D/m = 2.3, H = 9.2 R_h, "
+              "torque mode %s (fourier = the paper's 'additional FFTs', kernel = its second way, PAPER.md:335)" % (len(pos9d), p9d.nx, p9d.ny, p9d.nz, tm), p9d, pos9d, F9d, T9d, tm)
+        del pos9d, F9d, T9d
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -476,9 +497,11 @@ def main():
     t_solve = stages["solve"]["ms"] * 1e-3
     if t_solve > 0:
         ach = 2.0 * fma_mode * modes / t_solve / 1e12
-        roofline["solve_fp64"] = {"bound": "alu", "kernel": main_run["solve_kernel"], "achieved": ach, "peak": 2 * 148 * 64 * 1.965e9 / 1e12, "unit": "TFLOP/s",
-                                  "frac": ach / (2 * 148 * 64 * 1.965e9 / 1e12), "algorithmic_fma_per_mode": fma_mode, "modes": modes,
-                                  "peak_source": "148 SMs x 64 fp64 FMA lanes per clock x 1.965 GHz (B200_PROFILING.md unit counts; a DFMA-only probe reaches 0.92 of it)"}
+        sms = int(torch.cuda.get_device_properties(dev).multi_processor_count)
+        pk = 2 * sms * 64 * 1.965e9 / 1e12
+        roofline["solve_fp64"] = {"bound": "alu", "kernel": main_run["solve_kernel"], "achieved": ach, "peak": pk, "unit": "TFLOP/s",
+                                  "frac": ach / pk, "algorithmic_fma_per_mode": fma_mode, "modes": modes,
+                                  "peak_source": "%d SMs (queried) x 64 fp64 FMA lanes per clock x 1.965 GHz (B200_PROFILING.md unit counts)" % sms}
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:
@@ -497,6 +520,13 @@ def main():
         d["whole_product_frac"] = agg2["whole_product"]["frac"]
         return d
 
+    def extra_brief(pX, nX, r, what):
+        stX, aggX = summarise(pX, nX, r, peak, world)
+        return {"what": what, "ms_per_step": r["ms_per_step"], "value": nX / (r["ms_per_step"] * 1e-3), "unit": "particles/s", "fields_each_way": r["fields"],
+                "solve_kernel": r["solve_kernel"], "zero_planes_skipped": r["zero_planes"], "plan_device_GB": r["plan_device_GB"],
+                "stage_ms": {k: v for k, v in r["stage_ms"].items() if k != "total"}, "kernels": kernel_table(pX, nX, r, peak),
+                "fft_chebyshev_solve_stages": aggX["fft_chebyshev_solve_stages"], "whole_product_frac": aggX["whole_product"]["frac"]}
+
     fin = fout = main_run["fields"]
     by_total = sum(stage_bytes(prob, n, fin, fout, main_run["zero_planes"]).values())
     line = {"metric": METRIC, "value": value, "unit": "particles/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -510,7 +540,8 @@ def main():
             "clocks": main_run.get("clocks"), "e2e": main_run.get("e2e"), "gpu_launches": MY_KERNELS_PER_STEP[main_run["fft_backend"]] * args.steps,
             "stages": stages, "roofline": roofline, "cpu_baseline": cpu,
             ("fourier_curl_torques" if args.torque_mode == "kernel" else "kernel_derivative_torques"): brief(other),
-            "fp32_transfer_variant": brief(variant), "all_planes_dense": brief(dense), "tile_solve_kernel": brief(tile), "paper_fig9": fig9}
+            "fp32_transfer_variant": brief(variant), "all_planes_dense": brief(dense), "tile_solve_kernel": brief(tile), "paper_fig9": fig9,
+            "other_workloads": {k: extra_brief(*v) for k, v in extras.items()}}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

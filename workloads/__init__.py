@@ -121,15 +121,37 @@ def random_slit(n=4096, L=128.0, nxy=192, nz=48, H=8.0, margin=1.5, seed=1002, n
     return prob, pos, _normal(seed, 2, n), _normal(seed, 3, n)
 
 
-def monolayer_bw(n=65536, nz=32, H=13.0, seed=1003, name="cfg3", zclip=11.0):
-    """Configs 3, 5: sedimented microroller monolayer above one wall at area fraction 0.4."""
+def _xy_jittered_lattice(seed: int, n: int, L: float, a: float = 1.0) -> np.ndarray:
+    """Non-overlapping in-plane positions at the same area fraction: a square lattice of sqrt(n) x sqrt(n) sites of spacing d = L / sqrt(n)
+    (d = 2.80 a at area fraction 0.4), every site displaced uniformly by up to (d - 2a)/2 in x and in y, so that two centres are never closer
+    than 2a in the plane — the hard-disk constraint of the paper's equilibrated tile, which uniform draws violate (density
+    spikes).  Site order is shuffled so that particle index carries no spatial order, as in the uniform recipe."""
+    m = int(round(math.sqrt(n)))
+    if m * m != n:
+        raise ValueError("the jittered lattice needs a square number of particles")
+    d = L / m
+    if d < 2.0 * a:
+        raise ValueError("area fraction too high for a non-overlapping square lattice")
+    g = _rng(seed, 0)
+    ij = g.permutation(n)
+    jit = g.uniform(-0.5 * (d - 2.0 * a), 0.5 * (d - 2.0 * a), (n, 2))
+    xy = np.stack([(ij % m + 0.5) * d, (ij // m + 0.5) * d], axis=1) + jit
+    return xy
+
+
+def monolayer_bw(n=65536, nz=32, H=13.0, seed=1003, name="cfg3", zclip=11.0, xy="uniform"):
+    """Configs 3, 5: sedimented microroller monolayer above one wall at area fraction 0.4.  xy = "uniform" (BASELINE.json's recipe) or
+    "jittered": the non-overlapping jittered-lattice stand-in of SURVEY.md §8(d), same box, grid, heights and drives."""
     L = monolayer_L(n)
     nxy = smooth_at_least(math.ceil(1.5 * L))
     prob = Problem(name, BOTTOM_WALL, L, L, H, nxy, nxy, nz, 6, 6 * BETA_OVER_W_M_W6,
                    6 * BETA_OVER_W_D_W6, seed=seed, n=n)
     z = np.minimum(1.0 + _rng(seed, 1).exponential(0.5, n), zclip)
     F, T = _roller_drive(seed, n)
-    return prob, _pack(_xy(seed, n, L, L), z), F, T
+    if xy not in ("uniform", "jittered"):
+        raise ValueError("xy must be 'uniform' or 'jittered'")
+    pxy = _xy(seed, n, L, L) if xy == "uniform" else _xy_jittered_lattice(seed, n, L)
+    return prob, _pack(pxy, z), F, T
 
 
 def monolayer_slit(n=262144, nz=48, H=6.0, margin=1.2, seed=1004, name="cfg4"):
